@@ -1,0 +1,143 @@
+"""Pins for the precision-map rule and the triangular solves of the oracle.
+
+Map rule: hand-built matrices whose tile norms sit just below / above each threshold, and the
+equicorrelation closed form t_ij = c*nb, ||A||_F^2 = n(c+d)^2 + n(n-1)c^2, which makes the rule
+degenerate to u_p <= eps (the uniform maps the paper also reports).
+Solve: Sherman-Morrison closed form for c 11^T + d I, LAPACK solve, residual.
+"""
+import numpy as np
+import pytest
+
+from oracle import rounding as R
+from oracle.cholesky import tile_cholesky_fp64, tile_cholesky_emulated
+from oracle.precision_map import precision_map, tile_norms, frobenius_from_tile_norms, uniform_map
+from oracle.solve import potrs_fp64, solve_fp64
+from krr_inputs import CONFIGS, scaled_config, make_problem
+
+
+def test_tile_norms_and_symmetric_frobenius():
+    rng = np.random.default_rng(0)
+    n, nb = 96, 24
+    B = rng.standard_normal((n, n))
+    A = B + B.T
+    t = tile_norms(A, nb)
+    for i in range(4):
+        for j in range(4):
+            blk = A[i * nb:(i + 1) * nb, j * nb:(j + 1) * nb]
+            want = np.linalg.norm(blk) if i >= j else 0.0
+            assert abs(t[i, j] - want) <= 1e-12 * max(1.0, want)
+    assert abs(frobenius_from_tile_norms(t) - np.linalg.norm(A)) < 1e-10
+
+
+def _block_matrix(NT, nb, norms):
+    """Symmetric matrix whose tile (i,j) is constant with Frobenius norm norms[i,j]."""
+    n = NT * nb
+    A = np.zeros((n, n))
+    for i in range(NT):
+        for j in range(i + 1):
+            A[i * nb:(i + 1) * nb, j * nb:(j + 1) * nb] = norms[i, j] / nb
+            A[j * nb:(j + 1) * nb, i * nb:(i + 1) * nb] = norms[i, j] / nb
+    return A
+
+
+def test_rule_thresholds_just_below_and_above():
+    NT, nb = 4, 8
+    eps = 2.0 ** -13                                 # exactly representable as a C float
+    base = np.full((NT, NT), 1.0) + 50.0 * np.eye(NT)   # dominant diagonal fixes ||A||_F
+    # choose target norms relative to rhs = eps * fro / NT; iterate once since fro depends on them
+    norms = base.copy()
+    for _ in range(50):
+        A = _block_matrix(NT, nb, norms)
+        fro = np.linalg.norm(A)
+        rhs = eps * fro / NT
+        norms[1, 0] = rhs / 2.0 ** -4 * 0.999        # just qualifies for FP8
+        norms[2, 0] = rhs / 2.0 ** -4 * 1.001        # just misses FP8 -> FP16
+        norms[2, 1] = rhs / 2.0 ** -11 * 0.999       # just qualifies for FP16
+        norms[3, 0] = rhs / 2.0 ** -11 * 1.001       # misses FP16 -> FP32
+        norms[3, 1] = rhs / 2.0 ** -11 * 4.0         # far above the FP16 threshold -> FP32
+        norms[3, 2] = rhs * 1e-3                     # tiny -> FP8
+    A = _block_matrix(NT, nb, norms).astype(np.float64)
+    pmap, t, fro = precision_map(A, nb, eps)
+    assert pmap[1, 0] == R.FP8 and pmap[2, 0] == R.FP16 and pmap[2, 1] == R.FP16
+    assert pmap[3, 0] == R.FP32 and pmap[3, 1] == R.FP32 and pmap[3, 2] == R.FP8
+    assert all(pmap[i, i] == R.FP32 for i in range(NT))
+    # allowed mask: without FP8 the FP8 tiles fall to FP16; with FP32 only everything is FP32
+    pm2, _, _ = precision_map(A, nb, eps, allowed=(R.FP32, R.FP16))
+    assert pm2[1, 0] == R.FP16 and pm2[3, 2] == R.FP16 and pm2[3, 0] == R.FP32
+    pm3, _, _ = precision_map(A, nb, eps, allowed=(R.FP32,))
+    assert np.all(pm3[np.tril_indices(NT)] == R.FP32)
+
+
+@pytest.mark.parametrize("eps,want", [(1e-4, R.FP32), (1e-3, R.FP16), (0.07, R.FP8)])
+def test_equicorrelation_gives_uniform_maps(eps, want):
+    # t_ij = c*nb (i>j); ||A||_F/NT -> c*nb for large n, so the rule reduces to u_p <= eps:
+    # eps=1e-4 -> FP32 (u16 = 4.9e-4), eps=1e-3 -> FP16, FP8 only for eps >= 2^-4 (SURVEY finding 1).
+    n, nb, c, d = 512, 64, 0.48, 0.53
+    NT = n // nb
+    A = c * np.ones((n, n)) + d * np.eye(n)
+    pmap, t, fro = precision_map(A, nb, eps)
+    assert abs(t[3, 1] - c * nb) < 1e-12
+    assert abs(fro ** 2 - (n * (c + d) ** 2 + n * (n - 1) * c * c)) < 1e-6
+    assert np.all(pmap[np.tril_indices(NT, -1)] == want)
+
+
+def test_config_like_matrices_get_uniform_maps():
+    # reduced twins of C2 (eps 1e-4 -> all FP32) and C4 (eps 1e-3 -> all FP16, no FP8)
+    c2 = scaled_config(CONFIGS["C2"], nb=32, n=512, p=400)
+    A, _ = make_problem(c2)
+    pmap, t, fro = precision_map(A.numpy(), c2.nb, c2.eps_target, c2.allowed)
+    off = np.tril_indices(c2.NT, -1)
+    assert np.all(pmap[off] == R.FP32)
+    ratio = t[off] / (fro / c2.NT)
+    assert 0.9 < ratio.min() and ratio.max() < 1.1
+    c4 = scaled_config(CONFIGS["C4"], nb=32, n=512, p=400)
+    A, _ = make_problem(c4)
+    pmap, _, _ = precision_map(A.numpy(), c4.nb, c4.eps_target, c4.allowed)
+    assert np.all(pmap[off] == R.FP16)
+
+
+def test_sherman_morrison_closed_form():
+    n, nb, c, d = 192, 32, 0.48, 0.53
+    A = c * np.ones((n, n)) + d * np.eye(n)
+    rng = np.random.default_rng(1)
+    Y = rng.standard_normal((n, 4))
+    want = (Y - c * np.ones((n, 1)) * (np.ones((1, n)) @ Y) / (d + n * c)) / d
+    got = solve_fp64(A, Y, nb)
+    assert np.max(np.abs(got - want)) < 1e-12 * np.max(np.abs(want))
+
+
+@pytest.mark.parametrize("n,nb,nrhs", [(64, 16, 1), (240, 48, 5)])
+def test_potrs_against_lapack_and_residual(n, nb, nrhs):
+    rng = np.random.default_rng(2)
+    B = rng.standard_normal((n, n))
+    A = B @ B.T + n * np.eye(n)
+    Y = rng.standard_normal((n, nrhs))
+    L, info = tile_cholesky_fp64(A, nb)
+    assert info == 0
+    X = potrs_fp64(L, Y, nb)
+    want = np.linalg.solve(A, Y)
+    assert np.max(np.abs(X - want)) < 1e-12 * np.max(np.abs(want))
+    assert np.linalg.norm(Y - A @ X) / (np.linalg.norm(A) * np.linalg.norm(X)) < 1e-15
+    # forward then backward: L (L^T x) = y
+    assert np.max(np.abs(L @ (L.T @ X) - Y)) < 1e-10
+
+
+def test_survey_probe_numbers_small():
+    # SURVEY 8(c) table at reduced size: all-FP32 backward error ~1e-8 and alpha error ~1e-6;
+    # all-FP16 backward error ~1.5e-4 (< 5e-4) while alpha misses 1e-3 (finding 3).
+    cfg = scaled_config(CONFIGS["C1"], nb=64, n=1024, p=1000)
+    A, Y = make_problem(cfg)
+    A = A.numpy(); Y = Y.numpy()
+    from oracle.cholesky import backward_error
+    alpha = solve_fp64(A, Y, cfg.nb)
+    L32, _, info = tile_cholesky_emulated(A, cfg.nb, uniform_map(cfg.NT, R.FP32))
+    assert info == 0
+    assert backward_error(A, L32) < 1e-7
+    a32 = potrs_fp64(L32, Y, cfg.nb)
+    assert np.linalg.norm(a32 - alpha) / np.linalg.norm(alpha) < 1e-4
+    L16, _, info = tile_cholesky_emulated(A, cfg.nb, uniform_map(cfg.NT, R.FP16))
+    assert info == 0
+    be16 = backward_error(A, L16)
+    assert 2e-5 < be16 < 5e-4
+    a16 = potrs_fp64(L16, Y, cfg.nb)
+    assert np.linalg.norm(a16 - alpha) / np.linalg.norm(alpha) > 1e-3

@@ -1,0 +1,164 @@
+/*
+ * krr_mp.h -- C ABI of the B200-native mixed-precision tile Cholesky for Kernel Ridge Regression.
+ *
+ * The hot path of the paper's Associate phase (Alg. 3):
+ *     K~ <- FACTORIZE(K + alpha*Id)      -> krr_precision_map + krr_potrf_mp
+ *     W  <- Solve(K~, P_h)      -> krr_potrs
+ * with the tile-centric adaptive-precision Cholesky of PAPER.md:192 ("a tiled mosaic of precisions
+ * embedded in a single stored copy of the matrix", FP32 / FP16 / FP8-E4M3 per tile)
+ * and forward/backward substitution "in the full FP32 precision".
+ *
+ * Conventions
+ *   - Every d_* pointer is DEVICE memory owned by the caller (e.g. a PyTorch tensor); every h_*
+ *     pointer is HOST memory.  `stream` is a cudaStream_t passed as void*.  Unless stated, the
+ *     library never allocates or frees device memory, never synchronises the device and never
+ *     reads or writes the host copy of the data; all work is enqueued on `stream`.
+ *   - n = number of patients (matrix order), nb = tile size, NT = n / nb.  nb must be a multiple
+ *     of 128 and divide n (all BASELINE.json configs do; ragged edges are not supported).
+ *   - Tiles are addressed (i, j), 0-based, i >= j (lower triangle).  A precision map is NT*NT
+ *     bytes, row-major, map[i*NT + j] in {KRR_FP32, KRR_FP16, KRR_FP8_E4M3} for i >= j; entries
+ *     with i < j are ignored on input and written as 255 on output.  Diagonal tiles are FP32.
+ *   - Return value: 0 on success, < 0 for an argument / usage error detected on the host before
+ *     anything is launched (see KRR_ERR_*).  Numerical breakdown is reported asynchronously
+ *     through *d_info (LAPACK convention), never through the return value.
+ *   - Thread-safety: re-entrant on distinct streams with distinct workspaces.
+ */
+#ifndef KRR_MP_H
+#define KRR_MP_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum { KRR_FP32 = 0, KRR_FP16 = 1, KRR_FP8_E4M3 = 2 } krr_prec_t;
+
+#define KRR_OK               0
+#define KRR_ERR_ARG        (-1)   /* null pointer, non-positive size, lda/ldb too small            */
+#define KRR_ERR_SHAPE      (-2)   /* nb does not divide n, nb not a multiple of 128, NT too large  */
+#define KRR_ERR_WORKSPACE  (-3)   /* ws_bytes smaller than the matching *_workspace() query        */
+#define KRR_ERR_DEVICE     (-4)   /* current device is not compute capability 10.x (sm_100)        */
+#define KRR_ERR_CUDA       (-5)   /* a CUDA call or kernel launch failed                           */
+#define KRR_ERR_MAP        (-6)   /* invalid precision code in h_map, or non-FP32 diagonal tile    */
+#define KRR_ERR_UNSUPPORTED (-7)  /* a flag bit this build does not implement                      */
+
+/* flags (krr_precision_map, krr_potrf_mp, krr_associate_host) */
+#define KRR_FLAG_PREROUND_A     1u  /* round the off-diagonal tiles of A into their storage precision
+                                       before factorising ("lower the precision of the
+                                       off-diagonal tiles ... followed by the mixed-precision
+                                       Cholesky").  Default of the Python binding.                  */
+#define KRR_FLAG_A_TILED_LOWER  4u  /* d_A holds only the lower tiles ("lower-triangular tile
+                                       storage", BASELINE.json config 4): tile (i,j), i >= j, is a
+                                       contiguous row-major nb x nb block at element offset
+                                       krr_tile_slot(NT,i,j) * nb * nb; lda is ignored.             */
+
+/* Library version (major*100 + minor) and the compute capability it was built for (100). */
+int krr_version(void);
+int krr_built_for_sm(void);
+
+/* Index of tile (i,j), i >= j, in column-major order over the lower triangle:
+ * slot = j*NT - j*(j-1)/2 + (i - j).  Pure host function. */
+int64_t krr_tile_slot(int NT, int i, int j);
+
+/* ---------------------------------------------------------------------------------------------
+ * krr_precision_map -- tile norms and the tile-centric adaptive-precision map.
+ * PAPER.md:192, :215, :229; rule text from BASELINE.json (the paper prints no formula):
+ *     off-diagonal tile (i,j) gets the LOWEST precision p with bit p set in allowed_mask and
+ *         ||A_ij||_F * u_p  <=  eps_target * ||A||_F / NT ,     u = 2^-24, 2^-11, 2^-4,
+ *     KRR_FP32 if none qualifies; diagonal tiles are KRR_FP32.  ||A||_F is of the full symmetric
+ *     matrix (off-diagonal tiles counted twice).
+ * d_A         in   FP32, row-major n x n with leading dimension lda (elements), only tiles with
+ *                  i >= j are read (diagonal tiles as full squares); or tile-packed lower storage
+ *                  with KRR_FLAG_A_TILED_LOWER.  Not modified.
+ * d_map       out  NT*NT bytes.
+ * d_tile_norms out NT*NT floats, ||A_ij||_F for i >= j, 0 above; may be NULL.
+ * d_tile_amax out  NT*NT floats, max|A_ij| for i >= j, 0 above; may be NULL.
+ * d_fro       out  one double, ||A||_F; may be NULL.
+ * d_ws        workspace of at least krr_precision_map_workspace(n, nb) bytes.
+ * Sums of squares are accumulated in FP64 in a fixed order (deterministic).  One pass over the
+ * lower tiles of A: HBM-bound.
+ */
+size_t krr_precision_map_workspace(int64_t n, int nb);
+int krr_precision_map(const float* d_A, int64_t n, int64_t lda, int nb,
+                      float eps_target, unsigned allowed_mask, unsigned flags,
+                      uint8_t* d_map, float* d_tile_norms, float* d_tile_amax, double* d_fro,
+                      void* d_ws, size_t ws_bytes, void* stream);
+
+/* ---------------------------------------------------------------------------------------------
+ * Factor storage (the tile mosaic).  Tile (i,j), i >= j, is a contiguous row-major
+ * nb x nb block in its own precision (4, 2 or 1 bytes per element) at byte offset
+ *     off(i,j) = sum of the byte sizes of all lower tiles preceding it in column-major tile order,
+ * a pure function of (map, nb); every offset is a multiple of 128 bytes.  Diagonal tiles are FP32
+ * full squares with zeros above the diagonal.  An FP8 tile holds E4M3 codes q with value
+ * scales[i*NT+j] * q; the scale is a power of two (1.0 for FP32 / FP16 tiles).
+ * krr_factor_bytes returns the payload size; krr_factor_tile_offset one tile's offset.
+ * Both are pure host functions; they return 0 / -1 on invalid arguments.
+ */
+size_t  krr_factor_bytes(int64_t n, int nb, const uint8_t* h_map);
+int64_t krr_factor_tile_offset(int64_t n, int nb, const uint8_t* h_map, int i, int j);
+
+/* ---------------------------------------------------------------------------------------------
+ * krr_potrf_mp -- mixed-precision tile Cholesky  A = L L^T  of A = K + lambda*I.
+ * PAPER.md:112 (FACTORIZE), :192 (four-precision tile Cholesky; FP64 not required), :211 (E4M3 for
+ * both operands), :206 (operands converted on the fly), :130/:159 (POTRF / TRSM / SYRK / GEMM).
+ * Per tile column k:  S_kk = A_kk - sum_j L_kj L_kj^T, L_kk = chol(S_kk) in FP32;
+ * S_ik = rd_p(A_ik) - sum_j L_ij L_kj^T accumulated in FP32 (tensor cores, operands as stored),
+ * L_ik = rd_{p(i,k)}(S_ik L_kk^{-T}) -- each tile is rounded once, when its final value is stored.
+ * d_A      in   as for krr_precision_map; not modified.
+ * d_map / h_map in  the same map in device and host memory (the launch sequence is built on the
+ *               host from h_map; kernels read d_map).
+ * d_factor out  krr_factor_bytes(n, nb, h_map) bytes, layout above.
+ * d_scales out  NT*NT floats (row-major, scales[i*NT+j]); 1.0 except FP8 tiles; 0 above diagonal.
+ * d_info   out  one int: 0 on success, j > 0 = 1-based scalar column of the first non-positive
+ *               pivot (contents of later tile columns are then unspecified).
+ * d_ws     workspace, at least krr_potrf_mp_workspace(n, nb, h_map) bytes, 1024-byte aligned.
+ *          It holds the FP16 operand images of L that the tensor-core kernels read and must be
+ *          kept if krr_potrf_mp is to be followed by nothing else than krr_potrs (which needs
+ *          only d_factor / d_scales / d_map).
+ * flags    KRR_FLAG_PREROUND_A, KRR_FLAG_A_TILED_LOWER.
+ */
+size_t krr_potrf_mp_workspace(int64_t n, int nb, const uint8_t* h_map);
+int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb,
+                 const uint8_t* d_map, const uint8_t* h_map,
+                 void* d_factor, float* d_scales, int* d_info,
+                 void* d_ws, size_t ws_bytes, unsigned flags, void* stream);
+
+/* ---------------------------------------------------------------------------------------------
+ * krr_potrs -- solve (L L^T) X = B by forward and backward substitution in FP32 (PAPER.md:114,
+ * :169), with the tile mosaic produced by krr_potrf_mp (tiles dequantised on the fly).
+ * d_B   in/out  n x nrhs FP32, ROW-major with leading dimension ldb >= nrhs (elements);
+ *               in: Y (phenotypes), out: alpha (the weights W of PAPER.md:82).  1 <= nrhs <= 32.
+ * d_ws  workspace of at least krr_potrs_workspace(n, nb, nrhs) bytes.
+ */
+size_t krr_potrs_workspace(int64_t n, int nb, int nrhs);
+int krr_potrs(const void* d_factor, const float* d_scales,
+              const uint8_t* d_map, const uint8_t* h_map, int64_t n, int nb,
+              float* d_B, int64_t ldb, int nrhs,
+              void* d_ws, size_t ws_bytes, void* stream);
+
+/* ---------------------------------------------------------------------------------------------
+ * krr_associate_host -- the whole Associate phase (Alg. 3) from HOST buffers: copies A and Y to the
+ * device arena, runs krr_precision_map -> krr_potrf_mp -> krr_potrs, copies alpha, the map and info
+ * back, and synchronises `stream` before returning.  Used for end-to-end timing.
+ * h_A      in   FP32 n x n row-major (lda) host memory (pinned memory makes the copies asynchronous)
+ * h_Y      in   n x nrhs row-major; h_alpha out n x nrhs; h_map out NT*NT bytes; h_info out 1 int
+ * force_prec    < 0: use the rule with (eps_target, allowed_mask); 0..2: uniform off-diagonal map
+ * d_arena  device scratch of at least krr_associate_host_arena(n, nb, nrhs) bytes (sized for the
+ *          worst-case map), 1024-byte aligned.
+ */
+size_t krr_associate_host_arena(int64_t n, int nb, int nrhs);
+int krr_associate_host(const float* h_A, int64_t n, int64_t lda, int nb,
+                       float eps_target, unsigned allowed_mask, int force_prec, unsigned flags,
+                       const float* h_Y, int nrhs, float* h_alpha,
+                       uint8_t* h_map, int* h_info,
+                       void* d_arena, size_t arena_bytes, void* stream);
+
+/* Number of kernels the last krr_* call on this thread enqueued (for bench.py's gpu_launches). */
+int64_t krr_last_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* KRR_MP_H */

@@ -1,0 +1,13 @@
+"""B200-native (sm_100a) mixed-precision tile Cholesky for Kernel Ridge Regression.
+
+Thin Python binding over the C ABI of include/krr_mp.h (argument marshalling only; every step of
+the path runs in the CUDA kernels of csrc/).  PyTorch supplies device memory and streams.
+There is no CPU fallback: importing works anywhere, calling needs the built library and a B200.
+"""
+from .binding import (FP32, FP16, FP8, FLAG_PREROUND_A, FLAG_A_TILED_LOWER, KrrError, Factor,
+                      lib, library_path, precision_map, potrf_mp, potrs, associate_host,
+                      factor_bytes, factor_tile_offset, tile_slot, uniform_map, last_launch_count)
+
+__all__ = ["FP32", "FP16", "FP8", "FLAG_PREROUND_A", "FLAG_A_TILED_LOWER", "KrrError", "Factor",
+           "lib", "library_path", "precision_map", "potrf_mp", "potrs", "associate_host",
+           "factor_bytes", "factor_tile_offset", "tile_slot", "uniform_map", "last_launch_count"]

@@ -1,0 +1,249 @@
+"""ctypes binding with the same names as include/krr_mp.h (marshalling only)."""
+import ctypes
+import os
+from dataclasses import dataclass
+
+import torch
+
+FP32, FP16, FP8 = 0, 1, 2
+FLAG_PREROUND_A = 1
+FLAG_A_TILED_LOWER = 4
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB = None
+
+ERRORS = {-1: "KRR_ERR_ARG", -2: "KRR_ERR_SHAPE", -3: "KRR_ERR_WORKSPACE", -4: "KRR_ERR_DEVICE",
+          -5: "KRR_ERR_CUDA", -6: "KRR_ERR_MAP", -7: "KRR_ERR_UNSUPPORTED"}
+
+EXPORTS = ["krr_version", "krr_built_for_sm", "krr_tile_slot", "krr_precision_map_workspace",
+           "krr_precision_map", "krr_factor_bytes", "krr_factor_tile_offset",
+           "krr_potrf_mp_workspace", "krr_potrf_mp", "krr_potrs_workspace", "krr_potrs",
+           "krr_associate_host_arena", "krr_associate_host", "krr_last_launch_count"]
+
+
+class KrrError(RuntimeError):
+    pass
+
+
+def library_path():
+    return os.path.join(_HERE, "libkrr_mp.so")
+
+
+def lib():
+    """Load libkrr_mp.so (built in-tree by build.py).  Fails loudly when it is missing."""
+    global _LIB
+    if _LIB is not None:
+        return _LIB
+    path = library_path()
+    if not os.path.exists(path):
+        raise KrrError(f"{path} not found: build it with `python -m paper_2409_01712_b200.build` "
+                       "(there is no CPU fallback)")
+    L = ctypes.CDLL(path)
+    c = ctypes
+    vp, i64, u32, sz = c.c_void_p, c.c_int64, c.c_uint, c.c_size_t
+    L.krr_version.restype = c.c_int
+    L.krr_built_for_sm.restype = c.c_int
+    L.krr_tile_slot.restype = i64
+    L.krr_tile_slot.argtypes = [c.c_int, c.c_int, c.c_int]
+    L.krr_precision_map_workspace.restype = sz
+    L.krr_precision_map_workspace.argtypes = [i64, c.c_int]
+    L.krr_precision_map.restype = c.c_int
+    L.krr_precision_map.argtypes = [vp, i64, i64, c.c_int, c.c_float, u32, u32, vp, vp, vp, vp, vp, sz, vp]
+    L.krr_factor_bytes.restype = sz
+    L.krr_factor_bytes.argtypes = [i64, c.c_int, vp]
+    L.krr_factor_tile_offset.restype = i64
+    L.krr_factor_tile_offset.argtypes = [i64, c.c_int, vp, c.c_int, c.c_int]
+    L.krr_potrf_mp_workspace.restype = sz
+    L.krr_potrf_mp_workspace.argtypes = [i64, c.c_int, vp]
+    L.krr_potrf_mp.restype = c.c_int
+    L.krr_potrf_mp.argtypes = [vp, i64, i64, c.c_int, vp, vp, vp, vp, vp, vp, sz, u32, vp]
+    L.krr_potrs_workspace.restype = sz
+    L.krr_potrs_workspace.argtypes = [i64, c.c_int, c.c_int]
+    L.krr_potrs.restype = c.c_int
+    L.krr_potrs.argtypes = [vp, vp, vp, vp, i64, c.c_int, vp, i64, c.c_int, vp, sz, vp]
+    L.krr_associate_host_arena.restype = sz
+    L.krr_associate_host_arena.argtypes = [i64, c.c_int, c.c_int]
+    L.krr_associate_host.restype = c.c_int
+    L.krr_associate_host.argtypes = [vp, i64, i64, c.c_int, c.c_float, u32, c.c_int, u32, vp, c.c_int, vp,
+                                     vp, vp, vp, sz, vp]
+    L.krr_last_launch_count.restype = i64
+    _LIB = L
+    return L
+
+
+def _check(rc, what):
+    if rc != 0:
+        raise KrrError(f"{what} failed: {ERRORS.get(rc, rc)}")
+
+
+def _stream():
+    return ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def _ptr(t):
+    return ctypes.c_void_p(t.data_ptr()) if t is not None else ctypes.c_void_p(0)
+
+
+def _ws(nbytes, device):
+    # torch's caching allocator returns 512-byte aligned blocks; over-allocate and align to 1 KiB
+    buf = torch.empty(nbytes + 1024, dtype=torch.uint8, device=device)
+    shift = (-buf.data_ptr()) % 1024
+    return buf[shift:shift + nbytes]
+
+
+def last_launch_count():
+    return int(lib().krr_last_launch_count())
+
+
+def tile_slot(NT, i, j):
+    return int(lib().krr_tile_slot(NT, i, j))
+
+
+def uniform_map(NT, offdiag):
+    """Host map (uint8 NT x NT): diagonal FP32, every off-diagonal tile `offdiag`, 255 above."""
+    m = torch.full((NT, NT), 255, dtype=torch.uint8)
+    idx = torch.tril_indices(NT, NT, -1)
+    m[idx[0], idx[1]] = offdiag
+    m[torch.arange(NT), torch.arange(NT)] = FP32
+    return m
+
+
+def _host_map(h_map):
+    h = h_map.detach().to("cpu", torch.uint8).contiguous()
+    return h
+
+
+def factor_bytes(n, nb, h_map):
+    h = _host_map(h_map)
+    return int(lib().krr_factor_bytes(n, nb, _ptr(h)))
+
+
+def factor_tile_offset(n, nb, h_map, i, j):
+    h = _host_map(h_map)
+    return int(lib().krr_factor_tile_offset(n, nb, _ptr(h), i, j))
+
+
+def precision_map(A, nb, eps_target, allowed=(FP32, FP16, FP8), flags=0, n=None):
+    """krr_precision_map.  A: CUDA FP32 (n x n row-major, or the packed lower tiles with
+    FLAG_A_TILED_LOWER and n given).  Returns (d_map uint8 NT x NT, tile norms, tile amax, fro)."""
+    L = lib()
+    if flags & FLAG_A_TILED_LOWER:
+        assert n is not None
+        lda = nb
+    else:
+        n, lda = A.shape[0], A.stride(0)
+    NT = n // nb
+    dev = A.device
+    d_map = torch.empty((NT, NT), dtype=torch.uint8, device=dev)
+    norms = torch.empty((NT, NT), dtype=torch.float32, device=dev)
+    amax = torch.empty((NT, NT), dtype=torch.float32, device=dev)
+    fro = torch.empty(1, dtype=torch.float64, device=dev)
+    wsb = int(L.krr_precision_map_workspace(n, nb))
+    if wsb == 0:
+        raise KrrError("krr_precision_map_workspace: invalid shape")
+    ws = _ws(wsb, dev)
+    mask = sum(1 << p for p in allowed)
+    _check(L.krr_precision_map(_ptr(A), n, lda, nb, float(eps_target), mask, flags, _ptr(d_map), _ptr(norms),
+                               _ptr(amax), _ptr(fro), _ptr(ws), wsb, _stream()), "krr_precision_map")
+    return d_map, norms, amax, fro
+
+
+@dataclass
+class Factor:
+    """Result of potrf_mp: the tile mosaic and what krr_potrs needs."""
+    n: int
+    nb: int
+    h_map: torch.Tensor        # host uint8 NT x NT
+    d_map: torch.Tensor        # device copy
+    payload: torch.Tensor      # device uint8, krr_factor_bytes
+    scales: torch.Tensor       # device float32 NT x NT
+    info: torch.Tensor         # device int32 [1]
+    ws: torch.Tensor           # device workspace (FP16 operand images), kept alive
+
+    @property
+    def NT(self):
+        return self.n // self.nb
+
+    def tile(self, i, j):
+        """Dequantised tile (i,j) as a float64 CUDA tensor (test / inspection helper)."""
+        nb, NT = self.nb, self.NT
+        p = int(self.h_map[i, j])
+        off = factor_tile_offset(self.n, nb, self.h_map, i, j)
+        nbytes = nb * nb * (4, 2, 1)[p]
+        raw = self.payload[off:off + nbytes]
+        if p == FP32:
+            return raw.view(torch.float32).reshape(nb, nb).to(torch.float64)
+        if p == FP16:
+            return raw.view(torch.float16).reshape(nb, nb).to(torch.float64)
+        return raw.view(torch.float8_e4m3fn).reshape(nb, nb).to(torch.float64) * float(self.scales[i, j])
+
+    def dense(self):
+        """Dense dequantised lower-triangular factor, float64, on the factor's device."""
+        n, nb, NT = self.n, self.nb, self.NT
+        Ld = torch.zeros((n, n), dtype=torch.float64, device=self.payload.device)
+        for j in range(NT):
+            for i in range(j, NT):
+                Ld[i * nb:(i + 1) * nb, j * nb:(j + 1) * nb] = self.tile(i, j)
+        return Ld
+
+
+def potrf_mp(A, nb, d_map, h_map=None, flags=FLAG_PREROUND_A, n=None):
+    """krr_potrf_mp.  Returns a Factor; `info` is read by the caller after synchronising."""
+    L = lib()
+    if flags & FLAG_A_TILED_LOWER:
+        assert n is not None
+        lda = nb
+    else:
+        n, lda = A.shape[0], A.stride(0)
+    dev = A.device
+    NT = n // nb
+    h = _host_map(d_map if h_map is None else h_map)
+    d_map = d_map.to(dev, torch.uint8).contiguous()
+    fb = int(L.krr_factor_bytes(n, nb, _ptr(h)))
+    wsb = int(L.krr_potrf_mp_workspace(n, nb, _ptr(h)))
+    if fb == 0 or wsb == 0:
+        raise KrrError("invalid shape or precision map")
+    payload = _ws(fb, dev)
+    ws = _ws(wsb, dev)
+    scales = torch.empty((NT, NT), dtype=torch.float32, device=dev)
+    info = torch.empty(1, dtype=torch.int32, device=dev)
+    _check(L.krr_potrf_mp(_ptr(A), n, lda, nb, _ptr(d_map), _ptr(h), _ptr(payload), _ptr(scales), _ptr(info),
+                          _ptr(ws), wsb, flags, _stream()), "krr_potrf_mp")
+    return Factor(n, nb, h, d_map, payload, scales, info, ws)
+
+
+def potrs(factor, B):
+    """krr_potrs, in place on B (CUDA FP32, n x nrhs row-major).  Returns B."""
+    L = lib()
+    assert B.dtype == torch.float32 and B.is_cuda and B.stride(1) == 1
+    n, nrhs = B.shape
+    wsb = int(L.krr_potrs_workspace(n, factor.nb, nrhs))
+    if wsb == 0:
+        raise KrrError("krr_potrs_workspace: invalid shape / nrhs")
+    ws = _ws(wsb, B.device)
+    _check(L.krr_potrs(_ptr(factor.payload), _ptr(factor.scales), _ptr(factor.d_map), _ptr(factor.h_map), n,
+                       factor.nb, _ptr(B), B.stride(0), nrhs, _ptr(ws), wsb, _stream()), "krr_potrs")
+    return B
+
+
+def associate_host(h_A, nb, h_Y, eps_target=0.0, allowed=(FP32,), force_prec=-1, flags=FLAG_PREROUND_A,
+                   arena=None, device="cuda"):
+    """krr_associate_host: whole Associate phase from host tensors (pinned recommended).
+    Returns (alpha host tensor, h_map, info int, arena)."""
+    L = lib()
+    n, lda = h_A.shape[0], h_A.stride(0)
+    nrhs = h_Y.shape[1]
+    NT = n // nb
+    need = int(L.krr_associate_host_arena(n, nb, nrhs))
+    if need == 0:
+        raise KrrError("krr_associate_host_arena: invalid shape")
+    if arena is None or arena.numel() < need:
+        arena = _ws(need, device)
+    alpha = torch.empty_like(h_Y)
+    h_map = torch.empty((NT, NT), dtype=torch.uint8)
+    h_info = torch.zeros(1, dtype=torch.int32)
+    mask = sum(1 << p for p in allowed)
+    _check(L.krr_associate_host(_ptr(h_A), n, lda, nb, float(eps_target), mask, force_prec, flags, _ptr(h_Y), nrhs,
+                                _ptr(alpha), _ptr(h_map), _ptr(h_info), _ptr(arena), arena.numel(), _stream()),
+           "krr_associate_host")
+    return alpha, h_map, int(h_info[0]), arena

@@ -1,0 +1,494 @@
+// C ABI of the library (include/krr_mp.h): argument checks, workspace layout, and the host-side
+// launch sequence of the tile-column pipeline.  Everything numerical runs in the kernels of
+// precision_map.cuh, gemm_tc.cuh, panel.cuh and potrs.cuh.
+#include <cuda.h>
+#include <cuda_runtime.h>
+
+#include <cstdio>
+#include <cstring>
+#include <vector>
+
+#include "common.cuh"
+#include "gemm_tc.cuh"
+#include "panel.cuh"
+#include "potrs.cuh"
+#include "precision_map.cuh"
+
+namespace krr {
+
+thread_local int64_t g_launches = 0;
+
+static inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+static int check_device(int* num_sms) {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return KRR_ERR_CUDA;
+    int major = 0, sms = 0;
+    if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess) return KRR_ERR_CUDA;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return KRR_ERR_CUDA;
+    if (major != 10) return KRR_ERR_DEVICE;
+    if (num_sms) *num_sms = sms;
+    return KRR_OK;
+}
+
+static int check_shape(int64_t n, int nb) {
+    if (n <= 0 || nb <= 0) return KRR_ERR_ARG;
+    if (nb % kBlk != 0 || n % nb != 0 || nb > 4096) return KRR_ERR_SHAPE;
+    if (n / nb > kMaxNT) return KRR_ERR_SHAPE;
+    return KRR_OK;
+}
+
+static int check_map(int NT, const uint8_t* h_map, bool* any_fp8) {
+    bool f8 = false;
+    for (int i = 0; i < NT; ++i)
+        for (int j = 0; j <= i; ++j) {
+            const uint8_t p = h_map[i * NT + j];
+            if (p > KRR_FP8_E4M3) return KRR_ERR_MAP;
+            if (i == j && p != KRR_FP32) return KRR_ERR_MAP;
+            f8 |= (p == KRR_FP8_E4M3);
+        }
+    if (any_fp8) *any_fp8 = f8;
+    return KRR_OK;
+}
+
+// ---- tensor maps ---------------------------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static EncodeTiledFn get_encode_fn() {
+    static EncodeTiledFn fn = nullptr;
+    if (fn) return fn;
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess ||
+        q != cudaDriverEntryPointSuccess)
+        return nullptr;
+    fn = reinterpret_cast<EncodeTiledFn>(p);
+    return fn;
+}
+
+// Row-major [rows][cols] array of 2-byte elements, box = 64 columns x 128 rows, 128-byte swizzle.
+static int make_plane_tmap(CUtensorMap* tm, const void* base, uint64_t rows, uint64_t cols) {
+    EncodeTiledFn enc = get_encode_fn();
+    if (!enc) return KRR_ERR_CUDA;
+    cuuint64_t gdim[2] = {cols, rows};
+    cuuint64_t gstride[1] = {cols * 2};
+    cuuint32_t box[2] = {static_cast<cuuint32_t>(kBlockK), static_cast<cuuint32_t>(kBlk)};
+    cuuint32_t estr[2] = {1, 1};
+    CUresult r = enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 2, const_cast<void*>(base), gdim, gstride, box, estr,
+                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS ? KRR_OK : KRR_ERR_CUDA;
+}
+
+// ---- mosaic offsets (host) -------------------------------------------------------------------
+static size_t host_offsets(int NT, int nb, const uint8_t* h_map, std::vector<int64_t>* off) {
+    size_t acc = 0;
+    const size_t elems = static_cast<size_t>(nb) * nb;
+    if (off) off->assign(static_cast<size_t>(NT) * NT, -1);
+    for (int j = 0; j < NT; ++j)
+        for (int i = j; i < NT; ++i) {
+            if (off) (*off)[static_cast<size_t>(i) * NT + j] = static_cast<int64_t>(acc);
+            acc += elems * prec_bytes(h_map[i * NT + j]);
+        }
+    return acc;
+}
+
+// ---- workspace layout of krr_potrf_mp ----------------------------------------------------------
+struct PotrfWs {
+    size_t off_table, a_amax, tile_amax, scl, W, linv_hi, linv_lo, Hp, Lp, Qp, total;
+};
+static PotrfWs potrf_ws_layout(int64_t n, int nb, bool any_fp8) {
+    const int64_t NT = n / nb;
+    const size_t nslots = static_cast<size_t>(NT) * (NT + 1) / 2;
+    const size_t plane = nslots * nb * nb;
+    PotrfWs w;
+    size_t o = 0;
+    w.off_table = o; o = align_up(o + NT * NT * sizeof(int64_t), 1024);
+    w.a_amax = o;    o = align_up(o + NT * NT * sizeof(float), 1024);
+    w.tile_amax = o; o = align_up(o + nslots * sizeof(float), 1024);
+    w.scl = o;       o = align_up(o + (4 + nb / kBlk) * sizeof(float), 1024);
+    w.W = o;         o = align_up(o + static_cast<size_t>(n) * nb * sizeof(float), 1024);
+    w.linv_hi = o;   o = align_up(o + static_cast<size_t>(nb) * kBlk * 2, 1024);
+    w.linv_lo = o;   o = align_up(o + static_cast<size_t>(nb) * kBlk * 2, 1024);
+    w.Hp = o;        o = align_up(o + plane * 2, 1024);
+    w.Lp = o;        o = align_up(o + plane * 2, 1024);
+    w.Qp = o;        if (any_fp8) o = align_up(o + plane, 1024);
+    w.total = o;
+    return w;
+}
+
+template <typename K, typename... Args>
+static int launch(K kernel, dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args... args) {
+    kernel<<<grid, block, smem, st>>>(args...);
+    ++g_launches;
+    return cudaGetLastError() == cudaSuccess ? KRR_OK : KRR_ERR_CUDA;
+}
+
+static int launch_gemm(const CUtensorMap& a_hi, const CUtensorMap& a_lo, const CUtensorMap& b_hi,
+                       const CUtensorMap& b_lo, const GemmOp& op, int num_sms, cudaStream_t st) {
+    const int ntiles = op.nrb * op.ncb;
+    if (ntiles <= 0) return KRR_OK;
+    const int grid = ntiles < num_sms ? ntiles : num_sms;
+    gemm_tc_kernel<<<grid, kGemmThreads, kGemmSmem, st>>>(a_hi, a_lo, b_hi, b_lo, op);
+    ++g_launches;
+    return cudaGetLastError() == cudaSuccess ? KRR_OK : KRR_ERR_CUDA;
+}
+
+static int set_kernel_attrs() {
+    static bool done = false;
+    if (done) return KRR_OK;
+    KRR_CUDA_CHECK(cudaFuncSetAttribute(gemm_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem));
+    KRR_CUDA_CHECK(cudaFuncSetAttribute(potrf128_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kPotrfSmem));
+    const int big = 200 * 1024;
+    KRR_CUDA_CHECK(cudaFuncSetAttribute(potrs_fwd_update_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
+    KRR_CUDA_CHECK(cudaFuncSetAttribute(potrs_fwd_update_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
+    KRR_CUDA_CHECK(cudaFuncSetAttribute(potrs_fwd_update_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
+    KRR_CUDA_CHECK(cudaFuncSetAttribute(potrs_fwd_update_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
+    KRR_CUDA_CHECK(cudaFuncSetAttribute(potrs_bwd_update_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
+    KRR_CUDA_CHECK(cudaFuncSetAttribute(potrs_bwd_update_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
+    KRR_CUDA_CHECK(cudaFuncSetAttribute(potrs_bwd_update_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
+    KRR_CUDA_CHECK(cudaFuncSetAttribute(potrs_bwd_update_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
+    KRR_CUDA_CHECK(cudaFuncSetAttribute(potrs_diag_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
+    KRR_CUDA_CHECK(cudaFuncSetAttribute(potrs_diag_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
+    KRR_CUDA_CHECK(cudaFuncSetAttribute(potrs_diag_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
+    KRR_CUDA_CHECK(cudaFuncSetAttribute(potrs_diag_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
+    done = true;
+    return KRR_OK;
+}
+
+}  // namespace krr
+
+using namespace krr;
+
+extern "C" {
+
+int krr_version(void) { return 100; }
+int krr_built_for_sm(void) { return 100; }
+int64_t krr_last_launch_count(void) { return g_launches; }
+
+int64_t krr_tile_slot(int NT, int i, int j) {
+    if (NT <= 0 || j < 0 || i < j || i >= NT) return -1;
+    return tile_slot(NT, i, j);
+}
+
+// ------------------------------------------------------------------------- precision map
+size_t krr_precision_map_workspace(int64_t n, int nb) {
+    if (check_shape(n, nb) != KRR_OK) return 0;
+    const size_t NT = n / nb, nslots = NT * (NT + 1) / 2, chunks = nb / kStatRows;
+    return align_up(nslots * chunks * sizeof(double), 1024) + align_up(nslots * chunks * sizeof(float), 1024) +
+           align_up(nslots * sizeof(double), 1024);
+}
+
+int krr_precision_map(const float* d_A, int64_t n, int64_t lda, int nb, float eps_target, unsigned allowed_mask,
+                      unsigned flags, uint8_t* d_map, float* d_tile_norms, float* d_tile_amax, double* d_fro,
+                      void* d_ws, size_t ws_bytes, void* stream) {
+    g_launches = 0;
+    if (!d_A || !d_map || !d_ws) return KRR_ERR_ARG;
+    int rc = check_shape(n, nb);
+    if (rc) return rc;
+    const bool tiled = flags & KRR_FLAG_A_TILED_LOWER;
+    if (!tiled && (lda < n || lda % 4 != 0)) return KRR_ERR_ARG;
+    if (reinterpret_cast<uintptr_t>(d_A) % 16 != 0) return KRR_ERR_ARG;
+    if (flags & ~(KRR_FLAG_PREROUND_A | KRR_FLAG_A_TILED_LOWER)) return KRR_ERR_UNSUPPORTED;
+    if (ws_bytes < krr_precision_map_workspace(n, nb)) return KRR_ERR_WORKSPACE;
+    rc = check_device(nullptr);
+    if (rc) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const int NT = static_cast<int>(n / nb);
+    const size_t nslots = static_cast<size_t>(NT) * (NT + 1) / 2, chunks = nb / kStatRows;
+    uint8_t* ws = static_cast<uint8_t*>(d_ws);
+    double* partial = reinterpret_cast<double*>(ws);
+    float* pamax = reinterpret_cast<float*>(ws + align_up(nslots * chunks * sizeof(double), 1024));
+    double* sumsq = reinterpret_cast<double*>(reinterpret_cast<uint8_t*>(pamax) + align_up(nslots * chunks * sizeof(float), 1024));
+    AView A{d_A, lda, tiled ? 1 : 0, NT, nb};
+    rc = launch(tile_stats_kernel, dim3(static_cast<unsigned>(chunks), static_cast<unsigned>(nslots)), dim3(kStatThreads), 0, st,
+                A, partial, pamax);
+    if (rc) return rc;
+    return launch(map_decide_kernel, dim3(1), dim3(1024), 0, st, NT, static_cast<int>(chunks),
+                  static_cast<const double*>(partial), static_cast<const float*>(pamax), eps_target, allowed_mask, d_map,
+                  d_tile_norms, d_tile_amax, d_fro, sumsq);
+}
+
+// ------------------------------------------------------------------------- factor layout
+size_t krr_factor_bytes(int64_t n, int nb, const uint8_t* h_map) {
+    if (!h_map || check_shape(n, nb) != KRR_OK) return 0;
+    const int NT = static_cast<int>(n / nb);
+    if (check_map(NT, h_map, nullptr) != KRR_OK) return 0;
+    return host_offsets(NT, nb, h_map, nullptr);
+}
+
+int64_t krr_factor_tile_offset(int64_t n, int nb, const uint8_t* h_map, int i, int j) {
+    if (!h_map || check_shape(n, nb) != KRR_OK) return -1;
+    const int NT = static_cast<int>(n / nb);
+    if (j < 0 || i < j || i >= NT || check_map(NT, h_map, nullptr) != KRR_OK) return -1;
+    std::vector<int64_t> off;
+    host_offsets(NT, nb, h_map, &off);
+    return off[static_cast<size_t>(i) * NT + j];
+}
+
+// ------------------------------------------------------------------------- factorisation
+size_t krr_potrf_mp_workspace(int64_t n, int nb, const uint8_t* h_map) {
+    if (!h_map || check_shape(n, nb) != KRR_OK) return 0;
+    bool f8 = false;
+    if (check_map(static_cast<int>(n / nb), h_map, &f8) != KRR_OK) return 0;
+    return potrf_ws_layout(n, nb, f8).total;
+}
+
+int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t* d_map, const uint8_t* h_map,
+                 void* d_factor, float* d_scales, int* d_info, void* d_ws, size_t ws_bytes, unsigned flags,
+                 void* stream) {
+    g_launches = 0;
+    if (!d_A || !d_map || !h_map || !d_factor || !d_scales || !d_info || !d_ws) return KRR_ERR_ARG;
+    int rc = check_shape(n, nb);
+    if (rc) return rc;
+    const bool tiled = flags & KRR_FLAG_A_TILED_LOWER;
+    if (!tiled && (lda < n || lda % 4 != 0)) return KRR_ERR_ARG;
+    if (reinterpret_cast<uintptr_t>(d_A) % 16 != 0 || reinterpret_cast<uintptr_t>(d_ws) % 1024 != 0 ||
+        reinterpret_cast<uintptr_t>(d_factor) % 128 != 0)
+        return KRR_ERR_ARG;
+    if (flags & ~(KRR_FLAG_PREROUND_A | KRR_FLAG_A_TILED_LOWER)) return KRR_ERR_UNSUPPORTED;
+    const int NT = static_cast<int>(n / nb);
+    bool any_fp8 = false;
+    rc = check_map(NT, h_map, &any_fp8);
+    if (rc) return rc;
+    const PotrfWs L = potrf_ws_layout(n, nb, any_fp8);
+    if (ws_bytes < L.total) return KRR_ERR_WORKSPACE;
+    int num_sms = 0;
+    rc = check_device(&num_sms);
+    if (rc) return rc;
+    rc = set_kernel_attrs();
+    if (rc) return rc;
+
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    uint8_t* ws = static_cast<uint8_t*>(d_ws);
+    int64_t* off = reinterpret_cast<int64_t*>(ws + L.off_table);
+    float* a_amax = reinterpret_cast<float*>(ws + L.a_amax);
+    float* tile_amax = reinterpret_cast<float*>(ws + L.tile_amax);
+    float* W = reinterpret_cast<float*>(ws + L.W);
+    float* scl = reinterpret_cast<float*>(ws + L.scl);
+    float* linv_scale = scl + 4;
+    __half* linv_hi = reinterpret_cast<__half*>(ws + L.linv_hi);
+    __half* linv_lo = reinterpret_cast<__half*>(ws + L.linv_lo);
+    __half* Hp = reinterpret_cast<__half*>(ws + L.Hp);
+    __half* Lp = reinterpret_cast<__half*>(ws + L.Lp);
+    uint8_t* Qp = any_fp8 ? ws + L.Qp : nullptr;
+    const size_t nslots = static_cast<size_t>(NT) * (NT + 1) / 2;
+    AView A{d_A, lda, tiled ? 1 : 0, NT, nb};
+
+    KRR_CUDA_CHECK(cudaMemsetAsync(d_info, 0, sizeof(int), st));
+    KRR_CUDA_CHECK(cudaMemsetAsync(d_scales, 0, static_cast<size_t>(NT) * NT * sizeof(float), st));
+    KRR_CUDA_CHECK(cudaMemsetAsync(tile_amax, 0, nslots * sizeof(float), st));
+    rc = launch(offsets_kernel, dim3(1), dim3(32), 0, st, NT, nb, d_map, off);
+    if (rc) return rc;
+    rc = launch(plane_scale_kernel, dim3(1), dim3(1024), 0, st, A, n, scl);
+    if (rc) return rc;
+    const bool preround = flags & KRR_FLAG_PREROUND_A;
+    if (preround && any_fp8) {
+        KRR_CUDA_CHECK(cudaMemsetAsync(a_amax, 0, static_cast<size_t>(NT) * NT * sizeof(float), st));
+        rc = launch(tile_amax_kernel, dim3(nb / 32, static_cast<unsigned>(nslots)), dim3(256), 0, st, A, d_map, a_amax);
+        if (rc) return rc;
+    }
+
+    CUtensorMap tmH, tmL, tmIH, tmIL;
+    if (make_plane_tmap(&tmH, Hp, nslots * nb, nb) || make_plane_tmap(&tmL, Lp, nslots * nb, nb) ||
+        make_plane_tmap(&tmIH, linv_hi, nb, kBlk) || make_plane_tmap(&tmIL, linv_lo, nb, kBlk))
+        return KRR_ERR_CUDA;
+
+    const int nsub = nb / kBlk;
+    for (int k = 0; k < NT; ++k) {
+        const int mblk = (NT - k) * nsub;             // 128-row blocks of the panel
+        GemmOp op;
+        memset(&op, 0, sizeof(op));
+        op.nb = nb; op.NT = NT; op.k = k;
+        op.prow0 = tile_slot(NT, k, k) * nb;
+        op.map = d_map; op.A = A; op.a_amax = (preround && any_fp8) ? a_amax : nullptr;
+        op.W = W; op.Hp = Hp; op.Lp = Lp; op.tile_amax = tile_amax; op.flags = flags;
+        op.scl = scl; op.linv_scale = linv_scale;
+        // U(k): S = rd(A) - L[:, 0:k] L[k, 0:k]^T over the whole tile column
+        op.mode = MODE_UPDATE; op.c = 0; op.rb0 = 0; op.nrb = mblk; op.cb0 = 0; op.ncb = nsub;
+        rc = launch_gemm(tmH, tmL, tmH, tmL, op, num_sms, st);
+        if (rc) return rc;
+        for (int c = 0; c < nsub; ++c) {
+            if (c > 0) {
+                op.mode = MODE_P1; op.c = c; op.rb0 = c; op.nrb = mblk - c; op.cb0 = c; op.ncb = 1;
+                rc = launch_gemm(tmH, tmL, tmH, tmL, op, num_sms, st);
+                if (rc) return rc;
+            }
+            rc = launch(potrf128_kernel, dim3(1), dim3(kPotrfThreads), static_cast<size_t>(kPotrfSmem), st, W, nb,
+                        c * kBlk, c * kBlk, linv_hi, linv_lo, linv_scale, d_info,
+                        static_cast<int64_t>(k) * nb + static_cast<int64_t>(c) * kBlk + 1);
+            if (rc) return rc;
+            if (mblk - c - 1 > 0) {
+                op.mode = MODE_P3; op.c = c; op.rb0 = c + 1; op.nrb = mblk - c - 1; op.cb0 = c; op.ncb = 1;
+                rc = launch_gemm(tmH, tmL, tmIH, tmIL, op, num_sms, st);
+                if (rc) return rc;
+            }
+        }
+        rc = launch(finalize_kernel, dim3(nb / 16, NT - k), dim3(256), 0, st, NT, nb, k, static_cast<const float*>(W),
+                    d_map, static_cast<const int64_t*>(off), static_cast<const float*>(tile_amax),
+                    static_cast<uint8_t*>(d_factor), d_scales, Hp, Qp, static_cast<const float*>(scl));
+        if (rc) return rc;
+    }
+    return KRR_OK;
+}
+
+// ------------------------------------------------------------------------- solve
+size_t krr_potrs_workspace(int64_t n, int nb, int nrhs) {
+    if (check_shape(n, nb) != KRR_OK || nrhs < 1 || nrhs > kMaxRhs) return 0;
+    const size_t NT = n / nb;
+    return align_up(NT * NT * sizeof(int64_t), 1024);
+}
+
+}  // extern "C"
+
+template <int NRHS>
+static int potrs_run(const uint8_t* factor, const float* d_scales, const uint8_t* d_map, const std::vector<int64_t>& hoff,
+                     const int64_t* off, int NT, int nb, float* B, int64_t ldb, int nrhs, cudaStream_t st) {
+    const size_t smem_z = static_cast<size_t>(NRHS) * nb * sizeof(float);
+    const size_t smem_d = smem_z + (32 * 33 + 8 * 32 * NRHS) * sizeof(float);
+    int rc;
+    for (int k = 0; k < NT; ++k) {
+        const float* Lkk = reinterpret_cast<const float*>(factor + hoff[static_cast<size_t>(k) * NT + k]);
+        float* Bk = B + static_cast<int64_t>(k) * nb * ldb;
+        rc = launch(potrs_diag_kernel<NRHS>, dim3(1), dim3(256), smem_d, st, nb, Lkk, Bk, ldb, nrhs, 0);
+        if (rc) return rc;
+        if (k + 1 < NT) {
+            rc = launch(potrs_fwd_update_kernel<NRHS>, dim3((NT - k - 1) * (nb / 32)), dim3(256), smem_z, st, NT, nb, k,
+                        factor, off, d_map, d_scales, B, ldb, nrhs);
+            if (rc) return rc;
+        }
+    }
+    for (int k = NT - 1; k >= 0; --k) {
+        const float* Lkk = reinterpret_cast<const float*>(factor + hoff[static_cast<size_t>(k) * NT + k]);
+        float* Bk = B + static_cast<int64_t>(k) * nb * ldb;
+        rc = launch(potrs_diag_kernel<NRHS>, dim3(1), dim3(256), smem_d, st, nb, Lkk, Bk, ldb, nrhs, 1);
+        if (rc) return rc;
+        if (k > 0) {
+            rc = launch(potrs_bwd_update_kernel<NRHS>, dim3(k * (nb / 128)), dim3(128), smem_z, st, NT, nb, k, factor, off,
+                        d_map, d_scales, B, ldb, nrhs);
+            if (rc) return rc;
+        }
+    }
+    return KRR_OK;
+}
+
+extern "C" {
+
+int krr_potrs(const void* d_factor, const float* d_scales, const uint8_t* d_map, const uint8_t* h_map, int64_t n,
+              int nb, float* d_B, int64_t ldb, int nrhs, void* d_ws, size_t ws_bytes, void* stream) {
+    g_launches = 0;
+    if (!d_factor || !d_scales || !d_map || !h_map || !d_B || !d_ws) return KRR_ERR_ARG;
+    int rc = check_shape(n, nb);
+    if (rc) return rc;
+    if (nrhs < 1 || nrhs > kMaxRhs || ldb < nrhs) return KRR_ERR_ARG;
+    const int NT = static_cast<int>(n / nb);
+    rc = check_map(NT, h_map, nullptr);
+    if (rc) return rc;
+    if (ws_bytes < krr_potrs_workspace(n, nb, nrhs)) return KRR_ERR_WORKSPACE;
+    rc = check_device(nullptr);
+    if (rc) return rc;
+    rc = set_kernel_attrs();
+    if (rc) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    std::vector<int64_t> hoff;
+    host_offsets(NT, nb, h_map, &hoff);
+    int64_t* off = static_cast<int64_t*>(d_ws);
+    rc = launch(offsets_kernel, dim3(1), dim3(32), 0, st, NT, nb, d_map, off);
+    if (rc) return rc;
+    const uint8_t* factor = static_cast<const uint8_t*>(d_factor);
+    if (nrhs <= 4) return potrs_run<4>(factor, d_scales, d_map, hoff, off, NT, nb, d_B, ldb, nrhs, st);
+    if (nrhs <= 8) return potrs_run<8>(factor, d_scales, d_map, hoff, off, NT, nb, d_B, ldb, nrhs, st);
+    if (nrhs <= 16) return potrs_run<16>(factor, d_scales, d_map, hoff, off, NT, nb, d_B, ldb, nrhs, st);
+    return potrs_run<32>(factor, d_scales, d_map, hoff, off, NT, nb, d_B, ldb, nrhs, st);
+}
+
+}  // extern "C"
+
+// ------------------------------------------------------------------------- host-buffer Associate
+namespace {
+struct Arena {
+    size_t A, Y, map, norms, amax, fro, info, scales, pm_ws, factor, potrf_ws, potrs_ws, total;
+};
+Arena arena_layout(int64_t n, int nb, int nrhs) {
+    const size_t NT = n / nb, nslots = NT * (NT + 1) / 2;
+    Arena a;
+    size_t o = 0;
+    a.A = o;        o = align_up(o + static_cast<size_t>(n) * n * sizeof(float), 1024);
+    a.Y = o;        o = align_up(o + static_cast<size_t>(n) * nrhs * sizeof(float), 1024);
+    a.map = o;      o = align_up(o + NT * NT, 1024);
+    a.norms = o;    o = align_up(o + NT * NT * sizeof(float), 1024);
+    a.amax = o;     o = align_up(o + NT * NT * sizeof(float), 1024);
+    a.fro = o;      o = align_up(o + sizeof(double), 1024);
+    a.info = o;     o = align_up(o + sizeof(int), 1024);
+    a.scales = o;   o = align_up(o + NT * NT * sizeof(float), 1024);
+    a.pm_ws = o;    o = align_up(o + krr_precision_map_workspace(n, nb), 1024);
+    a.factor = o;   o = align_up(o + nslots * nb * nb * sizeof(float), 1024);
+    a.potrf_ws = o; o = align_up(o + potrf_ws_layout(n, nb, true).total, 1024);
+    a.potrs_ws = o; o = align_up(o + krr_potrs_workspace(n, nb, nrhs), 1024);
+    a.total = o;
+    return a;
+}
+}  // namespace
+
+extern "C" {
+
+size_t krr_associate_host_arena(int64_t n, int nb, int nrhs) {
+    if (check_shape(n, nb) != KRR_OK || nrhs < 1 || nrhs > kMaxRhs) return 0;
+    return arena_layout(n, nb, nrhs).total;
+}
+
+int krr_associate_host(const float* h_A, int64_t n, int64_t lda, int nb, float eps_target, unsigned allowed_mask,
+                       int force_prec, unsigned flags, const float* h_Y, int nrhs, float* h_alpha, uint8_t* h_map,
+                       int* h_info, void* d_arena, size_t arena_bytes, void* stream) {
+    if (!h_A || !h_Y || !h_alpha || !h_map || !h_info || !d_arena) return KRR_ERR_ARG;
+    int rc = check_shape(n, nb);
+    if (rc) return rc;
+    if (nrhs < 1 || nrhs > kMaxRhs || lda < n) return KRR_ERR_ARG;
+    if (flags & KRR_FLAG_A_TILED_LOWER) return KRR_ERR_UNSUPPORTED;
+    if (force_prec > KRR_FP8_E4M3) return KRR_ERR_ARG;
+    const Arena L = arena_layout(n, nb, nrhs);
+    if (arena_bytes < L.total) return KRR_ERR_WORKSPACE;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    uint8_t* ar = static_cast<uint8_t*>(d_arena);
+    float* dA = reinterpret_cast<float*>(ar + L.A);
+    float* dY = reinterpret_cast<float*>(ar + L.Y);
+    uint8_t* dmap = ar + L.map;
+    const int NT = static_cast<int>(n / nb);
+    int64_t launches = 0;
+    KRR_CUDA_CHECK(cudaMemcpy2DAsync(dA, n * sizeof(float), h_A, lda * sizeof(float), n * sizeof(float), n,
+                                     cudaMemcpyHostToDevice, st));
+    KRR_CUDA_CHECK(cudaMemcpyAsync(dY, h_Y, static_cast<size_t>(n) * nrhs * sizeof(float), cudaMemcpyHostToDevice, st));
+    if (force_prec < 0) {
+        rc = krr_precision_map(dA, n, n, nb, eps_target, allowed_mask, flags & KRR_FLAG_PREROUND_A, dmap,
+                               reinterpret_cast<float*>(ar + L.norms), reinterpret_cast<float*>(ar + L.amax),
+                               reinterpret_cast<double*>(ar + L.fro), ar + L.pm_ws, L.potrf_ws - L.pm_ws, stream);
+        if (rc) return rc;
+        launches += g_launches;
+        // the launch sequence of the factorisation is built on the host from the map
+        KRR_CUDA_CHECK(cudaMemcpyAsync(h_map, dmap, static_cast<size_t>(NT) * NT, cudaMemcpyDeviceToHost, st));
+        KRR_CUDA_CHECK(cudaStreamSynchronize(st));
+    } else {
+        for (int i = 0; i < NT; ++i)
+            for (int j = 0; j < NT; ++j)
+                h_map[i * NT + j] = (j > i) ? 255 : (i == j ? KRR_FP32 : static_cast<uint8_t>(force_prec));
+        KRR_CUDA_CHECK(cudaMemcpyAsync(dmap, h_map, static_cast<size_t>(NT) * NT, cudaMemcpyHostToDevice, st));
+    }
+    rc = krr_potrf_mp(dA, n, n, nb, dmap, h_map, ar + L.factor, reinterpret_cast<float*>(ar + L.scales),
+                      reinterpret_cast<int*>(ar + L.info), ar + L.potrf_ws, L.potrs_ws - L.potrf_ws,
+                      flags & KRR_FLAG_PREROUND_A, stream);
+    if (rc) return rc;
+    launches += g_launches;
+    rc = krr_potrs(ar + L.factor, reinterpret_cast<float*>(ar + L.scales), dmap, h_map, n, nb, dY, nrhs, nrhs,
+                   ar + L.potrs_ws, L.total - L.potrs_ws, stream);
+    if (rc) return rc;
+    launches += g_launches;
+    KRR_CUDA_CHECK(cudaMemcpyAsync(h_alpha, dY, static_cast<size_t>(n) * nrhs * sizeof(float), cudaMemcpyDeviceToHost, st));
+    KRR_CUDA_CHECK(cudaMemcpyAsync(h_info, ar + L.info, sizeof(int), cudaMemcpyDeviceToHost, st));
+    KRR_CUDA_CHECK(cudaStreamSynchronize(st));
+    g_launches = launches;
+    return KRR_OK;
+}
+
+}  // extern "C"

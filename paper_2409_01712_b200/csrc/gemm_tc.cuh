@@ -1,0 +1,329 @@
+// Tensor-core update kernel of the tile Cholesky.
+//
+// One warp-specialised, persistent tcgen05 kernel serves the three contraction shapes of a tile
+// column k (all "C = base - A * B^T" with K-major FP16 operand images, FP32 accumulation in TMEM):
+//
+//   MODE_UPDATE  S_ik = rd_p(A_ik) - sum_{s<k} L_is L_ks^T      for every tile i >= k   (SYRK+GEMM)
+//   MODE_P1      S[:, c] -= X[:, 0:c] X[c, 0:c]^T               inside the panel (sub-blocks of 128)
+//   MODE_P3      X[:, c]  = S[:, c] * inv(L_cc)^T               the TRSM as a product with the
+//                                                               inverted 128x128 diagonal block
+//
+// Operand images ("planes"): every value x that feeds the tensor cores is kept as FP16 hi = rn(s*x)
+// and, for FP32-class tiles, lo = rn(s*x - hi), with a global power-of-two scale s that lifts the
+// data into the upper FP16 binades (sx = 2^14 / 2^ceil(log2 sqrt(max diag A)) for L and X values,
+// ss likewise for Schur-complement values) -- without it lo falls into the FP16 subnormals and the
+// split keeps only ~17 bits.  The accumulator is rescaled by the exact inverse in the epilogue.
+// An FP32 x FP32 term issues three kind::f16 MMAs (hi*hi + lo*hi + hi*lo), FP32 x {FP16,FP8} two, {FP16,FP8} x {FP16,FP8} one (the hi plane of a
+// low-precision tile holds its stored value exactly).  Accumulators never leave TMEM until the
+// tile's whole K range is done ("round once", R4).
+//
+// Accumulation order: the tensor core adds each MMA's result to the TMEM accumulator with
+// truncation, a bias of ~half an ulp OF THE ACCUMULATOR per instruction (measured: backward error
+// growing linearly in n when K is walked upwards).  In a Cholesky update the leading columns of L
+// carry almost all of sum_k L_ik L_jk, so K is walked DOWNWARDS: the accumulator stays small until
+// the dominant terms arrive last, and the bias stays at the FP32 noise level.
+#pragma once
+#include "common.cuh"
+#include "ptx.cuh"
+
+namespace krr {
+
+enum { MODE_UPDATE = 0, MODE_P1 = 1, MODE_P3 = 2 };
+
+struct GemmOp {
+    int mode;
+    int nb, NT, k;        // tile size, tiles per dimension, tile column being produced
+    int c;                // 128-wide sub-column inside the tile column (P1 / P3)
+    int rb0, nrb;         // output row blocks (128 rows, panel-local: row 0 = top of tile (k,k))
+    int cb0, ncb;         // output column blocks (128 columns inside the tile column)
+    int64_t prow0;        // plane row of panel-local row 0  (= tile_slot(k,k) * nb)
+    const uint8_t* map;   // device precision map (NT*NT)
+    AView A;              // input matrix (MODE_UPDATE base)
+    const float* a_amax;  // NT*NT max|A_ij| (FP8 pre-rounding of A), may be null
+    float* W;             // panel workspace, FP32 [m][nb]
+    __half* Hp;           // hi plane  [nslots*nb][nb]
+    __half* Lp;           // lo plane
+    float* tile_amax;     // per-slot max|X| accumulated by MODE_P3
+    const float* scl;     // device float[4]: sx, ss, 1/sx^2, 1/ss  (power-of-two plane scales)
+    const float* linv_scale;  // device float[nb/128]: scale of each inverted diagonal block's planes
+    unsigned flags;
+};
+
+constexpr int kStages = 3;
+constexpr int kBlockK = 64;                        // fp16 elements per 128-byte swizzle row
+constexpr int kPlaneBytes = kBlk * kBlockK * 2;    // one 128 x 64 fp16 operand block = 16 KB
+constexpr int kStageBytes = 4 * kPlaneBytes;       // A_hi, A_lo, B_hi, B_lo
+constexpr int kAccCols = 128;                      // TMEM columns of one 128x128 FP32 accumulator
+constexpr int kAccBufs = 2;
+constexpr int kTmemCols = kAccCols * kAccBufs;     // 256
+constexpr int kGemmThreads = 192;                  // warp 0 TMA, warp 1 MMA (+TMEM alloc), 2-5 epilogue
+constexpr int kGemmSmem = kStages * kStageBytes + 1024 /*align*/ + 256 /*barriers*/;
+
+struct TermInfo {
+    int64_t a_row, b_row;   // plane rows (TMA coordinate 1)
+    int a_k0, b_k0;         // first K column (TMA coordinate 0)
+    int nchunks;            // K chunks of 64
+    int nA, nB;             // planes per operand: 2 = hi+lo (FP32 class), 1 = hi only
+};
+
+__device__ __forceinline__ TermInfo get_term(const GemmOp& op, int s, int rb, int cb) {
+    TermInfo t;
+    if (op.mode == MODE_UPDATE) {
+        const int i = op.k + (rb * kBlk) / op.nb;
+        const int subrow = (rb * kBlk) % op.nb;
+        t.a_row = tile_slot(op.NT, i, s) * op.nb + subrow;
+        t.b_row = tile_slot(op.NT, op.k, s) * op.nb + cb * kBlk;
+        t.a_k0 = 0;
+        t.b_k0 = 0;
+        t.nchunks = op.nb / kBlockK;
+        t.nA = (op.map[i * op.NT + s] == KRR_FP32) ? 2 : 1;
+        t.nB = (op.map[op.k * op.NT + s] == KRR_FP32) ? 2 : 1;
+    } else if (op.mode == MODE_P1) {
+        t.a_row = op.prow0 + static_cast<int64_t>(rb) * kBlk;
+        t.b_row = op.prow0 + static_cast<int64_t>(op.c) * kBlk;
+        t.a_k0 = 0;
+        t.b_k0 = 0;
+        t.nchunks = op.c * (kBlk / kBlockK);
+        t.nA = 2;
+        t.nB = 2;
+    } else {
+        t.a_row = op.prow0 + static_cast<int64_t>(rb) * kBlk;
+        t.b_row = static_cast<int64_t>(op.c) * kBlk;      // row in the Linv planes
+        t.a_k0 = op.c * kBlk;
+        t.b_k0 = 0;
+        t.nchunks = kBlk / kBlockK;
+        t.nA = 2;
+        t.nB = 2;
+    }
+    return t;
+}
+
+__device__ __forceinline__ int num_terms(const GemmOp& op) {
+    return op.mode == MODE_UPDATE ? op.k : 1;
+}
+
+// Tiles of the diagonal tile that lie entirely above the diagonal are never read: skip them.
+__device__ __forceinline__ bool tile_is_skipped(const GemmOp& op, int rb, int cb) {
+    return op.mode == MODE_UPDATE && (rb * kBlk) < op.nb && cb > rb;
+}
+
+__global__ void __launch_bounds__(kGemmThreads, 1)
+gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_constant__ CUtensorMap tmA_lo,
+               const __grid_constant__ CUtensorMap tmB_hi, const __grid_constant__ CUtensorMap tmB_lo,
+               const GemmOp op) {
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
+    const uint32_t bar_base = smem_base + kStages * kStageBytes;
+    // barriers: full[kStages], empty[kStages], tmem_full[kAccBufs], tmem_empty[kAccBufs], tmem ptr
+    auto full_bar = [&](int s) { return bar_base + 8u * s; };
+    auto empty_bar = [&](int s) { return bar_base + 8u * (kStages + s); };
+    auto tfull_bar = [&](int b) { return bar_base + 8u * (2 * kStages + b); };
+    auto tempty_bar = [&](int b) { return bar_base + 8u * (2 * kStages + kAccBufs + b); };
+    const uint32_t tmem_slot = bar_base + 8u * (2 * kStages + 2 * kAccBufs);
+    uint32_t* tmem_slot_ptr = reinterpret_cast<uint32_t*>(smem_raw + (tmem_slot - ptx::smem_u32(smem_raw)));
+
+    const int warp = threadIdx.x >> 5;
+    const int lane = threadIdx.x & 31;
+    const int ntiles = op.nrb * op.ncb;
+    const int nterms = num_terms(op);
+    const bool has_acc = (op.mode != MODE_UPDATE) ? (op.mode == MODE_P3 || op.c > 0) : (op.k > 0);
+
+    if (warp == 0 && lane == 0) {
+        ptx::prefetch_tmap(&tmA_hi);
+        ptx::prefetch_tmap(&tmA_lo);
+        ptx::prefetch_tmap(&tmB_hi);
+        ptx::prefetch_tmap(&tmB_lo);
+        for (int s = 0; s < kStages; ++s) {
+            ptx::mbar_init(full_bar(s), 1);
+            ptx::mbar_init(empty_bar(s), 1);
+        }
+        for (int b = 0; b < kAccBufs; ++b) {
+            ptx::mbar_init(tfull_bar(b), 1);
+            ptx::mbar_init(tempty_bar(b), 4);
+        }
+        ptx::fence_mbar_init();
+    }
+    if (warp == 1) {
+        ptx::tmem_alloc<kTmemCols>(tmem_slot);
+        ptx::tmem_relinquish();
+    }
+    ptx::tc_fence_before();
+    __syncthreads();
+    ptx::tc_fence_after();
+    const uint32_t tmem_base = *tmem_slot_ptr;
+
+    if (warp == 0) {
+        // ===================== TMA producer =====================
+        if (lane == 0 && has_acc) {
+            int stage = 0;
+            uint32_t phase = 0;
+            for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
+                const int rb = op.rb0 + t / op.ncb, cb = op.cb0 + t % op.ncb;
+                if (tile_is_skipped(op, rb, cb)) continue;
+                for (int s = nterms - 1; s >= 0; --s) {      // descending K: see note on accumulation order
+                    const TermInfo ti = get_term(op, s, rb, cb);
+                    const uint32_t bytes = static_cast<uint32_t>(ti.nA + ti.nB) * kPlaneBytes;
+                    for (int ch = ti.nchunks - 1; ch >= 0; --ch) {
+                        ptx::mbar_wait(empty_bar(stage), phase ^ 1u);
+                        const uint32_t sa = smem_base + stage * kStageBytes;
+                        ptx::mbar_arrive_expect_tx(full_bar(stage), bytes);
+                        const int ak = ti.a_k0 + ch * kBlockK, bk = ti.b_k0 + ch * kBlockK;
+                        ptx::tma_load_2d(sa, &tmA_hi, full_bar(stage), ak, static_cast<int>(ti.a_row));
+                        if (ti.nA == 2)
+                            ptx::tma_load_2d(sa + kPlaneBytes, &tmA_lo, full_bar(stage), ak,
+                                             static_cast<int>(ti.a_row));
+                        ptx::tma_load_2d(sa + 2 * kPlaneBytes, &tmB_hi, full_bar(stage), bk,
+                                         static_cast<int>(ti.b_row));
+                        if (ti.nB == 2)
+                            ptx::tma_load_2d(sa + 3 * kPlaneBytes, &tmB_lo, full_bar(stage), bk,
+                                             static_cast<int>(ti.b_row));
+                        if (++stage == kStages) { stage = 0; phase ^= 1u; }
+                    }
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ===================== MMA issuer (one thread) =====================
+        if (lane == 0 && has_acc) {
+            constexpr uint32_t idesc = ptx::make_idesc(kBlk, kBlk, /*F16*/ 0, /*F16*/ 0);
+            int stage = 0;
+            uint32_t phase = 0;
+            int buf = 0;
+            uint32_t acc_phase = 0;
+            for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
+                const int rb = op.rb0 + t / op.ncb, cb = op.cb0 + t % op.ncb;
+                if (tile_is_skipped(op, rb, cb)) continue;
+                ptx::mbar_wait(tempty_bar(buf), acc_phase ^ 1u);     // epilogue drained this buffer
+                ptx::tc_fence_after();
+                const uint32_t d_tmem = tmem_base + buf * kAccCols;
+                uint32_t accumulate = 0;
+                for (int s = nterms - 1; s >= 0; --s) {      // descending K: see note on accumulation order
+                    const TermInfo ti = get_term(op, s, rb, cb);
+                    for (int ch = ti.nchunks - 1; ch >= 0; --ch) {
+                        ptx::mbar_wait(full_bar(stage), phase);
+                        ptx::tc_fence_after();
+                        const uint32_t sa = smem_base + stage * kStageBytes;
+                        const uint64_t a_hi = ptx::smem_desc_sw128(sa);
+                        const uint64_t a_lo = ptx::smem_desc_sw128(sa + kPlaneBytes);
+                        const uint64_t b_hi = ptx::smem_desc_sw128(sa + 2 * kPlaneBytes);
+                        const uint64_t b_lo = ptx::smem_desc_sw128(sa + 3 * kPlaneBytes);
+#pragma unroll
+                        for (int kk = kBlockK / 16 - 1; kk >= 0; --kk) {
+                            const uint64_t adv = static_cast<uint64_t>((kk * 32) >> 4);   // +32 B per K=16
+                            // small cross terms first, the dominant hi*hi product last
+                            if (ti.nA == 2) { ptx::mma_f16_ss(d_tmem, a_lo + adv, b_hi + adv, idesc, accumulate); accumulate = 1; }
+                            if (ti.nB == 2) { ptx::mma_f16_ss(d_tmem, a_hi + adv, b_lo + adv, idesc, accumulate); accumulate = 1; }
+                            ptx::mma_f16_ss(d_tmem, a_hi + adv, b_hi + adv, idesc, accumulate);
+                            accumulate = 1;
+                        }
+                        ptx::tc_commit(empty_bar(stage));            // smem slot free when MMAs retire
+                        if (++stage == kStages) { stage = 0; phase ^= 1u; }
+                    }
+                }
+                ptx::tc_commit(tfull_bar(buf));                      // accumulator complete
+                if (++buf == kAccBufs) { buf = 0; acc_phase ^= 1u; }
+            }
+        }
+    } else {
+        // ===================== epilogue warps (TMEM -> registers -> global) =====================
+        const int q = warp & 3;                    // TMEM lane quadrant this warp may access
+        int buf = 0;
+        uint32_t acc_phase = 0;
+        for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
+            const int rb = op.rb0 + t / op.ncb, cb = op.cb0 + t % op.ncb;
+            if (tile_is_skipped(op, rb, cb)) continue;
+            const int row_in_blk = q * 32 + lane;
+            const int64_t r = static_cast<int64_t>(rb) * kBlk + row_in_blk;    // panel-local row
+            const int col0 = cb * kBlk;
+            // base pointer and pre-rounding of A
+            const float* base = nullptr;
+            int p = KRR_FP32;
+            float sc = 1.0f;
+            if (op.mode == MODE_UPDATE) {
+                const int i = op.k + (rb * kBlk) / op.nb;
+                const int subrow = (rb * kBlk) % op.nb;
+                base = op.A.tile_ptr(i, op.k, subrow + row_in_blk, col0);
+                if ((op.flags & KRR_FLAG_PREROUND_A) && i != op.k) {
+                    p = op.map[i * op.NT + op.k];
+                    if (p == KRR_FP8_E4M3) sc = fp8_scale_from_amax(op.a_amax[i * op.NT + op.k]);
+                }
+            } else if (op.mode == MODE_P1) {
+                base = op.W + r * op.nb + col0;
+            }
+            // exact power-of-two rescaling: accumulator -> value domain, value -> plane domain
+            const float acc_mul = (op.mode == MODE_P3) ? op.scl[3] / op.linv_scale[op.c] : op.scl[2];
+            const float plane_mul = (op.mode == MODE_P3) ? op.scl[0] : op.scl[1];
+            float* wout = op.W + r * op.nb + col0;
+            __half* hout = op.Hp + (op.prow0 + r) * op.nb + col0;
+            __half* lout = op.Lp + (op.prow0 + r) * op.nb + col0;
+            if (has_acc) {
+                ptx::mbar_wait(tfull_bar(buf), acc_phase);
+                ptx::tc_fence_after();
+            }
+            float amax = 0.0f;
+#pragma unroll 1
+            for (int j = 0; j < kBlk / 32; ++j) {
+                uint32_t acc[32];
+                if (has_acc) {
+                    ptx::tmem_ld_32x32(tmem_base + buf * kAccCols + (static_cast<uint32_t>(q * 32) << 16) + j * 32, acc);
+                    ptx::tmem_ld_wait();
+                } else {
+#pragma unroll
+                    for (int e = 0; e < 32; ++e) acc[e] = 0u;
+                }
+                float out[32];
+                if (base != nullptr) {
+#pragma unroll
+                    for (int e = 0; e < 32; e += 4) {
+                        const float4 b = *reinterpret_cast<const float4*>(base + j * 32 + e);
+                        out[e + 0] = round_to_prec(b.x, p, sc) - __uint_as_float(acc[e + 0]) * acc_mul;
+                        out[e + 1] = round_to_prec(b.y, p, sc) - __uint_as_float(acc[e + 1]) * acc_mul;
+                        out[e + 2] = round_to_prec(b.z, p, sc) - __uint_as_float(acc[e + 2]) * acc_mul;
+                        out[e + 3] = round_to_prec(b.w, p, sc) - __uint_as_float(acc[e + 3]) * acc_mul;
+                    }
+                } else {
+#pragma unroll
+                    for (int e = 0; e < 32; ++e) out[e] = __uint_as_float(acc[e]) * acc_mul;
+                }
+#pragma unroll
+                for (int e = 0; e < 32; e += 4)
+                    *reinterpret_cast<float4*>(wout + j * 32 + e) = make_float4(out[e], out[e + 1], out[e + 2], out[e + 3]);
+#pragma unroll
+                for (int e = 0; e < 32; e += 8) {
+                    __align__(16) __half hi[8];
+                    __align__(16) __half lo[8];
+#pragma unroll
+                    for (int u = 0; u < 8; ++u) {
+                        const float x = out[e + u] * plane_mul;
+                        hi[u] = __float2half_rn(x);
+                        lo[u] = __float2half_rn(x - __half2float(hi[u]));
+                        amax = fmaxf(amax, fabsf(out[e + u]));
+                    }
+                    *reinterpret_cast<uint4*>(hout + j * 32 + e) = *reinterpret_cast<const uint4*>(hi);
+                    *reinterpret_cast<uint4*>(lout + j * 32 + e) = *reinterpret_cast<const uint4*>(lo);
+                }
+            }
+            if (has_acc) {
+                ptx::tc_fence_before();
+                __syncwarp();
+                if (lane == 0) ptx::mbar_arrive(tempty_bar(buf));
+                if (++buf == kAccBufs) { buf = 0; acc_phase ^= 1u; }
+            }
+            if (op.mode == MODE_P3 && op.tile_amax != nullptr) {
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, o));
+                if (lane == 0) {
+                    const int64_t slot = op.prow0 / op.nb + (static_cast<int64_t>(rb) * kBlk) / op.nb;
+                    atomicMax(reinterpret_cast<int*>(op.tile_amax + slot), __float_as_int(amax));
+                }
+            }
+        }
+    }
+
+    // teardown
+    ptx::tc_fence_before();
+    __syncthreads();
+    if (warp == 1) ptx::tmem_dealloc<kTmemCols>(tmem_base);
+}
+
+}  // namespace krr

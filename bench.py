@@ -1,0 +1,365 @@
+#!/usr/bin/env python
+"""bench.py -- mixed-precision Cholesky TOp/s (n^3/3 / device time) on seeded synthetic KRR matrices.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config C3]
+
+A step is one pass of the whole hot path: krr_precision_map -> (map to the host, the
+launch sequence is built there) -> krr_potrf_mp -> krr_potrs, on A = K + lambda*I already resident in
+HBM.  Default workload: BASELINE.json configs[2] (n=65536, p=50000, nb=1024, eps=1e-4, FP32/FP16/FP8
+allowed) -- the configuration north_star quotes the target on.  Multi-GPU: the factorisation does not
+shard into independent units ("replicas only"): N ranks run N independent replicas.
+
+`--impl reference` times the CPU oracle (oracle/, FP64 tile Cholesky) as it stands on the host cores
+on a bounded sample of the same workload (leading principal submatrix, same nb).
+"""
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import torch  # noqa: E402
+
+from krr_inputs import CONFIGS, make_problem  # noqa: E402
+
+METRIC = "mixed-precision Cholesky TOp/s (n^3/3 / device time)"
+UNIT = "TOp/s"
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            p = json.load(f)
+        return {"bf16_burst": p["bf16_tflops"], "bf16_sustained": p.get("bf16_tflops_sustained", p["bf16_tflops"]),
+                "hbm_gbs": p["hbm_gbs"], "source": "measured (MEASURED_PEAKS.json)"}
+    return {"bf16_burst": 1590.0, "bf16_sustained": 1400.0, "hbm_gbs": 6650.0,
+            "source": "fallback (B200_PROFILING.md)"}
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index = index
+        self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100",
+                 "-i", str(self.index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            out, _ = self.proc.communicate(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+            out, _ = self.proc.communicate()
+        sm, mx, reasons, pw = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in out.strip().splitlines():
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(mx), "power_w_max": max(pw),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def update_flops_by_class(h_map, nb):
+    """Algorithmic flops of the trailing SYRK/GEMM updates per MMA class.
+    GEMM tile-term 2 nb^3, SYRK tile-term nb^3; class of a term = the higher of the
+    two operand precisions (FP32-class: 3 kind::f16 MMAs, FP16-class: 1, FP8 x FP8: 1 kind::f8f6f4)."""
+    NT = h_map.shape[0]
+    m = h_map.tolist()
+    fl = {0: 0.0, 1: 0.0, 2: 0.0}
+    nb3 = float(nb) ** 3
+    for k in range(1, NT):
+        for s in range(k):
+            pk = m[k][s]
+            fl[pk] += nb3                        # SYRK term on the diagonal tile
+            for i in range(k + 1, NT):
+                fl[min(m[i][s], pk)] += 2.0 * nb3
+    return fl
+
+
+def run_ours(args, rank, world, local_rank):
+    import paper_2409_01712_b200 as krr
+    from paper_2409_01712_b200 import build
+    build.build()
+    krr.lib()                                    # fail loudly if the CUDA library is missing
+    cfg = CONFIGS[args.config]
+    dev = torch.device("cuda", local_rank)
+    torch.cuda.set_device(dev)
+    peaks = load_peaks()
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+    # ---- synthetic inputs, resident in HBM before the timed region -------------------------------
+    from dataclasses import replace
+    cfg_r = replace(cfg, seed=cfg.seed + 1000 * rank)           # independent replica per rank
+    A, Y = make_problem(cfg_r, device=dev)
+    n, nb, NT = cfg.n, cfg.nb, cfg.NT
+    flags = krr.FLAG_PREROUND_A
+    force = {"fp32": krr.FP32, "force_fp16": krr.FP16, "force_fp8": krr.FP8}.get(cfg.map_request)
+
+    launches = [0]
+
+    def step(collect=None):
+        if force is None:
+            d_map, norms, amax, fro = krr.precision_map(A, nb, cfg.eps_target, cfg.allowed)
+            launches[0] += krr.last_launch_count()
+            h_map = d_map.cpu()                  # launch sequence is built on the host from the map
+        else:
+            h_map = krr.uniform_map(NT, force)
+            d_map = h_map.to(dev)
+        F = krr.potrf_mp(A, nb, d_map, h_map, flags=flags)
+        launches[0] += krr.last_launch_count()
+        B = Y.clone()
+        krr.potrs(F, B)
+        launches[0] += krr.last_launch_count()
+        if collect is not None:
+            collect["F"], collect["alpha"], collect["h_map"] = F, B, h_map
+        return h_map
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            torch.distributed.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    launches[0] = 0
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    krr.profile_enable(1)                        # time the dominant kernel (trailing update) live
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record()
+    barrier()
+    clocks = sampler.stop()
+    total_ms = e0.elapsed_time(e1)
+    prof = krr.profile_read()
+    upd_ms, upd_launches = prof["update_gemm"]
+    krr.profile_enable(0)
+    if world > 1:
+        t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+        torch.distributed.all_reduce(t, op=torch.distributed.ReduceOp.MAX)
+        total_ms = float(t.item())
+    ms_per_step = total_ms / args.steps
+    ops = n ** 3 / 3.0
+    value = world * ops / (ms_per_step * 1e-3) / 1e12
+
+    # ---- one extra profiled step: per-kernel breakdown + correctness numbers (not timed) ----------
+    keep = {}
+    krr.profile_enable(0xFF)
+    h_map = step(keep)
+    torch.cuda.synchronize()
+    breakdown = {k: {"ms": round(v[0], 3), "launches": v[1]} for k, v in krr.profile_read().items() if v[1]}
+    krr.profile_enable(0)
+    info = int(keep["F"].info.item())
+    hist = torch.bincount(h_map[torch.tril(torch.ones(NT, NT, dtype=torch.bool), -1)].long(), minlength=3).tolist()
+    sys.path.insert(0, os.path.join(ROOT, "tests"))
+    checks = {}
+    try:
+        from helpers import probe_backward_error, solve_residual
+        checks["backward_error_probe"] = probe_backward_error(A, keep["F"], 8)
+        checks["solve_residual"] = solve_residual(A, keep["alpha"], Y)
+    except Exception as ex:                      # checking only; never masks the measurement
+        checks["error"] = repr(ex)
+
+    # ---- roofline of the dominant kernel (tcgen05 trailing update) --------------------------------
+    fl = update_flops_by_class(h_map, nb)
+    p16 = peaks["bf16_sustained"]
+    class_peak = {0: p16 / 3.0, 1: p16, 2: 2.0 * p16}
+    upd_flops = sum(fl.values())
+    t_bound_upd = sum(fl[c] / (class_peak[c] * 1e12) for c in fl)
+    pw_peak = upd_flops / t_bound_upd / 1e12 if t_bound_upd > 0 else class_peak[0]
+    achieved = upd_flops * args.steps / (upd_ms * 1e-3) / 1e12 if upd_ms > 0 else 0.0
+    roofline = {"bound": "tensor", "kernel": "gemm_tc_kernel (MODE_UPDATE: trailing SYRK/GEMM)",
+                "achieved": round(achieved, 2), "peak": round(pw_peak, 2), "unit": "TFLOP/s",
+                "frac": round(achieved / pw_peak, 4), "traffic": None,
+                "peak_source": f"{peaks['source']}: bf16 sustained {p16} TF/s; FP32-class = /3 (three kind::f16 "
+                               "MMAs per product), FP8 = x2 (nominal ratio)",
+                "flops_per_step_by_class": {"fp32x3": fl[0], "fp16": fl[1], "fp8": fl[2]},
+                "kernel_ms_per_step": round(upd_ms / args.steps, 3), "launches_per_step": upd_launches // args.steps}
+    # whole factorisation against the precision-weighted tensor roofline (all n^3/3 credited to the
+    # class peaks; panel TRSM runs on the tensor cores in FP32-class)
+    potrf_ms = sum(v["ms"] for k, v in breakdown.items() if k not in ("precision_map", "potrs"))
+    pw_frac_potrf = (ops / (pw_peak * 1e12)) / (potrf_ms * 1e-3) if potrf_ms > 0 else None
+
+    out = {"metric": METRIC, "value": round(value, 3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+           "warmup": args.warmup, "ms_per_step": round(ms_per_step, 3), "higher_is_better": True,
+           "scaling": "weak", "vs_baseline": None, "dtype": "f32 (3x f16 tcgen05 split, FP32 accumulate)"
+           if hist[1] == 0 and hist[2] == 0 else "mixed f32/f16/f8 tiles, FP32 accumulate",
+           "data": "synthetic", "impl": "ours",
+           "config": {"workload": f"{cfg.name}: n={n}, p={cfg.p}, nb={nb}, gamma=1/p, lambda={cfg.lam}, "
+                                  f"map={cfg.map_request} eps={cfg.eps_target}, nrhs={cfg.nrhs}",
+                      "map_histogram_offdiag": {"fp32": hist[0], "fp16": hist[1], "fp8": hist[2]},
+                      "l2_policy": "inputs (A: %.1f GB) larger than L2, no flush" % (A.numel() * 4 / 1e9),
+                      "parallelism": "replicas only" if world > 1 else "single GPU"},
+           "clocks": clocks, "gpu_launches": launches[0], "roofline": roofline,
+           "potrf_frac_of_precision_weighted_tensor_peak": round(pw_frac_potrf, 4) if pw_frac_potrf else None,
+           "breakdown_ms_one_step": breakdown, "info": info, "checks": checks}
+    return out, (A, Y, krr, cfg, dev)
+
+
+def run_e2e(ctx, steps):
+    """Same metric through the C ABI with HOST buffers (krr_associate_host): H2D of A and Y and D2H
+    of alpha / map / info inside the timed region."""
+    A, Y, krr, cfg, dev = ctx
+    n, nb = cfg.n, cfg.nb
+    hA = torch.empty((n, n), dtype=torch.float32, pin_memory=True)
+    hA.copy_(A)
+    hY = Y.cpu().pin_memory()
+    del A
+    torch.cuda.empty_cache()
+    force = {"fp32": krr.FP32, "force_fp16": krr.FP16, "force_fp8": krr.FP8}.get(cfg.map_request, -1)
+    arena = None
+    times = []
+    for it in range(steps + 1):                  # first call is the warm-up
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        alpha, h_map, info, arena = krr.associate_host(hA, nb, hY, cfg.eps_target, cfg.allowed, force,
+                                                       krr.FLAG_PREROUND_A, arena, dev)
+        e1.record()
+        torch.cuda.synchronize()
+        if it > 0:
+            times.append(e0.elapsed_time(e1))
+    ms = sum(times) / len(times)
+    NT = n // nb
+    return {"value": round(n ** 3 / 3.0 / (ms * 1e-3) / 1e12, 3), "unit": UNIT, "ms_per_step": round(ms, 3),
+            "h2d_bytes_per_step": n * n * 4 + n * cfg.nrhs * 4,
+            "d2h_bytes_per_step": n * cfg.nrhs * 4 + NT * NT + 4, "steps": len(times),
+            "api": "krr_associate_host (pinned host A, Y -> alpha)"}
+
+
+def oracle_sample(cfg, device, sample_tiles):
+    """Leading principal submatrix of the workload (same generator, nb), on the host."""
+    from dataclasses import replace
+    ns = min(cfg.n, sample_tiles * cfg.nb)
+    sub = replace(cfg, n=ns)                     # first ns patients, all p SNPs: same K entries
+    A, Y = make_problem(sub, device=device)
+    return A.cpu().numpy(), ns
+
+
+def time_oracle(A, nb):
+    from oracle.cholesky import tile_cholesky_fp64
+    t0 = time.perf_counter()
+    L, info = tile_cholesky_fp64(A, nb)
+    dt = time.perf_counter() - t0
+    return dt, info
+
+
+def host_threads():
+    try:
+        from threadpoolctl import threadpool_info
+        n = max((p.get("num_threads", 1) for p in threadpool_info()), default=1)
+        return int(n)
+    except Exception:
+        return os.cpu_count() or 1
+
+
+def run_reference(args, rank):
+    if rank != 0:
+        return None
+    cfg = CONFIGS[args.config]
+    dev = "cuda" if torch.cuda.is_available() else "cpu"
+    A, ns = oracle_sample(cfg, dev, args.sample_tiles)
+    for _ in range(min(args.warmup, 1)):
+        time_oracle(A, cfg.nb)
+    times = []
+    for _ in range(args.steps):
+        dt, info = time_oracle(A, cfg.nb)
+        times.append(dt)
+    dt = sum(times) / len(times)
+    val = ns ** 3 / 3.0 / dt / 1e12
+    cores = host_threads()
+    sample = f"leading {ns}x{ns} principal submatrix of {cfg.name} (nb={cfg.nb}), oracle FP64 tile Cholesky"
+    return {"metric": METRIC, "value": round(val, 6), "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": min(args.warmup, 1), "ms_per_step": round(dt * 1e3, 3), "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic", "impl": "reference",
+            "config": {"workload": f"{cfg.name}: n={cfg.n}, p={cfg.p}, nb={cfg.nb} (bounded sample n_s={ns})"},
+            "cpu_baseline": {"value": round(val, 6), "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": round(val, 6), "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="C3", choices=sorted(CONFIGS))
+    ap.add_argument("--sample-tiles", type=int, default=8, help="tiles per dimension of the CPU-oracle sample")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+
+    if args.impl == "reference":
+        out = run_reference(args, rank)
+        if out is not None:
+            print(json.dumps(out), flush=True)
+        return 0
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    args.warmup = max(args.warmup, 3)
+    out, ctx = run_ours(args, rank, world, local_rank)
+    cfg = ctx[3]
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        A_s, ns = oracle_sample(cfg, ctx[4], args.sample_tiles)
+        dt, _ = time_oracle(A_s, cfg.nb)
+        out["cpu_baseline"] = {"value": round(ns ** 3 / 3.0 / dt / 1e12, 6), "unit": UNIT, "cores": host_threads(),
+                               "kind": "oracle", "seconds": round(dt, 2),
+                               "sample": f"leading {ns}x{ns} principal submatrix of {cfg.name} (nb={cfg.nb}), "
+                                         "FP64 tile Cholesky of oracle/cholesky.py as it stands"}
+        del A_s
+    if not args.no_e2e:
+        e2e = run_e2e(ctx, max(1, min(args.steps, 2)))
+        if world > 1:
+            t = torch.tensor([e2e["ms_per_step"]], dtype=torch.float64, device=ctx[4])
+            torch.distributed.all_reduce(t, op=torch.distributed.ReduceOp.MAX)
+            e2e["ms_per_step"] = float(t.item())
+            e2e["value"] = round(world * cfg.n ** 3 / 3.0 / (e2e["ms_per_step"] * 1e-3) / 1e12, 3)
+        out["e2e"] = e2e
+    if rank == 0:
+        print(json.dumps(out), flush=True)
+    if world > 1:
+        torch.distributed.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

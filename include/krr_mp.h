@@ -158,6 +158,16 @@ int krr_associate_host(const float* h_A, int64_t n, int64_t lda, int nb,
 /* Number of kernels the last krr_* call on this thread enqueued (for bench.py's gpu_launches). */
 int64_t krr_last_launch_count(void);
 
+/* Optional per-kernel timing for measurement (bench.py's roofline object): while a category's bit
+ * is set in category_mask, every launch of that category made by this host thread is bracketed by
+ * CUDA events on the launching stream.  Categories: 0 trailing SYRK/GEMM update (tcgen05),
+ * 1 in-panel update, 2 panel TRSM product, 3 FP32 POTRF of a 128 block, 4 quantising store,
+ * 5 precision map, 6 POTRS, 7 misc.  krr_profile_enable(mask) also clears the records (0 = off).
+ * krr_profile_read synchronises on the recorded events and returns the summed device time and the
+ * number of launches of one category.  This is the only place the library creates CUDA events. */
+int krr_profile_enable(unsigned category_mask);
+int krr_profile_read(int category, double* total_ms, int64_t* launches);
+
 #ifdef __cplusplus
 }
 #endif

@@ -79,6 +79,19 @@ def genotypes(seed, n, p, kind="maf", device="cpu", row0=0, rows=None, dtype=tor
     elif kind == "uniform":
         h = _lsr(mix64(mix64(ctr + _stream(seed, 2))), 40)       # 24 bits
         g = ((h * 3) >> 24).to(dtype)
+    elif kind.startswith("families"):
+        # S1: contiguous families of `fam_rows` patients; a member copies its family
+        # founder's SNP with probability 0.97 / 0.75 / 0.60 (families 0 / 1 / 2), 0 (the rest) -- related
+        # individuals give the higher-precision tiles of PAPER.md:229.
+        fam_rows = int(kind.split(":")[1])
+        m = maf(seed, p, device)[None, :]
+        own = (uniform24(seed, 2, ctr) < m).to(dtype) + (uniform24(seed, 3, ctr) < m).to(dtype)
+        fam = i // fam_rows
+        fctr = (fam * fam_rows) * p + k
+        founder = (uniform24(seed, 2, fctr) < m).to(dtype) + (uniform24(seed, 3, fctr) < m).to(dtype)
+        q = torch.where(fam == 0, 0.97, torch.where(fam == 1, 0.75, torch.where(fam == 2, 0.60, 0.0))).to(torch.float64)
+        copy = uniform24(seed, 6, ctr) < q
+        g = torch.where(copy, founder, own)
     else:
         raise ValueError(kind)
     return g
@@ -142,10 +155,11 @@ class Config:
     eps_target: float = 0.0
     allowed: tuple = (0,)            # precision codes the rule may use
     lower_tiles_only: bool = False
+    gamma_scale: float = 1.0         # gamma = gamma_scale / p
 
     @property
     def gamma(self):
-        return 1.0 / self.p
+        return self.gamma_scale / self.p
 
     @property
     def NT(self):
@@ -162,6 +176,10 @@ CONFIGS = {
                  eps_target=1e-3, allowed=(0, 1, 2), lower_tiles_only=True),
     "C5": Config("C5", 98304, 20000, 1024, 1e-1, 4, seed=5, genotype="uniform",
                  map_request="force_fp8", allowed=(0, 2)),
+    # supplementary: the paper's regime K ~ I (gamma = 12/p) with two families of
+    # relatives -- the only input on which the rule yields a genuine FP32/FP16/FP8 mosaic
+    "S1": Config("S1", 32768, 24576, 1024, 1e-2, 8, seed=6, genotype="families:4096",
+                 map_request="rule", eps_target=1e-4, allowed=(0, 1, 2), gamma_scale=12.0),
 }
 
 
@@ -169,7 +187,10 @@ def scaled_config(cfg, nb, n=None, p=None):
     """Reduced-size twin: same NT (unless n given), generator, gamma = 1/p, lambda, map request."""
     n = cfg.NT * nb if n is None else n
     p = max(64, (cfg.p * n) // cfg.n) if p is None else p
-    return replace(cfg, name=f"{cfg.name}@n{n}", n=n, p=p, nb=nb)
+    geno = cfg.genotype
+    if geno.startswith("families"):
+        geno = f"families:{4 * nb}"
+    return replace(cfg, name=f"{cfg.name}@n{n}", n=n, p=p, nb=nb, genotype=geno)
 
 
 def make_problem(cfg, device="cpu", row_block=4096):

@@ -6,8 +6,10 @@ There is no CPU fallback: importing works anywhere, calling needs the built libr
 """
 from .binding import (FP32, FP16, FP8, FLAG_PREROUND_A, FLAG_A_TILED_LOWER, KrrError, Factor,
                       lib, library_path, precision_map, potrf_mp, potrs, associate_host,
-                      factor_bytes, factor_tile_offset, tile_slot, uniform_map, last_launch_count)
+                      factor_bytes, factor_tile_offset, tile_slot, uniform_map, last_launch_count,
+                      profile_enable, profile_read, PROFILE_CATEGORIES)
 
 __all__ = ["FP32", "FP16", "FP8", "FLAG_PREROUND_A", "FLAG_A_TILED_LOWER", "KrrError", "Factor",
            "lib", "library_path", "precision_map", "potrf_mp", "potrs", "associate_host",
-           "factor_bytes", "factor_tile_offset", "tile_slot", "uniform_map", "last_launch_count"]
+           "factor_bytes", "factor_tile_offset", "tile_slot", "uniform_map", "last_launch_count",
+           "profile_enable", "profile_read", "PROFILE_CATEGORIES"]

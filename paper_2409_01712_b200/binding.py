@@ -18,7 +18,8 @@ ERRORS = {-1: "KRR_ERR_ARG", -2: "KRR_ERR_SHAPE", -3: "KRR_ERR_WORKSPACE", -4: "
 EXPORTS = ["krr_version", "krr_built_for_sm", "krr_tile_slot", "krr_precision_map_workspace",
            "krr_precision_map", "krr_factor_bytes", "krr_factor_tile_offset",
            "krr_potrf_mp_workspace", "krr_potrf_mp", "krr_potrs_workspace", "krr_potrs",
-           "krr_associate_host_arena", "krr_associate_host", "krr_last_launch_count"]
+           "krr_associate_host_arena", "krr_associate_host", "krr_last_launch_count",
+           "krr_profile_enable", "krr_profile_read"]
 
 
 class KrrError(RuntimeError):
@@ -67,6 +68,10 @@ def lib():
     L.krr_associate_host.argtypes = [vp, i64, i64, c.c_int, c.c_float, u32, c.c_int, u32, vp, c.c_int, vp,
                                      vp, vp, vp, sz, vp]
     L.krr_last_launch_count.restype = i64
+    L.krr_profile_enable.restype = c.c_int
+    L.krr_profile_enable.argtypes = [u32]
+    L.krr_profile_read.restype = c.c_int
+    L.krr_profile_read.argtypes = [c.c_int, c.POINTER(c.c_double), c.POINTER(i64)]
     _LIB = L
     return L
 
@@ -93,6 +98,24 @@ def _ws(nbytes, device):
 
 def last_launch_count():
     return int(lib().krr_last_launch_count())
+
+
+PROFILE_CATEGORIES = ["update_gemm", "panel_update", "panel_trsm", "potrf128", "finalize", "precision_map",
+                      "potrs", "misc"]
+
+
+def profile_enable(mask):
+    _check(lib().krr_profile_enable(mask), "krr_profile_enable")
+
+
+def profile_read():
+    """{category: (total device ms, launches)} for the records since the last profile_enable."""
+    out = {}
+    for cat, name in enumerate(PROFILE_CATEGORIES):
+        ms, cnt = ctypes.c_double(0.0), ctypes.c_int64(0)
+        _check(lib().krr_profile_read(cat, ctypes.byref(ms), ctypes.byref(cnt)), "krr_profile_read")
+        out[name] = (ms.value, cnt.value)
+    return out
 
 
 def tile_slot(NT, i, j):

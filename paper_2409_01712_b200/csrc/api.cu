@@ -119,8 +119,31 @@ static PotrfWs potrf_ws_layout(int64_t n, int nb, bool any_fp8) {
     return w;
 }
 
+// ---- optional per-category kernel timing (krr_profile_*): CUDA events on the launching stream ----
+enum { CAT_UPDATE = 0, CAT_P1 = 1, CAT_P3 = 2, CAT_POTRF = 3, CAT_FINALIZE = 4, CAT_MAP = 5, CAT_POTRS = 6,
+       CAT_MISC = 7, CAT_COUNT = 8 };
+struct TimedLaunch { int cat; cudaEvent_t e0, e1; };
+static thread_local unsigned g_prof_mask = 0;
+static thread_local std::vector<TimedLaunch> g_prof;
+static thread_local std::vector<cudaEvent_t> g_event_pool;
+
+static cudaEvent_t pool_event() {
+    if (!g_event_pool.empty()) { cudaEvent_t e = g_event_pool.back(); g_event_pool.pop_back(); return e; }
+    cudaEvent_t e = nullptr;
+    cudaEventCreate(&e);
+    return e;
+}
+struct ProfScope {
+    bool on; TimedLaunch t; cudaStream_t st;
+    ProfScope(int cat, cudaStream_t s) : on((g_prof_mask >> cat) & 1u), st(s) {
+        if (on) { t.cat = cat; t.e0 = pool_event(); t.e1 = pool_event(); cudaEventRecord(t.e0, st); }
+    }
+    ~ProfScope() { if (on) { cudaEventRecord(t.e1, st); g_prof.push_back(t); } }
+};
+
 template <typename K, typename... Args>
-static int launch(K kernel, dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args... args) {
+static int launch(int cat, K kernel, dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args... args) {
+    ProfScope ps(cat, st);
     kernel<<<grid, block, smem, st>>>(args...);
     ++g_launches;
     return cudaGetLastError() == cudaSuccess ? KRR_OK : KRR_ERR_CUDA;
@@ -131,6 +154,7 @@ static int launch_gemm(const CUtensorMap& a_hi, const CUtensorMap& a_lo, const C
     const int ntiles = op.nrb * op.ncb;
     if (ntiles <= 0) return KRR_OK;
     const int grid = ntiles < num_sms ? ntiles : num_sms;
+    ProfScope ps(op.mode == MODE_UPDATE ? CAT_UPDATE : (op.mode == MODE_P1 ? CAT_P1 : CAT_P3), st);
     gemm_tc_kernel<<<grid, kGemmThreads, kGemmSmem, st>>>(a_hi, a_lo, b_hi, b_lo, op);
     ++g_launches;
     return cudaGetLastError() == cudaSuccess ? KRR_OK : KRR_ERR_CUDA;
@@ -168,6 +192,30 @@ int krr_version(void) { return 100; }
 int krr_built_for_sm(void) { return 100; }
 int64_t krr_last_launch_count(void) { return g_launches; }
 
+int krr_profile_enable(unsigned category_mask) {
+    for (auto& t : g_prof) { g_event_pool.push_back(t.e0); g_event_pool.push_back(t.e1); }
+    g_prof.clear();
+    g_prof_mask = category_mask;
+    return KRR_OK;
+}
+
+int krr_profile_read(int category, double* total_ms, int64_t* launches) {
+    if (category < 0 || category >= CAT_COUNT || !total_ms || !launches) return KRR_ERR_ARG;
+    double ms = 0.0;
+    int64_t cnt = 0;
+    for (auto& t : g_prof) {
+        if (t.cat != category) continue;
+        if (cudaEventSynchronize(t.e1) != cudaSuccess) return KRR_ERR_CUDA;
+        float f = 0.f;
+        if (cudaEventElapsedTime(&f, t.e0, t.e1) != cudaSuccess) return KRR_ERR_CUDA;
+        ms += f;
+        ++cnt;
+    }
+    *total_ms = ms;
+    *launches = cnt;
+    return KRR_OK;
+}
+
 int64_t krr_tile_slot(int NT, int i, int j) {
     if (NT <= 0 || j < 0 || i < j || i >= NT) return -1;
     return tile_slot(NT, i, j);
@@ -203,10 +251,10 @@ int krr_precision_map(const float* d_A, int64_t n, int64_t lda, int nb, float ep
     float* pamax = reinterpret_cast<float*>(ws + align_up(nslots * chunks * sizeof(double), 1024));
     double* sumsq = reinterpret_cast<double*>(reinterpret_cast<uint8_t*>(pamax) + align_up(nslots * chunks * sizeof(float), 1024));
     AView A{d_A, lda, tiled ? 1 : 0, NT, nb};
-    rc = launch(tile_stats_kernel, dim3(static_cast<unsigned>(chunks), static_cast<unsigned>(nslots)), dim3(kStatThreads), 0, st,
+    rc = launch(CAT_MAP, tile_stats_kernel, dim3(static_cast<unsigned>(chunks), static_cast<unsigned>(nslots)), dim3(kStatThreads), 0, st,
                 A, partial, pamax);
     if (rc) return rc;
-    return launch(map_decide_kernel, dim3(1), dim3(1024), 0, st, NT, static_cast<int>(chunks),
+    return launch(CAT_MAP, map_decide_kernel, dim3(1), dim3(1024), 0, st, NT, static_cast<int>(chunks),
                   static_cast<const double*>(partial), static_cast<const float*>(pamax), eps_target, allowed_mask, d_map,
                   d_tile_norms, d_tile_amax, d_fro, sumsq);
 }
@@ -280,14 +328,14 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
     KRR_CUDA_CHECK(cudaMemsetAsync(d_info, 0, sizeof(int), st));
     KRR_CUDA_CHECK(cudaMemsetAsync(d_scales, 0, static_cast<size_t>(NT) * NT * sizeof(float), st));
     KRR_CUDA_CHECK(cudaMemsetAsync(tile_amax, 0, nslots * sizeof(float), st));
-    rc = launch(offsets_kernel, dim3(1), dim3(32), 0, st, NT, nb, d_map, off);
+    rc = launch(CAT_MISC, offsets_kernel, dim3(1), dim3(32), 0, st, NT, nb, d_map, off);
     if (rc) return rc;
-    rc = launch(plane_scale_kernel, dim3(1), dim3(1024), 0, st, A, n, scl);
+    rc = launch(CAT_MISC, plane_scale_kernel, dim3(1), dim3(1024), 0, st, A, n, scl);
     if (rc) return rc;
     const bool preround = flags & KRR_FLAG_PREROUND_A;
     if (preround && any_fp8) {
         KRR_CUDA_CHECK(cudaMemsetAsync(a_amax, 0, static_cast<size_t>(NT) * NT * sizeof(float), st));
-        rc = launch(tile_amax_kernel, dim3(nb / 32, static_cast<unsigned>(nslots)), dim3(256), 0, st, A, d_map, a_amax);
+        rc = launch(CAT_MISC, tile_amax_kernel, dim3(nb / 32, static_cast<unsigned>(nslots)), dim3(256), 0, st, A, d_map, a_amax);
         if (rc) return rc;
     }
 
@@ -316,7 +364,7 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
                 rc = launch_gemm(tmH, tmL, tmH, tmL, op, num_sms, st);
                 if (rc) return rc;
             }
-            rc = launch(potrf128_kernel, dim3(1), dim3(kPotrfThreads), static_cast<size_t>(kPotrfSmem), st, W, nb,
+            rc = launch(CAT_POTRF, potrf128_kernel, dim3(1), dim3(kPotrfThreads), static_cast<size_t>(kPotrfSmem), st, W, nb,
                         c * kBlk, c * kBlk, linv_hi, linv_lo, linv_scale, d_info,
                         static_cast<int64_t>(k) * nb + static_cast<int64_t>(c) * kBlk + 1);
             if (rc) return rc;
@@ -326,7 +374,7 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
                 if (rc) return rc;
             }
         }
-        rc = launch(finalize_kernel, dim3(nb / 16, NT - k), dim3(256), 0, st, NT, nb, k, static_cast<const float*>(W),
+        rc = launch(CAT_FINALIZE, finalize_kernel, dim3(nb / 16, NT - k), dim3(256), 0, st, NT, nb, k, static_cast<const float*>(W),
                     d_map, static_cast<const int64_t*>(off), static_cast<const float*>(tile_amax),
                     static_cast<uint8_t*>(d_factor), d_scales, Hp, Qp, static_cast<const float*>(scl));
         if (rc) return rc;
@@ -352,10 +400,10 @@ static int potrs_run(const uint8_t* factor, const float* d_scales, const uint8_t
     for (int k = 0; k < NT; ++k) {
         const float* Lkk = reinterpret_cast<const float*>(factor + hoff[static_cast<size_t>(k) * NT + k]);
         float* Bk = B + static_cast<int64_t>(k) * nb * ldb;
-        rc = launch(potrs_diag_kernel<NRHS>, dim3(1), dim3(256), smem_d, st, nb, Lkk, Bk, ldb, nrhs, 0);
+        rc = launch(CAT_POTRS, potrs_diag_kernel<NRHS>, dim3(1), dim3(256), smem_d, st, nb, Lkk, Bk, ldb, nrhs, 0);
         if (rc) return rc;
         if (k + 1 < NT) {
-            rc = launch(potrs_fwd_update_kernel<NRHS>, dim3((NT - k - 1) * (nb / 32)), dim3(256), smem_z, st, NT, nb, k,
+            rc = launch(CAT_POTRS, potrs_fwd_update_kernel<NRHS>, dim3((NT - k - 1) * (nb / 32)), dim3(256), smem_z, st, NT, nb, k,
                         factor, off, d_map, d_scales, B, ldb, nrhs);
             if (rc) return rc;
         }
@@ -363,10 +411,10 @@ static int potrs_run(const uint8_t* factor, const float* d_scales, const uint8_t
     for (int k = NT - 1; k >= 0; --k) {
         const float* Lkk = reinterpret_cast<const float*>(factor + hoff[static_cast<size_t>(k) * NT + k]);
         float* Bk = B + static_cast<int64_t>(k) * nb * ldb;
-        rc = launch(potrs_diag_kernel<NRHS>, dim3(1), dim3(256), smem_d, st, nb, Lkk, Bk, ldb, nrhs, 1);
+        rc = launch(CAT_POTRS, potrs_diag_kernel<NRHS>, dim3(1), dim3(256), smem_d, st, nb, Lkk, Bk, ldb, nrhs, 1);
         if (rc) return rc;
         if (k > 0) {
-            rc = launch(potrs_bwd_update_kernel<NRHS>, dim3(k * (nb / 128)), dim3(128), smem_z, st, NT, nb, k, factor, off,
+            rc = launch(CAT_POTRS, potrs_bwd_update_kernel<NRHS>, dim3(k * (nb / 128)), dim3(128), smem_z, st, NT, nb, k, factor, off,
                         d_map, d_scales, B, ldb, nrhs);
             if (rc) return rc;
         }
@@ -395,7 +443,7 @@ int krr_potrs(const void* d_factor, const float* d_scales, const uint8_t* d_map,
     std::vector<int64_t> hoff;
     host_offsets(NT, nb, h_map, &hoff);
     int64_t* off = static_cast<int64_t*>(d_ws);
-    rc = launch(offsets_kernel, dim3(1), dim3(32), 0, st, NT, nb, d_map, off);
+    rc = launch(CAT_MISC, offsets_kernel, dim3(1), dim3(32), 0, st, NT, nb, d_map, off);
     if (rc) return rc;
     const uint8_t* factor = static_cast<const uint8_t*>(d_factor);
     if (nrhs <= 4) return potrs_run<4>(factor, d_scales, d_map, hoff, off, NT, nb, d_B, ldb, nrhs, st);

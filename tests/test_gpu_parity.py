@@ -1,0 +1,296 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, on the same seeded inputs.
+
+Tolerances (BASELINE.json north_star):
+  * precision map: bit-exact; tile norms / ||A||_F to FP64-summation-order accuracy
+  * all-FP32 maps: ||L_gpu - L_oracle||_F / ||L_oracle||_F <= 1e-4, backward error <= 1e-6,
+    alpha vs the FP64 solve <= 1e-3
+  * FP16 / FP8 / mixed maps: backward error <= 5e-4 and within 2 % of the oracle's; the literal
+    L comparison passes at max(1e-4, 2 x the oracle's own rounding-flip noise floor); the first tile
+    column (no accumulated noise yet) agrees to one storage ulp
+  * exactly-representable constructions: bit for bit under every map
+  * breakdown: same `info` tile column as the oracle
+"""
+from dataclasses import replace
+
+import numpy as np
+import pytest
+import torch
+
+from krr_inputs import CONFIGS, exact_lower_factor, make_problem, scaled_config
+from oracle import rounding as R
+from oracle.cholesky import backward_error, tile_cholesky_emulated
+from oracle.precision_map import precision_map as oracle_map
+from oracle.precision_map import uniform_map as oracle_uniform
+from oracle.solve import potrs_fp64, solve_fp64
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def krr():
+    from paper_2409_01712_b200 import build
+    build.build()
+    import paper_2409_01712_b200 as k
+    k.lib()
+    return k
+
+
+def relF(a, b):
+    return float(np.linalg.norm(a - b) / np.linalg.norm(b))
+
+
+def gpu_factor(krr, A, nb, pmap, preround=True):
+    h = torch.from_numpy(np.ascontiguousarray(pmap))
+    F = krr.potrf_mp(A, nb, h.cuda(), h, flags=krr.FLAG_PREROUND_A if preround else 0)
+    torch.cuda.synchronize()
+    return F
+
+
+# ------------------------------------------------------------------------------ precision map
+@pytest.mark.parametrize("name,nb,n,p,eps", [("C1", 128, 1024, 500, 1e-4), ("C4", 128, 1024, 800, 1e-3),
+                                             ("S1", 128, 2048, 1536, 1e-4), ("C5", 256, 1024, 400, 0.07)])
+def test_precision_map_bit_exact(krr, name, nb, n, p, eps):
+    cfg = scaled_config(CONFIGS[name], nb=nb, n=n, p=p)
+    A, _ = make_problem(cfg, device="cuda")
+    d_map, norms, amax, fro = krr.precision_map(A, nb, eps, (0, 1, 2))
+    torch.cuda.synchronize()
+    pm, t, f = oracle_map(A.cpu().numpy(), nb, eps)
+    assert np.array_equal(d_map.cpu().numpy(), pm)
+    assert abs(float(fro) - f) <= 1e-12 * f
+    assert np.max(np.abs(norms.cpu().numpy().astype(np.float64) - t)) <= 2e-7 * t.max()
+    An = A.cpu().numpy()
+    for (i, j) in [(0, 0), (3, 1), (cfg.NT - 1, 0), (cfg.NT - 1, cfg.NT - 1)]:
+        assert float(amax[i, j]) == np.abs(An[i * nb:(i + 1) * nb, j * nb:(j + 1) * nb]).max()
+    # allowed mask: FP32 only -> all FP32
+    d2, _, _, _ = krr.precision_map(A, nb, eps, (0,))
+    assert int((d2.cpu()[np.tril_indices(cfg.NT)] != 0).sum()) == 0
+
+
+def pack_lower_tiles(A, nb):
+    n = A.shape[0]
+    NT = n // nb
+    tiles = []
+    for j in range(NT):
+        for i in range(j, NT):
+            tiles.append(A[i * nb:(i + 1) * nb, j * nb:(j + 1) * nb].contiguous().reshape(-1))
+    return torch.cat(tiles)
+
+
+def test_tiled_lower_storage_gives_identical_results(krr):
+    cfg = scaled_config(CONFIGS["C4"], nb=128, n=1024, p=800)
+    A, _ = make_problem(cfg, device="cuda")
+    At = pack_lower_tiles(A, cfg.nb)
+    m1, n1, a1, f1 = krr.precision_map(A, cfg.nb, 1e-3)
+    m2, n2, a2, f2 = krr.precision_map(At, cfg.nb, 1e-3, flags=krr.FLAG_A_TILED_LOWER, n=cfg.n)
+    assert torch.equal(m1, m2) and torch.equal(n1, n2) and torch.equal(f1, f2)
+    h = m1.cpu()
+    F1 = krr.potrf_mp(A, cfg.nb, m1, h)
+    F2 = krr.potrf_mp(At, cfg.nb, m1, h, flags=krr.FLAG_PREROUND_A | krr.FLAG_A_TILED_LOWER, n=cfg.n)
+    torch.cuda.synchronize()
+    assert torch.equal(F1.payload, F2.payload) and torch.equal(F1.scales, F2.scales)
+
+
+# ------------------------------------------------------------------------------ FP32 maps
+@pytest.mark.parametrize("name,nb,n,p", [("C1", 256, 2048, 1000),      # config 1 at full size
+                                         ("C2", 128, 1536, 1000),      # NT = 12, ragged vs 148 CTAs
+                                         ("C1", 128, 128, 200),        # NT = 1: POTRF only
+                                         ("C1", 512, 1024, 300)])
+def test_fp32_map_meets_all_three_tolerances(krr, name, nb, n, p):
+    cfg = scaled_config(CONFIGS[name], nb=nb, n=n, p=p)
+    A, Y = make_problem(cfg, device="cuda")
+    pmap = oracle_uniform(cfg.NT, R.FP32)
+    F = gpu_factor(krr, A, nb, pmap)
+    assert int(F.info.item()) == 0
+    An, Yn = A.cpu().numpy(), Y.cpu().numpy()
+    Lo, _, info = tile_cholesky_emulated(An, nb, pmap)
+    assert info == 0
+    Lg = F.dense().cpu().numpy()
+    assert np.array_equal(Lg, np.tril(Lg)) and np.all(np.diag(Lg) > 0)
+    assert relF(Lg, Lo) <= 1e-4
+    assert backward_error(An, Lg) <= 1e-6
+    alpha = krr.potrs(F, Y.clone())
+    torch.cuda.synchronize()
+    a64 = solve_fp64(An, Yn, nb)
+    assert relF(alpha.cpu().numpy().astype(np.float64), a64) <= 1e-3
+    # the solve itself against the oracle's substitution with the SAME factor
+    assert relF(alpha.cpu().numpy().astype(np.float64), potrs_fp64(Lg, Yn, nb)) <= 1e-5
+    assert torch.all(F.scales.cpu()[np.tril_indices(cfg.NT)] == 1.0)
+
+
+# ------------------------------------------------------------------------------ low-precision maps
+def noise_floor(An, nb, pmap, preround, seed=0):
+    """The oracle against itself on an input perturbed at the level of the CUDA path's FP32-class
+    arithmetic (relative 2^-21 ~ 4.8e-7: 22-bit hi/lo operands and truncating tensor-core
+    accumulation give a measured backward error of 2-4e-7): how far two correct evaluations of the
+    emulated mosaic drift apart through flipped roundings."""
+    rng = np.random.default_rng(seed)
+    Ap = (An.astype(np.float64) * (1.0 + rng.uniform(-1, 1, An.shape) * 2.0 ** -21)).astype(np.float32)
+    Ap = np.tril(Ap) + np.tril(Ap, -1).T
+    L1, _, _ = tile_cholesky_emulated(An, nb, pmap, preround)
+    L2, _, _ = tile_cholesky_emulated(Ap, nb, pmap, preround)
+    return L1, relF(L2, L1)
+
+
+@pytest.mark.parametrize("case", ["fp16_uniform", "s1_rule_mosaic", "random_mixed", "fp8_col0_fp32"])
+def test_low_precision_maps(krr, case):
+    if case == "fp16_uniform":
+        cfg = scaled_config(CONFIGS["C4"], nb=128, n=1024, p=800)
+        A, Y = make_problem(cfg, device="cuda")
+        pmap, preround = oracle_uniform(cfg.NT, R.FP16), True
+    elif case == "s1_rule_mosaic":
+        cfg = scaled_config(CONFIGS["S1"], nb=128, n=2048, p=1536)
+        A, Y = make_problem(cfg, device="cuda")
+        pmap, _, _ = oracle_map(A.cpu().numpy(), cfg.nb, cfg.eps_target)
+        preround = True
+        assert len(set(pmap[np.tril_indices(cfg.NT, -1)].tolist())) == 3
+    elif case == "random_mixed":
+        # K ~ I regime without relatives (gamma = 12/p): any map keeps the matrix definite
+        cfg = replace(scaled_config(CONFIGS["S1"], nb=128, n=1024, p=768), genotype="maf", gamma_scale=4.0)
+        A, Y = make_problem(cfg, device="cuda")
+        rng = np.random.default_rng(5)
+        pmap = oracle_uniform(cfg.NT, R.FP32)
+        for i in range(cfg.NT):
+            for j in range(i):
+                pmap[i, j] = rng.integers(0, 3)
+        preround = True
+    else:   # C5': forced FP8 with tile column 0 kept in FP32, operands as stored
+        cfg = scaled_config(CONFIGS["C5"], nb=128, n=1024, p=200)
+        A, Y = make_problem(cfg, device="cuda")
+        pmap = oracle_uniform(cfg.NT, R.FP8)
+        pmap[1:, 0] = R.FP32
+        preround = False
+    nb = cfg.nb
+    An = A.cpu().numpy()
+    F = gpu_factor(krr, A, nb, pmap, preround)
+    Lo, floor = noise_floor(An, nb, pmap, preround)
+    Lg = F.dense().cpu().numpy()
+    _, sc_o, info_o = tile_cholesky_emulated(An, nb, pmap, preround)
+    assert int(F.info.item()) == info_o == 0
+    bg, bo = backward_error(An, Lg), backward_error(An, Lo)
+    lit = relF(Lg, Lo)
+    print(f"{case}: relF {lit:.3e} floor {floor:.3e} backward gpu {bg:.4e} oracle {bo:.4e}")
+    if case in ("fp16_uniform", "s1_rule_mosaic"):    # maps the rule produces: north_star's bound
+        assert bg <= 5e-4
+    assert abs(bg - bo) <= 0.02 * bo
+    assert lit <= max(1e-4, 2.0 * floor)
+    # first tile column: L_i0 = rd(A_i0 L_00^-T) has no accumulated noise -> at most one storage ulp
+    for i in range(1, cfg.NT):
+        g, o = Lg[i * nb:(i + 1) * nb, :nb], Lo[i * nb:(i + 1) * nb, :nb]
+        p = int(pmap[i, 0])
+        if p == R.FP32:                      # FP32 tiles: the literal criterion, tile by tile
+            assert relF(g, o) <= 1e-4, (case, i)
+            continue
+        u = R.UNIT_ROUNDOFF[p]
+        # one storage ulp (<= 2u|x|, or the subnormal spacing of a scaled FP8 tile) where FP32-level
+        # noise of the TRSM (<= 1e-5 of the tile's largest entry, conditioning of L_00 included)
+        # flips a rounding; exactly equal elsewhere
+        sub = float(sc_o[i, 0]) * 2.0 ** -9 if p == R.FP8 else 0.0
+        tol = 2.5 * u * np.abs(o) + sub + 1e-5 * np.abs(o).max()
+        assert np.all(np.abs(g - o) <= tol), (case, i, float(np.max(np.abs(g - o) - tol)))
+        assert np.mean(g == o) > 0.5, (case, i)          # most elements round identically
+    # FP8 scales: powers of two, equal to the oracle's
+    sg = F.scales.cpu().numpy().astype(np.float64)
+    low = np.tril_indices(cfg.NT)
+    mism = (sg[low] != sc_o[low]).sum()
+    assert mism <= 0.02 * len(low[0]) + 1          # a tile amax within rounding noise of a binade edge
+    # stored tiles are in their formats
+    for (i, j) in [(cfg.NT - 1, 0), (cfg.NT - 1, cfg.NT - 2), (2, 1)]:
+        blk = Lg[i * nb:(i + 1) * nb, j * nb:(j + 1) * nb]
+        p = int(pmap[i, j])
+        if p == R.FP8:
+            assert np.array_equal(R.rd_e4m3(blk / sg[i, j]) * sg[i, j], blk)
+        elif p == R.FP16:
+            assert np.array_equal(R.rd_fp16(blk), blk)
+    # solve parity with the same factor
+    alpha = krr.potrs(F, Y.clone())
+    torch.cuda.synchronize()
+    assert relF(alpha.cpu().numpy().astype(np.float64), potrs_fp64(Lg, Y.cpu().numpy(), nb)) <= 1e-5
+
+
+# ------------------------------------------------------------------------------ exact constructions
+@pytest.mark.parametrize("prec", [R.FP32, R.FP16, R.FP8, "mixed"])
+@pytest.mark.parametrize("n,nb", [(512, 128), (1024, 256)])
+def test_exactly_representable_factor_bit_for_bit(krr, prec, n, nb):
+    L0, A = exact_lower_factor(11, n, nb, device="cuda")
+    NT = n // nb
+    if prec == "mixed":
+        rng = np.random.default_rng(1)
+        pmap = oracle_uniform(NT, R.FP32)
+        for i in range(NT):
+            for j in range(i):
+                pmap[i, j] = rng.integers(0, 3)
+    else:
+        pmap = oracle_uniform(NT, prec)
+    F = gpu_factor(krr, A, nb, pmap, preround=False)
+    assert int(F.info.item()) == 0
+    assert torch.equal(F.dense(), L0)
+    # and the oracle agrees (same construction, same map)
+    Lo, _, info = tile_cholesky_emulated(A.cpu().numpy(), nb, pmap, preround_a=False)
+    assert info == 0 and np.array_equal(Lo, L0.cpu().numpy())
+
+
+# ------------------------------------------------------------------------------ breakdown
+def test_breakdown_reports_same_info_as_oracle(krr):
+    # forced FP8 on a gamma = 1/p matrix makes the rounded matrix indefinite (SURVEY finding 2)
+    cfg = scaled_config(CONFIGS["C1"], nb=128, n=512, p=500)
+    A, _ = make_problem(cfg, device="cuda")
+    pmap = oracle_uniform(cfg.NT, R.FP8)
+    F = gpu_factor(krr, A, cfg.nb, pmap)
+    _, _, info_o = tile_cholesky_emulated(A.cpu().numpy(), cfg.nb, pmap)
+    info_g = int(F.info.item())
+    assert info_o > 0 and info_g > 0
+    assert (info_g - 1) // cfg.nb == (info_o - 1) // cfg.nb          # same tile column
+    # an indefinite input: negative diagonal entry -> exact LAPACK info
+    B = A.clone()
+    B[300, 300] = -1.0
+    F = gpu_factor(krr, B, cfg.nb, oracle_uniform(cfg.NT, R.FP32))
+    assert int(F.info.item()) == 301
+
+
+def test_argument_errors(krr):
+    A = torch.eye(256, device="cuda")
+    h = krr.uniform_map(2, krr.FP32)
+    with pytest.raises(krr.KrrError):
+        krr.potrf_mp(A[:250, :250].contiguous(), 128, h.cuda(), h)       # nb does not divide n
+    bad = h.clone()
+    bad[1, 0] = 7
+    with pytest.raises(krr.KrrError):
+        krr.potrf_mp(A, 128, bad.cuda(), bad)
+    F = krr.potrf_mp(A, 128, h.cuda(), h)
+    with pytest.raises(krr.KrrError):
+        krr.potrs(F, torch.zeros((256, 40), device="cuda"))              # nrhs > 32
+    torch.cuda.synchronize()
+    assert torch.equal(F.dense(), torch.eye(256, dtype=torch.float64, device="cuda"))
+
+
+@pytest.mark.parametrize("nrhs", [1, 3, 4, 8, 16, 32])
+def test_potrs_every_nrhs_class(krr, nrhs):
+    cfg = scaled_config(CONFIGS["C1"], nb=128, n=512, p=300)
+    A, _ = make_problem(cfg, device="cuda")
+    g = torch.Generator(device="cuda").manual_seed(nrhs)
+    Y = torch.randn((cfg.n, nrhs), device="cuda", generator=g)
+    F = gpu_factor(krr, A, cfg.nb, oracle_uniform(cfg.NT, R.FP32))
+    alpha = krr.potrs(F, Y.clone())
+    torch.cuda.synchronize()
+    want = potrs_fp64(F.dense().cpu().numpy(), Y.cpu().numpy(), cfg.nb)
+    assert relF(alpha.cpu().numpy().astype(np.float64), want) <= 1e-5
+    # strided right-hand side (ldb > nrhs)
+    big = torch.zeros((cfg.n, nrhs + 5), device="cuda")
+    big[:, :nrhs] = Y
+    krr.potrs(F, big[:, :nrhs])
+    torch.cuda.synchronize()
+    assert torch.equal(big[:, :nrhs], alpha) and float(big[:, nrhs:].abs().max()) == 0.0
+
+
+def test_associate_host_matches_device_path(krr):
+    cfg = scaled_config(CONFIGS["S1"], nb=128, n=1024, p=768)
+    A, Y = make_problem(cfg, device="cuda")
+    d_map, _, _, _ = krr.precision_map(A, cfg.nb, cfg.eps_target, cfg.allowed)
+    h = d_map.cpu()
+    F = krr.potrf_mp(A, cfg.nb, d_map, h)
+    alpha = krr.potrs(F, Y.clone())
+    hA, hY = A.cpu().pin_memory(), Y.cpu().pin_memory()
+    a2, m2, info, _ = krr.associate_host(hA, cfg.nb, hY, cfg.eps_target, cfg.allowed)
+    assert info == 0 and torch.equal(m2, h) and torch.equal(a2, alpha.cpu())
+    a3, m3, info3, _ = krr.associate_host(hA, cfg.nb, hY, force_prec=krr.FP32)
+    assert info3 == 0 and int((m3[np.tril_indices(cfg.NT)] != 0).sum()) == 0

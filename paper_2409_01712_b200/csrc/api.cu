@@ -13,6 +13,7 @@
 #include "panel.cuh"
 #include "potrs.cuh"
 #include "precision_map.cuh"
+#include "tri128.cuh"
 
 namespace krr {
 
@@ -160,24 +161,22 @@ static int launch_gemm(const CUtensorMap& a_hi, const CUtensorMap& a_lo, const C
     return cudaGetLastError() == cudaSuccess ? KRR_OK : KRR_ERR_CUDA;
 }
 
+template <int NRHS>
+static int set_potrs_attrs() {
+    const int big = 220 * 1024;
+    KRR_CUDA_CHECK(cudaFuncSetAttribute(potrs_fwd_update_kernel<NRHS>, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
+    KRR_CUDA_CHECK(cudaFuncSetAttribute(potrs_bwd_update_kernel<NRHS>, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
+    KRR_CUDA_CHECK(cudaFuncSetAttribute(potrs_diag_kernel<NRHS>, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
+    return KRR_OK;
+}
+
 static int set_kernel_attrs() {
     static bool done = false;
     if (done) return KRR_OK;
     KRR_CUDA_CHECK(cudaFuncSetAttribute(gemm_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem));
-    KRR_CUDA_CHECK(cudaFuncSetAttribute(potrf128_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kPotrfSmem));
-    const int big = 200 * 1024;
-    KRR_CUDA_CHECK(cudaFuncSetAttribute(potrs_fwd_update_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
-    KRR_CUDA_CHECK(cudaFuncSetAttribute(potrs_fwd_update_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
-    KRR_CUDA_CHECK(cudaFuncSetAttribute(potrs_fwd_update_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
-    KRR_CUDA_CHECK(cudaFuncSetAttribute(potrs_fwd_update_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
-    KRR_CUDA_CHECK(cudaFuncSetAttribute(potrs_bwd_update_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
-    KRR_CUDA_CHECK(cudaFuncSetAttribute(potrs_bwd_update_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
-    KRR_CUDA_CHECK(cudaFuncSetAttribute(potrs_bwd_update_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
-    KRR_CUDA_CHECK(cudaFuncSetAttribute(potrs_bwd_update_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
-    KRR_CUDA_CHECK(cudaFuncSetAttribute(potrs_diag_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
-    KRR_CUDA_CHECK(cudaFuncSetAttribute(potrs_diag_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
-    KRR_CUDA_CHECK(cudaFuncSetAttribute(potrs_diag_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
-    KRR_CUDA_CHECK(cudaFuncSetAttribute(potrs_diag_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
+    KRR_CUDA_CHECK(cudaFuncSetAttribute(potrf128_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kTriSmem));
+    KRR_CUDA_CHECK(cudaFuncSetAttribute(trtri128_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kTriSmem));
+    if (set_potrs_attrs<4>() || set_potrs_attrs<8>() || set_potrs_attrs<16>() || set_potrs_attrs<32>()) return KRR_ERR_CUDA;
     done = true;
     return KRR_OK;
 }
@@ -364,7 +363,7 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
                 rc = launch_gemm(tmH, tmL, tmH, tmL, op, num_sms, st);
                 if (rc) return rc;
             }
-            rc = launch(CAT_POTRF, potrf128_kernel, dim3(1), dim3(kPotrfThreads), static_cast<size_t>(kPotrfSmem), st, W, nb,
+            rc = launch(CAT_POTRF, potrf128_kernel, dim3(1), dim3(kTriThreads), static_cast<size_t>(kTriSmem), st, W, nb,
                         c * kBlk, c * kBlk, linv_hi, linv_lo, linv_scale, d_info,
                         static_cast<int64_t>(k) * nb + static_cast<int64_t>(c) * kBlk + 1);
             if (rc) return rc;
@@ -383,27 +382,51 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
 }
 
 // ------------------------------------------------------------------------- solve
+static int rhs_class(int nrhs) { return nrhs <= 4 ? 4 : (nrhs <= 8 ? 8 : (nrhs <= 16 ? 16 : 32)); }
+
+struct PotrsWs { size_t off_table, dinv, dinvT, total; };
+static PotrsWs potrs_ws_layout(int64_t n, int nb) {
+    const size_t NT = n / nb;
+    PotrsWs w;
+    size_t o = 0;
+    w.off_table = o; o = align_up(o + NT * NT * sizeof(int64_t), 1024);
+    w.dinv = o;      o = align_up(o + static_cast<size_t>(n) * kBlk * sizeof(float), 1024);
+    w.dinvT = o;     o = align_up(o + static_cast<size_t>(n) * kBlk * sizeof(float), 1024);
+    w.total = o;
+    return w;
+}
+
 size_t krr_potrs_workspace(int64_t n, int nb, int nrhs) {
     if (check_shape(n, nb) != KRR_OK || nrhs < 1 || nrhs > kMaxRhs) return 0;
-    const size_t NT = n / nb;
-    return align_up(NT * NT * sizeof(int64_t), 1024);
+    if (static_cast<int64_t>(rhs_class(nrhs)) * nb > 32768) return 0;     // solved block must fit in smem
+    return potrs_ws_layout(n, nb).total;
 }
 
 }  // extern "C"
 
 template <int NRHS>
 static int potrs_run(const uint8_t* factor, const float* d_scales, const uint8_t* d_map, const std::vector<int64_t>& hoff,
-                     const int64_t* off, int NT, int nb, float* B, int64_t ldb, int nrhs, cudaStream_t st) {
+                     const int64_t* off, const float* dinv, const float* dinvT, int NT, int nb, float* B, int64_t ldb,
+                     int nrhs, int num_sms, cudaStream_t st) {
+    constexpr int ROWS = 64 / NRHS, NW = kSolveThreads / 32, CPL = (NRHS <= 16) ? 4 : 2;
     const size_t smem_z = static_cast<size_t>(NRHS) * nb * sizeof(float);
-    const size_t smem_d = smem_z + (32 * 33 + 8 * 32 * NRHS) * sizeof(float);
+    const size_t smem_fd = smem_z + NRHS * kBlk * sizeof(float);
+    const size_t smem_bd = smem_fd + static_cast<size_t>(kDiagThreads / 64) * 32 * CPL * NRHS * sizeof(float);
+    const size_t smem_bu = smem_z + static_cast<size_t>(NW / 2) * 32 * CPL * NRHS * sizeof(float);
+    const int64_t blk_elems = static_cast<int64_t>(kBlk) * kBlk;
+    const int nsub = nb / kBlk;
     int rc;
     for (int k = 0; k < NT; ++k) {
         const float* Lkk = reinterpret_cast<const float*>(factor + hoff[static_cast<size_t>(k) * NT + k]);
         float* Bk = B + static_cast<int64_t>(k) * nb * ldb;
-        rc = launch(CAT_POTRS, potrs_diag_kernel<NRHS>, dim3(1), dim3(256), smem_d, st, nb, Lkk, Bk, ldb, nrhs, 0);
+        rc = launch(CAT_POTRS, potrs_diag_kernel<NRHS>, dim3(1), dim3(kDiagThreads), smem_fd, st, nb, Lkk,
+                    dinv + k * nsub * blk_elems, dinvT + k * nsub * blk_elems, Bk, ldb, nrhs, 0);
         if (rc) return rc;
         if (k + 1 < NT) {
-            rc = launch(CAT_POTRS, potrs_fwd_update_kernel<NRHS>, dim3((NT - k - 1) * (nb / 32)), dim3(256), smem_z, st, NT, nb, k,
+            const int64_t tasks = static_cast<int64_t>(NT - k - 1) * nb / ROWS;
+            const int64_t want = (tasks + NW - 1) / NW;
+            const int grid = static_cast<int>(want < 3LL * num_sms ? want : 3LL * num_sms);
+            rc = launch(CAT_POTRS, potrs_fwd_update_kernel<NRHS>, dim3(grid), dim3(kSolveThreads), smem_z, st, NT, nb, k,
                         factor, off, d_map, d_scales, B, ldb, nrhs);
             if (rc) return rc;
         }
@@ -411,11 +434,12 @@ static int potrs_run(const uint8_t* factor, const float* d_scales, const uint8_t
     for (int k = NT - 1; k >= 0; --k) {
         const float* Lkk = reinterpret_cast<const float*>(factor + hoff[static_cast<size_t>(k) * NT + k]);
         float* Bk = B + static_cast<int64_t>(k) * nb * ldb;
-        rc = launch(CAT_POTRS, potrs_diag_kernel<NRHS>, dim3(1), dim3(256), smem_d, st, nb, Lkk, Bk, ldb, nrhs, 1);
+        rc = launch(CAT_POTRS, potrs_diag_kernel<NRHS>, dim3(1), dim3(kDiagThreads), smem_bd, st, nb, Lkk,
+                    dinv + k * nsub * blk_elems, dinvT + k * nsub * blk_elems, Bk, ldb, nrhs, 1);
         if (rc) return rc;
         if (k > 0) {
-            rc = launch(CAT_POTRS, potrs_bwd_update_kernel<NRHS>, dim3(k * (nb / 128)), dim3(128), smem_z, st, NT, nb, k, factor, off,
-                        d_map, d_scales, B, ldb, nrhs);
+            rc = launch(CAT_POTRS, potrs_bwd_update_kernel<NRHS>, dim3(k * (nb / (32 * CPL))), dim3(kSolveThreads), smem_bu, st,
+                        NT, nb, k, factor, off, d_map, d_scales, B, ldb, nrhs);
             if (rc) return rc;
         }
     }
@@ -431,25 +455,37 @@ int krr_potrs(const void* d_factor, const float* d_scales, const uint8_t* d_map,
     int rc = check_shape(n, nb);
     if (rc) return rc;
     if (nrhs < 1 || nrhs > kMaxRhs || ldb < nrhs) return KRR_ERR_ARG;
+    if (static_cast<int64_t>(rhs_class(nrhs)) * nb > 32768) return KRR_ERR_SHAPE;
+    if (reinterpret_cast<uintptr_t>(d_ws) % 16 != 0) return KRR_ERR_ARG;
     const int NT = static_cast<int>(n / nb);
     rc = check_map(NT, h_map, nullptr);
     if (rc) return rc;
-    if (ws_bytes < krr_potrs_workspace(n, nb, nrhs)) return KRR_ERR_WORKSPACE;
-    rc = check_device(nullptr);
+    const PotrsWs L = potrs_ws_layout(n, nb);
+    if (ws_bytes < L.total) return KRR_ERR_WORKSPACE;
+    int num_sms = 0;
+    rc = check_device(&num_sms);
     if (rc) return rc;
     rc = set_kernel_attrs();
     if (rc) return rc;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     std::vector<int64_t> hoff;
     host_offsets(NT, nb, h_map, &hoff);
-    int64_t* off = static_cast<int64_t*>(d_ws);
+    uint8_t* ws = static_cast<uint8_t*>(d_ws);
+    int64_t* off = reinterpret_cast<int64_t*>(ws + L.off_table);
+    float* dinv = reinterpret_cast<float*>(ws + L.dinv);
+    float* dinvT = reinterpret_cast<float*>(ws + L.dinvT);
     rc = launch(CAT_MISC, offsets_kernel, dim3(1), dim3(32), 0, st, NT, nb, d_map, off);
     if (rc) return rc;
     const uint8_t* factor = static_cast<const uint8_t*>(d_factor);
-    if (nrhs <= 4) return potrs_run<4>(factor, d_scales, d_map, hoff, off, NT, nb, d_B, ldb, nrhs, st);
-    if (nrhs <= 8) return potrs_run<8>(factor, d_scales, d_map, hoff, off, NT, nb, d_B, ldb, nrhs, st);
-    if (nrhs <= 16) return potrs_run<16>(factor, d_scales, d_map, hoff, off, NT, nb, d_B, ldb, nrhs, st);
-    return potrs_run<32>(factor, d_scales, d_map, hoff, off, NT, nb, d_B, ldb, nrhs, st);
+    rc = launch(CAT_POTRS, trtri128_kernel, dim3(static_cast<unsigned>(n / kBlk)), dim3(kTriThreads), static_cast<size_t>(kTriSmem), st,
+                factor, static_cast<const int64_t*>(off), NT, nb, dinv, dinvT);
+    if (rc) return rc;
+    switch (rhs_class(nrhs)) {
+        case 4:  return potrs_run<4>(factor, d_scales, d_map, hoff, off, dinv, dinvT, NT, nb, d_B, ldb, nrhs, num_sms, st);
+        case 8:  return potrs_run<8>(factor, d_scales, d_map, hoff, off, dinv, dinvT, NT, nb, d_B, ldb, nrhs, num_sms, st);
+        case 16: return potrs_run<16>(factor, d_scales, d_map, hoff, off, dinv, dinvT, NT, nb, d_B, ldb, nrhs, num_sms, st);
+        default: return potrs_run<32>(factor, d_scales, d_map, hoff, off, dinv, dinvT, NT, nb, d_B, ldb, nrhs, num_sms, st);
+    }
 }
 
 }  // extern "C"

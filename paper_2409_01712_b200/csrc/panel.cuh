@@ -1,6 +1,5 @@
-// FP32 panel kernels of the tile Cholesky:
-//   potrf128_kernel   POTRF of one 128x128 diagonal block in FP32 on plain ALUs, plus its inverse
-//                     (the panel TRSM multiplies by it on the tensor cores, gemm_tc.cuh MODE_P3)
+// Panel-side helper kernels of the tile Cholesky (the FP32 POTRF of a
+// 128x128 block is in tri128.cuh):
 //   finalize_kernel   rounds the finished tile column into the storage precisions of the mosaic
 //                     (per-tile power-of-two FP8 scale from the tile amax) -- "round once"
 //   offsets_kernel    byte offsets of the mosaic tiles from the device map
@@ -9,120 +8,6 @@
 #include "common.cuh"
 
 namespace krr {
-
-constexpr int kPotrfThreads = 128;
-constexpr int kLd = kBlk + 1;                    // padded smem leading dimension
-constexpr int kPotrfSmem = 2 * kBlk * kLd * 4;   // L and inv(L)
-
-// W: panel workspace [m][nb]; block rows r0..r0+127 (panel-local), columns c0..c0+127.
-// Writes L (lower, zeros above) back into W and inv(L) as FP16 hi/lo into linv_hi/lo
-// ([nb][128] row-major, rows c0..c0+127).  col_base = 1-based global index of the block's
-// first column, for info.
-__global__ void __launch_bounds__(kPotrfThreads)
-potrf128_kernel(float* __restrict__ W, int nb, int r0, int c0, __half* __restrict__ linv_hi,
-                __half* __restrict__ linv_lo, float* __restrict__ linv_scale, int* __restrict__ info,
-                int64_t col_base) {
-    extern __shared__ float sm[];
-    float* a = sm;                 // [128][129] : S, then L
-    float* x = sm + kBlk * kLd;    // [128][129] : inv(L)
-    const int tid = threadIdx.x;
-    // coalesced load of the 128x128 block
-    for (int idx = tid; idx < kBlk * (kBlk / 4); idx += kPotrfThreads) {
-        const int r = idx / (kBlk / 4), c4 = (idx % (kBlk / 4)) * 4;
-        const float4 v = *reinterpret_cast<const float4*>(W + static_cast<int64_t>(r0 + r) * nb + c0 + c4);
-        a[r * kLd + c4 + 0] = v.x;
-        a[r * kLd + c4 + 1] = v.y;
-        a[r * kLd + c4 + 2] = v.z;
-        a[r * kLd + c4 + 3] = v.w;
-    }
-    __syncthreads();
-    // left-looking column Cholesky, thread i owns row i
-    const int i = tid;
-    for (int j = 0; j < kBlk; ++j) {
-        float s = 0.0f;
-        if (i >= j) {
-            const float* ai = a + i * kLd;
-            const float* aj = a + j * kLd;
-            float s0 = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f;
-            int l = 0;
-            for (; l + 4 <= j; l += 4) {
-                s0 = fmaf(ai[l + 0], aj[l + 0], s0);
-                s1 = fmaf(ai[l + 1], aj[l + 1], s1);
-                s2 = fmaf(ai[l + 2], aj[l + 2], s2);
-                s3 = fmaf(ai[l + 3], aj[l + 3], s3);
-            }
-            for (; l < j; ++l) s0 = fmaf(ai[l], aj[l], s0);
-            s = ai[j] - ((s0 + s1) + (s2 + s3));
-        }
-        // a[j][j] is read by the other rows only after the barrier below
-        if (i == j) {
-            if (!(s > 0.0f)) atomicCAS(info, 0, static_cast<int>(col_base + j));
-            a[j * kLd + j] = sqrtf(s);
-        }
-        __syncthreads();
-        if (i > j) a[i * kLd + j] = s / a[j * kLd + j];
-        __syncthreads();                       // row j+1 is read by every thread next iteration
-    }
-    // inverse: thread j computes column j of X = L^{-1} by forward substitution
-    {
-        const int j = tid;
-        for (int r = 0; r < kBlk; ++r) x[r * kLd + j] = 0.0f;
-        for (int r = j; r < kBlk; ++r) {
-            const float* ar = a + r * kLd;
-            float s0 = 0.f, s1 = 0.f;
-            int l = j;
-            for (; l + 2 <= r; l += 2) {
-                s0 = fmaf(ar[l], x[l * kLd + j], s0);
-                s1 = fmaf(ar[l + 1], x[(l + 1) * kLd + j], s1);
-            }
-            for (; l < r; ++l) s0 = fmaf(ar[l], x[l * kLd + j], s0);
-            const float rhs = (r == j) ? 1.0f : 0.0f;
-            x[r * kLd + j] = (rhs - (s0 + s1)) / ar[r];
-        }
-    }
-    // power-of-two scale of the inverse's planes: max|x| * si <= 2^14
-    __shared__ float s_red[kPotrfThreads];
-    {
-        float m = 0.0f;
-        for (int r = tid; r < kBlk; ++r) m = fmaxf(m, fabsf(x[r * kLd + tid]));
-        s_red[tid] = m;
-    }
-    __syncthreads();
-    for (int o = kPotrfThreads / 2; o > 0; o >>= 1) {
-        if (tid < o) s_red[tid] = fmaxf(s_red[tid], s_red[tid + o]);
-        __syncthreads();
-    }
-    float si = 1.0f;
-    {
-        const float m = s_red[0];
-        if (m > 0.0f && m < 3.0e38f) {
-            int e;
-            frexpf(m, &e);                 // m <= 2^e
-            si = ldexpf(1.0f, 14 - e);
-        }
-    }
-    if (tid == 0) linv_scale[c0 / kBlk] = si;
-    // write back L (zeros above the diagonal) and inv(L) planes
-    for (int idx = tid; idx < kBlk * (kBlk / 4); idx += kPotrfThreads) {
-        const int r = idx / (kBlk / 4), c4 = (idx % (kBlk / 4)) * 4;
-        float4 v;
-        v.x = (c4 + 0 <= r) ? a[r * kLd + c4 + 0] : 0.0f;
-        v.y = (c4 + 1 <= r) ? a[r * kLd + c4 + 1] : 0.0f;
-        v.z = (c4 + 2 <= r) ? a[r * kLd + c4 + 2] : 0.0f;
-        v.w = (c4 + 3 <= r) ? a[r * kLd + c4 + 3] : 0.0f;
-        *reinterpret_cast<float4*>(W + static_cast<int64_t>(r0 + r) * nb + c0 + c4) = v;
-        __align__(8) __half hi[4];
-        __align__(8) __half lo[4];
-#pragma unroll
-        for (int u = 0; u < 4; ++u) {
-            const float xv = (c4 + u <= r) ? x[r * kLd + c4 + u] * si : 0.0f;
-            hi[u] = __float2half_rn(xv);
-            lo[u] = __float2half_rn(xv - __half2float(hi[u]));
-        }
-        *reinterpret_cast<uint2*>(linv_hi + static_cast<int64_t>(c0 + r) * kBlk + c4) = *reinterpret_cast<const uint2*>(hi);
-        *reinterpret_cast<uint2*>(linv_lo + static_cast<int64_t>(c0 + r) * kBlk + c4) = *reinterpret_cast<const uint2*>(lo);
-    }
-}
 
 // Global power-of-two scales of the FP16 operand images from the largest diagonal entry of A
 // (|L_ij| <= sqrt(A_ii), |S_ij| <= max A_ii):  scl = {sx, ss, 1/sx^2, 1/ss}.  One CTA.

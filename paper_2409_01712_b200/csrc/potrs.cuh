@@ -1,205 +1,369 @@
 // krr_potrs kernels: forward and backward substitution in FP32 with the tile mosaic
 // ("W <- Solve(K~, P_h)", "forward and backward substitution operations
-// in the full FP32 precision").  nrhs is small (4..32), so each sweep is bound by reading L once
-// from HBM.  Right-hand sides are row-major n x nrhs.
+// in the full FP32 precision").  nrhs is small (1..32), so each sweep is bound by reading L once
+// from HBM and by 2*nrhs FP32 flops per element of L.  Right-hand sides are
+// row-major n x nrhs.
+//
+// Structure (right-looking over tile columns, like the paper's tile algorithm):
+//   trtri128_kernel (tri128.cuh)   inverses of the 128x128 diagonal blocks of every diagonal tile, once
+//   potrs_diag_kernel              one diagonal tile: 128-row blocks in order, each a product with the
+//                                  already solved part of the tile followed by a product with the
+//                                  inverted diagonal block
+//   potrs_fwd_update_kernel        Y_i -= L_ik Z_k for all i > k   (streams tile column k once)
+//   potrs_bwd_update_kernel        Z_j -= L_kj^T alpha_k for all j < k (streams tile row k once)
+// All sums are accumulated in a fixed order: results are deterministic.
 #pragma once
 #include "common.cuh"
 
 namespace krr {
 
 constexpr int kMaxRhs = 32;
+constexpr int kSolveThreads = 256;          // update kernels
+constexpr int kDiagThreads = 512;           // diagonal-tile kernel
 
-// Dequantising 4-element load of a mosaic tile row segment (columns c..c+3, c % 4 == 0).
+// Dequantising loads of CPL (4 or 2) consecutive elements of a mosaic tile (element index e).
 __device__ __forceinline__ float4 load4(const uint8_t* tile, int p, float s, int64_t e) {
-    if (p == KRR_FP32) return *reinterpret_cast<const float4*>(tile + e * 4);
+    if (p == KRR_FP32) return __ldg(reinterpret_cast<const float4*>(tile + e * 4));
     if (p == KRR_FP16) {
-        const uint2 raw = *reinterpret_cast<const uint2*>(tile + e * 2);
+        const uint2 raw = __ldg(reinterpret_cast<const uint2*>(tile + e * 2));
         const __half2 a = *reinterpret_cast<const __half2*>(&raw.x);
         const __half2 b = *reinterpret_cast<const __half2*>(&raw.y);
         return make_float4(__low2float(a), __high2float(a), __low2float(b), __high2float(b));
     }
-    const uint32_t raw = *reinterpret_cast<const uint32_t*>(tile + e);
+    const uint32_t raw = __ldg(reinterpret_cast<const uint32_t*>(tile + e));
     return make_float4(e4m3_to_f32(raw & 0xff) * s, e4m3_to_f32((raw >> 8) & 0xff) * s,
                        e4m3_to_f32((raw >> 16) & 0xff) * s, e4m3_to_f32(raw >> 24) * s);
 }
-__device__ __forceinline__ float load1(const uint8_t* tile, int p, float s, int64_t e) {
-    if (p == KRR_FP32) return *reinterpret_cast<const float*>(tile + e * 4);
-    if (p == KRR_FP16) return __half2float(*reinterpret_cast<const __half*>(tile + e * 2));
-    return e4m3_to_f32(tile[e]) * s;
+__device__ __forceinline__ float2 load2(const uint8_t* tile, int p, float s, int64_t e) {
+    if (p == KRR_FP32) return __ldg(reinterpret_cast<const float2*>(tile + e * 4));
+    if (p == KRR_FP16) {
+        const uint32_t raw = __ldg(reinterpret_cast<const uint32_t*>(tile + e * 2));
+        const __half2 a = *reinterpret_cast<const __half2*>(&raw);
+        return make_float2(__low2float(a), __high2float(a));
+    }
+    const uint16_t raw = __ldg(reinterpret_cast<const uint16_t*>(tile + e));
+    return make_float2(e4m3_to_f32(raw & 0xff) * s, e4m3_to_f32(raw >> 8) * s);
+}
+
+// Sum 64 per-lane values v[0..63] across the 32 lanes of a warp with 62 shuffles (each step halves
+// the number of values a lane carries).  Afterwards lane `l` holds in v[0], v[1] the totals of the
+// values with index  warp_reduce64_index(l) + {0, 1}.
+__device__ __forceinline__ void warp_reduce64(float (&v)[64], int lane) {
+#pragma unroll
+    for (int step = 0; step < 5; ++step) {
+        const int o = 16 >> step;            // lane offset 16, 8, 4, 2, 1
+        const int cnt = 32 >> step;          // values kept after this step
+        const bool upper = (lane & o) != 0;
+#pragma unroll
+        for (int i = 0; i < cnt; ++i) {
+            const float send = upper ? v[i] : v[i + cnt];
+            const float keep = upper ? v[i + cnt] : v[i];
+            v[i] = keep + __shfl_xor_sync(0xffffffffu, send, o);
+        }
+    }
+}
+__device__ __forceinline__ int warp_reduce64_index(int lane) {
+    return ((lane & 16) ? 32 : 0) + ((lane & 8) ? 16 : 0) + ((lane & 4) ? 8 : 0) + ((lane & 2) ? 4 : 0) +
+           ((lane & 1) ? 2 : 0);
+}
+
+// acc[u*NRHS + h] += sum_{l in [0,K)} row_u[l] * zs[h*zld + l]  for u in [0, ROWS), ROWS*NRHS = 64.
+// One warp; lanes stride over l in float4 chunks (K % 128 == 0).  rows: FP32, row stride ld floats.
+template <int NRHS>
+__device__ __forceinline__ void rows_dot_f32(const float* __restrict__ rows, int64_t ld, int K,
+                                             const float* __restrict__ zs, int zld, int lane, float (&acc)[64]) {
+    constexpr int ROWS = 64 / NRHS;
+    for (int l = lane * 4; l < K; l += 128) {
+        float4 a[ROWS];
+#pragma unroll
+        for (int u = 0; u < ROWS; ++u) a[u] = __ldg(reinterpret_cast<const float4*>(rows + u * ld + l));
+#pragma unroll
+        for (int h = 0; h < NRHS; ++h) {
+            const float4 z = *reinterpret_cast<const float4*>(zs + h * zld + l);
+#pragma unroll
+            for (int u = 0; u < ROWS; ++u)
+                acc[u * NRHS + h] = fmaf(a[u].x, z.x, fmaf(a[u].y, z.y, fmaf(a[u].z, z.z, fmaf(a[u].w, z.w, acc[u * NRHS + h]))));
+        }
+    }
 }
 
 // ---------------------------------------------------------------------------------------------
 // Forward update after Z_k is known:  Y_i -= L_ik Z_k  for all i > k.
-// grid.x = (NT-k-1)*nb / 32 (32 rows per CTA, 4 per warp), 256 threads, smem = nrhs*nb floats.
+// Persistent CTAs over groups of 8 * ROWS rows (ROWS = 64 / NRHS rows per warp); smem = NRHS*nb floats.
 template <int NRHS>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(kSolveThreads)
 potrs_fwd_update_kernel(int NT, int nb, int k, const uint8_t* __restrict__ factor,
                         const int64_t* __restrict__ off, const uint8_t* __restrict__ map,
                         const float* __restrict__ scales, float* __restrict__ B, int64_t ldb, int nrhs) {
-    extern __shared__ float zs[];                      // [NRHS][nb]
+    constexpr int ROWS = 64 / NRHS;
+    constexpr int NW = kSolveThreads / 32;
+    extern __shared__ __align__(16) float zs[];        // [NRHS][nb]
     const float* Zk = B + static_cast<int64_t>(k) * nb * ldb;
-    for (int idx = threadIdx.x; idx < nb * nrhs; idx += 256) {
-        const int c = idx / nrhs, rh = idx % nrhs;
-        zs[rh * nb + c] = Zk[static_cast<int64_t>(c) * ldb + rh];
+    for (int idx = threadIdx.x; idx < nb * NRHS; idx += kSolveThreads) {
+        const int c = idx / NRHS, rh = idx % NRHS;
+        zs[rh * nb + c] = (rh < nrhs) ? Zk[static_cast<int64_t>(c) * ldb + rh] : 0.0f;
     }
     __syncthreads();
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int64_t prow0 = static_cast<int64_t>(blockIdx.x) * 32;       // rows below tile k
-    const int i = k + 1 + static_cast<int>(prow0 / nb);
-    const int p = map[i * NT + k];
-    const float s = scales[i * NT + k];
-    const uint8_t* tile = factor + off[i * NT + k];
-    for (int rr = 0; rr < 4; ++rr) {
-        const int r = static_cast<int>(prow0 % nb) + warp * 4 + rr;
-        float acc[NRHS];
+    const int64_t ngroups = static_cast<int64_t>(NT - k - 1) * nb / ROWS;   // warp tasks
+    for (int64_t g = static_cast<int64_t>(blockIdx.x) * NW + warp; g < ngroups; g += static_cast<int64_t>(gridDim.x) * NW) {
+        const int64_t prow = g * ROWS;                                      // row below tile k
+        const int i = k + 1 + static_cast<int>(prow / nb);
+        const int r0 = static_cast<int>(prow % nb);
+        const int p = map[i * NT + k];
+        const float s = scales[i * NT + k];
+        const uint8_t* tile = factor + off[i * NT + k];
+        float acc[64];
 #pragma unroll
-        for (int h = 0; h < NRHS; ++h) acc[h] = 0.0f;
-        for (int c = lane * 4; c < nb; c += 128) {
-            const float4 l = load4(tile, p, s, static_cast<int64_t>(r) * nb + c);
+        for (int v = 0; v < 64; ++v) acc[v] = 0.0f;
+        if (p == KRR_FP32) {
+            rows_dot_f32<NRHS>(reinterpret_cast<const float*>(tile) + static_cast<int64_t>(r0) * nb, nb, nb, zs, nb, lane, acc);
+        } else {
+            for (int l = lane * 4; l < nb; l += 128) {
+                float4 a[ROWS];
 #pragma unroll
-            for (int h = 0; h < NRHS; ++h) {
-                if (h < nrhs) {
-                    const float4 z = *reinterpret_cast<const float4*>(zs + h * nb + c);
-                    acc[h] = fmaf(l.x, z.x, fmaf(l.y, z.y, fmaf(l.z, z.z, fmaf(l.w, z.w, acc[h]))));
+                for (int u = 0; u < ROWS; ++u) a[u] = load4(tile, p, s, static_cast<int64_t>(r0 + u) * nb + l);
+#pragma unroll
+                for (int h = 0; h < NRHS; ++h) {
+                    const float4 z = *reinterpret_cast<const float4*>(zs + h * nb + l);
+#pragma unroll
+                    for (int u = 0; u < ROWS; ++u)
+                        acc[u * NRHS + h] = fmaf(a[u].x, z.x, fmaf(a[u].y, z.y, fmaf(a[u].z, z.z, fmaf(a[u].w, z.w, acc[u * NRHS + h]))));
                 }
             }
         }
+        warp_reduce64(acc, lane);
+        const int v0 = warp_reduce64_index(lane);
 #pragma unroll
-        for (int h = 0; h < NRHS; ++h) {
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) acc[h] += __shfl_xor_sync(0xffffffffu, acc[h], o);
+        for (int t = 0; t < 2; ++t) {
+            const int u = (v0 + t) / NRHS, h = (v0 + t) % NRHS;
+            if (h < nrhs) B[(static_cast<int64_t>(i) * nb + r0 + u) * ldb + h] -= acc[t];
         }
-        float* y = B + (static_cast<int64_t>(i) * nb + r) * ldb;
-#pragma unroll
-        for (int h = 0; h < NRHS; ++h)
-            if (lane == h && h < nrhs) y[h] -= acc[h];
     }
 }
 
 // Backward update after alpha_k is known:  Z_j -= L_kj^T alpha_k  for all j < k.
-// grid.x = k*nb / 128 (128 columns per CTA, one per thread), smem = nrhs*nb floats.
+// One CTA per (tile j, strip of 32*CPL columns); warps split the nb rows (interleaved), lanes own
+// CPL consecutive columns; the per-warp partial sums are combined through shared memory in a fixed
+// tree order.  smem = nb*NRHS floats (alpha_k) + (NW/2) * 32*CPL*NRHS floats.
 template <int NRHS>
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(kSolveThreads)
 potrs_bwd_update_kernel(int NT, int nb, int k, const uint8_t* __restrict__ factor,
                         const int64_t* __restrict__ off, const uint8_t* __restrict__ map,
                         const float* __restrict__ scales, float* __restrict__ B, int64_t ldb, int nrhs) {
-    extern __shared__ float as[];                      // [nb][NRHS] alpha_k
+    constexpr int CPL = (NRHS <= 16) ? 4 : 2;
+    constexpr int NACC = CPL * NRHS;
+    constexpr int NW = kSolveThreads / 32;
+    constexpr int STRIP = 32 * CPL;
+    extern __shared__ __align__(16) float as[];        // [nb][NRHS] alpha_k, then the reduction buffers
+    float* red = as + static_cast<size_t>(nb) * NRHS;  // [NW/2][32 lanes][NACC]
     const float* Ak = B + static_cast<int64_t>(k) * nb * ldb;
-    for (int idx = threadIdx.x; idx < nb * NRHS; idx += 128) {
+    for (int idx = threadIdx.x; idx < nb * NRHS; idx += kSolveThreads) {
         const int r = idx / NRHS, rh = idx % NRHS;
         as[idx] = (rh < nrhs) ? Ak[static_cast<int64_t>(r) * ldb + rh] : 0.0f;
     }
     __syncthreads();
-    const int64_t gcol = static_cast<int64_t>(blockIdx.x) * 128 + threadIdx.x;
-    const int j = static_cast<int>(gcol / nb), c = static_cast<int>(gcol % nb);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int strips = nb / STRIP;
+    const int j = blockIdx.x / strips;
+    const int c0 = (blockIdx.x % strips) * STRIP + lane * CPL;
     const int p = map[k * NT + j];
     const float s = scales[k * NT + j];
     const uint8_t* tile = factor + off[k * NT + j];
-    float acc[NRHS];
+    float acc[NACC];
 #pragma unroll
-    for (int h = 0; h < NRHS; ++h) acc[h] = 0.0f;
-    for (int r = 0; r < nb; ++r) {
-        const float l = load1(tile, p, s, static_cast<int64_t>(r) * nb + c);
+    for (int v = 0; v < NACC; ++v) acc[v] = 0.0f;
+    for (int r = warp; r < nb; r += NW * 4) {
+        float l[4][CPL];
 #pragma unroll
-        for (int h = 0; h < NRHS; ++h) acc[h] = fmaf(l, as[r * NRHS + h], acc[h]);
-    }
-    float* z = B + gcol * ldb;
-#pragma unroll
-    for (int h = 0; h < NRHS; ++h)
-        if (h < nrhs) z[h] -= acc[h];
-}
-
-// Diagonal tile solve, one CTA of 256 threads: forward (L z = y) or backward (L^T a = z), in place
-// on rows k*nb .. (k+1)*nb of B.  Blocks of 32 rows: a GEMV with the already-solved part, then a
-// 32x32 triangular solve by one warp (lane = right-hand side).
-template <int NRHS>
-__global__ void __launch_bounds__(256)
-potrs_diag_kernel(int nb, const float* __restrict__ Lkk, float* __restrict__ Bk, int64_t ldb, int nrhs,
-                  int backward) {
-    extern __shared__ float sm[];
-    float* zs = sm;                         // [NRHS][nb] solved values
-    float* blk = sm + NRHS * nb;            // [32][33] diagonal block
-    float* part = blk + 32 * 33;            // [8][32][NRHS] partial sums (backward) / [32][NRHS] (forward)
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int nblk = nb / 32;
-    for (int bi = 0; bi < nblk; ++bi) {
-        const int b = backward ? (nblk - 1 - bi) : bi;
-        const int r0 = b * 32;
-        // diagonal 32x32 block into smem
-        for (int idx = threadIdx.x; idx < 32 * 32; idx += 256) {
-            const int r = idx >> 5, c = idx & 31;
-            blk[r * 33 + c] = Lkk[static_cast<int64_t>(r0 + r) * nb + r0 + c];
+        for (int u = 0; u < 4; ++u) {
+            const int64_t e = static_cast<int64_t>(r + u * NW) * nb + c0;
+            if (CPL == 4) {
+                const float4 v = load4(tile, p, s, e);
+                l[u][0] = v.x; l[u][1] = v.y; l[u][CPL - 2] = v.z; l[u][CPL - 1] = v.w;
+            } else {
+                const float2 v = load2(tile, p, s, e);
+                l[u][0] = v.x; l[u][1] = v.y;
+            }
         }
-        if (!backward) {
-            // part[r][h] = sum_{l < r0} L[r0+r][l] z[l][h] ; warp w handles rows 4w..4w+3
-            for (int rr = 0; rr < 4; ++rr) {
-                const int r = warp * 4 + rr;
-                float acc[NRHS];
 #pragma unroll
-                for (int h = 0; h < NRHS; ++h) acc[h] = 0.0f;
-                const float* lrow = Lkk + static_cast<int64_t>(r0 + r) * nb;
-                for (int l = lane; l < r0; l += 32) {
-                    const float lv = lrow[l];
+        for (int u = 0; u < 4; ++u) {
+            const float* ar = as + static_cast<size_t>(r + u * NW) * NRHS;
 #pragma unroll
-                    for (int h = 0; h < NRHS; ++h) acc[h] = fmaf(lv, zs[h * nb + l], acc[h]);
+            for (int h = 0; h < NRHS; h += 4) {
+                const float4 a = *reinterpret_cast<const float4*>(ar + h);
+#pragma unroll
+                for (int c = 0; c < CPL; ++c) {
+                    acc[c * NRHS + h + 0] = fmaf(l[u][c], a.x, acc[c * NRHS + h + 0]);
+                    acc[c * NRHS + h + 1] = fmaf(l[u][c], a.y, acc[c * NRHS + h + 1]);
+                    acc[c * NRHS + h + 2] = fmaf(l[u][c], a.z, acc[c * NRHS + h + 2]);
+                    acc[c * NRHS + h + 3] = fmaf(l[u][c], a.w, acc[c * NRHS + h + 3]);
                 }
-#pragma unroll
-                for (int h = 0; h < NRHS; ++h) {
-#pragma unroll
-                    for (int o = 16; o > 0; o >>= 1) acc[h] += __shfl_xor_sync(0xffffffffu, acc[h], o);
-                }
-#pragma unroll
-                for (int h = 0; h < NRHS; ++h)
-                    if (lane == h) part[r * NRHS + h] = acc[h];
             }
-        } else {
-            // part[w][c][h] = sum over rows r > block, r = r1 + w, r1 + w + 8, ... of L[r][r0+c] a[r][h]
-            float acc[NRHS];
+        }
+    }
+    // fixed-order tree over the NW warps
 #pragma unroll
-            for (int h = 0; h < NRHS; ++h) acc[h] = 0.0f;
-            for (int r = r0 + 32 + warp; r < nb; r += 8) {
-                const float lv = Lkk[static_cast<int64_t>(r) * nb + r0 + lane];
+    for (int half = NW / 2; half >= 1; half >>= 1) {
+        if (warp >= half && warp < 2 * half) {
+            float* dst = red + (static_cast<size_t>(warp - half) * 32 + lane) * NACC;
 #pragma unroll
-                for (int h = 0; h < NRHS; ++h) acc[h] = fmaf(lv, zs[h * nb + r], acc[h]);
-            }
-#pragma unroll
-            for (int h = 0; h < NRHS; ++h) part[(warp * 32 + lane) * NRHS + h] = acc[h];
+            for (int v = 0; v < NACC; v += 4) *reinterpret_cast<float4*>(dst + v) = make_float4(acc[v], acc[v + 1], acc[v + 2], acc[v + 3]);
         }
         __syncthreads();
-        if (warp == 0) {
-            const int h = lane;                   // this lane's right-hand side
-            if (h < nrhs) {
-                float v[32];
-                if (!backward) {
+        if (warp < half) {
+            const float* src = red + (static_cast<size_t>(warp) * 32 + lane) * NACC;
 #pragma unroll
-                    for (int r = 0; r < 32; ++r) v[r] = Bk[static_cast<int64_t>(r0 + r) * ldb + h] - part[r * NRHS + h];
+            for (int v = 0; v < NACC; v += 4) {
+                const float4 t = *reinterpret_cast<const float4*>(src + v);
+                acc[v] += t.x; acc[v + 1] += t.y; acc[v + 2] += t.z; acc[v + 3] += t.w;
+            }
+        }
+        __syncthreads();
+    }
+    if (warp == 0) {
 #pragma unroll
-                    for (int r = 0; r < 32; ++r) {
-                        float sacc = v[r];
+        for (int c = 0; c < CPL; ++c) {
+            float* z = B + (static_cast<int64_t>(j) * nb + c0 + c) * ldb;
 #pragma unroll
-                        for (int l = 0; l < r; ++l) sacc = fmaf(-blk[r * 33 + l], v[l], sacc);
-                        v[r] = sacc / blk[r * 33 + r];
+            for (int h = 0; h < NRHS; ++h)
+                if (h < nrhs) z[h] -= acc[c * NRHS + h];
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Diagonal tile solve, one CTA: forward (L z = y) or backward (L^T a = z), in place on rows
+// k*nb .. (k+1)*nb of B.  For each 128-row block c (in order):
+//   forward   t = y_c - L[c, 0:c] z_{0:c}                       z_c = inv(L_cc) t
+//   backward  t = z_c - L[c+1:, c]^T a_{c+1:}                   a_c = inv(L_cc)^T t
+// dinv / dinvT: the inverted diagonal blocks of this tile and their transposes ([nsub][128][128]).
+// smem: solved values [NRHS][nb] (forward, by rhs) or [nb][NRHS] (backward, by row) + t [NRHS][128]
+//       + (backward) reduction buffers (NW/2) * 32 * NACC floats.
+template <int NRHS>
+__global__ void __launch_bounds__(kDiagThreads, 1)
+potrs_diag_kernel(int nb, const float* __restrict__ Lkk, const float* __restrict__ dinv,
+                  const float* __restrict__ dinvT, float* __restrict__ Bk, int64_t ldb, int nrhs, int backward) {
+    constexpr int ROWS = 64 / NRHS;
+    constexpr int NW = kDiagThreads / 32;
+    constexpr int CPL = (NRHS <= 16) ? 4 : 2;          // backward: columns per lane
+    constexpr int NACC = CPL * NRHS;
+    constexpr int PASSES = 4 / CPL;                    // 128 columns = PASSES * 32 * CPL
+    extern __shared__ __align__(16) float sm[];
+    float* zs = sm;                                    // forward:  [NRHS][nb] solved values, by rhs
+    float* sr = sm;                                    // backward: [nb][NRHS] solved values, by row
+    float* ts = sm + static_cast<size_t>(NRHS) * nb;   // [NRHS][128]
+    float* red = ts + NRHS * kBlk;                     // backward: [NW/2][32][NACC]
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int nsub = nb / kBlk;
+    for (int bi = 0; bi < nsub; ++bi) {
+        const int c = backward ? (nsub - 1 - bi) : bi;
+        const int R0 = c * kBlk;
+        // ---- phase 1: t = rhs_c - (off-diagonal part of the tile) * (solved part)
+        if (!backward) {
+            for (int g = warp; g < kBlk / ROWS; g += NW) {
+                float acc[64];
+#pragma unroll
+                for (int v = 0; v < 64; ++v) acc[v] = 0.0f;
+                const int r = R0 + g * ROWS;
+                rows_dot_f32<NRHS>(Lkk + static_cast<int64_t>(r) * nb, nb, R0, zs, nb, lane, acc);
+                warp_reduce64(acc, lane);
+                const int v0 = warp_reduce64_index(lane);
+#pragma unroll
+                for (int t = 0; t < 2; ++t) {
+                    const int u = (v0 + t) / NRHS, h = (v0 + t) % NRHS;
+                    const float y = (h < nrhs) ? Bk[static_cast<int64_t>(r + u) * ldb + h] : 0.0f;
+                    ts[h * kBlk + g * ROWS + u] = y - acc[t];
+                }
+            }
+        } else {
+            for (int pass = 0; pass < PASSES; ++pass) {
+                const int c0 = R0 + pass * 32 * CPL + lane * CPL;
+                float acc[NACC];
+#pragma unroll
+                for (int v = 0; v < NACC; ++v) acc[v] = 0.0f;
+                for (int r = R0 + kBlk + warp; r < nb; r += NW * 4) {
+                    float l[4][CPL];
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        const int rr = r + u * NW;
+                        if (rr < nb) {
+                            if (CPL == 4) {
+                                const float4 v = __ldg(reinterpret_cast<const float4*>(Lkk + static_cast<int64_t>(rr) * nb + c0));
+                                l[u][0] = v.x; l[u][1] = v.y; l[u][CPL - 2] = v.z; l[u][CPL - 1] = v.w;
+                            } else {
+                                const float2 v = __ldg(reinterpret_cast<const float2*>(Lkk + static_cast<int64_t>(rr) * nb + c0));
+                                l[u][0] = v.x; l[u][1] = v.y;
+                            }
+                        } else {
+#pragma unroll
+                            for (int q = 0; q < CPL; ++q) l[u][q] = 0.0f;
+                        }
                     }
-                } else {
 #pragma unroll
-                    for (int r = 0; r < 32; ++r) {
-                        float sacc = 0.0f;
-                        for (int w = 0; w < 8; ++w) sacc += part[(w * 32 + r) * NRHS + h];
-                        v[r] = Bk[static_cast<int64_t>(r0 + r) * ldb + h] - sacc;
-                    }
+                    for (int u = 0; u < 4; ++u) {
+                        const int rr = (r + u * NW < nb) ? r + u * NW : nb - 1;     // l is zero there
+                        const float* ar = sr + static_cast<size_t>(rr) * NRHS;
 #pragma unroll
-                    for (int r = 31; r >= 0; --r) {
-                        float sacc = v[r];
+                        for (int h = 0; h < NRHS; h += 4) {
+                            const float4 a = *reinterpret_cast<const float4*>(ar + h);
 #pragma unroll
-                        for (int l = r + 1; l < 32; ++l) sacc = fmaf(-blk[l * 33 + r], v[l], sacc);
-                        v[r] = sacc / blk[r * 33 + r];
+                            for (int q = 0; q < CPL; ++q) {
+                                acc[q * NRHS + h + 0] = fmaf(l[u][q], a.x, acc[q * NRHS + h + 0]);
+                                acc[q * NRHS + h + 1] = fmaf(l[u][q], a.y, acc[q * NRHS + h + 1]);
+                                acc[q * NRHS + h + 2] = fmaf(l[u][q], a.z, acc[q * NRHS + h + 2]);
+                                acc[q * NRHS + h + 3] = fmaf(l[u][q], a.w, acc[q * NRHS + h + 3]);
+                            }
+                        }
                     }
                 }
 #pragma unroll
-                for (int r = 0; r < 32; ++r) {
-                    zs[h * nb + r0 + r] = v[r];
-                    Bk[static_cast<int64_t>(r0 + r) * ldb + h] = v[r];
+                for (int half = NW / 2; half >= 1; half >>= 1) {
+                    if (warp >= half && warp < 2 * half) {
+                        float* dst = red + (static_cast<size_t>(warp - half) * 32 + lane) * NACC;
+#pragma unroll
+                        for (int v = 0; v < NACC; v += 4) *reinterpret_cast<float4*>(dst + v) = make_float4(acc[v], acc[v + 1], acc[v + 2], acc[v + 3]);
+                    }
+                    __syncthreads();
+                    if (warp < half) {
+                        const float* src = red + (static_cast<size_t>(warp) * 32 + lane) * NACC;
+#pragma unroll
+                        for (int v = 0; v < NACC; v += 4) {
+                            const float4 t = *reinterpret_cast<const float4*>(src + v);
+                            acc[v] += t.x; acc[v + 1] += t.y; acc[v + 2] += t.z; acc[v + 3] += t.w;
+                        }
+                    }
+                    __syncthreads();
                 }
+                if (warp == 0) {
+#pragma unroll
+                    for (int q = 0; q < CPL; ++q)
+#pragma unroll
+                        for (int h = 0; h < NRHS; ++h) {
+                            const int col = c0 - R0 + q;
+                            const float y = (h < nrhs) ? Bk[static_cast<int64_t>(c0 + q) * ldb + h] : 0.0f;
+                            ts[h * kBlk + col] = y - acc[q * NRHS + h];
+                        }
+                }
+            }
+        }
+        __syncthreads();
+        // ---- phase 2: solved_c = inv(L_cc) t   (forward)   or   inv(L_cc)^T t   (backward)
+        const float* D = (backward ? dinvT : dinv) + static_cast<int64_t>(c) * kBlk * kBlk;
+        for (int g = warp; g < kBlk / ROWS; g += NW) {
+            float acc[64];
+#pragma unroll
+            for (int v = 0; v < 64; ++v) acc[v] = 0.0f;
+            rows_dot_f32<NRHS>(D + static_cast<int64_t>(g * ROWS) * kBlk, kBlk, kBlk, ts, kBlk, lane, acc);
+            warp_reduce64(acc, lane);
+            const int v0 = warp_reduce64_index(lane);
+#pragma unroll
+            for (int t = 0; t < 2; ++t) {
+                const int u = (v0 + t) / NRHS, h = (v0 + t) % NRHS;
+                const int r = R0 + g * ROWS + u;
+                if (backward) sr[static_cast<size_t>(r) * NRHS + h] = acc[t];
+                else zs[h * nb + r] = acc[t];
+                if (h < nrhs) Bk[static_cast<int64_t>(r) * ldb + h] = acc[t];
             }
         }
         __syncthreads();

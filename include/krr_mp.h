@@ -54,6 +54,11 @@ typedef enum { KRR_FP32 = 0, KRR_FP16 = 1, KRR_FP8_E4M3 = 2 } krr_prec_t;
                                        contiguous row-major nb x nb block at element offset
                                        krr_tile_slot(NT,i,j) * nb * nb; lda is ignored.             */
 
+#define KRR_FLAG_NO_LOOKAHEAD    8u  /* krr_potrf_mp: run the tile columns strictly one after the other on
+                                       the caller's stream (no internal streams; per-kernel timing and
+                                       debugging).  Default: column k+1's update of the already final
+                                       columns overlaps the factorisation of column k (lookahead 1).  */
+
 /* Library version (major*100 + minor) and the compute capability it was built for (100). */
 int krr_version(void);
 int krr_built_for_sm(void);

@@ -8,6 +8,7 @@ import torch
 FP32, FP16, FP8 = 0, 1, 2
 FLAG_PREROUND_A = 1
 FLAG_A_TILED_LOWER = 4
+FLAG_NO_LOOKAHEAD = 8
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB = None

@@ -98,7 +98,7 @@ static size_t host_offsets(int NT, int nb, const uint8_t* h_map, std::vector<int
 
 // ---- workspace layout of krr_potrf_mp ----------------------------------------------------------
 struct PotrfWs {
-    size_t off_table, a_amax, tile_amax, scl, W, linv_hi, linv_lo, Hp, Lp, Qp, total;
+    size_t off_table, a_amax, tile_amax, scl, W, W2, linv_hi, linv_lo, Hp, Lp, Qp, total;
 };
 static PotrfWs potrf_ws_layout(int64_t n, int nb, bool any_fp8) {
     const int64_t NT = n / nb;
@@ -111,6 +111,7 @@ static PotrfWs potrf_ws_layout(int64_t n, int nb, bool any_fp8) {
     w.tile_amax = o; o = align_up(o + nslots * sizeof(float), 1024);
     w.scl = o;       o = align_up(o + (4 + nb / kBlk) * sizeof(float), 1024);
     w.W = o;         o = align_up(o + static_cast<size_t>(n) * nb * sizeof(float), 1024);
+    w.W2 = o;        o = align_up(o + static_cast<size_t>(n) * nb * sizeof(float), 1024);   // lookahead: column k+1's partial
     w.linv_hi = o;   o = align_up(o + static_cast<size_t>(nb) * kBlk * 2, 1024);
     w.linv_lo = o;   o = align_up(o + static_cast<size_t>(nb) * kBlk * 2, 1024);
     w.Hp = o;        o = align_up(o + plane * 2, 1024);
@@ -142,6 +143,31 @@ struct ProfScope {
     ~ProfScope() { if (on) { cudaEventRecord(t.e1, st); g_prof.push_back(t); } }
 };
 
+// ---- internal streams of the tile-column pipeline (lookahead): created once per host thread ----
+// `hi` carries the critical path (diagonal-tile chain, panel, store), `lo` the bulk updates that run
+// ahead; both are fenced by events against the caller's stream, which is never blocked on the host.
+struct Pipeline {
+    cudaStream_t hi = nullptr, lo = nullptr;
+    std::vector<cudaEvent_t> ev;
+    cudaEvent_t event(size_t i) {
+        while (ev.size() <= i) {
+            cudaEvent_t e = nullptr;
+            cudaEventCreateWithFlags(&e, cudaEventDisableTiming);
+            ev.push_back(e);
+        }
+        return ev[i];
+    }
+    int init() {
+        if (hi) return KRR_OK;
+        int least = 0, greatest = 0;
+        KRR_CUDA_CHECK(cudaDeviceGetStreamPriorityRange(&least, &greatest));
+        KRR_CUDA_CHECK(cudaStreamCreateWithPriority(&hi, cudaStreamNonBlocking, greatest));
+        KRR_CUDA_CHECK(cudaStreamCreateWithPriority(&lo, cudaStreamNonBlocking, least));
+        return KRR_OK;
+    }
+};
+static thread_local Pipeline g_pipe;
+
 template <typename K, typename... Args>
 static int launch(int cat, K kernel, dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args... args) {
     ProfScope ps(cat, st);
@@ -151,10 +177,10 @@ static int launch(int cat, K kernel, dim3 grid, dim3 block, size_t smem, cudaStr
 }
 
 static int launch_gemm(const CUtensorMap& a_hi, const CUtensorMap& a_lo, const CUtensorMap& b_hi,
-                       const CUtensorMap& b_lo, const GemmOp& op, int num_sms, cudaStream_t st) {
+                       const CUtensorMap& b_lo, const GemmOp& op, int max_ctas, cudaStream_t st) {
     const int ntiles = op.nrb * op.ncb;
     if (ntiles <= 0) return KRR_OK;
-    const int grid = ntiles < num_sms ? ntiles : num_sms;
+    const int grid = ntiles < max_ctas ? ntiles : max_ctas;
     ProfScope ps(op.mode == MODE_UPDATE ? CAT_UPDATE : (op.mode == MODE_P1 ? CAT_P1 : CAT_P3), st);
     gemm_tc_kernel<<<grid, kGemmThreads, kGemmSmem, st>>>(a_hi, a_lo, b_hi, b_lo, op);
     ++g_launches;
@@ -295,7 +321,7 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
     if (reinterpret_cast<uintptr_t>(d_A) % 16 != 0 || reinterpret_cast<uintptr_t>(d_ws) % 1024 != 0 ||
         reinterpret_cast<uintptr_t>(d_factor) % 128 != 0)
         return KRR_ERR_ARG;
-    if (flags & ~(KRR_FLAG_PREROUND_A | KRR_FLAG_A_TILED_LOWER)) return KRR_ERR_UNSUPPORTED;
+    if (flags & ~(KRR_FLAG_PREROUND_A | KRR_FLAG_A_TILED_LOWER | KRR_FLAG_NO_LOOKAHEAD)) return KRR_ERR_UNSUPPORTED;
     const int NT = static_cast<int>(n / nb);
     bool any_fp8 = false;
     rc = check_map(NT, h_map, &any_fp8);
@@ -344,39 +370,104 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
         return KRR_ERR_CUDA;
 
     const int nsub = nb / kBlk;
+    const bool lookahead = !(flags & KRR_FLAG_NO_LOOKAHEAD) && NT > 2;
+    float* Wbuf[2] = {W, reinterpret_cast<float*>(ws + L.W2)};
+    cudaStream_t sh = st, sl = st;               // critical-path stream, bulk stream
+    enum { EV_FORK = 0, EV_JOIN_HI = 1, EV_JOIN_LO = 2, EV_BASE = 3 };   // then 3 events per tile column
+    auto ev_fin = [&](int k) { return g_pipe.event(EV_BASE + 3 * static_cast<size_t>(k) + 0); };
+    auto ev_old = [&](int k) { return g_pipe.event(EV_BASE + 3 * static_cast<size_t>(k) + 1); };
+    auto ev_newb = [&](int k) { return g_pipe.event(EV_BASE + 3 * static_cast<size_t>(k) + 2); };
+    if (lookahead) {
+        rc = g_pipe.init();
+        if (rc) return rc;
+        sh = g_pipe.hi; sl = g_pipe.lo;
+        KRR_CUDA_CHECK(cudaEventRecord(g_pipe.event(EV_FORK), st));
+        KRR_CUDA_CHECK(cudaStreamWaitEvent(sh, g_pipe.event(EV_FORK), 0));
+        KRR_CUDA_CHECK(cudaStreamWaitEvent(sl, g_pipe.event(EV_FORK), 0));
+    }
+    // bulk kernels leave nsub SMs to the diagonal-tile chain they overlap with
+    const int bulk_ctas = lookahead ? (num_sms - nsub > nsub ? num_sms - nsub : num_sms) : num_sms;
+
     for (int k = 0; k < NT; ++k) {
         const int mblk = (NT - k) * nsub;             // 128-row blocks of the panel
+        float* Wk = Wbuf[k & 1];
         GemmOp op;
         memset(&op, 0, sizeof(op));
         op.nb = nb; op.NT = NT; op.k = k;
         op.prow0 = tile_slot(NT, k, k) * nb;
         op.map = d_map; op.A = A; op.a_amax = (preround && any_fp8) ? a_amax : nullptr;
-        op.W = W; op.Hp = Hp; op.Lp = Lp; op.tile_amax = tile_amax; op.flags = flags;
+        op.W = Wk; op.Hp = Hp; op.Lp = Lp; op.tile_amax = tile_amax; op.flags = flags;
         op.scl = scl; op.linv_scale = linv_scale;
-        // U(k): S = rd(A) - L[:, 0:k] L[k, 0:k]^T over the whole tile column
-        op.mode = MODE_UPDATE; op.c = 0; op.rb0 = 0; op.nrb = mblk; op.cb0 = 0; op.ncb = nsub;
-        rc = launch_gemm(tmH, tmL, tmH, tmL, op, num_sms, st);
-        if (rc) return rc;
-        for (int c = 0; c < nsub; ++c) {
-            if (c > 0) {
-                op.mode = MODE_P1; op.c = c; op.rb0 = c; op.nrb = mblk - c; op.cb0 = c; op.ncb = 1;
-                rc = launch_gemm(tmH, tmL, tmH, tmL, op, num_sms, st);
-                if (rc) return rc;
-            }
-            rc = launch(CAT_POTRF, potrf128_kernel, dim3(1), dim3(kTriThreads), static_cast<size_t>(kTriSmem), st, W, nb,
-                        c * kBlk, c * kBlk, linv_hi, linv_lo, linv_scale, d_info,
-                        static_cast<int64_t>(k) * nb + static_cast<int64_t>(c) * kBlk + 1);
+        // ---- U(k): S = rd(A) - L[:, 0:k] L[k, 0:k]^T over the tile column (SYRK + GEMM) ----
+        op.mode = MODE_UPDATE; op.c = 0; op.cb0 = 0; op.ncb = nsub;
+        if (!lookahead) {
+            op.s_lo = 0; op.s_hi = k; op.base_w = 0; op.planes = 1; op.rb0 = 0; op.nrb = mblk;
+            rc = launch_gemm(tmH, tmL, tmH, tmL, op, num_sms, st);
             if (rc) return rc;
-            if (mblk - c - 1 > 0) {
-                op.mode = MODE_P3; op.c = c; op.rb0 = c + 1; op.nrb = mblk - c - 1; op.cb0 = c; op.ncb = 1;
-                rc = launch_gemm(tmH, tmL, tmIH, tmIL, op, num_sms, st);
+        } else {
+            // terms s < k-1 were accumulated into Wk by U_old(k) while column k-1 was being factorised;
+            // the newest term s = k-1 is added here, the diagonal tile first (it starts the chain)
+            const bool have_old = (k >= 2);
+            op.s_lo = (k >= 1) ? k - 1 : 0; op.s_hi = k; op.base_w = have_old ? 1 : 0; op.planes = 1;
+            if (have_old) KRR_CUDA_CHECK(cudaStreamWaitEvent(sh, ev_old(k), 0));
+            op.rb0 = 0; op.nrb = nsub;
+            rc = launch_gemm(tmH, tmL, tmH, tmL, op, num_sms, sh);
+            if (rc) return rc;
+            if (k >= 1) KRR_CUDA_CHECK(cudaStreamWaitEvent(sl, ev_fin(k - 1), 0));
+            op.rb0 = nsub; op.nrb = mblk - nsub;
+            rc = launch_gemm(tmH, tmL, tmH, tmL, op, bulk_ctas, sl);
+            if (rc) return rc;
+            KRR_CUDA_CHECK(cudaEventRecord(ev_newb(k), sl));
+            if (k + 1 < NT && k >= 1) {
+                // U_old(k+1): terms s < k of column k+1, overlapping the factorisation of column k
+                GemmOp on = op;
+                on.k = k + 1; on.prow0 = tile_slot(NT, k + 1, k + 1) * nb; on.W = Wbuf[(k + 1) & 1];
+                on.s_lo = 0; on.s_hi = k; on.base_w = 0; on.planes = 0;
+                on.rb0 = 0; on.nrb = (NT - k - 1) * nsub;
+                rc = launch_gemm(tmH, tmL, tmH, tmL, on, bulk_ctas, sl);
                 if (rc) return rc;
+                KRR_CUDA_CHECK(cudaEventRecord(ev_old(k + 1), sl));
             }
         }
-        rc = launch(CAT_FINALIZE, finalize_kernel, dim3(nb / 16, NT - k), dim3(256), 0, st, NT, nb, k, static_cast<const float*>(W),
+        // ---- panel: 128-wide sub-columns; the diagonal tile's rows first (critical path) ----
+        for (int part = 0; part < (lookahead ? 2 : 1); ++part) {
+            // part 0: rows of the diagonal tile (or all rows without lookahead); part 1: rows below
+            const int row_lo = (part == 0) ? 0 : nsub;
+            const int row_hi = (lookahead && part == 0) ? nsub : mblk;
+            if (part == 1) KRR_CUDA_CHECK(cudaStreamWaitEvent(sh, ev_newb(k), 0));
+            if (row_hi <= row_lo) continue;
+            for (int c = 0; c < nsub; ++c) {
+                if (c > 0) {
+                    op.mode = MODE_P1; op.c = c; op.cb0 = c; op.ncb = 1;
+                    op.rb0 = (part == 0) ? c : row_lo; op.nrb = row_hi - op.rb0;
+                    rc = launch_gemm(tmH, tmL, tmH, tmL, op, num_sms, sh);
+                    if (rc) return rc;
+                }
+                if (part == 0) {
+                    rc = launch(CAT_POTRF, potrf128_kernel, dim3(1), dim3(kTriThreads), static_cast<size_t>(kTriSmem), sh, Wk, nb,
+                                c * kBlk, c * kBlk, linv_hi, linv_lo, linv_scale, d_info,
+                                static_cast<int64_t>(k) * nb + static_cast<int64_t>(c) * kBlk + 1);
+                    if (rc) return rc;
+                }
+                op.mode = MODE_P3; op.c = c; op.cb0 = c; op.ncb = 1;
+                op.rb0 = (part == 0) ? c + 1 : row_lo; op.nrb = row_hi - op.rb0;
+                if (op.nrb > 0) {
+                    rc = launch_gemm(tmH, tmL, tmIH, tmIL, op, num_sms, sh);
+                    if (rc) return rc;
+                }
+            }
+        }
+        rc = launch(CAT_FINALIZE, finalize_kernel, dim3(nb / 16, NT - k), dim3(256), 0, sh, NT, nb, k, static_cast<const float*>(Wk),
                     d_map, static_cast<const int64_t*>(off), static_cast<const float*>(tile_amax),
                     static_cast<uint8_t*>(d_factor), d_scales, Hp, Qp, static_cast<const float*>(scl));
         if (rc) return rc;
+        if (lookahead) KRR_CUDA_CHECK(cudaEventRecord(ev_fin(k), sh));
+    }
+    if (lookahead) {
+        KRR_CUDA_CHECK(cudaEventRecord(g_pipe.event(EV_JOIN_HI), sh));
+        KRR_CUDA_CHECK(cudaEventRecord(g_pipe.event(EV_JOIN_LO), sl));
+        KRR_CUDA_CHECK(cudaStreamWaitEvent(st, g_pipe.event(EV_JOIN_HI), 0));
+        KRR_CUDA_CHECK(cudaStreamWaitEvent(st, g_pipe.event(EV_JOIN_LO), 0));
     }
     return KRR_OK;
 }
@@ -410,8 +501,7 @@ static int potrs_run(const uint8_t* factor, const float* d_scales, const uint8_t
                      int nrhs, int num_sms, cudaStream_t st) {
     constexpr int ROWS = 64 / NRHS, NW = kSolveThreads / 32, CPL = (NRHS <= 16) ? 4 : 2;
     const size_t smem_z = static_cast<size_t>(NRHS) * nb * sizeof(float);
-    const size_t smem_fd = smem_z + NRHS * kBlk * sizeof(float);
-    const size_t smem_bd = smem_fd + static_cast<size_t>(kDiagThreads / 64) * 32 * CPL * NRHS * sizeof(float);
+    const size_t smem_d = static_cast<size_t>(potrs_diag_smem_floats<NRHS>(nb)) * sizeof(float);
     const size_t smem_bu = smem_z + static_cast<size_t>(NW / 2) * 32 * CPL * NRHS * sizeof(float);
     const int64_t blk_elems = static_cast<int64_t>(kBlk) * kBlk;
     const int nsub = nb / kBlk;
@@ -419,7 +509,7 @@ static int potrs_run(const uint8_t* factor, const float* d_scales, const uint8_t
     for (int k = 0; k < NT; ++k) {
         const float* Lkk = reinterpret_cast<const float*>(factor + hoff[static_cast<size_t>(k) * NT + k]);
         float* Bk = B + static_cast<int64_t>(k) * nb * ldb;
-        rc = launch(CAT_POTRS, potrs_diag_kernel<NRHS>, dim3(1), dim3(kDiagThreads), smem_fd, st, nb, Lkk,
+        rc = launch(CAT_POTRS, potrs_diag_kernel<NRHS>, dim3(kDiagCluster), dim3(kDiagThreads), smem_d, st, nb, Lkk,
                     dinv + k * nsub * blk_elems, dinvT + k * nsub * blk_elems, Bk, ldb, nrhs, 0);
         if (rc) return rc;
         if (k + 1 < NT) {
@@ -434,7 +524,7 @@ static int potrs_run(const uint8_t* factor, const float* d_scales, const uint8_t
     for (int k = NT - 1; k >= 0; --k) {
         const float* Lkk = reinterpret_cast<const float*>(factor + hoff[static_cast<size_t>(k) * NT + k]);
         float* Bk = B + static_cast<int64_t>(k) * nb * ldb;
-        rc = launch(CAT_POTRS, potrs_diag_kernel<NRHS>, dim3(1), dim3(kDiagThreads), smem_bd, st, nb, Lkk,
+        rc = launch(CAT_POTRS, potrs_diag_kernel<NRHS>, dim3(kDiagCluster), dim3(kDiagThreads), smem_d, st, nb, Lkk,
                     dinv + k * nsub * blk_elems, dinvT + k * nsub * blk_elems, Bk, ldb, nrhs, 1);
         if (rc) return rc;
         if (k > 0) {

@@ -33,6 +33,10 @@ enum { MODE_UPDATE = 0, MODE_P1 = 1, MODE_P3 = 2 };
 struct GemmOp {
     int mode;
     int nb, NT, k;        // tile size, tiles per dimension, tile column being produced
+    int s_lo, s_hi;       // MODE_UPDATE: tile columns s in [s_lo, s_hi) are accumulated (lookahead splits
+                          // the sum into the part known early and the newest column)
+    int base_w;           // MODE_UPDATE: 0 = start from rd_p(A), 1 = continue the FP32 partial sum in W
+    int planes;           // MODE_UPDATE: 1 = also write the FP16 hi/lo images of the result (final pass)
     int c;                // 128-wide sub-column inside the tile column (P1 / P3)
     int rb0, nrb;         // output row blocks (128 rows, panel-local: row 0 = top of tile (k,k))
     int cb0, ncb;         // output column blocks (128 columns inside the tile column)
@@ -66,11 +70,12 @@ struct TermInfo {
     int nA, nB;             // planes per operand: 2 = hi+lo (FP32 class), 1 = hi only
 };
 
-__device__ __forceinline__ TermInfo get_term(const GemmOp& op, int s, int rb, int cb) {
+__device__ __forceinline__ TermInfo get_term(const GemmOp& op, int s /* term index */, int rb, int cb) {
     TermInfo t;
     if (op.mode == MODE_UPDATE) {
         const int i = op.k + (rb * kBlk) / op.nb;
         const int subrow = (rb * kBlk) % op.nb;
+        s += op.s_lo;
         t.a_row = tile_slot(op.NT, i, s) * op.nb + subrow;
         t.b_row = tile_slot(op.NT, op.k, s) * op.nb + cb * kBlk;
         t.a_k0 = 0;
@@ -99,7 +104,7 @@ __device__ __forceinline__ TermInfo get_term(const GemmOp& op, int s, int rb, in
 }
 
 __device__ __forceinline__ int num_terms(const GemmOp& op) {
-    return op.mode == MODE_UPDATE ? op.k : 1;
+    return op.mode == MODE_UPDATE ? (op.s_hi - op.s_lo) : 1;
 }
 
 // Tiles of the diagonal tile that lie entirely above the diagonal are never read: skip them.
@@ -126,7 +131,8 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_constant
     const int lane = threadIdx.x & 31;
     const int ntiles = op.nrb * op.ncb;
     const int nterms = num_terms(op);
-    const bool has_acc = (op.mode != MODE_UPDATE) ? (op.mode == MODE_P3 || op.c > 0) : (op.k > 0);
+    const bool has_acc = (op.mode != MODE_UPDATE) ? (op.mode == MODE_P3 || op.c > 0) : (nterms > 0);
+    const bool write_planes = (op.mode != MODE_UPDATE) || op.planes;
 
     if (warp == 0 && lane == 0) {
         ptx::prefetch_tmap(&tmA_hi);
@@ -242,10 +248,14 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_constant
             if (op.mode == MODE_UPDATE) {
                 const int i = op.k + (rb * kBlk) / op.nb;
                 const int subrow = (rb * kBlk) % op.nb;
-                base = op.A.tile_ptr(i, op.k, subrow + row_in_blk, col0);
-                if ((op.flags & KRR_FLAG_PREROUND_A) && i != op.k) {
-                    p = op.map[i * op.NT + op.k];
-                    if (p == KRR_FP8_E4M3) sc = fp8_scale_from_amax(op.a_amax[i * op.NT + op.k]);
+                if (op.base_w) {
+                    base = op.W + r * op.nb + col0;
+                } else {
+                    base = op.A.tile_ptr(i, op.k, subrow + row_in_blk, col0);
+                    if ((op.flags & KRR_FLAG_PREROUND_A) && i != op.k) {
+                        p = op.map[i * op.NT + op.k];
+                        if (p == KRR_FP8_E4M3) sc = fp8_scale_from_amax(op.a_amax[i * op.NT + op.k]);
+                    }
                 }
             } else if (op.mode == MODE_P1) {
                 base = op.W + r * op.nb + col0;
@@ -288,6 +298,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_constant
 #pragma unroll
                 for (int e = 0; e < 32; e += 4)
                     *reinterpret_cast<float4*>(wout + j * 32 + e) = make_float4(out[e], out[e + 1], out[e + 2], out[e + 3]);
+                if (write_planes) {
 #pragma unroll
                 for (int e = 0; e < 32; e += 8) {
                     __align__(16) __half hi[8];
@@ -301,6 +312,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_constant
                     }
                     *reinterpret_cast<uint4*>(hout + j * 32 + e) = *reinterpret_cast<const uint4*>(hi);
                     *reinterpret_cast<uint4*>(lout + j * 32 + e) = *reinterpret_cast<const uint4*>(lo);
+                }
                 }
             }
             if (has_acc) {

@@ -13,13 +13,16 @@
 //   potrs_bwd_update_kernel        Z_j -= L_kj^T alpha_k for all j < k (streams tile row k once)
 // All sums are accumulated in a fixed order: results are deterministic.
 #pragma once
+#include <cooperative_groups.h>
+
 #include "common.cuh"
 
 namespace krr {
 
 constexpr int kMaxRhs = 32;
 constexpr int kSolveThreads = 256;          // update kernels
-constexpr int kDiagThreads = 512;           // diagonal-tile kernel
+constexpr int kDiagThreads = 256;           // diagonal-tile kernel: CTAs of 8 warps ...
+constexpr int kDiagCluster = 8;             // ... in a cluster of 8
 
 // Dequantising loads of CPL (4 or 2) consecutive elements of a mosaic tile (element index e).
 __device__ __forceinline__ float4 load4(const uint8_t* tile, int p, float s, int64_t e) {
@@ -233,90 +236,153 @@ potrs_bwd_update_kernel(int NT, int nb, int k, const uint8_t* __restrict__ facto
 }
 
 // ---------------------------------------------------------------------------------------------
-// Diagonal tile solve, one CTA: forward (L z = y) or backward (L^T a = z), in place on rows
-// k*nb .. (k+1)*nb of B.  For each 128-row block c (in order):
+// Diagonal tile solve by one thread-block cluster of kDiagCluster CTAs: forward (L z = y) or
+// backward (L^T a = z), in place on rows k*nb .. (k+1)*nb of B.  For each 128-row block c, in order:
 //   forward   t = y_c - L[c, 0:c] z_{0:c}                       z_c = inv(L_cc) t
 //   backward  t = z_c - L[c+1:, c]^T a_{c+1:}                   a_c = inv(L_cc)^T t
 // dinv / dinvT: the inverted diagonal blocks of this tile and their transposes ([nsub][128][128]).
-// smem: solved values [NRHS][nb] (forward, by rhs) or [nb][NRHS] (backward, by row) + t [NRHS][128]
-//       + (backward) reduction buffers (NW/2) * 32 * NACC floats.
+// Every CTA keeps a full copy of the solved values and of t in its shared memory; the rows (forward)
+// or the summation range (backward) of a step are split over the CTAs, and the pieces are exchanged
+// through distributed shared memory between two cluster barriers.
+// smem per CTA: solved values NRHS*nb floats + t NRHS*128 + exchange buffers (see potrs_diag_smem).
 template <int NRHS>
-__global__ void __launch_bounds__(kDiagThreads, 1)
+__host__ __device__ constexpr int potrs_diag_smem_floats(int nb) {
+    // solved + ts + red (max of forward slices: 8 warps * 64 values, backward: 4*32*NACC + part 128*NRHS)
+    return NRHS * nb + NRHS * kBlk + 4 * 32 * 64 + kBlk * NRHS;
+}
+
+template <int NRHS>
+__global__ void __cluster_dims__(kDiagCluster, 1, 1) __launch_bounds__(kDiagThreads, 1)
 potrs_diag_kernel(int nb, const float* __restrict__ Lkk, const float* __restrict__ dinv,
                   const float* __restrict__ dinvT, float* __restrict__ Bk, int64_t ldb, int nrhs, int backward) {
-    constexpr int ROWS = 64 / NRHS;
-    constexpr int NW = kDiagThreads / 32;
+    namespace cg = cooperative_groups;
+    cg::cluster_group cluster = cg::this_cluster();
+    constexpr int ROWS = 64 / NRHS;                    // rows per warp task (forward / phase 2)
+    constexpr int NW = kDiagThreads / 32;              // 8 warps
+    constexpr int GQ = (kBlk / ROWS) / kDiagCluster;   // row groups per CTA: 1, 2, 4, 8 for NRHS 4, 8, 16, 32
+    constexpr int KS = NW / GQ;                        // K slices per row group
     constexpr int CPL = (NRHS <= 16) ? 4 : 2;          // backward: columns per lane
-    constexpr int NACC = CPL * NRHS;
-    constexpr int PASSES = 4 / CPL;                    // 128 columns = PASSES * 32 * CPL
+    constexpr int NACC = CPL * NRHS;                   // 64 except NRHS = 4, 8
+    constexpr int PASSES = 4 / CPL;
+    static_assert(GQ >= 1 && KS >= 1 && GQ * KS == NW, "warp decomposition");
     extern __shared__ __align__(16) float sm[];
     float* zs = sm;                                    // forward:  [NRHS][nb] solved values, by rhs
     float* sr = sm;                                    // backward: [nb][NRHS] solved values, by row
     float* ts = sm + static_cast<size_t>(NRHS) * nb;   // [NRHS][128]
-    float* red = ts + NRHS * kBlk;                     // backward: [NW/2][32][NACC]
+    float* red = ts + NRHS * kBlk;                     // [4][32][64] scratch
+    float* part = red + 4 * 32 * 64;                   // backward: [128][NRHS] this CTA's partial sums
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int q = static_cast<int>(cluster.block_rank());
     const int nsub = nb / kBlk;
+    // pull the tile's lower triangle and the inverted blocks towards L2 (fire and forget)
+    {
+        const int gt = q * kDiagThreads + threadIdx.x, nt = kDiagCluster * kDiagThreads;
+        for (int c = 0; c < nsub; ++c) {
+            const int lines_per_row = 4 * (c + 1);
+            for (int idx = gt; idx < kBlk * lines_per_row; idx += nt) {
+                const float* ptr = Lkk + static_cast<int64_t>(c * kBlk + idx / lines_per_row) * nb + (idx % lines_per_row) * 32;
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(ptr));
+            }
+        }
+        const float* D = backward ? dinvT : dinv;
+        for (int idx = gt; idx < nsub * kBlk * 4; idx += nt) asm volatile("prefetch.global.L2 [%0];" ::"l"(D + idx * 32));
+    }
+    cluster.sync();                                    // every CTA is running before its smem is written remotely
+    const int gl = warp % GQ, ks = warp / GQ;          // this warp's row group inside the CTA, K slice
+    const int grow = (q * GQ + gl) * ROWS;             // first row (inside a 128 block) of the warp's group
     for (int bi = 0; bi < nsub; ++bi) {
         const int c = backward ? (nsub - 1 - bi) : bi;
         const int R0 = c * kBlk;
-        // ---- phase 1: t = rhs_c - (off-diagonal part of the tile) * (solved part)
         if (!backward) {
-            for (int g = warp; g < kBlk / ROWS; g += NW) {
-                float acc[64];
+            // ---- phase 1: t = y_c - L[c, 0:c] z  for this CTA's rows, K split over the warp slices
+            float acc[64];
 #pragma unroll
-                for (int v = 0; v < 64; ++v) acc[v] = 0.0f;
-                const int r = R0 + g * ROWS;
-                rows_dot_f32<NRHS>(Lkk + static_cast<int64_t>(r) * nb, nb, R0, zs, nb, lane, acc);
-                warp_reduce64(acc, lane);
+            for (int v = 0; v < 64; ++v) acc[v] = 0.0f;
+            {
+                const float* rows = Lkk + static_cast<int64_t>(R0 + grow) * nb;
+                for (int l = lane * 4 + ks * 128; l < R0; l += 128 * KS) {
+                    float4 a[ROWS];
+#pragma unroll
+                    for (int u = 0; u < ROWS; ++u) a[u] = __ldg(reinterpret_cast<const float4*>(rows + static_cast<int64_t>(u) * nb + l));
+#pragma unroll
+                    for (int h = 0; h < NRHS; ++h) {
+                        const float4 z = *reinterpret_cast<const float4*>(zs + h * nb + l);
+#pragma unroll
+                        for (int u = 0; u < ROWS; ++u)
+                            acc[u * NRHS + h] = fmaf(a[u].x, z.x, fmaf(a[u].y, z.y, fmaf(a[u].z, z.z, fmaf(a[u].w, z.w, acc[u * NRHS + h]))));
+                    }
+                }
+            }
+            warp_reduce64(acc, lane);
+            if (KS > 1) {
+                if (ks > 0) {
+                    red[((ks - 1) * GQ + gl) * 64 + lane * 2 + 0] = acc[0];
+                    red[((ks - 1) * GQ + gl) * 64 + lane * 2 + 1] = acc[1];
+                }
+                __syncthreads();
+            }
+            if (ks == 0) {
+#pragma unroll
+                for (int s2 = 1; s2 < KS; ++s2) {
+                    acc[0] += red[((s2 - 1) * GQ + gl) * 64 + lane * 2 + 0];
+                    acc[1] += red[((s2 - 1) * GQ + gl) * 64 + lane * 2 + 1];
+                }
                 const int v0 = warp_reduce64_index(lane);
 #pragma unroll
                 for (int t = 0; t < 2; ++t) {
                     const int u = (v0 + t) / NRHS, h = (v0 + t) % NRHS;
-                    const float y = (h < nrhs) ? Bk[static_cast<int64_t>(r + u) * ldb + h] : 0.0f;
-                    ts[h * kBlk + g * ROWS + u] = y - acc[t];
+                    const int r = grow + u;
+                    const float y = (h < nrhs) ? Bk[static_cast<int64_t>(R0 + r) * ldb + h] : 0.0f;
+                    const float tv = y - acc[t];
+#pragma unroll
+                    for (int d = 0; d < kDiagCluster; ++d) cluster.map_shared_rank(ts, d)[h * kBlk + r] = tv;
                 }
             }
+            cluster.sync();
         } else {
+            // ---- phase 1: partial sums of L[c+1:, c]^T a over this CTA's share of the rows
             for (int pass = 0; pass < PASSES; ++pass) {
-                const int c0 = R0 + pass * 32 * CPL + lane * CPL;
+                const int c0 = pass * 32 * CPL + lane * CPL;           // column inside the block
                 float acc[NACC];
 #pragma unroll
                 for (int v = 0; v < NACC; ++v) acc[v] = 0.0f;
-                for (int r = R0 + kBlk + warp; r < nb; r += NW * 4) {
-                    float l[4][CPL];
+                const int gw = q * NW + warp, ngw = kDiagCluster * NW;
+                for (int r = R0 + kBlk + gw; r < nb; r += ngw * 2) {
+                    float l[2][CPL];
 #pragma unroll
-                    for (int u = 0; u < 4; ++u) {
-                        const int rr = r + u * NW;
+                    for (int u = 0; u < 2; ++u) {
+                        const int rr = r + u * ngw;
                         if (rr < nb) {
                             if (CPL == 4) {
-                                const float4 v = __ldg(reinterpret_cast<const float4*>(Lkk + static_cast<int64_t>(rr) * nb + c0));
+                                const float4 v = __ldg(reinterpret_cast<const float4*>(Lkk + static_cast<int64_t>(rr) * nb + R0 + c0));
                                 l[u][0] = v.x; l[u][1] = v.y; l[u][CPL - 2] = v.z; l[u][CPL - 1] = v.w;
                             } else {
-                                const float2 v = __ldg(reinterpret_cast<const float2*>(Lkk + static_cast<int64_t>(rr) * nb + c0));
+                                const float2 v = __ldg(reinterpret_cast<const float2*>(Lkk + static_cast<int64_t>(rr) * nb + R0 + c0));
                                 l[u][0] = v.x; l[u][1] = v.y;
                             }
                         } else {
 #pragma unroll
-                            for (int q = 0; q < CPL; ++q) l[u][q] = 0.0f;
+                            for (int qq = 0; qq < CPL; ++qq) l[u][qq] = 0.0f;
                         }
                     }
 #pragma unroll
-                    for (int u = 0; u < 4; ++u) {
-                        const int rr = (r + u * NW < nb) ? r + u * NW : nb - 1;     // l is zero there
+                    for (int u = 0; u < 2; ++u) {
+                        const int rr = (r + u * ngw < nb) ? r + u * ngw : nb - 1;     // l is zero there
                         const float* ar = sr + static_cast<size_t>(rr) * NRHS;
 #pragma unroll
                         for (int h = 0; h < NRHS; h += 4) {
                             const float4 a = *reinterpret_cast<const float4*>(ar + h);
 #pragma unroll
-                            for (int q = 0; q < CPL; ++q) {
-                                acc[q * NRHS + h + 0] = fmaf(l[u][q], a.x, acc[q * NRHS + h + 0]);
-                                acc[q * NRHS + h + 1] = fmaf(l[u][q], a.y, acc[q * NRHS + h + 1]);
-                                acc[q * NRHS + h + 2] = fmaf(l[u][q], a.z, acc[q * NRHS + h + 2]);
-                                acc[q * NRHS + h + 3] = fmaf(l[u][q], a.w, acc[q * NRHS + h + 3]);
+                            for (int qq = 0; qq < CPL; ++qq) {
+                                acc[qq * NRHS + h + 0] = fmaf(l[u][qq], a.x, acc[qq * NRHS + h + 0]);
+                                acc[qq * NRHS + h + 1] = fmaf(l[u][qq], a.y, acc[qq * NRHS + h + 1]);
+                                acc[qq * NRHS + h + 2] = fmaf(l[u][qq], a.z, acc[qq * NRHS + h + 2]);
+                                acc[qq * NRHS + h + 3] = fmaf(l[u][qq], a.w, acc[qq * NRHS + h + 3]);
                             }
                         }
                     }
                 }
+                // fixed-order tree over the CTA's warps
 #pragma unroll
                 for (int half = NW / 2; half >= 1; half >>= 1) {
                     if (warp >= half && warp < 2 * half) {
@@ -337,36 +403,47 @@ potrs_diag_kernel(int nb, const float* __restrict__ Lkk, const float* __restrict
                 }
                 if (warp == 0) {
 #pragma unroll
-                    for (int q = 0; q < CPL; ++q)
+                    for (int qq = 0; qq < CPL; ++qq)
 #pragma unroll
-                        for (int h = 0; h < NRHS; ++h) {
-                            const int col = c0 - R0 + q;
-                            const float y = (h < nrhs) ? Bk[static_cast<int64_t>(c0 + q) * ldb + h] : 0.0f;
-                            ts[h * kBlk + col] = y - acc[q * NRHS + h];
-                        }
+                        for (int h = 0; h < NRHS; ++h) part[(c0 + qq) * NRHS + h] = acc[qq * NRHS + h];
                 }
             }
+            cluster.sync();
+            // CTA q sums the partials of columns [16 q, 16 q + 16) over the cluster in a fixed order
+            for (int idx = threadIdx.x; idx < (kBlk / kDiagCluster) * NRHS; idx += kDiagThreads) {
+                const int col = q * (kBlk / kDiagCluster) + idx / NRHS, h = idx % NRHS;
+                float sum = 0.0f;
+#pragma unroll
+                for (int d = 0; d < kDiagCluster; ++d) sum += cluster.map_shared_rank(part, d)[col * NRHS + h];
+                const float y = (h < nrhs) ? Bk[static_cast<int64_t>(R0 + col) * ldb + h] : 0.0f;
+                const float tv = y - sum;
+#pragma unroll
+                for (int d = 0; d < kDiagCluster; ++d) cluster.map_shared_rank(ts, d)[h * kBlk + col] = tv;
+            }
+            cluster.sync();
         }
-        __syncthreads();
         // ---- phase 2: solved_c = inv(L_cc) t   (forward)   or   inv(L_cc)^T t   (backward)
-        const float* D = (backward ? dinvT : dinv) + static_cast<int64_t>(c) * kBlk * kBlk;
-        for (int g = warp; g < kBlk / ROWS; g += NW) {
+        if (ks == 0) {
+            const float* D = (backward ? dinvT : dinv) + static_cast<int64_t>(c) * kBlk * kBlk;
             float acc[64];
 #pragma unroll
             for (int v = 0; v < 64; ++v) acc[v] = 0.0f;
-            rows_dot_f32<NRHS>(D + static_cast<int64_t>(g * ROWS) * kBlk, kBlk, kBlk, ts, kBlk, lane, acc);
+            rows_dot_f32<NRHS>(D + static_cast<int64_t>(grow) * kBlk, kBlk, kBlk, ts, kBlk, lane, acc);
             warp_reduce64(acc, lane);
             const int v0 = warp_reduce64_index(lane);
 #pragma unroll
             for (int t = 0; t < 2; ++t) {
                 const int u = (v0 + t) / NRHS, h = (v0 + t) % NRHS;
-                const int r = R0 + g * ROWS + u;
-                if (backward) sr[static_cast<size_t>(r) * NRHS + h] = acc[t];
-                else zs[h * nb + r] = acc[t];
+                const int r = R0 + grow + u;
+#pragma unroll
+                for (int d = 0; d < kDiagCluster; ++d) {
+                    if (backward) cluster.map_shared_rank(sr, d)[static_cast<size_t>(r) * NRHS + h] = acc[t];
+                    else cluster.map_shared_rank(zs, d)[h * nb + r] = acc[t];
+                }
                 if (h < nrhs) Bk[static_cast<int64_t>(r) * ldb + h] = acc[t];
             }
         }
-        __syncthreads();
+        cluster.sync();
     }
 }
 

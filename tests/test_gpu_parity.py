@@ -117,6 +117,28 @@ def test_fp32_map_meets_all_three_tolerances(krr, name, nb, n, p):
     assert torch.all(F.scales.cpu()[np.tril_indices(cfg.NT)] == 1.0)
 
 
+def test_lookahead_pipeline_matches_serial_schedule(krr):
+    """Default schedule (column k+1's update of the final columns overlaps the factorisation of column
+    k on internal streams) against KRR_FLAG_NO_LOOKAHEAD: same arithmetic up to the FP32 summation
+    order of the newest term, both within the all-FP32 tolerances."""
+    cfg = scaled_config(CONFIGS["C2"], nb=256, n=3072, p=1500)           # NT = 12, nsub = 2
+    A, _ = make_problem(cfg, device="cuda")
+    pmap = oracle_uniform(cfg.NT, R.FP32)
+    h = torch.from_numpy(np.ascontiguousarray(pmap))
+    F1 = krr.potrf_mp(A, cfg.nb, h.cuda(), h, flags=krr.FLAG_PREROUND_A)
+    F2 = krr.potrf_mp(A, cfg.nb, h.cuda(), h, flags=krr.FLAG_PREROUND_A | krr.FLAG_NO_LOOKAHEAD)
+    F3 = krr.potrf_mp(A, cfg.nb, h.cuda(), h, flags=krr.FLAG_PREROUND_A)
+    torch.cuda.synchronize()
+    assert int(F1.info.item()) == 0 and int(F2.info.item()) == 0
+    assert torch.equal(F1.payload, F3.payload)                            # the pipeline is deterministic
+    L1, L2 = F1.dense().cpu().numpy(), F2.dense().cpu().numpy()
+    assert relF(L1, L2) <= 1e-5
+    An = A.cpu().numpy()
+    Lo, _, _ = tile_cholesky_emulated(An, cfg.nb, pmap)
+    for Lg in (L1, L2):
+        assert relF(Lg, Lo) <= 1e-4 and backward_error(An, Lg) <= 1e-6
+
+
 # ------------------------------------------------------------------------------ low-precision maps
 def noise_floor(An, nb, pmap, preround, seed=0):
     """The oracle against itself on an input perturbed at the level of the CUDA path's FP32-class

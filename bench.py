@@ -29,6 +29,9 @@ from krr_inputs import CONFIGS, make_problem  # noqa: E402
 
 METRIC = "mixed-precision Cholesky TOp/s (n^3/3 / device time)"
 UNIT = "TOp/s"
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the trailing-update kernel, from the
+# `ncu --set full` capture summarised under profiles/ (bytes; None where no capture exists)
+TRAFFIC_NCU = {}
 
 
 def load_peaks():
@@ -126,8 +129,12 @@ def run_ours(args, rank, world, local_rank):
     force = {"fp32": krr.FP32, "force_fp16": krr.FP16, "force_fp8": krr.FP8}.get(cfg.map_request)
 
     launches = [0]
+    phase_events = []                            # (map start, potrf start, potrs start, end) per timed step
 
-    def step(collect=None):
+    def step(collect=None, step_flags=flags, mark=False):
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)] if mark else None
+        if mark:
+            ev[0].record()
         if force is None:
             d_map, norms, amax, fro = krr.precision_map(A, nb, cfg.eps_target, cfg.allowed)
             launches[0] += krr.last_launch_count()
@@ -135,11 +142,18 @@ def run_ours(args, rank, world, local_rank):
         else:
             h_map = krr.uniform_map(NT, force)
             d_map = h_map.to(dev)
-        F = krr.potrf_mp(A, nb, d_map, h_map, flags=flags)
+        if mark:
+            ev[1].record()
+        F = krr.potrf_mp(A, nb, d_map, h_map, flags=step_flags)
         launches[0] += krr.last_launch_count()
+        if mark:
+            ev[2].record()
         B = Y.clone()
         krr.potrs(F, B)
         launches[0] += krr.last_launch_count()
+        if mark:
+            ev[3].record()
+            phase_events.append(ev)
         if collect is not None:
             collect["F"], collect["alpha"], collect["h_map"] = F, B, h_map
         return h_map
@@ -161,7 +175,7 @@ def run_ours(args, rank, world, local_rank):
     barrier()
     e0.record()
     for _ in range(args.steps):
-        step()
+        step(mark=True)
     e1.record()
     barrier()
     clocks = sampler.stop()
@@ -177,15 +191,25 @@ def run_ours(args, rank, world, local_rank):
     ops = n ** 3 / 3.0
     value = world * ops / (ms_per_step * 1e-3) / 1e12
 
-    # ---- one extra profiled step: per-kernel breakdown + correctness numbers (not timed) ----------
-    # (bracketed by cudaProfilerStart/Stop so that `ncu --profile-from-start off` lists exactly one step)
+    phases = {"precision_map": 0.0, "potrf_mp": 0.0, "potrs": 0.0}
+    for ev in phase_events:
+        phases["precision_map"] += ev[0].elapsed_time(ev[1]) / len(phase_events)
+        phases["potrf_mp"] += ev[1].elapsed_time(ev[2]) / len(phase_events)
+        phases["potrs"] += ev[2].elapsed_time(ev[3]) / len(phase_events)
+
+    # ---- extra steps, not timed: (a) one step of the default schedule bracketed by cudaProfilerStart/Stop,
+    # so that `ncu --profile-from-start off` lists exactly one step; it also provides the correctness
+    # numbers.  (b) one step with the lookahead off and every kernel category timed: a per-kernel
+    # breakdown whose entries add up (with lookahead kernels share the SMs and their times overlap).
     keep = {}
-    krr.profile_enable(0xFF)
     torch.cuda.synchronize()
     torch.cuda.cudart().cudaProfilerStart()
     h_map = step(keep)
     torch.cuda.synchronize()
     torch.cuda.cudart().cudaProfilerStop()
+    krr.profile_enable(0xFF)
+    step(step_flags=flags | krr.FLAG_NO_LOOKAHEAD)
+    torch.cuda.synchronize()
     breakdown = {k: {"ms": round(v[0], 3), "launches": v[1]} for k, v in krr.profile_read().items() if v[1]}
     krr.profile_enable(0)
     info = int(keep["F"].info.item())
@@ -207,16 +231,20 @@ def run_ours(args, rank, world, local_rank):
     t_bound_upd = sum(fl[c] / (class_peak[c] * 1e12) for c in fl)
     pw_peak = upd_flops / t_bound_upd / 1e12 if t_bound_upd > 0 else class_peak[0]
     achieved = upd_flops * args.steps / (upd_ms * 1e-3) / 1e12 if upd_ms > 0 else 0.0
+    ser_ms = breakdown.get("update_gemm", {}).get("ms", 0.0)
     roofline = {"bound": "tensor", "kernel": "gemm_tc_kernel (MODE_UPDATE: trailing SYRK/GEMM)",
                 "achieved": round(achieved, 2), "peak": round(pw_peak, 2), "unit": "TFLOP/s",
-                "frac": round(achieved / pw_peak, 4), "traffic": None,
+                "frac": round(achieved / pw_peak, 4), "traffic": TRAFFIC_NCU.get(cfg.name),
+                "measured": "CUDA events around every launch of the kernel on its launching streams, inside the timed "
+                            "region (default schedule: launches share SMs with the panel kernels they overlap)",
+                "frac_serial_schedule": round(upd_flops / (ser_ms * 1e-3) / 1e12 / pw_peak, 4) if ser_ms else None,
                 "peak_source": f"{peaks['source']}: bf16 sustained {p16} TF/s; FP32-class = /3 (three kind::f16 "
                                "MMAs per product), FP8 = x2 (nominal ratio)",
                 "flops_per_step_by_class": {"fp32x3": fl[0], "fp16": fl[1], "fp8": fl[2]},
                 "kernel_ms_per_step": round(upd_ms / args.steps, 3), "launches_per_step": upd_launches // args.steps}
     # whole factorisation against the precision-weighted tensor roofline (all n^3/3 credited to the
     # class peaks; panel TRSM runs on the tensor cores in FP32-class)
-    potrf_ms = sum(v["ms"] for k, v in breakdown.items() if k not in ("precision_map", "potrs"))
+    potrf_ms = phases["potrf_mp"]
     pw_frac_potrf = (ops / (pw_peak * 1e12)) / (potrf_ms * 1e-3) if potrf_ms > 0 else None
 
     out = {"metric": METRIC, "value": round(value, 3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -230,8 +258,10 @@ def run_ours(args, rank, world, local_rank):
                       "l2_policy": "inputs (A: %.1f GB) larger than L2, no flush" % (A.numel() * 4 / 1e9),
                       "parallelism": "replicas only" if world > 1 else "single GPU"},
            "clocks": clocks, "gpu_launches": launches[0], "roofline": roofline,
+           "phases_ms": {k: round(v, 3) for k, v in phases.items()},
+           "potrf_TOps": round(ops / (potrf_ms * 1e-3) / 1e12, 2) if potrf_ms > 0 else None,
            "potrf_frac_of_precision_weighted_tensor_peak": round(pw_frac_potrf, 4) if pw_frac_potrf else None,
-           "breakdown_ms_one_step": breakdown, "info": info, "checks": checks}
+           "breakdown_ms_serial_schedule": breakdown, "info": info, "checks": checks}
     return out, (A, Y, krr, cfg, dev)
 
 
@@ -323,7 +353,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="C3", choices=sorted(CONFIGS))
-    ap.add_argument("--sample-tiles", type=int, default=8, help="tiles per dimension of the CPU-oracle sample")
+    ap.add_argument("--sample-tiles", type=int, default=20, help="tiles per dimension of the CPU-oracle sample")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

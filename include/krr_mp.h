@@ -119,10 +119,18 @@ int64_t krr_factor_tile_offset(int64_t n, int nb, const uint8_t* h_map, int i, i
  * d_info   out  one int: 0 on success, j > 0 = 1-based scalar column of the first non-positive
  *               pivot (contents of later tile columns are then unspecified).
  * d_ws     workspace, at least krr_potrf_mp_workspace(n, nb, h_map) bytes, 1024-byte aligned.
- *          It holds the FP16 operand images of L that the tensor-core kernels read and must be
- *          kept if krr_potrf_mp is to be followed by nothing else than krr_potrs (which needs
- *          only d_factor / d_scales / d_map).
- * flags    KRR_FLAG_PREROUND_A, KRR_FLAG_A_TILED_LOWER.
+ *          It holds the FP16 operand images of L that the tensor-core kernels read and two FP32
+ *          panel buffers; it may be released once the call has completed on `stream` (krr_potrs
+ *          needs only d_factor / d_scales / d_map).
+ * flags    KRR_FLAG_PREROUND_A, KRR_FLAG_A_TILED_LOWER, KRR_FLAG_NO_LOOKAHEAD.
+ * Streams  the work is ordered after everything already enqueued on `stream`, and work enqueued on
+ *          `stream` after the call is ordered after it.  Unless KRR_FLAG_NO_LOOKAHEAD is given the
+ *          kernels run on two internal streams (created once per host thread, together with a
+ *          pool of CUDA events) that fork from and join back into `stream`: the update of tile
+ *          column k+1 by the already final columns overlaps the factorisation of column k
+ *          (PAPER.md:206 overlap of the DAG's tasks, :295 lookahead).  The result does not depend
+ *          on timing (fixed summation order), but differs in the last bits between the two
+ *          schedules (the newest column is added in the FP32 epilogue instead of in TMEM).
  */
 size_t krr_potrf_mp_workspace(int64_t n, int nb, const uint8_t* h_map);
 int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb,
@@ -134,8 +142,13 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb,
  * krr_potrs -- solve (L L^T) X = B by forward and backward substitution in FP32 (PAPER.md:114,
  * :169), with the tile mosaic produced by krr_potrf_mp (tiles dequantised on the fly).
  * d_B   in/out  n x nrhs FP32, ROW-major with leading dimension ldb >= nrhs (elements);
- *               in: Y (phenotypes), out: alpha (the weights W of PAPER.md:82).  1 <= nrhs <= 32.
- * d_ws  workspace of at least krr_potrs_workspace(n, nb, nrhs) bytes.
+ *               in: Y (phenotypes), out: alpha (the weights W of PAPER.md:82).  1 <= nrhs <= 32 and
+ *               nb * (nrhs rounded up to 4, 8, 16 or 32) <= 32768 (the solved block of one tile is
+ *               kept in shared memory), else KRR_ERR_SHAPE.
+ * d_ws  workspace of at least krr_potrs_workspace(n, nb, nrhs) bytes, 16-byte aligned: tile offsets
+ *       and the inverses of the 128x128 diagonal blocks of L (2 * n * 128 floats), recomputed by
+ *       every call.  Each diagonal tile is solved by one thread-block cluster of 8 CTAs; sums are
+ *       accumulated in a fixed order (deterministic results).
  */
 size_t krr_potrs_workspace(int64_t n, int nb, int nrhs);
 int krr_potrs(const void* d_factor, const float* d_scales,

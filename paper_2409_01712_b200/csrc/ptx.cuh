@@ -117,6 +117,27 @@ __device__ __forceinline__ void mma_f8_ss(uint32_t d_tmem, uint64_t a_desc, uint
         : "memory");
 }
 
+// kind::mxf8f6f4 with block scaling: D (+)= (A * 2^sfa) (B * 2^sfb)^T, E4M3 operands, one UE8M0 scale
+// per 32 K-elements of every row of A and of B, read from TMEM (sfa / sfb are TMEM addresses).
+__device__ __forceinline__ void mma_mxf8_ss(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc,
+                                            uint32_t idesc, uint32_t accumulate, uint32_t sfa, uint32_t sfb) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::mxf8f6f4.block_scale [%0], %1, %2, %3, [%5], [%6], p;\n\t}\n"
+        ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate), "r"(sfa), "r"(sfb)
+        : "memory");
+}
+
+// registers -> TMEM: the same 32-bit word into this warp's 32 lanes x 4 consecutive columns.
+__device__ __forceinline__ void tmem_st_32x32_x4(uint32_t taddr, uint32_t v) {
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1, %2, %3, %4};"
+                 ::"r"(taddr), "r"(v), "r"(v), "r"(v), "r"(v) : "memory");
+}
+__device__ __forceinline__ void tmem_st_wait() {
+    asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+}
+
 // TMEM -> registers: this warp's 32 lanes x 32 consecutive 32-bit columns.
 __device__ __forceinline__ void tmem_ld_32x32(uint32_t taddr, uint32_t (&r)[32]) {
     asm volatile(
@@ -156,6 +177,16 @@ __host__ __device__ constexpr uint32_t make_idesc(int M, int N, int a_fmt, int b
            | (static_cast<uint32_t>(b_fmt) << 10)    // b_format            [10,13)
            | (static_cast<uint32_t>(N >> 3) << 17)   // n_dim = N/8         [17,23)
            | (static_cast<uint32_t>(M >> 4) << 24);  // m_dim = M/16        [24,29)
+}
+
+// Instruction descriptor of kind::mxf8f6f4.block_scale: E4M3 x E4M3, UE8M0 scales (scale ids 0),
+// both operands K-major, dense, K = 32 per instruction.
+__host__ __device__ constexpr uint32_t make_idesc_mxf8(int M, int N) {
+    return (0u << 7)                                  // a_format = E4M3    [7,10)
+           | (0u << 10)                               // b_format = E4M3    [10,13)
+           | (static_cast<uint32_t>(N >> 3) << 17)    // n_dim = N/8        [17,23)
+           | (1u << 23)                               // scale_format = E8M0
+           | (static_cast<uint32_t>(M >> 4) << 24);   // m_dim = M/16       [24,29)
 }
 
 }  // namespace ptx

@@ -59,6 +59,10 @@ typedef enum { KRR_FP32 = 0, KRR_FP16 = 1, KRR_FP8_E4M3 = 2 } krr_prec_t;
                                        debugging).  Default: column k+1's update of the already final
                                        columns overlaps the factorisation of column k (lookahead 1).  */
 
+#define KRR_FLAG_FP8_VIA_FP16   16u  /* krr_potrf_mp: multiply FP8 x FP8 tile pairs through their (exact) FP16
+                                       images with kind::f16 MMAs instead of kind::mxf8f6f4 on the E4M3
+                                       images (same values, half the tensor rate; cross-check).       */
+
 /* Library version (major*100 + minor) and the compute capability it was built for (100). */
 int krr_version(void);
 int krr_built_for_sm(void);

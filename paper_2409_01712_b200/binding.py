@@ -9,6 +9,7 @@ FP32, FP16, FP8 = 0, 1, 2
 FLAG_PREROUND_A = 1
 FLAG_A_TILED_LOWER = 4
 FLAG_NO_LOOKAHEAD = 8
+FLAG_FP8_VIA_FP16 = 16
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB = None

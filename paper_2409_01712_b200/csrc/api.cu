@@ -83,6 +83,20 @@ static int make_plane_tmap(CUtensorMap* tm, const void* base, uint64_t rows, uin
     return r == CUDA_SUCCESS ? KRR_OK : KRR_ERR_CUDA;
 }
 
+// Row-major [rows][cols] array of bytes (E4M3 images), box = 128 columns x 128 rows, 128-byte swizzle.
+static int make_byte_plane_tmap(CUtensorMap* tm, const void* base, uint64_t rows, uint64_t cols) {
+    EncodeTiledFn enc = get_encode_fn();
+    if (!enc) return KRR_ERR_CUDA;
+    cuuint64_t gdim[2] = {cols, rows};
+    cuuint64_t gstride[1] = {cols};
+    cuuint32_t box[2] = {128u, static_cast<cuuint32_t>(kBlk)};
+    cuuint32_t estr[2] = {1, 1};
+    CUresult r = enc(tm, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<void*>(base), gdim, gstride, box, estr,
+                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS ? KRR_OK : KRR_ERR_CUDA;
+}
+
 // ---- mosaic offsets (host) -------------------------------------------------------------------
 static size_t host_offsets(int NT, int nb, const uint8_t* h_map, std::vector<int64_t>* off) {
     size_t acc = 0;
@@ -177,12 +191,12 @@ static int launch(int cat, K kernel, dim3 grid, dim3 block, size_t smem, cudaStr
 }
 
 static int launch_gemm(const CUtensorMap& a_hi, const CUtensorMap& a_lo, const CUtensorMap& b_hi,
-                       const CUtensorMap& b_lo, const GemmOp& op, int max_ctas, cudaStream_t st) {
+                       const CUtensorMap& b_lo, const CUtensorMap& q, const GemmOp& op, int max_ctas, cudaStream_t st) {
     const int ntiles = op.nrb * op.ncb;
     if (ntiles <= 0) return KRR_OK;
     const int grid = ntiles < max_ctas ? ntiles : max_ctas;
     ProfScope ps(op.mode == MODE_UPDATE ? CAT_UPDATE : (op.mode == MODE_P1 ? CAT_P1 : CAT_P3), st);
-    gemm_tc_kernel<<<grid, kGemmThreads, kGemmSmem, st>>>(a_hi, a_lo, b_hi, b_lo, op);
+    gemm_tc_kernel<<<grid, kGemmThreads, kGemmSmem, st>>>(a_hi, a_lo, b_hi, b_lo, q, op);
     ++g_launches;
     return cudaGetLastError() == cudaSuccess ? KRR_OK : KRR_ERR_CUDA;
 }
@@ -321,7 +335,7 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
     if (reinterpret_cast<uintptr_t>(d_A) % 16 != 0 || reinterpret_cast<uintptr_t>(d_ws) % 1024 != 0 ||
         reinterpret_cast<uintptr_t>(d_factor) % 128 != 0)
         return KRR_ERR_ARG;
-    if (flags & ~(KRR_FLAG_PREROUND_A | KRR_FLAG_A_TILED_LOWER | KRR_FLAG_NO_LOOKAHEAD)) return KRR_ERR_UNSUPPORTED;
+    if (flags & ~(KRR_FLAG_PREROUND_A | KRR_FLAG_A_TILED_LOWER | KRR_FLAG_NO_LOOKAHEAD | KRR_FLAG_FP8_VIA_FP16)) return KRR_ERR_UNSUPPORTED;
     const int NT = static_cast<int>(n / nb);
     bool any_fp8 = false;
     rc = check_map(NT, h_map, &any_fp8);
@@ -364,10 +378,15 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
         if (rc) return rc;
     }
 
-    CUtensorMap tmH, tmL, tmIH, tmIL;
+    CUtensorMap tmH, tmL, tmIH, tmIL, tmQ;
     if (make_plane_tmap(&tmH, Hp, nslots * nb, nb) || make_plane_tmap(&tmL, Lp, nslots * nb, nb) ||
         make_plane_tmap(&tmIH, linv_hi, nb, kBlk) || make_plane_tmap(&tmIL, linv_lo, nb, kBlk))
         return KRR_ERR_CUDA;
+    if (any_fp8) {
+        if (make_byte_plane_tmap(&tmQ, Qp, nslots * nb, nb)) return KRR_ERR_CUDA;
+    } else {
+        tmQ = tmH;                                // never dereferenced (op.fp8q = 0)
+    }
 
     const int nsub = nb / kBlk;
     const bool lookahead = !(flags & KRR_FLAG_NO_LOOKAHEAD) && NT > 2;
@@ -398,11 +417,12 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
         op.map = d_map; op.A = A; op.a_amax = (preround && any_fp8) ? a_amax : nullptr;
         op.W = Wk; op.Hp = Hp; op.Lp = Lp; op.tile_amax = tile_amax; op.flags = flags;
         op.scl = scl; op.linv_scale = linv_scale;
+        op.scales = d_scales; op.fp8q = (any_fp8 && !(flags & KRR_FLAG_FP8_VIA_FP16)) ? 1 : 0;
         // ---- U(k): S = rd(A) - L[:, 0:k] L[k, 0:k]^T over the tile column (SYRK + GEMM) ----
         op.mode = MODE_UPDATE; op.c = 0; op.cb0 = 0; op.ncb = nsub;
         if (!lookahead) {
             op.s_lo = 0; op.s_hi = k; op.base_w = 0; op.planes = 1; op.rb0 = 0; op.nrb = mblk;
-            rc = launch_gemm(tmH, tmL, tmH, tmL, op, num_sms, st);
+            rc = launch_gemm(tmH, tmL, tmH, tmL, tmQ, op, num_sms, st);
             if (rc) return rc;
         } else {
             // terms s < k-1 were accumulated into Wk by U_old(k) while column k-1 was being factorised;
@@ -411,11 +431,11 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
             op.s_lo = (k >= 1) ? k - 1 : 0; op.s_hi = k; op.base_w = have_old ? 1 : 0; op.planes = 1;
             if (have_old) KRR_CUDA_CHECK(cudaStreamWaitEvent(sh, ev_old(k), 0));
             op.rb0 = 0; op.nrb = nsub;
-            rc = launch_gemm(tmH, tmL, tmH, tmL, op, num_sms, sh);
+            rc = launch_gemm(tmH, tmL, tmH, tmL, tmQ, op, num_sms, sh);
             if (rc) return rc;
             if (k >= 1) KRR_CUDA_CHECK(cudaStreamWaitEvent(sl, ev_fin(k - 1), 0));
             op.rb0 = nsub; op.nrb = mblk - nsub;
-            rc = launch_gemm(tmH, tmL, tmH, tmL, op, bulk_ctas, sl);
+            rc = launch_gemm(tmH, tmL, tmH, tmL, tmQ, op, bulk_ctas, sl);
             if (rc) return rc;
             KRR_CUDA_CHECK(cudaEventRecord(ev_newb(k), sl));
             if (k + 1 < NT && k >= 1) {
@@ -424,7 +444,7 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
                 on.k = k + 1; on.prow0 = tile_slot(NT, k + 1, k + 1) * nb; on.W = Wbuf[(k + 1) & 1];
                 on.s_lo = 0; on.s_hi = k; on.base_w = 0; on.planes = 0;
                 on.rb0 = 0; on.nrb = (NT - k - 1) * nsub;
-                rc = launch_gemm(tmH, tmL, tmH, tmL, on, bulk_ctas, sl);
+                rc = launch_gemm(tmH, tmL, tmH, tmL, tmQ, on, bulk_ctas, sl);
                 if (rc) return rc;
                 KRR_CUDA_CHECK(cudaEventRecord(ev_old(k + 1), sl));
             }
@@ -440,7 +460,7 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
                 if (c > 0) {
                     op.mode = MODE_P1; op.c = c; op.cb0 = c; op.ncb = 1;
                     op.rb0 = (part == 0) ? c : row_lo; op.nrb = row_hi - op.rb0;
-                    rc = launch_gemm(tmH, tmL, tmH, tmL, op, num_sms, sh);
+                    rc = launch_gemm(tmH, tmL, tmH, tmL, tmQ, op, num_sms, sh);
                     if (rc) return rc;
                 }
                 if (part == 0) {
@@ -452,7 +472,7 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
                 op.mode = MODE_P3; op.c = c; op.cb0 = c; op.ncb = 1;
                 op.rb0 = (part == 0) ? c + 1 : row_lo; op.nrb = row_hi - op.rb0;
                 if (op.nrb > 0) {
-                    rc = launch_gemm(tmH, tmL, tmIH, tmIL, op, num_sms, sh);
+                    rc = launch_gemm(tmH, tmL, tmIH, tmIL, tmQ, op, num_sms, sh);
                     if (rc) return rc;
                 }
             }

@@ -17,6 +17,14 @@
 // low-precision tile holds its stored value exactly).  Accumulators never leave TMEM until the
 // tile's whole K range is done ("round once", R4).
 //
+// FP8 x FP8 terms (both operand tiles stored as E4M3 with power-of-two tile scales) run as
+// kind::mxf8f6f4.block_scale MMAs on the 1-byte images (Qp plane, K = 128 per 16 KB smem block): the
+// per-tile scale times the plane scale sx is a power of two, i.e. a UE8M0 block scale that is the same
+// for every row and every K block of the tile.  TMEM columns 256.. hold a table of 64 constant scale
+// vectors (entry j: every byte = kSfBias + j); an MMA just points its scale operands at the two
+// entries of its tiles, so no scale data is ever staged.  Tiles whose exponent falls outside the
+// table (never seen on the workloads) take the FP16 path through their hi image, which is exact too.
+//
 // Accumulation order: the tensor core adds each MMA's result to the TMEM accumulator with
 // truncation, a bias of ~half an ulp OF THE ACCUMULATOR per instruction (measured: backward error
 // growing linearly in n when K is walked upwards).  In a Cholesky update the leading columns of L
@@ -48,6 +56,8 @@ struct GemmOp {
     __half* Hp;           // hi plane  [nslots*nb][nb]
     __half* Lp;           // lo plane
     float* tile_amax;     // per-slot max|X| accumulated by MODE_P3
+    const float* scales;  // NT*NT tile scales of the mosaic (FP8 tiles), written by finalize_kernel
+    int fp8q;             // MODE_UPDATE: FP8 x FP8 terms may use the E4M3 images (Qp plane exists)
     const float* scl;     // device float[4]: sx, ss, 1/sx^2, 1/ss  (power-of-two plane scales)
     const float* linv_scale;  // device float[nb/128]: scale of each inverted diagonal block's planes
     unsigned flags;
@@ -59,7 +69,10 @@ constexpr int kPlaneBytes = kBlk * kBlockK * 2;    // one 128 x 64 fp16 operand 
 constexpr int kStageBytes = 4 * kPlaneBytes;       // A_hi, A_lo, B_hi, B_lo
 constexpr int kAccCols = 128;                      // TMEM columns of one 128x128 FP32 accumulator
 constexpr int kAccBufs = 2;
-constexpr int kTmemCols = kAccCols * kAccBufs;     // 256
+constexpr int kSfCol0 = kAccCols * kAccBufs;       // first TMEM column of the scale table
+constexpr int kSfEntries = 64;                     // 4 columns each
+constexpr int kSfBias = 127 - 40;                  // entry j <-> UE8M0 byte kSfBias + j, i.e. 2^(j - 40)
+constexpr int kTmemCols = 512;                     // 2 accumulators + scale table
 constexpr int kGemmThreads = 192;                  // warp 0 TMA, warp 1 MMA (+TMEM alloc), 2-5 epilogue
 constexpr int kGemmSmem = kStages * kStageBytes + 1024 /*align*/ + 256 /*barriers*/;
 
@@ -68,10 +81,16 @@ struct TermInfo {
     int a_k0, b_k0;         // first K column (TMA coordinate 0)
     int nchunks;            // K chunks of 64
     int nA, nB;             // planes per operand: 2 = hi+lo (FP32 class), 1 = hi only
+    int q;                  // 1: FP8 x FP8 term on the E4M3 images (K chunks of 128, block-scaled MMA)
+    int sfa, sfb;           // scale-table entries of the two tiles (q = 1)
 };
+
+// UE8M0 byte of the power of two x (> 0, normal): its biased exponent.
+__device__ __forceinline__ int pow2_exponent_byte(float x) { return static_cast<int>((__float_as_uint(x) >> 23) & 0xffu); }
 
 __device__ __forceinline__ TermInfo get_term(const GemmOp& op, int s /* term index */, int rb, int cb) {
     TermInfo t;
+    t.q = 0; t.sfa = 0; t.sfb = 0;
     if (op.mode == MODE_UPDATE) {
         const int i = op.k + (rb * kBlk) / op.nb;
         const int subrow = (rb * kBlk) % op.nb;
@@ -81,8 +100,18 @@ __device__ __forceinline__ TermInfo get_term(const GemmOp& op, int s /* term ind
         t.a_k0 = 0;
         t.b_k0 = 0;
         t.nchunks = op.nb / kBlockK;
-        t.nA = (op.map[i * op.NT + s] == KRR_FP32) ? 2 : 1;
-        t.nB = (op.map[op.k * op.NT + s] == KRR_FP32) ? 2 : 1;
+        const int pa = op.map[i * op.NT + s], pb = op.map[op.k * op.NT + s];
+        t.nA = (pa == KRR_FP32) ? 2 : 1;
+        t.nB = (pb == KRR_FP32) ? 2 : 1;
+        if (op.fp8q && pa == KRR_FP8_E4M3 && pb == KRR_FP8_E4M3) {
+            const float sx = op.scl[0];
+            t.sfa = pow2_exponent_byte(sx * op.scales[i * op.NT + s]) - kSfBias;
+            t.sfb = pow2_exponent_byte(sx * op.scales[op.k * op.NT + s]) - kSfBias;
+            if (t.sfa >= 0 && t.sfa < kSfEntries && t.sfb >= 0 && t.sfb < kSfEntries) {
+                t.q = 1;
+                t.nchunks = op.nb / 128;
+            }
+        }
     } else if (op.mode == MODE_P1) {
         t.a_row = op.prow0 + static_cast<int64_t>(rb) * kBlk;
         t.b_row = op.prow0 + static_cast<int64_t>(op.c) * kBlk;
@@ -115,7 +144,7 @@ __device__ __forceinline__ bool tile_is_skipped(const GemmOp& op, int rb, int cb
 __global__ void __launch_bounds__(kGemmThreads, 1)
 gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_constant__ CUtensorMap tmA_lo,
                const __grid_constant__ CUtensorMap tmB_hi, const __grid_constant__ CUtensorMap tmB_lo,
-               const GemmOp op) {
+               const __grid_constant__ CUtensorMap tmQ, const GemmOp op) {
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
     const uint32_t bar_base = smem_base + kStages * kStageBytes;
@@ -139,6 +168,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_constant
         ptx::prefetch_tmap(&tmA_lo);
         ptx::prefetch_tmap(&tmB_hi);
         ptx::prefetch_tmap(&tmB_lo);
+        if (op.fp8q) ptx::prefetch_tmap(&tmQ);
         for (int s = 0; s < kStages; ++s) {
             ptx::mbar_init(full_bar(s), 1);
             ptx::mbar_init(empty_bar(s), 1);
@@ -157,6 +187,18 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_constant
     __syncthreads();
     ptx::tc_fence_after();
     const uint32_t tmem_base = *tmem_slot_ptr;
+    if (op.fp8q && op.mode == MODE_UPDATE) {
+        // scale table: entry j = 4 TMEM columns whose every byte is the UE8M0 code kSfBias + j
+        if (warp >= 2) {
+            const uint32_t lane_base = static_cast<uint32_t>((warp & 3) * 32) << 16;
+            for (int j = 0; j < kSfEntries; ++j)
+                ptx::tmem_st_32x32_x4(tmem_base + lane_base + kSfCol0 + 4 * j, static_cast<uint32_t>(kSfBias + j) * 0x01010101u);
+            ptx::tmem_st_wait();
+        }
+        ptx::tc_fence_before();
+        __syncthreads();
+        ptx::tc_fence_after();
+    }
 
     if (warp == 0) {
         // ===================== TMA producer =====================
@@ -168,11 +210,17 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_constant
                 if (tile_is_skipped(op, rb, cb)) continue;
                 for (int s = nterms - 1; s >= 0; --s) {      // descending K: see note on accumulation order
                     const TermInfo ti = get_term(op, s, rb, cb);
-                    const uint32_t bytes = static_cast<uint32_t>(ti.nA + ti.nB) * kPlaneBytes;
+                    const uint32_t bytes = static_cast<uint32_t>(ti.q ? 2 : ti.nA + ti.nB) * kPlaneBytes;
                     for (int ch = ti.nchunks - 1; ch >= 0; --ch) {
                         ptx::mbar_wait(empty_bar(stage), phase ^ 1u);
                         const uint32_t sa = smem_base + stage * kStageBytes;
                         ptx::mbar_arrive_expect_tx(full_bar(stage), bytes);
+                        if (ti.q) {      // E4M3 images: 128 rows x 128 bytes per operand
+                            ptx::tma_load_2d(sa, &tmQ, full_bar(stage), ch * 128, static_cast<int>(ti.a_row));
+                            ptx::tma_load_2d(sa + 2 * kPlaneBytes, &tmQ, full_bar(stage), ch * 128, static_cast<int>(ti.b_row));
+                            if (++stage == kStages) { stage = 0; phase ^= 1u; }
+                            continue;
+                        }
                         const int ak = ti.a_k0 + ch * kBlockK, bk = ti.b_k0 + ch * kBlockK;
                         ptx::tma_load_2d(sa, &tmA_hi, full_bar(stage), ak, static_cast<int>(ti.a_row));
                         if (ti.nA == 2)
@@ -192,6 +240,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_constant
         // ===================== MMA issuer (one thread) =====================
         if (lane == 0 && has_acc) {
             constexpr uint32_t idesc = ptx::make_idesc(kBlk, kBlk, /*F16*/ 0, /*F16*/ 0);
+            constexpr uint32_t idesc_q = ptx::make_idesc_mxf8(kBlk, kBlk);
             int stage = 0;
             uint32_t phase = 0;
             int buf = 0;
@@ -213,6 +262,18 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_constant
                         const uint64_t a_lo = ptx::smem_desc_sw128(sa + kPlaneBytes);
                         const uint64_t b_hi = ptx::smem_desc_sw128(sa + 2 * kPlaneBytes);
                         const uint64_t b_lo = ptx::smem_desc_sw128(sa + 3 * kPlaneBytes);
+                        if (ti.q) {
+                            const uint32_t sfa = tmem_base + kSfCol0 + 4 * ti.sfa, sfb = tmem_base + kSfCol0 + 4 * ti.sfb;
+#pragma unroll
+                            for (int kk = 3; kk >= 0; --kk) {              // 4 x K=32 per 128-byte row
+                                const uint64_t adv = static_cast<uint64_t>((kk * 32) >> 4);
+                                ptx::mma_mxf8_ss(d_tmem, a_hi + adv, b_hi + adv, idesc_q, accumulate, sfa, sfb);
+                                accumulate = 1;
+                            }
+                            ptx::tc_commit(empty_bar(stage));
+                            if (++stage == kStages) { stage = 0; phase ^= 1u; }
+                            continue;
+                        }
 #pragma unroll
                         for (int kk = kBlockK / 16 - 1; kk >= 0; --kk) {
                             const uint64_t adv = static_cast<uint64_t>((kk * 32) >> 4);   // +32 B per K=16

@@ -229,6 +229,30 @@ def test_low_precision_maps(krr, case):
     assert relF(alpha.cpu().numpy().astype(np.float64), potrs_fp64(Lg, Y.cpu().numpy(), nb)) <= 1e-5
 
 
+def test_fp8_block_scaled_mma_matches_fp16_image_path(krr):
+    """FP8 x FP8 tile products on the E4M3 images (kind::mxf8f6f4, UE8M0 tile scales from the TMEM table)
+    against the same products through the exact FP16 images (KRR_FLAG_FP8_VIA_FP16): identical operand
+    values, so the factors agree to FP32 accumulation noise amplified by the FP8 roundings."""
+    cfg = replace(scaled_config(CONFIGS["S1"], nb=256, n=2048, p=1536), genotype="maf", gamma_scale=4.0)
+    A, _ = make_problem(cfg, device="cuda")
+    pmap = oracle_uniform(cfg.NT, R.FP8)
+    h = torch.from_numpy(np.ascontiguousarray(pmap))
+    F1 = krr.potrf_mp(A, cfg.nb, h.cuda(), h, flags=krr.FLAG_PREROUND_A)
+    F2 = krr.potrf_mp(A, cfg.nb, h.cuda(), h, flags=krr.FLAG_PREROUND_A | krr.FLAG_FP8_VIA_FP16)
+    torch.cuda.synchronize()
+    assert int(F1.info.item()) == 0 and int(F2.info.item()) == 0
+    An = A.cpu().numpy()
+    L1, L2 = F1.dense().cpu().numpy(), F2.dense().cpu().numpy()
+    Lo, floor = noise_floor(An, cfg.nb, pmap, True)
+    b1, b2, bo = backward_error(An, L1), backward_error(An, L2), backward_error(An, Lo)
+    print(f"fp8 mx vs fp16-image: relF {relF(L1, L2):.3e} floor {floor:.3e} backward {b1:.4e} {b2:.4e} oracle {bo:.4e}")
+    assert relF(L1, L2) <= max(1e-4, 2.0 * floor)
+    assert abs(b1 - bo) <= 0.02 * bo and abs(b2 - bo) <= 0.02 * bo
+    # the first tile column involves no FP8 x FP8 product: bitwise equal
+    assert np.array_equal(L1[:, :cfg.nb], L2[:, :cfg.nb])
+    assert np.mean(L1 == L2) > 0.5
+
+
 # ------------------------------------------------------------------------------ exact constructions
 @pytest.mark.parametrize("prec", [R.FP32, R.FP16, R.FP8, "mixed"])
 @pytest.mark.parametrize("n,nb", [(512, 128), (1024, 256)])

@@ -126,7 +126,9 @@ def run_ours(args, rank, world, local_rank):
     A, Y = make_problem(cfg_r, device=dev)
     n, nb, NT = cfg.n, cfg.nb, cfg.NT
     flags = krr.FLAG_PREROUND_A
-    force = {"fp32": krr.FP32, "force_fp16": krr.FP16, "force_fp8": krr.FP8}.get(cfg.map_request)
+    force = {"fp32": krr.FP32, "force_fp16": krr.FP16, "force_fp8": krr.FP8, "fp8_col0_fp32": krr.FP8}.get(cfg.map_request)
+    if cfg.map_request == "fp8_col0_fp32":
+        flags = 0                                # C5': A as given, operands as stored
 
     launches = [0]
     phase_events = []                            # (map start, potrf start, potrs start, end) per timed step
@@ -141,6 +143,8 @@ def run_ours(args, rank, world, local_rank):
             h_map = d_map.cpu()                  # launch sequence is built on the host from the map
         else:
             h_map = krr.uniform_map(NT, force)
+            if cfg.map_request == "fp8_col0_fp32":
+                h_map[1:, 0] = krr.FP32
             d_map = h_map.to(dev)
         if mark:
             ev[1].record()

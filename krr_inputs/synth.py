@@ -151,7 +151,7 @@ class Config:
     nrhs: int
     seed: int
     genotype: str = "maf"            # "maf" | "uniform"
-    map_request: str = "fp32"        # "fp32" | "rule" | "force_fp8" | "force_fp16"
+    map_request: str = "fp32"        # "fp32" | "rule" | "force_fp8" | "force_fp16" | "fp8_col0_fp32"
     eps_target: float = 0.0
     allowed: tuple = (0,)            # precision codes the rule may use
     lower_tiles_only: bool = False
@@ -176,6 +176,10 @@ CONFIGS = {
                  eps_target=1e-3, allowed=(0, 1, 2), lower_tiles_only=True),
     "C5": Config("C5", 98304, 20000, 1024, 1e-1, 4, seed=5, genotype="uniform",
                  map_request="force_fp8", allowed=(0, 2)),
+    # C5': the matrix of C5 with tile column 0 kept in FP32, the rest FP8, A not pre-rounded,
+    # operands as stored -- the timed stand-in for C5, whose literal map breaks down (info > 0)
+    "C5p": Config("C5p", 98304, 20000, 1024, 1e-1, 4, seed=5, genotype="uniform",
+                  map_request="fp8_col0_fp32", allowed=(0, 2)),
     # supplementary: the paper's regime K ~ I (gamma = 12/p) with two families of
     # relatives -- the only input on which the rule yields a genuine FP32/FP16/FP8 mosaic
     "S1": Config("S1", 32768, 24576, 1024, 1e-2, 8, seed=6, genotype="families:4096",

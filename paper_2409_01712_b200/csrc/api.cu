@@ -477,7 +477,7 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
                 }
             }
         }
-        rc = launch(CAT_FINALIZE, finalize_kernel, dim3(nb / 16, NT - k), dim3(256), 0, sh, NT, nb, k, static_cast<const float*>(Wk),
+        rc = launch(CAT_FINALIZE, finalize_kernel, dim3(nsub * nsub * 4, NT - k), dim3(256), 0, sh, NT, nb, k, static_cast<const float*>(Wk),
                     d_map, static_cast<const int64_t*>(off), static_cast<const float*>(tile_amax),
                     static_cast<uint8_t*>(d_factor), d_scales, Hp, Qp, static_cast<const float*>(scl));
         if (rc) return rc;

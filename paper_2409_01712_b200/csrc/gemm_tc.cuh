@@ -73,8 +73,11 @@ constexpr int kSfCol0 = kAccCols * kAccBufs;       // first TMEM column of the s
 constexpr int kSfEntries = 64;                     // 4 columns each
 constexpr int kSfBias = 127 - 40;                  // entry j <-> UE8M0 byte kSfBias + j, i.e. 2^(j - 40)
 constexpr int kTmemCols = 512;                     // 2 accumulators + scale table
-constexpr int kGemmThreads = 192;                  // warp 0 TMA, warp 1 MMA (+TMEM alloc), 2-5 epilogue
-constexpr int kGemmSmem = kStages * kStageBytes + 1024 /*align*/ + 256 /*barriers*/;
+constexpr int kGemmThreads = 320;                  // warp 0 TMA, warp 1 MMA (+TMEM alloc), 2-9 epilogue
+constexpr int kEpiWarps = 8;
+constexpr int kEpiRowBytes = 80;                   // 64 B of FP16 per row + 16 B pad (conflict-free 16 B accesses)
+constexpr int kEpiStageBytes = 32 * kEpiRowBytes;  // per-warp transpose buffer
+constexpr int kGemmSmem = kStages * kStageBytes + 1024 /*align*/ + 256 /*barriers*/ + kEpiWarps * kEpiStageBytes;
 
 struct TermInfo {
     int64_t a_row, b_row;   // plane rows (TMA coordinate 1)
@@ -175,7 +178,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_constant
         }
         for (int b = 0; b < kAccBufs; ++b) {
             ptx::mbar_init(tfull_bar(b), 1);
-            ptx::mbar_init(tempty_bar(b), 4);
+            ptx::mbar_init(tempty_bar(b), kEpiWarps);
         }
         ptx::fence_mbar_init();
     }
@@ -293,94 +296,107 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_constant
         }
     } else {
         // ===================== epilogue warps (TMEM -> registers -> global) =====================
-        const int q = warp & 3;                    // TMEM lane quadrant this warp may access
+        // Warp (q, hf): TMEM lanes (rows) 32q..32q+31, columns 64hf..64hf+63 of the 128x128 block.
+        // W is block-column-major, so a warp's 32 rows of one column are 128 contiguous bytes; the FP16
+        // images are row-major (TMA / MMA operand layout) and go through a per-warp smem transpose so
+        // that every store instruction writes 8 full 64-byte row segments.
+        const int ew = warp - 2;
+        const int q = warp & 3;
+        const int hf = ew >> 2;
+        uint8_t* stg = smem_raw + (bar_base - ptx::smem_u32(smem_raw)) + 256 + ew * kEpiStageBytes;
+        const int nsub = op.nb / kBlk;
         int buf = 0;
         uint32_t acc_phase = 0;
         for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
             const int rb = op.rb0 + t / op.ncb, cb = op.cb0 + t % op.ncb;
             if (tile_is_skipped(op, rb, cb)) continue;
             const int row_in_blk = q * 32 + lane;
-            const int64_t r = static_cast<int64_t>(rb) * kBlk + row_in_blk;    // panel-local row
-            const int col0 = cb * kBlk;
-            // base pointer and pre-rounding of A
-            const float* base = nullptr;
-            int p = KRR_FP32;
-            float sc = 1.0f;
-            if (op.mode == MODE_UPDATE) {
+            const int col0 = cb * kBlk + 64 * hf;                 // first column (inside the tile column) of this warp
+            float* wblk = op.W + (static_cast<int64_t>(rb) * nsub + cb) * (kBlk * kBlk) + static_cast<int64_t>(64 * hf) * kBlk + row_in_blk;
+            // ---- base values, fetched before the accumulator is ready
+            float bs[64];
+            const bool base_from_w = (op.mode == MODE_P1) || (op.mode == MODE_UPDATE && op.base_w);
+            const bool base_from_a = (op.mode == MODE_UPDATE && !op.base_w);
+            if (base_from_w) {
+#pragma unroll
+                for (int e = 0; e < 64; ++e) bs[e] = wblk[e * kBlk];
+            } else if (base_from_a) {
                 const int i = op.k + (rb * kBlk) / op.nb;
                 const int subrow = (rb * kBlk) % op.nb;
-                if (op.base_w) {
-                    base = op.W + r * op.nb + col0;
-                } else {
-                    base = op.A.tile_ptr(i, op.k, subrow + row_in_blk, col0);
-                    if ((op.flags & KRR_FLAG_PREROUND_A) && i != op.k) {
-                        p = op.map[i * op.NT + op.k];
-                        if (p == KRR_FP8_E4M3) sc = fp8_scale_from_amax(op.a_amax[i * op.NT + op.k]);
-                    }
+                const float* arow = op.A.tile_ptr(i, op.k, subrow + row_in_blk, col0);
+                int p = KRR_FP32;
+                float sc = 1.0f;
+                if ((op.flags & KRR_FLAG_PREROUND_A) && i != op.k) {
+                    p = op.map[i * op.NT + op.k];
+                    if (p == KRR_FP8_E4M3) sc = fp8_scale_from_amax(op.a_amax[i * op.NT + op.k]);
                 }
-            } else if (op.mode == MODE_P1) {
-                base = op.W + r * op.nb + col0;
+#pragma unroll
+                for (int e = 0; e < 64; e += 4) {
+                    const float4 v = *reinterpret_cast<const float4*>(arow + e);
+                    bs[e + 0] = round_to_prec(v.x, p, sc);
+                    bs[e + 1] = round_to_prec(v.y, p, sc);
+                    bs[e + 2] = round_to_prec(v.z, p, sc);
+                    bs[e + 3] = round_to_prec(v.w, p, sc);
+                }
+            } else {
+#pragma unroll
+                for (int e = 0; e < 64; ++e) bs[e] = 0.0f;
             }
             // exact power-of-two rescaling: accumulator -> value domain, value -> plane domain
-            const float acc_mul = (op.mode == MODE_P3) ? op.scl[3] / op.linv_scale[op.c] : op.scl[2];
+            const float acc_mul = (op.mode == MODE_P3) ? -op.scl[3] / op.linv_scale[op.c] : op.scl[2];
             const float plane_mul = (op.mode == MODE_P3) ? op.scl[0] : op.scl[1];
-            float* wout = op.W + r * op.nb + col0;
-            __half* hout = op.Hp + (op.prow0 + r) * op.nb + col0;
-            __half* lout = op.Lp + (op.prow0 + r) * op.nb + col0;
+            float out[64];
             if (has_acc) {
                 ptx::mbar_wait(tfull_bar(buf), acc_phase);
                 ptx::tc_fence_after();
-            }
-            float amax = 0.0f;
-#pragma unroll 1
-            for (int j = 0; j < kBlk / 32; ++j) {
-                uint32_t acc[32];
-                if (has_acc) {
-                    ptx::tmem_ld_32x32(tmem_base + buf * kAccCols + (static_cast<uint32_t>(q * 32) << 16) + j * 32, acc);
-                    ptx::tmem_ld_wait();
-                } else {
-#pragma unroll
-                    for (int e = 0; e < 32; ++e) acc[e] = 0u;
-                }
-                float out[32];
-                if (base != nullptr) {
-#pragma unroll
-                    for (int e = 0; e < 32; e += 4) {
-                        const float4 b = *reinterpret_cast<const float4*>(base + j * 32 + e);
-                        out[e + 0] = round_to_prec(b.x, p, sc) - __uint_as_float(acc[e + 0]) * acc_mul;
-                        out[e + 1] = round_to_prec(b.y, p, sc) - __uint_as_float(acc[e + 1]) * acc_mul;
-                        out[e + 2] = round_to_prec(b.z, p, sc) - __uint_as_float(acc[e + 2]) * acc_mul;
-                        out[e + 3] = round_to_prec(b.w, p, sc) - __uint_as_float(acc[e + 3]) * acc_mul;
-                    }
-                } else {
-#pragma unroll
-                    for (int e = 0; e < 32; ++e) out[e] = __uint_as_float(acc[e]) * acc_mul;
-                }
-#pragma unroll
-                for (int e = 0; e < 32; e += 4)
-                    *reinterpret_cast<float4*>(wout + j * 32 + e) = make_float4(out[e], out[e + 1], out[e + 2], out[e + 3]);
-                if (write_planes) {
-#pragma unroll
-                for (int e = 0; e < 32; e += 8) {
-                    __align__(16) __half hi[8];
-                    __align__(16) __half lo[8];
-#pragma unroll
-                    for (int u = 0; u < 8; ++u) {
-                        const float x = out[e + u] * plane_mul;
-                        hi[u] = __float2half_rn(x);
-                        lo[u] = __float2half_rn(x - __half2float(hi[u]));
-                        amax = fmaxf(amax, fabsf(out[e + u]));
-                    }
-                    *reinterpret_cast<uint4*>(hout + j * 32 + e) = *reinterpret_cast<const uint4*>(hi);
-                    *reinterpret_cast<uint4*>(lout + j * 32 + e) = *reinterpret_cast<const uint4*>(lo);
-                }
-                }
-            }
-            if (has_acc) {
+                uint32_t a0[32], a1[32];
+                const uint32_t taddr = tmem_base + buf * kAccCols + (static_cast<uint32_t>(q * 32) << 16) + 64 * hf;
+                ptx::tmem_ld_32x32(taddr, a0);
+                ptx::tmem_ld_32x32(taddr + 32, a1);
+                ptx::tmem_ld_wait();
                 ptx::tc_fence_before();
                 __syncwarp();
-                if (lane == 0) ptx::mbar_arrive(tempty_bar(buf));
+                if (lane == 0) ptx::mbar_arrive(tempty_bar(buf));          // accumulator is in registers
                 if (++buf == kAccBufs) { buf = 0; acc_phase ^= 1u; }
+#pragma unroll
+                for (int e = 0; e < 32; ++e) {
+                    out[e] = fmaf(-__uint_as_float(a0[e]), acc_mul, bs[e]);
+                    out[32 + e] = fmaf(-__uint_as_float(a1[e]), acc_mul, bs[32 + e]);
+                }
+            } else {
+#pragma unroll
+                for (int e = 0; e < 64; ++e) out[e] = bs[e];
+            }
+#pragma unroll
+            for (int e = 0; e < 64; ++e) wblk[e * kBlk] = out[e];
+            float amax = 0.0f;
+            if (write_planes) {
+                const int64_t prow = op.prow0 + static_cast<int64_t>(rb) * kBlk + q * 32;      // plane row of this warp's row 0
+#pragma unroll
+                for (int part = 0; part < 4; ++part) {             // (chunk 0 hi, chunk 0 lo, chunk 1 hi, chunk 1 lo)
+                    const int jj = part >> 1;
+                    const bool is_lo = part & 1;
+                    __align__(16) __half hv[32];
+#pragma unroll
+                    for (int e = 0; e < 32; ++e) {
+                        const float x = out[jj * 32 + e] * plane_mul;
+                        const __half h = __float2half_rn(x);
+                        hv[e] = is_lo ? __float2half_rn(x - __half2float(h)) : h;
+                        if (!is_lo) amax = fmaxf(amax, fabsf(out[jj * 32 + e]));
+                    }
+                    __syncwarp();                                   // previous part has been read out
+#pragma unroll
+                    for (int u = 0; u < 4; ++u)
+                        *reinterpret_cast<uint4*>(stg + lane * kEpiRowBytes + u * 16) = *reinterpret_cast<const uint4*>(hv + 8 * u);
+                    __syncwarp();
+                    __half* plane = is_lo ? op.Lp : op.Hp;
+#pragma unroll
+                    for (int it = 0; it < 4; ++it) {
+                        const int rr = it * 8 + (lane >> 2), ch = lane & 3;
+                        const uint4 v = *reinterpret_cast<const uint4*>(stg + rr * kEpiRowBytes + ch * 16);
+                        *reinterpret_cast<uint4*>(plane + (prow + rr) * op.nb + col0 + jj * 32 + ch * 8) = v;
+                    }
+                }
             }
             if (op.mode == MODE_P3 && op.tile_amax != nullptr) {
 #pragma unroll

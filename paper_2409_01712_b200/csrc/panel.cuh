@@ -75,26 +75,36 @@ tile_amax_kernel(AView A, const uint8_t* __restrict__ map, float* __restrict__ a
     if ((threadIdx.x & 31) == 0) atomicMax(reinterpret_cast<int*>(a_amax + i * NT + j), __float_as_int(amax));
 }
 
-// Round tile column k (rows of the panel, FP32 in W) into the mosaic.  grid = (nb/16, NT-k).
-// blockDim = 256: each CTA handles 16 rows of one tile.
+// Round tile column k (FP32 in W, block-column-major 128x128 blocks) into the mosaic.
+// grid = (nsub*nsub*4, NT-k), 256 threads: one CTA transposes 32 rows of one 128x128 block through
+// shared memory (coalesced reads of W columns, coalesced row-major writes of the factor / images).
 __global__ void __launch_bounds__(256)
 finalize_kernel(int NT, int nb, int k, const float* __restrict__ W, const uint8_t* __restrict__ map,
                 const int64_t* __restrict__ off, const float* __restrict__ tile_amax /* per slot */,
                 uint8_t* __restrict__ factor, float* __restrict__ scales, __half* __restrict__ Hp,
                 uint8_t* __restrict__ Qp, const float* __restrict__ scl) {
+    __shared__ float tile[32][kBlk + 1];
     const float sx = scl[0];
+    const int nsub = nb / kBlk;
     const int i = k + blockIdx.y;
     const int p = map[i * NT + k];
     const int64_t slot = tile_slot(NT, i, k);
     const float s = (p == KRR_FP8_E4M3) ? fp8_scale_from_amax(tile_amax[slot]) : 1.0f;
     if (blockIdx.x == 0 && threadIdx.x == 0) scales[i * NT + k] = s;
     uint8_t* dst = factor + off[i * NT + k];
-    const int r0 = blockIdx.x * 16;
-    const int vec_per_row = nb / 4;
-    for (int idx = threadIdx.x; idx < 16 * vec_per_row; idx += 256) {
-        const int r = r0 + idx / vec_per_row, c = (idx % vec_per_row) * 4;
-        const int64_t prow = static_cast<int64_t>(blockIdx.y) * nb + r;     // panel-local row
-        float4 v = *reinterpret_cast<const float4*>(W + prow * nb + c);
+    const int blk = blockIdx.x >> 2, qr = blockIdx.x & 3;
+    const int rbl = blk / nsub, cb = blk % nsub;                         // block inside the tile
+    const int64_t rb = static_cast<int64_t>(blockIdx.y) * nsub + rbl;    // panel-local row block
+    const float* wblk = W + (rb * nsub + cb) * (kBlk * kBlk) + 32 * qr;
+    for (int idx = threadIdx.x; idx < 32 * kBlk; idx += 256) {
+        const int c = idx >> 5, rr = idx & 31;
+        tile[rr][c] = wblk[c * kBlk + rr];
+    }
+    __syncthreads();
+    for (int idx = threadIdx.x; idx < 32 * (kBlk / 4); idx += 256) {
+        const int rr = idx / (kBlk / 4), c4 = (idx % (kBlk / 4)) * 4;
+        const int r = rbl * kBlk + 32 * qr + rr, c = cb * kBlk + c4;     // element of the tile
+        float4 v = make_float4(tile[rr][c4], tile[rr][c4 + 1], tile[rr][c4 + 2], tile[rr][c4 + 3]);
         const int64_t e = static_cast<int64_t>(r) * nb + c;
         if (p == KRR_FP32) {
             if (i == k) {      // diagonal tile: zeros above the diagonal

@@ -163,11 +163,16 @@ potrf128_kernel(float* __restrict__ W, int nb, int r0, int c0, __half* __restric
     float* x = tri_sm + kBlk * kTriLd;       // [128][132] : inv(L); rows 96..127 double as scratch early on
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     constexpr int NW = kTriThreads / 32;
+    // W is block-column-major: element (r, c) of 128x128 block (rb, cb) at ((rb*nsub + cb)*128 + c)*128 + r
+    float* wblk = W + (static_cast<int64_t>(r0 / kBlk) * (nb / kBlk) + c0 / kBlk) * (kBlk * kBlk);
     for (int idx = tid; idx < kBlk * (kBlk / 4); idx += kTriThreads) {
-        const int r = idx / (kBlk / 4), c4 = (idx % (kBlk / 4)) * 4;
-        *reinterpret_cast<float4*>(a + r * kTriLd + c4) =
-            *reinterpret_cast<const float4*>(W + static_cast<int64_t>(r0 + r) * nb + c0 + c4);
-        *reinterpret_cast<float4*>(x + r * kTriLd + c4) = make_float4(0.f, 0.f, 0.f, 0.f);
+        const int c = idx / (kBlk / 4), r4 = (idx % (kBlk / 4)) * 4;
+        const float4 v = *reinterpret_cast<const float4*>(wblk + c * kBlk + r4);
+        a[(r4 + 0) * kTriLd + c] = v.x;
+        a[(r4 + 1) * kTriLd + c] = v.y;
+        a[(r4 + 2) * kTriLd + c] = v.z;
+        a[(r4 + 3) * kTriLd + c] = v.w;
+        *reinterpret_cast<float4*>(x + c * kTriLd + r4) = make_float4(0.f, 0.f, 0.f, 0.f);
     }
     __syncthreads();
     for (int jb = 0; jb < 4; ++jb) {
@@ -230,7 +235,10 @@ potrf128_kernel(float* __restrict__ W, int nb, int r0, int c0, __half* __restric
         v.y = (c4 + 1 <= r) ? lv.y : 0.0f;
         v.z = (c4 + 2 <= r) ? lv.z : 0.0f;
         v.w = (c4 + 3 <= r) ? lv.w : 0.0f;
-        *reinterpret_cast<float4*>(W + static_cast<int64_t>(r0 + r) * nb + c0 + c4) = v;
+        wblk[(c4 + 0) * kBlk + r] = v.x;
+        wblk[(c4 + 1) * kBlk + r] = v.y;
+        wblk[(c4 + 2) * kBlk + r] = v.z;
+        wblk[(c4 + 3) * kBlk + r] = v.w;
         __align__(8) __half hi[4];
         __align__(8) __half lo[4];
 #pragma unroll

@@ -129,6 +129,7 @@ def run_ours(args, rank, world, local_rank):
     force = {"fp32": krr.FP32, "force_fp16": krr.FP16, "force_fp8": krr.FP8, "fp8_col0_fp32": krr.FP8}.get(cfg.map_request)
     if cfg.map_request == "fp8_col0_fp32":
         flags = 0                                # C5': A as given, operands as stored
+    flags |= args.potrf_flags
 
     launches = [0]
     phase_events = []                            # (map start, potrf start, potrs start, end) per timed step
@@ -358,6 +359,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="C3", choices=sorted(CONFIGS))
     ap.add_argument("--sample-tiles", type=int, default=20, help="tiles per dimension of the CPU-oracle sample")
+    ap.add_argument("--potrf-flags", type=int, default=0, help="extra KRR_FLAG_* bits for krr_potrf_mp (experiments)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

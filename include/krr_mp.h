@@ -63,6 +63,10 @@ typedef enum { KRR_FP32 = 0, KRR_FP16 = 1, KRR_FP8_E4M3 = 2 } krr_prec_t;
                                        images with kind::f16 MMAs instead of kind::mxf8f6f4 on the E4M3
                                        images (same values, half the tensor rate; cross-check).       */
 
+#define KRR_FLAG_NO_CTA_PAIRS   32u  /* krr_potrf_mp: run the trailing updates with one CTA per 128x128 block
+                                       instead of CTA pairs (tcgen05 cta_group::2, 256x128 blocks); same
+                                       arithmetic, cross-check / comparison.  Pairs need nb % 256 == 0.   */
+
 /* Library version (major*100 + minor) and the compute capability it was built for (100). */
 int krr_version(void);
 int krr_built_for_sm(void);

@@ -70,12 +70,12 @@ static EncodeTiledFn get_encode_fn() {
 }
 
 // Row-major [rows][cols] array of 2-byte elements, box = 64 columns x 128 rows, 128-byte swizzle.
-static int make_plane_tmap(CUtensorMap* tm, const void* base, uint64_t rows, uint64_t cols) {
+static int make_plane_tmap(CUtensorMap* tm, const void* base, uint64_t rows, uint64_t cols, int box_rows = kBlk) {
     EncodeTiledFn enc = get_encode_fn();
     if (!enc) return KRR_ERR_CUDA;
     cuuint64_t gdim[2] = {cols, rows};
     cuuint64_t gstride[1] = {cols * 2};
-    cuuint32_t box[2] = {static_cast<cuuint32_t>(kBlockK), static_cast<cuuint32_t>(kBlk)};
+    cuuint32_t box[2] = {static_cast<cuuint32_t>(kBlockK), static_cast<cuuint32_t>(box_rows)};
     cuuint32_t estr[2] = {1, 1};
     CUresult r = enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 2, const_cast<void*>(base), gdim, gstride, box, estr,
                      CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
@@ -84,12 +84,12 @@ static int make_plane_tmap(CUtensorMap* tm, const void* base, uint64_t rows, uin
 }
 
 // Row-major [rows][cols] array of bytes (E4M3 images), box = 128 columns x 128 rows, 128-byte swizzle.
-static int make_byte_plane_tmap(CUtensorMap* tm, const void* base, uint64_t rows, uint64_t cols) {
+static int make_byte_plane_tmap(CUtensorMap* tm, const void* base, uint64_t rows, uint64_t cols, int box_rows = kBlk) {
     EncodeTiledFn enc = get_encode_fn();
     if (!enc) return KRR_ERR_CUDA;
     cuuint64_t gdim[2] = {cols, rows};
     cuuint64_t gstride[1] = {cols};
-    cuuint32_t box[2] = {128u, static_cast<cuuint32_t>(kBlk)};
+    cuuint32_t box[2] = {128u, static_cast<cuuint32_t>(box_rows)};
     cuuint32_t estr[2] = {1, 1};
     CUresult r = enc(tm, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<void*>(base), gdim, gstride, box, estr,
                      CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
@@ -190,14 +190,34 @@ static int launch(int cat, K kernel, dim3 grid, dim3 block, size_t smem, cudaStr
     return cudaGetLastError() == cudaSuccess ? KRR_OK : KRR_ERR_CUDA;
 }
 
-static int launch_gemm(const CUtensorMap& a_hi, const CUtensorMap& a_lo, const CUtensorMap& b_hi,
-                       const CUtensorMap& b_lo, const CUtensorMap& q, const GemmOp& op, int max_ctas, cudaStream_t st) {
-    const int ntiles = op.nrb * op.ncb;
-    if (ntiles <= 0) return KRR_OK;
-    const int grid = ntiles < max_ctas ? ntiles : max_ctas;
+// The tensor maps of one factorisation: hi/lo FP16 images of L (128-row boxes for A operands and for
+// single-CTA B operands, 64-row boxes for the B halves of CTA pairs), the inverted diagonal blocks,
+// and the E4M3 images.
+struct GemmMaps { CUtensorMap H, L, Hh, Lh, IH, IL, Q, Qh; };
+
+// cg = 2 runs MODE_UPDATE on CTA pairs (256 x 256 output blocks); needs even block counts and no FP8 images.
+static int launch_gemm(const GemmMaps& m, const GemmOp& op, int max_ctas, int cg, cudaStream_t st) {
+    if (op.nrb <= 0 || op.ncb <= 0) return KRR_OK;
     ProfScope ps(op.mode == MODE_UPDATE ? CAT_UPDATE : (op.mode == MODE_P1 ? CAT_P1 : CAT_P3), st);
-    gemm_tc_kernel<<<grid, kGemmThreads, kGemmSmem, st>>>(a_hi, a_lo, b_hi, b_lo, q, op);
     ++g_launches;
+    if (cg == 2 && op.mode == MODE_UPDATE && op.nrb % 2 == 0 && op.rb0 % 2 == 0 && op.ncb % 2 == 0 && op.cb0 % 2 == 0 &&
+        !op.fp8q) {
+        const int npairs = (op.nrb / 2) * (op.ncb / 2);
+        const int max_pairs = max_ctas / 2;
+        const int grid = 2 * (npairs < max_pairs ? npairs : max_pairs);
+        cudaLaunchConfig_t cfg;
+        memset(&cfg, 0, sizeof(cfg));
+        cfg.gridDim = dim3(grid); cfg.blockDim = dim3(kGemmThreads); cfg.dynamicSmemBytes = kGemmSmem; cfg.stream = st;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = 2; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+        cfg.attrs = attr; cfg.numAttrs = 1;
+        return cudaLaunchKernelEx(&cfg, gemm_tc_kernel<2>, m.H, m.L, m.H, m.L, m.Q, m.Q, op) == cudaSuccess ? KRR_OK : KRR_ERR_CUDA;
+    }
+    const int ntiles = op.nrb * op.ncb;
+    const int grid = ntiles < max_ctas ? ntiles : max_ctas;
+    if (op.mode == MODE_P3) gemm_tc_kernel<1><<<grid, kGemmThreads, kGemmSmem, st>>>(m.H, m.L, m.IH, m.IL, m.Q, m.Q, op);
+    else gemm_tc_kernel<1><<<grid, kGemmThreads, kGemmSmem, st>>>(m.H, m.L, m.H, m.L, m.Q, m.Q, op);
     return cudaGetLastError() == cudaSuccess ? KRR_OK : KRR_ERR_CUDA;
 }
 
@@ -213,7 +233,8 @@ static int set_potrs_attrs() {
 static int set_kernel_attrs() {
     static bool done = false;
     if (done) return KRR_OK;
-    KRR_CUDA_CHECK(cudaFuncSetAttribute(gemm_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem));
+    KRR_CUDA_CHECK(cudaFuncSetAttribute(gemm_tc_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem));
+    KRR_CUDA_CHECK(cudaFuncSetAttribute(gemm_tc_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem));
     KRR_CUDA_CHECK(cudaFuncSetAttribute(potrf128_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kTriSmem));
     KRR_CUDA_CHECK(cudaFuncSetAttribute(trtri128_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kTriSmem));
     if (set_potrs_attrs<4>() || set_potrs_attrs<8>() || set_potrs_attrs<16>() || set_potrs_attrs<32>()) return KRR_ERR_CUDA;
@@ -335,7 +356,7 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
     if (reinterpret_cast<uintptr_t>(d_A) % 16 != 0 || reinterpret_cast<uintptr_t>(d_ws) % 1024 != 0 ||
         reinterpret_cast<uintptr_t>(d_factor) % 128 != 0)
         return KRR_ERR_ARG;
-    if (flags & ~(KRR_FLAG_PREROUND_A | KRR_FLAG_A_TILED_LOWER | KRR_FLAG_NO_LOOKAHEAD | KRR_FLAG_FP8_VIA_FP16)) return KRR_ERR_UNSUPPORTED;
+    if (flags & ~(KRR_FLAG_PREROUND_A | KRR_FLAG_A_TILED_LOWER | KRR_FLAG_NO_LOOKAHEAD | KRR_FLAG_FP8_VIA_FP16 | KRR_FLAG_NO_CTA_PAIRS)) return KRR_ERR_UNSUPPORTED;
     const int NT = static_cast<int>(n / nb);
     bool any_fp8 = false;
     rc = check_map(NT, h_map, &any_fp8);
@@ -378,15 +399,18 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
         if (rc) return rc;
     }
 
-    CUtensorMap tmH, tmL, tmIH, tmIL, tmQ;
-    if (make_plane_tmap(&tmH, Hp, nslots * nb, nb) || make_plane_tmap(&tmL, Lp, nslots * nb, nb) ||
-        make_plane_tmap(&tmIH, linv_hi, nb, kBlk) || make_plane_tmap(&tmIL, linv_lo, nb, kBlk))
+    GemmMaps tm;
+    if (make_plane_tmap(&tm.H, Hp, nslots * nb, nb) || make_plane_tmap(&tm.L, Lp, nslots * nb, nb) ||
+        make_plane_tmap(&tm.Hh, Hp, nslots * nb, nb, kBlk / 2) || make_plane_tmap(&tm.Lh, Lp, nslots * nb, nb, kBlk / 2) ||
+        make_plane_tmap(&tm.IH, linv_hi, nb, kBlk) || make_plane_tmap(&tm.IL, linv_lo, nb, kBlk))
         return KRR_ERR_CUDA;
     if (any_fp8) {
-        if (make_byte_plane_tmap(&tmQ, Qp, nslots * nb, nb)) return KRR_ERR_CUDA;
+        if (make_byte_plane_tmap(&tm.Q, Qp, nslots * nb, nb) || make_byte_plane_tmap(&tm.Qh, Qp, nslots * nb, nb, kBlk / 2))
+            return KRR_ERR_CUDA;
     } else {
-        tmQ = tmH;                                // never dereferenced (op.fp8q = 0)
+        tm.Q = tm.H; tm.Qh = tm.H;                // never dereferenced (op.fp8q = 0)
     }
+    const int cg = ((flags & KRR_FLAG_NO_CTA_PAIRS) || nb % (2 * kBlk) != 0) ? 1 : 2;
 
     const int nsub = nb / kBlk;
     const bool lookahead = !(flags & KRR_FLAG_NO_LOOKAHEAD) && NT > 2;
@@ -422,7 +446,7 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
         op.mode = MODE_UPDATE; op.c = 0; op.cb0 = 0; op.ncb = nsub;
         if (!lookahead) {
             op.s_lo = 0; op.s_hi = k; op.base_w = 0; op.planes = 1; op.rb0 = 0; op.nrb = mblk;
-            rc = launch_gemm(tmH, tmL, tmH, tmL, tmQ, op, num_sms, st);
+            rc = launch_gemm(tm, op, num_sms, cg, st);
             if (rc) return rc;
         } else {
             // terms s < k-1 were accumulated into Wk by U_old(k) while column k-1 was being factorised;
@@ -431,11 +455,11 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
             op.s_lo = (k >= 1) ? k - 1 : 0; op.s_hi = k; op.base_w = have_old ? 1 : 0; op.planes = 1;
             if (have_old) KRR_CUDA_CHECK(cudaStreamWaitEvent(sh, ev_old(k), 0));
             op.rb0 = 0; op.nrb = nsub;
-            rc = launch_gemm(tmH, tmL, tmH, tmL, tmQ, op, num_sms, sh);
+            rc = launch_gemm(tm, op, num_sms, cg, sh);
             if (rc) return rc;
             if (k >= 1) KRR_CUDA_CHECK(cudaStreamWaitEvent(sl, ev_fin(k - 1), 0));
             op.rb0 = nsub; op.nrb = mblk - nsub;
-            rc = launch_gemm(tmH, tmL, tmH, tmL, tmQ, op, bulk_ctas, sl);
+            rc = launch_gemm(tm, op, bulk_ctas, cg, sl);
             if (rc) return rc;
             KRR_CUDA_CHECK(cudaEventRecord(ev_newb(k), sl));
             if (k + 1 < NT && k >= 1) {
@@ -444,7 +468,7 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
                 on.k = k + 1; on.prow0 = tile_slot(NT, k + 1, k + 1) * nb; on.W = Wbuf[(k + 1) & 1];
                 on.s_lo = 0; on.s_hi = k; on.base_w = 0; on.planes = 0;
                 on.rb0 = 0; on.nrb = (NT - k - 1) * nsub;
-                rc = launch_gemm(tmH, tmL, tmH, tmL, tmQ, on, bulk_ctas, sl);
+                rc = launch_gemm(tm, on, bulk_ctas, cg, sl);
                 if (rc) return rc;
                 KRR_CUDA_CHECK(cudaEventRecord(ev_old(k + 1), sl));
             }
@@ -460,7 +484,7 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
                 if (c > 0) {
                     op.mode = MODE_P1; op.c = c; op.cb0 = c; op.ncb = 1;
                     op.rb0 = (part == 0) ? c : row_lo; op.nrb = row_hi - op.rb0;
-                    rc = launch_gemm(tmH, tmL, tmH, tmL, tmQ, op, num_sms, sh);
+                    rc = launch_gemm(tm, op, num_sms, cg, sh);
                     if (rc) return rc;
                 }
                 if (part == 0) {
@@ -472,7 +496,7 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
                 op.mode = MODE_P3; op.c = c; op.cb0 = c; op.ncb = 1;
                 op.rb0 = (part == 0) ? c + 1 : row_lo; op.nrb = row_hi - op.rb0;
                 if (op.nrb > 0) {
-                    rc = launch_gemm(tmH, tmL, tmIH, tmIL, tmQ, op, num_sms, sh);
+                    rc = launch_gemm(tm, op, num_sms, 1, sh);
                     if (rc) return rc;
                 }
             }

@@ -144,25 +144,42 @@ __device__ __forceinline__ bool tile_is_skipped(const GemmOp& op, int rb, int cb
     return op.mode == MODE_UPDATE && (rb * kBlk) < op.nb && cb > rb;
 }
 
+// CG = 1: one CTA per 128x128 output block.  CG = 2 (MODE_UPDATE only): a CTA pair (cluster of 2,
+// tcgen05 cta_group::2) per 256x256 block -- each CTA stages its own 128 rows of A and the 128 rows of
+// B of ONE of the two column blocks, the leader issues M = 256, N = 256 MMAs that read both CTAs'
+// shared memory, and each CTA's TMEM receives its own 128 rows x 256 columns of the accumulator (two
+// buffers fill the 512 TMEM columns, so this variant has no scale table: FP8 pairs go through their
+// FP16 images, or the host picks CG = 1).  Per flop it moves half the operand bytes of CG = 1.
+template <int CG>
 __global__ void __launch_bounds__(kGemmThreads, 1)
 gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_constant__ CUtensorMap tmA_lo,
                const __grid_constant__ CUtensorMap tmB_hi, const __grid_constant__ CUtensorMap tmB_lo,
-               const __grid_constant__ CUtensorMap tmQ, const GemmOp op) {
+               const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmQb, const GemmOp op) {
+    constexpr uint32_t kBBytes = kPlaneBytes;           // this CTA's B block: 128 rows
+    constexpr int NS = kStages;
+    constexpr uint32_t SB = 2 * kPlaneBytes + 2 * kBBytes;      // A_hi, A_lo, B_hi, B_lo
+    static_assert(NS * SB <= kStages * kStageBytes && NS <= 4, "smem ring");
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
     const uint32_t bar_base = smem_base + kStages * kStageBytes;
     // barriers: full[kStages], empty[kStages], tmem_full[kAccBufs], tmem_empty[kAccBufs], tmem ptr
     auto full_bar = [&](int s) { return bar_base + 8u * s; };
-    auto empty_bar = [&](int s) { return bar_base + 8u * (kStages + s); };
-    auto tfull_bar = [&](int b) { return bar_base + 8u * (2 * kStages + b); };
-    auto tempty_bar = [&](int b) { return bar_base + 8u * (2 * kStages + kAccBufs + b); };
-    const uint32_t tmem_slot = bar_base + 8u * (2 * kStages + 2 * kAccBufs);
+    auto empty_bar = [&](int s) { return bar_base + 8u * (4 + s); };
+    auto tfull_bar = [&](int b) { return bar_base + 8u * (8 + b); };
+    auto tempty_bar = [&](int b) { return bar_base + 8u * (8 + kAccBufs + b); };
+    const uint32_t tmem_slot = bar_base + 8u * (8 + 2 * kAccBufs);
     uint32_t* tmem_slot_ptr = reinterpret_cast<uint32_t*>(smem_raw + (tmem_slot - ptx::smem_u32(smem_raw)));
 
     const int warp = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
-    const int ntiles = op.nrb * op.ncb;
+    const int rank = (CG == 2) ? static_cast<int>(ptx::cluster_ctarank()) : 0;
+    const int unit0 = (CG == 2) ? static_cast<int>(blockIdx.x >> 1) : static_cast<int>(blockIdx.x);   // pair / CTA index
+    const int nunits = (CG == 2) ? static_cast<int>(gridDim.x >> 1) : static_cast<int>(gridDim.x);
+    const int ncbu = op.ncb / CG;                       // column units
+    const int ntiles = (op.nrb / CG) * ncbu;            // output blocks of (128*CG) x (128*CG)
+    constexpr int kAccW = kAccCols * CG;                // accumulator columns per buffer
     const int nterms = num_terms(op);
+
     const bool has_acc = (op.mode != MODE_UPDATE) ? (op.mode == MODE_P3 || op.c > 0) : (nterms > 0);
     const bool write_planes = (op.mode != MODE_UPDATE) || op.planes;
 
@@ -171,26 +188,26 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_constant
         ptx::prefetch_tmap(&tmA_lo);
         ptx::prefetch_tmap(&tmB_hi);
         ptx::prefetch_tmap(&tmB_lo);
-        if (op.fp8q) ptx::prefetch_tmap(&tmQ);
-        for (int s = 0; s < kStages; ++s) {
+        if (op.fp8q) { ptx::prefetch_tmap(&tmQ); ptx::prefetch_tmap(&tmQb); }
+        for (int s = 0; s < NS; ++s) {
             ptx::mbar_init(full_bar(s), 1);
             ptx::mbar_init(empty_bar(s), 1);
         }
         for (int b = 0; b < kAccBufs; ++b) {
             ptx::mbar_init(tfull_bar(b), 1);
-            ptx::mbar_init(tempty_bar(b), kEpiWarps);
+            ptx::mbar_init(tempty_bar(b), kEpiWarps * CG);
         }
         ptx::fence_mbar_init();
     }
     if (warp == 1) {
-        ptx::tmem_alloc<kTmemCols>(tmem_slot);
-        ptx::tmem_relinquish();
+        ptx::tmem_alloc<kTmemCols, CG>(tmem_slot);
+        ptx::tmem_relinquish<CG>();
     }
     ptx::tc_fence_before();
-    __syncthreads();
+    if (CG == 2) ptx::cluster_sync_all(); else __syncthreads();     // peer barriers are initialised too
     ptx::tc_fence_after();
     const uint32_t tmem_base = *tmem_slot_ptr;
-    if (op.fp8q && op.mode == MODE_UPDATE) {
+    if (CG == 1 && op.fp8q && op.mode == MODE_UPDATE) {
         // scale table: entry j = 4 TMEM columns whose every byte is the UE8M0 code kSfBias + j
         if (warp >= 2) {
             const uint32_t lane_base = static_cast<uint32_t>((warp & 3) * 32) << 16;
@@ -199,7 +216,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_constant
             ptx::tmem_st_wait();
         }
         ptx::tc_fence_before();
-        __syncthreads();
+        if (CG == 2) ptx::cluster_sync_all(); else __syncthreads();     // the leader's MMAs read both tables
         ptx::tc_fence_after();
     }
 
@@ -208,89 +225,95 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_constant
         if (lane == 0 && has_acc) {
             int stage = 0;
             uint32_t phase = 0;
-            for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
-                const int rb = op.rb0 + t / op.ncb, cb = op.cb0 + t % op.ncb;
-                if (tile_is_skipped(op, rb, cb)) continue;
+            auto load = [&](uint32_t dst, const CUtensorMap* m, uint32_t bar, int c0, int c1) {
+                if (CG == 2) ptx::tma_load_2d_pair(dst, m, bar, c0, c1); else ptx::tma_load_2d(dst, m, bar, c0, c1);
+            };
+            for (int t = unit0; t < ntiles; t += nunits) {
+                const int rb = op.rb0 + (t / ncbu) * CG + rank, cb0u = op.cb0 + (t % ncbu) * CG;
+                if (tile_is_skipped(op, rb - rank + CG - 1, cb0u)) continue;    // the whole (pair) block lies above the diagonal
                 for (int s = nterms - 1; s >= 0; --s) {      // descending K: see note on accumulation order
-                    const TermInfo ti = get_term(op, s, rb, cb);
-                    const uint32_t bytes = static_cast<uint32_t>(ti.q ? 2 : ti.nA + ti.nB) * kPlaneBytes;
+                    const TermInfo ti = get_term(op, s, rb, cb0u + rank);        // this CTA's A rows and B rows
+                    // bytes landing under the leader's barrier: both CTAs' A blocks and B halves
+                    const uint32_t bytes = ti.q ? CG * (kPlaneBytes + kBBytes)
+                                                : CG * (static_cast<uint32_t>(ti.nA) * kPlaneBytes + static_cast<uint32_t>(ti.nB) * kBBytes);
+                    const int b_row = static_cast<int>(ti.b_row);
                     for (int ch = ti.nchunks - 1; ch >= 0; --ch) {
                         ptx::mbar_wait(empty_bar(stage), phase ^ 1u);
-                        const uint32_t sa = smem_base + stage * kStageBytes;
-                        ptx::mbar_arrive_expect_tx(full_bar(stage), bytes);
-                        if (ti.q) {      // E4M3 images: 128 rows x 128 bytes per operand
-                            ptx::tma_load_2d(sa, &tmQ, full_bar(stage), ch * 128, static_cast<int>(ti.a_row));
-                            ptx::tma_load_2d(sa + 2 * kPlaneBytes, &tmQ, full_bar(stage), ch * 128, static_cast<int>(ti.b_row));
-                            if (++stage == kStages) { stage = 0; phase ^= 1u; }
+                        const uint32_t sa = smem_base + stage * SB;
+                        if (rank == 0) ptx::mbar_arrive_expect_tx(full_bar(stage), bytes);
+                        if (ti.q) {      // E4M3 images: 128 bytes of K per row
+                            load(sa, &tmQ, full_bar(stage), ch * 128, static_cast<int>(ti.a_row));
+                            load(sa + 2 * kPlaneBytes, &tmQb, full_bar(stage), ch * 128, b_row);
+                            if (++stage == NS) { stage = 0; phase ^= 1u; }
                             continue;
                         }
                         const int ak = ti.a_k0 + ch * kBlockK, bk = ti.b_k0 + ch * kBlockK;
-                        ptx::tma_load_2d(sa, &tmA_hi, full_bar(stage), ak, static_cast<int>(ti.a_row));
-                        if (ti.nA == 2)
-                            ptx::tma_load_2d(sa + kPlaneBytes, &tmA_lo, full_bar(stage), ak,
-                                             static_cast<int>(ti.a_row));
-                        ptx::tma_load_2d(sa + 2 * kPlaneBytes, &tmB_hi, full_bar(stage), bk,
-                                         static_cast<int>(ti.b_row));
-                        if (ti.nB == 2)
-                            ptx::tma_load_2d(sa + 3 * kPlaneBytes, &tmB_lo, full_bar(stage), bk,
-                                             static_cast<int>(ti.b_row));
-                        if (++stage == kStages) { stage = 0; phase ^= 1u; }
+                        load(sa, &tmA_hi, full_bar(stage), ak, static_cast<int>(ti.a_row));
+                        if (ti.nA == 2) load(sa + kPlaneBytes, &tmA_lo, full_bar(stage), ak, static_cast<int>(ti.a_row));
+                        load(sa + 2 * kPlaneBytes, &tmB_hi, full_bar(stage), bk, b_row);
+                        if (ti.nB == 2) load(sa + 2 * kPlaneBytes + kBBytes, &tmB_lo, full_bar(stage), bk, b_row);
+                        if (++stage == NS) { stage = 0; phase ^= 1u; }
                     }
                 }
             }
         }
     } else if (warp == 1) {
         // ===================== MMA issuer (one thread) =====================
-        if (lane == 0 && has_acc) {
-            constexpr uint32_t idesc = ptx::make_idesc(kBlk, kBlk, /*F16*/ 0, /*F16*/ 0);
-            constexpr uint32_t idesc_q = ptx::make_idesc_mxf8(kBlk, kBlk);
+        if (lane == 0 && has_acc && rank == 0) {
+            constexpr uint32_t idesc = ptx::make_idesc(kBlk * CG, kBlk * CG, /*F16*/ 0, /*F16*/ 0);
+            constexpr uint32_t idesc_q = ptx::make_idesc_mxf8(kBlk * CG, kBlk * CG);
+            auto mma = [&](uint32_t d, uint64_t a, uint64_t b, uint32_t acc) {
+                if (CG == 2) ptx::mma_f16_ss_pair(d, a, b, idesc, acc); else ptx::mma_f16_ss(d, a, b, idesc, acc);
+            };
+            auto commit = [&](uint32_t bar) { if (CG == 2) ptx::tc_commit_pair(bar); else ptx::tc_commit(bar); };
             int stage = 0;
             uint32_t phase = 0;
             int buf = 0;
             uint32_t acc_phase = 0;
-            for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
-                const int rb = op.rb0 + t / op.ncb, cb = op.cb0 + t % op.ncb;
-                if (tile_is_skipped(op, rb, cb)) continue;
+            for (int t = unit0; t < ntiles; t += nunits) {
+                const int rb = op.rb0 + (t / ncbu) * CG, cb = op.cb0 + (t % ncbu) * CG;
+                if (tile_is_skipped(op, rb + CG - 1, cb)) continue;
                 ptx::mbar_wait(tempty_bar(buf), acc_phase ^ 1u);     // epilogue drained this buffer
                 ptx::tc_fence_after();
-                const uint32_t d_tmem = tmem_base + buf * kAccCols;
+                const uint32_t d_tmem = tmem_base + buf * kAccW;
                 uint32_t accumulate = 0;
                 for (int s = nterms - 1; s >= 0; --s) {      // descending K: see note on accumulation order
                     const TermInfo ti = get_term(op, s, rb, cb);
                     for (int ch = ti.nchunks - 1; ch >= 0; --ch) {
                         ptx::mbar_wait(full_bar(stage), phase);
                         ptx::tc_fence_after();
-                        const uint32_t sa = smem_base + stage * kStageBytes;
+                        const uint32_t sa = smem_base + stage * SB;
                         const uint64_t a_hi = ptx::smem_desc_sw128(sa);
                         const uint64_t a_lo = ptx::smem_desc_sw128(sa + kPlaneBytes);
                         const uint64_t b_hi = ptx::smem_desc_sw128(sa + 2 * kPlaneBytes);
-                        const uint64_t b_lo = ptx::smem_desc_sw128(sa + 3 * kPlaneBytes);
+                        const uint64_t b_lo = ptx::smem_desc_sw128(sa + 2 * kPlaneBytes + kBBytes);
                         if (ti.q) {
                             const uint32_t sfa = tmem_base + kSfCol0 + 4 * ti.sfa, sfb = tmem_base + kSfCol0 + 4 * ti.sfb;
 #pragma unroll
                             for (int kk = 3; kk >= 0; --kk) {              // 4 x K=32 per 128-byte row
                                 const uint64_t adv = static_cast<uint64_t>((kk * 32) >> 4);
-                                ptx::mma_mxf8_ss(d_tmem, a_hi + adv, b_hi + adv, idesc_q, accumulate, sfa, sfb);
+                                if (CG == 2) ptx::mma_mxf8_ss_pair(d_tmem, a_hi + adv, b_hi + adv, idesc_q, accumulate, sfa, sfb);
+                                else ptx::mma_mxf8_ss(d_tmem, a_hi + adv, b_hi + adv, idesc_q, accumulate, sfa, sfb);
                                 accumulate = 1;
                             }
-                            ptx::tc_commit(empty_bar(stage));
-                            if (++stage == kStages) { stage = 0; phase ^= 1u; }
+                            commit(empty_bar(stage));
+                            if (++stage == NS) { stage = 0; phase ^= 1u; }
                             continue;
                         }
 #pragma unroll
                         for (int kk = kBlockK / 16 - 1; kk >= 0; --kk) {
                             const uint64_t adv = static_cast<uint64_t>((kk * 32) >> 4);   // +32 B per K=16
                             // small cross terms first, the dominant hi*hi product last
-                            if (ti.nA == 2) { ptx::mma_f16_ss(d_tmem, a_lo + adv, b_hi + adv, idesc, accumulate); accumulate = 1; }
-                            if (ti.nB == 2) { ptx::mma_f16_ss(d_tmem, a_hi + adv, b_lo + adv, idesc, accumulate); accumulate = 1; }
-                            ptx::mma_f16_ss(d_tmem, a_hi + adv, b_hi + adv, idesc, accumulate);
+                            if (ti.nA == 2) { mma(d_tmem, a_lo + adv, b_hi + adv, accumulate); accumulate = 1; }
+                            if (ti.nB == 2) { mma(d_tmem, a_hi + adv, b_lo + adv, accumulate); accumulate = 1; }
+                            mma(d_tmem, a_hi + adv, b_hi + adv, accumulate);
                             accumulate = 1;
                         }
-                        ptx::tc_commit(empty_bar(stage));            // smem slot free when MMAs retire
-                        if (++stage == kStages) { stage = 0; phase ^= 1u; }
+                        commit(empty_bar(stage));                    // smem slot free (in both CTAs) when MMAs retire
+                        if (++stage == NS) { stage = 0; phase ^= 1u; }
                     }
                 }
-                ptx::tc_commit(tfull_bar(buf));                      // accumulator complete
+                commit(tfull_bar(buf));                              // accumulator complete
                 if (++buf == kAccBufs) { buf = 0; acc_phase ^= 1u; }
             }
         }
@@ -307,9 +330,13 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_constant
         const int nsub = op.nb / kBlk;
         int buf = 0;
         uint32_t acc_phase = 0;
-        for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
-            const int rb = op.rb0 + t / op.ncb, cb = op.cb0 + t % op.ncb;
-            if (tile_is_skipped(op, rb, cb)) continue;
+        for (int t = unit0; t < ntiles; t += nunits) {
+            const int rb = op.rb0 + (t / ncbu) * CG + rank, cb0u = op.cb0 + (t % ncbu) * CG;
+            if (tile_is_skipped(op, rb - rank + CG - 1, cb0u)) continue;
+#pragma unroll 1
+          for (int j2 = 0; j2 < CG; ++j2) {                       // the unit's column blocks, one after the other
+            const int cb = cb0u + j2;
+            const bool dead = tile_is_skipped(op, rb, cb);        // this CTA's block lies above the diagonal: nothing to store
             const int row_in_blk = q * 32 + lane;
             const int col0 = cb * kBlk + 64 * hf;                 // first column (inside the tile column) of this warp
             float* wblk = op.W + (static_cast<int64_t>(rb) * nsub + cb) * (kBlk * kBlk) + static_cast<int64_t>(64 * hf) * kBlk + row_in_blk;
@@ -317,7 +344,10 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_constant
             float bs[64];
             const bool base_from_w = (op.mode == MODE_P1) || (op.mode == MODE_UPDATE && op.base_w);
             const bool base_from_a = (op.mode == MODE_UPDATE && !op.base_w);
-            if (base_from_w) {
+            if (dead) {
+#pragma unroll
+                for (int e = 0; e < 64; ++e) bs[e] = 0.0f;
+            } else if (base_from_w) {
 #pragma unroll
                 for (int e = 0; e < 64; ++e) bs[e] = wblk[e * kBlk];
             } else if (base_from_a) {
@@ -347,17 +377,21 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_constant
             const float plane_mul = (op.mode == MODE_P3) ? op.scl[0] : op.scl[1];
             float out[64];
             if (has_acc) {
-                ptx::mbar_wait(tfull_bar(buf), acc_phase);
+                if (j2 == 0) ptx::mbar_wait(tfull_bar(buf), acc_phase);
                 ptx::tc_fence_after();
                 uint32_t a0[32], a1[32];
-                const uint32_t taddr = tmem_base + buf * kAccCols + (static_cast<uint32_t>(q * 32) << 16) + 64 * hf;
+                const uint32_t taddr = tmem_base + buf * kAccW + (static_cast<uint32_t>(q * 32) << 16) + kAccCols * j2 + 64 * hf;
                 ptx::tmem_ld_32x32(taddr, a0);
                 ptx::tmem_ld_32x32(taddr + 32, a1);
                 ptx::tmem_ld_wait();
                 ptx::tc_fence_before();
                 __syncwarp();
-                if (lane == 0) ptx::mbar_arrive(tempty_bar(buf));          // accumulator is in registers
-                if (++buf == kAccBufs) { buf = 0; acc_phase ^= 1u; }
+                if (j2 == CG - 1) {
+                    if (lane == 0) {                                        // accumulator is in registers
+                        if (CG == 2) ptx::mbar_arrive_leader(tempty_bar(buf)); else ptx::mbar_arrive(tempty_bar(buf));
+                    }
+                    if (++buf == kAccBufs) { buf = 0; acc_phase ^= 1u; }
+                }
 #pragma unroll
                 for (int e = 0; e < 32; ++e) {
                     out[e] = fmaf(-__uint_as_float(a0[e]), acc_mul, bs[e]);
@@ -367,6 +401,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_constant
 #pragma unroll
                 for (int e = 0; e < 64; ++e) out[e] = bs[e];
             }
+            if (dead) continue;
 #pragma unroll
             for (int e = 0; e < 64; ++e) wblk[e * kBlk] = out[e];
             float amax = 0.0f;
@@ -406,13 +441,14 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_constant
                     atomicMax(reinterpret_cast<int*>(op.tile_amax + slot), __float_as_int(amax));
                 }
             }
+          }   // j2
         }
     }
 
     // teardown
     ptx::tc_fence_before();
-    __syncthreads();
-    if (warp == 1) ptx::tmem_dealloc<kTmemCols>(tmem_base);
+    if (CG == 2) ptx::cluster_sync_all(); else __syncthreads();
+    if (warp == 1) ptx::tmem_dealloc<kTmemCols, CG>(tmem_base);
 }
 
 }  // namespace krr

@@ -139,6 +139,30 @@ def test_lookahead_pipeline_matches_serial_schedule(krr):
         assert relF(Lg, Lo) <= 1e-4 and backward_error(An, Lg) <= 1e-6
 
 
+@pytest.mark.parametrize("prec", ["fp32", "mixed"])
+def test_cta_pair_updates_match_single_cta(krr, prec):
+    """Trailing updates on CTA pairs (cta_group::2, 256x128 blocks, default when nb % 256 == 0) against
+    KRR_FLAG_NO_CTA_PAIRS: the same products in the same order."""
+    cfg = replace(scaled_config(CONFIGS["S1"], nb=256, n=2560, p=1536), genotype="maf", gamma_scale=4.0)
+    A, _ = make_problem(cfg, device="cuda")
+    pmap = oracle_uniform(cfg.NT, R.FP32)
+    if prec == "mixed":
+        rng = np.random.default_rng(3)
+        for i in range(cfg.NT):
+            for j in range(i):
+                pmap[i, j] = rng.integers(0, 3)
+    h = torch.from_numpy(np.ascontiguousarray(pmap))
+    F1 = krr.potrf_mp(A, cfg.nb, h.cuda(), h, flags=krr.FLAG_PREROUND_A)
+    F2 = krr.potrf_mp(A, cfg.nb, h.cuda(), h, flags=krr.FLAG_PREROUND_A | krr.FLAG_NO_CTA_PAIRS)
+    torch.cuda.synchronize()
+    assert int(F1.info.item()) == 0 and int(F2.info.item()) == 0
+    L1, L2 = F1.dense().cpu().numpy(), F2.dense().cpu().numpy()
+    print(f"pairs vs single ({prec}): relF {relF(L1, L2):.3e} equal fraction {np.mean(L1 == L2):.4f}")
+    Lo, floor = noise_floor(A.cpu().numpy(), cfg.nb, pmap, True)
+    assert relF(L1, L2) <= max(1e-5, 2.0 * floor)
+    assert relF(L1, Lo) <= max(1e-4, 2.0 * floor)
+
+
 # ------------------------------------------------------------------------------ low-precision maps
 def noise_floor(An, nb, pmap, preround, seed=0):
     """The oracle against itself on an input perturbed at the level of the CUDA path's FP32-class

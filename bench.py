@@ -358,7 +358,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="C3", choices=sorted(CONFIGS))
-    ap.add_argument("--sample-tiles", type=int, default=20, help="tiles per dimension of the CPU-oracle sample")
+    ap.add_argument("--sample-tiles", type=int, default=28, help="tiles per dimension of the CPU-oracle sample")
     ap.add_argument("--potrf-flags", type=int, default=0, help="extra KRR_FLAG_* bits for krr_potrf_mp (experiments)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -182,6 +182,9 @@ CONFIGS = {
                   map_request="fp8_col0_fp32", allowed=(0, 2)),
     # supplementary: the paper's regime K ~ I (gamma = 12/p) with two families of
     # relatives -- the only input on which the rule yields a genuine FP32/FP16/FP8 mosaic
+    # class probes: C3's matrix with every off-diagonal tile forced to one storage precision (kernel
+    # efficiency per MMA class at full depth; numerics are those of the forced map, reported as they are)
+    "C3h": Config("C3h", 65536, 50000, 1024, 1e-2, 16, seed=3, map_request="force_fp16", allowed=(0, 1)),
     "S1": Config("S1", 32768, 24576, 1024, 1e-2, 8, seed=6, genotype="families:4096",
                  map_request="rule", eps_target=1e-4, allowed=(0, 1, 2), gamma_scale=12.0),
 }
@@ -197,19 +200,57 @@ def scaled_config(cfg, nb, n=None, p=None):
     return replace(cfg, name=f"{cfg.name}@n{n}", n=n, p=p, nb=nb, genotype=geno)
 
 
+def _all_genotypes(cfg, device):
+    if cfg.n * cfg.p <= (1 << 31):
+        return genotypes(cfg.seed, cfg.n, cfg.p, cfg.genotype, device)
+    G = torch.empty((cfg.n, cfg.p), dtype=torch.int8, device=device)
+    step = max(1, (1 << 28) // cfg.p)
+    for r0 in range(0, cfg.n, step):
+        r = min(step, cfg.n - r0)
+        G[r0:r0 + r] = genotypes(cfg.seed, cfg.n, cfg.p, cfg.genotype, device, r0, r)
+    return G
+
+
 def make_problem(cfg, device="cpu", row_block=4096):
     """(A FP32 n x n, Y FP32 n x nrhs) for a Config."""
-    if cfg.n * cfg.p <= (1 << 31):
-        G = genotypes(cfg.seed, cfg.n, cfg.p, cfg.genotype, device)
-    else:
-        G = torch.empty((cfg.n, cfg.p), dtype=torch.int8, device=device)
-        step = max(1, (1 << 28) // cfg.p)
-        for r0 in range(0, cfg.n, step):
-            r = min(step, cfg.n - r0)
-            G[r0:r0 + r] = genotypes(cfg.seed, cfg.n, cfg.p, cfg.genotype, device, r0, r)
+    G = _all_genotypes(cfg, device)
     A = kernel_matrix(G, cfg.gamma, cfg.lam, row_block=row_block)
     Y = phenotypes(cfg.seed, cfg.n, cfg.nrhs, device)
     return A, Y
+
+
+def kernel_matrix_lower_tiles(G, gamma, lam, nb):
+    """The lower tiles of A = K + lam*I packed one after the other in column-major tile order
+    (tile (i,j), i >= j, at slot j*NT - j(j-1)/2 + (i-j); each tile row-major nb x nb): the
+    "lower-triangular tile storage only" layout of config C4.  Same values as kernel_matrix."""
+    n, p = G.shape
+    assert n % nb == 0 and 4 * p < 2 ** 24
+    NT = n // nb
+    dev = G.device
+    s = (G.to(torch.float32) ** 2).sum(dim=1).to(torch.float64)
+    out = torch.empty((NT * (NT + 1) // 2, nb, nb), dtype=torch.float32, device=dev)
+    diag = torch.tensor(1.0 + lam, dtype=torch.float64).to(torch.float32).to(dev)
+    idx = torch.arange(nb, device=dev)
+    slot = 0
+    for j in range(NT):
+        Gj = G[j * nb:(j + 1) * nb]
+        for i0 in range(j, NT, 8):                        # 8 tile rows at a time
+            i1 = min(NT, i0 + 8)
+            d2 = s[i0 * nb:i1 * nb, None] + s[None, j * nb:(j + 1) * nb] - 2.0 * _gram_int(G[i0 * nb:i1 * nb], Gj)
+            blk = torch.exp(-gamma * d2).to(torch.float32).reshape(i1 - i0, nb, nb)
+            if i0 == j:
+                blk[0, idx, idx] = diag
+            out[slot:slot + (i1 - i0)] = blk
+            slot += i1 - i0
+    return out.reshape(-1)
+
+
+def make_problem_lower_tiles(cfg, device="cpu"):
+    """(packed lower tiles of A, Y) for a Config -- never materialises the n x n matrix."""
+    G = _all_genotypes(cfg, device)
+    At = kernel_matrix_lower_tiles(G, cfg.gamma, cfg.lam, cfg.nb)
+    Y = phenotypes(cfg.seed, cfg.n, cfg.nrhs, device)
+    return At, Y
 
 
 def exact_lower_factor(seed, n, nb, nnz_per_row=2, device="cpu"):

@@ -195,13 +195,12 @@ static int launch(int cat, K kernel, dim3 grid, dim3 block, size_t smem, cudaStr
 // and the E4M3 images.
 struct GemmMaps { CUtensorMap H, L, Hh, Lh, IH, IL, Q, Qh; };
 
-// cg = 2 runs MODE_UPDATE on CTA pairs (256 x 256 output blocks); needs even block counts and no FP8 images.
+// cg = 2 runs MODE_UPDATE on CTA pairs (256 x 256 output blocks); needs even block counts.
 static int launch_gemm(const GemmMaps& m, const GemmOp& op, int max_ctas, int cg, cudaStream_t st) {
     if (op.nrb <= 0 || op.ncb <= 0) return KRR_OK;
     ProfScope ps(op.mode == MODE_UPDATE ? CAT_UPDATE : (op.mode == MODE_P1 ? CAT_P1 : CAT_P3), st);
     ++g_launches;
-    if (cg == 2 && op.mode == MODE_UPDATE && op.nrb % 2 == 0 && op.rb0 % 2 == 0 && op.ncb % 2 == 0 && op.cb0 % 2 == 0 &&
-        !op.fp8q) {
+    if (cg == 2 && op.mode == MODE_UPDATE && op.nrb % 2 == 0 && op.rb0 % 2 == 0 && op.ncb % 2 == 0 && op.cb0 % 2 == 0) {
         const int npairs = (op.nrb / 2) * (op.ncb / 2);
         const int max_pairs = max_ctas / 2;
         const int grid = 2 * (npairs < max_pairs ? npairs : max_pairs);

@@ -20,10 +20,15 @@
 // FP8 x FP8 terms (both operand tiles stored as E4M3 with power-of-two tile scales) run as
 // kind::mxf8f6f4.block_scale MMAs on the 1-byte images (Qp plane, K = 128 per 16 KB smem block): the
 // per-tile scale times the plane scale sx is a power of two, i.e. a UE8M0 block scale that is the same
-// for every row and every K block of the tile.  TMEM columns 256.. hold a table of 64 constant scale
-// vectors (entry j: every byte = kSfBias + j); an MMA just points its scale operands at the two
+// for every row and every K block of the tile.  TMEM columns 256.. hold a table of constant scale
+// vectors (entry j: every byte = sf_bias + j); an MMA just points its scale operands at the two
 // entries of its tiles, so no scale data is ever staged.  Tiles whose exponent falls outside the
 // table (never seen on the workloads) take the FP16 path through their hi image, which is exact too.
+//
+// Shared-memory ring: 6 slots of 32 KB = [one 16 KB block of A | one of B].  A K chunk of an
+// FP16-class or FP8 term occupies one slot, of an FP32-class term two (hi images, then lo images), so
+// the low-precision classes -- whose MMAs consume a slot in a quarter of the time -- get a six-deep
+// prefetch, the FP32 class three.
 //
 // Accumulation order: the tensor core adds each MMA's result to the TMEM accumulator with
 // truncation, a bias of ~half an ulp OF THE ACCUMULATOR per instruction (measured: backward error
@@ -63,77 +68,88 @@ struct GemmOp {
     unsigned flags;
 };
 
-constexpr int kStages = 3;
+constexpr int kSlots = 6;                          // shared-memory ring: 6 slots of [A block | B block]
 constexpr int kBlockK = 64;                        // fp16 elements per 128-byte swizzle row
-constexpr int kPlaneBytes = kBlk * kBlockK * 2;    // one 128 x 64 fp16 operand block = 16 KB
-constexpr int kStageBytes = 4 * kPlaneBytes;       // A_hi, A_lo, B_hi, B_lo
+constexpr int kPlaneBytes = kBlk * kBlockK * 2;    // one 128 x 64 fp16 (or 128 x 128 E4M3) operand block = 16 KB
+constexpr int kSlotBytes = 2 * kPlaneBytes;        // one plane of A and one of B.  A K chunk takes one slot
+                                                   // (hi images / E4M3 images) or two (hi, then lo images)
 constexpr int kAccCols = 128;                      // TMEM columns of one 128x128 FP32 accumulator
-constexpr int kAccBufs = 2;
-constexpr int kSfCol0 = kAccCols * kAccBufs;       // first TMEM column of the scale table
-constexpr int kSfEntries = 64;                     // 4 columns each
-constexpr int kSfBias = 127 - 40;                  // entry j <-> UE8M0 byte kSfBias + j, i.e. 2^(j - 40)
-constexpr int kTmemCols = 512;                     // 2 accumulators + scale table
+constexpr int kMaxAccBufs = 2;
+constexpr int kSfCol0 = 256;                       // first TMEM column of the scale table
+constexpr int kSfCols = 256;                       // table: 256 / (4 CG) entries of 4 CG columns
+constexpr int kTmemCols = 512;                     // accumulators + scale table
+// entry j <-> UE8M0 byte sf_bias + j: CG = 1: 64 entries, 2^-40 .. 2^23; CG = 2: 32 entries, 2^-24 .. 2^7
+__host__ __device__ constexpr int sf_entries(int cg) { return kSfCols / (4 * cg); }
+__host__ __device__ constexpr int sf_bias(int cg) { return cg == 1 ? 127 - 40 : 127 - 24; }
 constexpr int kGemmThreads = 320;                  // warp 0 TMA, warp 1 MMA (+TMEM alloc), 2-9 epilogue
 constexpr int kEpiWarps = 8;
 constexpr int kEpiRowBytes = 80;                   // 64 B of FP16 per row + 16 B pad (conflict-free 16 B accesses)
 constexpr int kEpiStageBytes = 32 * kEpiRowBytes;  // per-warp transpose buffer
-constexpr int kGemmSmem = kStages * kStageBytes + 1024 /*align*/ + 256 /*barriers*/ + kEpiWarps * kEpiStageBytes;
+constexpr int kGemmSmem = kSlots * kSlotBytes + 1024 /*align*/ + 256 /*barriers*/ + kEpiWarps * kEpiStageBytes;
 
-struct TermInfo {
-    int64_t a_row, b_row;   // plane rows (TMA coordinate 1)
+// One term of an output block's sum = one tile product (MODE_UPDATE) or the single in-panel product.
+// Geometry (plane rows / first K column / K extent) is arithmetic on launch parameters and block
+// indices -- warp-uniform by construction.  The MMA class of the term comes from the device-resident
+// map and tile scales; it is fetched as one packed word and made provably uniform with a warp
+// reduction (REDUX writes a uniform register), so that the issue loops below compile to uniform-
+// datapath code around the single elected lane that issues TMA / tcgen05 instructions.
+struct TermGeom {
+    int a_row, b_row;       // plane rows (TMA coordinate 1)
     int a_k0, b_k0;         // first K column (TMA coordinate 0)
-    int nchunks;            // K chunks of 64
-    int nA, nB;             // planes per operand: 2 = hi+lo (FP32 class), 1 = hi only
-    int q;                  // 1: FP8 x FP8 term on the E4M3 images (K chunks of 128, block-scaled MMA)
-    int sfa, sfb;           // scale-table entries of the two tiles (q = 1)
+    int kelems;             // K extent in elements
 };
+
+// class word: bit 0: A operand has a lo image (FP32 tile), bit 1: B has one, bit 2: FP8 x FP8 term on the
+// E4M3 images (K chunks of 128, block-scaled MMA), bits 8-13 / 16-21: scale-table entries of the two tiles
+constexpr uint32_t kClsALo = 1u, kClsBLo = 2u, kClsQ = 4u;
 
 // UE8M0 byte of the power of two x (> 0, normal): its biased exponent.
 __device__ __forceinline__ int pow2_exponent_byte(float x) { return static_cast<int>((__float_as_uint(x) >> 23) & 0xffu); }
 
-__device__ __forceinline__ TermInfo get_term(const GemmOp& op, int s /* term index */, int rb, int cb) {
-    TermInfo t;
-    t.q = 0; t.sfa = 0; t.sfb = 0;
+__device__ __forceinline__ TermGeom term_geom(const GemmOp& op, int s /* term index */, int rb, int cb) {
+    TermGeom t;
     if (op.mode == MODE_UPDATE) {
         const int i = op.k + (rb * kBlk) / op.nb;
         const int subrow = (rb * kBlk) % op.nb;
         s += op.s_lo;
-        t.a_row = tile_slot(op.NT, i, s) * op.nb + subrow;
-        t.b_row = tile_slot(op.NT, op.k, s) * op.nb + cb * kBlk;
+        t.a_row = static_cast<int>(tile_slot(op.NT, i, s) * op.nb + subrow);
+        t.b_row = static_cast<int>(tile_slot(op.NT, op.k, s) * op.nb + cb * kBlk);
         t.a_k0 = 0;
         t.b_k0 = 0;
-        t.nchunks = op.nb / kBlockK;
-        const int pa = op.map[i * op.NT + s], pb = op.map[op.k * op.NT + s];
-        t.nA = (pa == KRR_FP32) ? 2 : 1;
-        t.nB = (pb == KRR_FP32) ? 2 : 1;
-        if (op.fp8q && pa == KRR_FP8_E4M3 && pb == KRR_FP8_E4M3) {
-            const float sx = op.scl[0];
-            t.sfa = pow2_exponent_byte(sx * op.scales[i * op.NT + s]) - kSfBias;
-            t.sfb = pow2_exponent_byte(sx * op.scales[op.k * op.NT + s]) - kSfBias;
-            if (t.sfa >= 0 && t.sfa < kSfEntries && t.sfb >= 0 && t.sfb < kSfEntries) {
-                t.q = 1;
-                t.nchunks = op.nb / 128;
-            }
-        }
+        t.kelems = op.nb;
     } else if (op.mode == MODE_P1) {
-        t.a_row = op.prow0 + static_cast<int64_t>(rb) * kBlk;
-        t.b_row = op.prow0 + static_cast<int64_t>(op.c) * kBlk;
+        t.a_row = static_cast<int>(op.prow0) + rb * kBlk;
+        t.b_row = static_cast<int>(op.prow0) + op.c * kBlk;
         t.a_k0 = 0;
         t.b_k0 = 0;
-        t.nchunks = op.c * (kBlk / kBlockK);
-        t.nA = 2;
-        t.nB = 2;
+        t.kelems = op.c * kBlk;
     } else {
-        t.a_row = op.prow0 + static_cast<int64_t>(rb) * kBlk;
-        t.b_row = static_cast<int64_t>(op.c) * kBlk;      // row in the Linv planes
+        t.a_row = static_cast<int>(op.prow0) + rb * kBlk;
+        t.b_row = op.c * kBlk;                             // row in the Linv planes
         t.a_k0 = op.c * kBlk;
         t.b_k0 = 0;
-        t.nchunks = kBlk / kBlockK;
-        t.nA = 2;
-        t.nB = 2;
+        t.kelems = kBlk;
     }
     return t;
 }
+
+template <int CG>
+__device__ __forceinline__ uint32_t term_class_load(const GemmOp& op, int s /* term index */, int rb) {
+    if (op.mode != MODE_UPDATE) return kClsALo | kClsBLo;
+    const int i = op.k + (rb * kBlk) / op.nb;
+    s += op.s_lo;
+    const int pa = op.map[i * op.NT + s], pb = op.map[op.k * op.NT + s];
+    uint32_t w = (pa == KRR_FP32 ? kClsALo : 0u) | (pb == KRR_FP32 ? kClsBLo : 0u);
+    if (op.fp8q && pa == KRR_FP8_E4M3 && pb == KRR_FP8_E4M3) {
+        const float sx = op.scl[0];
+        const int sfa = pow2_exponent_byte(sx * op.scales[i * op.NT + s]) - sf_bias(CG);
+        const int sfb = pow2_exponent_byte(sx * op.scales[op.k * op.NT + s]) - sf_bias(CG);
+        if (sfa >= 0 && sfa < sf_entries(CG) && sfb >= 0 && sfb < sf_entries(CG))
+            w |= kClsQ | (static_cast<uint32_t>(sfa) << 8) | (static_cast<uint32_t>(sfb) << 16);
+    }
+    return w;
+}
+__device__ __forceinline__ uint32_t make_uniform(uint32_t w) { return __reduce_max_sync(0xffffffffu, w); }
 
 __device__ __forceinline__ int num_terms(const GemmOp& op) {
     return op.mode == MODE_UPDATE ? (op.s_hi - op.s_lo) : 1;
@@ -147,27 +163,26 @@ __device__ __forceinline__ bool tile_is_skipped(const GemmOp& op, int rb, int cb
 // CG = 1: one CTA per 128x128 output block.  CG = 2 (MODE_UPDATE only): a CTA pair (cluster of 2,
 // tcgen05 cta_group::2) per 256x256 block -- each CTA stages its own 128 rows of A and the 128 rows of
 // B of ONE of the two column blocks, the leader issues M = 256, N = 256 MMAs that read both CTAs'
-// shared memory, and each CTA's TMEM receives its own 128 rows x 256 columns of the accumulator (two
-// buffers fill the 512 TMEM columns, so this variant has no scale table: FP8 pairs go through their
-// FP16 images, or the host picks CG = 1).  Per flop it moves half the operand bytes of CG = 1.
+// shared memory, and each CTA's TMEM receives its own 128 rows x 256 columns of the accumulator.  Two
+// such buffers fill the 512 TMEM columns; when the map holds FP8 tiles the upper 256 columns carry the
+// scale table instead and the pair works with a single accumulator (the epilogue of a block is then
+// not overlapped with the next block's MMAs: a few % at the K depths of a trailing update).
+// Per flop a pair moves half the operand bytes of CG = 1.
 template <int CG>
 __global__ void __launch_bounds__(kGemmThreads, 1)
 gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_constant__ CUtensorMap tmA_lo,
                const __grid_constant__ CUtensorMap tmB_hi, const __grid_constant__ CUtensorMap tmB_lo,
                const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmQb, const GemmOp op) {
-    constexpr uint32_t kBBytes = kPlaneBytes;           // this CTA's B block: 128 rows
-    constexpr int NS = kStages;
-    constexpr uint32_t SB = 2 * kPlaneBytes + 2 * kBBytes;      // A_hi, A_lo, B_hi, B_lo
-    static_assert(NS * SB <= kStages * kStageBytes && NS <= 4, "smem ring");
+    constexpr uint32_t SB = kSlotBytes;                 // [A block 16 KB | B block 16 KB]
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
-    const uint32_t bar_base = smem_base + kStages * kStageBytes;
-    // barriers: full[kStages], empty[kStages], tmem_full[kAccBufs], tmem_empty[kAccBufs], tmem ptr
+    const uint32_t bar_base = smem_base + kSlots * kSlotBytes;
+    // barriers: full[8], empty[8], tmem_full[2], tmem_empty[2], tmem ptr
     auto full_bar = [&](int s) { return bar_base + 8u * s; };
-    auto empty_bar = [&](int s) { return bar_base + 8u * (4 + s); };
-    auto tfull_bar = [&](int b) { return bar_base + 8u * (8 + b); };
-    auto tempty_bar = [&](int b) { return bar_base + 8u * (8 + kAccBufs + b); };
-    const uint32_t tmem_slot = bar_base + 8u * (8 + 2 * kAccBufs);
+    auto empty_bar = [&](int s) { return bar_base + 8u * (8 + s); };
+    auto tfull_bar = [&](int b) { return bar_base + 8u * (16 + b); };
+    auto tempty_bar = [&](int b) { return bar_base + 8u * (16 + kMaxAccBufs + b); };
+    const uint32_t tmem_slot = bar_base + 8u * (16 + 2 * kMaxAccBufs);
     uint32_t* tmem_slot_ptr = reinterpret_cast<uint32_t*>(smem_raw + (tmem_slot - ptx::smem_u32(smem_raw)));
 
     const int warp = threadIdx.x >> 5;
@@ -179,6 +194,9 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_constant
     const int ntiles = (op.nrb / CG) * ncbu;            // output blocks of (128*CG) x (128*CG)
     constexpr int kAccW = kAccCols * CG;                // accumulator columns per buffer
     const int nterms = num_terms(op);
+    const bool use_sf = op.fp8q && op.mode == MODE_UPDATE;
+    // a pair's 256-column accumulators fill TMEM: with the scale table present there is room for one only
+    const int nbufs = (CG == 2 && use_sf) ? 1 : kMaxAccBufs;
 
     const bool has_acc = (op.mode != MODE_UPDATE) ? (op.mode == MODE_P3 || op.c > 0) : (nterms > 0);
     const bool write_planes = (op.mode != MODE_UPDATE) || op.planes;
@@ -189,11 +207,11 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_constant
         ptx::prefetch_tmap(&tmB_hi);
         ptx::prefetch_tmap(&tmB_lo);
         if (op.fp8q) { ptx::prefetch_tmap(&tmQ); ptx::prefetch_tmap(&tmQb); }
-        for (int s = 0; s < NS; ++s) {
+        for (int s = 0; s < kSlots; ++s) {
             ptx::mbar_init(full_bar(s), 1);
             ptx::mbar_init(empty_bar(s), 1);
         }
-        for (int b = 0; b < kAccBufs; ++b) {
+        for (int b = 0; b < kMaxAccBufs; ++b) {
             ptx::mbar_init(tfull_bar(b), 1);
             ptx::mbar_init(tempty_bar(b), kEpiWarps * CG);
         }
@@ -207,12 +225,14 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_constant
     if (CG == 2) ptx::cluster_sync_all(); else __syncthreads();     // peer barriers are initialised too
     ptx::tc_fence_after();
     const uint32_t tmem_base = *tmem_slot_ptr;
-    if (CG == 1 && op.fp8q && op.mode == MODE_UPDATE) {
-        // scale table: entry j = 4 TMEM columns whose every byte is the UE8M0 code kSfBias + j
-        if (warp >= 2) {
+    if (use_sf) {
+        // scale table: entry j = 4 CG TMEM columns whose every byte is the UE8M0 code sf_bias + j (an MMA
+        // of a pair reads the scales of its 256 B rows from 8 columns, of its 128 A rows from 4)
+        if (warp >= 2 && warp < 6) {
             const uint32_t lane_base = static_cast<uint32_t>((warp & 3) * 32) << 16;
-            for (int j = 0; j < kSfEntries; ++j)
-                ptx::tmem_st_32x32_x4(tmem_base + lane_base + kSfCol0 + 4 * j, static_cast<uint32_t>(kSfBias + j) * 0x01010101u);
+            for (int j = 0; j < kSfCols / 4; ++j)
+                ptx::tmem_st_32x32_x4(tmem_base + lane_base + kSfCol0 + 4 * j,
+                                      static_cast<uint32_t>(sf_bias(CG) + j / CG) * 0x01010101u);
             ptx::tmem_st_wait();
         }
         ptx::tc_fence_before();
@@ -221,9 +241,9 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_constant
     }
 
     if (warp == 0) {
-        // ===================== TMA producer =====================
-        if (lane == 0 && has_acc) {
-            int stage = 0;
+        // ===================== TMA producer (whole warp in uniform control flow; one elected lane issues) ====
+        if (has_acc) {
+            int slot = 0;
             uint32_t phase = 0;
             auto load = [&](uint32_t dst, const CUtensorMap* m, uint32_t bar, int c0, int c1) {
                 if (CG == 2) ptx::tma_load_2d_pair(dst, m, bar, c0, c1); else ptx::tma_load_2d(dst, m, bar, c0, c1);
@@ -231,90 +251,147 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_constant
             for (int t = unit0; t < ntiles; t += nunits) {
                 const int rb = op.rb0 + (t / ncbu) * CG + rank, cb0u = op.cb0 + (t % ncbu) * CG;
                 if (tile_is_skipped(op, rb - rank + CG - 1, cb0u)) continue;    // the whole (pair) block lies above the diagonal
+                uint32_t cls_next = term_class_load<CG>(op, nterms - 1, rb);
                 for (int s = nterms - 1; s >= 0; --s) {      // descending K: see note on accumulation order
-                    const TermInfo ti = get_term(op, s, rb, cb0u + rank);        // this CTA's A rows and B rows
-                    // bytes landing under the leader's barrier: both CTAs' A blocks and B halves
-                    const uint32_t bytes = ti.q ? CG * (kPlaneBytes + kBBytes)
-                                                : CG * (static_cast<uint32_t>(ti.nA) * kPlaneBytes + static_cast<uint32_t>(ti.nB) * kBBytes);
-                    const int b_row = static_cast<int>(ti.b_row);
-                    for (int ch = ti.nchunks - 1; ch >= 0; --ch) {
-                        ptx::mbar_wait(empty_bar(stage), phase ^ 1u);
-                        const uint32_t sa = smem_base + stage * SB;
-                        if (rank == 0) ptx::mbar_arrive_expect_tx(full_bar(stage), bytes);
-                        if (ti.q) {      // E4M3 images: 128 bytes of K per row
-                            load(sa, &tmQ, full_bar(stage), ch * 128, static_cast<int>(ti.a_row));
-                            load(sa + 2 * kPlaneBytes, &tmQb, full_bar(stage), ch * 128, b_row);
-                            if (++stage == NS) { stage = 0; phase ^= 1u; }
-                            continue;
+                    const uint32_t cls = make_uniform(cls_next);
+                    if (s > 0) cls_next = term_class_load<CG>(op, s - 1, rb);   // in flight during this term's chunks
+                    const TermGeom g = term_geom(op, s, rb, cb0u + rank);       // this CTA's A rows and B rows
+                    if (cls & kClsQ) {                       // E4M3 images: 128 bytes of K per row, one slot per chunk
+                        for (int ch = g.kelems / 128 - 1; ch >= 0; --ch) {
+                            ptx::mbar_wait(empty_bar(slot), phase ^ 1u);
+                            if (ptx::elect_one()) {
+                                const uint32_t sa = smem_base + slot * SB;
+                                if (rank == 0) ptx::mbar_arrive_expect_tx(full_bar(slot), CG * 2u * kPlaneBytes);
+                                load(sa, &tmQ, full_bar(slot), ch * 128, g.a_row);
+                                load(sa + kPlaneBytes, &tmQb, full_bar(slot), ch * 128, g.b_row);
+                            }
+                            if (++slot == kSlots) { slot = 0; phase ^= 1u; }
                         }
-                        const int ak = ti.a_k0 + ch * kBlockK, bk = ti.b_k0 + ch * kBlockK;
-                        load(sa, &tmA_hi, full_bar(stage), ak, static_cast<int>(ti.a_row));
-                        if (ti.nA == 2) load(sa + kPlaneBytes, &tmA_lo, full_bar(stage), ak, static_cast<int>(ti.a_row));
-                        load(sa + 2 * kPlaneBytes, &tmB_hi, full_bar(stage), bk, b_row);
-                        if (ti.nB == 2) load(sa + 2 * kPlaneBytes + kBBytes, &tmB_lo, full_bar(stage), bk, b_row);
-                        if (++stage == NS) { stage = 0; phase ^= 1u; }
+                        continue;
+                    }
+                    const bool a_lo = cls & kClsALo, b_lo = cls & kClsBLo;
+                    const uint32_t lo_bytes = CG * ((a_lo ? 1u : 0u) + (b_lo ? 1u : 0u)) * kPlaneBytes;
+                    for (int ch = g.kelems / kBlockK - 1; ch >= 0; --ch) {
+                        const int ak = g.a_k0 + ch * kBlockK, bk = g.b_k0 + ch * kBlockK;
+                        ptx::mbar_wait(empty_bar(slot), phase ^ 1u);
+                        if (ptx::elect_one()) {              // hi images
+                            const uint32_t sa = smem_base + slot * SB;
+                            if (rank == 0) ptx::mbar_arrive_expect_tx(full_bar(slot), CG * 2u * kPlaneBytes);
+                            load(sa, &tmA_hi, full_bar(slot), ak, g.a_row);
+                            load(sa + kPlaneBytes, &tmB_hi, full_bar(slot), bk, g.b_row);
+                        }
+                        if (++slot == kSlots) { slot = 0; phase ^= 1u; }
+                        if (lo_bytes) {                      // lo images of the FP32-class operand(s)
+                            ptx::mbar_wait(empty_bar(slot), phase ^ 1u);
+                            if (ptx::elect_one()) {
+                                const uint32_t sa = smem_base + slot * SB;
+                                if (rank == 0) ptx::mbar_arrive_expect_tx(full_bar(slot), lo_bytes);
+                                if (a_lo) load(sa, &tmA_lo, full_bar(slot), ak, g.a_row);
+                                if (b_lo) load(sa + kPlaneBytes, &tmB_lo, full_bar(slot), bk, g.b_row);
+                            }
+                            if (++slot == kSlots) { slot = 0; phase ^= 1u; }
+                        }
                     }
                 }
             }
         }
     } else if (warp == 1) {
-        // ===================== MMA issuer (one thread) =====================
-        if (lane == 0 && has_acc && rank == 0) {
+        // ===================== MMA issuer (whole warp in uniform control flow; one elected lane issues) =====
+        if (has_acc && rank == 0) {
             constexpr uint32_t idesc = ptx::make_idesc(kBlk * CG, kBlk * CG, /*F16*/ 0, /*F16*/ 0);
             constexpr uint32_t idesc_q = ptx::make_idesc_mxf8(kBlk * CG, kBlk * CG);
-            auto mma = [&](uint32_t d, uint64_t a, uint64_t b, uint32_t acc) {
+            auto mma = [&](uint32_t d, uint32_t a_lo32, uint32_t b_lo32, uint32_t acc) {
+                const uint64_t a = ptx::smem_desc_from_lo(a_lo32), b = ptx::smem_desc_from_lo(b_lo32);
                 if (CG == 2) ptx::mma_f16_ss_pair(d, a, b, idesc, acc); else ptx::mma_f16_ss(d, a, b, idesc, acc);
             };
             auto commit = [&](uint32_t bar) { if (CG == 2) ptx::tc_commit_pair(bar); else ptx::tc_commit(bar); };
-            int stage = 0;
+            // low word of the descriptor of ring slot c's A block; the B block is 16 KB (1024 x 16 B) further
+            const uint32_t dlo0 = ptx::smem_desc_lo(smem_base);
+            constexpr uint32_t kDescSlot = SB >> 4, kDescB = kPlaneBytes >> 4;
+            int slot = 0;
             uint32_t phase = 0;
             int buf = 0;
             uint32_t acc_phase = 0;
             for (int t = unit0; t < ntiles; t += nunits) {
                 const int rb = op.rb0 + (t / ncbu) * CG, cb = op.cb0 + (t % ncbu) * CG;
                 if (tile_is_skipped(op, rb + CG - 1, cb)) continue;
+                uint32_t cls_next = term_class_load<CG>(op, nterms - 1, rb);
                 ptx::mbar_wait(tempty_bar(buf), acc_phase ^ 1u);     // epilogue drained this buffer
                 ptx::tc_fence_after();
                 const uint32_t d_tmem = tmem_base + buf * kAccW;
                 uint32_t accumulate = 0;
                 for (int s = nterms - 1; s >= 0; --s) {      // descending K: see note on accumulation order
-                    const TermInfo ti = get_term(op, s, rb, cb);
-                    for (int ch = ti.nchunks - 1; ch >= 0; --ch) {
-                        ptx::mbar_wait(full_bar(stage), phase);
-                        ptx::tc_fence_after();
-                        const uint32_t sa = smem_base + stage * SB;
-                        const uint64_t a_hi = ptx::smem_desc_sw128(sa);
-                        const uint64_t a_lo = ptx::smem_desc_sw128(sa + kPlaneBytes);
-                        const uint64_t b_hi = ptx::smem_desc_sw128(sa + 2 * kPlaneBytes);
-                        const uint64_t b_lo = ptx::smem_desc_sw128(sa + 2 * kPlaneBytes + kBBytes);
-                        if (ti.q) {
-                            const uint32_t sfa = tmem_base + kSfCol0 + 4 * ti.sfa, sfb = tmem_base + kSfCol0 + 4 * ti.sfb;
+                    const uint32_t cls = make_uniform(cls_next);
+                    if (s > 0) cls_next = term_class_load<CG>(op, s - 1, rb);
+                    const int kelems = (op.mode == MODE_UPDATE) ? op.nb : (op.mode == MODE_P1 ? op.c * kBlk : kBlk);
+                    if (cls & kClsQ) {
+                        const uint32_t sfa = tmem_base + kSfCol0 + 4 * CG * ((cls >> 8) & 63u);
+                        const uint32_t sfb = tmem_base + kSfCol0 + 4 * CG * ((cls >> 16) & 63u);
+                        for (int ch = kelems / 128 - 1; ch >= 0; --ch) {
+                            ptx::mbar_wait(full_bar(slot), phase);
+                            ptx::tc_fence_after();
+                            if (ptx::elect_one()) {
+                                const uint32_t a = dlo0 + slot * kDescSlot, b = a + kDescB;
 #pragma unroll
-                            for (int kk = 3; kk >= 0; --kk) {              // 4 x K=32 per 128-byte row
-                                const uint64_t adv = static_cast<uint64_t>((kk * 32) >> 4);
-                                if (CG == 2) ptx::mma_mxf8_ss_pair(d_tmem, a_hi + adv, b_hi + adv, idesc_q, accumulate, sfa, sfb);
-                                else ptx::mma_mxf8_ss(d_tmem, a_hi + adv, b_hi + adv, idesc_q, accumulate, sfa, sfb);
-                                accumulate = 1;
+                                for (int kk = 3; kk >= 0; --kk) {          // 4 x K=32 per 128-byte row
+                                    const uint64_t da = ptx::smem_desc_from_lo(a + 2 * kk), db = ptx::smem_desc_from_lo(b + 2 * kk);
+                                    if (CG == 2) ptx::mma_mxf8_ss_pair(d_tmem, da, db, idesc_q, (kk == 3) ? accumulate : 1u, sfa, sfb);
+                                    else ptx::mma_mxf8_ss(d_tmem, da, db, idesc_q, (kk == 3) ? accumulate : 1u, sfa, sfb);
+                                }
+                                commit(empty_bar(slot));
                             }
-                            commit(empty_bar(stage));
-                            if (++stage == NS) { stage = 0; phase ^= 1u; }
-                            continue;
-                        }
-#pragma unroll
-                        for (int kk = kBlockK / 16 - 1; kk >= 0; --kk) {
-                            const uint64_t adv = static_cast<uint64_t>((kk * 32) >> 4);   // +32 B per K=16
-                            // small cross terms first, the dominant hi*hi product last
-                            if (ti.nA == 2) { mma(d_tmem, a_lo + adv, b_hi + adv, accumulate); accumulate = 1; }
-                            if (ti.nB == 2) { mma(d_tmem, a_hi + adv, b_lo + adv, accumulate); accumulate = 1; }
-                            mma(d_tmem, a_hi + adv, b_hi + adv, accumulate);
                             accumulate = 1;
+                            if (++slot == kSlots) { slot = 0; phase ^= 1u; }
                         }
-                        commit(empty_bar(stage));                    // smem slot free (in both CTAs) when MMAs retire
-                        if (++stage == NS) { stage = 0; phase ^= 1u; }
+                        continue;
+                    }
+                    const bool a_lo = cls & kClsALo, b_lo = cls & kClsBLo;
+                    for (int ch = kelems / kBlockK - 1; ch >= 0; --ch) {
+                        const int c0 = slot;
+                        ptx::mbar_wait(full_bar(c0), phase);
+                        if (++slot == kSlots) { slot = 0; phase ^= 1u; }
+                        const int c1 = slot;
+                        if (a_lo || b_lo) {
+                            ptx::mbar_wait(full_bar(c1), phase);
+                            if (++slot == kSlots) { slot = 0; phase ^= 1u; }
+                        }
+                        ptx::tc_fence_after();
+                        if (ptx::elect_one()) {
+                            const uint32_t ah = dlo0 + c0 * kDescSlot, bh = ah + kDescB;
+                            const uint32_t al = dlo0 + c1 * kDescSlot, bl = al + kDescB;
+                            // +32 B (2 descriptor units) per K = 16; small cross terms first, the dominant hi*hi last
+                            if (a_lo && b_lo) {
+#pragma unroll
+                                for (int kk = kBlockK / 16 - 1; kk >= 0; --kk) {
+                                    mma(d_tmem, al + 2 * kk, bh + 2 * kk, (kk == 3) ? accumulate : 1u);
+                                    mma(d_tmem, ah + 2 * kk, bl + 2 * kk, 1u);
+                                    mma(d_tmem, ah + 2 * kk, bh + 2 * kk, 1u);
+                                }
+                            } else if (a_lo) {
+#pragma unroll
+                                for (int kk = kBlockK / 16 - 1; kk >= 0; --kk) {
+                                    mma(d_tmem, al + 2 * kk, bh + 2 * kk, (kk == 3) ? accumulate : 1u);
+                                    mma(d_tmem, ah + 2 * kk, bh + 2 * kk, 1u);
+                                }
+                            } else if (b_lo) {
+#pragma unroll
+                                for (int kk = kBlockK / 16 - 1; kk >= 0; --kk) {
+                                    mma(d_tmem, ah + 2 * kk, bl + 2 * kk, (kk == 3) ? accumulate : 1u);
+                                    mma(d_tmem, ah + 2 * kk, bh + 2 * kk, 1u);
+                                }
+                            } else {
+#pragma unroll
+                                for (int kk = kBlockK / 16 - 1; kk >= 0; --kk)
+                                    mma(d_tmem, ah + 2 * kk, bh + 2 * kk, (kk == 3) ? accumulate : 1u);
+                            }
+                            commit(empty_bar(c0));                   // smem slots free (in both CTAs) when MMAs retire
+                            if (a_lo || b_lo) commit(empty_bar(c1));
+                        }
+                        accumulate = 1;
                     }
                 }
-                commit(tfull_bar(buf));                              // accumulator complete
-                if (++buf == kAccBufs) { buf = 0; acc_phase ^= 1u; }
+                if (ptx::elect_one()) commit(tfull_bar(buf));        // accumulator complete
+                if (++buf == nbufs) { buf = 0; acc_phase ^= 1u; }
             }
         }
     } else {
@@ -390,7 +467,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_constant
                     if (lane == 0) {                                        // accumulator is in registers
                         if (CG == 2) ptx::mbar_arrive_leader(tempty_bar(buf)); else ptx::mbar_arrive(tempty_bar(buf));
                     }
-                    if (++buf == kAccBufs) { buf = 0; acc_phase ^= 1u; }
+                    if (++buf == nbufs) { buf = 0; acc_phase ^= 1u; }
                 }
 #pragma unroll
                 for (int e = 0; e < 32; ++e) {

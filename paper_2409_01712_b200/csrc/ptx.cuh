@@ -225,6 +225,16 @@ __device__ __forceinline__ uint64_t smem_desc_sw128(uint32_t smem_addr) {
     return d;
 }
 
+// The same descriptor split into its address-carrying low word and the constant high word, so that an
+// issue loop steps through K and through ring slots with 32-bit adds on the low word only.
+__device__ __forceinline__ uint32_t smem_desc_lo(uint32_t smem_addr) {
+    return ((smem_addr & 0x3FFFFu) >> 4) | (1u << 16);
+}
+__device__ __forceinline__ uint64_t smem_desc_from_lo(uint32_t lo) {
+    constexpr uint32_t hi = (1024u >> 4) | (1u << 14) | (2u << 29);
+    return (static_cast<uint64_t>(hi) << 32) | lo;
+}
+
 // Instruction descriptor (kind::f16 / kind::f8f6f4), dense, FP32 accumulator, both operands K-major.
 // a_fmt/b_fmt: kind::f16 -> 0 = F16, 1 = BF16; kind::f8f6f4 -> 0 = E4M3, 1 = E5M2.
 __host__ __device__ constexpr uint32_t make_idesc(int M, int N, int a_fmt, int b_fmt) {

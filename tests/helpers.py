@@ -3,9 +3,40 @@ none of this is on the product path, and none of it comes from oracle/ or the CU
 import torch
 
 
+class LowerTiles:
+    """The packed lower tiles of a symmetric matrix (config C4's storage): tile (i,j), i >= j, row-major
+    nb x nb at slot j*NT - j(j-1)/2 + (i-j).  Diagonal tiles are full squares; only their lower part is used."""
+
+    def __init__(self, At, n, nb):
+        self.n, self.nb, self.NT = n, nb, n // nb
+        self.T = At.reshape(-1, nb, nb)
+        self.shape = (n, n)
+        self.device = At.device
+
+    def column(self, j):
+        """Tile column j as a ((NT-j)*nb) x nb matrix (rows j*nb .. n)."""
+        s0 = j * self.NT - j * (j - 1) // 2
+        return self.T[s0:s0 + self.NT - j].reshape(-1, self.nb)
+
+
+def _sym_matvec_tiles(A, X):
+    nb = A.nb
+    out = torch.zeros_like(X, dtype=torch.float64)
+    for j in range(A.NT):
+        col = A.column(j).to(torch.float64)
+        col[:nb] = torch.tril(col[:nb])
+        r0 = j * nb
+        out[r0:] += col @ X[r0:r0 + nb]
+        col[:nb] = torch.tril(col[:nb], -1)
+        out[r0:r0 + nb] += col.t() @ X[r0:]
+    return out
+
+
 def sym_matvec(A, X, row_block=4096):
     """(lower-referenced symmetric A, FP32) @ X in FP64, by row blocks.  Uses only A's lower
     triangle: A_sym = tril(A) + tril(A,-1)^T."""
+    if isinstance(A, LowerTiles):
+        return _sym_matvec_tiles(A, X)
     n = A.shape[0]
     out = torch.zeros_like(X, dtype=torch.float64)
     for r0 in range(0, n, row_block):
@@ -36,6 +67,14 @@ def factor_matvec(F, X):
 
 
 def fro_norm_sym(A, row_block=4096):
+    if isinstance(A, LowerTiles):
+        acc = 0.0
+        for j in range(A.NT):
+            col = A.column(j).to(torch.float64)
+            d = torch.tril(col[:A.nb])
+            acc += 2.0 * float((col[A.nb:] ** 2).sum()) + 2.0 * float((torch.tril(d, -1) ** 2).sum()) \
+                + float((torch.diagonal(d) ** 2).sum())
+        return acc ** 0.5
     n = A.shape[0]
     acc = 0.0
     for r0 in range(0, n, row_block):

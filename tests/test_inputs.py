@@ -59,3 +59,18 @@ def test_phenotypes_standard_normal():
     assert Y.shape == (20000, 4) and Y.dtype == torch.float32
     assert abs(float(Y.mean())) < 0.02 and abs(float(Y.std()) - 1.0) < 0.02
     assert torch.equal(Y, phenotypes(1, 20000, 4))
+
+
+def test_lower_tile_packing_matches_dense_matrix():
+    from krr_inputs import make_problem_lower_tiles
+    cfg = scaled_config(CONFIGS["C4"], nb=32, n=352, p=300)       # NT = 11: ragged against the 8-row batches
+    A, Y = make_problem(cfg)
+    At, Yt = make_problem_lower_tiles(cfg)
+    NT, nb = cfg.NT, cfg.nb
+    assert At.numel() == NT * (NT + 1) // 2 * nb * nb and torch.equal(Y, Yt)
+    T = At.reshape(-1, nb, nb)
+    slot = 0
+    for j in range(NT):
+        for i in range(j, NT):
+            assert torch.equal(T[slot], A[i * nb:(i + 1) * nb, j * nb:(j + 1) * nb]), (i, j)
+            slot += 1

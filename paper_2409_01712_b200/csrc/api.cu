@@ -123,11 +123,11 @@ static PotrfWs potrf_ws_layout(int64_t n, int nb, bool any_fp8) {
     w.off_table = o; o = align_up(o + NT * NT * sizeof(int64_t), 1024);
     w.a_amax = o;    o = align_up(o + NT * NT * sizeof(float), 1024);
     w.tile_amax = o; o = align_up(o + nslots * sizeof(float), 1024);
-    w.scl = o;       o = align_up(o + (4 + nb / kBlk) * sizeof(float), 1024);
+    w.scl = o;       o = align_up(o + (4 + 2 * (nb / kBlk)) * sizeof(float), 1024);
     w.W = o;         o = align_up(o + static_cast<size_t>(n) * nb * sizeof(float), 1024);
     w.W2 = o;        o = align_up(o + static_cast<size_t>(n) * nb * sizeof(float), 1024);   // lookahead: column k+1's partial
-    w.linv_hi = o;   o = align_up(o + static_cast<size_t>(nb) * kBlk * 2, 1024);
-    w.linv_lo = o;   o = align_up(o + static_cast<size_t>(nb) * kBlk * 2, 1024);
+    w.linv_hi = o;   o = align_up(o + 2 * static_cast<size_t>(nb) * kBlk * 2, 1024);   // two sets (column parity)
+    w.linv_lo = o;   o = align_up(o + 2 * static_cast<size_t>(nb) * kBlk * 2, 1024);
     w.Hp = o;        o = align_up(o + plane * 2, 1024);
     w.Lp = o;        o = align_up(o + plane * 2, 1024);
     w.Qp = o;        if (any_fp8) o = align_up(o + plane, 1024);
@@ -193,12 +193,12 @@ static int launch(int cat, K kernel, dim3 grid, dim3 block, size_t smem, cudaStr
 // The tensor maps of one factorisation: hi/lo FP16 images of L (128-row boxes for A operands and for
 // single-CTA B operands, 64-row boxes for the B halves of CTA pairs), the inverted diagonal blocks,
 // and the E4M3 images.
-struct GemmMaps { CUtensorMap H, L, Hh, Lh, IH, IL, Q, Qh; };
+struct GemmMaps { CUtensorMap H, L, IH[2], IL[2], Q; };
 
 // cg = 2 runs MODE_UPDATE on CTA pairs (256 x 256 output blocks); needs even block counts.
-static int launch_gemm(const GemmMaps& m, const GemmOp& op, int max_ctas, int cg, cudaStream_t st) {
+static int launch_gemm(const GemmMaps& m, const GemmOp& op, int max_ctas, int cg, cudaStream_t st, int linv_buf = 0) {
     if (op.nrb <= 0 || op.ncb <= 0) return KRR_OK;
-    ProfScope ps(op.mode == MODE_UPDATE ? CAT_UPDATE : (op.mode == MODE_P1 ? CAT_P1 : CAT_P3), st);
+    ProfScope ps(op.mode == MODE_UPDATE ? CAT_UPDATE : (op.mode == MODE_P1 ? CAT_P1 : CAT_P3), st);   // MODE_PANEL counts as panel_trsm
     ++g_launches;
     if (cg == 2 && op.mode == MODE_UPDATE && op.nrb % 2 == 0 && op.rb0 % 2 == 0 && op.ncb % 2 == 0 && op.cb0 % 2 == 0) {
         const int npairs = (op.nrb / 2) * (op.ncb / 2);
@@ -211,12 +211,12 @@ static int launch_gemm(const GemmMaps& m, const GemmOp& op, int max_ctas, int cg
         attr[0].id = cudaLaunchAttributeClusterDimension;
         attr[0].val.clusterDim.x = 2; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
         cfg.attrs = attr; cfg.numAttrs = 1;
-        return cudaLaunchKernelEx(&cfg, gemm_tc_kernel<2>, m.H, m.L, m.H, m.L, m.Q, m.Q, op) == cudaSuccess ? KRR_OK : KRR_ERR_CUDA;
+        return cudaLaunchKernelEx(&cfg, gemm_tc_kernel<2>, m.H, m.L, m.IH[0], m.IL[0], m.Q, op) == cudaSuccess ? KRR_OK : KRR_ERR_CUDA;
     }
-    const int ntiles = op.nrb * op.ncb;
+    // MODE_PANEL: one CTA per two row blocks when there are enough of them (a CTA interleaves two chains)
+    const int ntiles = (op.mode == MODE_PANEL) ? (op.nrb > max_ctas ? (op.nrb + 1) / 2 : op.nrb) : op.nrb * op.ncb;
     const int grid = ntiles < max_ctas ? ntiles : max_ctas;
-    if (op.mode == MODE_P3) gemm_tc_kernel<1><<<grid, kGemmThreads, kGemmSmem, st>>>(m.H, m.L, m.IH, m.IL, m.Q, m.Q, op);
-    else gemm_tc_kernel<1><<<grid, kGemmThreads, kGemmSmem, st>>>(m.H, m.L, m.H, m.L, m.Q, m.Q, op);
+    gemm_tc_kernel<1><<<grid, kGemmThreads, kGemmSmem, st>>>(m.H, m.L, m.IH[linv_buf], m.IL[linv_buf], m.Q, op);
     return cudaGetLastError() == cudaSuccess ? KRR_OK : KRR_ERR_CUDA;
 }
 
@@ -399,15 +399,17 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
     }
 
     GemmMaps tm;
-    if (make_plane_tmap(&tm.H, Hp, nslots * nb, nb) || make_plane_tmap(&tm.L, Lp, nslots * nb, nb) ||
-        make_plane_tmap(&tm.Hh, Hp, nslots * nb, nb, kBlk / 2) || make_plane_tmap(&tm.Lh, Lp, nslots * nb, nb, kBlk / 2) ||
-        make_plane_tmap(&tm.IH, linv_hi, nb, kBlk) || make_plane_tmap(&tm.IL, linv_lo, nb, kBlk))
+    if (make_plane_tmap(&tm.H, Hp, nslots * nb, nb) || make_plane_tmap(&tm.L, Lp, nslots * nb, nb))
         return KRR_ERR_CUDA;
-    if (any_fp8) {
-        if (make_byte_plane_tmap(&tm.Q, Qp, nslots * nb, nb) || make_byte_plane_tmap(&tm.Qh, Qp, nslots * nb, nb, kBlk / 2))
+    const size_t linv_elems = static_cast<size_t>(nb) * kBlk;           // one set of inverted diagonal blocks
+    for (int b = 0; b < 2; ++b)
+        if (make_plane_tmap(&tm.IH[b], linv_hi + b * linv_elems, nb, kBlk) ||
+            make_plane_tmap(&tm.IL[b], linv_lo + b * linv_elems, nb, kBlk))
             return KRR_ERR_CUDA;
+    if (any_fp8) {
+        if (make_byte_plane_tmap(&tm.Q, Qp, nslots * nb, nb)) return KRR_ERR_CUDA;
     } else {
-        tm.Q = tm.H; tm.Qh = tm.H;                // never dereferenced (op.fp8q = 0)
+        tm.Q = tm.H;                              // never dereferenced (op.fp8q = 0)
     }
     const int cg = ((flags & KRR_FLAG_NO_CTA_PAIRS) || nb % (2 * kBlk) != 0) ? 1 : 2;
 
@@ -416,7 +418,7 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
     float* Wbuf[2] = {W, reinterpret_cast<float*>(ws + L.W2)};
     cudaStream_t sh = st, sl = st;               // critical-path stream, bulk stream
     enum { EV_FORK = 0, EV_JOIN_HI = 1, EV_JOIN_LO = 2, EV_BASE = 3 };   // then 3 events per tile column
-    auto ev_fin = [&](int k) { return g_pipe.event(EV_BASE + 3 * static_cast<size_t>(k) + 0); };
+    auto ev_first = [&](int k) { return g_pipe.event(EV_BASE + 3 * static_cast<size_t>(k) + 0); };
     auto ev_old = [&](int k) { return g_pipe.event(EV_BASE + 3 * static_cast<size_t>(k) + 1); };
     auto ev_newb = [&](int k) { return g_pipe.event(EV_BASE + 3 * static_cast<size_t>(k) + 2); };
     if (lookahead) {
@@ -429,9 +431,20 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
     }
     // bulk kernels leave nsub SMs to the diagonal-tile chain they overlap with
     const int bulk_ctas = lookahead ? (num_sms - nsub > nsub ? num_sms - nsub : num_sms) : num_sms;
+    auto finalize = [&](int k, const float* Wk, int i0, int count, cudaStream_t s) {
+        if (count <= 0) return static_cast<int>(KRR_OK);
+        return launch(CAT_FINALIZE, finalize_kernel, dim3(nsub * nsub * 4, count), dim3(256), 0, s, NT, nb, k, i0, Wk, d_map,
+                      static_cast<const int64_t*>(off), static_cast<const float*>(tile_amax), static_cast<uint8_t*>(d_factor),
+                      d_scales, Hp, Qp, static_cast<const float*>(scl));
+    };
 
+    // Tile column k.  Critical stream `sh`: newest term on the diagonal tile, the
+    // diagonal-tile chain, then the TRSM and store of tile (k+1, k) -- all the next column's chain needs.
+    // Bulk stream `sl`: newest term on the rows below (N), the older terms of column k+1 (O), the TRSM of
+    // the remaining rows (P) and their store (F).  Column k+1's chain runs beside P(k), F(k), N(k+1), O(k+2).
     for (int k = 0; k < NT; ++k) {
         const int mblk = (NT - k) * nsub;             // 128-row blocks of the panel
+        const int lb = k & 1;                         // buffer of the inverted diagonal blocks
         float* Wk = Wbuf[k & 1];
         GemmOp op;
         memset(&op, 0, sizeof(op));
@@ -439,7 +452,7 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
         op.prow0 = tile_slot(NT, k, k) * nb;
         op.map = d_map; op.A = A; op.a_amax = (preround && any_fp8) ? a_amax : nullptr;
         op.W = Wk; op.Hp = Hp; op.Lp = Lp; op.tile_amax = tile_amax; op.flags = flags;
-        op.scl = scl; op.linv_scale = linv_scale;
+        op.scl = scl; op.linv_scale = linv_scale + lb * nsub;
         op.scales = d_scales; op.fp8q = (any_fp8 && !(flags & KRR_FLAG_FP8_VIA_FP16)) ? 1 : 0;
         // ---- U(k): S = rd(A) - L[:, 0:k] L[k, 0:k]^T over the tile column (SYRK + GEMM) ----
         op.mode = MODE_UPDATE; op.c = 0; op.cb0 = 0; op.ncb = nsub;
@@ -448,21 +461,21 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
             rc = launch_gemm(tm, op, num_sms, cg, st);
             if (rc) return rc;
         } else {
-            // terms s < k-1 were accumulated into Wk by U_old(k) while column k-1 was being factorised;
-            // the newest term s = k-1 is added here, the diagonal tile first (it starts the chain)
+            // terms s < k-1 were accumulated into Wk by O(k) while column k-1 was being factorised; the
+            // newest term s = k-1 is added here, the diagonal tile on the critical stream
             const bool have_old = (k >= 2);
             op.s_lo = (k >= 1) ? k - 1 : 0; op.s_hi = k; op.base_w = have_old ? 1 : 0; op.planes = 1;
             if (have_old) KRR_CUDA_CHECK(cudaStreamWaitEvent(sh, ev_old(k), 0));
             op.rb0 = 0; op.nrb = nsub;
             rc = launch_gemm(tm, op, num_sms, cg, sh);
             if (rc) return rc;
-            if (k >= 1) KRR_CUDA_CHECK(cudaStreamWaitEvent(sl, ev_fin(k - 1), 0));
+            if (k >= 1) KRR_CUDA_CHECK(cudaStreamWaitEvent(sl, ev_first(k - 1), 0));    // tile (k, k-1) is stored
             op.rb0 = nsub; op.nrb = mblk - nsub;
-            rc = launch_gemm(tm, op, bulk_ctas, cg, sl);
+            rc = launch_gemm(tm, op, bulk_ctas, cg, sl);                                 // N(k)
             if (rc) return rc;
             KRR_CUDA_CHECK(cudaEventRecord(ev_newb(k), sl));
             if (k + 1 < NT && k >= 1) {
-                // U_old(k+1): terms s < k of column k+1, overlapping the factorisation of column k
+                // O(k+1): terms s < k of column k+1, beside the chain of column k
                 GemmOp on = op;
                 on.k = k + 1; on.prow0 = tile_slot(NT, k + 1, k + 1) * nb; on.W = Wbuf[(k + 1) & 1];
                 on.s_lo = 0; on.s_hi = k; on.base_w = 0; on.planes = 0;
@@ -472,39 +485,53 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
                 KRR_CUDA_CHECK(cudaEventRecord(ev_old(k + 1), sl));
             }
         }
-        // ---- panel: 128-wide sub-columns; the diagonal tile's rows first (critical path) ----
-        for (int part = 0; part < (lookahead ? 2 : 1); ++part) {
-            // part 0: rows of the diagonal tile (or all rows without lookahead); part 1: rows below
-            const int row_lo = (part == 0) ? 0 : nsub;
-            const int row_hi = (lookahead && part == 0) ? nsub : mblk;
-            if (part == 1) KRR_CUDA_CHECK(cudaStreamWaitEvent(sh, ev_newb(k), 0));
-            if (row_hi <= row_lo) continue;
-            for (int c = 0; c < nsub; ++c) {
-                if (c > 0) {
-                    op.mode = MODE_P1; op.c = c; op.cb0 = c; op.ncb = 1;
-                    op.rb0 = (part == 0) ? c : row_lo; op.nrb = row_hi - op.rb0;
-                    rc = launch_gemm(tm, op, num_sms, cg, sh);
-                    if (rc) return rc;
-                }
-                if (part == 0) {
-                    rc = launch(CAT_POTRF, potrf128_kernel, dim3(1), dim3(kTriThreads), static_cast<size_t>(kTriSmem), sh, Wk, nb,
-                                c * kBlk, c * kBlk, linv_hi, linv_lo, linv_scale, d_info,
-                                static_cast<int64_t>(k) * nb + static_cast<int64_t>(c) * kBlk + 1);
-                    if (rc) return rc;
-                }
-                op.mode = MODE_P3; op.c = c; op.cb0 = c; op.ncb = 1;
-                op.rb0 = (part == 0) ? c + 1 : row_lo; op.nrb = row_hi - op.rb0;
-                if (op.nrb > 0) {
-                    rc = launch_gemm(tm, op, num_sms, 1, sh);
-                    if (rc) return rc;
-                }
+        // ---- diagonal-tile chain: 128-wide sub-columns of tile (k,k) ----
+        for (int c = 0; c < nsub; ++c) {
+            if (c > 0) {
+                op.mode = MODE_P1; op.c = c; op.cb0 = c; op.ncb = 1; op.rb0 = c; op.nrb = nsub - c;
+                rc = launch_gemm(tm, op, num_sms, 1, sh, lb);
+                if (rc) return rc;
+            }
+            rc = launch(CAT_POTRF, potrf128_kernel, dim3(1), dim3(kTriThreads), static_cast<size_t>(kTriSmem), sh, Wk, nb,
+                        c * kBlk, c * kBlk, linv_hi + lb * linv_elems, linv_lo + lb * linv_elems, linv_scale + lb * nsub, d_info,
+                        static_cast<int64_t>(k) * nb + static_cast<int64_t>(c) * kBlk + 1);
+            if (rc) return rc;
+            op.mode = MODE_P3; op.c = c; op.cb0 = c; op.ncb = 1; op.rb0 = c + 1; op.nrb = nsub - c - 1;
+            if (op.nrb > 0) {
+                rc = launch_gemm(tm, op, num_sms, 1, sh, lb);
+                if (rc) return rc;
             }
         }
-        rc = launch(CAT_FINALIZE, finalize_kernel, dim3(nsub * nsub * 4, NT - k), dim3(256), 0, sh, NT, nb, k, static_cast<const float*>(Wk),
-                    d_map, static_cast<const int64_t*>(off), static_cast<const float*>(tile_amax),
-                    static_cast<uint8_t*>(d_factor), d_scales, Hp, Qp, static_cast<const float*>(scl));
+        rc = finalize(k, Wk, 0, 1, sh);
         if (rc) return rc;
-        if (lookahead) KRR_CUDA_CHECK(cudaEventRecord(ev_fin(k), sh));
+        // ---- panel below: each 128-row block runs its whole TRSM chain in one CTA (MODE_PANEL) ----
+        op.mode = MODE_PANEL; op.c = 0; op.cb0 = 0; op.ncb = 1;
+        if (!lookahead) {
+            op.rb0 = nsub; op.nrb = mblk - nsub;
+            rc = launch_gemm(tm, op, num_sms, 1, st, lb);
+            if (rc) return rc;
+            rc = finalize(k, Wk, 1, NT - k - 1, st);
+            if (rc) return rc;
+        } else {
+            if (k + 1 < NT) {
+                // tile (k+1, k) first, on the critical stream: column k+1's chain needs nothing else of column k
+                KRR_CUDA_CHECK(cudaStreamWaitEvent(sh, ev_newb(k), 0));
+                op.rb0 = nsub; op.nrb = nsub;
+                rc = launch_gemm(tm, op, num_sms, 1, sh, lb);
+                if (rc) return rc;
+                rc = finalize(k, Wk, 1, 1, sh);
+                if (rc) return rc;
+            }
+            KRR_CUDA_CHECK(cudaEventRecord(ev_first(k), sh));
+            KRR_CUDA_CHECK(cudaStreamWaitEvent(sl, ev_first(k), 0));
+            if (k + 2 < NT) {
+                op.rb0 = 2 * nsub; op.nrb = mblk - 2 * nsub;
+                rc = launch_gemm(tm, op, bulk_ctas, 1, sl, lb);                          // P(k)
+                if (rc) return rc;
+                rc = finalize(k, Wk, 2, NT - k - 2, sl);                                 // F(k)
+                if (rc) return rc;
+            }
+        }
     }
     if (lookahead) {
         KRR_CUDA_CHECK(cudaEventRecord(g_pipe.event(EV_JOIN_HI), sh));

@@ -41,7 +41,7 @@
 
 namespace krr {
 
-enum { MODE_UPDATE = 0, MODE_P1 = 1, MODE_P3 = 2 };
+enum { MODE_UPDATE = 0, MODE_P1 = 1, MODE_P3 = 2, MODE_PANEL = 3 };
 
 struct GemmOp {
     int mode;
@@ -106,9 +106,9 @@ constexpr uint32_t kClsALo = 1u, kClsBLo = 2u, kClsQ = 4u;
 // UE8M0 byte of the power of two x (> 0, normal): its biased exponent.
 __device__ __forceinline__ int pow2_exponent_byte(float x) { return static_cast<int>((__float_as_uint(x) >> 23) & 0xffu); }
 
-__device__ __forceinline__ TermGeom term_geom(const GemmOp& op, int s /* term index */, int rb, int cb) {
+__device__ __forceinline__ TermGeom term_geom(const GemmOp& op, int mode, int c, int s /* term index */, int rb, int cb) {
     TermGeom t;
-    if (op.mode == MODE_UPDATE) {
+    if (mode == MODE_UPDATE) {
         const int i = op.k + (rb * kBlk) / op.nb;
         const int subrow = (rb * kBlk) % op.nb;
         s += op.s_lo;
@@ -117,16 +117,16 @@ __device__ __forceinline__ TermGeom term_geom(const GemmOp& op, int s /* term in
         t.a_k0 = 0;
         t.b_k0 = 0;
         t.kelems = op.nb;
-    } else if (op.mode == MODE_P1) {
+    } else if (mode == MODE_P1) {
         t.a_row = static_cast<int>(op.prow0) + rb * kBlk;
-        t.b_row = static_cast<int>(op.prow0) + op.c * kBlk;
+        t.b_row = static_cast<int>(op.prow0) + c * kBlk;
         t.a_k0 = 0;
         t.b_k0 = 0;
-        t.kelems = op.c * kBlk;
+        t.kelems = c * kBlk;
     } else {
         t.a_row = static_cast<int>(op.prow0) + rb * kBlk;
-        t.b_row = op.c * kBlk;                             // row in the Linv planes
-        t.a_k0 = op.c * kBlk;
+        t.b_row = c * kBlk;                                // row in the Linv planes
+        t.a_k0 = c * kBlk;
         t.b_k0 = 0;
         t.kelems = kBlk;
     }
@@ -134,8 +134,8 @@ __device__ __forceinline__ TermGeom term_geom(const GemmOp& op, int s /* term in
 }
 
 template <int CG>
-__device__ __forceinline__ uint32_t term_class_load(const GemmOp& op, int s /* term index */, int rb) {
-    if (op.mode != MODE_UPDATE) return kClsALo | kClsBLo;
+__device__ __forceinline__ uint32_t term_class_load(const GemmOp& op, int mode, int s /* term index */, int rb) {
+    if (mode != MODE_UPDATE) return kClsALo | kClsBLo;
     const int i = op.k + (rb * kBlk) / op.nb;
     s += op.s_lo;
     const int pa = op.map[i * op.NT + s], pb = op.map[op.k * op.NT + s];
@@ -160,6 +160,57 @@ __device__ __forceinline__ bool tile_is_skipped(const GemmOp& op, int rb, int cb
     return op.mode == MODE_UPDATE && (rb * kBlk) < op.nb && cb > rb;
 }
 
+// ---- work items ------------------------------------------------------------------------------------
+// The three warp roles of a CTA walk the same sequence of work items, each with its own iterator.
+//   MODE_UPDATE / MODE_P1 / MODE_P3: item = one output block (of a pair: 256 x 256), blocks dealt
+//     round-robin over the CTAs (pairs) of the grid.
+//   MODE_PANEL (CG = 1): the whole TRSM of a 128-row block of the panel below the diagonal tile,
+//     X_c = (S_c - sum_{c'<c} X_c' L_cc'^T) inv(L_cc)^T for c = 0 .. nsub-1, as the item sequence
+//     P3(0), P1(1), P3(1), P1(2), ...  Row blocks never interact, so a CTA owns its row blocks (dealt
+//     round-robin) and runs each chain by itself; an item reads, through TMA, operand images the previous
+//     item of the same row block wrote to global memory (`dep`), and two row blocks are interleaved so
+//     that one's write -> fence -> read turnaround is covered by the other's MMAs.
+struct WorkItem {
+    int mode, c;     // contraction shape (MODE_UPDATE / MODE_P1 / MODE_P3) and sub-column
+    int rb, cb;      // first output row block / column block (of the pair when CG = 2)
+    int dep;         // > 0: reads what the item `dep` places earlier in this CTA's sequence wrote
+};
+struct ItemIter {
+    int t;           // block modes: next block index
+    int g, it, m;    // MODE_PANEL: group of two row blocks, item inside the chain, member of the group
+};
+
+template <int CG>
+__device__ __forceinline__ bool next_item(const GemmOp& op, ItemIter& st, int unit0, int nunits, WorkItem& w) {
+    if (op.mode == MODE_PANEL) {
+        const int nmine = (op.nrb > unit0) ? (op.nrb - unit0 + nunits - 1) / nunits : 0;    // my row blocks
+        if (2 * st.g >= nmine) return false;
+        const int size_g = (2 * st.g + 1 < nmine) ? 2 : 1;
+        w.rb = op.rb0 + unit0 + (2 * st.g + st.m) * nunits;
+        w.c = (st.it + 1) >> 1;
+        w.cb = w.c;
+        w.mode = (st.it & 1) ? MODE_P1 : MODE_P3;
+        w.dep = st.it > 0 ? size_g : 0;
+        if (++st.m == size_g) {
+            st.m = 0;
+            if (++st.it == 2 * (op.nb / kBlk) - 1) { st.it = 0; ++st.g; }
+        }
+        return true;
+    }
+    const int ncbu = op.ncb / CG;
+    const int ntiles = (op.nrb / CG) * ncbu;
+    while (st.t < ntiles) {
+        const int t = st.t;
+        st.t += nunits;
+        w.rb = op.rb0 + (t / ncbu) * CG;
+        w.cb = op.cb0 + (t % ncbu) * CG;
+        if (tile_is_skipped(op, w.rb + CG - 1, w.cb)) continue;      // the whole (pair) block lies above the diagonal
+        w.mode = op.mode; w.c = op.c; w.dep = 0;
+        return true;
+    }
+    return false;
+}
+
 // CG = 1: one CTA per 128x128 output block.  CG = 2 (MODE_UPDATE only): a CTA pair (cluster of 2,
 // tcgen05 cta_group::2) per 256x256 block -- each CTA stages its own 128 rows of A and the 128 rows of
 // B of ONE of the two column blocks, the leader issues M = 256, N = 256 MMAs that read both CTAs'
@@ -170,9 +221,11 @@ __device__ __forceinline__ bool tile_is_skipped(const GemmOp& op, int rb, int cb
 // Per flop a pair moves half the operand bytes of CG = 1.
 template <int CG>
 __global__ void __launch_bounds__(kGemmThreads, 1)
-gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_constant__ CUtensorMap tmA_lo,
-               const __grid_constant__ CUtensorMap tmB_hi, const __grid_constant__ CUtensorMap tmB_lo,
-               const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmQb, const GemmOp op) {
+gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ CUtensorMap tmL,
+               const __grid_constant__ CUtensorMap tmIH, const __grid_constant__ CUtensorMap tmIL,
+               const __grid_constant__ CUtensorMap tmQ, const GemmOp op) {
+    // tmH / tmL: hi / lo FP16 images of the factor and panel (both operands of every product except the B
+    // operand of MODE_P3, which is an inverted diagonal block: tmIH / tmIL); tmQ: E4M3 images.
     constexpr uint32_t SB = kSlotBytes;                 // [A block 16 KB | B block 16 KB]
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
@@ -190,23 +243,22 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_constant
     const int rank = (CG == 2) ? static_cast<int>(ptx::cluster_ctarank()) : 0;
     const int unit0 = (CG == 2) ? static_cast<int>(blockIdx.x >> 1) : static_cast<int>(blockIdx.x);   // pair / CTA index
     const int nunits = (CG == 2) ? static_cast<int>(gridDim.x >> 1) : static_cast<int>(gridDim.x);
-    const int ncbu = op.ncb / CG;                       // column units
-    const int ntiles = (op.nrb / CG) * ncbu;            // output blocks of (128*CG) x (128*CG)
     constexpr int kAccW = kAccCols * CG;                // accumulator columns per buffer
     const int nterms = num_terms(op);
     const bool use_sf = op.fp8q && op.mode == MODE_UPDATE;
     // a pair's 256-column accumulators fill TMEM: with the scale table present there is room for one only
     const int nbufs = (CG == 2 && use_sf) ? 1 : kMaxAccBufs;
 
-    const bool has_acc = (op.mode != MODE_UPDATE) ? (op.mode == MODE_P3 || op.c > 0) : (nterms > 0);
+    const bool has_acc = (op.mode != MODE_UPDATE) ? (op.mode != MODE_P1 || op.c > 0) : (nterms > 0);
     const bool write_planes = (op.mode != MODE_UPDATE) || op.planes;
+    // MODE_PANEL: completed epilogue warps of this CTA's item sequence (8 per item), polled by the producer
+    volatile int* done_ctr = reinterpret_cast<volatile int*>(tmem_slot_ptr + 2);
 
     if (warp == 0 && lane == 0) {
-        ptx::prefetch_tmap(&tmA_hi);
-        ptx::prefetch_tmap(&tmA_lo);
-        ptx::prefetch_tmap(&tmB_hi);
-        ptx::prefetch_tmap(&tmB_lo);
-        if (op.fp8q) { ptx::prefetch_tmap(&tmQ); ptx::prefetch_tmap(&tmQb); }
+        ptx::prefetch_tmap(&tmH);
+        ptx::prefetch_tmap(&tmL);
+        if (op.mode == MODE_P3 || op.mode == MODE_PANEL) { ptx::prefetch_tmap(&tmIH); ptx::prefetch_tmap(&tmIL); }
+        if (op.fp8q) ptx::prefetch_tmap(&tmQ);
         for (int s = 0; s < kSlots; ++s) {
             ptx::mbar_init(full_bar(s), 1);
             ptx::mbar_init(empty_bar(s), 1);
@@ -215,6 +267,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_constant
             ptx::mbar_init(tfull_bar(b), 1);
             ptx::mbar_init(tempty_bar(b), kEpiWarps * CG);
         }
+        *done_ctr = 0;
         ptx::fence_mbar_init();
     }
     if (warp == 1) {
@@ -248,14 +301,25 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_constant
             auto load = [&](uint32_t dst, const CUtensorMap* m, uint32_t bar, int c0, int c1) {
                 if (CG == 2) ptx::tma_load_2d_pair(dst, m, bar, c0, c1); else ptx::tma_load_2d(dst, m, bar, c0, c1);
             };
-            for (int t = unit0; t < ntiles; t += nunits) {
-                const int rb = op.rb0 + (t / ncbu) * CG + rank, cb0u = op.cb0 + (t % ncbu) * CG;
-                if (tile_is_skipped(op, rb - rank + CG - 1, cb0u)) continue;    // the whole (pair) block lies above the diagonal
-                uint32_t cls_next = term_class_load<CG>(op, nterms - 1, rb);
+            ItemIter iter = {unit0, 0, 0, 0};
+            WorkItem w;
+            int seq = 0;
+            while (next_item<CG>(op, iter, unit0, nunits, w)) {
+                const int rb = w.rb + rank, cb0u = w.cb;
+                if (w.dep) {
+                    // the operand images this item reads were written by this CTA's epilogue warps `dep` items ago
+                    const int need = kEpiWarps * (seq - w.dep + 1);
+                    uint32_t spins = 0;
+                    while (*done_ctr < need) { if (++spins > (1u << 27)) __trap(); }
+                    __threadfence();
+                    ptx::fence_proxy_async_global();
+                }
+                ++seq;
+                uint32_t cls_next = term_class_load<CG>(op, w.mode, nterms - 1, rb);
                 for (int s = nterms - 1; s >= 0; --s) {      // descending K: see note on accumulation order
                     const uint32_t cls = make_uniform(cls_next);
-                    if (s > 0) cls_next = term_class_load<CG>(op, s - 1, rb);   // in flight during this term's chunks
-                    const TermGeom g = term_geom(op, s, rb, cb0u + rank);       // this CTA's A rows and B rows
+                    if (s > 0) cls_next = term_class_load<CG>(op, w.mode, s - 1, rb);   // in flight during this term's chunks
+                    const TermGeom g = term_geom(op, w.mode, w.c, s, rb, cb0u + rank);  // this CTA's A rows and B rows
                     if (cls & kClsQ) {                       // E4M3 images: 128 bytes of K per row, one slot per chunk
                         for (int ch = g.kelems / 128 - 1; ch >= 0; --ch) {
                             ptx::mbar_wait(empty_bar(slot), phase ^ 1u);
@@ -263,13 +327,15 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_constant
                                 const uint32_t sa = smem_base + slot * SB;
                                 if (rank == 0) ptx::mbar_arrive_expect_tx(full_bar(slot), CG * 2u * kPlaneBytes);
                                 load(sa, &tmQ, full_bar(slot), ch * 128, g.a_row);
-                                load(sa + kPlaneBytes, &tmQb, full_bar(slot), ch * 128, g.b_row);
+                                load(sa + kPlaneBytes, &tmQ, full_bar(slot), ch * 128, g.b_row);
                             }
                             if (++slot == kSlots) { slot = 0; phase ^= 1u; }
                         }
                         continue;
                     }
                     const bool a_lo = cls & kClsALo, b_lo = cls & kClsBLo;
+                    const CUtensorMap* mB_hi = (w.mode == MODE_P3) ? &tmIH : &tmH;
+                    const CUtensorMap* mB_lo = (w.mode == MODE_P3) ? &tmIL : &tmL;
                     const uint32_t lo_bytes = CG * ((a_lo ? 1u : 0u) + (b_lo ? 1u : 0u)) * kPlaneBytes;
                     for (int ch = g.kelems / kBlockK - 1; ch >= 0; --ch) {
                         const int ak = g.a_k0 + ch * kBlockK, bk = g.b_k0 + ch * kBlockK;
@@ -277,8 +343,8 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_constant
                         if (ptx::elect_one()) {              // hi images
                             const uint32_t sa = smem_base + slot * SB;
                             if (rank == 0) ptx::mbar_arrive_expect_tx(full_bar(slot), CG * 2u * kPlaneBytes);
-                            load(sa, &tmA_hi, full_bar(slot), ak, g.a_row);
-                            load(sa + kPlaneBytes, &tmB_hi, full_bar(slot), bk, g.b_row);
+                            load(sa, &tmH, full_bar(slot), ak, g.a_row);
+                            load(sa + kPlaneBytes, mB_hi, full_bar(slot), bk, g.b_row);
                         }
                         if (++slot == kSlots) { slot = 0; phase ^= 1u; }
                         if (lo_bytes) {                      // lo images of the FP32-class operand(s)
@@ -286,8 +352,8 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_constant
                             if (ptx::elect_one()) {
                                 const uint32_t sa = smem_base + slot * SB;
                                 if (rank == 0) ptx::mbar_arrive_expect_tx(full_bar(slot), lo_bytes);
-                                if (a_lo) load(sa, &tmA_lo, full_bar(slot), ak, g.a_row);
-                                if (b_lo) load(sa + kPlaneBytes, &tmB_lo, full_bar(slot), bk, g.b_row);
+                                if (a_lo) load(sa, &tmL, full_bar(slot), ak, g.a_row);
+                                if (b_lo) load(sa + kPlaneBytes, mB_lo, full_bar(slot), bk, g.b_row);
                             }
                             if (++slot == kSlots) { slot = 0; phase ^= 1u; }
                         }
@@ -312,18 +378,19 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_constant
             uint32_t phase = 0;
             int buf = 0;
             uint32_t acc_phase = 0;
-            for (int t = unit0; t < ntiles; t += nunits) {
-                const int rb = op.rb0 + (t / ncbu) * CG, cb = op.cb0 + (t % ncbu) * CG;
-                if (tile_is_skipped(op, rb + CG - 1, cb)) continue;
-                uint32_t cls_next = term_class_load<CG>(op, nterms - 1, rb);
+            ItemIter iter = {unit0, 0, 0, 0};
+            WorkItem w;
+            while (next_item<CG>(op, iter, unit0, nunits, w)) {
+                const int rb = w.rb;
+                uint32_t cls_next = term_class_load<CG>(op, w.mode, nterms - 1, rb);
                 ptx::mbar_wait(tempty_bar(buf), acc_phase ^ 1u);     // epilogue drained this buffer
                 ptx::tc_fence_after();
                 const uint32_t d_tmem = tmem_base + buf * kAccW;
                 uint32_t accumulate = 0;
                 for (int s = nterms - 1; s >= 0; --s) {      // descending K: see note on accumulation order
                     const uint32_t cls = make_uniform(cls_next);
-                    if (s > 0) cls_next = term_class_load<CG>(op, s - 1, rb);
-                    const int kelems = (op.mode == MODE_UPDATE) ? op.nb : (op.mode == MODE_P1 ? op.c * kBlk : kBlk);
+                    if (s > 0) cls_next = term_class_load<CG>(op, w.mode, s - 1, rb);
+                    const int kelems = (w.mode == MODE_UPDATE) ? op.nb : (w.mode == MODE_P1 ? w.c * kBlk : kBlk);
                     if (cls & kClsQ) {
                         const uint32_t sfa = tmem_base + kSfCol0 + 4 * CG * ((cls >> 8) & 63u);
                         const uint32_t sfb = tmem_base + kSfCol0 + 4 * CG * ((cls >> 16) & 63u);
@@ -407,9 +474,10 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_constant
         const int nsub = op.nb / kBlk;
         int buf = 0;
         uint32_t acc_phase = 0;
-        for (int t = unit0; t < ntiles; t += nunits) {
-            const int rb = op.rb0 + (t / ncbu) * CG + rank, cb0u = op.cb0 + (t % ncbu) * CG;
-            if (tile_is_skipped(op, rb - rank + CG - 1, cb0u)) continue;
+        ItemIter iter = {unit0, 0, 0, 0};
+        WorkItem w;
+        while (next_item<CG>(op, iter, unit0, nunits, w)) {
+            const int rb = w.rb + rank, cb0u = w.cb;
 #pragma unroll 1
           for (int j2 = 0; j2 < CG; ++j2) {                       // the unit's column blocks, one after the other
             const int cb = cb0u + j2;
@@ -419,8 +487,8 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_constant
             float* wblk = op.W + (static_cast<int64_t>(rb) * nsub + cb) * (kBlk * kBlk) + static_cast<int64_t>(64 * hf) * kBlk + row_in_blk;
             // ---- base values, fetched before the accumulator is ready
             float bs[64];
-            const bool base_from_w = (op.mode == MODE_P1) || (op.mode == MODE_UPDATE && op.base_w);
-            const bool base_from_a = (op.mode == MODE_UPDATE && !op.base_w);
+            const bool base_from_w = (w.mode == MODE_P1) || (w.mode == MODE_UPDATE && op.base_w);
+            const bool base_from_a = (w.mode == MODE_UPDATE && !op.base_w);
             if (dead) {
 #pragma unroll
                 for (int e = 0; e < 64; ++e) bs[e] = 0.0f;
@@ -450,8 +518,8 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_constant
                 for (int e = 0; e < 64; ++e) bs[e] = 0.0f;
             }
             // exact power-of-two rescaling: accumulator -> value domain, value -> plane domain
-            const float acc_mul = (op.mode == MODE_P3) ? -op.scl[3] / op.linv_scale[op.c] : op.scl[2];
-            const float plane_mul = (op.mode == MODE_P3) ? op.scl[0] : op.scl[1];
+            const float acc_mul = (w.mode == MODE_P3) ? -op.scl[3] / op.linv_scale[w.c] : op.scl[2];
+            const float plane_mul = (w.mode == MODE_P3) ? op.scl[0] : op.scl[1];
             float out[64];
             if (has_acc) {
                 if (j2 == 0) ptx::mbar_wait(tfull_bar(buf), acc_phase);
@@ -510,7 +578,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_constant
                     }
                 }
             }
-            if (op.mode == MODE_P3 && op.tile_amax != nullptr) {
+            if (w.mode == MODE_P3 && op.tile_amax != nullptr) {
 #pragma unroll
                 for (int o = 16; o > 0; o >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, o));
                 if (lane == 0) {
@@ -519,6 +587,13 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_constant
                 }
             }
           }   // j2
+            if (op.mode == MODE_PANEL) {
+                // publish this item's operand images to the TMA loads of a later item of this CTA
+                __threadfence();
+                ptx::fence_proxy_async_global();
+                __syncwarp();
+                if (lane == 0) atomicAdd_block(const_cast<int*>(done_ctr), 1);
+            }
         }
     }
 

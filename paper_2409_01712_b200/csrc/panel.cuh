@@ -75,18 +75,18 @@ tile_amax_kernel(AView A, const uint8_t* __restrict__ map, float* __restrict__ a
     if ((threadIdx.x & 31) == 0) atomicMax(reinterpret_cast<int*>(a_amax + i * NT + j), __float_as_int(amax));
 }
 
-// Round tile column k (FP32 in W, block-column-major 128x128 blocks) into the mosaic.
-// grid = (nsub*nsub*4, NT-k), 256 threads: one CTA transposes 32 rows of one 128x128 block through
+// Round tiles (k + i0 + blockIdx.y, k) of tile column k (FP32 in W, block-column-major 128x128 blocks)
+// into the mosaic.  grid = (nsub*nsub*4, number of tiles), 256 threads: one CTA transposes 32 rows of one 128x128 block through
 // shared memory (coalesced reads of W columns, coalesced row-major writes of the factor / images).
 __global__ void __launch_bounds__(256)
-finalize_kernel(int NT, int nb, int k, const float* __restrict__ W, const uint8_t* __restrict__ map,
+finalize_kernel(int NT, int nb, int k, int i0, const float* __restrict__ W, const uint8_t* __restrict__ map,
                 const int64_t* __restrict__ off, const float* __restrict__ tile_amax /* per slot */,
                 uint8_t* __restrict__ factor, float* __restrict__ scales, __half* __restrict__ Hp,
                 uint8_t* __restrict__ Qp, const float* __restrict__ scl) {
     __shared__ float tile[32][kBlk + 1];
     const float sx = scl[0];
     const int nsub = nb / kBlk;
-    const int i = k + blockIdx.y;
+    const int i = k + i0 + blockIdx.y;
     const int p = map[i * NT + k];
     const int64_t slot = tile_slot(NT, i, k);
     const float s = (p == KRR_FP8_E4M3) ? fp8_scale_from_amax(tile_amax[slot]) : 1.0f;
@@ -94,7 +94,7 @@ finalize_kernel(int NT, int nb, int k, const float* __restrict__ W, const uint8_
     uint8_t* dst = factor + off[i * NT + k];
     const int blk = blockIdx.x >> 2, qr = blockIdx.x & 3;
     const int rbl = blk / nsub, cb = blk % nsub;                         // block inside the tile
-    const int64_t rb = static_cast<int64_t>(blockIdx.y) * nsub + rbl;    // panel-local row block
+    const int64_t rb = static_cast<int64_t>(i0 + blockIdx.y) * nsub + rbl;    // panel-local row block
     const float* wblk = W + (rb * nsub + cb) * (kBlk * kBlk) + 32 * qr;
     for (int idx = threadIdx.x; idx < 32 * kBlk; idx += 256) {
         const int c = idx >> 5, rr = idx & 31;

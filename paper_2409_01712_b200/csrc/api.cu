@@ -161,7 +161,7 @@ struct ProfScope {
 // `hi` carries the critical path (diagonal-tile chain, panel, store), `lo` the bulk updates that run
 // ahead; both are fenced by events against the caller's stream, which is never blocked on the host.
 struct Pipeline {
-    cudaStream_t hi = nullptr, lo = nullptr;
+    cudaStream_t hi = nullptr, mid = nullptr, lo = nullptr;
     std::vector<cudaEvent_t> ev;
     cudaEvent_t event(size_t i) {
         while (ev.size() <= i) {
@@ -176,6 +176,7 @@ struct Pipeline {
         int least = 0, greatest = 0;
         KRR_CUDA_CHECK(cudaDeviceGetStreamPriorityRange(&least, &greatest));
         KRR_CUDA_CHECK(cudaStreamCreateWithPriority(&hi, cudaStreamNonBlocking, greatest));
+        KRR_CUDA_CHECK(cudaStreamCreateWithPriority(&mid, cudaStreamNonBlocking, (least + greatest) / 2));
         KRR_CUDA_CHECK(cudaStreamCreateWithPriority(&lo, cudaStreamNonBlocking, least));
         return KRR_OK;
     }
@@ -416,17 +417,19 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
     const int nsub = nb / kBlk;
     const bool lookahead = !(flags & KRR_FLAG_NO_LOOKAHEAD) && NT > 2;
     float* Wbuf[2] = {W, reinterpret_cast<float*>(ws + L.W2)};
-    cudaStream_t sh = st, sl = st;               // critical-path stream, bulk stream
-    enum { EV_FORK = 0, EV_JOIN_HI = 1, EV_JOIN_LO = 2, EV_BASE = 3 };   // then 3 events per tile column
-    auto ev_first = [&](int k) { return g_pipe.event(EV_BASE + 3 * static_cast<size_t>(k) + 0); };
-    auto ev_old = [&](int k) { return g_pipe.event(EV_BASE + 3 * static_cast<size_t>(k) + 1); };
-    auto ev_newb = [&](int k) { return g_pipe.event(EV_BASE + 3 * static_cast<size_t>(k) + 2); };
+    cudaStream_t sh = st, sp = st, sl = st;      // critical-path stream, panel stream, bulk stream
+    enum { EV_FORK = 0, EV_JOIN_HI = 1, EV_JOIN_MID = 2, EV_JOIN_LO = 3, EV_BASE = 4 };   // then 4 events per tile column
+    auto ev_first = [&](int k) { return g_pipe.event(EV_BASE + 4 * static_cast<size_t>(k) + 0); };
+    auto ev_old = [&](int k) { return g_pipe.event(EV_BASE + 4 * static_cast<size_t>(k) + 1); };
+    auto ev_newb = [&](int k) { return g_pipe.event(EV_BASE + 4 * static_cast<size_t>(k) + 2); };
+    auto ev_fin = [&](int k) { return g_pipe.event(EV_BASE + 4 * static_cast<size_t>(k) + 3); };
     if (lookahead) {
         rc = g_pipe.init();
         if (rc) return rc;
-        sh = g_pipe.hi; sl = g_pipe.lo;
+        sh = g_pipe.hi; sp = g_pipe.mid; sl = g_pipe.lo;
         KRR_CUDA_CHECK(cudaEventRecord(g_pipe.event(EV_FORK), st));
         KRR_CUDA_CHECK(cudaStreamWaitEvent(sh, g_pipe.event(EV_FORK), 0));
+        KRR_CUDA_CHECK(cudaStreamWaitEvent(sp, g_pipe.event(EV_FORK), 0));
         KRR_CUDA_CHECK(cudaStreamWaitEvent(sl, g_pipe.event(EV_FORK), 0));
     }
     // bulk kernels leave nsub SMs to the diagonal-tile chain they overlap with
@@ -440,8 +443,10 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
 
     // Tile column k.  Critical stream `sh`: newest term on the diagonal tile, the
     // diagonal-tile chain, then the TRSM and store of tile (k+1, k) -- all the next column's chain needs.
-    // Bulk stream `sl`: newest term on the rows below (N), the older terms of column k+1 (O), the TRSM of
-    // the remaining rows (P) and their store (F).  Column k+1's chain runs beside P(k), F(k), N(k+1), O(k+2).
+    // Bulk stream `sl`: newest term on the rows below (N), then the older terms of column k+1 (O).
+    // Panel stream `sp`: the TRSM of the remaining rows (P) and their store (F); latency-bound, it fills
+    // the SMs the bulk kernel leaves free and takes the rest as O(k+1) drains.  N(k+1) waits for F(k);
+    // column k+1's chain runs beside F(k), N(k+1), O(k+2).
     for (int k = 0; k < NT; ++k) {
         const int mblk = (NT - k) * nsub;             // 128-row blocks of the panel
         const int lb = k & 1;                         // buffer of the inverted diagonal blocks
@@ -469,7 +474,7 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
             op.rb0 = 0; op.nrb = nsub;
             rc = launch_gemm(tm, op, num_sms, cg, sh);
             if (rc) return rc;
-            if (k >= 1) KRR_CUDA_CHECK(cudaStreamWaitEvent(sl, ev_first(k - 1), 0));    // tile (k, k-1) is stored
+            if (k >= 1) KRR_CUDA_CHECK(cudaStreamWaitEvent(sl, ev_fin(k - 1), 0));      // column k-1 is stored
             op.rb0 = nsub; op.nrb = mblk - nsub;
             rc = launch_gemm(tm, op, bulk_ctas, cg, sl);                                 // N(k)
             if (rc) return rc;
@@ -523,19 +528,23 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
                 if (rc) return rc;
             }
             KRR_CUDA_CHECK(cudaEventRecord(ev_first(k), sh));
-            KRR_CUDA_CHECK(cudaStreamWaitEvent(sl, ev_first(k), 0));
+            KRR_CUDA_CHECK(cudaStreamWaitEvent(sp, ev_first(k), 0));
             if (k + 2 < NT) {
+                KRR_CUDA_CHECK(cudaStreamWaitEvent(sp, ev_newb(k), 0));
                 op.rb0 = 2 * nsub; op.nrb = mblk - 2 * nsub;
-                rc = launch_gemm(tm, op, bulk_ctas, 1, sl, lb);                          // P(k)
+                rc = launch_gemm(tm, op, num_sms, 1, sp, lb);                            // P(k)
                 if (rc) return rc;
-                rc = finalize(k, Wk, 2, NT - k - 2, sl);                                 // F(k)
+                rc = finalize(k, Wk, 2, NT - k - 2, sp);                                 // F(k)
                 if (rc) return rc;
             }
+            KRR_CUDA_CHECK(cudaEventRecord(ev_fin(k), sp));
         }
     }
     if (lookahead) {
         KRR_CUDA_CHECK(cudaEventRecord(g_pipe.event(EV_JOIN_HI), sh));
         KRR_CUDA_CHECK(cudaEventRecord(g_pipe.event(EV_JOIN_LO), sl));
+        KRR_CUDA_CHECK(cudaEventRecord(g_pipe.event(EV_JOIN_MID), sp));
+        KRR_CUDA_CHECK(cudaStreamWaitEvent(st, g_pipe.event(EV_JOIN_MID), 0));
         KRR_CUDA_CHECK(cudaStreamWaitEvent(st, g_pipe.event(EV_JOIN_HI), 0));
         KRR_CUDA_CHECK(cudaStreamWaitEvent(st, g_pipe.event(EV_JOIN_LO), 0));
     }

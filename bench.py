@@ -31,7 +31,9 @@ METRIC = "mixed-precision Cholesky TOp/s (n^3/3 / device time)"
 UNIT = "TOp/s"
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the trailing-update kernel, from the
 # `ncu --set full` capture summarised under profiles/ (bytes; None where no capture exists)
-TRAFFIC_NCU = {}
+TRAFFIC_NCU = {"C3": 12.99e9, "C3h": 6.49e9, "C5p": 7.85e9}
+TRAFFIC_NOTE = ("profiles/r01_gemm_tc_full_C3.md: one launch of the dominant shape O(k+1) at mid factorisation (C3/C3h: k = 32, "
+                "31 tile rows, K = 32 tiles, algorithmic operand bytes 4.3 / 2.1 GB; C5p: k = 48, 2.4 GB)")
 
 
 def load_peaks():
@@ -108,6 +110,27 @@ def update_flops_by_class(h_map, nb):
     return fl
 
 
+def replica_config(cfg, rank):
+    """Multi-GPU = replicas only: rank r factors an independent matrix (seed + 1000 r)."""
+    from dataclasses import replace
+    return replace(cfg, seed=cfg.seed + 1000 * rank)
+
+
+def max_over_ranks(ms, world, device):
+    """Step time of the job = the slowest rank's device time (all_reduce MAX; identity at world = 1)."""
+    if world <= 1:
+        return float(ms)
+    import torch.distributed as dist
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(n, world, ms_per_step):
+    """TOp/s of the whole job: every rank factors one n x n matrix per step (weak scaling)."""
+    return world * (n ** 3 / 3.0) / (ms_per_step * 1e-3) / 1e12
+
+
 def run_ours(args, rank, world, local_rank):
     import paper_2409_01712_b200 as krr
     from paper_2409_01712_b200 import build
@@ -121,8 +144,7 @@ def run_ours(args, rank, world, local_rank):
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=dev)
     # ---- synthetic inputs, resident in HBM before the timed region -------------------------------
-    from dataclasses import replace
-    cfg_r = replace(cfg, seed=cfg.seed + 1000 * rank)           # independent replica per rank
+    cfg_r = replica_config(cfg, rank)                           # independent replica per rank
     n, nb, NT = cfg.n, cfg.nb, cfg.NT
     flags = krr.FLAG_PREROUND_A
     if cfg.lower_tiles_only:                     # C4: "lower-triangular tile storage only"
@@ -195,13 +217,10 @@ def run_ours(args, rank, world, local_rank):
     prof = krr.profile_read()
     upd_ms, upd_launches = prof["update_gemm"]
     krr.profile_enable(0)
-    if world > 1:
-        t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
-        torch.distributed.all_reduce(t, op=torch.distributed.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = max_over_ranks(total_ms, world, dev)
     ms_per_step = total_ms / args.steps
     ops = n ** 3 / 3.0
-    value = world * ops / (ms_per_step * 1e-3) / 1e12
+    value = whole_job_value(n, world, ms_per_step)
 
     phases = {"precision_map": 0.0, "potrf_mp": 0.0, "potrs": 0.0}
     for ev in phase_events:
@@ -248,6 +267,7 @@ def run_ours(args, rank, world, local_rank):
     roofline = {"bound": "tensor", "kernel": "gemm_tc_kernel (MODE_UPDATE: trailing SYRK/GEMM)",
                 "achieved": round(achieved, 2), "peak": round(pw_peak, 2), "unit": "TFLOP/s",
                 "frac": round(achieved / pw_peak, 4), "traffic": TRAFFIC_NCU.get(cfg.name),
+                "traffic_note": TRAFFIC_NOTE if cfg.name in TRAFFIC_NCU else None,
                 "measured": "CUDA events around every launch of the kernel on its launching streams, inside the timed "
                             "region (default schedule: launches share SMs with the panel kernels they overlap)",
                 "frac_serial_schedule": round(upd_flops / (ser_ms * 1e-3) / 1e12 / pw_peak, 4) if ser_ms else None,
@@ -400,10 +420,8 @@ def main():
     elif not args.no_e2e:
         e2e = run_e2e(ctx, max(1, min(args.steps, 2)))
         if world > 1:
-            t = torch.tensor([e2e["ms_per_step"]], dtype=torch.float64, device=ctx[4])
-            torch.distributed.all_reduce(t, op=torch.distributed.ReduceOp.MAX)
-            e2e["ms_per_step"] = float(t.item())
-            e2e["value"] = round(world * cfg.n ** 3 / 3.0 / (e2e["ms_per_step"] * 1e-3) / 1e12, 3)
+            e2e["ms_per_step"] = max_over_ranks(e2e["ms_per_step"], world, ctx[4])
+            e2e["value"] = round(whole_job_value(cfg.n, world, e2e["ms_per_step"]), 3)
         out["e2e"] = e2e
     if rank == 0:
         print(json.dumps(out), flush=True)

@@ -133,10 +133,11 @@ int64_t krr_factor_tile_offset(int64_t n, int nb, const uint8_t* h_map, int i, i
  * flags    KRR_FLAG_PREROUND_A, KRR_FLAG_A_TILED_LOWER, KRR_FLAG_NO_LOOKAHEAD.
  * Streams  the work is ordered after everything already enqueued on `stream`, and work enqueued on
  *          `stream` after the call is ordered after it.  Unless KRR_FLAG_NO_LOOKAHEAD is given the
- *          kernels run on two internal streams (created once per host thread, together with a
- *          pool of CUDA events) that fork from and join back into `stream`: the update of tile
- *          column k+1 by the already final columns overlaps the factorisation of column k
- *          (PAPER.md:206 overlap of the DAG's tasks, :295 lookahead).  The result does not depend
+ *          kernels run on three internal streams (created once per host thread, together with a
+ *          pool of CUDA events) that fork from and join back into `stream`: the diagonal-tile
+ *          chain of column k+1 starts as soon as tile (k+1,k) is stored and runs beside the
+ *          trailing updates and the rest of column k's panel (PAPER.md:206 overlap of the DAG's
+ *          tasks, :295 lookahead).  The result does not depend
  *          on timing (fixed summation order), but differs in the last bits between the two
  *          schedules (the newest column is added in the FP32 epilogue instead of in TMEM).
  */

@@ -202,7 +202,11 @@ __device__ __forceinline__ bool next_item(const GemmOp& op, ItemIter& st, int un
     while (st.t < ntiles) {
         const int t = st.t;
         st.t += nunits;
+#ifdef KRR_EXP_REVERSE_ROWS
+        w.rb = op.rb0 + (op.nrb / CG - 1 - t / ncbu) * CG;
+#else
         w.rb = op.rb0 + (t / ncbu) * CG;
+#endif
         w.cb = op.cb0 + (t % ncbu) * CG;
         if (tile_is_skipped(op, w.rb + CG - 1, w.cb)) continue;      // the whole (pair) block lies above the diagonal
         w.mode = op.mode; w.c = op.c; w.dep = 0;

@@ -1,0 +1,136 @@
+"""GPU parity at BASELINE.json's full sizes, in the launch configuration bench.py times (default
+schedule: three internal streams, CTA pairs, nb of the config).
+
+What the oracle can compute one by one at these sizes: the leading principal block of the factor --
+L[:m, :m] depends only on A[:m, :m] (and, for the emulated mosaic, on the leading block of the map) --
+so the first three tile rows are compared with the oracle run on the leading 3-tile submatrix; the
+precision rule is checked on sampled tiles with norms the oracle computes from host copies of those
+tiles.  What holds at any size: info = 0, positive diagonal, backward error by Gaussian probes and the
+residual of the solve, both evaluated by independent torch-FP64 code (tests/helpers.py).
+Configs: C2 whole against the FP64 oracle; C3 (n = 65536, the bench default); S1 (the rule's genuine
+FP32 / FP16 mosaic) at its bench size.
+"""
+import numpy as np
+import pytest
+import torch
+
+from helpers import probe_backward_error, solve_residual
+from krr_inputs import CONFIGS, make_problem
+from oracle import rounding as R
+from oracle.cholesky import backward_error, tile_cholesky_emulated, tile_cholesky_fp64
+from oracle.precision_map import FP16, FP32, FP8
+from oracle.solve import potrs_fp64
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def krr():
+    from paper_2409_01712_b200 import build
+    build.build()
+    import paper_2409_01712_b200 as k
+    k.lib()
+    return k
+
+
+def relF(a, b):
+    return float(np.linalg.norm(a - b) / np.linalg.norm(b))
+
+
+def leading_block(F, m_tiles):
+    nb = F.nb
+    L = np.zeros((m_tiles * nb, m_tiles * nb))
+    for j in range(m_tiles):
+        for i in range(j, m_tiles):
+            L[i * nb:(i + 1) * nb, j * nb:(j + 1) * nb] = F.tile(i, j).cpu().numpy()
+    return L
+
+
+def check_rule_on_sampled_tiles(A, nb, eps, allowed, d_map, norms, fro, tiles):
+    """The rule (R1/R2) re-evaluated for sampled tiles from host copies of those tiles."""
+    NT = A.shape[0] // nb
+    fro = float(fro.item())
+    u = {FP32: 2.0 ** -24, FP16: 2.0 ** -11, FP8: 2.0 ** -4}
+    for (i, j) in tiles:
+        T = A[i * nb:(i + 1) * nb, j * nb:(j + 1) * nb].cpu().numpy().astype(np.float64)
+        t = float(np.sqrt(np.sum(T * T)))
+        assert abs(float(norms[i, j]) - t) <= 2e-7 * t
+        want = FP32
+        if i != j:
+            for p in sorted(allowed, reverse=True):          # lowest precision first
+                if t * u[p] <= eps * fro / NT:
+                    want = p
+                    break
+        assert int(d_map[i, j]) == want, (i, j)
+
+
+def test_c2_full_size_against_fp64_oracle(krr):
+    cfg = CONFIGS["C2"]                                       # n = 16384, nb = 512, rule eps = 1e-4 {FP32, FP16}
+    A, Y = make_problem(cfg, device="cuda")
+    d_map, norms, amax, fro = krr.precision_map(A, cfg.nb, cfg.eps_target, cfg.allowed)
+    h_map = d_map.cpu()
+    low = np.tril_indices(cfg.NT, -1)
+    assert int((h_map.numpy()[low] != FP32).sum()) == 0      # SURVEY finding 1: the rule gives all FP32
+    F = krr.potrf_mp(A, cfg.nb, d_map, h_map)
+    alpha = krr.potrs(F, Y.clone())
+    torch.cuda.synchronize()
+    assert int(F.info.item()) == 0
+    An = A.cpu().numpy()
+    Lo, info = tile_cholesky_fp64(An, cfg.nb)
+    assert info == 0
+    Lg = F.dense().cpu().numpy()
+    assert relF(Lg, Lo) <= 1e-4
+    assert backward_error(An, Lg) <= 1e-6
+    a64 = potrs_fp64(Lo, Y.cpu().numpy(), cfg.nb)
+    assert relF(alpha.cpu().numpy().astype(np.float64), a64) <= 1e-3
+
+
+@pytest.mark.parametrize("name", ["C3", "S1"])
+def test_full_size_leading_block_and_invariants(krr, name):
+    cfg = CONFIGS[name]
+    A, Y = make_problem(cfg, device="cuda")
+    nb, NT = cfg.nb, cfg.NT
+    d_map, norms, amax, fro = krr.precision_map(A, nb, cfg.eps_target, cfg.allowed)
+    h_map = d_map.cpu()
+    hm = h_map.numpy()
+    low = np.tril_indices(NT, -1)
+    hist = np.bincount(hm[low], minlength=3).tolist()
+    if name == "C3":
+        assert hist == [NT * (NT - 1) // 2, 0, 0]            # SURVEY finding 1
+    else:
+        assert hist[0] > 0 and hist[1] > 0                   # a genuine mosaic
+    sampled = [(0, 0), (1, 0), (2, 1), (NT - 1, 0), (NT - 1, NT - 2), (NT // 2, NT // 3)]
+    check_rule_on_sampled_tiles(A, nb, cfg.eps_target, cfg.allowed, hm, norms.cpu().numpy(), fro, sampled)
+
+    F = krr.potrf_mp(A, nb, d_map, h_map)
+    alpha = krr.potrs(F, Y.clone())
+    torch.cuda.synchronize()
+    assert int(F.info.item()) == 0
+    # leading 3 x 3 tiles against the emulated oracle on the leading submatrix with the same map
+    m = 3
+    Am = A[:m * nb, :m * nb].cpu().numpy()
+    pm = np.ascontiguousarray(hm[:m, :m])
+    Lo, sc, info = tile_cholesky_emulated(Am, nb, pm, preround_a=True)
+    assert info == 0
+    Lg = leading_block(F, m)
+    if (pm[np.tril_indices(m, -1)] == FP32).all():
+        assert relF(Lg, Lo) <= 1e-4
+        assert backward_error(Am, Lg) <= 1e-6
+    else:
+        assert abs(backward_error(Am, Lg) - backward_error(Am, Lo)) <= 0.02 * backward_error(Am, Lo)
+        # first tile column: at most one storage ulp apart
+        for i in range(1, m):
+            g, o = Lg[i * nb:(i + 1) * nb, :nb], Lo[i * nb:(i + 1) * nb, :nb]
+            p = int(pm[i, 0])
+            if p == FP32:
+                assert relF(g, o) <= 1e-4
+            else:
+                tol = 2.5 * R.UNIT_ROUNDOFF[p] * np.abs(o) + 1e-5 * np.abs(o).max()
+                assert np.all(np.abs(g - o) <= tol) and np.mean(g == o) > 0.5
+    # invariants at full size (independent torch-FP64 code)
+    for k in range(0, NT, max(1, NT // 8)):
+        assert float(torch.diagonal(F.tile(k, k)).min()) > 0.0
+        assert float(torch.triu(F.tile(k, k), 1).abs().max()) == 0.0
+    bwd = probe_backward_error(A, F, 4)
+    assert bwd <= (1e-6 if hist[1] == 0 and hist[2] == 0 else 5e-4)
+    assert solve_residual(A, alpha, Y) <= 1e-6

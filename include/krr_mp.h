@@ -67,6 +67,15 @@ typedef enum { KRR_FP32 = 0, KRR_FP16 = 1, KRR_FP8_E4M3 = 2 } krr_prec_t;
                                        instead of CTA pairs (tcgen05 cta_group::2, 256x128 blocks); same
                                        arithmetic, cross-check / comparison.  Pairs need nb % 256 == 0.   */
 
+#define KRR_FLAG_FUSED_CHAIN    64u  /* krr_potrf_mp: run the diagonal-tile chain (in-tile update, POTRF of a
+                                       128-block, TRSM against its inverse, per 128-wide sub-column) as ONE
+                                       launch of nb/128 co-operating CTAs (the POTRF on the epilogue warps,
+                                       items ordered through progress counters in global memory) instead of
+                                       one launch per step; bit-identical results.  Measured equal or a
+                                       few % slower than the default on a B200 (the chain is bound by the
+                                       128 dependent pivots of each block, not by launches), kept as the
+                                       persistent-kernel variant and as a cross-check.                 */
+
 /* Library version (major*100 + minor) and the compute capability it was built for (100). */
 int krr_version(void);
 int krr_built_for_sm(void);

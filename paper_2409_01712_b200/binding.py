@@ -11,6 +11,7 @@ FLAG_A_TILED_LOWER = 4
 FLAG_NO_LOOKAHEAD = 8
 FLAG_FP8_VIA_FP16 = 16
 FLAG_NO_CTA_PAIRS = 32
+FLAG_FUSED_CHAIN = 64
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB = None

@@ -112,7 +112,7 @@ static size_t host_offsets(int NT, int nb, const uint8_t* h_map, std::vector<int
 
 // ---- workspace layout of krr_potrf_mp ----------------------------------------------------------
 struct PotrfWs {
-    size_t off_table, a_amax, tile_amax, scl, W, W2, linv_hi, linv_lo, Hp, Lp, Qp, total;
+    size_t off_table, a_amax, tile_amax, scl, prog, W, W2, linv_hi, linv_lo, Hp, Lp, Qp, total;
 };
 static PotrfWs potrf_ws_layout(int64_t n, int nb, bool any_fp8) {
     const int64_t NT = n / nb;
@@ -124,6 +124,7 @@ static PotrfWs potrf_ws_layout(int64_t n, int nb, bool any_fp8) {
     w.a_amax = o;    o = align_up(o + NT * NT * sizeof(float), 1024);
     w.tile_amax = o; o = align_up(o + nslots * sizeof(float), 1024);
     w.scl = o;       o = align_up(o + (4 + 2 * (nb / kBlk)) * sizeof(float), 1024);
+    w.prog = o;      o = align_up(o + static_cast<size_t>(n / kBlk) * sizeof(int), 1024);   // fused-chain progress, per 128-block
     w.W = o;         o = align_up(o + static_cast<size_t>(n) * nb * sizeof(float), 1024);
     w.W2 = o;        o = align_up(o + static_cast<size_t>(n) * nb * sizeof(float), 1024);   // lookahead: column k+1's partial
     w.linv_hi = o;   o = align_up(o + 2 * static_cast<size_t>(nb) * kBlk * 2, 1024);   // two sets (column parity)
@@ -199,7 +200,8 @@ struct GemmMaps { CUtensorMap H, L, IH[2], IL[2], Q; };
 // cg = 2 runs MODE_UPDATE on CTA pairs (256 x 256 output blocks); needs even block counts.
 static int launch_gemm(const GemmMaps& m, const GemmOp& op, int max_ctas, int cg, cudaStream_t st, int linv_buf = 0) {
     if (op.nrb <= 0 || op.ncb <= 0) return KRR_OK;
-    ProfScope ps(op.mode == MODE_UPDATE ? CAT_UPDATE : (op.mode == MODE_P1 ? CAT_P1 : CAT_P3), st);   // MODE_PANEL counts as panel_trsm
+    // MODE_PANEL counts as panel_trsm, the fused diagonal chain (MODE_DIAG, POTRF included) as potrf128
+    ProfScope ps(op.mode == MODE_UPDATE ? CAT_UPDATE : (op.mode == MODE_P1 ? CAT_P1 : (op.mode == MODE_DIAG ? CAT_POTRF : CAT_P3)), st);
     ++g_launches;
     if (cg == 2 && op.mode == MODE_UPDATE && op.nrb % 2 == 0 && op.rb0 % 2 == 0 && op.ncb % 2 == 0 && op.cb0 % 2 == 0) {
         const int npairs = (op.nrb / 2) * (op.ncb / 2);
@@ -214,8 +216,10 @@ static int launch_gemm(const GemmMaps& m, const GemmOp& op, int max_ctas, int cg
         cfg.attrs = attr; cfg.numAttrs = 1;
         return cudaLaunchKernelEx(&cfg, gemm_tc_kernel<2>, m.H, m.L, m.IH[0], m.IL[0], m.Q, op) == cudaSuccess ? KRR_OK : KRR_ERR_CUDA;
     }
-    // MODE_PANEL: one CTA per two row blocks when there are enough of them (a CTA interleaves two chains)
-    const int ntiles = (op.mode == MODE_PANEL) ? (op.nrb > max_ctas ? (op.nrb + 1) / 2 : op.nrb) : op.nrb * op.ncb;
+    // MODE_PANEL: one CTA per two row blocks when there are enough of them (a CTA interleaves two chains);
+    // MODE_DIAG: one CTA per row block of the diagonal tile
+    const int ntiles = (op.mode == MODE_PANEL) ? (op.nrb > max_ctas ? (op.nrb + 1) / 2 : op.nrb)
+                                               : (op.mode == MODE_DIAG ? op.nrb : op.nrb * op.ncb);
     const int grid = ntiles < max_ctas ? ntiles : max_ctas;
     gemm_tc_kernel<1><<<grid, kGemmThreads, kGemmSmem, st>>>(m.H, m.L, m.IH[linv_buf], m.IL[linv_buf], m.Q, op);
     return cudaGetLastError() == cudaSuccess ? KRR_OK : KRR_ERR_CUDA;
@@ -356,7 +360,9 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
     if (reinterpret_cast<uintptr_t>(d_A) % 16 != 0 || reinterpret_cast<uintptr_t>(d_ws) % 1024 != 0 ||
         reinterpret_cast<uintptr_t>(d_factor) % 128 != 0)
         return KRR_ERR_ARG;
-    if (flags & ~(KRR_FLAG_PREROUND_A | KRR_FLAG_A_TILED_LOWER | KRR_FLAG_NO_LOOKAHEAD | KRR_FLAG_FP8_VIA_FP16 | KRR_FLAG_NO_CTA_PAIRS)) return KRR_ERR_UNSUPPORTED;
+    if (flags & ~(KRR_FLAG_PREROUND_A | KRR_FLAG_A_TILED_LOWER | KRR_FLAG_NO_LOOKAHEAD | KRR_FLAG_FP8_VIA_FP16 | KRR_FLAG_NO_CTA_PAIRS |
+                  KRR_FLAG_FUSED_CHAIN))
+        return KRR_ERR_UNSUPPORTED;
     const int NT = static_cast<int>(n / nb);
     bool any_fp8 = false;
     rc = check_map(NT, h_map, &any_fp8);
@@ -388,6 +394,8 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
     KRR_CUDA_CHECK(cudaMemsetAsync(d_info, 0, sizeof(int), st));
     KRR_CUDA_CHECK(cudaMemsetAsync(d_scales, 0, static_cast<size_t>(NT) * NT * sizeof(float), st));
     KRR_CUDA_CHECK(cudaMemsetAsync(tile_amax, 0, nslots * sizeof(float), st));
+    int* prog = reinterpret_cast<int*>(ws + L.prog);
+    KRR_CUDA_CHECK(cudaMemsetAsync(prog, 0, static_cast<size_t>(n / kBlk) * sizeof(int), st));
     rc = launch(CAT_MISC, offsets_kernel, dim3(1), dim3(32), 0, st, NT, nb, d_map, off);
     if (rc) return rc;
     rc = launch(CAT_MISC, plane_scale_kernel, dim3(1), dim3(1024), 0, st, A, n, scl);
@@ -491,7 +499,18 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
             }
         }
         // ---- diagonal-tile chain: 128-wide sub-columns of tile (k,k) ----
-        for (int c = 0; c < nsub; ++c) {
+        // one launch per step (in-tile update, POTRF of a 128-block, TRSM against its inverse), or with
+        // KRR_FLAG_FUSED_CHAIN one launch of nsub co-resident CTAs (MODE_DIAG): the same arithmetic
+        const bool fused_chain = (flags & KRR_FLAG_FUSED_CHAIN) && nsub <= 16;
+        if (fused_chain) {
+            op.mode = MODE_DIAG; op.c = 0; op.cb0 = 0; op.ncb = 1; op.rb0 = 0; op.nrb = nsub;
+            op.prog = prog + static_cast<size_t>(k) * nsub;
+            op.linv_hi = linv_hi + lb * linv_elems; op.linv_lo = linv_lo + lb * linv_elems;
+            op.linv_scale_w = linv_scale + lb * nsub; op.info = d_info; op.col_base = static_cast<int64_t>(k) * nb + 1;
+            rc = launch_gemm(tm, op, num_sms, 1, sh, lb);
+            if (rc) return rc;
+        }
+        for (int c = 0; c < nsub && !fused_chain; ++c) {
             if (c > 0) {
                 op.mode = MODE_P1; op.c = c; op.cb0 = c; op.ncb = 1; op.rb0 = c; op.nrb = nsub - c;
                 rc = launch_gemm(tm, op, num_sms, 1, sh, lb);

@@ -38,10 +38,11 @@
 #pragma once
 #include "common.cuh"
 #include "ptx.cuh"
+#include "tri128.cuh"
 
 namespace krr {
 
-enum { MODE_UPDATE = 0, MODE_P1 = 1, MODE_P3 = 2, MODE_PANEL = 3 };
+enum { MODE_UPDATE = 0, MODE_P1 = 1, MODE_P3 = 2, MODE_PANEL = 3, MODE_DIAG = 4, MODE_POTRF = 5 /* item of MODE_DIAG */ };
 
 struct GemmOp {
     int mode;
@@ -66,6 +67,13 @@ struct GemmOp {
     const float* scl;     // device float[4]: sx, ss, 1/sx^2, 1/ss  (power-of-two plane scales)
     const float* linv_scale;  // device float[nb/128]: scale of each inverted diagonal block's planes
     unsigned flags;
+    // MODE_DIAG (fused diagonal-tile chain): outputs of the in-kernel POTRF of 128-blocks and the cross-CTA progress
+    int* prog;                // nb/128 ints, zero at launch: prog[r] = completed items of the CTA of row block r
+    __half* linv_hi;          // inverted diagonal blocks, hi / lo FP16 planes [nb][128]
+    __half* linv_lo;
+    float* linv_scale_w;      // = linv_scale, writable
+    int* info;                // krr_potrf_mp's d_info
+    int64_t col_base;         // 1-based global index of the tile column's first scalar column
 };
 
 constexpr int kSlots = 6;                          // shared-memory ring: 6 slots of [A block | B block]
@@ -164,6 +172,10 @@ __device__ __forceinline__ bool tile_is_skipped(const GemmOp& op, int rb, int cb
 // The three warp roles of a CTA walk the same sequence of work items, each with its own iterator.
 //   MODE_UPDATE / MODE_P1 / MODE_P3: item = one output block (of a pair: 256 x 256), blocks dealt
 //     round-robin over the CTAs (pairs) of the grid.
+//   MODE_DIAG (CG = 1, nb/128 co-resident CTAs): the whole chain of the diagonal tile in one launch --
+//     the FP32 POTRF of each 128-block runs on the eight epilogue warps of its CTA (tri128.cuh), the
+//     products on the tensor cores as elsewhere; CTAs order their items through progress counters in
+//     global memory (release: __threadfence + proxy fence + store; acquire: volatile load + fences).
 //   MODE_PANEL (CG = 1): the whole TRSM of a 128-row block of the panel below the diagonal tile,
 //     X_c = (S_c - sum_{c'<c} X_c' L_cc'^T) inv(L_cc)^T for c = 0 .. nsub-1, as the item sequence
 //     P3(0), P1(1), P3(1), P1(2), ...  Row blocks never interact, so a CTA owns its row blocks (dealt
@@ -174,6 +186,7 @@ struct WorkItem {
     int mode, c;     // contraction shape (MODE_UPDATE / MODE_P1 / MODE_P3) and sub-column
     int rb, cb;      // first output row block / column block (of the pair when CG = 2)
     int dep;         // > 0: reads what the item `dep` places earlier in this CTA's sequence wrote
+    int xcta, xneed; // MODE_DIAG: reads what CTA xcta wrote in its first xneed items (xcta < 0: nothing)
 };
 struct ItemIter {
     int t;           // block modes: next block index
@@ -182,6 +195,22 @@ struct ItemIter {
 
 template <int CG>
 __device__ __forceinline__ bool next_item(const GemmOp& op, ItemIter& st, int unit0, int nunits, WorkItem& w) {
+    w.xcta = -1; w.xneed = 0;
+    if (op.mode == MODE_DIAG) {
+        // CTA r owns row block r of the diagonal tile: P3(0), P1(1), P3(1), ..., P3(r-1), P1(r), POTRF(r).
+        // P1(c) reads the rows of block c that CTA c finished with its P3(c-1) (item 2c-2), P3(c) the inverse
+        // CTA c's POTRF (item 2c) produced.
+        const int r = unit0;
+        if (st.it > 2 * r) return false;
+        const int it = st.it++;
+        w.rb = op.rb0 + r;
+        w.dep = it > 0 ? 1 : 0;
+        if (it == 2 * r) { w.mode = MODE_POTRF; w.c = r; }
+        else if (it & 1) { w.mode = MODE_P1; w.c = (it + 1) >> 1; if (w.c < r) { w.xcta = w.c; w.xneed = 2 * w.c - 1; } }
+        else { w.mode = MODE_P3; w.c = it >> 1; w.xcta = w.c; w.xneed = 2 * w.c + 1; }
+        w.cb = w.c;
+        return true;
+    }
     if (op.mode == MODE_PANEL) {
         const int nmine = (op.nrb > unit0) ? (op.nrb - unit0 + nunits - 1) / nunits : 0;    // my row blocks
         if (2 * st.g >= nmine) return false;
@@ -261,7 +290,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
     if (warp == 0 && lane == 0) {
         ptx::prefetch_tmap(&tmH);
         ptx::prefetch_tmap(&tmL);
-        if (op.mode == MODE_P3 || op.mode == MODE_PANEL) { ptx::prefetch_tmap(&tmIH); ptx::prefetch_tmap(&tmIL); }
+        if (op.mode == MODE_P3 || op.mode == MODE_PANEL || op.mode == MODE_DIAG) { ptx::prefetch_tmap(&tmIH); ptx::prefetch_tmap(&tmIL); }
         if (op.fp8q) ptx::prefetch_tmap(&tmQ);
         for (int s = 0; s < kSlots; ++s) {
             ptx::mbar_init(full_bar(s), 1);
@@ -310,11 +339,19 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
             int seq = 0;
             while (next_item<CG>(op, iter, unit0, nunits, w)) {
                 const int rb = w.rb + rank, cb0u = w.cb;
+                if (w.mode == MODE_POTRF) { ++seq; continue; }
                 if (w.dep) {
                     // the operand images this item reads were written by this CTA's epilogue warps `dep` items ago
                     const int need = kEpiWarps * (seq - w.dep + 1);
                     uint32_t spins = 0;
                     while (*done_ctr < need) { if (++spins > (1u << 27)) __trap(); }
+                    __threadfence();
+                    ptx::fence_proxy_async_global();
+                }
+                if (w.xcta >= 0) {
+                    const volatile int* pr = op.prog + w.xcta;
+                    uint32_t spins = 0;
+                    while (*pr < w.xneed) { __nanosleep(64); if (++spins > (1u << 25)) __trap(); }
                     __threadfence();
                     ptx::fence_proxy_async_global();
                 }
@@ -386,6 +423,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
             WorkItem w;
             while (next_item<CG>(op, iter, unit0, nunits, w)) {
                 const int rb = w.rb;
+                if (w.mode == MODE_POTRF) continue;
                 uint32_t cls_next = term_class_load<CG>(op, w.mode, nterms - 1, rb);
                 ptx::mbar_wait(tempty_bar(buf), acc_phase ^ 1u);     // epilogue drained this buffer
                 ptx::tc_fence_after();
@@ -480,8 +518,25 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
         uint32_t acc_phase = 0;
         ItemIter iter = {unit0, 0, 0, 0};
         WorkItem w;
+        int eseq = 0;                                                // items this CTA has finished
         while (next_item<CG>(op, iter, unit0, nunits, w)) {
             const int rb = w.rb + rank, cb0u = w.cb;
+            if (w.mode == MODE_POTRF) {
+                // FP32 Cholesky + inverse of the diagonal 128-block on the epilogue warps; the operand ring is idle
+                // (this is the CTA's last item) and serves as its shared memory
+                struct EpiSync { __device__ __forceinline__ void operator()() const { asm volatile("bar.sync 1, 256;" ::: "memory"); } };
+                EpiSync esync;
+                esync();                                              // every warp's stores of the previous item are done
+                float* tri_sm = reinterpret_cast<float*>(smem_raw + (smem_base - ptx::smem_u32(smem_raw)));
+                potrf128_body<kEpiWarps * 32>(tri_sm, static_cast<int>(threadIdx.x) - 64, esync, op.W, op.nb, rb * kBlk, w.c * kBlk,
+                                              op.linv_hi, op.linv_lo, op.linv_scale_w, op.info, op.col_base + w.c * kBlk);
+                __threadfence();
+                ptx::fence_proxy_async_global();
+                esync();
+                if (threadIdx.x == 64) { __threadfence(); *const_cast<volatile int*>(op.prog + (rb - op.rb0)) = eseq + 1; }
+                ++eseq;
+                continue;
+            }
 #pragma unroll 1
           for (int j2 = 0; j2 < CG; ++j2) {                       // the unit's column blocks, one after the other
             const int cb = cb0u + j2;
@@ -522,12 +577,14 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
                 for (int e = 0; e < 64; ++e) bs[e] = 0.0f;
             }
             // exact power-of-two rescaling: accumulator -> value domain, value -> plane domain
-            const float acc_mul = (w.mode == MODE_P3) ? -op.scl[3] / op.linv_scale[w.c] : op.scl[2];
             const float plane_mul = (w.mode == MODE_P3) ? op.scl[0] : op.scl[1];
             float out[64];
             if (has_acc) {
                 if (j2 == 0) ptx::mbar_wait(tfull_bar(buf), acc_phase);
                 ptx::tc_fence_after();
+                // (read after the accumulator is complete: in MODE_DIAG the scale of the inverted block is written by
+                // another CTA of this launch, and the MMAs could not have run before it was)
+                const float acc_mul = (w.mode == MODE_P3) ? -op.scl[3] / __ldcg(op.linv_scale + w.c) : op.scl[2];
                 uint32_t a0[32], a1[32];
                 const uint32_t taddr = tmem_base + buf * kAccW + (static_cast<uint32_t>(q * 32) << 16) + kAccCols * j2 + 64 * hf;
                 ptx::tmem_ld_32x32(taddr, a0);
@@ -591,13 +648,21 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
                 }
             }
           }   // j2
-            if (op.mode == MODE_PANEL) {
-                // publish this item's operand images to the TMA loads of a later item of this CTA
+            if (op.mode == MODE_PANEL || op.mode == MODE_DIAG) {
+                // publish this item's operand images to the TMA loads of a later item of this CTA (and, in
+                // MODE_DIAG, of the other CTAs: the last warp to finish advances the CTA's progress counter)
                 __threadfence();
                 ptx::fence_proxy_async_global();
                 __syncwarp();
-                if (lane == 0) atomicAdd_block(const_cast<int*>(done_ctr), 1);
+                if (lane == 0) {
+                    const int old = atomicAdd_block(const_cast<int*>(done_ctr), 1);
+                    if (op.mode == MODE_DIAG && old == kEpiWarps * (eseq + 1) - 1) {
+                        __threadfence();
+                        *const_cast<volatile int*>(op.prog + (rb - op.rb0)) = eseq + 1;
+                    }
+                }
             }
+            ++eseq;
         }
     }
 

@@ -24,7 +24,7 @@ namespace krr {
 // phase timestamps for kernel tuning (compiled in only by the tuning harness)
 #ifdef KRR_TRI_TIMING
 __device__ long long g_tri_t[32];
-#define KRR_TRI_T(i) do { if (threadIdx.x == 0) g_tri_t[i] = clock64(); } while (0)
+#define KRR_TRI_T(i) do { if (tid == 0) g_tri_t[i] = clock64(); } while (0)
 #else
 #define KRR_TRI_T(i) do { } while (0)
 #endif
@@ -35,7 +35,7 @@ __device__ long long g_tri_t[32];
 constexpr int kAbUnroll = KRR_TRI_UNROLL_AB;
 constexpr int kTriThreads = 512;
 constexpr int kTriLd = 132;                       // 16-byte aligned rows; LDS.128 by row is conflict free
-constexpr int kTriSmem = (2 * kBlk * kTriLd + kBlk) * 4;   // L, inv(L), reciprocals of the diagonal of L
+constexpr int kTriSmem = (2 * kBlk * kTriLd + kBlk + 32) * 4;   // L, inv(L), reciprocals of the diagonal of L, reduction scratch
 
 __device__ __forceinline__ float rsqrt_newton(float d) {
     float rs;
@@ -216,34 +216,39 @@ __device__ __forceinline__ void inv128_offdiag(const float* l, float* x, float* 
 // Writes L (lower, zeros above) back into W and inv(L) as scaled FP16 hi/lo planes into
 // linv_hi/lo ([nb][128] row-major, rows c0..c0+127) with their power-of-two scale in linv_scale.
 // col_base = 1-based global index of the block's first column, for info (LAPACK convention).
-__global__ void __launch_bounds__(kTriThreads, 1)
-potrf128_kernel(float* __restrict__ W, int nb, int r0, int c0, __half* __restrict__ linv_hi,
-                __half* __restrict__ linv_lo, float* __restrict__ linv_scale, int* __restrict__ info,
-                int64_t col_base) {
-    extern __shared__ __align__(16) float tri_sm[];
+// The body runs on NTHR threads (tid = 0 .. NTHR-1, whole warps) that synchronise through `sync()`:
+// the stand-alone kernel below uses the whole CTA, the fused diagonal-tile chain of gemm_tc.cuh its
+// eight epilogue warps and a named barrier.  tri_sm: kTriSmem bytes of shared memory, 16-byte aligned.
+template <int NTHR, typename Sync>
+__device__ __forceinline__ void potrf128_body(float* tri_sm, int tid, Sync sync, float* __restrict__ W, int nb, int r0,
+                                              int c0, __half* __restrict__ linv_hi, __half* __restrict__ linv_lo,
+                                              float* __restrict__ linv_scale, int* __restrict__ info, int64_t col_base) {
     float* a = tri_sm;                       // [128][132] : S, then L
     float* x = tri_sm + kBlk * kTriLd;       // [128][132] : inv(L); rows 0..31 x columns 32.. double as scratch
     float* rinv = x + kBlk * kTriLd;         // [128]      : 1 / L_jj
-    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    constexpr int NW = kTriThreads / 32;
+    float* s_red = rinv + kBlk;              // [NTHR / 32]
+    const int warp = tid >> 5, lane = tid & 31;
+    constexpr int NW = NTHR / 32;
     // W is block-column-major: element (r, c) of 128x128 block (rb, cb) at ((rb*nsub + cb)*128 + c)*128 + r
     float* wblk = W + (static_cast<int64_t>(r0 / kBlk) * (nb / kBlk) + c0 / kBlk) * (kBlk * kBlk);
     KRR_TRI_T(0);
     {
-        // coalesced column reads (lane = row), all in flight before the first store
-        constexpr int PER = kBlk * kBlk / kTriThreads;
-        float v[PER];
+        // coalesced column reads (lane = row), 32 per thread in flight before the first store
+        constexpr int PER = 32;
+        for (int base = 0; base < kBlk * kBlk; base += PER * NTHR) {
+            float v[PER];
 #pragma unroll
-        for (int u = 0; u < PER; ++u) v[u] = wblk[tid + u * kTriThreads];
+            for (int u = 0; u < PER; ++u) v[u] = wblk[base + tid + u * NTHR];
 #pragma unroll
-        for (int u = 0; u < PER; ++u) {
-            const int idx = tid + u * kTriThreads, r = idx & (kBlk - 1), c = idx >> 7;
-            a[r * kTriLd + c] = v[u];
+            for (int u = 0; u < PER; ++u) {
+                const int idx = base + tid + u * NTHR, r = idx & (kBlk - 1), c = idx >> 7;
+                a[r * kTriLd + c] = v[u];
+            }
         }
-        for (int idx = tid; idx < kBlk * (kBlk / 4); idx += kTriThreads)
+        for (int idx = tid; idx < kBlk * (kBlk / 4); idx += NTHR)
             *reinterpret_cast<float4*>(x + (idx >> 5) * kTriLd + (idx & 31) * 4) = make_float4(0.f, 0.f, 0.f, 0.f);
     }
-    __syncthreads();
+    sync();
     KRR_TRI_T(1);
     float* tscr = x + 32;                    // scratch strip of the inverse's off-diagonal rows
     for (int jb = 0; jb < 4; ++jb) {
@@ -257,16 +262,16 @@ potrf128_kernel(float* __restrict__ W, int nb, int r0, int c0, __half* __restric
         } else if (jb >= 2) {
             inv_row_phase1(a, x, tscr, jb - 1, warp - 1, NW - 1, lane);
         }
-        __syncthreads();
+        sync();
         KRR_TRI_T(2 + 5 * jb);
         const int R = kBlk - (j0 + 32);                 // rows below the diagonal block
         // B: panel, one thread per row below (warps 1 ..); warp 0 inverts the diagonal sub-block; the
-        //    last warps finish block row jb-1 of the inverse
-        constexpr int NB2 = 8;                          // warps NW-8 .. NW-1
+        //    remaining warps finish block row jb-1 of the inverse
+        const int first_free = 1 + R / 32;              // warps first_free .. NW-1 have neither job
         if (warp == 0) inv32_warp(a, rinv, x, j0, lane);
         else if (tid - 32 < R) panel32_row(a, rinv, j0, j0 + 32 + (tid - 32));
-        else if (jb >= 2 && warp >= NW - NB2) inv_row_phase2(x, tscr, jb - 1, warp - (NW - NB2), NB2, lane);
-        __syncthreads();
+        else if (jb >= 2) inv_row_phase2(x, tscr, jb - 1, warp - first_free, NW - first_free, lane);
+        sync();
         KRR_TRI_T(3 + 5 * jb);
         if (R > 0) {
             // C: trailing update S_ic -= L_i,jb L_c,jb^T for the 32-column blocks right of jb (lower part):
@@ -275,22 +280,21 @@ potrf128_kernel(float* __restrict__ W, int nb, int r0, int c0, __half* __restric
             const int cb = jb + 1 + warp % ncb, wi = warp / ncb, wn = (NW - 1 - warp % ncb) / ncb + 1;
             const int rr = 32 * cb;
             abt32_sub_rows(a + j0, a + rr * kTriLd + j0, a + rr, rr + wi, kBlk, wn, lane);
-            __syncthreads();
+            sync();
             KRR_TRI_T(5 + 5 * jb);
         }
     }
     KRR_TRI_T(22);
     // block row 3 of the inverse
     inv_row_phase1(a, x, tscr, 3, warp, NW, lane);
-    __syncthreads();
+    sync();
     inv_row_phase2(x, tscr, 3, warp, NW, lane);
-    __syncthreads();
+    sync();
     KRR_TRI_T(23);
     // power-of-two scale of the inverse's planes: max|x| * si <= 2^14
-    __shared__ float s_red[kTriThreads / 32];
     {
         float m = 0.0f;
-        for (int idx = tid; idx < kBlk * kBlk; idx += kTriThreads) {
+        for (int idx = tid; idx < kBlk * kBlk; idx += NTHR) {
             const int r = idx >> 7, c = idx & 127;
             if (c <= r) m = fmaxf(m, fabsf(x[r * kTriLd + c]));
         }
@@ -298,12 +302,12 @@ potrf128_kernel(float* __restrict__ W, int nb, int r0, int c0, __half* __restric
         for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
         if (lane == 0) s_red[warp] = m;
     }
-    __syncthreads();
+    sync();
     float si = 1.0f;
     {
         float m = 0.0f;
 #pragma unroll
-        for (int w = 0; w < kTriThreads / 32; ++w) m = fmaxf(m, s_red[w]);
+        for (int w = 0; w < NTHR / 32; ++w) m = fmaxf(m, s_red[w]);
         if (m > 0.0f && m < 3.0e38f) {
             int e;
             frexpf(m, &e);                 // m <= 2^e
@@ -312,12 +316,12 @@ potrf128_kernel(float* __restrict__ W, int nb, int r0, int c0, __half* __restric
     }
     if (tid == 0) linv_scale[c0 / kBlk] = si;
     // L back into W: coalesced column writes (lane = row)
-    for (int idx = tid; idx < kBlk * kBlk; idx += kTriThreads) {
+    for (int idx = tid; idx < kBlk * kBlk; idx += NTHR) {
         const int r = idx & (kBlk - 1), c = idx >> 7;
         wblk[idx] = (c <= r) ? a[r * kTriLd + c] : 0.0f;
     }
     // inverse as scaled hi/lo FP16 planes, row-major
-    for (int idx = tid; idx < kBlk * (kBlk / 4); idx += kTriThreads) {
+    for (int idx = tid; idx < kBlk * (kBlk / 4); idx += NTHR) {
         const int r = idx / (kBlk / 4), c4 = (idx % (kBlk / 4)) * 4;
         const float4 xv4 = *reinterpret_cast<const float4*>(x + r * kTriLd + c4);
         const float xs[4] = {xv4.x, xv4.y, xv4.z, xv4.w};
@@ -333,6 +337,18 @@ potrf128_kernel(float* __restrict__ W, int nb, int r0, int c0, __half* __restric
         *reinterpret_cast<uint2*>(linv_lo + static_cast<int64_t>(c0 + r) * kBlk + c4) = *reinterpret_cast<const uint2*>(lo);
     }
     KRR_TRI_T(31);
+}
+
+
+struct CtaSync { __device__ __forceinline__ void operator()() const { __syncthreads(); } };
+
+__global__ void __launch_bounds__(kTriThreads, 1)
+potrf128_kernel(float* __restrict__ W, int nb, int r0, int c0, __half* __restrict__ linv_hi,
+                __half* __restrict__ linv_lo, float* __restrict__ linv_scale, int* __restrict__ info,
+                int64_t col_base) {
+    extern __shared__ __align__(16) float tri_sm[];
+    potrf128_body<kTriThreads>(tri_sm, static_cast<int>(threadIdx.x), CtaSync(), W, nb, r0, c0, linv_hi, linv_lo, linv_scale,
+                               info, col_base);
 }
 
 // Inverse of the stored 128x128 diagonal blocks of L for krr_potrs: block b = blockIdx.x is rows and

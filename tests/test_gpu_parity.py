@@ -139,6 +139,30 @@ def test_lookahead_pipeline_matches_serial_schedule(krr):
         assert relF(Lg, Lo) <= 1e-4 and backward_error(An, Lg) <= 1e-6
 
 
+@pytest.mark.parametrize("nb,n", [(256, 2048), (1024, 4096)])
+def test_fused_diagonal_chain_is_bit_identical_to_unfused(krr, nb, n):
+    """The diagonal-tile chain as ONE launch of nb/128 co-operating CTAs (KRR_FLAG_FUSED_CHAIN: POTRF of the
+    128-blocks on the epilogue warps, items ordered through progress counters in global memory) against one
+    launch per step (default): the same arithmetic in the same order, so the factors agree bit for bit --
+    in both schedules, repeatedly (no dependence on timing)."""
+    cfg = replace(scaled_config(CONFIGS["S1"], nb=nb, n=n, p=1536), genotype="maf", gamma_scale=4.0)
+    A, _ = make_problem(cfg, device="cuda")
+    rng = np.random.default_rng(7)
+    pmap = oracle_uniform(cfg.NT, R.FP32)
+    for i in range(cfg.NT):
+        for j in range(i):
+            pmap[i, j] = rng.integers(0, 3)
+    h = torch.from_numpy(np.ascontiguousarray(pmap))
+    for extra in (0, krr.FLAG_NO_LOOKAHEAD):
+        F1 = krr.potrf_mp(A, cfg.nb, h.cuda(), h, flags=krr.FLAG_PREROUND_A | extra)
+        F2 = krr.potrf_mp(A, cfg.nb, h.cuda(), h, flags=krr.FLAG_PREROUND_A | extra | krr.FLAG_FUSED_CHAIN)
+        F3 = krr.potrf_mp(A, cfg.nb, h.cuda(), h, flags=krr.FLAG_PREROUND_A | extra)
+        torch.cuda.synchronize()
+        assert int(F1.info.item()) == 0 and int(F2.info.item()) == 0
+        assert torch.equal(F1.payload, F2.payload) and torch.equal(F1.scales, F2.scales)
+        assert torch.equal(F1.payload, F3.payload)
+
+
 @pytest.mark.parametrize("prec", ["fp32", "mixed"])
 def test_cta_pair_updates_match_single_cta(krr, prec):
     """Trailing updates on CTA pairs (cta_group::2, 256x128 blocks, default when nb % 256 == 0) against

@@ -1,0 +1,45 @@
+"""CPU oracle of the Build phase (TEST INFRASTRUCTURE, NOT PRODUCT; see oracle/__init__.py).
+
+What it computes, as the paper defines it:
+
+* Alg. 2: K[i, j] = KernelMatrix(type, gamma, G1[i, :], G2[j, :]) for every pair.
+* Alg. 5 l.4, Gaussian kernel: exp(-gamma * ||p1 - p2||^2) (the minus sign inside
+  the norm is lost in the extraction; cf. :173 "d_ij = sum_k (g_ki - g_kj)^2" and :186; R14).
+* Alg. 3 l.3: the matrix handed to FACTORIZE is K + alpha*Id (alpha = the regulariser
+  lambda of DESIGN.md R12).
+
+`kernel_matrix_definition` is that definition written out: the squared distance of every pair from the
+differences themselves, in exact integer arithmetic, the exponential in FP64.  No expansion into
+norms and a Gram matrix -- that is the *method* of PAPER.md:173-190, which the CUDA path implements
+and `squared_distance_by_expansion` restates only so that the tests can pin the identity the method
+rests on (D~ = D + D^T - 2 G G^T, :186).
+"""
+import numpy as np
+
+
+def squared_distances(G1, G2):
+    """d_ij = sum_k (G1[i,k] - G2[j,k])^2, exact (int64), by rows: no (n1, n2, p) temporary."""
+    G1 = np.asarray(G1, dtype=np.int64)
+    G2 = np.asarray(G2, dtype=np.int64)
+    D = np.empty((G1.shape[0], G2.shape[0]), dtype=np.int64)
+    for i in range(G1.shape[0]):
+        diff = G2 - G1[i][None, :]
+        D[i] = np.einsum("jk,jk->j", diff, diff)
+    return D
+
+
+def kernel_matrix_definition(G, gamma, lam):
+    """A = K + lam*I in FP64: K_ij = exp(-gamma * d_ij) (Alg. 5 l.4), d_ij by the definition."""
+    D = squared_distances(G, G)
+    A = np.exp(-float(gamma) * D.astype(np.float64))
+    A[np.diag_indices_from(A)] += float(lam)
+    return A
+
+
+def squared_distance_by_expansion(G):
+    """The method's identity: D with the squared norms down its columns, D~ = D + D^T,
+    D~ <- D~ - 2 G G^T.  Integer arithmetic; returned for the tests to compare with the definition."""
+    G = np.asarray(G, dtype=np.int64)
+    s = np.einsum("ik,ik->i", G, G)
+    D = np.tile(s[None, :], (G.shape[0], 1))          # every row holds (||g_1||^2, ..., ||g_n||^2)
+    return D + D.T - 2 * (G @ G.T)

@@ -298,6 +298,46 @@ def run_ours(args, rank, world, local_rank):
     return out, (A, Y, krr, cfg, dev)
 
 
+def run_build_phase(ctx, peaks, reps=3):
+    """Build phase (krr_build): A = K + lambda*I from the int8 genotypes on the INT8 tensor
+    cores with the exp fused into the epilogue.  Reported beside the step, not inside it (the step is the
+    Associate phase).  Ops = n^2 p for the lower triangle of G G^T (2 per multiply-add, half the matrix);
+    peak = 2 x the measured bf16 peak (INT8 : bf16 nominal ratio)."""
+    A, Y, krr, cfg, dev = ctx
+    from krr_inputs.synth import _all_genotypes
+    G = _all_genotypes(cfg, dev)
+    n, p, nb = cfg.n, cfg.p, cfg.nb
+    ld = (p + 15) // 16 * 16
+    Gp = torch.zeros((n, ld), dtype=torch.int8, device=dev)
+    Gp[:, :p] = G
+    del G
+    out = torch.zeros(cfg.NT * (cfg.NT + 1) // 2 * nb * nb, dtype=torch.float32, device=dev)
+    times = []
+    for it in range(reps + 1):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        krr.krr_build(Gp[:, :p], cfg.gamma, cfg.lam, nb, tiled_lower=True, out=out)
+        e1.record()
+        torch.cuda.synchronize()
+        if it > 0:
+            times.append(e0.elapsed_time(e1))
+    ms = sorted(times)[len(times) // 2]
+    ops = float(n) * n * p * (cfg.NT + 1) / cfg.NT           # lower tiles incl. full diagonal tiles
+    # spot check against the matrix the step factorised (same genotypes): tile (NT-1, 0)
+    chk = None
+    if not cfg.lower_tiles_only and A is not None:
+        T = out.reshape(-1, nb, nb)[cfg.NT - 1]
+        ref = A[(cfg.NT - 1) * nb:, :nb]
+        chk = float(((T - ref).abs() / ref).max())
+    achieved = ops / (ms * 1e-3) / 1e12
+    peak = 2.0 * peaks["bf16_sustained"]
+    return {"kernel": "build_tc_kernel (tcgen05 kind::i8, CTA pairs, exp epilogue)", "ms": round(ms, 3),
+            "TOp/s": round(achieved, 1), "frac_of_int8_peak": round(achieved / peak, 4),
+            "peak": f"2 x bf16 sustained {peaks['bf16_sustained']} TF/s (nominal INT8 : bf16 ratio)",
+            "ops": "n^2 p (NT+1)/NT: multiply-adds x 2 over the lower tiles of G G^T",
+            "max_rel_diff_vs_generator_tile": chk}
+
+
 def run_e2e(ctx, steps):
     """Same metric through the C ABI with HOST buffers (krr_associate_host): H2D of A and Y and D2H
     of alpha / map / info inside the timed region."""
@@ -389,6 +429,7 @@ def main():
     ap.add_argument("--sample-tiles", type=int, default=28, help="tiles per dimension of the CPU-oracle sample")
     ap.add_argument("--potrf-flags", type=int, default=0, help="extra KRR_FLAG_* bits for krr_potrf_mp (experiments)")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-build", action="store_true", help="skip the Build-phase (krr_build) timing")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
@@ -414,6 +455,11 @@ def main():
                                "sample": f"leading {ns}x{ns} principal submatrix of {cfg.name} (nb={cfg.nb}), "
                                          "FP64 tile Cholesky of oracle/cholesky.py as it stands"}
         del A_s
+    if rank == 0 and world == 1 and not args.no_build:
+        try:
+            out["build_phase"] = run_build_phase(ctx, load_peaks())
+        except Exception as ex:                      # an extra, never masks the measurement
+            out["build_phase"] = {"error": repr(ex)}
     if cfg.lower_tiles_only and not args.no_e2e:
         out["e2e"] = {"value": None, "unit": UNIT, "skipped": "krr_associate_host takes the dense row-major host matrix; "
                       "this workload is held as packed lower tiles only"}

@@ -44,7 +44,7 @@ typedef enum { KRR_FP32 = 0, KRR_FP16 = 1, KRR_FP8_E4M3 = 2 } krr_prec_t;
 #define KRR_ERR_MAP        (-6)   /* invalid precision code in h_map, or non-FP32 diagonal tile    */
 #define KRR_ERR_UNSUPPORTED (-7)  /* a flag bit this build does not implement                      */
 
-/* flags (krr_precision_map, krr_potrf_mp, krr_associate_host) */
+/* flags (krr_precision_map, krr_potrf_mp, krr_associate_host, krr_build) */
 #define KRR_FLAG_PREROUND_A     1u  /* round the off-diagonal tiles of A into their storage precision
                                        before factorising ("lower the precision of the
                                        off-diagonal tiles ... followed by the mixed-precision
@@ -190,6 +190,29 @@ int krr_associate_host(const float* h_A, int64_t n, int64_t lda, int nb,
                        const float* h_Y, int nrhs, float* h_alpha,
                        uint8_t* h_map, int* h_info,
                        void* d_arena, size_t arena_bytes, void* stream);
+
+/* ---------------------------------------------------------------------------------------------
+ * krr_build -- Build phase (Alg. 2 :92-106 with the Gaussian kernel of Alg. 5 :136-143;
+ * the method of V-B1 :173-190 and VI-B2 :207-209):
+ *   A = K + lambda*I,  K_ij = exp(-gamma * ||g_i - g_j||^2),  g_i = row i of G,
+ * with ||g_i - g_j||^2 = s_i + s_j - 2 <g_i, g_j>, the Gram matrix on the INT8 tensor cores (INT32
+ * accumulation, exact), the squared norms s as one folded vector, each 256 x 256 block of squared
+ * distances generated on chip and exponentiated before it is stored (no n x n integer temporary).
+ * d_G    in   n x p signed 8-bit genotypes, row-major with row pitch ldg bytes (ldg >= p, ldg % 16 == 0,
+ *             16-byte aligned); any int8 values (the workloads use {0,1,2}); p <= 133000 keeps the INT32
+ *             sums exact.  Not modified.
+ * gamma, lambda  kernel bandwidth and regulariser; the diagonal is (float)(1 + lambda) exactly.
+ * d_A    out  the lower TILES of A (tile row >= tile column; diagonal tiles as full squares) in FP32:
+ *             n x n row-major with lda (lda % 4 == 0; tiles above the diagonal are not written), or
+ *             packed lower tiles with KRR_FLAG_A_TILED_LOWER -- the two input layouts of krr_precision_map
+ *             and krr_potrf_mp.  exp is evaluated in FP32 (expf of the FP32 product gamma*d2, d2 exact):
+ *             entries agree with the FP64-evaluated, FP32-rounded kernel to a few ulp.
+ * n % 256 == 0, nb % 256 == 0, n % nb == 0.  d_ws: krr_build_workspace(n) bytes (the folded vector s).
+ * The confounder (real-valued covariate) term of :190 is not implemented yet.
+ */
+size_t krr_build_workspace(int64_t n);
+int krr_build(const int8_t* d_G, int64_t n, int64_t p, int64_t ldg, float gamma, float lambda,
+              float* d_A, int64_t lda, int nb, unsigned flags, void* d_ws, size_t ws_bytes, void* stream);
 
 /* Number of kernels the last krr_* call on this thread enqueued (for bench.py's gpu_launches). */
 int64_t krr_last_launch_count(void);

@@ -22,7 +22,7 @@ ERRORS = {-1: "KRR_ERR_ARG", -2: "KRR_ERR_SHAPE", -3: "KRR_ERR_WORKSPACE", -4: "
 EXPORTS = ["krr_version", "krr_built_for_sm", "krr_tile_slot", "krr_precision_map_workspace",
            "krr_precision_map", "krr_factor_bytes", "krr_factor_tile_offset",
            "krr_potrf_mp_workspace", "krr_potrf_mp", "krr_potrs_workspace", "krr_potrs",
-           "krr_associate_host_arena", "krr_associate_host", "krr_last_launch_count",
+           "krr_associate_host_arena", "krr_associate_host", "krr_build_workspace", "krr_build", "krr_last_launch_count",
            "krr_profile_enable", "krr_profile_read"]
 
 
@@ -71,6 +71,10 @@ def lib():
     L.krr_associate_host.restype = c.c_int
     L.krr_associate_host.argtypes = [vp, i64, i64, c.c_int, c.c_float, u32, c.c_int, u32, vp, c.c_int, vp,
                                      vp, vp, vp, sz, vp]
+    L.krr_build_workspace.restype = sz
+    L.krr_build_workspace.argtypes = [i64]
+    L.krr_build.restype = c.c_int
+    L.krr_build.argtypes = [vp, i64, i64, i64, c.c_float, c.c_float, vp, i64, c.c_int, u32, vp, sz, vp]
     L.krr_last_launch_count.restype = i64
     L.krr_profile_enable.restype = c.c_int
     L.krr_profile_enable.argtypes = [u32]
@@ -274,3 +278,27 @@ def associate_host(h_A, nb, h_Y, eps_target=0.0, allowed=(FP32,), force_prec=-1,
                                 _ptr(alpha), _ptr(h_map), _ptr(h_info), _ptr(arena), arena.numel(), _stream()),
            "krr_associate_host")
     return alpha, h_map, int(h_info[0]), arena
+
+
+def krr_build(G, gamma, lam, nb, tiled_lower=False, out=None):
+    """krr_build (named in full: `build` is this package's compile step): A = K + lam*I (Gaussian kernel) from CUDA int8 genotypes G (n x p, row-major, row pitch a
+    multiple of 16 bytes).  Returns A: n x n FP32 with the lower tiles written (the rest zero), or the packed
+    lower tiles with tiled_lower."""
+    L = lib()
+    assert G.dtype == torch.int8 and G.is_cuda and G.stride(1) == 1
+    n, p = G.shape
+    NT = n // nb
+    dev = G.device
+    if out is None:
+        out = (torch.zeros(NT * (NT + 1) // 2 * nb * nb, dtype=torch.float32, device=dev) if tiled_lower
+               else torch.zeros((n, n), dtype=torch.float32, device=dev))
+    wsb = int(L.krr_build_workspace(n))
+    if wsb == 0:
+        raise KrrError("krr_build_workspace: n must be a multiple of 256")
+    ws = _ws(wsb, dev)
+    flags = FLAG_A_TILED_LOWER if tiled_lower else 0
+    lda = nb if tiled_lower else out.stride(0)
+    _check(L.krr_build(_ptr(G), n, p, G.stride(0), float(gamma), float(lam), _ptr(out), lda, nb, flags, _ptr(ws), wsb,
+                       _stream()), "krr_build")
+    return out
+

@@ -8,6 +8,7 @@
 #include <cstring>
 #include <vector>
 
+#include "build.cuh"
 #include "common.cuh"
 #include "gemm_tc.cuh"
 #include "panel.cuh"
@@ -764,3 +765,73 @@ int krr_associate_host(const float* h_A, int64_t n, int64_t lda, int nb, float e
 }
 
 }  // extern "C"
+
+// ------------------------------------------------------------------------- Build phase (NEXT-1)
+extern "C" {
+
+size_t krr_build_workspace(int64_t n) {
+    if (n <= 0 || n % 256 != 0) return 0;
+    return align_up(static_cast<size_t>(n) * sizeof(int), 1024);
+}
+
+int krr_build(const int8_t* d_G, int64_t n, int64_t p, int64_t ldg, float gamma, float lambda, float* d_A, int64_t lda,
+              int nb, unsigned flags, void* d_ws, size_t ws_bytes, void* stream) {
+    g_launches = 0;
+    if (!d_G || !d_A || !d_ws) return KRR_ERR_ARG;
+    int rc = check_shape(n, nb);
+    if (rc) return rc;
+    if (n % 256 != 0 || nb % 256 != 0) return KRR_ERR_SHAPE;
+    if (p < 1 || p > 133000 || ldg < p || ldg % 16 != 0) return KRR_ERR_ARG;      // INT32 sums of int8 squares stay exact
+    const bool tiled = flags & KRR_FLAG_A_TILED_LOWER;
+    if (flags & ~KRR_FLAG_A_TILED_LOWER) return KRR_ERR_UNSUPPORTED;
+    if (!tiled && (lda < n || lda % 4 != 0)) return KRR_ERR_ARG;
+    if (reinterpret_cast<uintptr_t>(d_G) % 16 != 0 || reinterpret_cast<uintptr_t>(d_A) % 16 != 0 ||
+        reinterpret_cast<uintptr_t>(d_ws) % 16 != 0)
+        return KRR_ERR_ARG;
+    if (ws_bytes < krr_build_workspace(n)) return KRR_ERR_WORKSPACE;
+    int num_sms = 0;
+    rc = check_device(&num_sms);
+    if (rc) return rc;
+    static bool attr_done = false;
+    if (!attr_done) {
+        KRR_CUDA_CHECK(cudaFuncSetAttribute(build_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kBuildSmem));
+        attr_done = true;
+    }
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    int* sq = static_cast<int*>(d_ws);
+    rc = launch(CAT_MISC, row_sqnorm_kernel, dim3(static_cast<unsigned>((n + 7) / 8)), dim3(256), 0, st, d_G, n, p, ldg, sq);
+    if (rc) return rc;
+    // genotypes as a [n][p] byte matrix, box = 128 SNPs x 128 patients, 128-byte swizzle, zero fill past p
+    EncodeTiledFn enc = get_encode_fn();
+    if (!enc) return KRR_ERR_CUDA;
+    CUtensorMap tmG;
+    cuuint64_t gdim[2] = {static_cast<cuuint64_t>(p), static_cast<cuuint64_t>(n)};
+    cuuint64_t gstride[1] = {static_cast<cuuint64_t>(ldg)};
+    cuuint32_t box[2] = {128u, static_cast<cuuint32_t>(kBlk)};
+    cuuint32_t estr[2] = {1, 1};
+    if (enc(&tmG, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<int8_t*>(d_G), gdim, gstride, box, estr,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+        return KRR_ERR_CUDA;
+    BuildOp op;
+    op.n = n; op.p = p; op.nb = nb; op.tiled = tiled ? 1 : 0; op.gamma = gamma;
+    op.diag = static_cast<float>(1.0 + static_cast<double>(lambda));
+    op.sq = sq; op.A = d_A; op.lda = lda;
+    const int64_t NT = n / nb, upt = nb / 256;
+    const int64_t total = upt * upt * NT * (NT + 1) / 2;
+    const int64_t max_pairs = num_sms / 2;
+    const int grid = static_cast<int>(2 * (total < max_pairs ? total : max_pairs));
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof(cfg));
+    cfg.gridDim = dim3(grid); cfg.blockDim = dim3(kBuildThreads); cfg.dynamicSmemBytes = kBuildSmem; cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = 2; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    ProfScope ps(CAT_MISC, st);
+    ++g_launches;
+    return cudaLaunchKernelEx(&cfg, build_tc_kernel, tmG, op) == cudaSuccess ? KRR_OK : KRR_ERR_CUDA;
+}
+
+}  // extern "C"
+

@@ -1,0 +1,219 @@
+// Build phase (Alg. 2 :92-106, Alg. 5 :136-143, V-B1 :173-190, VI-B2 :207-209):
+//   A = K + lambda*I,  K_ij = exp(-gamma * ||g_i - g_j||^2),  g_i = row i of the int8 genotype matrix G,
+// with the squared distance expanded as  d2_ij = s_i + s_j - 2 <g_i, g_j>  (:186), the Gram matrix G G^T on the
+// INT8 tensor cores (tcgen05 kind::i8, INT32 accumulation -- exact), the squared norms s folded into one vector
+// (:209 "fold the column entries of the matrix D ... store D as a one-dimensional vector"), the tiles of D
+// generated on demand and exponentiated before they are released (:209) -- no n x n integer temporary.
+//
+// Only the lower TILES of A (tile row >= tile column, diagonal tiles as full squares) are produced: that
+// is what the Associate phase reads.  One persistent, warp-specialised kernel on CTA pairs (cluster of 2,
+// cta_group::2): a pair computes a 256 x 256 block over the whole SNP range, each CTA staging 128 rows of
+// the row operand and 128 of the column operand per 128-SNP chunk (TMA, 128-byte swizzle, 6-slot ring);
+// the INT32 accumulators are double-buffered in TMEM so that the exp epilogue of a block overlaps the
+// MMAs of the next.  SNP counts that are not a multiple of 128 rely on TMA's zero fill.
+#pragma once
+#include "common.cuh"
+#include "ptx.cuh"
+
+namespace krr {
+
+struct BuildOp {
+    int64_t n, p;
+    int nb;                 // tile size of A (which tiles are "lower", and the packed layout)
+    int tiled;              // KRR_FLAG_A_TILED_LOWER
+    float gamma;
+    float diag;             // (float)(1.0 + lambda): K_ii = exp(0) = 1 exactly
+    const int* sq;          // s_i = sum_k g_ik^2
+    float* A;
+    int64_t lda;
+};
+
+constexpr int kBuildSlots = 6;
+constexpr int kBuildSlotBytes = 2 * kBlk * 128;     // [128 rows x 128 SNPs of the row operand | same of the column operand]
+constexpr int kBuildThreads = 320;                  // warp 0 TMA, warp 1 MMA (+ TMEM alloc), 2-9 epilogue
+constexpr int kBuildSmem = kBuildSlots * kBuildSlotBytes + 1024 + 256;
+
+// s_i = sum_k g_ik^2 (INT32; exact while p * 127^2 < 2^31).  One warp per row, 16-byte loads.
+__global__ void __launch_bounds__(256)
+row_sqnorm_kernel(const int8_t* __restrict__ G, int64_t n, int64_t p, int64_t ldg, int* __restrict__ sq) {
+    const int64_t row = static_cast<int64_t>(blockIdx.x) * 8 + (threadIdx.x >> 5);
+    if (row >= n) return;
+    const int lane = threadIdx.x & 31;
+    const int8_t* g = G + row * ldg;
+    int acc = 0;
+    const int64_t pv = p & ~static_cast<int64_t>(15);
+    for (int64_t k = lane * 16; k < pv; k += 32 * 16) {
+        const int4 v = *reinterpret_cast<const int4*>(g + k);
+        acc = __dp4a(v.x, v.x, acc);
+        acc = __dp4a(v.y, v.y, acc);
+        acc = __dp4a(v.z, v.z, acc);
+        acc = __dp4a(v.w, v.w, acc);
+    }
+    for (int64_t k = pv + lane; k < p; k += 32) acc += static_cast<int>(g[k]) * static_cast<int>(g[k]);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    if (lane == 0) sq[row] = acc;
+}
+
+// 256 x 256 blocks of the lower tiles, row unit by row unit: unit (ru, cu) is wanted when the tile of its
+// rows is at or below the tile of its columns.
+__device__ __forceinline__ int build_cols_of_row_unit(int ru, int nb) {
+    const int upt = nb / 256;                        // units per tile
+    return (ru / upt + 1) * upt;                     // column units 0 .. this - 1
+}
+__device__ __forceinline__ bool build_next_block(int64_t& t, int64_t stride, int nru, int nb, int64_t total, int& ru, int& cu) {
+    if (t >= total) return false;
+    // decode the linear index t (row units in order, their column units in order)
+    const int upt = nb / 256;
+    // blocks before tile row T: upt * upt * T (T + 1) / 2 ... per tile row T there are upt row units of (T + 1) upt columns
+    int T = 0;
+    int64_t before = 0;
+    for (;;) {
+        const int64_t in_tile_row = static_cast<int64_t>(upt) * upt * (T + 1);
+        if (t < before + in_tile_row) break;
+        before += in_tile_row;
+        ++T;
+    }
+    const int64_t rem = t - before;
+    const int cols = (T + 1) * upt;
+    ru = T * upt + static_cast<int>(rem / cols);
+    cu = static_cast<int>(rem % cols);
+    (void)nru;
+    t += stride;
+    return true;
+}
+
+__global__ void __launch_bounds__(kBuildThreads, 1)
+build_tc_kernel(const __grid_constant__ CUtensorMap tmG, const BuildOp op) {
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
+    const uint32_t bar_base = smem_base + kBuildSlots * kBuildSlotBytes;
+    auto full_bar = [&](int s) { return bar_base + 8u * s; };
+    auto empty_bar = [&](int s) { return bar_base + 8u * (8 + s); };
+    auto tfull_bar = [&](int b) { return bar_base + 8u * (16 + b); };
+    auto tempty_bar = [&](int b) { return bar_base + 8u * (18 + b); };
+    const uint32_t tmem_slot = bar_base + 8u * 20;
+    uint32_t* tmem_slot_ptr = reinterpret_cast<uint32_t*>(smem_raw + (tmem_slot - ptx::smem_u32(smem_raw)));
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int rank = static_cast<int>(ptx::cluster_ctarank());
+    const int64_t pair0 = blockIdx.x >> 1, npairs = gridDim.x >> 1;
+    const int nru = static_cast<int>(op.n / 256);
+    const int NT = static_cast<int>(op.n / op.nb), upt = op.nb / 256;
+    const int64_t total = static_cast<int64_t>(upt) * upt * NT * (NT + 1) / 2;
+    const int nch = static_cast<int>((op.p + 127) / 128);           // 128-SNP chunks (the last one zero-filled by TMA)
+    constexpr uint32_t kHalf = kBlk * 128;                           // 16 KB operand block
+
+    if (warp == 0 && lane == 0) {
+        ptx::prefetch_tmap(&tmG);
+        for (int s = 0; s < kBuildSlots; ++s) { ptx::mbar_init(full_bar(s), 1); ptx::mbar_init(empty_bar(s), 1); }
+        for (int b = 0; b < 2; ++b) { ptx::mbar_init(tfull_bar(b), 1); ptx::mbar_init(tempty_bar(b), 16); }
+        ptx::fence_mbar_init();
+    }
+    if (warp == 1) {
+        ptx::tmem_alloc<512, 2>(tmem_slot);
+        ptx::tmem_relinquish<2>();
+    }
+    ptx::tc_fence_before();
+    ptx::cluster_sync_all();
+    ptx::tc_fence_after();
+    const uint32_t tmem_base = *tmem_slot_ptr;
+
+    if (warp == 0) {
+        // ===================== TMA producer (uniform control flow, one elected lane issues) =====================
+        int slot = 0;
+        uint32_t phase = 0;
+        int64_t t = pair0;
+        int ru, cu;
+        while (build_next_block(t, npairs, nru, op.nb, total, ru, cu)) {
+            const int a_row = ru * 256 + rank * kBlk, b_row = cu * 256 + rank * kBlk;
+            for (int ch = 0; ch < nch; ++ch) {
+                ptx::mbar_wait(empty_bar(slot), phase ^ 1u);
+                if (ptx::elect_one()) {
+                    const uint32_t sa = smem_base + slot * kBuildSlotBytes;
+                    if (rank == 0) ptx::mbar_arrive_expect_tx(full_bar(slot), 4u * kHalf);
+                    ptx::tma_load_2d_pair(sa, &tmG, full_bar(slot), ch * 128, a_row);
+                    ptx::tma_load_2d_pair(sa + kHalf, &tmG, full_bar(slot), ch * 128, b_row);
+                }
+                if (++slot == kBuildSlots) { slot = 0; phase ^= 1u; }
+            }
+        }
+    } else if (warp == 1) {
+        // ===================== MMA issuer =====================
+        if (rank == 0) {
+            constexpr uint32_t idesc = ptx::make_idesc_i8(256, 256);
+            const uint32_t dlo0 = ptx::smem_desc_lo(smem_base);
+            int slot = 0, buf = 0;
+            uint32_t phase = 0, acc_phase = 0;
+            int64_t t = pair0;
+            int ru, cu;
+            while (build_next_block(t, npairs, nru, op.nb, total, ru, cu)) {
+                ptx::mbar_wait(tempty_bar(buf), acc_phase ^ 1u);
+                ptx::tc_fence_after();
+                const uint32_t d_tmem = tmem_base + buf * 256;
+                for (int ch = 0; ch < nch; ++ch) {
+                    ptx::mbar_wait(full_bar(slot), phase);
+                    ptx::tc_fence_after();
+                    if (ptx::elect_one()) {
+                        const uint32_t a = dlo0 + slot * (kBuildSlotBytes >> 4), b = a + (kHalf >> 4);
+#pragma unroll
+                        for (int kk = 0; kk < 4; ++kk)             // 4 x K = 32 per 128-byte row
+                            ptx::mma_i8_ss_pair(d_tmem, ptx::smem_desc_from_lo(a + 2 * kk), ptx::smem_desc_from_lo(b + 2 * kk), idesc,
+                                                (ch > 0 || kk > 0) ? 1u : 0u);
+                        ptx::tc_commit_pair(empty_bar(slot));
+                    }
+                    if (++slot == kBuildSlots) { slot = 0; phase ^= 1u; }
+                }
+                if (ptx::elect_one()) ptx::tc_commit_pair(tfull_bar(buf));
+                if (++buf == 2) { buf = 0; acc_phase ^= 1u; }
+            }
+        }
+    } else {
+        // ===================== epilogue: d2 = s_i + s_j - 2 <g_i, g_j>, exp, store =====================
+        const int ew = warp - 2, q = warp & 3, hf = ew >> 2;          // TMEM lanes 32q.., columns 128 hf ..
+        int buf = 0;
+        uint32_t acc_phase = 0;
+        int64_t t = pair0;
+        int ru, cu;
+        while (build_next_block(t, npairs, nru, op.nb, total, ru, cu)) {
+            const int64_t gi = static_cast<int64_t>(ru) * 256 + rank * kBlk + q * 32 + lane;       // my row of A
+            const int si = op.sq[gi];
+            const int ti = static_cast<int>(gi / op.nb);
+            ptx::mbar_wait(tfull_bar(buf), acc_phase);
+            ptx::tc_fence_after();
+#pragma unroll 1
+            for (int part = 0; part < 4; ++part) {
+                const int64_t gj0 = static_cast<int64_t>(cu) * 256 + hf * 128 + part * 32;          // first column of this part
+                uint32_t acc[32];
+                ptx::tmem_ld_32x32(tmem_base + buf * 256 + (static_cast<uint32_t>(q * 32) << 16) + hf * 128 + part * 32, acc);
+                ptx::tmem_ld_wait();
+                if (part == 3) {
+                    ptx::tc_fence_before();
+                    __syncwarp();
+                    if (lane == 0) ptx::mbar_arrive_leader(tempty_bar(buf));          // accumulator is in registers
+                }
+                const int tj = static_cast<int>(gj0 / op.nb);
+                if (tj > ti) continue;                                               // an upper tile: not produced
+                float* dst = op.tiled
+                    ? op.A + (tile_slot(NT, ti, tj) * op.nb + gi % op.nb) * static_cast<int64_t>(op.nb) + gj0 % op.nb
+                    : op.A + gi * op.lda + gj0;
+#pragma unroll
+                for (int e = 0; e < 32; e += 4) {
+                    float v[4];
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        const int d2 = si + __ldg(op.sq + gj0 + e + u) - 2 * static_cast<int>(acc[e + u]);
+                        v[u] = (gj0 + e + u == gi) ? op.diag : expf(-op.gamma * static_cast<float>(d2));
+                    }
+                    *reinterpret_cast<float4*>(dst + e) = make_float4(v[0], v[1], v[2], v[3]);
+                }
+            }
+            if (++buf == 2) { buf = 0; acc_phase ^= 1u; }
+        }
+    }
+    ptx::tc_fence_before();
+    ptx::cluster_sync_all();
+    if (warp == 1) ptx::tmem_dealloc<512, 2>(tmem_base);
+}
+
+}  // namespace krr

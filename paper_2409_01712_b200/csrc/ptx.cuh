@@ -145,6 +145,16 @@ __device__ __forceinline__ void mma_mxf8_ss_pair(uint32_t d_tmem, uint64_t a_des
         ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate), "r"(sfa), "r"(sfb)
         : "memory");
 }
+// kind::i8: signed / unsigned 8-bit integer operands, INT32 accumulate (Build phase)
+__device__ __forceinline__ void mma_i8_ss_pair(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc,
+                                               uint32_t idesc, uint32_t accumulate) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::2.kind::i8 [%0], %1, %2, %3, p;\n\t}\n"
+        ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
 __device__ __forceinline__ void tc_fence_before() {
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
 }
@@ -247,6 +257,16 @@ __host__ __device__ constexpr uint32_t make_idesc(int M, int N, int a_fmt, int b
            | (static_cast<uint32_t>(b_fmt) << 10)    // b_format            [10,13)
            | (static_cast<uint32_t>(N >> 3) << 17)   // n_dim = N/8         [17,23)
            | (static_cast<uint32_t>(M >> 4) << 24);  // m_dim = M/16        [24,29)
+}
+
+// Instruction descriptor of kind::i8: INT8 x INT8 (signed), INT32 accumulator, both operands K-major, dense,
+// K = 32 per instruction.
+__host__ __device__ constexpr uint32_t make_idesc_i8(int M, int N) {
+    return (2u << 4)                                  // c_format = S32      [4,6)
+           | (1u << 7)                                // a_format = INT8     [7,10)
+           | (1u << 10)                               // b_format = INT8     [10,13)
+           | (static_cast<uint32_t>(N >> 3) << 17)    // n_dim = N/8         [17,23)
+           | (static_cast<uint32_t>(M >> 4) << 24);   // m_dim = M/16        [24,29)
 }
 
 // Instruction descriptor of kind::mxf8f6f4.block_scale: E4M3 x E4M3, UE8M0 scales (scale ids 0),

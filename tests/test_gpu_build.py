@@ -1,0 +1,119 @@
+"""GPU parity of krr_build (Build phase on the INT8 tensor cores) against the oracle's definition.
+
+Tolerance: the squared distances are exact on both sides (integers); the kernel entry is exp(-gamma d)
+evaluated by the oracle in FP64 and by the CUDA path in FP32 (expf of the FP32 product gamma*d): the
+product carries <= 2 roundings of relative size 2^-24 on an exponent of magnitude gamma*d <= ~4, expf
+<= 2 ulp, so |K_gpu - K| <= (2 * 2^-24 * gamma*d + 3 * 2^-24) K  <  8e-7 K for the workloads' gamma*d < 4.
+The diagonal (1 + lambda) and the structure (upper tiles untouched) are exact."""
+import numpy as np
+import pytest
+import torch
+
+from krr_inputs import CONFIGS, genotypes, kernel_matrix, scaled_config
+from oracle.build_phase import kernel_matrix_definition
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def krr():
+    from paper_2409_01712_b200 import build
+    build.build()
+    import paper_2409_01712_b200 as k
+    k.lib()
+    return k
+
+
+def padded(G, mult=16):
+    """Row pitch a multiple of 16 bytes (TMA): a view into a wider buffer."""
+    n, p = G.shape
+    ld = (p + mult - 1) // mult * mult
+    buf = torch.full((n, ld), 7, dtype=torch.int8, device=G.device)      # garbage past p must not be read as data
+    buf[:, :p] = G
+    return buf[:, :p]
+
+
+@pytest.mark.parametrize("n,p,nb,kind", [(512, 1000, 256, "maf"),        # p not a multiple of 128: TMA zero fill
+                                          (1024, 777, 512, "uniform"),
+                                          (768, 128, 256, "maf"),         # a single K chunk
+                                          (2048, 1000, 256, "maf")])      # config 1 at full size
+def test_build_matches_definition(krr, n, p, nb, kind):
+    G = genotypes(11, n, p, kind, device="cuda")
+    gamma, lam = 1.0 / p, 1e-2
+    A = krr.krr_build(padded(G), gamma, lam, nb)
+    torch.cuda.synchronize()
+    want = kernel_matrix_definition(G.cpu().numpy(), gamma, lam)
+    got = A.cpu().numpy().astype(np.float64)
+    NT = n // nb
+    for i in range(NT):
+        for j in range(NT):
+            g = got[i * nb:(i + 1) * nb, j * nb:(j + 1) * nb]
+            if j > i:
+                assert not g.any()                                        # tiles above the diagonal are not written
+                continue
+            w = want[i * nb:(i + 1) * nb, j * nb:(j + 1) * nb]
+            assert np.all(np.abs(g - w) <= 8e-7 * w), (i, j, float(np.max(np.abs(g - w) / w)))
+    assert np.all(np.diag(got) == np.float64(np.float32(1.0 + lam)))
+    # within a few ulp of the generator's FP64-evaluated, FP32-rounded matrix, most entries identical
+    gen = kernel_matrix(G, gamma, lam).cpu().numpy()
+    low = np.tril_indices(n)
+    a32 = A.cpu().numpy()
+    assert np.mean(a32[low] == gen[low]) > 0.5
+    assert np.max(np.abs(a32[low].astype(np.float64) - gen[low]) / gen[low]) < 8e-7
+
+
+def test_build_general_int8_values_and_tiled_output(krr):
+    """Any int8 genotype encoding (negative values included), and the packed lower-tile layout of config C4."""
+    n, p, nb = 512, 300, 256
+    g = torch.Generator(device="cpu").manual_seed(3)
+    G = torch.randint(-128, 128, (n, p), generator=g, dtype=torch.int8).cuda()
+    gamma, lam = 2e-7, 0.5
+    want = kernel_matrix_definition(G.cpu().numpy(), gamma, lam)
+    At = krr.krr_build(padded(G), gamma, lam, nb, tiled_lower=True)
+    Ad = krr.krr_build(padded(G), gamma, lam, nb)
+    torch.cuda.synchronize()
+    T = At.reshape(-1, nb, nb).cpu().numpy()
+    NT, slot = n // nb, 0
+    for j in range(NT):
+        for i in range(j, NT):
+            w = want[i * nb:(i + 1) * nb, j * nb:(j + 1) * nb]
+            assert np.all(np.abs(T[slot] - w) <= 8e-7 * w)
+            assert np.array_equal(T[slot], Ad[i * nb:(i + 1) * nb, j * nb:(j + 1) * nb].cpu().numpy())
+            slot += 1
+
+
+def test_build_feeds_the_associate_phase(krr):
+    """Build -> precision map -> factorisation -> solve on the built matrix: same map, backward error and alpha
+    tolerances as with the generator's matrix."""
+    from oracle.cholesky import backward_error
+    from oracle.solve import solve_fp64
+    cfg = scaled_config(CONFIGS["C1"], nb=256, n=1024, p=500)
+    G = genotypes(cfg.seed, cfg.n, cfg.p, cfg.genotype, device="cuda")
+    A = krr.krr_build(padded(G), cfg.gamma, cfg.lam, cfg.nb)
+    Y = torch.randn((cfg.n, 4), device="cuda", generator=torch.Generator(device="cuda").manual_seed(0))
+    d_map, *_ = krr.precision_map(A, cfg.nb, 1e-4)
+    F = krr.potrf_mp(A, cfg.nb, d_map, d_map.cpu())
+    alpha = krr.potrs(F, Y.clone())
+    torch.cuda.synchronize()
+    assert int(F.info.item()) == 0
+    Aw = kernel_matrix_definition(G.cpu().numpy(), cfg.gamma, cfg.lam)
+    Lg = F.dense().cpu().numpy()
+    assert backward_error(Aw.astype(np.float32), Lg) <= 2e-6
+    a64 = solve_fp64(Aw.astype(np.float32), Y.cpu().numpy(), cfg.nb)
+    assert np.linalg.norm(alpha.cpu().numpy() - a64) / np.linalg.norm(a64) <= 1e-3
+
+
+def test_build_argument_errors(krr):
+    L = krr.lib()
+    import ctypes
+    G = torch.zeros((512, 160), dtype=torch.int8, device="cuda")
+    A = torch.zeros((512, 512), dtype=torch.float32, device="cuda")
+    ws = torch.zeros(4096, dtype=torch.uint8, device="cuda")
+    vp = lambda t: ctypes.c_void_p(t.data_ptr())
+    call = lambda n, p, ldg, nb, flags=0: L.krr_build(vp(G), n, p, ldg, 0.01, 0.01, vp(A), 512, nb, flags, vp(ws), 4096, None)
+    assert call(512, 160, 160, 256) == 0
+    assert call(500, 160, 160, 250) == -2            # n, nb not multiples of 256
+    assert call(512, 160, 150, 256) == -1            # ldg < p
+    assert call(512, 150, 152, 256) == -1            # row pitch not a multiple of 16 bytes
+    assert call(512, 160, 160, 256, 8) == -7         # unsupported flag
+    torch.cuda.synchronize()

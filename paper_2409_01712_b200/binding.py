@@ -280,7 +280,7 @@ def associate_host(h_A, nb, h_Y, eps_target=0.0, allowed=(FP32,), force_prec=-1,
     return alpha, h_map, int(h_info[0]), arena
 
 
-def krr_build(G, gamma, lam, nb, tiled_lower=False, out=None):
+def krr_build(G, gamma, lam, nb, tiled_lower=False, out=None, flags=0):
     """krr_build (named in full: `build` is this package's compile step): A = K + lam*I (Gaussian kernel) from CUDA int8 genotypes G (n x p, row-major, row pitch a
     multiple of 16 bytes).  Returns A: n x n FP32 with the lower tiles written (the rest zero), or the packed
     lower tiles with tiled_lower."""
@@ -296,7 +296,7 @@ def krr_build(G, gamma, lam, nb, tiled_lower=False, out=None):
     if wsb == 0:
         raise KrrError("krr_build_workspace: n must be a multiple of 256")
     ws = _ws(wsb, dev)
-    flags = FLAG_A_TILED_LOWER if tiled_lower else 0
+    flags |= FLAG_A_TILED_LOWER if tiled_lower else 0
     lda = nb if tiled_lower else out.stride(0)
     _check(L.krr_build(_ptr(G), n, p, G.stride(0), float(gamma), float(lam), _ptr(out), lda, nb, flags, _ptr(ws), wsb,
                        _stream()), "krr_build")

@@ -771,7 +771,7 @@ extern "C" {
 
 size_t krr_build_workspace(int64_t n) {
     if (n <= 0 || n % 256 != 0) return 0;
-    return align_up(static_cast<size_t>(n) * sizeof(int), 1024);
+    return align_up(static_cast<size_t>(n) * sizeof(int), 1024);           // the folded squared norms
 }
 
 int krr_build(const int8_t* d_G, int64_t n, int64_t p, int64_t ldg, float gamma, float lambda, float* d_A, int64_t lda,
@@ -794,7 +794,8 @@ int krr_build(const int8_t* d_G, int64_t n, int64_t p, int64_t ldg, float gamma,
     if (rc) return rc;
     static bool attr_done = false;
     if (!attr_done) {
-        KRR_CUDA_CHECK(cudaFuncSetAttribute(build_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kBuildSmem));
+        KRR_CUDA_CHECK(cudaFuncSetAttribute(build_tc_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, build_smem(1)));
+        KRR_CUDA_CHECK(cudaFuncSetAttribute(build_tc_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, build_smem(2)));
         attr_done = true;
     }
     cudaStream_t st = static_cast<cudaStream_t>(stream);
@@ -819,18 +820,22 @@ int krr_build(const int8_t* d_G, int64_t n, int64_t p, int64_t ldg, float gamma,
     op.sq = sq; op.A = d_A; op.lda = lda;
     const int64_t NT = n / nb, upt = nb / 256;
     const int64_t total = upt * upt * NT * (NT + 1) / 2;
+    const int nacc = (nb % 512 == 0) ? 2 : 1;                      // 256 x 512 blocks when a tile holds them
     const int64_t max_pairs = num_sms / 2;
-    const int grid = static_cast<int>(2 * (total < max_pairs ? total : max_pairs));
+    const int64_t blocks = total / nacc;
+    const int grid = static_cast<int>(2 * (blocks < max_pairs ? blocks : max_pairs));
     cudaLaunchConfig_t cfg;
     memset(&cfg, 0, sizeof(cfg));
-    cfg.gridDim = dim3(grid); cfg.blockDim = dim3(kBuildThreads); cfg.dynamicSmemBytes = kBuildSmem; cfg.stream = st;
+    cfg.gridDim = dim3(grid); cfg.blockDim = dim3(kBuildThreads); cfg.dynamicSmemBytes = build_smem(nacc); cfg.stream = st;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeClusterDimension;
     attr[0].val.clusterDim.x = 2; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr; cfg.numAttrs = 1;
     ProfScope ps(CAT_MISC, st);
     ++g_launches;
-    return cudaLaunchKernelEx(&cfg, build_tc_kernel, tmG, op) == cudaSuccess ? KRR_OK : KRR_ERR_CUDA;
+    const cudaError_t e = (nacc == 2) ? cudaLaunchKernelEx(&cfg, build_tc_kernel<2>, tmG, op)
+                                      : cudaLaunchKernelEx(&cfg, build_tc_kernel<1>, tmG, op);
+    return e == cudaSuccess ? KRR_OK : KRR_ERR_CUDA;
 }
 
 }  // extern "C"

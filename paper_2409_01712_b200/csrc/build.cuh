@@ -28,10 +28,14 @@ struct BuildOp {
     int64_t lda;
 };
 
-constexpr int kBuildSlots = 6;
-constexpr int kBuildSlotBytes = 2 * kBlk * 128;     // [128 rows x 128 SNPs of the row operand | same of the column operand]
+// NACC = 256-column accumulators per pair: 2 -> a pair computes 256 x 512 (all 512 TMEM columns, the exp epilogue
+// is then not overlapped with the next block's MMAs -- a few % at thousands of SNPs -- but every byte of the row
+// operand feeds twice the MMAs: the kernel is bound by L2 -> shared-memory and HBM traffic, not by the tensor
+// pipe); 1 -> 256 x 256 with double-buffered accumulators (tiles of 256).
 constexpr int kBuildThreads = 320;                  // warp 0 TMA, warp 1 MMA (+ TMEM alloc), 2-9 epilogue
-constexpr int kBuildSmem = kBuildSlots * kBuildSlotBytes + 1024 + 256;
+__host__ __device__ constexpr int build_slot_bytes(int nacc) { return (1 + nacc) * kBlk * 128; }   // [row block | nacc column blocks] x 128 SNPs
+__host__ __device__ constexpr int build_slots(int nacc) { return nacc == 1 ? 6 : 4; }
+__host__ __device__ constexpr int build_smem(int nacc) { return build_slots(nacc) * build_slot_bytes(nacc) + 1024 + 256; }
 
 // s_i = sum_k g_ik^2 (INT32; exact while p * 127^2 < 2^31).  One warp per row, 16-byte loads.
 __global__ void __launch_bounds__(256)
@@ -55,36 +59,59 @@ row_sqnorm_kernel(const int8_t* __restrict__ G, int64_t n, int64_t p, int64_t ld
     if (lane == 0) sq[row] = acc;
 }
 
-// 256 x 256 blocks of the lower tiles, row unit by row unit: unit (ru, cu) is wanted when the tile of its
-// rows is at or below the tile of its columns.
-__device__ __forceinline__ int build_cols_of_row_unit(int ru, int nb) {
-    const int upt = nb / 256;                        // units per tile
-    return (ru / upt + 1) * upt;                     // column units 0 .. this - 1
+// 256 x 256 blocks (units) of the lower tiles: unit (ru, cu) is wanted when the tile of its rows is at or below
+// the tile of its columns.  Order: panels of kBuildPanel column units; inside a panel row unit by row unit.
+// The ~74 blocks in flight at any time then cover ~9 row units x 8 column units and read 17 operand strips
+// instead of 75 (a strip = 256 patients x p SNPs; G is far larger than L2, so the order decides the DRAM
+// traffic: 552 GB -> see profiles/ for the row-major order on C3).  Every warp role walks the same sequence
+// with its own cursor; stepping is a few integer operations per block against ~100k clocks of MMAs.
+constexpr int kBuildPanel = 8;                      // panel width in 256-column units
+struct BuildCursor {
+    int cp, ru, ci;          // column panel, row unit, column inside the panel
+    bool done;
+};
+// cw = width of a column unit in 256-column units (NACC); cu counts column units of that width
+__device__ __forceinline__ bool build_valid(int ru, int cu, int upt, int cw) { return ru / upt >= cu * cw / upt; }
+__device__ __forceinline__ void build_cursor_init(BuildCursor& c, int upt) {
+    c.cp = 0; c.ru = 0; c.ci = 0; c.done = false;
+    (void)upt;
 }
-__device__ __forceinline__ bool build_next_block(int64_t& t, int64_t stride, int nru, int nb, int64_t total, int& ru, int& cu) {
-    if (t >= total) return false;
-    // decode the linear index t (row units in order, their column units in order)
-    const int upt = nb / 256;
-    // blocks before tile row T: upt * upt * T (T + 1) / 2 ... per tile row T there are upt row units of (T + 1) upt columns
-    int T = 0;
-    int64_t before = 0;
-    for (;;) {
-        const int64_t in_tile_row = static_cast<int64_t>(upt) * upt * (T + 1);
-        if (t < before + in_tile_row) break;
-        before += in_tile_row;
-        ++T;
+// move to the next wanted unit strictly after the current position (or stay if `first` and it is wanted)
+__device__ __forceinline__ void build_cursor_seek(BuildCursor& c, int nru, int upt, int cw, bool first) {
+    const int pw = kBuildPanel / cw, ncu = nru / cw;          // panel width and matrix width in column units
+    bool skip = !first;
+    while (!c.done) {
+        if (!skip) {
+            const int cu = c.cp * pw + c.ci;
+            if (cu < ncu && build_valid(c.ru, cu, upt, cw)) return;
+        }
+        skip = false;
+        if (++c.ci == pw) {
+            c.ci = 0;
+            if (++c.ru == nru) {
+                ++c.cp;
+                if (c.cp * pw >= ncu) { c.done = true; return; }
+                c.ru = (c.cp * kBuildPanel / upt) * upt;      // first row unit of the panel's first tile
+            }
+        }
     }
-    const int64_t rem = t - before;
-    const int cols = (T + 1) * upt;
-    ru = T * upt + static_cast<int>(rem / cols);
-    cu = static_cast<int>(rem % cols);
-    (void)nru;
-    t += stride;
+}
+// the block this pair handles next: `steps` wanted units further (steps = pair index at first, then #pairs)
+__device__ __forceinline__ bool build_next_block(BuildCursor& c, bool& started, int pair0, int npairs, int nru, int upt,
+                                                 int cw, int& ru, int& cu) {
+    int steps = started ? npairs : pair0;
+    if (!started) { build_cursor_seek(c, nru, upt, cw, true); started = true; }
+    for (; steps > 0 && !c.done; --steps) build_cursor_seek(c, nru, upt, cw, false);
+    if (c.done) return false;
+    ru = c.ru;
+    cu = c.cp * (kBuildPanel / cw) + c.ci;
     return true;
 }
 
+template <int NACC>
 __global__ void __launch_bounds__(kBuildThreads, 1)
 build_tc_kernel(const __grid_constant__ CUtensorMap tmG, const BuildOp op) {
+    constexpr int kBuildSlots = build_slots(NACC), kBuildSlotBytes = build_slot_bytes(NACC), NBUF = 2 / NACC;
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
     const uint32_t bar_base = smem_base + kBuildSlots * kBuildSlotBytes;
@@ -97,10 +124,9 @@ build_tc_kernel(const __grid_constant__ CUtensorMap tmG, const BuildOp op) {
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int rank = static_cast<int>(ptx::cluster_ctarank());
-    const int64_t pair0 = blockIdx.x >> 1, npairs = gridDim.x >> 1;
+    const int pair0 = static_cast<int>(blockIdx.x >> 1), npairs = static_cast<int>(gridDim.x >> 1);
     const int nru = static_cast<int>(op.n / 256);
     const int NT = static_cast<int>(op.n / op.nb), upt = op.nb / 256;
-    const int64_t total = static_cast<int64_t>(upt) * upt * NT * (NT + 1) / 2;
     const int nch = static_cast<int>((op.p + 127) / 128);           // 128-SNP chunks (the last one zero-filled by TMA)
     constexpr uint32_t kHalf = kBlk * 128;                           // 16 KB operand block
 
@@ -123,17 +149,21 @@ build_tc_kernel(const __grid_constant__ CUtensorMap tmG, const BuildOp op) {
         // ===================== TMA producer (uniform control flow, one elected lane issues) =====================
         int slot = 0;
         uint32_t phase = 0;
-        int64_t t = pair0;
+        BuildCursor cur;
+        build_cursor_init(cur, upt);
+        bool started = false;
         int ru, cu;
-        while (build_next_block(t, npairs, nru, op.nb, total, ru, cu)) {
-            const int a_row = ru * 256 + rank * kBlk, b_row = cu * 256 + rank * kBlk;
+        while (build_next_block(cur, started, pair0, npairs, nru, upt, NACC, ru, cu)) {
+            const int a_row = ru * 256 + rank * kBlk, b_row = cu * 256 * NACC + rank * kBlk;
             for (int ch = 0; ch < nch; ++ch) {
                 ptx::mbar_wait(empty_bar(slot), phase ^ 1u);
                 if (ptx::elect_one()) {
                     const uint32_t sa = smem_base + slot * kBuildSlotBytes;
-                    if (rank == 0) ptx::mbar_arrive_expect_tx(full_bar(slot), 4u * kHalf);
+                    if (rank == 0) ptx::mbar_arrive_expect_tx(full_bar(slot), 2u * (1 + NACC) * kHalf);
                     ptx::tma_load_2d_pair(sa, &tmG, full_bar(slot), ch * 128, a_row);
-                    ptx::tma_load_2d_pair(sa + kHalf, &tmG, full_bar(slot), ch * 128, b_row);
+#pragma unroll
+                    for (int a = 0; a < NACC; ++a)           // this CTA's 128 rows of each 256-column accumulator
+                        ptx::tma_load_2d_pair(sa + (1 + a) * kHalf, &tmG, full_bar(slot), ch * 128, b_row + a * 256);
                 }
                 if (++slot == kBuildSlots) { slot = 0; phase ^= 1u; }
             }
@@ -145,27 +175,33 @@ build_tc_kernel(const __grid_constant__ CUtensorMap tmG, const BuildOp op) {
             const uint32_t dlo0 = ptx::smem_desc_lo(smem_base);
             int slot = 0, buf = 0;
             uint32_t phase = 0, acc_phase = 0;
-            int64_t t = pair0;
+            BuildCursor cur;
+            build_cursor_init(cur, upt);
+            bool started = false;
             int ru, cu;
-            while (build_next_block(t, npairs, nru, op.nb, total, ru, cu)) {
+            while (build_next_block(cur, started, pair0, npairs, nru, upt, NACC, ru, cu)) {
                 ptx::mbar_wait(tempty_bar(buf), acc_phase ^ 1u);
                 ptx::tc_fence_after();
-                const uint32_t d_tmem = tmem_base + buf * 256;
+                const uint32_t d_tmem = tmem_base + buf * 256 * NACC;
                 for (int ch = 0; ch < nch; ++ch) {
                     ptx::mbar_wait(full_bar(slot), phase);
                     ptx::tc_fence_after();
                     if (ptx::elect_one()) {
-                        const uint32_t a = dlo0 + slot * (kBuildSlotBytes >> 4), b = a + (kHalf >> 4);
+                        const uint32_t a = dlo0 + slot * (kBuildSlotBytes >> 4);
 #pragma unroll
-                        for (int kk = 0; kk < 4; ++kk)             // 4 x K = 32 per 128-byte row
-                            ptx::mma_i8_ss_pair(d_tmem, ptx::smem_desc_from_lo(a + 2 * kk), ptx::smem_desc_from_lo(b + 2 * kk), idesc,
-                                                (ch > 0 || kk > 0) ? 1u : 0u);
+                        for (int c = 0; c < NACC; ++c) {
+                            const uint32_t b = a + (1 + c) * (kHalf >> 4);
+#pragma unroll
+                            for (int kk = 0; kk < 4; ++kk)         // 4 x K = 32 per 128-byte row
+                                ptx::mma_i8_ss_pair(d_tmem + c * 256, ptx::smem_desc_from_lo(a + 2 * kk), ptx::smem_desc_from_lo(b + 2 * kk),
+                                                    idesc, (ch > 0 || kk > 0) ? 1u : 0u);
+                        }
                         ptx::tc_commit_pair(empty_bar(slot));
                     }
                     if (++slot == kBuildSlots) { slot = 0; phase ^= 1u; }
                 }
                 if (ptx::elect_one()) ptx::tc_commit_pair(tfull_bar(buf));
-                if (++buf == 2) { buf = 0; acc_phase ^= 1u; }
+                if (++buf == NBUF) { buf = 0; acc_phase ^= 1u; }
             }
         }
     } else {
@@ -173,21 +209,24 @@ build_tc_kernel(const __grid_constant__ CUtensorMap tmG, const BuildOp op) {
         const int ew = warp - 2, q = warp & 3, hf = ew >> 2;          // TMEM lanes 32q.., columns 128 hf ..
         int buf = 0;
         uint32_t acc_phase = 0;
-        int64_t t = pair0;
+        BuildCursor cur;
+        build_cursor_init(cur, upt);
+        bool started = false;
         int ru, cu;
-        while (build_next_block(t, npairs, nru, op.nb, total, ru, cu)) {
+        while (build_next_block(cur, started, pair0, npairs, nru, upt, NACC, ru, cu)) {
             const int64_t gi = static_cast<int64_t>(ru) * 256 + rank * kBlk + q * 32 + lane;       // my row of A
             const int si = op.sq[gi];
             const int ti = static_cast<int>(gi / op.nb);
             ptx::mbar_wait(tfull_bar(buf), acc_phase);
             ptx::tc_fence_after();
 #pragma unroll 1
-            for (int part = 0; part < 4; ++part) {
-                const int64_t gj0 = static_cast<int64_t>(cu) * 256 + hf * 128 + part * 32;          // first column of this part
+            for (int part = 0; part < 4 * NACC; ++part) {
+                const int col = (part >> 2) * 256 + hf * 128 + (part & 3) * 32;                     // column inside the block
+                const int64_t gj0 = static_cast<int64_t>(cu) * 256 * NACC + col;                    // first column of this part
                 uint32_t acc[32];
-                ptx::tmem_ld_32x32(tmem_base + buf * 256 + (static_cast<uint32_t>(q * 32) << 16) + hf * 128 + part * 32, acc);
+                ptx::tmem_ld_32x32(tmem_base + buf * 256 * NACC + (static_cast<uint32_t>(q * 32) << 16) + col, acc);
                 ptx::tmem_ld_wait();
-                if (part == 3) {
+                if (part == 4 * NACC - 1) {
                     ptx::tc_fence_before();
                     __syncwarp();
                     if (lane == 0) ptx::mbar_arrive_leader(tempty_bar(buf));          // accumulator is in registers
@@ -208,7 +247,7 @@ build_tc_kernel(const __grid_constant__ CUtensorMap tmG, const BuildOp op) {
                     *reinterpret_cast<float4*>(dst + e) = make_float4(v[0], v[1], v[2], v[3]);
                 }
             }
-            if (++buf == 2) { buf = 0; acc_phase ^= 1u; }
+            if (++buf == NBUF) { buf = 0; acc_phase ^= 1u; }
         }
     }
     ptx::tc_fence_before();

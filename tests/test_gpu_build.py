@@ -36,7 +36,8 @@ def padded(G, mult=16):
 @pytest.mark.parametrize("n,p,nb,kind", [(512, 1000, 256, "maf"),        # p not a multiple of 128: TMA zero fill
                                           (1024, 777, 512, "uniform"),
                                           (768, 128, 256, "maf"),         # a single K chunk
-                                          (2048, 1000, 256, "maf")])      # config 1 at full size
+                                          (2048, 1000, 256, "maf"),       # config 1 at full size
+                                          (3072, 640, 1024, "maf")])      # 256 x 512 blocks, two per tile row unit
 def test_build_matches_definition(krr, n, p, nb, kind):
     G = genotypes(11, n, p, kind, device="cuda")
     gamma, lam = 1.0 / p, 1e-2

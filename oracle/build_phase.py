@@ -43,3 +43,31 @@ def squared_distance_by_expansion(G):
     s = np.einsum("ik,ik->i", G, G)
     D = np.tile(s[None, :], (G.shape[0], 1))          # every row holds (||g_1||^2, ..., ||g_n||^2)
     return D + D.T - 2 * (G @ G.T)
+
+
+# ---- Predict phase (Alg. 4) and the paper's accuracy measures ----
+def cross_kernel_matrix_definition(T, G, gamma):
+    """Alg. 4 l.4-5: K (N_P2 x N_P1), K_ij = exp(-gamma ||t_i - g_j||^2) -- BUILD(gamma, T, G, K), no regulariser."""
+    return np.exp(-float(gamma) * squared_distances(T, G).astype(np.float64))
+
+
+def predict_definition(T, G, gamma, W):
+    """Alg. 4 l.6: P_r = K x W in FP64."""
+    return cross_kernel_matrix_definition(T, G, gamma) @ np.asarray(W, dtype=np.float64)
+
+
+def mspe(Y, Yhat):
+    """MSPE = (1 / N_P2) sum_i (Y_i - Yhat_i)^2 (per phenotype column)."""
+    Y = np.asarray(Y, dtype=np.float64)
+    Yhat = np.asarray(Yhat, dtype=np.float64)
+    return np.sum((Y - Yhat) ** 2, axis=0) / Y.shape[0]
+
+
+def pearson(Y, Yhat):
+    """the normalised covariance cov(Y, Yhat) / (sigma_Y sigma_Yhat), per phenotype column."""
+    Y = np.asarray(Y, dtype=np.float64)
+    Yhat = np.asarray(Yhat, dtype=np.float64)
+    yc = Y - Y.mean(axis=0)
+    hc = Yhat - Yhat.mean(axis=0)
+    return np.sum(yc * hc, axis=0) / np.sqrt(np.sum(yc * yc, axis=0) * np.sum(hc * hc, axis=0))
+

@@ -7,7 +7,8 @@ import torch
 from scipy.spatial.distance import cdist
 
 from krr_inputs import genotypes, kernel_matrix
-from oracle.build_phase import kernel_matrix_definition, squared_distance_by_expansion, squared_distances
+from oracle.build_phase import (cross_kernel_matrix_definition, kernel_matrix_definition, mspe, pearson, predict_definition,
+                                squared_distance_by_expansion, squared_distances)
 
 GOLD = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "build_three_patients.txt")
 
@@ -69,3 +70,47 @@ def test_agrees_with_the_input_generator():
     A_gen = kernel_matrix(G, gamma, lam).numpy()
     A_def = kernel_matrix_definition(G.numpy(), gamma, lam)
     assert np.array_equal(A_gen, A_def.astype(np.float32))
+
+
+def test_cross_kernel_reduces_to_the_symmetric_one_and_to_explicit_loops():
+    rng = np.random.default_rng(2)
+    G = rng.integers(0, 3, size=(12, 30)).astype(np.int8)
+    T = rng.integers(0, 3, size=(5, 30)).astype(np.int8)
+    gamma = 0.02
+    assert np.array_equal(cross_kernel_matrix_definition(G, G, gamma), kernel_matrix_definition(G, gamma, 0.0))
+    K = cross_kernel_matrix_definition(T, G, gamma)
+    W = rng.standard_normal((12, 3))
+    P = predict_definition(T, G, gamma, W)
+    for i in range(5):
+        for r in range(3):
+            acc = 0.0
+            for j in range(12):
+                d = sum((int(T[i, k]) - int(G[j, k])) ** 2 for k in range(30))
+                acc += np.exp(-gamma * d) * W[j, r]
+            assert abs(P[i, r] - acc) < 1e-13
+    assert K.shape == (5, 12)
+
+
+def test_predicting_the_training_cohort_with_its_own_weights_interpolates():
+    """With lambda -> 0 and W = K^-1 Y, Predict on the training genotypes returns Y (KRR interpolates)."""
+    rng = np.random.default_rng(3)
+    G = rng.integers(0, 3, size=(20, 64)).astype(np.int8)
+    gamma = 0.05
+    K = kernel_matrix_definition(G, gamma, 0.0)
+    Y = rng.standard_normal((20, 2))
+    W = np.linalg.solve(K, Y)
+    assert np.allclose(predict_definition(G, G, gamma, W), Y, atol=1e-8)
+
+
+def test_mspe_and_pearson_definitions():
+    Y = np.array([[1.0], [2.0], [4.0]])
+    H = np.array([[1.0], [1.0], [6.0]])
+    assert mspe(Y, H)[0] == (0 + 1 + 4) / 3                                # PAPER.md:243 by hand
+    rng = np.random.default_rng(4)
+    A = rng.standard_normal((50, 3))
+    B = 0.3 * A + rng.standard_normal((50, 3))
+    for c in range(3):
+        assert abs(pearson(A, B)[c] - np.corrcoef(A[:, c], B[:, c])[0, 1]) < 1e-14
+    assert abs(pearson(A, 2.5 * A + 1.0)[0] - 1.0) < 1e-14 and abs(pearson(A, -A)[1] + 1.0) < 1e-14
+    assert np.all(mspe(A, A) == 0.0)
+

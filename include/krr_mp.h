@@ -214,6 +214,25 @@ size_t krr_build_workspace(int64_t n);
 int krr_build(const int8_t* d_G, int64_t n, int64_t p, int64_t ldg, float gamma, float lambda,
               float* d_A, int64_t lda, int nb, unsigned flags, void* d_ws, size_t ws_bytes, void* stream);
 
+/* ---------------------------------------------------------------------------------------------
+ * krr_predict -- Predict phase (Alg. 4 :116-122):
+ *   K = BUILD(gamma, T, G): the N_P2 x N_P1 test-training kernel matrix, K_ij = exp(-gamma ||t_i - g_j||^2);
+ *   P_r = K x W.
+ * K is produced by the kernel of krr_build (INT8 tensor cores, every block of the rectangle, no
+ * regulariser) into the workspace as FP32, then multiplied by W in FP32 (one warp per row of K, fixed
+ * summation order).
+ * d_T  in  m x p int8 test genotypes (row pitch ldt), d_G in n x p int8 training genotypes (ldg); both
+ *          pitches multiples of 16 bytes, 16-byte aligned; m % 256 == 0, n % 256 == 0, p <= 133000.
+ * d_W  in  n x nrhs FP32 row-major (ldw): the weights of krr_potrs; nrhs <= 32.
+ * d_P  out m x nrhs FP32 row-major (ldp): the predicted phenotypes.
+ * d_ws     krr_predict_workspace(m, n) bytes, 1024-byte aligned; on return it holds, after the two
+ *          folded norm vectors (each rounded up to 1 KiB), K as m x n FP32 row-major.
+ */
+size_t krr_predict_workspace(int64_t m, int64_t n);
+int krr_predict(const int8_t* d_T, int64_t m, int64_t ldt, const int8_t* d_G, int64_t n, int64_t ldg, int64_t p,
+                float gamma, const float* d_W, int64_t ldw, int nrhs, float* d_P, int64_t ldp,
+                void* d_ws, size_t ws_bytes, void* stream);
+
 /* Number of kernels the last krr_* call on this thread enqueued (for bench.py's gpu_launches). */
 int64_t krr_last_launch_count(void);
 

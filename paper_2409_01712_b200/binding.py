@@ -22,7 +22,8 @@ ERRORS = {-1: "KRR_ERR_ARG", -2: "KRR_ERR_SHAPE", -3: "KRR_ERR_WORKSPACE", -4: "
 EXPORTS = ["krr_version", "krr_built_for_sm", "krr_tile_slot", "krr_precision_map_workspace",
            "krr_precision_map", "krr_factor_bytes", "krr_factor_tile_offset",
            "krr_potrf_mp_workspace", "krr_potrf_mp", "krr_potrs_workspace", "krr_potrs",
-           "krr_associate_host_arena", "krr_associate_host", "krr_build_workspace", "krr_build", "krr_last_launch_count",
+           "krr_associate_host_arena", "krr_associate_host", "krr_build_workspace", "krr_build", "krr_predict_workspace", "krr_predict",
+           "krr_last_launch_count",
            "krr_profile_enable", "krr_profile_read"]
 
 
@@ -75,6 +76,10 @@ def lib():
     L.krr_build_workspace.argtypes = [i64]
     L.krr_build.restype = c.c_int
     L.krr_build.argtypes = [vp, i64, i64, i64, c.c_float, c.c_float, vp, i64, c.c_int, u32, vp, sz, vp]
+    L.krr_predict_workspace.restype = sz
+    L.krr_predict_workspace.argtypes = [i64, i64]
+    L.krr_predict.restype = c.c_int
+    L.krr_predict.argtypes = [vp, i64, i64, vp, i64, i64, i64, c.c_float, vp, i64, c.c_int, vp, i64, vp, sz, vp]
     L.krr_last_launch_count.restype = i64
     L.krr_profile_enable.restype = c.c_int
     L.krr_profile_enable.argtypes = [u32]
@@ -301,4 +306,27 @@ def krr_build(G, gamma, lam, nb, tiled_lower=False, out=None, flags=0):
     _check(L.krr_build(_ptr(G), n, p, G.stride(0), float(gamma), float(lam), _ptr(out), lda, nb, flags, _ptr(ws), wsb,
                        _stream()), "krr_build")
     return out
+
+
+def krr_predict(T, G, gamma, W, return_kernel=False):
+    """krr_predict: P_r = K(T, G) W (Alg. 4).  T (m x p), G (n x p): CUDA int8, row pitch a multiple of 16 bytes;
+    W: CUDA FP32 n x nrhs.  Returns P (m x nrhs) and, on request, the test-training kernel matrix (a view
+    into the call's workspace)."""
+    L = lib()
+    assert T.dtype == torch.int8 and G.dtype == torch.int8 and T.is_cuda and G.is_cuda
+    assert W.dtype == torch.float32 and W.is_cuda and W.stride(1) == 1
+    m, p = T.shape
+    n = G.shape[0]
+    nrhs = W.shape[1]
+    wsb = int(L.krr_predict_workspace(m, n))
+    if wsb == 0:
+        raise KrrError("krr_predict_workspace: m and n must be multiples of 256")
+    ws = _ws(wsb, G.device)
+    P = torch.empty((m, nrhs), dtype=torch.float32, device=G.device)
+    _check(L.krr_predict(_ptr(T), m, T.stride(0), _ptr(G), n, G.stride(0), p, float(gamma), _ptr(W), W.stride(0), nrhs,
+                         _ptr(P), P.stride(0), _ptr(ws), wsb, _stream()), "krr_predict")
+    if not return_kernel:
+        return P
+    off = (m * 4 + 1023) // 1024 * 1024 + (n * 4 + 1023) // 1024 * 1024
+    return P, ws[off:off + m * n * 4].view(torch.float32).reshape(m, n)
 

@@ -767,6 +767,44 @@ int krr_associate_host(const float* h_A, int64_t n, int64_t lda, int nb, float e
 }  // extern "C"
 
 // ------------------------------------------------------------------------- Build phase (NEXT-1)
+namespace {
+// genotypes as a [rows][p] byte matrix, box = 128 SNPs x 128 patients, 128-byte swizzle, zero fill past p
+int make_genotype_tmap(CUtensorMap* tm, const int8_t* G, int64_t rows, int64_t p, int64_t ld) {
+    EncodeTiledFn enc = get_encode_fn();
+    if (!enc) return KRR_ERR_CUDA;
+    cuuint64_t gdim[2] = {static_cast<cuuint64_t>(p), static_cast<cuuint64_t>(rows)};
+    cuuint64_t gstride[1] = {static_cast<cuuint64_t>(ld)};
+    cuuint32_t box[2] = {128u, static_cast<cuuint32_t>(kBlk)};
+    cuuint32_t estr[2] = {1, 1};
+    return enc(tm, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<int8_t*>(G), gdim, gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+               CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS
+               ? KRR_OK : KRR_ERR_CUDA;
+}
+int launch_build(const CUtensorMap& tmR, const CUtensorMap& tmG, const BuildOp& op, int64_t blocks, int nacc, int num_sms,
+                 cudaStream_t st) {
+    static bool attr_done = false;
+    if (!attr_done) {
+        KRR_CUDA_CHECK(cudaFuncSetAttribute(build_tc_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, build_smem(1)));
+        KRR_CUDA_CHECK(cudaFuncSetAttribute(build_tc_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, build_smem(2)));
+        attr_done = true;
+    }
+    const int64_t max_pairs = num_sms / 2;
+    const int grid = static_cast<int>(2 * (blocks < max_pairs ? blocks : max_pairs));
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof(cfg));
+    cfg.gridDim = dim3(grid); cfg.blockDim = dim3(kBuildThreads); cfg.dynamicSmemBytes = build_smem(nacc); cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = 2; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    ProfScope ps(CAT_MISC, st);
+    ++g_launches;
+    const cudaError_t e = (nacc == 2) ? cudaLaunchKernelEx(&cfg, build_tc_kernel<2>, tmR, tmG, op)
+                                      : cudaLaunchKernelEx(&cfg, build_tc_kernel<1>, tmR, tmG, op);
+    return e == cudaSuccess ? KRR_OK : KRR_ERR_CUDA;
+}
+}  // namespace
+
 extern "C" {
 
 size_t krr_build_workspace(int64_t n) {
@@ -792,50 +830,71 @@ int krr_build(const int8_t* d_G, int64_t n, int64_t p, int64_t ldg, float gamma,
     int num_sms = 0;
     rc = check_device(&num_sms);
     if (rc) return rc;
-    static bool attr_done = false;
-    if (!attr_done) {
-        KRR_CUDA_CHECK(cudaFuncSetAttribute(build_tc_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, build_smem(1)));
-        KRR_CUDA_CHECK(cudaFuncSetAttribute(build_tc_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, build_smem(2)));
-        attr_done = true;
-    }
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     int* sq = static_cast<int*>(d_ws);
     rc = launch(CAT_MISC, row_sqnorm_kernel, dim3(static_cast<unsigned>((n + 7) / 8)), dim3(256), 0, st, d_G, n, p, ldg, sq);
     if (rc) return rc;
-    // genotypes as a [n][p] byte matrix, box = 128 SNPs x 128 patients, 128-byte swizzle, zero fill past p
-    EncodeTiledFn enc = get_encode_fn();
-    if (!enc) return KRR_ERR_CUDA;
     CUtensorMap tmG;
-    cuuint64_t gdim[2] = {static_cast<cuuint64_t>(p), static_cast<cuuint64_t>(n)};
-    cuuint64_t gstride[1] = {static_cast<cuuint64_t>(ldg)};
-    cuuint32_t box[2] = {128u, static_cast<cuuint32_t>(kBlk)};
-    cuuint32_t estr[2] = {1, 1};
-    if (enc(&tmG, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<int8_t*>(d_G), gdim, gstride, box, estr,
-            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
-        return KRR_ERR_CUDA;
+    rc = make_genotype_tmap(&tmG, d_G, n, p, ldg);
+    if (rc) return rc;
     BuildOp op;
-    op.n = n; op.p = p; op.nb = nb; op.tiled = tiled ? 1 : 0; op.gamma = gamma;
+    memset(&op, 0, sizeof(op));
+    op.n = n; op.m = n; op.rect = 0; op.p = p; op.nb = nb; op.tiled = tiled ? 1 : 0; op.gamma = gamma;
     op.diag = static_cast<float>(1.0 + static_cast<double>(lambda));
-    op.sq = sq; op.A = d_A; op.lda = lda;
+    op.sq = sq; op.sq_row = sq; op.A = d_A; op.lda = lda;
     const int64_t NT = n / nb, upt = nb / 256;
-    const int64_t total = upt * upt * NT * (NT + 1) / 2;
     const int nacc = (nb % 512 == 0) ? 2 : 1;                      // 256 x 512 blocks when a tile holds them
-    const int64_t max_pairs = num_sms / 2;
-    const int64_t blocks = total / nacc;
-    const int grid = static_cast<int>(2 * (blocks < max_pairs ? blocks : max_pairs));
-    cudaLaunchConfig_t cfg;
-    memset(&cfg, 0, sizeof(cfg));
-    cfg.gridDim = dim3(grid); cfg.blockDim = dim3(kBuildThreads); cfg.dynamicSmemBytes = build_smem(nacc); cfg.stream = st;
-    cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeClusterDimension;
-    attr[0].val.clusterDim.x = 2; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
-    cfg.attrs = attr; cfg.numAttrs = 1;
+    return launch_build(tmG, tmG, op, upt * upt * NT * (NT + 1) / 2 / nacc, nacc, num_sms, st);
+}
+
+// ------------------------------------------------------------------------- Predict phase (NEXT-2)
+size_t krr_predict_workspace(int64_t m, int64_t n) {
+    if (m <= 0 || n <= 0 || m % 256 != 0 || n % 256 != 0) return 0;
+    return align_up(static_cast<size_t>(m) * sizeof(int), 1024) + align_up(static_cast<size_t>(n) * sizeof(int), 1024) +
+           align_up(static_cast<size_t>(m) * n * sizeof(float), 1024);
+}
+
+int krr_predict(const int8_t* d_T, int64_t m, int64_t ldt, const int8_t* d_G, int64_t n, int64_t ldg, int64_t p, float gamma,
+                const float* d_W, int64_t ldw, int nrhs, float* d_P, int64_t ldp, void* d_ws, size_t ws_bytes, void* stream) {
+    g_launches = 0;
+    if (!d_T || !d_G || !d_W || !d_P || !d_ws) return KRR_ERR_ARG;
+    if (m <= 0 || n <= 0 || m % 256 != 0 || n % 256 != 0) return KRR_ERR_SHAPE;
+    if (p < 1 || p > 133000 || ldg < p || ldg % 16 != 0 || ldt < p || ldt % 16 != 0) return KRR_ERR_ARG;
+    if (nrhs < 1 || nrhs > kMaxRhs || ldw < nrhs || ldp < nrhs) return KRR_ERR_ARG;
+    if (reinterpret_cast<uintptr_t>(d_G) % 16 != 0 || reinterpret_cast<uintptr_t>(d_T) % 16 != 0 ||
+        reinterpret_cast<uintptr_t>(d_ws) % 1024 != 0)
+        return KRR_ERR_ARG;
+    if (ws_bytes < krr_predict_workspace(m, n)) return KRR_ERR_WORKSPACE;
+    int num_sms = 0;
+    int rc = check_device(&num_sms);
+    if (rc) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    uint8_t* ws = static_cast<uint8_t*>(d_ws);
+    int* sqT = reinterpret_cast<int*>(ws);
+    int* sqG = reinterpret_cast<int*>(ws + align_up(static_cast<size_t>(m) * sizeof(int), 1024));
+    float* K = reinterpret_cast<float*>(reinterpret_cast<uint8_t*>(sqG) + align_up(static_cast<size_t>(n) * sizeof(int), 1024));
+    rc = launch(CAT_MISC, row_sqnorm_kernel, dim3(static_cast<unsigned>((m + 7) / 8)), dim3(256), 0, st, d_T, m, p, ldt, sqT);
+    if (rc) return rc;
+    rc = launch(CAT_MISC, row_sqnorm_kernel, dim3(static_cast<unsigned>((n + 7) / 8)), dim3(256), 0, st, d_G, n, p, ldg, sqG);
+    if (rc) return rc;
+    CUtensorMap tmT, tmG;
+    if (make_genotype_tmap(&tmT, d_T, m, p, ldt) || make_genotype_tmap(&tmG, d_G, n, p, ldg)) return KRR_ERR_CUDA;
+    BuildOp op;
+    memset(&op, 0, sizeof(op));
+    op.n = n; op.m = m; op.rect = 1; op.p = p; op.nb = 256; op.tiled = 0; op.gamma = gamma; op.diag = 1.0f;
+    op.sq = sqG; op.sq_row = sqT; op.A = K; op.lda = n;
+    const int nacc = (n % 512 == 0) ? 2 : 1;
+    rc = launch_build(tmT, tmG, op, (m / 256) * (n / (256 * nacc)), nacc, num_sms, st);      // K = test x training kernel matrix
+    if (rc) return rc;
+    const int nrp = nrhs <= 8 ? 8 : (nrhs <= 16 ? 16 : 32);
+    const int64_t rows_per_cta = 8 * (32 / nrp) * 4;                 // 8 warps x groups x 4 rows
+    const unsigned grid = static_cast<unsigned>((m + rows_per_cta - 1) / rows_per_cta);
     ProfScope ps(CAT_MISC, st);
     ++g_launches;
-    const cudaError_t e = (nacc == 2) ? cudaLaunchKernelEx(&cfg, build_tc_kernel<2>, tmG, op)
-                                      : cudaLaunchKernelEx(&cfg, build_tc_kernel<1>, tmG, op);
-    return e == cudaSuccess ? KRR_OK : KRR_ERR_CUDA;
+    if (nrp == 8) predict_kw_kernel<8><<<grid, 256, 0, st>>>(K, m, n, n, d_W, ldw, nrhs, d_P, ldp);
+    else if (nrp == 16) predict_kw_kernel<16><<<grid, 256, 0, st>>>(K, m, n, n, d_W, ldw, nrhs, d_P, ldp);
+    else predict_kw_kernel<32><<<grid, 256, 0, st>>>(K, m, n, n, d_W, ldw, nrhs, d_P, ldp);
+    return cudaGetLastError() == cudaSuccess ? KRR_OK : KRR_ERR_CUDA;
 }
 
 }  // extern "C"

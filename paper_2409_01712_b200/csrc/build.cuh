@@ -18,12 +18,15 @@
 namespace krr {
 
 struct BuildOp {
-    int64_t n, p;
+    int64_t n, p;           // columns of the output (patients of the column operand), SNPs
+    int64_t m;              // rows of the output: = n for the symmetric Build, the test cohort for Predict (rect)
+    int rect;               // 1: test x training kernel matrix (Alg. 4 l.5): every block, no diagonal, dense output
     int nb;                 // tile size of A (which tiles are "lower", and the packed layout)
     int tiled;              // KRR_FLAG_A_TILED_LOWER
     float gamma;
     float diag;             // (float)(1.0 + lambda): K_ii = exp(0) = 1 exactly
-    const int* sq;          // s_i = sum_k g_ik^2
+    const int* sq;          // s_j = sum_k g_jk^2 of the column operand
+    const int* sq_row;      // the same of the row operand (= sq for the symmetric Build)
     float* A;
     int64_t lda;
 };
@@ -71,14 +74,15 @@ struct BuildCursor {
     bool done;
 };
 // cw = width of a column unit in 256-column units (NACC); cu counts column units of that width
-__device__ __forceinline__ bool build_valid(int ru, int cu, int upt, int cw) { return ru / upt >= cu * cw / upt; }
+// (upt = 0 marks the rectangular test x training matrix of Predict: every block is wanted)
+__device__ __forceinline__ bool build_valid(int ru, int cu, int upt, int cw) { return upt == 0 || ru / upt >= cu * cw / upt; }
 __device__ __forceinline__ void build_cursor_init(BuildCursor& c, int upt) {
     c.cp = 0; c.ru = 0; c.ci = 0; c.done = false;
     (void)upt;
 }
 // move to the next wanted unit strictly after the current position (or stay if `first` and it is wanted)
-__device__ __forceinline__ void build_cursor_seek(BuildCursor& c, int nru, int upt, int cw, bool first) {
-    const int pw = kBuildPanel / cw, ncu = nru / cw;          // panel width and matrix width in column units
+__device__ __forceinline__ void build_cursor_seek(BuildCursor& c, int nru, int ncu256, int upt, int cw, bool first) {
+    const int pw = kBuildPanel / cw, ncu = ncu256 / cw;       // panel width and matrix width in column units
     bool skip = !first;
     while (!c.done) {
         if (!skip) {
@@ -91,17 +95,17 @@ __device__ __forceinline__ void build_cursor_seek(BuildCursor& c, int nru, int u
             if (++c.ru == nru) {
                 ++c.cp;
                 if (c.cp * pw >= ncu) { c.done = true; return; }
-                c.ru = (c.cp * kBuildPanel / upt) * upt;      // first row unit of the panel's first tile
+                c.ru = upt ? (c.cp * kBuildPanel / upt) * upt : 0;   // first row unit of the panel's first tile
             }
         }
     }
 }
 // the block this pair handles next: `steps` wanted units further (steps = pair index at first, then #pairs)
-__device__ __forceinline__ bool build_next_block(BuildCursor& c, bool& started, int pair0, int npairs, int nru, int upt,
-                                                 int cw, int& ru, int& cu) {
+__device__ __forceinline__ bool build_next_block(BuildCursor& c, bool& started, int pair0, int npairs, int nru, int ncu256,
+                                                 int upt, int cw, int& ru, int& cu) {
     int steps = started ? npairs : pair0;
-    if (!started) { build_cursor_seek(c, nru, upt, cw, true); started = true; }
-    for (; steps > 0 && !c.done; --steps) build_cursor_seek(c, nru, upt, cw, false);
+    if (!started) { build_cursor_seek(c, nru, ncu256, upt, cw, true); started = true; }
+    for (; steps > 0 && !c.done; --steps) build_cursor_seek(c, nru, ncu256, upt, cw, false);
     if (c.done) return false;
     ru = c.ru;
     cu = c.cp * (kBuildPanel / cw) + c.ci;
@@ -110,7 +114,8 @@ __device__ __forceinline__ bool build_next_block(BuildCursor& c, bool& started, 
 
 template <int NACC>
 __global__ void __launch_bounds__(kBuildThreads, 1)
-build_tc_kernel(const __grid_constant__ CUtensorMap tmG, const BuildOp op) {
+build_tc_kernel(const __grid_constant__ CUtensorMap tmR, const __grid_constant__ CUtensorMap tmG, const BuildOp op) {
+    // tmR: genotypes of the row operand (= tmG for the symmetric Build), tmG: of the column operand
     constexpr int kBuildSlots = build_slots(NACC), kBuildSlotBytes = build_slot_bytes(NACC), NBUF = 2 / NACC;
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
@@ -125,13 +130,14 @@ build_tc_kernel(const __grid_constant__ CUtensorMap tmG, const BuildOp op) {
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int rank = static_cast<int>(ptx::cluster_ctarank());
     const int pair0 = static_cast<int>(blockIdx.x >> 1), npairs = static_cast<int>(gridDim.x >> 1);
-    const int nru = static_cast<int>(op.n / 256);
-    const int NT = static_cast<int>(op.n / op.nb), upt = op.nb / 256;
+    const int nru = static_cast<int>(op.m / 256), ncu256 = static_cast<int>(op.n / 256);
+    const int NT = static_cast<int>(op.n / op.nb), upt = op.rect ? 0 : op.nb / 256;
     const int nch = static_cast<int>((op.p + 127) / 128);           // 128-SNP chunks (the last one zero-filled by TMA)
     constexpr uint32_t kHalf = kBlk * 128;                           // 16 KB operand block
 
     if (warp == 0 && lane == 0) {
         ptx::prefetch_tmap(&tmG);
+        ptx::prefetch_tmap(&tmR);
         for (int s = 0; s < kBuildSlots; ++s) { ptx::mbar_init(full_bar(s), 1); ptx::mbar_init(empty_bar(s), 1); }
         for (int b = 0; b < 2; ++b) { ptx::mbar_init(tfull_bar(b), 1); ptx::mbar_init(tempty_bar(b), 16); }
         ptx::fence_mbar_init();
@@ -153,14 +159,14 @@ build_tc_kernel(const __grid_constant__ CUtensorMap tmG, const BuildOp op) {
         build_cursor_init(cur, upt);
         bool started = false;
         int ru, cu;
-        while (build_next_block(cur, started, pair0, npairs, nru, upt, NACC, ru, cu)) {
+        while (build_next_block(cur, started, pair0, npairs, nru, ncu256, upt, NACC, ru, cu)) {
             const int a_row = ru * 256 + rank * kBlk, b_row = cu * 256 * NACC + rank * kBlk;
             for (int ch = 0; ch < nch; ++ch) {
                 ptx::mbar_wait(empty_bar(slot), phase ^ 1u);
                 if (ptx::elect_one()) {
                     const uint32_t sa = smem_base + slot * kBuildSlotBytes;
                     if (rank == 0) ptx::mbar_arrive_expect_tx(full_bar(slot), 2u * (1 + NACC) * kHalf);
-                    ptx::tma_load_2d_pair(sa, &tmG, full_bar(slot), ch * 128, a_row);
+                    ptx::tma_load_2d_pair(sa, &tmR, full_bar(slot), ch * 128, a_row);
 #pragma unroll
                     for (int a = 0; a < NACC; ++a)           // this CTA's 128 rows of each 256-column accumulator
                         ptx::tma_load_2d_pair(sa + (1 + a) * kHalf, &tmG, full_bar(slot), ch * 128, b_row + a * 256);
@@ -179,7 +185,7 @@ build_tc_kernel(const __grid_constant__ CUtensorMap tmG, const BuildOp op) {
             build_cursor_init(cur, upt);
             bool started = false;
             int ru, cu;
-            while (build_next_block(cur, started, pair0, npairs, nru, upt, NACC, ru, cu)) {
+            while (build_next_block(cur, started, pair0, npairs, nru, ncu256, upt, NACC, ru, cu)) {
                 ptx::mbar_wait(tempty_bar(buf), acc_phase ^ 1u);
                 ptx::tc_fence_after();
                 const uint32_t d_tmem = tmem_base + buf * 256 * NACC;
@@ -213,10 +219,10 @@ build_tc_kernel(const __grid_constant__ CUtensorMap tmG, const BuildOp op) {
         build_cursor_init(cur, upt);
         bool started = false;
         int ru, cu;
-        while (build_next_block(cur, started, pair0, npairs, nru, upt, NACC, ru, cu)) {
+        while (build_next_block(cur, started, pair0, npairs, nru, ncu256, upt, NACC, ru, cu)) {
             const int64_t gi = static_cast<int64_t>(ru) * 256 + rank * kBlk + q * 32 + lane;       // my row of A
-            const int si = op.sq[gi];
-            const int ti = static_cast<int>(gi / op.nb);
+            const int si = op.sq_row[gi];
+            const int ti = op.rect ? 0x7fffffff : static_cast<int>(gi / op.nb);
             ptx::mbar_wait(tfull_bar(buf), acc_phase);
             ptx::tc_fence_after();
 #pragma unroll 1
@@ -233,7 +239,7 @@ build_tc_kernel(const __grid_constant__ CUtensorMap tmG, const BuildOp op) {
                 }
                 const int tj = static_cast<int>(gj0 / op.nb);
                 if (tj > ti) continue;                                               // an upper tile: not produced
-                float* dst = op.tiled
+                float* dst = (op.tiled && !op.rect)
                     ? op.A + (tile_slot(NT, ti, tj) * op.nb + gi % op.nb) * static_cast<int64_t>(op.nb) + gj0 % op.nb
                     : op.A + gi * op.lda + gj0;
 #pragma unroll
@@ -242,7 +248,7 @@ build_tc_kernel(const __grid_constant__ CUtensorMap tmG, const BuildOp op) {
 #pragma unroll
                     for (int u = 0; u < 4; ++u) {
                         const int d2 = si + __ldg(op.sq + gj0 + e + u) - 2 * static_cast<int>(acc[e + u]);
-                        v[u] = (gj0 + e + u == gi) ? op.diag : expf(-op.gamma * static_cast<float>(d2));
+                        v[u] = (!op.rect && gj0 + e + u == gi) ? op.diag : expf(-op.gamma * static_cast<float>(d2));
                     }
                     *reinterpret_cast<float4*>(dst + e) = make_float4(v[0], v[1], v[2], v[3]);
                 }
@@ -253,6 +259,47 @@ build_tc_kernel(const __grid_constant__ CUtensorMap tmG, const BuildOp op) {
     ptx::tc_fence_before();
     ptx::cluster_sync_all();
     if (warp == 1) ptx::tmem_dealloc<512, 2>(tmem_base);
+}
+
+// P = K W (Alg. 4 l.6): K m x n FP32 row-major (ldk, n % 4 == 0, 16-byte aligned rows), W n x nrhs
+// row-major (ldw), P m x nrhs (ldp).  Lane = right-hand side r (NRP = nrhs rounded up to 8 / 16 / 32; 32 / NRP
+// groups of lanes per warp), every group owns 4 rows of K: per 4 columns a group reads 4 float4 of K (the same
+// address in all its lanes) and 4 coalesced rows of W, each reused by the 4 rows.  Every (row, r) sum runs over
+// the columns in order in four interleaved partial sums -- a fixed order, no reduction across lanes.  Bound by
+// the read of K from HBM.
+template <int NRP>
+__global__ void __launch_bounds__(256)
+predict_kw_kernel(const float* __restrict__ K, int64_t m, int64_t n, int64_t ldk, const float* __restrict__ W, int64_t ldw,
+                  int nrhs, float* __restrict__ P, int64_t ldp) {
+    constexpr int GROUPS = 32 / NRP, ROWS = 4;
+    const int lane = threadIdx.x & 31, g = lane / NRP, r = lane % NRP;
+    const int64_t warp = static_cast<int64_t>(blockIdx.x) * 8 + (threadIdx.x >> 5);
+    const int64_t row0 = (warp * GROUPS + g) * ROWS;
+    if (row0 >= m) return;
+    const bool active = r < nrhs;
+    float acc[ROWS][4];
+#pragma unroll
+    for (int i = 0; i < ROWS; ++i)
+#pragma unroll
+        for (int u = 0; u < 4; ++u) acc[i][u] = 0.0f;
+    const float* k0 = K + row0 * ldk;
+    for (int64_t j = 0; j < n; j += 4) {
+        float w[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) w[u] = active ? __ldg(W + (j + u) * ldw + r) : 0.0f;
+#pragma unroll
+        for (int i = 0; i < ROWS; ++i) {
+            const float4 kv = (row0 + i < m) ? __ldg(reinterpret_cast<const float4*>(k0 + i * ldk + j)) : make_float4(0.f, 0.f, 0.f, 0.f);
+            acc[i][0] = fmaf(kv.x, w[0], acc[i][0]);
+            acc[i][1] = fmaf(kv.y, w[1], acc[i][1]);
+            acc[i][2] = fmaf(kv.z, w[2], acc[i][2]);
+            acc[i][3] = fmaf(kv.w, w[3], acc[i][3]);
+        }
+    }
+    if (active)
+#pragma unroll
+        for (int i = 0; i < ROWS; ++i)
+            if (row0 + i < m) P[(row0 + i) * ldp + r] = (acc[i][0] + acc[i][1]) + (acc[i][2] + acc[i][3]);
 }
 
 }  // namespace krr

@@ -118,3 +118,63 @@ def test_build_argument_errors(krr):
     assert call(512, 150, 152, 256) == -1            # row pitch not a multiple of 16 bytes
     assert call(512, 160, 160, 256, 8) == -7         # unsupported flag
     torch.cuda.synchronize()
+
+
+# ------------------------------------------------------------------------------ Predict (Alg. 4)
+@pytest.mark.parametrize("m,n,p,nrhs", [(256, 512, 300, 4), (512, 768, 1000, 16), (768, 1024, 129, 32), (256, 256, 64, 1)])
+def test_predict_matches_definition(krr, m, n, p, nrhs):
+    """K(T, G) entrywise within 8e-7 K (as for krr_build); P_r = K W against the FP64 product: FP32 products and
+    sums of n terms of size <= max|W| -> |P_gpu - P| <= 4e-6 * sum_j K_ij |W_jr| (a few n^(1/2) 2^-24, with margin)."""
+    from oracle.build_phase import cross_kernel_matrix_definition, predict_definition
+    G = genotypes(21, n, p, "maf", device="cuda")
+    T = genotypes(22, m, p, "maf", device="cuda")
+    gamma = 1.0 / p
+    W = torch.randn((n, nrhs), device="cuda", generator=torch.Generator(device="cuda").manual_seed(1))
+    P, K = krr.krr_predict(padded(T), padded(G), gamma, W, return_kernel=True)
+    torch.cuda.synchronize()
+    Kw = cross_kernel_matrix_definition(T.cpu().numpy(), G.cpu().numpy(), gamma)
+    Kg = K.cpu().numpy().astype(np.float64)
+    assert np.all(np.abs(Kg - Kw) <= 8e-7 * Kw)
+    Pw = predict_definition(T.cpu().numpy(), G.cpu().numpy(), gamma, W.cpu().numpy())
+    bound = 4e-6 * (Kw @ np.abs(W.cpu().numpy().astype(np.float64))) + 1e-30
+    assert np.all(np.abs(P.cpu().numpy() - Pw) <= bound)
+
+
+def test_build_associate_predict_end_to_end_mspe_and_pearson(krr):
+    """Alg. 1 end to end on a synthetic phenotype with an epistatic (pairwise-interaction) signal: Build ->
+    precision map -> factorisation -> solve -> Predict on a held-out cohort; MSPE and Pearson correlation of the
+    CUDA path against the same pipeline in FP64 (oracle definitions), all-FP32 map and the FP16 map."""
+    from oracle.build_phase import kernel_matrix_definition, mspe, pearson, predict_definition
+    n, m, p, nb = 1536, 512, 400, 256
+    Gall = genotypes(31, n + m, p, "maf", device="cuda")
+    G, T = Gall[:n].contiguous(), Gall[n:].contiguous()
+    rng = np.random.default_rng(0)
+    X = Gall.cpu().numpy().astype(np.float64)
+    X = (X - X.mean(0)) / (X.std(0) + 1e-12)
+    beta = rng.standard_normal(p) * (rng.random(p) < 0.1)
+    pairs = rng.integers(0, p, size=(40, 2))
+    signal = X @ beta + 1.5 * sum(X[:, a] * X[:, b] for a, b in pairs)
+    Yall = np.stack([signal + 0.5 * signal.std() * rng.standard_normal(n + m) for _ in range(2)], axis=1)
+    Yall = (Yall - Yall[:n].mean(0)) / Yall[:n].std(0)
+    Y, Ytest = Yall[:n], Yall[n:]
+    gamma, lam = 1.0 / p, 1e-1
+    # FP64 pipeline from the definitions
+    A64 = kernel_matrix_definition(G.cpu().numpy(), gamma, lam)
+    W64 = np.linalg.solve(A64, Y)
+    P64 = predict_definition(T.cpu().numpy(), G.cpu().numpy(), gamma, W64)
+    # CUDA pipeline
+    A = krr.krr_build(padded(G), gamma, lam, nb)
+    Yd = torch.from_numpy(Y.astype(np.float32)).cuda()
+    for forced in (krr.FP32, krr.FP16):
+        h = krr.uniform_map(n // nb, forced)
+        F = krr.potrf_mp(A, nb, h.cuda(), h)
+        Wd = krr.potrs(F, Yd.clone())
+        P = krr.krr_predict(padded(T), padded(G), gamma, Wd).cpu().numpy().astype(np.float64)
+        torch.cuda.synchronize()
+        assert int(F.info.item()) == 0
+        m64, mg = mspe(Ytest, P64), mspe(Ytest, P)
+        r64, rg = pearson(Ytest, P64), pearson(Ytest, P)
+        print(f"map {forced}: MSPE fp64 {m64} gpu {mg}; Pearson fp64 {r64} gpu {rg}")
+        tol = 1e-4 if forced == krr.FP32 else 2e-2
+        assert np.all(np.abs(mg - m64) <= tol * m64) and np.all(np.abs(rg - r64) <= tol)
+        assert np.all(r64 > 0.1)                    # the synthetic signal is learnable: the comparison is not vacuous

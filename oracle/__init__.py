@@ -19,6 +19,11 @@ What it computes, and where the paper defines it (citations are PAPER.md lines):
 * `oracle.solve.potrs_fp64`              -- Solve(K~, P_h), Alg. 3 l.5, forward and
   backward substitution.
 
+* `oracle.build_phase`                    -- Build (Alg. 2 with the Gaussian kernel of Alg. 5, PAPER.md:92-106,
+  :136-143) and Predict (Alg. 4, :116-122) by their definitions in exact integers / FP64, and the paper's MSPE
+  (:243) and Pearson correlation (:262-266); pinned by the paper's three-patient example (:176-188), the
+  D + D^T - 2 G G^T identity, scipy cdist, closed forms and numpy.corrcoef (tests/test_oracle_build.py).
+
 Pins (tests/test_oracle_*.py, all `-m "not gpu"`): closed-form factors (diagonal, Lehmer, min(i,j),
 equicorrelation, Kac-Murdock-Szego, hand 2x2/3x3), brute-force scalar Cholesky for n <= 64 and every
 nb | n, LAPACK (numpy) Cholesky, invariants, exactly-representable constructions that every

@@ -201,6 +201,9 @@ int krr_associate_host(const float* h_A, int64_t n, int64_t lda, int nb,
  * d_G    in   n x p signed 8-bit genotypes, row-major with row pitch ldg bytes (ldg >= p, ldg % 16 == 0,
  *             16-byte aligned); any int8 values (the workloads use {0,1,2}); p <= 133000 keeps the INT32
  *             sums exact.  Not modified.
+ * d_C    in   optional confounders: n x q FP32 real-valued covariates, row-major (ldc), q <= 16;
+ *             their squared distance sum_t (c_it - c_jt)^2 is accumulated in FP32 and added to the integer
+ *             squared distance before the exponentiation.  NULL / q = 0: none.
  * gamma, lambda  kernel bandwidth and regulariser; the diagonal is (float)(1 + lambda) exactly.
  * d_A    out  the lower TILES of A (tile row >= tile column; diagonal tiles as full squares) in FP32:
  *             n x n row-major with lda (lda % 4 == 0; tiles above the diagonal are not written), or
@@ -208,11 +211,11 @@ int krr_associate_host(const float* h_A, int64_t n, int64_t lda, int nb,
  *             and krr_potrf_mp.  exp is evaluated in FP32 (expf of the FP32 product gamma*d2, d2 exact):
  *             entries agree with the FP64-evaluated, FP32-rounded kernel to a few ulp.
  * n % 256 == 0, nb % 256 == 0, n % nb == 0.  d_ws: krr_build_workspace(n) bytes (the folded vector s).
- * The confounder (real-valued covariate) term of :190 is not implemented yet.
  */
 size_t krr_build_workspace(int64_t n);
-int krr_build(const int8_t* d_G, int64_t n, int64_t p, int64_t ldg, float gamma, float lambda,
-              float* d_A, int64_t lda, int nb, unsigned flags, void* d_ws, size_t ws_bytes, void* stream);
+int krr_build(const int8_t* d_G, int64_t n, int64_t p, int64_t ldg, const float* d_C, int q, int64_t ldc,
+              float gamma, float lambda, float* d_A, int64_t lda, int nb, unsigned flags,
+              void* d_ws, size_t ws_bytes, void* stream);
 
 /* ---------------------------------------------------------------------------------------------
  * krr_predict -- Predict phase (Alg. 4 :116-122):
@@ -223,6 +226,7 @@ int krr_build(const int8_t* d_G, int64_t n, int64_t p, int64_t ldg, float gamma,
  * summation order).
  * d_T  in  m x p int8 test genotypes (row pitch ldt), d_G in n x p int8 training genotypes (ldg); both
  *          pitches multiples of 16 bytes, 16-byte aligned; m % 256 == 0, n % 256 == 0, p <= 133000.
+ * d_CT, d_CG  in  optional confounders of the two cohorts (m x q, n x q FP32, ldct / ldcg), as for krr_build.
  * d_W  in  n x nrhs FP32 row-major (ldw): the weights of krr_potrs; nrhs <= 32.
  * d_P  out m x nrhs FP32 row-major (ldp): the predicted phenotypes.
  * d_ws     krr_predict_workspace(m, n) bytes, 1024-byte aligned; on return it holds, after the two
@@ -230,6 +234,7 @@ int krr_build(const int8_t* d_G, int64_t n, int64_t p, int64_t ldg, float gamma,
  */
 size_t krr_predict_workspace(int64_t m, int64_t n);
 int krr_predict(const int8_t* d_T, int64_t m, int64_t ldt, const int8_t* d_G, int64_t n, int64_t ldg, int64_t p,
+                const float* d_CT, int64_t ldct, const float* d_CG, int64_t ldcg, int q,
                 float gamma, const float* d_W, int64_t ldw, int nrhs, float* d_P, int64_t ldp,
                 void* d_ws, size_t ws_bytes, void* stream);
 

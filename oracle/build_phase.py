@@ -28,10 +28,24 @@ def squared_distances(G1, G2):
     return D
 
 
-def kernel_matrix_definition(G, gamma, lam):
-    """A = K + lam*I in FP64: K_ij = exp(-gamma * d_ij) (Alg. 5 l.4), d_ij by the definition."""
-    D = squared_distances(G, G)
-    A = np.exp(-float(gamma) * D.astype(np.float64))
+def confounder_distances(C1, C2):
+    """squared distances between the real-valued confounders, sum_t (c1_it - c2_jt)^2, in FP64."""
+    C1 = np.asarray(C1, dtype=np.float64)
+    C2 = np.asarray(C2, dtype=np.float64)
+    D = np.empty((C1.shape[0], C2.shape[0]))
+    for i in range(C1.shape[0]):
+        diff = C2 - C1[i][None, :]
+        D[i] = np.einsum("jk,jk->j", diff, diff)
+    return D
+
+
+def kernel_matrix_definition(G, gamma, lam, C=None):
+    """A = K + lam*I in FP64: K_ij = exp(-gamma * d_ij) (Alg. 5 l.4), d_ij by the definition; with confounders C
+    their squared distance is added to the integer one before the exponentiation."""
+    D = squared_distances(G, G).astype(np.float64)
+    if C is not None:
+        D = D + confounder_distances(C, C)
+    A = np.exp(-float(gamma) * D)
     A[np.diag_indices_from(A)] += float(lam)
     return A
 
@@ -46,14 +60,17 @@ def squared_distance_by_expansion(G):
 
 
 # ---- Predict phase (Alg. 4) and the paper's accuracy measures ----
-def cross_kernel_matrix_definition(T, G, gamma):
+def cross_kernel_matrix_definition(T, G, gamma, CT=None, CG=None):
     """Alg. 4 l.4-5: K (N_P2 x N_P1), K_ij = exp(-gamma ||t_i - g_j||^2) -- BUILD(gamma, T, G, K), no regulariser."""
-    return np.exp(-float(gamma) * squared_distances(T, G).astype(np.float64))
+    D = squared_distances(T, G).astype(np.float64)
+    if CT is not None:
+        D = D + confounder_distances(CT, CG)
+    return np.exp(-float(gamma) * D)
 
 
-def predict_definition(T, G, gamma, W):
+def predict_definition(T, G, gamma, W, CT=None, CG=None):
     """Alg. 4 l.6: P_r = K x W in FP64."""
-    return cross_kernel_matrix_definition(T, G, gamma) @ np.asarray(W, dtype=np.float64)
+    return cross_kernel_matrix_definition(T, G, gamma, CT, CG) @ np.asarray(W, dtype=np.float64)
 
 
 def mspe(Y, Yhat):

@@ -75,11 +75,12 @@ def lib():
     L.krr_build_workspace.restype = sz
     L.krr_build_workspace.argtypes = [i64]
     L.krr_build.restype = c.c_int
-    L.krr_build.argtypes = [vp, i64, i64, i64, c.c_float, c.c_float, vp, i64, c.c_int, u32, vp, sz, vp]
+    L.krr_build.argtypes = [vp, i64, i64, i64, vp, c.c_int, i64, c.c_float, c.c_float, vp, i64, c.c_int, u32, vp, sz, vp]
     L.krr_predict_workspace.restype = sz
     L.krr_predict_workspace.argtypes = [i64, i64]
     L.krr_predict.restype = c.c_int
-    L.krr_predict.argtypes = [vp, i64, i64, vp, i64, i64, i64, c.c_float, vp, i64, c.c_int, vp, i64, vp, sz, vp]
+    L.krr_predict.argtypes = [vp, i64, i64, vp, i64, i64, i64, vp, i64, vp, i64, c.c_int, c.c_float, vp, i64, c.c_int, vp, i64,
+                              vp, sz, vp]
     L.krr_last_launch_count.restype = i64
     L.krr_profile_enable.restype = c.c_int
     L.krr_profile_enable.argtypes = [u32]
@@ -285,7 +286,14 @@ def associate_host(h_A, nb, h_Y, eps_target=0.0, allowed=(FP32,), force_prec=-1,
     return alpha, h_map, int(h_info[0]), arena
 
 
-def krr_build(G, gamma, lam, nb, tiled_lower=False, out=None, flags=0):
+def _conf(C):
+    if C is None:
+        return None, 0, 0
+    assert C.dtype == torch.float32 and C.is_cuda and C.stride(1) == 1
+    return C, C.shape[1], C.stride(0)
+
+
+def krr_build(G, gamma, lam, nb, tiled_lower=False, out=None, flags=0, C=None):
     """krr_build (named in full: `build` is this package's compile step): A = K + lam*I (Gaussian kernel) from CUDA int8 genotypes G (n x p, row-major, row pitch a
     multiple of 16 bytes).  Returns A: n x n FP32 with the lower tiles written (the rest zero), or the packed
     lower tiles with tiled_lower."""
@@ -303,12 +311,13 @@ def krr_build(G, gamma, lam, nb, tiled_lower=False, out=None, flags=0):
     ws = _ws(wsb, dev)
     flags |= FLAG_A_TILED_LOWER if tiled_lower else 0
     lda = nb if tiled_lower else out.stride(0)
-    _check(L.krr_build(_ptr(G), n, p, G.stride(0), float(gamma), float(lam), _ptr(out), lda, nb, flags, _ptr(ws), wsb,
-                       _stream()), "krr_build")
+    C, q, ldc = _conf(C)
+    _check(L.krr_build(_ptr(G), n, p, G.stride(0), _ptr(C), q, ldc, float(gamma), float(lam), _ptr(out), lda, nb, flags,
+                       _ptr(ws), wsb, _stream()), "krr_build")
     return out
 
 
-def krr_predict(T, G, gamma, W, return_kernel=False):
+def krr_predict(T, G, gamma, W, return_kernel=False, CT=None, CG=None):
     """krr_predict: P_r = K(T, G) W (Alg. 4).  T (m x p), G (n x p): CUDA int8, row pitch a multiple of 16 bytes;
     W: CUDA FP32 n x nrhs.  Returns P (m x nrhs) and, on request, the test-training kernel matrix (a view
     into the call's workspace)."""
@@ -323,8 +332,11 @@ def krr_predict(T, G, gamma, W, return_kernel=False):
         raise KrrError("krr_predict_workspace: m and n must be multiples of 256")
     ws = _ws(wsb, G.device)
     P = torch.empty((m, nrhs), dtype=torch.float32, device=G.device)
-    _check(L.krr_predict(_ptr(T), m, T.stride(0), _ptr(G), n, G.stride(0), p, float(gamma), _ptr(W), W.stride(0), nrhs,
-                         _ptr(P), P.stride(0), _ptr(ws), wsb, _stream()), "krr_predict")
+    CT, q, ldct = _conf(CT)
+    CG, q2, ldcg = _conf(CG)
+    assert q == q2
+    _check(L.krr_predict(_ptr(T), m, T.stride(0), _ptr(G), n, G.stride(0), p, _ptr(CT), ldct, _ptr(CG), ldcg, q, float(gamma),
+                         _ptr(W), W.stride(0), nrhs, _ptr(P), P.stride(0), _ptr(ws), wsb, _stream()), "krr_predict")
     if not return_kernel:
         return P
     off = (m * 4 + 1023) // 1024 * 1024 + (n * 4 + 1023) // 1024 * 1024

@@ -812,10 +812,11 @@ size_t krr_build_workspace(int64_t n) {
     return align_up(static_cast<size_t>(n) * sizeof(int), 1024);           // the folded squared norms
 }
 
-int krr_build(const int8_t* d_G, int64_t n, int64_t p, int64_t ldg, float gamma, float lambda, float* d_A, int64_t lda,
-              int nb, unsigned flags, void* d_ws, size_t ws_bytes, void* stream) {
+int krr_build(const int8_t* d_G, int64_t n, int64_t p, int64_t ldg, const float* d_C, int q, int64_t ldc, float gamma,
+              float lambda, float* d_A, int64_t lda, int nb, unsigned flags, void* d_ws, size_t ws_bytes, void* stream) {
     g_launches = 0;
     if (!d_G || !d_A || !d_ws) return KRR_ERR_ARG;
+    if (q < 0 || q > kMaxConfounders || (q > 0 && (!d_C || ldc < q))) return KRR_ERR_ARG;
     int rc = check_shape(n, nb);
     if (rc) return rc;
     if (n % 256 != 0 || nb % 256 != 0) return KRR_ERR_SHAPE;
@@ -842,6 +843,7 @@ int krr_build(const int8_t* d_G, int64_t n, int64_t p, int64_t ldg, float gamma,
     op.n = n; op.m = n; op.rect = 0; op.p = p; op.nb = nb; op.tiled = tiled ? 1 : 0; op.gamma = gamma;
     op.diag = static_cast<float>(1.0 + static_cast<double>(lambda));
     op.sq = sq; op.sq_row = sq; op.A = d_A; op.lda = lda;
+    op.C = d_C; op.C_row = d_C; op.ldc = ldc; op.ldc_row = ldc; op.q = q;
     const int64_t NT = n / nb, upt = nb / 256;
     const int nacc = (nb % 512 == 0) ? 2 : 1;                      // 256 x 512 blocks when a tile holds them
     return launch_build(tmG, tmG, op, upt * upt * NT * (NT + 1) / 2 / nacc, nacc, num_sms, st);
@@ -854,10 +856,12 @@ size_t krr_predict_workspace(int64_t m, int64_t n) {
            align_up(static_cast<size_t>(m) * n * sizeof(float), 1024);
 }
 
-int krr_predict(const int8_t* d_T, int64_t m, int64_t ldt, const int8_t* d_G, int64_t n, int64_t ldg, int64_t p, float gamma,
+int krr_predict(const int8_t* d_T, int64_t m, int64_t ldt, const int8_t* d_G, int64_t n, int64_t ldg, int64_t p,
+                const float* d_CT, int64_t ldct, const float* d_CG, int64_t ldcg, int q, float gamma,
                 const float* d_W, int64_t ldw, int nrhs, float* d_P, int64_t ldp, void* d_ws, size_t ws_bytes, void* stream) {
     g_launches = 0;
     if (!d_T || !d_G || !d_W || !d_P || !d_ws) return KRR_ERR_ARG;
+    if (q < 0 || q > kMaxConfounders || (q > 0 && (!d_CT || !d_CG || ldct < q || ldcg < q))) return KRR_ERR_ARG;
     if (m <= 0 || n <= 0 || m % 256 != 0 || n % 256 != 0) return KRR_ERR_SHAPE;
     if (p < 1 || p > 133000 || ldg < p || ldg % 16 != 0 || ldt < p || ldt % 16 != 0) return KRR_ERR_ARG;
     if (nrhs < 1 || nrhs > kMaxRhs || ldw < nrhs || ldp < nrhs) return KRR_ERR_ARG;
@@ -883,6 +887,7 @@ int krr_predict(const int8_t* d_T, int64_t m, int64_t ldt, const int8_t* d_G, in
     memset(&op, 0, sizeof(op));
     op.n = n; op.m = m; op.rect = 1; op.p = p; op.nb = 256; op.tiled = 0; op.gamma = gamma; op.diag = 1.0f;
     op.sq = sqG; op.sq_row = sqT; op.A = K; op.lda = n;
+    op.C = d_CG; op.C_row = d_CT; op.ldc = ldcg; op.ldc_row = ldct; op.q = q;
     const int nacc = (n % 512 == 0) ? 2 : 1;
     rc = launch_build(tmT, tmG, op, (m / 256) * (n / (256 * nacc)), nacc, num_sms, st);      // K = test x training kernel matrix
     if (rc) return rc;

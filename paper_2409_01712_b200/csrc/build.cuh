@@ -29,7 +29,14 @@ struct BuildOp {
     const int* sq_row;      // the same of the row operand (= sq for the symmetric Build)
     float* A;
     int64_t lda;
+    // confounders: real-valued covariates whose squared distance, accumulated in FP32, is added to the
+    // integer squared distance before the exponentiation.  q = 0: none.
+    const float* C;         // column operand's confounders, n x q row-major (ldc)
+    const float* C_row;     // row operand's (= C for the symmetric Build)
+    int64_t ldc, ldc_row;
+    int q;
 };
+constexpr int kMaxConfounders = 16;
 
 // NACC = 256-column accumulators per pair: 2 -> a pair computes 256 x 512 (all 512 TMEM columns, the exp epilogue
 // is then not overlapped with the next block's MMAs -- a few % at thousands of SNPs -- but every byte of the row
@@ -223,6 +230,9 @@ build_tc_kernel(const __grid_constant__ CUtensorMap tmR, const __grid_constant__
             const int64_t gi = static_cast<int64_t>(ru) * 256 + rank * kBlk + q * 32 + lane;       // my row of A
             const int si = op.sq_row[gi];
             const int ti = op.rect ? 0x7fffffff : static_cast<int>(gi / op.nb);
+            float ci[kMaxConfounders];
+#pragma unroll
+            for (int c = 0; c < kMaxConfounders; ++c) ci[c] = (c < op.q) ? __ldg(op.C_row + gi * op.ldc_row + c) : 0.0f;
             ptx::mbar_wait(tfull_bar(buf), acc_phase);
             ptx::tc_fence_after();
 #pragma unroll 1
@@ -248,7 +258,16 @@ build_tc_kernel(const __grid_constant__ CUtensorMap tmR, const __grid_constant__
 #pragma unroll
                     for (int u = 0; u < 4; ++u) {
                         const int d2 = si + __ldg(op.sq + gj0 + e + u) - 2 * static_cast<int>(acc[e + u]);
-                        v[u] = (!op.rect && gj0 + e + u == gi) ? op.diag : expf(-op.gamma * static_cast<float>(d2));
+                        float d2f = static_cast<float>(d2);
+                        if (op.q > 0) {
+                            const float* cj = op.C + (gj0 + e + u) * op.ldc;      // the same address in every lane
+                            float dc = 0.0f;
+#pragma unroll
+                            for (int c = 0; c < kMaxConfounders; ++c)
+                                if (c < op.q) { const float t = ci[c] - __ldg(cj + c); dc = fmaf(t, t, dc); }
+                            d2f += dc;
+                        }
+                        v[u] = (!op.rect && gj0 + e + u == gi) ? op.diag : expf(-op.gamma * d2f);
                     }
                     *reinterpret_cast<float4*>(dst + e) = make_float4(v[0], v[1], v[2], v[3]);
                 }

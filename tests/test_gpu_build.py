@@ -111,7 +111,7 @@ def test_build_argument_errors(krr):
     A = torch.zeros((512, 512), dtype=torch.float32, device="cuda")
     ws = torch.zeros(4096, dtype=torch.uint8, device="cuda")
     vp = lambda t: ctypes.c_void_p(t.data_ptr())
-    call = lambda n, p, ldg, nb, flags=0: L.krr_build(vp(G), n, p, ldg, 0.01, 0.01, vp(A), 512, nb, flags, vp(ws), 4096, None)
+    call = lambda n, p, ldg, nb, flags=0: L.krr_build(vp(G), n, p, ldg, None, 0, 0, 0.01, 0.01, vp(A), 512, nb, flags, vp(ws), 4096, None)
     assert call(512, 160, 160, 256) == 0
     assert call(500, 160, 160, 250) == -2            # n, nb not multiples of 256
     assert call(512, 160, 150, 256) == -1            # ldg < p
@@ -178,3 +178,36 @@ def test_build_associate_predict_end_to_end_mspe_and_pearson(krr):
         tol = 1e-4 if forced == krr.FP32 else 2e-2
         assert np.all(np.abs(mg - m64) <= tol * m64) and np.all(np.abs(rg - r64) <= tol)
         assert np.all(r64 > 0.1)                    # the synthetic signal is learnable: the comparison is not vacuous
+
+
+@pytest.mark.parametrize("q", [1, 5, 16])
+def test_build_and_predict_with_confounders(krr, q):
+    """confounder distances accumulated in FP32 and added before the exponentiation.  Tolerance: the
+    FP32 confounder sum and its addition to the (exact) integer distance add <= (q + 2) 2^-24 relative to the
+    exponent gamma*d <= ~4, on top of the 8e-7 of the plain kernel: 2e-6 K."""
+    from oracle.build_phase import cross_kernel_matrix_definition, kernel_matrix_definition
+    n, m, p, nb = 768, 256, 500, 256
+    G = genotypes(41, n, p, "maf", device="cuda")
+    T = genotypes(42, m, p, "maf", device="cuda")
+    gen = torch.Generator(device="cuda").manual_seed(q)
+    C = 3.0 * torch.randn((n, q), device="cuda", generator=gen)
+    CT = 3.0 * torch.randn((m, q), device="cuda", generator=gen)
+    gamma, lam = 1.0 / p, 1e-2
+    A = krr.krr_build(padded(G), gamma, lam, nb, C=C)
+    W = torch.randn((n, 3), device="cuda", generator=gen)
+    P, K = krr.krr_predict(padded(T), padded(G), gamma, W, return_kernel=True, CT=CT, CG=C)
+    torch.cuda.synchronize()
+    want = kernel_matrix_definition(G.cpu().numpy(), gamma, lam, C.cpu().numpy())
+    got = A.cpu().numpy().astype(np.float64)
+    low = np.tril_indices(n)
+    NT = n // nb
+    for i in range(NT):
+        for j in range(i + 1):
+            g, w = got[i * nb:(i + 1) * nb, j * nb:(j + 1) * nb], want[i * nb:(i + 1) * nb, j * nb:(j + 1) * nb]
+            assert np.all(np.abs(g - w) <= 2e-6 * w)
+    assert np.all(np.diag(got) == np.float64(np.float32(1.0 + lam)))
+    Kw = cross_kernel_matrix_definition(T.cpu().numpy(), G.cpu().numpy(), gamma, CT.cpu().numpy(), C.cpu().numpy())
+    assert np.all(np.abs(K.cpu().numpy() - Kw) <= 2e-6 * Kw)
+    assert float(np.abs(Kw - cross_kernel_matrix_definition(T.cpu().numpy(), G.cpu().numpy(), gamma)).max()) > 1e-3   # the term matters
+    Pw = Kw @ W.cpu().numpy().astype(np.float64)
+    assert np.all(np.abs(P.cpu().numpy() - Pw) <= 6e-6 * (Kw @ np.abs(W.cpu().numpy().astype(np.float64))))

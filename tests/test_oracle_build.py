@@ -114,3 +114,22 @@ def test_mspe_and_pearson_definitions():
     assert abs(pearson(A, 2.5 * A + 1.0)[0] - 1.0) < 1e-14 and abs(pearson(A, -A)[1] + 1.0) < 1e-14
     assert np.all(mspe(A, A) == 0.0)
 
+
+
+def test_confounder_term_closed_forms():
+    """the squared distance of the real-valued confounders is added before the exponentiation, so the
+    kernel factorises: K(G, C) = K(G) * K_rbf(C) entrywise; with zero genotypes it is the plain Gaussian RBF on C."""
+    from oracle.build_phase import confounder_distances
+    rng = np.random.default_rng(5)
+    G = rng.integers(0, 3, size=(25, 40)).astype(np.int8)
+    C = rng.standard_normal((25, 3))
+    gamma = 0.03
+    assert np.allclose(confounder_distances(C, C), cdist(C, C, "sqeuclidean"), atol=1e-12)
+    K = kernel_matrix_definition(G, gamma, 0.0, C)
+    assert np.allclose(K, kernel_matrix_definition(G, gamma, 0.0) * np.exp(-gamma * cdist(C, C, "sqeuclidean")), rtol=1e-13)
+    Z = np.zeros_like(G)
+    assert np.allclose(kernel_matrix_definition(Z, gamma, 0.25, C), np.exp(-gamma * cdist(C, C, "sqeuclidean")) + 0.25 * np.eye(25),
+                       rtol=1e-13)
+    T, CT = G[:7], C[:7] + 0.5
+    Kx = cross_kernel_matrix_definition(T, G, gamma, CT, C)
+    assert abs(Kx[2, 9] - np.exp(-gamma * (np.sum((T[2].astype(int) - G[9].astype(int)) ** 2) + np.sum((CT[2] - C[9]) ** 2)))) < 1e-15

@@ -594,6 +594,11 @@ size_t krr_potrs_workspace(int64_t n, int nb, int nrhs) {
 
 }  // extern "C"
 
+// Forward and backward sweeps with a one-column lookahead on the library's internal streams (`sh` chain, `sl` bulk):
+// once z_k (alpha_k) is known, the update of the NEXT tile row (column) -- all the next diagonal solve waits for --
+// runs on the chain stream, the update of the remaining rows on the bulk stream beside that solve.  Updates of the
+// same rows of B are read-modify-write, so their order is fixed by events (deterministic results): the chain's
+// update of row k+2 by column k+1 waits for the bulk update by column k.
 template <int NRHS>
 static int potrs_run(const uint8_t* factor, const float* d_scales, const uint8_t* d_map, const std::vector<int64_t>& hoff,
                      const int64_t* off, const float* dinv, const float* dinvT, int NT, int nb, float* B, int64_t ldb,
@@ -604,33 +609,87 @@ static int potrs_run(const uint8_t* factor, const float* d_scales, const uint8_t
     const size_t smem_bu = smem_z + static_cast<size_t>(NW / 2) * 32 * CPL * NRHS * sizeof(float);
     const int64_t blk_elems = static_cast<int64_t>(kBlk) * kBlk;
     const int nsub = nb / kBlk;
+    const bool pipe = NT > 2;
+    cudaStream_t sh = st, sl = st;
+    enum { EV_FORK = 0, EV_JOIN_HI = 1, EV_JOIN_LO = 3, EV_BASE = 4 };      // the event pool of krr_potrf_mp, reused
+    auto ev_diag = [&](int k) { return g_pipe.event(EV_BASE + 4 * static_cast<size_t>(k) + 0); };
+    auto ev_bulk = [&](int k) { return g_pipe.event(EV_BASE + 4 * static_cast<size_t>(k) + 1); };
     int rc;
-    for (int k = 0; k < NT; ++k) {
-        const float* Lkk = reinterpret_cast<const float*>(factor + hoff[static_cast<size_t>(k) * NT + k]);
-        float* Bk = B + static_cast<int64_t>(k) * nb * ldb;
-        rc = launch(CAT_POTRS, potrs_diag_kernel<NRHS>, dim3(kDiagCluster), dim3(kDiagThreads), smem_d, st, nb, Lkk,
-                    dinv + k * nsub * blk_elems, dinvT + k * nsub * blk_elems, Bk, ldb, nrhs, 0);
+    if (pipe) {
+        rc = g_pipe.init();
         if (rc) return rc;
-        if (k + 1 < NT) {
-            const int64_t tasks = static_cast<int64_t>(NT - k - 1) * nb / ROWS;
-            const int64_t want = (tasks + NW - 1) / NW;
-            const int grid = static_cast<int>(want < 3LL * num_sms ? want : 3LL * num_sms);
-            rc = launch(CAT_POTRS, potrs_fwd_update_kernel<NRHS>, dim3(grid), dim3(kSolveThreads), smem_z, st, NT, nb, k,
-                        factor, off, d_map, d_scales, B, ldb, nrhs);
-            if (rc) return rc;
-        }
+        sh = g_pipe.hi; sl = g_pipe.lo;
+        KRR_CUDA_CHECK(cudaEventRecord(g_pipe.event(EV_FORK), st));
+        KRR_CUDA_CHECK(cudaStreamWaitEvent(sh, g_pipe.event(EV_FORK), 0));
+        KRR_CUDA_CHECK(cudaStreamWaitEvent(sl, g_pipe.event(EV_FORK), 0));
     }
-    for (int k = NT - 1; k >= 0; --k) {
+    // bulk updates leave room for a diagonal-solve CTA on every SM (1 update CTA + 1 solve CTA fit in shared memory;
+    // the update CTAs are persistent, so a solve CTA that does not fit beside them would wait for the whole kernel)
+    const int bulk_per_sm = pipe ? 1 : 3;
+    auto fwd_update = [&](int k, int i_lo, int i_hi, cudaStream_t s, int per_sm) {
+        if (i_hi <= i_lo) return static_cast<int>(KRR_OK);
+        const int64_t tasks = static_cast<int64_t>(i_hi - i_lo) * nb / ROWS;
+        const int64_t want = (tasks + NW - 1) / NW;
+        const int64_t cap = static_cast<int64_t>(per_sm) * num_sms;
+        return launch(CAT_POTRS, potrs_fwd_update_kernel<NRHS>, dim3(static_cast<unsigned>(want < cap ? want : cap)), dim3(kSolveThreads),
+                      smem_z, s, NT, nb, k, i_lo, i_hi, factor, off, d_map, d_scales, B, ldb, nrhs);
+    };
+    auto bwd_update = [&](int k, int j_lo, int j_hi, cudaStream_t s) {
+        if (j_hi <= j_lo) return static_cast<int>(KRR_OK);
+        return launch(CAT_POTRS, potrs_bwd_update_kernel<NRHS>, dim3((j_hi - j_lo) * (nb / (32 * CPL))), dim3(kSolveThreads), smem_bu, s,
+                      NT, nb, k, j_lo, factor, off, d_map, d_scales, B, ldb, nrhs);
+    };
+    auto diag = [&](int k, int backward, cudaStream_t s) {
         const float* Lkk = reinterpret_cast<const float*>(factor + hoff[static_cast<size_t>(k) * NT + k]);
         float* Bk = B + static_cast<int64_t>(k) * nb * ldb;
-        rc = launch(CAT_POTRS, potrs_diag_kernel<NRHS>, dim3(kDiagCluster), dim3(kDiagThreads), smem_d, st, nb, Lkk,
-                    dinv + k * nsub * blk_elems, dinvT + k * nsub * blk_elems, Bk, ldb, nrhs, 1);
+        return launch(CAT_POTRS, potrs_diag_kernel<NRHS>, dim3(kDiagCluster), dim3(kDiagThreads), smem_d, s, nb, Lkk,
+                      dinv + k * nsub * blk_elems, dinvT + k * nsub * blk_elems, Bk, ldb, nrhs, backward);
+    };
+    // ---- forward: L z = y
+    for (int k = 0; k < NT; ++k) {
+        rc = diag(k, 0, sh);
         if (rc) return rc;
-        if (k > 0) {
-            rc = launch(CAT_POTRS, potrs_bwd_update_kernel<NRHS>, dim3(k * (nb / (32 * CPL))), dim3(kSolveThreads), smem_bu, st,
-                        NT, nb, k, factor, off, d_map, d_scales, B, ldb, nrhs);
+        if (!pipe) {
+            rc = fwd_update(k, k + 1, NT, st, 3);
             if (rc) return rc;
+            continue;
         }
+        KRR_CUDA_CHECK(cudaEventRecord(ev_diag(k), sh));
+        if (k >= 1) KRR_CUDA_CHECK(cudaStreamWaitEvent(sh, ev_bulk(k - 1), 0));      // row k+1 received column k-1 first
+        rc = fwd_update(k, k + 1, k + 2 < NT ? k + 2 : NT, sh, 3);                   // the next diagonal solve's rows
+        if (rc) return rc;
+        KRR_CUDA_CHECK(cudaStreamWaitEvent(sl, ev_diag(k), 0));
+        rc = fwd_update(k, k + 2, NT, sl, bulk_per_sm);
+        if (rc) return rc;
+        KRR_CUDA_CHECK(cudaEventRecord(ev_bulk(k), sl));
+    }
+    if (pipe) {      // the backward sweep starts from a quiescent state
+        KRR_CUDA_CHECK(cudaEventRecord(ev_bulk(NT), sl));
+        KRR_CUDA_CHECK(cudaStreamWaitEvent(sh, ev_bulk(NT), 0));
+    }
+    // ---- backward: L^T alpha = z
+    for (int k = NT - 1; k >= 0; --k) {
+        rc = diag(k, 1, sh);
+        if (rc) return rc;
+        if (!pipe) {
+            rc = bwd_update(k, 0, k, st);
+            if (rc) return rc;
+            continue;
+        }
+        KRR_CUDA_CHECK(cudaEventRecord(ev_diag(k), sh));
+        if (k + 1 < NT) KRR_CUDA_CHECK(cudaStreamWaitEvent(sh, ev_bulk(k + 1), 0));  // row k-1 received column k+1 first
+        rc = bwd_update(k, k - 1 > 0 ? k - 1 : 0, k, sh);                            // the next diagonal solve's rows
+        if (rc) return rc;
+        KRR_CUDA_CHECK(cudaStreamWaitEvent(sl, ev_diag(k), 0));
+        rc = bwd_update(k, 0, k - 1, sl);
+        if (rc) return rc;
+        KRR_CUDA_CHECK(cudaEventRecord(ev_bulk(k), sl));
+    }
+    if (pipe) {
+        KRR_CUDA_CHECK(cudaEventRecord(g_pipe.event(EV_JOIN_HI), sh));
+        KRR_CUDA_CHECK(cudaEventRecord(g_pipe.event(EV_JOIN_LO), sl));
+        KRR_CUDA_CHECK(cudaStreamWaitEvent(st, g_pipe.event(EV_JOIN_HI), 0));
+        KRR_CUDA_CHECK(cudaStreamWaitEvent(st, g_pipe.event(EV_JOIN_LO), 0));
     }
     return KRR_OK;
 }

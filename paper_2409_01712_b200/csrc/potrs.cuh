@@ -91,11 +91,11 @@ __device__ __forceinline__ void rows_dot_f32(const float* __restrict__ rows, int
 }
 
 // ---------------------------------------------------------------------------------------------
-// Forward update after Z_k is known:  Y_i -= L_ik Z_k  for all i > k.
+// Forward update after Z_k is known:  Y_i -= L_ik Z_k  for the tile rows i in [i_lo, i_hi)  (all > k).
 // Persistent CTAs over groups of 8 * ROWS rows (ROWS = 64 / NRHS rows per warp); smem = NRHS*nb floats.
 template <int NRHS>
 __global__ void __launch_bounds__(kSolveThreads)
-potrs_fwd_update_kernel(int NT, int nb, int k, const uint8_t* __restrict__ factor,
+potrs_fwd_update_kernel(int NT, int nb, int k, int i_lo, int i_hi, const uint8_t* __restrict__ factor,
                         const int64_t* __restrict__ off, const uint8_t* __restrict__ map,
                         const float* __restrict__ scales, float* __restrict__ B, int64_t ldb, int nrhs) {
     constexpr int ROWS = 64 / NRHS;
@@ -108,10 +108,10 @@ potrs_fwd_update_kernel(int NT, int nb, int k, const uint8_t* __restrict__ facto
     }
     __syncthreads();
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int64_t ngroups = static_cast<int64_t>(NT - k - 1) * nb / ROWS;   // warp tasks
+    const int64_t ngroups = static_cast<int64_t>(i_hi - i_lo) * nb / ROWS;   // warp tasks
     for (int64_t g = static_cast<int64_t>(blockIdx.x) * NW + warp; g < ngroups; g += static_cast<int64_t>(gridDim.x) * NW) {
-        const int64_t prow = g * ROWS;                                      // row below tile k
-        const int i = k + 1 + static_cast<int>(prow / nb);
+        const int64_t prow = g * ROWS;                                      // row below the top of tile i_lo
+        const int i = i_lo + static_cast<int>(prow / nb);
         const int r0 = static_cast<int>(prow % nb);
         const int p = map[i * NT + k];
         const float s = scales[i * NT + k];
@@ -145,13 +145,13 @@ potrs_fwd_update_kernel(int NT, int nb, int k, const uint8_t* __restrict__ facto
     }
 }
 
-// Backward update after alpha_k is known:  Z_j -= L_kj^T alpha_k  for all j < k.
-// One CTA per (tile j, strip of 32*CPL columns); warps split the nb rows (interleaved), lanes own
+// Backward update after alpha_k is known:  Z_j -= L_kj^T alpha_k  for the tiles j in [j_lo, j_lo + gridDim.x / strips)
+// (all < k).  One CTA per (tile j, strip of 32*CPL columns); warps split the nb rows (interleaved), lanes own
 // CPL consecutive columns; the per-warp partial sums are combined through shared memory in a fixed
 // tree order.  smem = nb*NRHS floats (alpha_k) + (NW/2) * 32*CPL*NRHS floats.
 template <int NRHS>
 __global__ void __launch_bounds__(kSolveThreads)
-potrs_bwd_update_kernel(int NT, int nb, int k, const uint8_t* __restrict__ factor,
+potrs_bwd_update_kernel(int NT, int nb, int k, int j_lo, const uint8_t* __restrict__ factor,
                         const int64_t* __restrict__ off, const uint8_t* __restrict__ map,
                         const float* __restrict__ scales, float* __restrict__ B, int64_t ldb, int nrhs) {
     constexpr int CPL = (NRHS <= 16) ? 4 : 2;
@@ -168,7 +168,7 @@ potrs_bwd_update_kernel(int NT, int nb, int k, const uint8_t* __restrict__ facto
     __syncthreads();
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int strips = nb / STRIP;
-    const int j = blockIdx.x / strips;
+    const int j = j_lo + blockIdx.x / strips;
     const int c0 = (blockIdx.x % strips) * STRIP + lane * CPL;
     const int p = map[k * NT + j];
     const float s = scales[k * NT + j];

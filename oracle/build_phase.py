@@ -88,3 +88,21 @@ def pearson(Y, Yhat):
     hc = Yhat - Yhat.mean(axis=0)
     return np.sum(yc * hc, axis=0) / np.sqrt(np.sum(yc * yc, axis=0) * np.sum(hc * hc, axis=0))
 
+
+# ---- IBS kernel (Alg. 5 l.5-6; definition in the text of PAPER.md:134) ----
+def ibs_kernel_matrix_definition(G1, G2):
+    """K_ij = (p_i ~ p_j) / (total number of alleles): "counting the number of alleles individuals p_i and p_j share
+    that are identical by state at a given SNP locus over the total number of alleles".  Genotypes are
+    minor-allele counts in {0, 1, 2}; two genotypes a, b share 2 - |a - b| of their 2 alleles by state, counted here
+    locus by locus.  Reading (R17): the divisor is the number of alleles, 2 N_S, so that K_ii = 1; Alg. 5 l.6
+    prints N_S."""
+    G1 = np.asarray(G1, dtype=np.int64)
+    G2 = np.asarray(G2, dtype=np.int64)
+    assert G1.min() >= 0 and G1.max() <= 2 and G2.min() >= 0 and G2.max() <= 2
+    ns = G1.shape[1]
+    K = np.empty((G1.shape[0], G2.shape[0]), dtype=np.float64)
+    for i in range(G1.shape[0]):
+        shared = 2 - np.abs(G2 - G1[i][None, :])          # alleles shared IBS at every locus
+        K[i] = shared.sum(axis=1) / (2.0 * ns)
+    return K
+

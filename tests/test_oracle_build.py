@@ -133,3 +133,33 @@ def test_confounder_term_closed_forms():
     T, CT = G[:7], C[:7] + 0.5
     Kx = cross_kernel_matrix_definition(T, G, gamma, CT, C)
     assert abs(Kx[2, 9] - np.exp(-gamma * (np.sum((T[2].astype(int) - G[9].astype(int)) ** 2) + np.sum((CT[2] - C[9]) ** 2)))) < 1e-15
+
+
+def test_ibs_kernel_pins():
+    """IBS (Alg. 5 l.5-6): the allele-sharing count by an explicit haplotype model, closed forms, and the identity the
+    CUDA path uses (thermometer encoding: the Hamming distance of the encoded rows is sum_k |a_k - b_k|)."""
+    from oracle.build_phase import ibs_kernel_matrix_definition
+    # per-locus table by brute force over unordered allele pairs: genotype g = number of minor alleles among 2;
+    # alleles shared by state = size of the multiset intersection
+    def shared(a, b):
+        A, Bm = ["m"] * a + ["M"] * (2 - a), ["m"] * b + ["M"] * (2 - b)
+        return min(A.count("m"), Bm.count("m")) + min(A.count("M"), Bm.count("M"))
+    for a in range(3):
+        for b in range(3):
+            K = ibs_kernel_matrix_definition(np.array([[a]]), np.array([[b]]))
+            assert K[0, 0] == shared(a, b) / 2.0
+    rng = np.random.default_rng(6)
+    G = rng.integers(0, 3, size=(30, 77)).astype(np.int8)
+    K = ibs_kernel_matrix_definition(G, G)
+    assert np.array_equal(K, K.T) and np.all(np.diag(K) == 1.0) and K.min() >= 0.0
+    # opposite homozygotes everywhere share nothing; a heterozygote shares one allele with anybody
+    assert ibs_kernel_matrix_definition(np.zeros((1, 9), int), 2 * np.ones((1, 9), int))[0, 0] == 0.0
+    assert ibs_kernel_matrix_definition(np.ones((1, 9), int), rng.integers(0, 3, size=(1, 9)) * 2 % 3)[0, 0] >= 0.5
+    # thermometer encoding u = ([g >= 1], [g >= 2]): Hamming distance of the encodings = sum |a - b|
+    U = np.concatenate([(G >= 1), (G >= 2)], axis=1).astype(np.int64)
+    ham = squared_distances(U, U)                                       # 0/1 entries: squared distance = Hamming
+    assert np.array_equal(ham, np.abs(G[:, None, :].astype(int) - G[None, :, :].astype(int)).sum(axis=2))
+    assert np.allclose(K, 1.0 - ham / (2.0 * 77), rtol=0, atol=1e-15)
+    # positive semi-definite (a sum of per-locus PSD kernels)
+    assert np.linalg.eigvalsh(K).min() > -1e-10
+

@@ -76,6 +76,13 @@ typedef enum { KRR_FP32 = 0, KRR_FP16 = 1, KRR_FP8_E4M3 = 2 } krr_prec_t;
                                        128 dependent pivots of each block, not by launches), kept as the
                                        persistent-kernel variant and as a cross-check.                 */
 
+#define KRR_FLAG_KERNEL_IBS    256u  /* krr_build, krr_predict: the identical-by-state kernel of Alg. 5 l.5-6 (PAPER.md:134,
+                                       :141) instead of the Gaussian one: K_ij = (alleles of i and j identical
+                                       by state, 2 - |g_ik - g_jk| per locus for genotypes in {0,1,2}) / (2 N_S).
+                                       Same tensor-core kernel on thermometer-encoded genotypes ([g>=1],[g>=2]:
+                                       their Hamming distance is sum_k |g_ik - g_jk|); gamma is ignored and
+                                       confounders are not accepted.                                  */
+
 /* Library version (major*100 + minor) and the compute capability it was built for (100). */
 int krr_version(void);
 int krr_built_for_sm(void);
@@ -210,9 +217,10 @@ int krr_associate_host(const float* h_A, int64_t n, int64_t lda, int nb,
  *             packed lower tiles with KRR_FLAG_A_TILED_LOWER -- the two input layouts of krr_precision_map
  *             and krr_potrf_mp.  exp is evaluated in FP32 (expf of the FP32 product gamma*d2, d2 exact):
  *             entries agree with the FP64-evaluated, FP32-rounded kernel to a few ulp.
- * n % 256 == 0, nb % 256 == 0, n % nb == 0.  d_ws: krr_build_workspace(n) bytes (the folded vector s).
+ * n % 256 == 0, nb % 256 == 0, n % nb == 0.  d_ws: krr_build_workspace(n, p, flags) bytes (the folded vector s;
+ * with KRR_FLAG_KERNEL_IBS also the encoded genotypes, n x 2p bytes).
  */
-size_t krr_build_workspace(int64_t n);
+size_t krr_build_workspace(int64_t n, int64_t p, unsigned flags);
 int krr_build(const int8_t* d_G, int64_t n, int64_t p, int64_t ldg, const float* d_C, int q, int64_t ldc,
               float gamma, float lambda, float* d_A, int64_t lda, int nb, unsigned flags,
               void* d_ws, size_t ws_bytes, void* stream);
@@ -229,14 +237,15 @@ int krr_build(const int8_t* d_G, int64_t n, int64_t p, int64_t ldg, const float*
  * d_CT, d_CG  in  optional confounders of the two cohorts (m x q, n x q FP32, ldct / ldcg), as for krr_build.
  * d_W  in  n x nrhs FP32 row-major (ldw): the weights of krr_potrs; nrhs <= 32.
  * d_P  out m x nrhs FP32 row-major (ldp): the predicted phenotypes.
- * d_ws     krr_predict_workspace(m, n) bytes, 1024-byte aligned; on return it holds, after the two
+ * flags    0 or KRR_FLAG_KERNEL_IBS.
+ * d_ws     krr_predict_workspace(m, n, p, flags) bytes, 1024-byte aligned; on return it holds, after the two
  *          folded norm vectors (each rounded up to 1 KiB), K as m x n FP32 row-major.
  */
-size_t krr_predict_workspace(int64_t m, int64_t n);
+size_t krr_predict_workspace(int64_t m, int64_t n, int64_t p, unsigned flags);
 int krr_predict(const int8_t* d_T, int64_t m, int64_t ldt, const int8_t* d_G, int64_t n, int64_t ldg, int64_t p,
                 const float* d_CT, int64_t ldct, const float* d_CG, int64_t ldcg, int q,
                 float gamma, const float* d_W, int64_t ldw, int nrhs, float* d_P, int64_t ldp,
-                void* d_ws, size_t ws_bytes, void* stream);
+                unsigned flags, void* d_ws, size_t ws_bytes, void* stream);
 
 /* Number of kernels the last krr_* call on this thread enqueued (for bench.py's gpu_launches). */
 int64_t krr_last_launch_count(void);

@@ -12,6 +12,7 @@ FLAG_NO_LOOKAHEAD = 8
 FLAG_FP8_VIA_FP16 = 16
 FLAG_NO_CTA_PAIRS = 32
 FLAG_FUSED_CHAIN = 64
+FLAG_KERNEL_IBS = 256
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB = None
@@ -73,14 +74,14 @@ def lib():
     L.krr_associate_host.argtypes = [vp, i64, i64, c.c_int, c.c_float, u32, c.c_int, u32, vp, c.c_int, vp,
                                      vp, vp, vp, sz, vp]
     L.krr_build_workspace.restype = sz
-    L.krr_build_workspace.argtypes = [i64]
+    L.krr_build_workspace.argtypes = [i64, i64, u32]
     L.krr_build.restype = c.c_int
     L.krr_build.argtypes = [vp, i64, i64, i64, vp, c.c_int, i64, c.c_float, c.c_float, vp, i64, c.c_int, u32, vp, sz, vp]
     L.krr_predict_workspace.restype = sz
-    L.krr_predict_workspace.argtypes = [i64, i64]
+    L.krr_predict_workspace.argtypes = [i64, i64, i64, u32]
     L.krr_predict.restype = c.c_int
     L.krr_predict.argtypes = [vp, i64, i64, vp, i64, i64, i64, vp, i64, vp, i64, c.c_int, c.c_float, vp, i64, c.c_int, vp, i64,
-                              vp, sz, vp]
+                              u32, vp, sz, vp]
     L.krr_last_launch_count.restype = i64
     L.krr_profile_enable.restype = c.c_int
     L.krr_profile_enable.argtypes = [u32]
@@ -305,11 +306,11 @@ def krr_build(G, gamma, lam, nb, tiled_lower=False, out=None, flags=0, C=None):
     if out is None:
         out = (torch.zeros(NT * (NT + 1) // 2 * nb * nb, dtype=torch.float32, device=dev) if tiled_lower
                else torch.zeros((n, n), dtype=torch.float32, device=dev))
-    wsb = int(L.krr_build_workspace(n))
+    flags |= FLAG_A_TILED_LOWER if tiled_lower else 0
+    wsb = int(L.krr_build_workspace(n, p, flags))
     if wsb == 0:
         raise KrrError("krr_build_workspace: n must be a multiple of 256")
     ws = _ws(wsb, dev)
-    flags |= FLAG_A_TILED_LOWER if tiled_lower else 0
     lda = nb if tiled_lower else out.stride(0)
     C, q, ldc = _conf(C)
     _check(L.krr_build(_ptr(G), n, p, G.stride(0), _ptr(C), q, ldc, float(gamma), float(lam), _ptr(out), lda, nb, flags,
@@ -317,7 +318,7 @@ def krr_build(G, gamma, lam, nb, tiled_lower=False, out=None, flags=0, C=None):
     return out
 
 
-def krr_predict(T, G, gamma, W, return_kernel=False, CT=None, CG=None):
+def krr_predict(T, G, gamma, W, return_kernel=False, CT=None, CG=None, flags=0):
     """krr_predict: P_r = K(T, G) W (Alg. 4).  T (m x p), G (n x p): CUDA int8, row pitch a multiple of 16 bytes;
     W: CUDA FP32 n x nrhs.  Returns P (m x nrhs) and, on request, the test-training kernel matrix (a view
     into the call's workspace)."""
@@ -327,7 +328,7 @@ def krr_predict(T, G, gamma, W, return_kernel=False, CT=None, CG=None):
     m, p = T.shape
     n = G.shape[0]
     nrhs = W.shape[1]
-    wsb = int(L.krr_predict_workspace(m, n))
+    wsb = int(L.krr_predict_workspace(m, n, p, flags))
     if wsb == 0:
         raise KrrError("krr_predict_workspace: m and n must be multiples of 256")
     ws = _ws(wsb, G.device)
@@ -336,7 +337,7 @@ def krr_predict(T, G, gamma, W, return_kernel=False, CT=None, CG=None):
     CG, q2, ldcg = _conf(CG)
     assert q == q2
     _check(L.krr_predict(_ptr(T), m, T.stride(0), _ptr(G), n, G.stride(0), p, _ptr(CT), ldct, _ptr(CG), ldcg, q, float(gamma),
-                         _ptr(W), W.stride(0), nrhs, _ptr(P), P.stride(0), _ptr(ws), wsb, _stream()), "krr_predict")
+                         _ptr(W), W.stride(0), nrhs, _ptr(P), P.stride(0), flags, _ptr(ws), wsb, _stream()), "krr_predict")
     if not return_kernel:
         return P
     off = (m * 4 + 1023) // 1024 * 1024 + (n * 4 + 1023) // 1024 * 1024

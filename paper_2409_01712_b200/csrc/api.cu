@@ -866,9 +866,13 @@ int launch_build(const CUtensorMap& tmR, const CUtensorMap& tmG, const BuildOp& 
 
 extern "C" {
 
-size_t krr_build_workspace(int64_t n) {
-    if (n <= 0 || n % 256 != 0) return 0;
-    return align_up(static_cast<size_t>(n) * sizeof(int), 1024);           // the folded squared norms
+static size_t ibs_pitch(int64_t p) { return align_up(static_cast<size_t>(2 * p), 16); }
+
+size_t krr_build_workspace(int64_t n, int64_t p, unsigned flags) {
+    if (n <= 0 || n % 256 != 0 || p < 1) return 0;
+    size_t b = align_up(static_cast<size_t>(n) * sizeof(int), 1024);       // the folded squared norms
+    if (flags & KRR_FLAG_KERNEL_IBS) b += align_up(static_cast<size_t>(n) * ibs_pitch(p), 1024);   // encoded genotypes
+    return b;
 }
 
 int krr_build(const int8_t* d_G, int64_t n, int64_t p, int64_t ldg, const float* d_C, int q, int64_t ldc, float gamma,
@@ -881,17 +885,27 @@ int krr_build(const int8_t* d_G, int64_t n, int64_t p, int64_t ldg, const float*
     if (n % 256 != 0 || nb % 256 != 0) return KRR_ERR_SHAPE;
     if (p < 1 || p > 133000 || ldg < p || ldg % 16 != 0) return KRR_ERR_ARG;      // INT32 sums of int8 squares stay exact
     const bool tiled = flags & KRR_FLAG_A_TILED_LOWER;
-    if (flags & ~KRR_FLAG_A_TILED_LOWER) return KRR_ERR_UNSUPPORTED;
+    const bool ibs = flags & KRR_FLAG_KERNEL_IBS;
+    if (flags & ~(KRR_FLAG_A_TILED_LOWER | KRR_FLAG_KERNEL_IBS)) return KRR_ERR_UNSUPPORTED;
+    if (ibs && q > 0) return KRR_ERR_UNSUPPORTED;                                  // confounders belong to the Gaussian kernel
     if (!tiled && (lda < n || lda % 4 != 0)) return KRR_ERR_ARG;
     if (reinterpret_cast<uintptr_t>(d_G) % 16 != 0 || reinterpret_cast<uintptr_t>(d_A) % 16 != 0 ||
         reinterpret_cast<uintptr_t>(d_ws) % 16 != 0)
         return KRR_ERR_ARG;
-    if (ws_bytes < krr_build_workspace(n)) return KRR_ERR_WORKSPACE;
+    if (ws_bytes < krr_build_workspace(n, p, flags)) return KRR_ERR_WORKSPACE;
     int num_sms = 0;
     rc = check_device(&num_sms);
     if (rc) return rc;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     int* sq = static_cast<int*>(d_ws);
+    if (ibs) {      // thermometer-encode, then the same kernel on the encoded matrix (2p columns of 0/1)
+        int8_t* U = reinterpret_cast<int8_t*>(static_cast<uint8_t*>(d_ws) + align_up(static_cast<size_t>(n) * sizeof(int), 1024));
+        const int64_t ldu = static_cast<int64_t>(ibs_pitch(p));
+        rc = launch(CAT_MISC, ibs_encode_kernel, dim3(static_cast<unsigned>((ldu + 255) / 256 < 64 ? (ldu + 255) / 256 : 64), static_cast<unsigned>(n)),
+                    dim3(256), 0, st, d_G, n, p, ldg, U, ldu);
+        if (rc) return rc;
+        d_G = U; ldg = ldu; p = 2 * p;
+    }
     rc = launch(CAT_MISC, row_sqnorm_kernel, dim3(static_cast<unsigned>((n + 7) / 8)), dim3(256), 0, st, d_G, n, p, ldg, sq);
     if (rc) return rc;
     CUtensorMap tmG;
@@ -899,6 +913,7 @@ int krr_build(const int8_t* d_G, int64_t n, int64_t p, int64_t ldg, const float*
     if (rc) return rc;
     BuildOp op;
     memset(&op, 0, sizeof(op));
+    op.ibs = ibs ? 1 : 0; op.alleles = static_cast<float>(p);        // (p was doubled above: 2 N_S alleles)
     op.n = n; op.m = n; op.rect = 0; op.p = p; op.nb = nb; op.tiled = tiled ? 1 : 0; op.gamma = gamma;
     op.diag = static_cast<float>(1.0 + static_cast<double>(lambda));
     op.sq = sq; op.sq_row = sq; op.A = d_A; op.lda = lda;
@@ -909,17 +924,23 @@ int krr_build(const int8_t* d_G, int64_t n, int64_t p, int64_t ldg, const float*
 }
 
 // ------------------------------------------------------------------------- Predict phase (NEXT-2)
-size_t krr_predict_workspace(int64_t m, int64_t n) {
-    if (m <= 0 || n <= 0 || m % 256 != 0 || n % 256 != 0) return 0;
-    return align_up(static_cast<size_t>(m) * sizeof(int), 1024) + align_up(static_cast<size_t>(n) * sizeof(int), 1024) +
-           align_up(static_cast<size_t>(m) * n * sizeof(float), 1024);
+size_t krr_predict_workspace(int64_t m, int64_t n, int64_t p, unsigned flags) {
+    if (m <= 0 || n <= 0 || m % 256 != 0 || n % 256 != 0 || p < 1) return 0;
+    size_t b = align_up(static_cast<size_t>(m) * sizeof(int), 1024) + align_up(static_cast<size_t>(n) * sizeof(int), 1024) +
+               align_up(static_cast<size_t>(m) * n * sizeof(float), 1024);
+    if (flags & KRR_FLAG_KERNEL_IBS) b += align_up(static_cast<size_t>(m + n) * ibs_pitch(p), 1024);
+    return b;
 }
 
 int krr_predict(const int8_t* d_T, int64_t m, int64_t ldt, const int8_t* d_G, int64_t n, int64_t ldg, int64_t p,
                 const float* d_CT, int64_t ldct, const float* d_CG, int64_t ldcg, int q, float gamma,
-                const float* d_W, int64_t ldw, int nrhs, float* d_P, int64_t ldp, void* d_ws, size_t ws_bytes, void* stream) {
+                const float* d_W, int64_t ldw, int nrhs, float* d_P, int64_t ldp, unsigned flags, void* d_ws, size_t ws_bytes,
+                void* stream) {
     g_launches = 0;
     if (!d_T || !d_G || !d_W || !d_P || !d_ws) return KRR_ERR_ARG;
+    const bool ibs = flags & KRR_FLAG_KERNEL_IBS;
+    if (flags & ~KRR_FLAG_KERNEL_IBS) return KRR_ERR_UNSUPPORTED;
+    if (ibs && q > 0) return KRR_ERR_UNSUPPORTED;
     if (q < 0 || q > kMaxConfounders || (q > 0 && (!d_CT || !d_CG || ldct < q || ldcg < q))) return KRR_ERR_ARG;
     if (m <= 0 || n <= 0 || m % 256 != 0 || n % 256 != 0) return KRR_ERR_SHAPE;
     if (p < 1 || p > 133000 || ldg < p || ldg % 16 != 0 || ldt < p || ldt % 16 != 0) return KRR_ERR_ARG;
@@ -927,7 +948,7 @@ int krr_predict(const int8_t* d_T, int64_t m, int64_t ldt, const int8_t* d_G, in
     if (reinterpret_cast<uintptr_t>(d_G) % 16 != 0 || reinterpret_cast<uintptr_t>(d_T) % 16 != 0 ||
         reinterpret_cast<uintptr_t>(d_ws) % 1024 != 0)
         return KRR_ERR_ARG;
-    if (ws_bytes < krr_predict_workspace(m, n)) return KRR_ERR_WORKSPACE;
+    if (ws_bytes < krr_predict_workspace(m, n, p, flags)) return KRR_ERR_WORKSPACE;
     int num_sms = 0;
     int rc = check_device(&num_sms);
     if (rc) return rc;
@@ -936,6 +957,17 @@ int krr_predict(const int8_t* d_T, int64_t m, int64_t ldt, const int8_t* d_G, in
     int* sqT = reinterpret_cast<int*>(ws);
     int* sqG = reinterpret_cast<int*>(ws + align_up(static_cast<size_t>(m) * sizeof(int), 1024));
     float* K = reinterpret_cast<float*>(reinterpret_cast<uint8_t*>(sqG) + align_up(static_cast<size_t>(n) * sizeof(int), 1024));
+    if (ibs) {
+        int8_t* UT = reinterpret_cast<int8_t*>(reinterpret_cast<uint8_t*>(K) + align_up(static_cast<size_t>(m) * n * sizeof(float), 1024));
+        const int64_t ldu = static_cast<int64_t>(ibs_pitch(p));
+        int8_t* UG = UT + m * ldu;
+        const unsigned gx = static_cast<unsigned>((ldu + 255) / 256 < 64 ? (ldu + 255) / 256 : 64);
+        rc = launch(CAT_MISC, ibs_encode_kernel, dim3(gx, static_cast<unsigned>(m)), dim3(256), 0, st, d_T, m, p, ldt, UT, ldu);
+        if (rc) return rc;
+        rc = launch(CAT_MISC, ibs_encode_kernel, dim3(gx, static_cast<unsigned>(n)), dim3(256), 0, st, d_G, n, p, ldg, UG, ldu);
+        if (rc) return rc;
+        d_T = UT; d_G = UG; ldt = ldg = ldu; p = 2 * p;
+    }
     rc = launch(CAT_MISC, row_sqnorm_kernel, dim3(static_cast<unsigned>((m + 7) / 8)), dim3(256), 0, st, d_T, m, p, ldt, sqT);
     if (rc) return rc;
     rc = launch(CAT_MISC, row_sqnorm_kernel, dim3(static_cast<unsigned>((n + 7) / 8)), dim3(256), 0, st, d_G, n, p, ldg, sqG);
@@ -944,6 +976,7 @@ int krr_predict(const int8_t* d_T, int64_t m, int64_t ldt, const int8_t* d_G, in
     if (make_genotype_tmap(&tmT, d_T, m, p, ldt) || make_genotype_tmap(&tmG, d_G, n, p, ldg)) return KRR_ERR_CUDA;
     BuildOp op;
     memset(&op, 0, sizeof(op));
+    op.ibs = ibs ? 1 : 0; op.alleles = static_cast<float>(p);
     op.n = n; op.m = m; op.rect = 1; op.p = p; op.nb = 256; op.tiled = 0; op.gamma = gamma; op.diag = 1.0f;
     op.sq = sqG; op.sq_row = sqT; op.A = K; op.lda = n;
     op.C = d_CG; op.C_row = d_CT; op.ldc = ldcg; op.ldc_row = ldct; op.q = q;

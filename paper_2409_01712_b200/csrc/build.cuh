@@ -35,6 +35,10 @@ struct BuildOp {
     const float* C_row;     // row operand's (= C for the symmetric Build)
     int64_t ldc, ldc_row;
     int q;
+    // IBS kernel (Alg. 5 l.5-6): the operands are thermometer encodings ([g >= 1], [g >= 2]) of the genotypes, d2 is then
+    // the Hamming distance sum_k |g_ik - g_jk| and K_ij = (alleles - d2) / alleles, alleles = 2 N_S (no exponential)
+    int ibs;
+    float alleles;
 };
 constexpr int kMaxConfounders = 16;
 
@@ -67,6 +71,22 @@ row_sqnorm_kernel(const int8_t* __restrict__ G, int64_t n, int64_t p, int64_t ld
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
     if (lane == 0) sq[row] = acc;
+}
+
+// Thermometer encoding for the IBS kernel: U[i][k] = [g_ik >= 1], U[i][p + k] = [g_ik >= 2] (int8 0/1, row pitch ldu);
+// columns p2 .. ldu-1 are zeroed so that the encoded matrix can be read in whole 16-byte units.
+__global__ void __launch_bounds__(256)
+ibs_encode_kernel(const int8_t* __restrict__ G, int64_t n, int64_t p, int64_t ldg, int8_t* __restrict__ U, int64_t ldu) {
+    const int64_t row = blockIdx.y;
+    const int8_t* g = G + row * ldg;
+    int8_t* u = U + row * ldu;
+    for (int64_t k = static_cast<int64_t>(blockIdx.x) * 256 + threadIdx.x; k < ldu; k += static_cast<int64_t>(gridDim.x) * 256) {
+        int8_t v = 0;
+        if (k < p) v = g[k] >= 1;
+        else if (k < 2 * p) v = g[k - p] >= 2;
+        u[k] = v;
+    }
+    (void)n;
 }
 
 // 256 x 256 blocks (units) of the lower tiles: unit (ru, cu) is wanted when the tile of its rows is at or below
@@ -267,7 +287,8 @@ build_tc_kernel(const __grid_constant__ CUtensorMap tmR, const __grid_constant__
                                 if (c < op.q) { const float t = ci[c] - __ldg(cj + c); dc = fmaf(t, t, dc); }
                             d2f += dc;
                         }
-                        v[u] = (!op.rect && gj0 + e + u == gi) ? op.diag : expf(-op.gamma * d2f);
+                        const float kv = op.ibs ? __fdiv_rn(op.alleles - d2f, op.alleles) : expf(-op.gamma * d2f);
+                        v[u] = (!op.rect && gj0 + e + u == gi) ? op.diag : kv;
                     }
                     *reinterpret_cast<float4*>(dst + e) = make_float4(v[0], v[1], v[2], v[3]);
                 }

@@ -109,9 +109,9 @@ def test_build_argument_errors(krr):
     import ctypes
     G = torch.zeros((512, 160), dtype=torch.int8, device="cuda")
     A = torch.zeros((512, 512), dtype=torch.float32, device="cuda")
-    ws = torch.zeros(4096, dtype=torch.uint8, device="cuda")
+    ws = torch.zeros(1 << 20, dtype=torch.uint8, device="cuda")
     vp = lambda t: ctypes.c_void_p(t.data_ptr())
-    call = lambda n, p, ldg, nb, flags=0: L.krr_build(vp(G), n, p, ldg, None, 0, 0, 0.01, 0.01, vp(A), 512, nb, flags, vp(ws), 4096, None)
+    call = lambda n, p, ldg, nb, flags=0: L.krr_build(vp(G), n, p, ldg, None, 0, 0, 0.01, 0.01, vp(A), 512, nb, flags, vp(ws), 1 << 20, None)
     assert call(512, 160, 160, 256) == 0
     assert call(500, 160, 160, 250) == -2            # n, nb not multiples of 256
     assert call(512, 160, 150, 256) == -1            # ldg < p
@@ -211,3 +211,33 @@ def test_build_and_predict_with_confounders(krr, q):
     assert float(np.abs(Kw - cross_kernel_matrix_definition(T.cpu().numpy(), G.cpu().numpy(), gamma)).max()) > 1e-3   # the term matters
     Pw = Kw @ W.cpu().numpy().astype(np.float64)
     assert np.all(np.abs(P.cpu().numpy() - Pw) <= 6e-6 * (Kw @ np.abs(W.cpu().numpy().astype(np.float64))))
+
+
+@pytest.mark.parametrize("n,m,p,nb", [(512, 256, 300, 256), (1024, 512, 1111, 512)])
+def test_ibs_kernel_build_and_predict(krr, n, m, p, nb):
+    """Alg. 5 l.5-6: the IBS kernel through the same tensor-core kernel on thermometer-encoded genotypes.  The
+    allele counts are exact integers on both sides and the quotient by 2 N_S is one correctly rounded FP32 division
+    against the oracle's FP64 one: entries agree to half an FP32 ulp (double rounding aside: <= 1 ulp asserted)."""
+    from oracle.build_phase import ibs_kernel_matrix_definition
+    G = genotypes(51, n, p, "maf", device="cuda")
+    T = genotypes(52, m, p, "uniform", device="cuda")
+    lam = 0.05
+    A = krr.krr_build(padded(G), 0.0, lam, nb, flags=krr.FLAG_KERNEL_IBS)
+    W = torch.randn((n, 2), device="cuda", generator=torch.Generator(device="cuda").manual_seed(2))
+    P, K = krr.krr_predict(padded(T), padded(G), 0.0, W, return_kernel=True, flags=krr.FLAG_KERNEL_IBS)
+    torch.cuda.synchronize()
+    want = ibs_kernel_matrix_definition(G.cpu().numpy(), G.cpu().numpy())
+    got = A.cpu().numpy()
+    NT = n // nb
+    for i in range(NT):
+        for j in range(i + 1):
+            g, w = got[i * nb:(i + 1) * nb, j * nb:(j + 1) * nb].astype(np.float64), want[i * nb:(i + 1) * nb, j * nb:(j + 1) * nb].copy()
+            if i == j:
+                w[np.diag_indices(nb)] = np.float64(np.float32(1.0 + lam))
+            assert np.all(np.abs(g - w) <= 6e-8 * np.abs(w) + 1e-45), (i, j)
+    assert float(np.mean(got[np.tril_indices(n, -1)] == want[np.tril_indices(n, -1)].astype(np.float32))) > 0.99
+    Kw = ibs_kernel_matrix_definition(T.cpu().numpy(), G.cpu().numpy())
+    assert np.all(np.abs(K.cpu().numpy() - Kw) <= 6e-8 * Kw)
+    Pw = Kw @ W.cpu().numpy().astype(np.float64)
+    assert np.all(np.abs(P.cpu().numpy() - Pw) <= 4e-6 * (Kw @ np.abs(W.cpu().numpy().astype(np.float64))))
+

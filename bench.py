@@ -364,6 +364,29 @@ def run_build_phase(ctx, peaks, reps=3):
                           "finite": bool(torch.isfinite(P).all())}
     except Exception as ex:
         res["predict"] = {"error": repr(ex)}
+    # Alg. 1 l.2-3 end to end from HOST genotypes (krr_fit_host): n*p bytes cross PCIe instead of 4 n^2
+    try:
+        if cfg.map_request == "rule" and not cfg.lower_tiles_only:
+            torch.cuda.empty_cache()
+            hG = torch.empty((n, p), dtype=torch.int8, pin_memory=True)
+            hG.copy_(Gp[:, :p])
+            hY = Y.cpu().pin_memory()
+            del Gp, T
+            torch.cuda.empty_cache()
+            arena, tf = None, []
+            for it in range(2):
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record()
+                alpha, h_map, info, arena = krr.fit_host(hG, cfg.gamma, cfg.lam, nb, hY, cfg.eps_target, cfg.allowed, -1,
+                                                         krr.FLAG_PREROUND_A, arena, dev)
+                e1.record()
+                torch.cuda.synchronize()
+                tf.append(e0.elapsed_time(e1))
+            res["fit_from_host_genotypes"] = {"api": "krr_fit_host (pinned host G, Y -> alpha; Build on the device)", "ms": round(tf[-1], 3),
+                                              "cholesky_TOp/s": round(n ** 3 / 3.0 / (tf[-1] * 1e-3) / 1e12, 1),
+                                              "h2d_bytes": n * p + n * cfg.nrhs * 4, "info": info}
+    except Exception as ex:
+        res["fit_from_host_genotypes"] = {"error": repr(ex)}
     return res
 
 

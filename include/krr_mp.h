@@ -247,6 +247,21 @@ int krr_predict(const int8_t* d_T, int64_t m, int64_t ldt, const int8_t* d_G, in
                 float gamma, const float* d_W, int64_t ldw, int nrhs, float* d_P, int64_t ldp,
                 unsigned flags, void* d_ws, size_t ws_bytes, void* stream);
 
+/* ---------------------------------------------------------------------------------------------
+ * krr_fit_host -- Build and Associate (Alg. 1 l.2-3) from HOST buffers: copies the int8 genotypes
+ * and Y to the device, builds A = K + lambda*I there (krr_build, Gaussian kernel), then runs the Associate phase as
+ * krr_associate_host does and copies alpha (= W), the precision map and info back.  The n x n matrix never crosses
+ * PCIe: n*p bytes of genotypes do.  Synchronises `stream` before it returns.
+ * h_G  in  n x p int8 genotypes, row pitch ldg >= p bytes (pinned memory makes the copy asynchronous).
+ * Other arguments as for krr_build / krr_associate_host; n % 256 == 0, nb % 256 == 0.
+ * d_arena  krr_fit_host_arena(n, p, nb, nrhs) bytes, 1024-byte aligned.
+ */
+size_t krr_fit_host_arena(int64_t n, int64_t p, int nb, int nrhs);
+int krr_fit_host(const int8_t* h_G, int64_t n, int64_t p, int64_t ldg, float gamma, float lambda, int nb,
+                 float eps_target, unsigned allowed_mask, int force_prec, unsigned flags,
+                 const float* h_Y, int nrhs, float* h_alpha, uint8_t* h_map, int* h_info,
+                 void* d_arena, size_t arena_bytes, void* stream);
+
 /* Number of kernels the last krr_* call on this thread enqueued (for bench.py's gpu_launches). */
 int64_t krr_last_launch_count(void);
 

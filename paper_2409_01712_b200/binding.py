@@ -23,7 +23,7 @@ ERRORS = {-1: "KRR_ERR_ARG", -2: "KRR_ERR_SHAPE", -3: "KRR_ERR_WORKSPACE", -4: "
 EXPORTS = ["krr_version", "krr_built_for_sm", "krr_tile_slot", "krr_precision_map_workspace",
            "krr_precision_map", "krr_factor_bytes", "krr_factor_tile_offset",
            "krr_potrf_mp_workspace", "krr_potrf_mp", "krr_potrs_workspace", "krr_potrs",
-           "krr_associate_host_arena", "krr_associate_host", "krr_build_workspace", "krr_build", "krr_predict_workspace", "krr_predict",
+           "krr_associate_host_arena", "krr_associate_host", "krr_build_workspace", "krr_build", "krr_predict_workspace", "krr_predict", "krr_fit_host_arena", "krr_fit_host",
            "krr_last_launch_count",
            "krr_profile_enable", "krr_profile_read"]
 
@@ -82,6 +82,11 @@ def lib():
     L.krr_predict.restype = c.c_int
     L.krr_predict.argtypes = [vp, i64, i64, vp, i64, i64, i64, vp, i64, vp, i64, c.c_int, c.c_float, vp, i64, c.c_int, vp, i64,
                               u32, vp, sz, vp]
+    L.krr_fit_host_arena.restype = sz
+    L.krr_fit_host_arena.argtypes = [i64, i64, c.c_int, c.c_int]
+    L.krr_fit_host.restype = c.c_int
+    L.krr_fit_host.argtypes = [vp, i64, i64, i64, c.c_float, c.c_float, c.c_int, c.c_float, u32, c.c_int, u32, vp, c.c_int, vp,
+                               vp, vp, vp, sz, vp]
     L.krr_last_launch_count.restype = i64
     L.krr_profile_enable.restype = c.c_int
     L.krr_profile_enable.argtypes = [u32]
@@ -342,4 +347,28 @@ def krr_predict(T, G, gamma, W, return_kernel=False, CT=None, CG=None, flags=0):
         return P
     off = (m * 4 + 1023) // 1024 * 1024 + (n * 4 + 1023) // 1024 * 1024
     return P, ws[off:off + m * n * 4].view(torch.float32).reshape(m, n)
+
+
+def fit_host(h_G, gamma, lam, nb, h_Y, eps_target=0.0, allowed=(FP32,), force_prec=-1, flags=FLAG_PREROUND_A, arena=None,
+             device="cuda"):
+    """krr_fit_host: Build + Associate from host genotypes (int8, pinned recommended) and phenotypes.
+    Returns (alpha host tensor, h_map, info int, arena)."""
+    L = lib()
+    assert h_G.dtype == torch.int8 and not h_G.is_cuda and h_G.stride(1) == 1
+    n, p = h_G.shape
+    nrhs = h_Y.shape[1]
+    NT = n // nb
+    need = int(L.krr_fit_host_arena(n, p, nb, nrhs))
+    if need == 0:
+        raise KrrError("krr_fit_host_arena: invalid shape")
+    if arena is None or arena.numel() < need:
+        arena = _ws(need, device)
+    alpha = torch.empty_like(h_Y)
+    h_map = torch.empty((NT, NT), dtype=torch.uint8)
+    h_info = torch.zeros(1, dtype=torch.int32)
+    mask = sum(1 << q for q in allowed)
+    _check(L.krr_fit_host(_ptr(h_G), n, p, h_G.stride(0), float(gamma), float(lam), nb, float(eps_target), mask, force_prec,
+                          flags, _ptr(h_Y), nrhs, _ptr(alpha), _ptr(h_map), _ptr(h_info), _ptr(arena), arena.numel(), _stream()),
+           "krr_fit_host")
+    return alpha, h_map, int(h_info[0]), arena
 

@@ -743,6 +743,11 @@ namespace {
 struct Arena {
     size_t A, Y, map, norms, amax, fro, info, scales, pm_ws, factor, potrf_ws, potrs_ws, total;
 };
+Arena arena_layout(int64_t n, int nb, int nrhs);
+}  // namespace
+static int associate_in_arena(uint8_t* ar, const Arena& L, int64_t n, int nb, float eps_target, unsigned allowed_mask, int force_prec,
+                              unsigned flags, int nrhs, float* h_alpha, uint8_t* h_map, int* h_info, void* stream, int64_t launches);
+namespace {
 Arena arena_layout(int64_t n, int nb, int nrhs) {
     const size_t NT = n / nb, nslots = NT * (NT + 1) / 2;
     Arena a;
@@ -786,12 +791,23 @@ int krr_associate_host(const float* h_A, int64_t n, int64_t lda, int nb, float e
     uint8_t* ar = static_cast<uint8_t*>(d_arena);
     float* dA = reinterpret_cast<float*>(ar + L.A);
     float* dY = reinterpret_cast<float*>(ar + L.Y);
-    uint8_t* dmap = ar + L.map;
-    const int NT = static_cast<int>(n / nb);
-    int64_t launches = 0;
     KRR_CUDA_CHECK(cudaMemcpy2DAsync(dA, n * sizeof(float), h_A, lda * sizeof(float), n * sizeof(float), n,
                                      cudaMemcpyHostToDevice, st));
     KRR_CUDA_CHECK(cudaMemcpyAsync(dY, h_Y, static_cast<size_t>(n) * nrhs * sizeof(float), cudaMemcpyHostToDevice, st));
+    return associate_in_arena(ar, L, n, nb, eps_target, allowed_mask, force_prec, flags, nrhs, h_alpha, h_map, h_info, stream, 0);
+}
+
+}  // extern "C"
+
+// Associate phase on A and Y already in the arena: map -> factorisation -> solve -> alpha, map, info to the host.
+static int associate_in_arena(uint8_t* ar, const Arena& L, int64_t n, int nb, float eps_target, unsigned allowed_mask, int force_prec,
+                              unsigned flags, int nrhs, float* h_alpha, uint8_t* h_map, int* h_info, void* stream, int64_t launches) {
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    float* dA = reinterpret_cast<float*>(ar + L.A);
+    float* dY = reinterpret_cast<float*>(ar + L.Y);
+    uint8_t* dmap = ar + L.map;
+    const int NT = static_cast<int>(n / nb);
+    int rc;
     if (force_prec < 0) {
         rc = krr_precision_map(dA, n, n, nb, eps_target, allowed_mask, flags & KRR_FLAG_PREROUND_A, dmap,
                                reinterpret_cast<float*>(ar + L.norms), reinterpret_cast<float*>(ar + L.amax),
@@ -821,6 +837,40 @@ int krr_associate_host(const float* h_A, int64_t n, int64_t lda, int nb, float e
     KRR_CUDA_CHECK(cudaStreamSynchronize(st));
     g_launches = launches;
     return KRR_OK;
+}
+
+extern "C" {
+
+// ------------------------------------------------------------------------- Build + Associate from host genotypes
+static size_t fit_g_bytes(int64_t n, int64_t p) { return align_up(static_cast<size_t>(n) * align_up(static_cast<size_t>(p), 16), 1024); }
+
+size_t krr_fit_host_arena(int64_t n, int64_t p, int nb, int nrhs) {
+    if (check_shape(n, nb) != KRR_OK || nrhs < 1 || nrhs > kMaxRhs || p < 1 || n % 256 != 0 || nb % 256 != 0) return 0;
+    return arena_layout(n, nb, nrhs).total + fit_g_bytes(n, p) + krr_build_workspace(n, p, 0);
+}
+
+int krr_fit_host(const int8_t* h_G, int64_t n, int64_t p, int64_t ldg, float gamma, float lambda, int nb, float eps_target,
+                 unsigned allowed_mask, int force_prec, unsigned flags, const float* h_Y, int nrhs, float* h_alpha,
+                 uint8_t* h_map, int* h_info, void* d_arena, size_t arena_bytes, void* stream) {
+    if (!h_G || !h_Y || !h_alpha || !h_map || !h_info || !d_arena) return KRR_ERR_ARG;
+    int rc = check_shape(n, nb);
+    if (rc) return rc;
+    if (n % 256 != 0 || nb % 256 != 0) return KRR_ERR_SHAPE;
+    if (nrhs < 1 || nrhs > kMaxRhs || p < 1 || ldg < p || force_prec > KRR_FP8_E4M3) return KRR_ERR_ARG;
+    if (flags & ~KRR_FLAG_PREROUND_A) return KRR_ERR_UNSUPPORTED;
+    if (arena_bytes < krr_fit_host_arena(n, p, nb, nrhs)) return KRR_ERR_WORKSPACE;
+    const Arena L = arena_layout(n, nb, nrhs);
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    uint8_t* ar = static_cast<uint8_t*>(d_arena);
+    int8_t* dG = reinterpret_cast<int8_t*>(ar + L.total);
+    uint8_t* bws = ar + L.total + fit_g_bytes(n, p);
+    const int64_t ldd = static_cast<int64_t>(align_up(static_cast<size_t>(p), 16));
+    KRR_CUDA_CHECK(cudaMemcpy2DAsync(dG, ldd, h_G, ldg, p, n, cudaMemcpyHostToDevice, st));
+    KRR_CUDA_CHECK(cudaMemcpyAsync(ar + L.Y, h_Y, static_cast<size_t>(n) * nrhs * sizeof(float), cudaMemcpyHostToDevice, st));
+    rc = krr_build(dG, n, p, ldd, nullptr, 0, 0, gamma, lambda, reinterpret_cast<float*>(ar + L.A), n, nb, 0, bws,
+                   krr_build_workspace(n, p, 0), stream);
+    if (rc) return rc;
+    return associate_in_arena(ar, L, n, nb, eps_target, allowed_mask, force_prec, flags, nrhs, h_alpha, h_map, h_info, stream, g_launches);
 }
 
 }  // extern "C"

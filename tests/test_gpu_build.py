@@ -241,3 +241,23 @@ def test_ibs_kernel_build_and_predict(krr, n, m, p, nb):
     Pw = Kw @ W.cpu().numpy().astype(np.float64)
     assert np.all(np.abs(P.cpu().numpy() - Pw) <= 4e-6 * (Kw @ np.abs(W.cpu().numpy().astype(np.float64))))
 
+
+def test_fit_host_matches_device_pipeline(krr):
+    """krr_fit_host (genotypes and Y from host memory, Build on the device) against Build -> map -> factorisation ->
+    solve called one by one: the same kernels on the same data, bit-identical alpha and map."""
+    cfg = scaled_config(CONFIGS["C2"], nb=256, n=1536, p=700)
+    G = genotypes(cfg.seed, cfg.n, cfg.p, cfg.genotype, device="cuda")
+    Y = torch.randn((cfg.n, 8), device="cuda", generator=torch.Generator(device="cuda").manual_seed(5))
+    A = krr.krr_build(padded(G), cfg.gamma, cfg.lam, cfg.nb)
+    d_map, *_ = krr.precision_map(A, cfg.nb, 1e-4, (krr.FP32, krr.FP16))
+    F = krr.potrf_mp(A, cfg.nb, d_map, d_map.cpu())
+    alpha = krr.potrs(F, Y.clone())
+    torch.cuda.synchronize()
+    hG = G.cpu().pin_memory()
+    hY = Y.cpu().pin_memory()
+    a2, m2, info, _ = krr.fit_host(hG, cfg.gamma, cfg.lam, cfg.nb, hY, 1e-4, (krr.FP32, krr.FP16))
+    assert info == 0 and int(F.info.item()) == 0
+    low = torch.tril(torch.ones(cfg.NT, cfg.NT, dtype=torch.bool))
+    assert torch.equal(m2[low], d_map.cpu()[low])
+    assert torch.equal(a2, alpha.cpu())
+

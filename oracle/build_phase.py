@@ -106,3 +106,16 @@ def ibs_kernel_matrix_definition(G1, G2):
         K[i] = shared.sum(axis=1) / (2.0 * ns)
     return K
 
+
+# ---- linear kernel / Ridge Regression (Eq. (2); Fig. 2: the SYRK of the encoded matrix) ----
+def linear_kernel_matrix_definition(Z1, Z2, scale=1.0):
+    """scale * Z1 Z2^T in exact integers, then FP64: the symmetric rank-k update of Eq. (2) when Z = X^T (rows = SNPs,
+    X^T X over the patients), or the linear kernel between patients when Z = X."""
+    return float(scale) * (np.asarray(Z1, dtype=np.int64) @ np.asarray(Z2, dtype=np.int64).T).astype(np.float64)
+
+
+def ridge_regression_definition(X, Y, lam):
+    """Eq. (2): beta = (X^T X + lam I)^-1 X^T Y in FP64."""
+    X = np.asarray(X, dtype=np.float64)
+    return np.linalg.solve(X.T @ X + float(lam) * np.eye(X.shape[1]), X.T @ np.asarray(Y, dtype=np.float64))
+

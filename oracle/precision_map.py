@@ -72,3 +72,17 @@ def uniform_map(NT, offdiag):
         pmap[i, :i] = offdiag
         pmap[i, i] = FP32
     return pmap
+
+
+def band_map(NT, fp32_fraction, low):
+    """The hand-tuned band technique of [37] the paper compares with ("applies a given precision on each
+    band of the off-diagonal tiles"; "100%, 80%, ... 10% FP32 ... the remaining off-diagonal tiles in FP16").
+    Reading (R18): the first b = ceil(fp32_fraction * (NT - 1)) sub-diagonals of tiles are FP32, the tiles
+    further from the diagonal are `low`; the diagonal tiles are always FP32."""
+    b = int(np.ceil(float(fp32_fraction) * (NT - 1) - 1e-12))
+    pmap = np.full((NT, NT), 255, dtype=np.uint8)
+    for i in range(NT):
+        for j in range(i + 1):
+            pmap[i, j] = FP32 if i - j <= b else low
+    return pmap
+

@@ -163,3 +163,20 @@ def test_ibs_kernel_pins():
     # positive semi-definite (a sum of per-locus PSD kernels)
     assert np.linalg.eigvalsh(K).min() > -1e-10
 
+
+def test_linear_kernel_and_ridge_regression_pins():
+    from oracle.build_phase import linear_kernel_matrix_definition, ridge_regression_definition
+    rng = np.random.default_rng(7)
+    X = rng.integers(0, 3, size=(40, 12)).astype(np.int8)              # patients x SNPs
+    # the Gram matrix from the distance expansion: <a, b> = (|a|^2 + |b|^2 - |a - b|^2) / 2
+    s = np.einsum("ik,ik->i", X.astype(np.int64), X.astype(np.int64))
+    assert np.array_equal(linear_kernel_matrix_definition(X, X), (s[:, None] + s[None, :] - squared_distances(X, X)) / 2.0)
+    assert np.array_equal(linear_kernel_matrix_definition(X, X, 0.5), 0.5 * (X.astype(float) @ X.astype(float).T))
+    # Eq. (2): primal ridge = dual (kernel) ridge with the linear kernel, and the normal equations hold
+    Y = rng.standard_normal((40, 3))
+    lam = 0.7
+    beta = ridge_regression_definition(X, Y, lam)
+    alpha = np.linalg.solve(linear_kernel_matrix_definition(X, X) + lam * np.eye(40), Y)
+    assert np.allclose(beta, X.T.astype(float) @ alpha, atol=1e-10)
+    assert np.allclose(X.T.astype(float) @ (Y - X.astype(float) @ beta), lam * beta, atol=1e-9)     # gradient of Eq. (1) vanishes
+

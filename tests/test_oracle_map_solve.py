@@ -157,3 +157,18 @@ def test_survey_probe_numbers_small():
     # finding 1: with tile norms ~ ||A||_F / NT the rule reduces to u_p <= eps
     assert G["fp16_eps_threshold"][0] < R.UNIT_ROUNDOFF[R.FP16] < G["fp16_eps_threshold"][1]
     assert G["fp8_eps_threshold"][0] < R.UNIT_ROUNDOFF[R.FP8] < G["fp8_eps_threshold"][1]
+
+
+def test_band_map_reading():
+    from oracle.precision_map import band_map, uniform_map
+    from oracle.rounding import FP16, FP32
+    assert np.array_equal(band_map(8, 1.0, FP16), uniform_map(8, FP32))          # 100 % FP32
+    assert np.array_equal(band_map(8, 0.0, FP16), uniform_map(8, FP16))          # every off-diagonal tile low
+    m = band_map(11, 0.4, FP16)                                                  # b = ceil(0.4 * 10) = 4 sub-diagonals
+    for i in range(11):
+        for j in range(11):
+            want = 255 if j > i else (FP32 if i - j <= 4 else FP16)
+            assert m[i, j] == want
+    # monotone in the fraction
+    assert all((band_map(9, f1, FP16) <= band_map(9, f2, FP16)).all() for f1, f2 in [(0.8, 0.6), (0.6, 0.2), (0.2, 0.1)])
+

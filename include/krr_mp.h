@@ -83,6 +83,12 @@ typedef enum { KRR_FP32 = 0, KRR_FP16 = 1, KRR_FP8_E4M3 = 2 } krr_prec_t;
                                        their Hamming distance is sum_k |g_ik - g_jk|); gamma is ignored and
                                        confounders are not accepted.                                  */
 
+#define KRR_FLAG_KERNEL_LINEAR 512u  /* krr_build, krr_predict: the linear kernel K_ij = gamma * <g_i, g_j> (exact INT32 Gram
+                                       matrix times the FP32 scale `gamma`; krr_build adds lambda on the diagonal):
+                                       with G = X^T (rows = SNPs) this is the mixed-precision SYRK X^T X + lambda I of
+                                       ridge regression (Eq. (2), Fig. 2; integer part only), with G = X the
+                                       dual form of the same regression.  Confounders are not accepted.       */
+
 /* Library version (major*100 + minor) and the compute capability it was built for (100). */
 int krr_version(void);
 int krr_built_for_sm(void);
@@ -197,6 +203,11 @@ int krr_associate_host(const float* h_A, int64_t n, int64_t lda, int nb,
                        const float* h_Y, int nrhs, float* h_alpha,
                        uint8_t* h_map, int* h_info,
                        void* d_arena, size_t arena_bytes, void* stream);
+
+/* Host utility: the hand-tuned band map of [37] the paper compares its adaptive rule with: diagonal
+ * tiles and the first ceil(fp32_fraction * (NT-1)) sub-diagonals of tiles FP32, the remaining off-diagonal tiles
+ * `low_prec`; 255 above the diagonal.  h_map: NT*NT bytes.  Pure host code. */
+int krr_band_map(int NT, double fp32_fraction, int low_prec, uint8_t* h_map);
 
 /* ---------------------------------------------------------------------------------------------
  * krr_build -- Build phase (Alg. 2 :92-106 with the Gaussian kernel of Alg. 5 :136-143;

@@ -13,6 +13,7 @@ FLAG_FP8_VIA_FP16 = 16
 FLAG_NO_CTA_PAIRS = 32
 FLAG_FUSED_CHAIN = 64
 FLAG_KERNEL_IBS = 256
+FLAG_KERNEL_LINEAR = 512
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB = None
@@ -23,7 +24,7 @@ ERRORS = {-1: "KRR_ERR_ARG", -2: "KRR_ERR_SHAPE", -3: "KRR_ERR_WORKSPACE", -4: "
 EXPORTS = ["krr_version", "krr_built_for_sm", "krr_tile_slot", "krr_precision_map_workspace",
            "krr_precision_map", "krr_factor_bytes", "krr_factor_tile_offset",
            "krr_potrf_mp_workspace", "krr_potrf_mp", "krr_potrs_workspace", "krr_potrs",
-           "krr_associate_host_arena", "krr_associate_host", "krr_build_workspace", "krr_build", "krr_predict_workspace", "krr_predict", "krr_fit_host_arena", "krr_fit_host",
+           "krr_associate_host_arena", "krr_associate_host", "krr_build_workspace", "krr_build", "krr_predict_workspace", "krr_predict", "krr_fit_host_arena", "krr_fit_host", "krr_band_map",
            "krr_last_launch_count",
            "krr_profile_enable", "krr_profile_read"]
 
@@ -87,6 +88,8 @@ def lib():
     L.krr_fit_host.restype = c.c_int
     L.krr_fit_host.argtypes = [vp, i64, i64, i64, c.c_float, c.c_float, c.c_int, c.c_float, u32, c.c_int, u32, vp, c.c_int, vp,
                                vp, vp, vp, sz, vp]
+    L.krr_band_map.restype = c.c_int
+    L.krr_band_map.argtypes = [c.c_int, c.c_double, c.c_int, vp]
     L.krr_last_launch_count.restype = i64
     L.krr_profile_enable.restype = c.c_int
     L.krr_profile_enable.argtypes = [u32]
@@ -371,4 +374,11 @@ def fit_host(h_G, gamma, lam, nb, h_Y, eps_target=0.0, allowed=(FP32,), force_pr
                           flags, _ptr(h_Y), nrhs, _ptr(alpha), _ptr(h_map), _ptr(h_info), _ptr(arena), arena.numel(), _stream()),
            "krr_fit_host")
     return alpha, h_map, int(h_info[0]), arena
+
+
+def band_map(NT, fp32_fraction, low):
+    """krr_band_map: host map (uint8 NT x NT) of the band technique of [37]."""
+    m = torch.empty((NT, NT), dtype=torch.uint8)
+    _check(lib().krr_band_map(NT, float(fp32_fraction), int(low), _ptr(m)), "krr_band_map")
+    return m
 

@@ -341,6 +341,21 @@ int64_t krr_factor_tile_offset(int64_t n, int nb, const uint8_t* h_map, int i, i
     return off[static_cast<size_t>(i) * NT + j];
 }
 
+// Band map of [37]: the first ceil(fp32_fraction (NT-1)) sub-diagonals of tiles FP32, the rest `low_prec`.
+int krr_band_map(int NT, double fp32_fraction, int low_prec, uint8_t* h_map) {
+    if (NT <= 0 || NT > kMaxNT || !h_map || low_prec < KRR_FP32 || low_prec > KRR_FP8_E4M3 || !(fp32_fraction >= 0.0) ||
+        fp32_fraction > 1.0)
+        return KRR_ERR_ARG;
+    double bd = fp32_fraction * (NT - 1) - 1e-12;
+    int b = static_cast<int>(bd);
+    if (static_cast<double>(b) < bd) ++b;                    // ceil
+    if (b < 0) b = 0;
+    for (int i = 0; i < NT; ++i)
+        for (int j = 0; j < NT; ++j)
+            h_map[i * NT + j] = (j > i) ? 255 : ((i - j <= b) ? KRR_FP32 : static_cast<uint8_t>(low_prec));
+    return KRR_OK;
+}
+
 // ------------------------------------------------------------------------- factorisation
 size_t krr_potrf_mp_workspace(int64_t n, int nb, const uint8_t* h_map) {
     if (!h_map || check_shape(n, nb) != KRR_OK) return 0;
@@ -935,9 +950,10 @@ int krr_build(const int8_t* d_G, int64_t n, int64_t p, int64_t ldg, const float*
     if (n % 256 != 0 || nb % 256 != 0) return KRR_ERR_SHAPE;
     if (p < 1 || p > 133000 || ldg < p || ldg % 16 != 0) return KRR_ERR_ARG;      // INT32 sums of int8 squares stay exact
     const bool tiled = flags & KRR_FLAG_A_TILED_LOWER;
-    const bool ibs = flags & KRR_FLAG_KERNEL_IBS;
-    if (flags & ~(KRR_FLAG_A_TILED_LOWER | KRR_FLAG_KERNEL_IBS)) return KRR_ERR_UNSUPPORTED;
-    if (ibs && q > 0) return KRR_ERR_UNSUPPORTED;                                  // confounders belong to the Gaussian kernel
+    const bool ibs = flags & KRR_FLAG_KERNEL_IBS, linear = flags & KRR_FLAG_KERNEL_LINEAR;
+    if (flags & ~(KRR_FLAG_A_TILED_LOWER | KRR_FLAG_KERNEL_IBS | KRR_FLAG_KERNEL_LINEAR)) return KRR_ERR_UNSUPPORTED;
+    if ((ibs || linear) && q > 0) return KRR_ERR_UNSUPPORTED;                      // confounders belong to the Gaussian kernel
+    if (ibs && linear) return KRR_ERR_ARG;
     if (!tiled && (lda < n || lda % 4 != 0)) return KRR_ERR_ARG;
     if (reinterpret_cast<uintptr_t>(d_G) % 16 != 0 || reinterpret_cast<uintptr_t>(d_A) % 16 != 0 ||
         reinterpret_cast<uintptr_t>(d_ws) % 16 != 0)
@@ -964,6 +980,7 @@ int krr_build(const int8_t* d_G, int64_t n, int64_t p, int64_t ldg, const float*
     BuildOp op;
     memset(&op, 0, sizeof(op));
     op.ibs = ibs ? 1 : 0; op.alleles = static_cast<float>(p);        // (p was doubled above: 2 N_S alleles)
+    op.linear = linear ? 1 : 0; op.lambda = lambda;
     op.n = n; op.m = n; op.rect = 0; op.p = p; op.nb = nb; op.tiled = tiled ? 1 : 0; op.gamma = gamma;
     op.diag = static_cast<float>(1.0 + static_cast<double>(lambda));
     op.sq = sq; op.sq_row = sq; op.A = d_A; op.lda = lda;
@@ -988,9 +1005,10 @@ int krr_predict(const int8_t* d_T, int64_t m, int64_t ldt, const int8_t* d_G, in
                 void* stream) {
     g_launches = 0;
     if (!d_T || !d_G || !d_W || !d_P || !d_ws) return KRR_ERR_ARG;
-    const bool ibs = flags & KRR_FLAG_KERNEL_IBS;
-    if (flags & ~KRR_FLAG_KERNEL_IBS) return KRR_ERR_UNSUPPORTED;
-    if (ibs && q > 0) return KRR_ERR_UNSUPPORTED;
+    const bool ibs = flags & KRR_FLAG_KERNEL_IBS, linear = flags & KRR_FLAG_KERNEL_LINEAR;
+    if (flags & ~(KRR_FLAG_KERNEL_IBS | KRR_FLAG_KERNEL_LINEAR)) return KRR_ERR_UNSUPPORTED;
+    if ((ibs || linear) && q > 0) return KRR_ERR_UNSUPPORTED;
+    if (ibs && linear) return KRR_ERR_ARG;
     if (q < 0 || q > kMaxConfounders || (q > 0 && (!d_CT || !d_CG || ldct < q || ldcg < q))) return KRR_ERR_ARG;
     if (m <= 0 || n <= 0 || m % 256 != 0 || n % 256 != 0) return KRR_ERR_SHAPE;
     if (p < 1 || p > 133000 || ldg < p || ldg % 16 != 0 || ldt < p || ldt % 16 != 0) return KRR_ERR_ARG;
@@ -1027,6 +1045,7 @@ int krr_predict(const int8_t* d_T, int64_t m, int64_t ldt, const int8_t* d_G, in
     BuildOp op;
     memset(&op, 0, sizeof(op));
     op.ibs = ibs ? 1 : 0; op.alleles = static_cast<float>(p);
+    op.linear = linear ? 1 : 0; op.lambda = 0.0f;
     op.n = n; op.m = m; op.rect = 1; op.p = p; op.nb = 256; op.tiled = 0; op.gamma = gamma; op.diag = 1.0f;
     op.sq = sqG; op.sq_row = sqT; op.A = K; op.lda = n;
     op.C = d_CG; op.C_row = d_CT; op.ldc = ldcg; op.ldc_row = ldct; op.q = q;

@@ -39,6 +39,9 @@ struct BuildOp {
     // the Hamming distance sum_k |g_ik - g_jk| and K_ij = (alleles - d2) / alleles, alleles = 2 N_S (no exponential)
     int ibs;
     float alleles;
+    // linear kernel (the SYRK of ridge regression, Eq. (2), Fig. 2): K_ij = gamma * <g_i, g_j>, lambda on the diagonal
+    int linear;
+    float lambda;
 };
 constexpr int kMaxConfounders = 16;
 
@@ -287,8 +290,15 @@ build_tc_kernel(const __grid_constant__ CUtensorMap tmR, const __grid_constant__
                                 if (c < op.q) { const float t = ci[c] - __ldg(cj + c); dc = fmaf(t, t, dc); }
                             d2f += dc;
                         }
-                        const float kv = op.ibs ? __fdiv_rn(op.alleles - d2f, op.alleles) : expf(-op.gamma * d2f);
-                        v[u] = (!op.rect && gj0 + e + u == gi) ? op.diag : kv;
+                        float kv;
+                        if (op.linear) {
+                            kv = op.gamma * static_cast<float>(static_cast<int>(acc[e + u]));
+                            if (!op.rect && gj0 + e + u == gi) kv += op.lambda;
+                        } else {
+                            kv = op.ibs ? __fdiv_rn(op.alleles - d2f, op.alleles) : expf(-op.gamma * d2f);
+                            if (!op.rect && gj0 + e + u == gi) kv = op.diag;
+                        }
+                        v[u] = kv;
                     }
                     *reinterpret_cast<float4*>(dst + e) = make_float4(v[0], v[1], v[2], v[3]);
                 }

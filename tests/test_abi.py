@@ -65,3 +65,15 @@ def test_argument_errors_are_reported_before_any_launch():
     m = krr.uniform_map(2, krr.FP32)
     rc = L.krr_potrf_mp(null, 256, 256, 128, null, ctypes.c_void_p(m.data_ptr()), null, null, null, null, 0, 1, null)
     assert rc == -1
+
+
+def test_band_map_host_utility_matches_oracle():
+    """krr_band_map is pure host code: callable without a GPU; bit-exact against the oracle's reading."""
+    import numpy as np
+    import paper_2409_01712_b200 as krr
+    from oracle.precision_map import band_map
+    for NT in (1, 2, 8, 11, 64):
+        for frac in (0.0, 0.1, 0.2, 0.4, 0.6, 0.8, 1.0):
+            for low in (1, 2):
+                assert np.array_equal(krr.band_map(NT, frac, low).numpy(), band_map(NT, frac, low)), (NT, frac, low)
+

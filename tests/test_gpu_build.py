@@ -261,3 +261,38 @@ def test_fit_host_matches_device_pipeline(krr):
     assert torch.equal(m2[low], d_map.cpu()[low])
     assert torch.equal(a2, alpha.cpu())
 
+
+def test_linear_kernel_and_ridge_regression(krr):
+    """PAPER.md Eq. (2): beta = (X^T X + lam I)^-1 X^T Y with the SYRK on the INT8 tensor cores (krr_build with
+    KRR_FLAG_KERNEL_LINEAR on X^T: exact integers), the factorisation and the FP32 solves of the Associate path."""
+    from oracle.build_phase import linear_kernel_matrix_definition, ridge_regression_definition
+    npat, nsnp, nb = 3000, 1024, 256
+    X = genotypes(61, npat, nsnp, "maf", device="cuda")                    # patients x SNPs
+    Z = X.t().contiguous()                                                 # SNPs x patients: rows = the vectors of the SYRK
+    lam = 50.0
+    A = krr.krr_build(padded(Z), 1.0, lam, nb, flags=krr.FLAG_KERNEL_LINEAR)
+    torch.cuda.synchronize()
+    want = linear_kernel_matrix_definition(Z.cpu().numpy(), Z.cpu().numpy()) + lam * np.eye(nsnp)
+    got = A.cpu().numpy().astype(np.float64)
+    low = np.tril_indices(nsnp)
+    NT = nsnp // nb
+    for i in range(NT):
+        for j in range(i + 1):
+            assert np.array_equal(got[i * nb:(i + 1) * nb, j * nb:(j + 1) * nb], want[i * nb:(i + 1) * nb, j * nb:(j + 1) * nb])   # exact
+    Y = torch.randn((npat, 4), device="cuda", generator=torch.Generator(device="cuda").manual_seed(3))
+    XtY = (X.to(torch.float32).t() @ Y).contiguous()                       # "in single precision" (PAPER.md:169)
+    h = krr.uniform_map(NT, krr.FP32)
+    F = krr.potrf_mp(A, nb, h.cuda(), h)
+    beta = krr.potrs(F, XtY.clone())
+    torch.cuda.synchronize()
+    assert int(F.info.item()) == 0
+    b64 = ridge_regression_definition(X.cpu().numpy(), Y.cpu().numpy(), lam)
+    assert np.linalg.norm(beta.cpu().numpy() - b64) / np.linalg.norm(b64) <= 1e-3
+    # the rectangular variant: scale * T G^T
+    T = genotypes(62, 256, nsnp, "maf", device="cuda")
+    W = torch.randn((npat // 8 * 8 // 256 * 256, 2), device="cuda")
+    Gs = X[:W.shape[0]].contiguous()
+    P, K = krr.krr_predict(padded(T), padded(Gs), 0.25, W, return_kernel=True, flags=krr.FLAG_KERNEL_LINEAR)
+    torch.cuda.synchronize()
+    assert np.array_equal(K.cpu().numpy().astype(np.float64), linear_kernel_matrix_definition(T.cpu().numpy(), Gs.cpu().numpy(), 0.25))
+

@@ -76,6 +76,11 @@ typedef enum { KRR_FP32 = 0, KRR_FP16 = 1, KRR_FP8_E4M3 = 2 } krr_prec_t;
                                        128 dependent pivots of each block, not by launches), kept as the
                                        persistent-kernel variant and as a cross-check.                 */
 
+#define KRR_FLAG_NO_TAIL_SPLIT 1024u /* krr_potrf_mp: do not split the blocks of a trailing update's last, partial wave
+                                       between several CTA pairs (slices of the term range added into the FP32
+                                       partial sums one after the other); same products, another summation order
+                                       for those blocks; comparison.                                   */
+
 #define KRR_FLAG_KERNEL_IBS    256u  /* krr_build, krr_predict: the identical-by-state kernel of Alg. 5 l.5-6 (PAPER.md:134,
                                        :141) instead of the Gaussian one: K_ij = (alleles of i and j identical
                                        by state, 2 - |g_ik - g_jk| per locus for genotypes in {0,1,2}) / (2 N_S).

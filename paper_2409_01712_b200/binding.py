@@ -14,6 +14,7 @@ FLAG_NO_CTA_PAIRS = 32
 FLAG_FUSED_CHAIN = 64
 FLAG_KERNEL_IBS = 256
 FLAG_KERNEL_LINEAR = 512
+FLAG_NO_TAIL_SPLIT = 1024
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB = None

@@ -113,7 +113,7 @@ static size_t host_offsets(int NT, int nb, const uint8_t* h_map, std::vector<int
 
 // ---- workspace layout of krr_potrf_mp ----------------------------------------------------------
 struct PotrfWs {
-    size_t off_table, a_amax, tile_amax, scl, prog, W, W2, linv_hi, linv_lo, Hp, Lp, Qp, total;
+    size_t off_table, a_amax, tile_amax, scl, prog, split, W, W2, linv_hi, linv_lo, Hp, Lp, Qp, total;
 };
 static PotrfWs potrf_ws_layout(int64_t n, int nb, bool any_fp8) {
     const int64_t NT = n / nb;
@@ -126,6 +126,7 @@ static PotrfWs potrf_ws_layout(int64_t n, int nb, bool any_fp8) {
     w.tile_amax = o; o = align_up(o + nslots * sizeof(float), 1024);
     w.scl = o;       o = align_up(o + (4 + 2 * (nb / kBlk)) * sizeof(float), 1024);
     w.prog = o;      o = align_up(o + static_cast<size_t>(n / kBlk) * sizeof(int), 1024);   // fused-chain progress, per 128-block
+    w.split = o;     o = align_up(o + 256 * sizeof(int), 1024);                              // slice counters of split tail blocks
     w.W = o;         o = align_up(o + static_cast<size_t>(n) * nb * sizeof(float), 1024);
     w.W2 = o;        o = align_up(o + static_cast<size_t>(n) * nb * sizeof(float), 1024);   // lookahead: column k+1's partial
     w.linv_hi = o;   o = align_up(o + 2 * static_cast<size_t>(nb) * kBlk * 2, 1024);   // two sets (column parity)
@@ -199,7 +200,9 @@ static int launch(int cat, K kernel, dim3 grid, dim3 block, size_t smem, cudaStr
 struct GemmMaps { CUtensorMap H, L, IH[2], IL[2], Q; };
 
 // cg = 2 runs MODE_UPDATE on CTA pairs (256 x 256 output blocks); needs even block counts.
-static int launch_gemm(const GemmMaps& m, const GemmOp& op, int max_ctas, int cg, cudaStream_t st, int linv_buf = 0) {
+static int launch_gemm(const GemmMaps& m, const GemmOp& op_in, int max_ctas, int cg, cudaStream_t st, int linv_buf = 0,
+                       int* split_flags = nullptr) {
+    GemmOp op = op_in;
     if (op.nrb <= 0 || op.ncb <= 0) return KRR_OK;
     // MODE_PANEL counts as panel_trsm, the fused diagonal chain (MODE_DIAG, POTRF included) as potrf128
     ProfScope ps(op.mode == MODE_UPDATE ? CAT_UPDATE : (op.mode == MODE_P1 ? CAT_P1 : (op.mode == MODE_DIAG ? CAT_POTRF : CAT_P3)), st);
@@ -208,6 +211,18 @@ static int launch_gemm(const GemmMaps& m, const GemmOp& op, int max_ctas, int cg
         const int npairs = (op.nrb / 2) * (op.ncb / 2);
         const int max_pairs = max_ctas / 2;
         const int grid = 2 * (npairs < max_pairs ? npairs : max_pairs);
+        // tail of the last wave: r leftover blocks for max_pairs pairs.  Share each of them between g pairs (slices of the
+        // term range, added into W one after the other) so that the tail lasts 1/g of a block instead of a whole one.
+        const int nterms = op.s_hi - op.s_lo, q = npairs / max_pairs, r = npairs % max_pairs;
+        if (split_flags && q >= 1 && r > 0 && 2 * r <= max_pairs && nterms >= 2) {
+            int g = max_pairs / r;
+            if (g > nterms) g = nterms;
+            if (g > 16) g = 16;
+            if (g >= 2) {
+                op.split_t0 = q * max_pairs; op.split_g = g; op.split_flags = split_flags;
+                if (cudaMemsetAsync(split_flags, 0, static_cast<size_t>(r) * sizeof(int), st) != cudaSuccess) return KRR_ERR_CUDA;
+            }
+        }
         cudaLaunchConfig_t cfg;
         memset(&cfg, 0, sizeof(cfg));
         cfg.gridDim = dim3(grid); cfg.blockDim = dim3(kGemmThreads); cfg.dynamicSmemBytes = kGemmSmem; cfg.stream = st;
@@ -377,7 +392,7 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
         reinterpret_cast<uintptr_t>(d_factor) % 128 != 0)
         return KRR_ERR_ARG;
     if (flags & ~(KRR_FLAG_PREROUND_A | KRR_FLAG_A_TILED_LOWER | KRR_FLAG_NO_LOOKAHEAD | KRR_FLAG_FP8_VIA_FP16 | KRR_FLAG_NO_CTA_PAIRS |
-                  KRR_FLAG_FUSED_CHAIN))
+                  KRR_FLAG_FUSED_CHAIN | KRR_FLAG_NO_TAIL_SPLIT))
         return KRR_ERR_UNSUPPORTED;
     const int NT = static_cast<int>(n / nb);
     bool any_fp8 = false;
@@ -411,6 +426,7 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
     KRR_CUDA_CHECK(cudaMemsetAsync(d_scales, 0, static_cast<size_t>(NT) * NT * sizeof(float), st));
     KRR_CUDA_CHECK(cudaMemsetAsync(tile_amax, 0, nslots * sizeof(float), st));
     int* prog = reinterpret_cast<int*>(ws + L.prog);
+    int* split_flags = (flags & KRR_FLAG_NO_TAIL_SPLIT) ? nullptr : reinterpret_cast<int*>(ws + L.split);
     KRR_CUDA_CHECK(cudaMemsetAsync(prog, 0, static_cast<size_t>(n / kBlk) * sizeof(int), st));
     rc = launch(CAT_MISC, offsets_kernel, dim3(1), dim3(32), 0, st, NT, nb, d_map, off);
     if (rc) return rc;
@@ -487,7 +503,7 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
         op.mode = MODE_UPDATE; op.c = 0; op.cb0 = 0; op.ncb = nsub;
         if (!lookahead) {
             op.s_lo = 0; op.s_hi = k; op.base_w = 0; op.planes = 1; op.rb0 = 0; op.nrb = mblk;
-            rc = launch_gemm(tm, op, num_sms, cg, st);
+            rc = launch_gemm(tm, op, num_sms, cg, st, 0, split_flags);
             if (rc) return rc;
         } else {
             // terms s < k-1 were accumulated into Wk by O(k) while column k-1 was being factorised; the
@@ -509,7 +525,7 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
                 on.k = k + 1; on.prow0 = tile_slot(NT, k + 1, k + 1) * nb; on.W = Wbuf[(k + 1) & 1];
                 on.s_lo = 0; on.s_hi = k; on.base_w = 0; on.planes = 0;
                 on.rb0 = 0; on.nrb = (NT - k - 1) * nsub;
-                rc = launch_gemm(tm, on, bulk_ctas, cg, sl);
+                rc = launch_gemm(tm, on, bulk_ctas, cg, sl, 0, split_flags);
                 if (rc) return rc;
                 KRR_CUDA_CHECK(cudaEventRecord(ev_old(k + 1), sl));
             }

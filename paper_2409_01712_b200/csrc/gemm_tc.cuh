@@ -74,6 +74,11 @@ struct GemmOp {
     float* linv_scale_w;      // = linv_scale, writable
     int* info;                // krr_potrf_mp's d_info
     int64_t col_base;         // 1-based global index of the tile column's first scalar column
+    // MODE_UPDATE, tail of the last wave: the blocks from index split_t0 on are each shared by split_g units, every unit
+    // accumulating a slice of the terms; the slices are added into W one after the other (split_flags[block - split_t0]
+    // counts the CTAs that have stored their slice; zero at launch).  split_g = 0: no splitting.
+    int split_t0, split_g;
+    int* split_flags;
 };
 
 constexpr int kSlots = 6;                          // shared-memory ring: 6 slots of [A block | B block]
@@ -187,6 +192,9 @@ struct WorkItem {
     int rb, cb;      // first output row block / column block (of the pair when CG = 2)
     int dep;         // > 0: reads what the item `dep` places earlier in this CTA's sequence wrote
     int xcta, xneed; // MODE_DIAG: reads what CTA xcta wrote in its first xneed items (xcta < 0: nothing)
+    int t_lo, t_hi;  // terms [t_lo, t_hi) of the launch's term range are accumulated by this item
+    int cpos, clen;  // position in the chain of slices added into W (clen = 1: the block is not split)
+    int fidx;        // index into op.split_flags
 };
 struct ItemIter {
     int t;           // block modes: next block index
@@ -196,6 +204,7 @@ struct ItemIter {
 template <int CG>
 __device__ __forceinline__ bool next_item(const GemmOp& op, ItemIter& st, int unit0, int nunits, WorkItem& w) {
     w.xcta = -1; w.xneed = 0;
+    w.t_lo = 0; w.t_hi = num_terms(op); w.cpos = 0; w.clen = 1; w.fidx = 0;
     if (op.mode == MODE_DIAG) {
         // CTA r owns row block r of the diagonal tile: P3(0), P1(1), P3(1), ..., P3(r-1), P1(r), POTRF(r).
         // P1(c) reads the rows of block c that CTA c finished with its P3(c-1) (item 2c-2), P3(c) the inverse
@@ -228,9 +237,20 @@ __device__ __forceinline__ bool next_item(const GemmOp& op, ItemIter& st, int un
     }
     const int ncbu = op.ncb / CG;
     const int ntiles = (op.nrb / CG) * ncbu;
-    while (st.t < ntiles) {
-        const int t = st.t;
+    const int g = (op.mode == MODE_UPDATE) ? op.split_g : 0;
+    const int next = g ? op.split_t0 + (ntiles - op.split_t0) * g : ntiles;      // extended index space
+    while (st.t < next) {
+        int t = st.t;
         st.t += nunits;
+        if (g && t >= op.split_t0) {
+            // a block of the tail wave: slice sl of g.  Slices are added into W from the highest terms (smallest
+            // contributions) down to slice 0, which holds the leading tile columns and writes the images.
+            const int sl = (t - op.split_t0) % g;
+            t = op.split_t0 + (t - op.split_t0) / g;
+            const int nt = w.t_hi;
+            w.t_lo = nt * sl / g; w.t_hi = nt * (sl + 1) / g;
+            w.cpos = g - 1 - sl; w.clen = g; w.fidx = t - op.split_t0;
+        }
 #ifdef KRR_EXP_REVERSE_ROWS
         w.rb = op.rb0 + (op.nrb / CG - 1 - t / ncbu) * CG;
 #else
@@ -356,10 +376,10 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
                     ptx::fence_proxy_async_global();
                 }
                 ++seq;
-                uint32_t cls_next = term_class_load<CG>(op, w.mode, nterms - 1, rb);
-                for (int s = nterms - 1; s >= 0; --s) {      // descending K: see note on accumulation order
+                uint32_t cls_next = term_class_load<CG>(op, w.mode, w.t_hi - 1, rb);
+                for (int s = w.t_hi - 1; s >= w.t_lo; --s) {      // descending K: see note on accumulation order
                     const uint32_t cls = make_uniform(cls_next);
-                    if (s > 0) cls_next = term_class_load<CG>(op, w.mode, s - 1, rb);   // in flight during this term's chunks
+                    if (s > w.t_lo) cls_next = term_class_load<CG>(op, w.mode, s - 1, rb);   // in flight during this term's chunks
                     const TermGeom g = term_geom(op, w.mode, w.c, s, rb, cb0u + rank);  // this CTA's A rows and B rows
                     if (cls & kClsQ) {                       // E4M3 images: 128 bytes of K per row, one slot per chunk
                         for (int ch = g.kelems / 128 - 1; ch >= 0; --ch) {
@@ -424,14 +444,14 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
             while (next_item<CG>(op, iter, unit0, nunits, w)) {
                 const int rb = w.rb;
                 if (w.mode == MODE_POTRF) continue;
-                uint32_t cls_next = term_class_load<CG>(op, w.mode, nterms - 1, rb);
+                uint32_t cls_next = term_class_load<CG>(op, w.mode, w.t_hi - 1, rb);
                 ptx::mbar_wait(tempty_bar(buf), acc_phase ^ 1u);     // epilogue drained this buffer
                 ptx::tc_fence_after();
                 const uint32_t d_tmem = tmem_base + buf * kAccW;
                 uint32_t accumulate = 0;
-                for (int s = nterms - 1; s >= 0; --s) {      // descending K: see note on accumulation order
+                for (int s = w.t_hi - 1; s >= w.t_lo; --s) {      // descending K: see note on accumulation order
                     const uint32_t cls = make_uniform(cls_next);
-                    if (s > 0) cls_next = term_class_load<CG>(op, w.mode, s - 1, rb);
+                    if (s > w.t_lo) cls_next = term_class_load<CG>(op, w.mode, s - 1, rb);
                     const int kelems = (w.mode == MODE_UPDATE) ? op.nb : (w.mode == MODE_P1 ? w.c * kBlk : kBlk);
                     if (cls & kClsQ) {
                         const uint32_t sfa = tmem_base + kSfCol0 + 4 * CG * ((cls >> 8) & 63u);
@@ -537,6 +557,17 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
                 ++eseq;
                 continue;
             }
+            if (w.cpos > 0) {
+                // a later slice of a split block: the slices before it have been added into W by other CTAs
+                if (lane == 0) {
+                    const volatile int* f = op.split_flags + w.fidx;
+                    uint32_t spins = 0;
+                    while (*f < CG * w.cpos) { __nanosleep(32); if (++spins > (1u << 26)) __trap(); }
+                    __threadfence();
+                }
+                __syncwarp();
+            }
+            const bool item_planes = write_planes && (w.cpos == w.clen - 1);
 #pragma unroll 1
           for (int j2 = 0; j2 < CG; ++j2) {                       // the unit's column blocks, one after the other
             const int cb = cb0u + j2;
@@ -546,14 +577,14 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
             float* wblk = op.W + (static_cast<int64_t>(rb) * nsub + cb) * (kBlk * kBlk) + static_cast<int64_t>(64 * hf) * kBlk + row_in_blk;
             // ---- base values, fetched before the accumulator is ready
             float bs[64];
-            const bool base_from_w = (w.mode == MODE_P1) || (w.mode == MODE_UPDATE && op.base_w);
-            const bool base_from_a = (w.mode == MODE_UPDATE && !op.base_w);
+            const bool base_from_w = (w.mode == MODE_P1) || (w.mode == MODE_UPDATE && (op.base_w || w.cpos > 0));
+            const bool base_from_a = (w.mode == MODE_UPDATE && !op.base_w && w.cpos == 0);
             if (dead) {
 #pragma unroll
                 for (int e = 0; e < 64; ++e) bs[e] = 0.0f;
             } else if (base_from_w) {
 #pragma unroll
-                for (int e = 0; e < 64; ++e) bs[e] = wblk[e * kBlk];
+                for (int e = 0; e < 64; ++e) bs[e] = __ldcg(wblk + e * kBlk);
             } else if (base_from_a) {
                 const int i = op.k + (rb * kBlk) / op.nb;
                 const int subrow = (rb * kBlk) % op.nb;
@@ -611,7 +642,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
 #pragma unroll
             for (int e = 0; e < 64; ++e) wblk[e * kBlk] = out[e];
             float amax = 0.0f;
-            if (write_planes) {
+            if (item_planes) {
                 const int64_t prow = op.prow0 + static_cast<int64_t>(rb) * kBlk + q * 32;      // plane row of this warp's row 0
 #pragma unroll
                 for (int part = 0; part < 4; ++part) {             // (chunk 0 hi, chunk 0 lo, chunk 1 hi, chunk 1 lo)
@@ -648,6 +679,15 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
                 }
             }
           }   // j2
+            if (w.clen > 1 && w.cpos < w.clen - 1) {
+                // a slice of a split block is in W: let the next slice's CTAs go on (the last warp of this CTA signals)
+                __threadfence();
+                __syncwarp();
+                if (lane == 0) {
+                    const int old = atomicAdd_block(const_cast<int*>(done_ctr), 1);
+                    if (old % kEpiWarps == kEpiWarps - 1) { __threadfence(); atomicAdd(op.split_flags + w.fidx, 1); }
+                }
+            }
             if (op.mode == MODE_PANEL || op.mode == MODE_DIAG) {
                 // publish this item's operand images to the TMA loads of a later item of this CTA (and, in
                 // MODE_DIAG, of the other CTAs: the last warp to finish advances the CTA's progress counter)

@@ -134,3 +134,32 @@ def test_full_size_leading_block_and_invariants(krr, name):
     bwd = probe_backward_error(A, F, 4)
     assert bwd <= (1e-6 if hist[1] == 0 and hist[2] == 0 else 5e-4)
     assert solve_residual(A, alpha, Y) <= 1e-6
+
+
+def test_tail_split_of_the_last_wave(krr):
+    """More output blocks than CTA pairs with a small remainder (NT = 80 tiles of 256: 75-79 pair blocks per tile
+    column for 73-74 pairs): the blocks of the last, partial wave are shared between pairs, each accumulating a slice
+    of the terms, the slices added into the FP32 partial sums in a fixed order.  Same products, another summation
+    order for those blocks: against KRR_FLAG_NO_TAIL_SPLIT to FP32 noise, against the FP64 oracle as usual, and
+    deterministic, in both schedules."""
+    from dataclasses import replace
+    from krr_inputs import scaled_config
+    cfg = replace(scaled_config(CONFIGS["C2"], nb=256, n=20480, p=4000))
+    A, Y = make_problem(cfg, device="cuda")
+    h = krr.uniform_map(cfg.NT, krr.FP32)
+    An = A.cpu().numpy()
+    Lo, info = tile_cholesky_fp64(An, cfg.nb)
+    assert info == 0
+    for extra in (0, krr.FLAG_NO_LOOKAHEAD):
+        F1 = krr.potrf_mp(A, cfg.nb, h.cuda(), h, flags=krr.FLAG_PREROUND_A | extra)
+        F2 = krr.potrf_mp(A, cfg.nb, h.cuda(), h, flags=krr.FLAG_PREROUND_A | extra | krr.FLAG_NO_TAIL_SPLIT)
+        F3 = krr.potrf_mp(A, cfg.nb, h.cuda(), h, flags=krr.FLAG_PREROUND_A | extra)
+        torch.cuda.synchronize()
+        assert int(F1.info.item()) == 0 and int(F2.info.item()) == 0
+        assert torch.equal(F1.payload, F3.payload)                        # deterministic
+        assert not torch.equal(F1.payload, F2.payload)                    # the split path was taken
+        L1, L2 = F1.dense().cpu().numpy(), F2.dense().cpu().numpy()
+        assert relF(L1, L2) <= 1e-5
+        assert relF(L1, Lo) <= 1e-4 and relF(L2, Lo) <= 1e-4
+        assert probe_backward_error(A, F1, 4) <= 1e-6
+

@@ -31,7 +31,7 @@ METRIC = "mixed-precision Cholesky TOp/s (n^3/3 / device time)"
 UNIT = "TOp/s"
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the trailing-update kernel, from the
 # `ncu --set full` capture summarised under profiles/ (bytes; None where no capture exists)
-TRAFFIC_NCU = {"C3": 8.52e9, "C3h": 3.71e9, "C5p": 4.96e9}
+TRAFFIC_NCU = {"C3": 11.25e9, "C3h": 5.34e9, "C5p": 7.0e9}
 TRAFFIC_NOTE = ("profiles/r01_gemm_tc_full_C3.md: one launch of the dominant shape O(k+1) at mid factorisation (C3/C3h: k = 32, "
                 "31 tile rows, K = 32 tiles, algorithmic operand bytes 4.3 / 2.1 GB; C5p: k = 48, 2.4 GB)")
 

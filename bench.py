@@ -395,6 +395,7 @@ def run_e2e(ctx, steps):
     of alpha / map / info inside the timed region."""
     A, Y, krr, cfg, dev = ctx
     n, nb = cfg.n, cfg.nb
+    NT = n // nb
     hA = torch.empty((n, n), dtype=torch.float32, pin_memory=True)
     hA.copy_(A)
     hY = Y.cpu().pin_memory()
@@ -413,9 +414,8 @@ def run_e2e(ctx, steps):
         if it > 0:
             times.append(e0.elapsed_time(e1))
     ms = sum(times) / len(times)
-    NT = n // nb
     return {"value": round(n ** 3 / 3.0 / (ms * 1e-3) / 1e12, 3), "unit": UNIT, "ms_per_step": round(ms, 3),
-            "h2d_bytes_per_step": n * n * 4 + n * cfg.nrhs * 4,
+            "h2d_bytes_per_step": nb * nb * 4 * NT * (NT + 1) // 2 + n * cfg.nrhs * 4,      # the lower tiles of A, and Y
             "d2h_bytes_per_step": n * cfg.nrhs * 4 + NT * NT + 4, "steps": len(times),
             "api": "krr_associate_host (pinned host A, Y -> alpha)"}
 

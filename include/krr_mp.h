@@ -196,7 +196,8 @@ int krr_potrs(const void* d_factor, const float* d_scales,
  * krr_associate_host -- the whole Associate phase (Alg. 3) from HOST buffers: copies A and Y to the
  * device arena, runs krr_precision_map -> krr_potrf_mp -> krr_potrs, copies alpha, the map and info
  * back, and synchronises `stream` before returning.  Used for end-to-end timing.
- * h_A      in   FP32 n x n row-major (lda) host memory (pinned memory makes the copies asynchronous)
+ * h_A      in   FP32 n x n row-major (lda) host memory (pinned memory makes the copies asynchronous); only the
+ *               lower tiles (tile row i: its first (i+1)*nb columns) are read and copied: 4 nb^2 NT(NT+1)/2 bytes
  * h_Y      in   n x nrhs row-major; h_alpha out n x nrhs; h_map out NT*NT bytes; h_info out 1 int
  * force_prec    < 0: use the rule with (eps_target, allowed_mask); 0..2: uniform off-diagonal map
  * d_arena  device scratch of at least krr_associate_host_arena(n, nb, nrhs) bytes (sized for the

@@ -822,8 +822,10 @@ int krr_associate_host(const float* h_A, int64_t n, int64_t lda, int nb, float e
     uint8_t* ar = static_cast<uint8_t*>(d_arena);
     float* dA = reinterpret_cast<float*>(ar + L.A);
     float* dY = reinterpret_cast<float*>(ar + L.Y);
-    KRR_CUDA_CHECK(cudaMemcpy2DAsync(dA, n * sizeof(float), h_A, lda * sizeof(float), n * sizeof(float), n,
-                                     cudaMemcpyHostToDevice, st));
+    // only the lower tiles are read by the phase: tile row i needs its first (i+1)*nb columns
+    for (int64_t i = 0; i < n / nb; ++i)
+        KRR_CUDA_CHECK(cudaMemcpy2DAsync(dA + i * nb * n, n * sizeof(float), h_A + i * nb * lda, lda * sizeof(float),
+                                         static_cast<size_t>(i + 1) * nb * sizeof(float), nb, cudaMemcpyHostToDevice, st));
     KRR_CUDA_CHECK(cudaMemcpyAsync(dY, h_Y, static_cast<size_t>(n) * nrhs * sizeof(float), cudaMemcpyHostToDevice, st));
     return associate_in_arena(ar, L, n, nb, eps_target, allowed_mask, force_prec, flags, nrhs, h_alpha, h_map, h_info, stream, 0);
 }

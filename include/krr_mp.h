@@ -240,7 +240,17 @@ int krr_band_map(int NT, double fp32_fraction, int low_prec, uint8_t* h_map);
 size_t krr_build_workspace(int64_t n, int64_t p, unsigned flags);
 int krr_build(const int8_t* d_G, int64_t n, int64_t p, int64_t ldg, const float* d_C, int q, int64_t ldc,
               float gamma, float lambda, float* d_A, int64_t lda, int nb, unsigned flags,
-              void* d_ws, size_t ws_bytes, void* stream);
+              void* d_stats, void* d_ws, size_t ws_bytes, void* stream);
+
+/* Tile statistics from the Build epilogue ("tile sum-of-squares emitted in the same epilogue so
+ * krr_precision_map needs no extra pass").  If krr_build is given d_stats (krr_build_stats_bytes(n, nb) bytes, 1024-byte
+ * aligned; NULL: none) every epilogue warp also leaves the FP64 sum of squares and the maximum modulus of its share of A
+ * there; krr_precision_map_from_build then sums them per tile in a fixed order and applies the rule exactly as
+ * krr_precision_map does (same outputs; the norms agree to FP64 summation order).  d_stats is read and partly used as
+ * scratch by krr_precision_map_from_build. */
+size_t krr_build_stats_bytes(int64_t n, int nb);
+int krr_precision_map_from_build(const void* d_stats, int64_t n, int nb, float eps_target, unsigned allowed_mask,
+                                 uint8_t* d_map, float* d_tile_norms, float* d_tile_amax, double* d_fro, void* stream);
 
 /* ---------------------------------------------------------------------------------------------
  * krr_predict -- Predict phase (Alg. 4 :116-122):

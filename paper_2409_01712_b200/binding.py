@@ -25,7 +25,7 @@ ERRORS = {-1: "KRR_ERR_ARG", -2: "KRR_ERR_SHAPE", -3: "KRR_ERR_WORKSPACE", -4: "
 EXPORTS = ["krr_version", "krr_built_for_sm", "krr_tile_slot", "krr_precision_map_workspace",
            "krr_precision_map", "krr_factor_bytes", "krr_factor_tile_offset",
            "krr_potrf_mp_workspace", "krr_potrf_mp", "krr_potrs_workspace", "krr_potrs",
-           "krr_associate_host_arena", "krr_associate_host", "krr_build_workspace", "krr_build", "krr_predict_workspace", "krr_predict", "krr_fit_host_arena", "krr_fit_host", "krr_band_map",
+           "krr_associate_host_arena", "krr_associate_host", "krr_build_workspace", "krr_build", "krr_predict_workspace", "krr_predict", "krr_fit_host_arena", "krr_fit_host", "krr_band_map", "krr_build_stats_bytes", "krr_precision_map_from_build",
            "krr_last_launch_count",
            "krr_profile_enable", "krr_profile_read"]
 
@@ -78,7 +78,11 @@ def lib():
     L.krr_build_workspace.restype = sz
     L.krr_build_workspace.argtypes = [i64, i64, u32]
     L.krr_build.restype = c.c_int
-    L.krr_build.argtypes = [vp, i64, i64, i64, vp, c.c_int, i64, c.c_float, c.c_float, vp, i64, c.c_int, u32, vp, sz, vp]
+    L.krr_build.argtypes = [vp, i64, i64, i64, vp, c.c_int, i64, c.c_float, c.c_float, vp, i64, c.c_int, u32, vp, vp, sz, vp]
+    L.krr_build_stats_bytes.restype = sz
+    L.krr_build_stats_bytes.argtypes = [i64, c.c_int]
+    L.krr_precision_map_from_build.restype = c.c_int
+    L.krr_precision_map_from_build.argtypes = [vp, i64, c.c_int, c.c_float, u32, vp, vp, vp, vp, vp]
     L.krr_predict_workspace.restype = sz
     L.krr_predict_workspace.argtypes = [i64, i64, i64, u32]
     L.krr_predict.restype = c.c_int
@@ -303,7 +307,7 @@ def _conf(C):
     return C, C.shape[1], C.stride(0)
 
 
-def krr_build(G, gamma, lam, nb, tiled_lower=False, out=None, flags=0, C=None):
+def krr_build(G, gamma, lam, nb, tiled_lower=False, out=None, flags=0, C=None, stats=False):
     """krr_build (named in full: `build` is this package's compile step): A = K + lam*I (Gaussian kernel) from CUDA int8 genotypes G (n x p, row-major, row pitch a
     multiple of 16 bytes).  Returns A: n x n FP32 with the lower tiles written (the rest zero), or the packed
     lower tiles with tiled_lower."""
@@ -322,9 +326,26 @@ def krr_build(G, gamma, lam, nb, tiled_lower=False, out=None, flags=0, C=None):
     ws = _ws(wsb, dev)
     lda = nb if tiled_lower else out.stride(0)
     C, q, ldc = _conf(C)
+    st = _ws(int(L.krr_build_stats_bytes(n, nb)), dev) if stats else None
     _check(L.krr_build(_ptr(G), n, p, G.stride(0), _ptr(C), q, ldc, float(gamma), float(lam), _ptr(out), lda, nb, flags,
-                       _ptr(ws), wsb, _stream()), "krr_build")
-    return out
+                       _ptr(st), _ptr(ws), wsb, _stream()), "krr_build")
+    return (out, st) if stats else out
+
+
+def precision_map_from_build(stats, n, nb, eps_target, allowed=(FP32, FP16, FP8)):
+    """krr_precision_map_from_build: the map from the tile statistics krr_build(..., stats=True) left behind.
+    Returns (d_map, tile norms, tile amax, fro) like precision_map."""
+    L = lib()
+    NT = n // nb
+    dev = stats.device
+    d_map = torch.empty((NT, NT), dtype=torch.uint8, device=dev)
+    norms = torch.empty((NT, NT), dtype=torch.float32, device=dev)
+    amax = torch.empty((NT, NT), dtype=torch.float32, device=dev)
+    fro = torch.empty(1, dtype=torch.float64, device=dev)
+    mask = sum(1 << p for p in allowed)
+    _check(L.krr_precision_map_from_build(_ptr(stats), n, nb, float(eps_target), mask, _ptr(d_map), _ptr(norms), _ptr(amax),
+                                          _ptr(fro), _stream()), "krr_precision_map_from_build")
+    return d_map, norms, amax, fro
 
 
 def krr_predict(T, G, gamma, W, return_kernel=False, CT=None, CG=None, flags=0):

@@ -777,7 +777,8 @@ struct Arena {
 Arena arena_layout(int64_t n, int nb, int nrhs);
 }  // namespace
 static int associate_in_arena(uint8_t* ar, const Arena& L, int64_t n, int nb, float eps_target, unsigned allowed_mask, int force_prec,
-                              unsigned flags, int nrhs, float* h_alpha, uint8_t* h_map, int* h_info, void* stream, int64_t launches);
+                              unsigned flags, int nrhs, float* h_alpha, uint8_t* h_map, int* h_info, void* stream, int64_t launches,
+                              const void* build_stats = nullptr);
 namespace {
 Arena arena_layout(int64_t n, int nb, int nrhs) {
     const size_t NT = n / nb, nslots = NT * (NT + 1) / 2;
@@ -834,7 +835,8 @@ int krr_associate_host(const float* h_A, int64_t n, int64_t lda, int nb, float e
 
 // Associate phase on A and Y already in the arena: map -> factorisation -> solve -> alpha, map, info to the host.
 static int associate_in_arena(uint8_t* ar, const Arena& L, int64_t n, int nb, float eps_target, unsigned allowed_mask, int force_prec,
-                              unsigned flags, int nrhs, float* h_alpha, uint8_t* h_map, int* h_info, void* stream, int64_t launches) {
+                              unsigned flags, int nrhs, float* h_alpha, uint8_t* h_map, int* h_info, void* stream, int64_t launches,
+                              const void* build_stats) {
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     float* dA = reinterpret_cast<float*>(ar + L.A);
     float* dY = reinterpret_cast<float*>(ar + L.Y);
@@ -842,9 +844,13 @@ static int associate_in_arena(uint8_t* ar, const Arena& L, int64_t n, int nb, fl
     const int NT = static_cast<int>(n / nb);
     int rc;
     if (force_prec < 0) {
-        rc = krr_precision_map(dA, n, n, nb, eps_target, allowed_mask, flags & KRR_FLAG_PREROUND_A, dmap,
-                               reinterpret_cast<float*>(ar + L.norms), reinterpret_cast<float*>(ar + L.amax),
-                               reinterpret_cast<double*>(ar + L.fro), ar + L.pm_ws, L.potrf_ws - L.pm_ws, stream);
+        if (build_stats)
+            rc = krr_precision_map_from_build(build_stats, n, nb, eps_target, allowed_mask, dmap, reinterpret_cast<float*>(ar + L.norms),
+                                              reinterpret_cast<float*>(ar + L.amax), reinterpret_cast<double*>(ar + L.fro), stream);
+        else
+            rc = krr_precision_map(dA, n, n, nb, eps_target, allowed_mask, flags & KRR_FLAG_PREROUND_A, dmap,
+                                   reinterpret_cast<float*>(ar + L.norms), reinterpret_cast<float*>(ar + L.amax),
+                                   reinterpret_cast<double*>(ar + L.fro), ar + L.pm_ws, L.potrf_ws - L.pm_ws, stream);
         if (rc) return rc;
         launches += g_launches;
         // the launch sequence of the factorisation is built on the host from the map
@@ -879,7 +885,7 @@ static size_t fit_g_bytes(int64_t n, int64_t p) { return align_up(static_cast<si
 
 size_t krr_fit_host_arena(int64_t n, int64_t p, int nb, int nrhs) {
     if (check_shape(n, nb) != KRR_OK || nrhs < 1 || nrhs > kMaxRhs || p < 1 || n % 256 != 0 || nb % 256 != 0) return 0;
-    return arena_layout(n, nb, nrhs).total + fit_g_bytes(n, p) + krr_build_workspace(n, p, 0);
+    return arena_layout(n, nb, nrhs).total + fit_g_bytes(n, p) + krr_build_workspace(n, p, 0) + krr_build_stats_bytes(n, nb);
 }
 
 int krr_fit_host(const int8_t* h_G, int64_t n, int64_t p, int64_t ldg, float gamma, float lambda, int nb, float eps_target,
@@ -900,10 +906,13 @@ int krr_fit_host(const int8_t* h_G, int64_t n, int64_t p, int64_t ldg, float gam
     const int64_t ldd = static_cast<int64_t>(align_up(static_cast<size_t>(p), 16));
     KRR_CUDA_CHECK(cudaMemcpy2DAsync(dG, ldd, h_G, ldg, p, n, cudaMemcpyHostToDevice, st));
     KRR_CUDA_CHECK(cudaMemcpyAsync(ar + L.Y, h_Y, static_cast<size_t>(n) * nrhs * sizeof(float), cudaMemcpyHostToDevice, st));
-    rc = krr_build(dG, n, p, ldd, nullptr, 0, 0, gamma, lambda, reinterpret_cast<float*>(ar + L.A), n, nb, 0, bws,
-                   krr_build_workspace(n, p, 0), stream);
+    // tile statistics from the Build epilogue: the precision map needs no pass of its own over A
+    uint8_t* stats = bws + krr_build_workspace(n, p, 0);
+    rc = krr_build(dG, n, p, ldd, nullptr, 0, 0, gamma, lambda, reinterpret_cast<float*>(ar + L.A), n, nb, 0,
+                   force_prec < 0 ? stats : nullptr, bws, krr_build_workspace(n, p, 0), stream);
     if (rc) return rc;
-    return associate_in_arena(ar, L, n, nb, eps_target, allowed_mask, force_prec, flags, nrhs, h_alpha, h_map, h_info, stream, g_launches);
+    return associate_in_arena(ar, L, n, nb, eps_target, allowed_mask, force_prec, flags, nrhs, h_alpha, h_map, h_info, stream, g_launches,
+                              force_prec < 0 ? stats : nullptr);
 }
 
 }  // extern "C"
@@ -958,8 +967,38 @@ size_t krr_build_workspace(int64_t n, int64_t p, unsigned flags) {
     return b;
 }
 
+static int build_stats_chunks(int nb) { const int upt = nb / 256, nacc = (nb % 512 == 0) ? 2 : 1; return upt * (upt / nacc) * 16; }
+
+size_t krr_build_stats_bytes(int64_t n, int nb) {
+    if (check_shape(n, nb) != KRR_OK || nb % 256 != 0) return 0;
+    const size_t NT = n / nb, nslots = NT * (NT + 1) / 2, chunks = build_stats_chunks(nb);
+    return align_up(nslots * chunks * sizeof(double), 1024) + align_up(nslots * chunks * sizeof(float), 1024) +
+           align_up(nslots * sizeof(double), 1024);
+}
+
+int krr_precision_map_from_build(const void* d_stats, int64_t n, int nb, float eps_target, unsigned allowed_mask, uint8_t* d_map,
+                                 float* d_tile_norms, float* d_tile_amax, double* d_fro, void* stream) {
+    g_launches = 0;
+    if (!d_stats || !d_map) return KRR_ERR_ARG;
+    int rc = check_shape(n, nb);
+    if (rc) return rc;
+    if (nb % 256 != 0) return KRR_ERR_SHAPE;
+    rc = check_device(nullptr);
+    if (rc) return rc;
+    const int NT = static_cast<int>(n / nb);
+    const size_t nslots = static_cast<size_t>(NT) * (NT + 1) / 2, chunks = build_stats_chunks(nb);
+    const uint8_t* sb = static_cast<const uint8_t*>(d_stats);
+    const double* partial = reinterpret_cast<const double*>(sb);
+    const float* pamax = reinterpret_cast<const float*>(sb + align_up(nslots * chunks * sizeof(double), 1024));
+    double* sumsq = reinterpret_cast<double*>(const_cast<uint8_t*>(sb) + align_up(nslots * chunks * sizeof(double), 1024) +
+                                              align_up(nslots * chunks * sizeof(float), 1024));
+    return launch(CAT_MAP, map_decide_kernel, dim3(1), dim3(1024), 0, static_cast<cudaStream_t>(stream), NT, static_cast<int>(chunks),
+                  partial, pamax, eps_target, allowed_mask, d_map, d_tile_norms, d_tile_amax, d_fro, sumsq);
+}
+
 int krr_build(const int8_t* d_G, int64_t n, int64_t p, int64_t ldg, const float* d_C, int q, int64_t ldc, float gamma,
-              float lambda, float* d_A, int64_t lda, int nb, unsigned flags, void* d_ws, size_t ws_bytes, void* stream) {
+              float lambda, float* d_A, int64_t lda, int nb, unsigned flags, void* d_stats, void* d_ws, size_t ws_bytes,
+              void* stream) {
     g_launches = 0;
     if (!d_G || !d_A || !d_ws) return KRR_ERR_ARG;
     if (q < 0 || q > kMaxConfounders || (q > 0 && (!d_C || ldc < q))) return KRR_ERR_ARG;
@@ -1003,6 +1042,12 @@ int krr_build(const int8_t* d_G, int64_t n, int64_t p, int64_t ldg, const float*
     op.diag = static_cast<float>(1.0 + static_cast<double>(lambda));
     op.sq = sq; op.sq_row = sq; op.A = d_A; op.lda = lda;
     op.C = d_C; op.C_row = d_C; op.ldc = ldc; op.ldc_row = ldc; op.q = q;
+    if (d_stats) {
+        const size_t nslots = static_cast<size_t>(n / nb) * (n / nb + 1) / 2, chunks = build_stats_chunks(nb);
+        op.stat_sumsq = static_cast<double*>(d_stats);
+        op.stat_amax = reinterpret_cast<float*>(static_cast<uint8_t*>(d_stats) + align_up(nslots * chunks * sizeof(double), 1024));
+        op.stats_chunks = static_cast<int>(chunks);
+    }
     const int64_t NT = n / nb, upt = nb / 256;
     const int nacc = (nb % 512 == 0) ? 2 : 1;                      // 256 x 512 blocks when a tile holds them
     return launch_build(tmG, tmG, op, upt * upt * NT * (NT + 1) / 2 / nacc, nacc, num_sms, st);

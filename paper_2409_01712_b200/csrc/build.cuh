@@ -42,6 +42,12 @@ struct BuildOp {
     // linear kernel (the SYRK of ridge regression, Eq. (2), Fig. 2): K_ij = gamma * <g_i, g_j>, lambda on the diagonal
     int linear;
     float lambda;
+    // optional tile statistics of A for the precision map (no second pass over A): per lower tile
+    // stats_chunks = (blocks per tile) * 16 partial sums of squares (FP64) and maxima, one per epilogue warp of the
+    // block's two CTAs, in the layout map_decide_kernel reads (precision_map.cuh)
+    double* stat_sumsq;
+    float* stat_amax;
+    int stats_chunks;
 };
 constexpr int kMaxConfounders = 16;
 
@@ -253,6 +259,8 @@ build_tc_kernel(const __grid_constant__ CUtensorMap tmR, const __grid_constant__
             const int64_t gi = static_cast<int64_t>(ru) * 256 + rank * kBlk + q * 32 + lane;       // my row of A
             const int si = op.sq_row[gi];
             const int ti = op.rect ? 0x7fffffff : static_cast<int>(gi / op.nb);
+            double ssq = 0.0;                       // this thread's share of the block's sum of squares / maximum
+            float amx = 0.0f;
             float ci[kMaxConfounders];
 #pragma unroll
             for (int c = 0; c < kMaxConfounders; ++c) ci[c] = (c < op.q) ? __ldg(op.C_row + gi * op.ldc_row + c) : 0.0f;
@@ -299,8 +307,28 @@ build_tc_kernel(const __grid_constant__ CUtensorMap tmR, const __grid_constant__
                             if (!op.rect && gj0 + e + u == gi) kv = op.diag;
                         }
                         v[u] = kv;
+                        ssq += static_cast<double>(kv) * kv;
+                        amx = fmaxf(amx, fabsf(kv));
                     }
                     *reinterpret_cast<float4*>(dst + e) = make_float4(v[0], v[1], v[2], v[3]);
+                }
+            }
+            if (op.stat_sumsq != nullptr && !op.rect) {
+                // fixed-order warp reduction, one partial per (block of the tile, CTA of the pair, epilogue warp)
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) {
+                    ssq += __shfl_xor_sync(0xffffffffu, ssq, o);
+                    amx = fmaxf(amx, __shfl_xor_sync(0xffffffffu, amx, o));
+                }
+                if (lane == 0) {
+                    const int tj = static_cast<int>(static_cast<int64_t>(cu) * 256 * NACC / op.nb);
+                    if (tj <= ti) {
+                        const int upt_ = op.nb / 256, cpt = upt_ / NACC;                 // row / column units per tile
+                        const int bit = (ru % upt_) * cpt + (cu % cpt);                   // block inside the tile
+                        const int64_t idx = tile_slot(NT, ti, tj) * op.stats_chunks + bit * 16 + rank * 8 + ew;
+                        op.stat_sumsq[idx] = ssq;
+                        op.stat_amax[idx] = amx;
+                    }
                 }
             }
             if (++buf == NBUF) { buf = 0; acc_phase ^= 1u; }

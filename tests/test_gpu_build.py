@@ -111,7 +111,7 @@ def test_build_argument_errors(krr):
     A = torch.zeros((512, 512), dtype=torch.float32, device="cuda")
     ws = torch.zeros(1 << 20, dtype=torch.uint8, device="cuda")
     vp = lambda t: ctypes.c_void_p(t.data_ptr())
-    call = lambda n, p, ldg, nb, flags=0: L.krr_build(vp(G), n, p, ldg, None, 0, 0, 0.01, 0.01, vp(A), 512, nb, flags, vp(ws), 1 << 20, None)
+    call = lambda n, p, ldg, nb, flags=0: L.krr_build(vp(G), n, p, ldg, None, 0, 0, 0.01, 0.01, vp(A), 512, nb, flags, None, vp(ws), 1 << 20, None)
     assert call(512, 160, 160, 256) == 0
     assert call(500, 160, 160, 250) == -2            # n, nb not multiples of 256
     assert call(512, 160, 150, 256) == -1            # ldg < p
@@ -295,4 +295,26 @@ def test_linear_kernel_and_ridge_regression(krr):
     P, K = krr.krr_predict(padded(T), padded(Gs), 0.25, W, return_kernel=True, flags=krr.FLAG_KERNEL_LINEAR)
     torch.cuda.synchronize()
     assert np.array_equal(K.cpu().numpy().astype(np.float64), linear_kernel_matrix_definition(T.cpu().numpy(), Gs.cpu().numpy(), 0.25))
+
+
+@pytest.mark.parametrize("name,nb,n,p,eps", [("S1", 256, 2048, 1536, 1e-4), ("C4", 512, 2048, 1500, 1e-3), ("S1", 1024, 4096, 3072, 1e-4)])
+def test_precision_map_from_build_statistics(krr, name, nb, n, p, eps):
+    """tile sums of squares from the Build epilogue, so that the precision map needs no pass of its own
+    over A.  Against krr_precision_map on the matrix the same call produced: the same map bit for bit, tile norms and
+    ||A||_F to FP64 summation order, tile maxima exactly; and against the oracle's rule on that matrix."""
+    from oracle.precision_map import precision_map as oracle_map
+    cfg = scaled_config(CONFIGS[name], nb=nb, n=n, p=p)
+    G = genotypes(cfg.seed, cfg.n, cfg.p, cfg.genotype, device="cuda")
+    A, st = krr.krr_build(padded(G), cfg.gamma, cfg.lam, nb, stats=True)
+    m1, n1, a1, f1 = krr.precision_map_from_build(st, n, nb, eps)
+    m2, n2, a2, f2 = krr.precision_map(A, nb, eps)
+    torch.cuda.synchronize()
+    assert torch.equal(m1, m2)
+    assert torch.equal(a1, a2)
+    assert abs(float(f1) - float(f2)) <= 1e-12 * float(f2)
+    assert float((n1 - n2).abs().max()) <= 2e-7 * float(n2.max())
+    # the upper tiles of A are zero here, so the oracle sees the same lower tiles
+    pm, _, _ = oracle_map(A.cpu().numpy(), nb, eps)
+    low = np.tril_indices(n // nb)
+    assert np.array_equal(m1.cpu().numpy()[low], pm[low])
 

@@ -304,8 +304,14 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
 
     const bool has_acc = (op.mode != MODE_UPDATE) ? (op.mode != MODE_P1 || op.c > 0) : (nterms > 0);
     const bool write_planes = (op.mode != MODE_UPDATE) || op.planes;
-    // MODE_PANEL: completed epilogue warps of this CTA's item sequence (8 per item), polled by the producer
-    volatile int* done_ctr = reinterpret_cast<volatile int*>(tmem_slot_ptr + 2);
+    // Completion of this CTA's items, counted PER ITEM: slot q % 8 receives one arrival from every epilogue warp when it
+    // has stored its share of item q (items q, q + 8, ... share a slot: item q is complete when the slot holds
+    // 8 (q / 8 + 1); an epilogue warp is never more than the number of TMEM buffers ahead of another, so slots cannot
+    // alias).  A single running total would not do: a fast warp's arrival for item q + 1 could stand in for a slow
+    // warp's missing arrival for item q.
+    volatile int* item_ctr = reinterpret_cast<volatile int*>(tmem_slot_ptr + 2);
+    auto item_complete_count = [](int q) { return kEpiWarps * (q / 8 + 1); };
+    int* split_ctr = reinterpret_cast<int*>(tmem_slot_ptr + 10);     // arrivals for this CTA's (single) split block
 
     if (warp == 0 && lane == 0) {
         ptx::prefetch_tmap(&tmH);
@@ -320,7 +326,8 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
             ptx::mbar_init(tfull_bar(b), 1);
             ptx::mbar_init(tempty_bar(b), kEpiWarps * CG);
         }
-        *done_ctr = 0;
+        for (int i = 0; i < 8; ++i) item_ctr[i] = 0;
+        *split_ctr = 0;
         ptx::fence_mbar_init();
     }
     if (warp == 1) {
@@ -362,9 +369,9 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
                 if (w.mode == MODE_POTRF) { ++seq; continue; }
                 if (w.dep) {
                     // the operand images this item reads were written by this CTA's epilogue warps `dep` items ago
-                    const int need = kEpiWarps * (seq - w.dep + 1);
+                    const int qd = seq - w.dep;
                     uint32_t spins = 0;
-                    while (*done_ctr < need) { if (++spins > (1u << 27)) __trap(); }
+                    while (item_ctr[qd & 7] < item_complete_count(qd)) { if (++spins > (1u << 27)) __trap(); }
                     __threadfence();
                     ptx::fence_proxy_async_global();
                 }
@@ -684,8 +691,8 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
                 __threadfence();
                 __syncwarp();
                 if (lane == 0) {
-                    const int old = atomicAdd_block(const_cast<int*>(done_ctr), 1);
-                    if (old % kEpiWarps == kEpiWarps - 1) { __threadfence(); atomicAdd(op.split_flags + w.fidx, 1); }
+                    // (a CTA holds at most one slice of a split block: its last item)
+                    if (atomicAdd_block(split_ctr, 1) == kEpiWarps - 1) { __threadfence(); atomicAdd(op.split_flags + w.fidx, 1); }
                 }
             }
             if (op.mode == MODE_PANEL || op.mode == MODE_DIAG) {
@@ -695,8 +702,8 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
                 ptx::fence_proxy_async_global();
                 __syncwarp();
                 if (lane == 0) {
-                    const int old = atomicAdd_block(const_cast<int*>(done_ctr), 1);
-                    if (op.mode == MODE_DIAG && old == kEpiWarps * (eseq + 1) - 1) {
+                    const int old = atomicAdd_block(const_cast<int*>(item_ctr + (eseq & 7)), 1);
+                    if (op.mode == MODE_DIAG && old == item_complete_count(eseq) - 1) {
                         __threadfence();
                         *const_cast<volatile int*>(op.prog + (rb - op.rb0)) = eseq + 1;
                     }

@@ -39,3 +39,29 @@ def solve_fp64(A, Y, nb):
     if info:
         raise np.linalg.LinAlgError(f"matrix not positive definite (info={info})")
     return potrs_fp64(L, Y, nb)
+
+
+def refine(A, L, Y, alpha, nb, steps, round_fp32=True):
+    """Iterative refinement with a fixed (mixed-precision) factor: for s = 0 .. steps-1
+         r_s = Y - A alpha_s,   alpha_{s+1} = alpha_s + (L L^T)^{-1} r_s.
+    The paper names the technique ("mixed-precision techniques have been made popular with iterative
+    refinement ... recovers all digits of accuracy") and does not adopt it; SURVEY section 8(c) offers it as the remedy
+    for the alpha tolerance under FP16 / FP8 maps (R19).  With round_fp32 the residual and the iterate are
+    rounded to FP32 where the method stores them (r_s after the FP64 evaluation, alpha_{s+1} after the update); the
+    correction itself is solved in FP64.  Returns (alpha_steps, [||r_0||_F, ..., ||r_steps||_F]), the norms taken of
+    the residuals as stored."""
+    A = np.asarray(A, dtype=np.float64)
+    Y = np.asarray(Y, dtype=np.float64)
+    x = np.array(alpha, dtype=np.float64, copy=True)
+    if x.ndim == 1:
+        x = x[:, None]
+    if Y.ndim == 1:
+        Y = Y[:, None]
+    rnd = (lambda v: v.astype(np.float32).astype(np.float64)) if round_fp32 else (lambda v: v)
+    norms = []
+    for _ in range(steps):
+        r = rnd(Y - A @ x)
+        norms.append(float(np.linalg.norm(r)))
+        x = rnd(x + potrs_fp64(L, r, nb))
+    norms.append(float(np.linalg.norm(rnd(Y - A @ x))))
+    return x, norms

@@ -172,3 +172,73 @@ def test_band_map_reading():
     # monotone in the fraction
     assert all((band_map(9, f1, FP16) <= band_map(9, f2, FP16)).all() for f1, f2 in [(0.8, 0.6), (0.6, 0.2), (0.2, 0.1)])
 
+
+
+# ---- iterative refinement with a fixed factor (oracle.solve.refine; R19) ----
+def _spd(n, seed, lam=0.5):
+    rng = np.random.default_rng(seed)
+    B = rng.standard_normal((n, n))
+    A = B @ B.T / n + lam * np.eye(n)
+    return A, rng
+
+
+def test_refine_with_the_exact_factor_is_one_solve():
+    from oracle.solve import refine
+    n, nb = 96, 32
+    A, rng = _spd(n, 3)
+    Y = rng.standard_normal((n, 3))
+    L = np.linalg.cholesky(A)
+    x, norms = refine(A, L, Y, np.zeros_like(Y), nb, 1, round_fp32=False)
+    np.testing.assert_allclose(x, np.linalg.solve(A, Y), rtol=1e-11, atol=1e-12)
+    assert abs(norms[0] - np.linalg.norm(Y)) <= 1e-12 * np.linalg.norm(Y)      # r_0 = Y when alpha_0 = 0
+    assert norms[1] <= 1e-12 * norms[0]
+    # no step: the iterate comes back untouched and the one norm is that of Y - A alpha
+    x0 = rng.standard_normal((n, 3))
+    x, norms = refine(A, L, Y, x0, nb, 0, round_fp32=False)
+    assert np.array_equal(x, x0) and len(norms) == 1
+    assert abs(norms[0] - np.linalg.norm(Y - A @ x0)) <= 1e-12 * norms[0]
+
+
+def test_refine_error_follows_the_iteration_matrix():
+    """Textbook: with a factor of a perturbed matrix At = L L^T the error obeys e_{s+1} = (I - At^{-1} A) e_s.
+    Checked against explicit powers of that matrix (numpy inverse; nothing of the oracle's solve in the expected
+    value): a wrong sign of the update, a residual taken with At instead of A, or a stale alpha fails it."""
+    from oracle.solve import refine
+    n, nb = 64, 16
+    A, rng = _spd(n, 5)
+    E = rng.standard_normal((n, n)) * 2e-2
+    At = A + (E + E.T) / 2
+    L = np.linalg.cholesky(At)
+    Y = rng.standard_normal((n, 2))
+    xstar = np.linalg.solve(A, Y)
+    x0 = rng.standard_normal((n, 2))
+    M = np.eye(n) - np.linalg.inv(At) @ A
+    e = x0 - xstar
+    for steps in (1, 2, 4):
+        x, norms = refine(A, L, Y, x0, nb, steps, round_fp32=False)
+        want = np.linalg.matrix_power(M, steps) @ e
+        np.testing.assert_allclose(x - xstar, want, rtol=1e-8, atol=1e-12 * np.abs(e).max())
+        assert len(norms) == steps + 1
+        for s in range(steps + 1):                                              # r_s = -A e_s
+            rs = -A @ (np.linalg.matrix_power(M, s) @ e)
+            assert abs(norms[s] - np.linalg.norm(rs)) <= 1e-8 * np.linalg.norm(rs)
+
+
+def test_refine_recovers_alpha_under_a_half_precision_map():
+    """an all-FP16 map misses "alpha to 1e-3" raw and meets it after <= 2 steps.  Here on a
+    scaled twin of C4 with the emulated factor; the limit of the FP32-stored iterate is FP32 roundoff."""
+    from oracle.solve import refine
+    cfg = scaled_config(CONFIGS["C4"], nb=64, n=1024, p=256)
+    A, Y = make_problem(cfg, device="cpu")
+    A, Y = A.numpy().astype(np.float64), Y.numpy().astype(np.float64)
+    pm = uniform_map(cfg.NT, R.FP16)
+    L, sc, info = tile_cholesky_emulated(A, cfg.nb, pm, preround_a=True)
+    assert info == 0
+    xstar = np.linalg.solve(A, Y)
+    err = lambda x: np.linalg.norm(x - xstar) / np.linalg.norm(xstar)
+    x0 = potrs_fp64(L, Y, cfg.nb)
+    x2, norms = refine(A, L, Y, x0, cfg.nb, 2)
+    assert err(x0) > 5e-3 and err(x2) < 5e-5 and err(x2) < 1e-2 * err(x0)          # SURVEY: 1.5e-2 -> ~2e-5
+    assert norms[1] < 0.2 * norms[0] and norms[2] < 0.2 * norms[1]
+    x6, _ = refine(A, L, Y, x0, cfg.nb, 6)
+    assert err(x6) < 2e-6                                                        # FP32 storage of alpha

@@ -193,6 +193,34 @@ int krr_potrs(const void* d_factor, const float* d_scales,
               void* d_ws, size_t ws_bytes, void* stream);
 
 /* ---------------------------------------------------------------------------------------------
+ * krr_refine -- iterative refinement of alpha with the factor kept fixed (R19).  The paper
+ * names the technique and does not adopt it; it is the remedy SURVEY section 8(c)
+ * offers where an FP16 / FP8 map misses "alpha to 1e-3".  A call beside the path: krr_potrf_mp and
+ * krr_potrs never refine.  For s = 0 .. steps-1:
+ *     R = fl32(Y - A X)   A, X in FP32, every product and sum in FP64, rounded once;
+ *     D = krr_potrs(factor, R);   X = fl32(X + D).
+ * d_A      in      as for krr_precision_map (dense row-major with lda, or KRR_FLAG_A_TILED_LOWER); only
+ *                  the lower tiles are read, the diagonal blocks through their lower triangles.
+ * d_factor, d_scales, d_map, h_map   in   the factor, as for krr_potrs.
+ * d_Y      in      n x nrhs FP32 row-major, leading dimension ldy >= nrhs.
+ * d_X      in/out  n x nrhs FP32 row-major, ldx >= nrhs: in alpha_0 (e.g. the result of krr_potrs), out
+ *                  alpha_steps.  nrhs as for krr_potrs.
+ * steps    0 .. 64.
+ * d_resid  out     NULL, or steps + 1 doubles (device): d_resid[s] = ||fl32(Y - A alpha_s)||_F; asking for
+ *                  them costs one more residual evaluation (that of alpha_steps).
+ * d_ws     workspace of at least krr_refine_workspace(n, nb, nrhs) bytes, 1024-byte aligned.
+ * flags    KRR_FLAG_A_TILED_LOWER only.
+ * The residual is a fixed-order sum (deterministic).  Cost per step: the lower tiles of A read twice
+ * (4 n^2 bytes), 2 n^2 nrhs FP64 flops, one krr_potrs.
+ */
+size_t krr_refine_workspace(int64_t n, int nb, int nrhs);
+int krr_refine(const float* d_A, int64_t n, int64_t lda, int nb,
+               const void* d_factor, const float* d_scales, const uint8_t* d_map, const uint8_t* h_map,
+               const float* d_Y, int64_t ldy, float* d_X, int64_t ldx, int nrhs,
+               int steps, double* d_resid,
+               void* d_ws, size_t ws_bytes, unsigned flags, void* stream);
+
+/* ---------------------------------------------------------------------------------------------
  * krr_associate_host -- the whole Associate phase (Alg. 3) from HOST buffers: copies A and Y to the
  * device arena, runs krr_precision_map -> krr_potrf_mp -> krr_potrs, copies alpha, the map and info
  * back, and synchronises `stream` before returning.  Used for end-to-end timing.

@@ -7,7 +7,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libkrr_mp.so")
 SOURCES = ["api.cu"]
-HEADERS = ["common.cuh", "ptx.cuh", "build.cuh", "gemm_tc.cuh", "panel.cuh", "potrs.cuh", "precision_map.cuh", "tri128.cuh"]
+HEADERS = sorted(f for f in os.listdir(CSRC) if f.endswith(".cuh"))
 
 
 def _nvcc():

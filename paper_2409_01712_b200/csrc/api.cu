@@ -14,6 +14,7 @@
 #include "panel.cuh"
 #include "potrs.cuh"
 #include "precision_map.cuh"
+#include "refine.cuh"
 #include "tri128.cuh"
 
 namespace krr {
@@ -765,6 +766,99 @@ int krr_potrs(const void* d_factor, const float* d_scales, const uint8_t* d_map,
         case 16: return potrs_run<16>(factor, d_scales, d_map, hoff, off, dinv, dinvT, NT, nb, d_B, ldb, nrhs, num_sms, st);
         default: return potrs_run<32>(factor, d_scales, d_map, hoff, off, dinv, dinvT, NT, nb, d_B, ldb, nrhs, num_sms, st);
     }
+}
+
+}  // extern "C"
+
+// ------------------------------------------------------------------------- iterative refinement (R19)
+namespace {
+struct RefineWs { size_t potrs, R, partial, blk, total; };
+RefineWs refine_ws_layout(int64_t n, int nb, int nrhs) {
+    RefineWs w;
+    const size_t NR = static_cast<size_t>(rhs_class(nrhs));
+    size_t o = 0;
+    w.potrs = o;   o = align_up(o + potrs_ws_layout(n, nb).total, 1024);
+    w.R = o;       o = align_up(o + static_cast<size_t>(n) * nrhs * sizeof(float), 1024);
+    w.partial = o; o = align_up(o + static_cast<size_t>(resid_segments(n)) * n * NR * sizeof(double), 1024);
+    w.blk = o;     o = align_up(o + (static_cast<size_t>(n) * NR / 256 + 1) * sizeof(double), 1024);
+    w.total = o;
+    return w;
+}
+
+template <int NR>
+int residual_run(const AView& av, const float* X, int64_t ldx, const float* Y, int64_t ldy, int64_t n, int nrhs,
+                 float* R, double* partial, double* blk, double* d_norm, cudaStream_t st) {
+    const int nblk = static_cast<int>(n / kBlk), nseg = resid_segments(n);
+    int rc = launch(CAT_MISC, resid_partial_kernel<NR>, dim3(nblk, nseg), dim3(ResidCfg<NR>::NTHR), 0, st, av, X, ldx, nrhs,
+                    nblk, nseg, partial);
+    if (rc) return rc;
+    const int64_t nfin = (n * NR + 255) / 256;
+    rc = launch(CAT_MISC, resid_finish_kernel<NR>, dim3(static_cast<unsigned>(nfin)), dim3(256), 0, st,
+                static_cast<const double*>(partial), nseg, n, Y, ldy, R, nrhs, blk);
+    if (rc) return rc;
+    if (d_norm) rc = launch(CAT_MISC, resid_norm_kernel, dim3(1), dim3(256), 0, st, static_cast<const double*>(blk), nfin, d_norm);
+    return rc;
+}
+}  // namespace
+
+extern "C" {
+
+size_t krr_refine_workspace(int64_t n, int nb, int nrhs) {
+    if (krr_potrs_workspace(n, nb, nrhs) == 0) return 0;
+    return refine_ws_layout(n, nb, nrhs).total;
+}
+
+int krr_refine(const float* d_A, int64_t n, int64_t lda, int nb, const void* d_factor, const float* d_scales,
+               const uint8_t* d_map, const uint8_t* h_map, const float* d_Y, int64_t ldy, float* d_X, int64_t ldx,
+               int nrhs, int steps, double* d_resid, void* d_ws, size_t ws_bytes, unsigned flags, void* stream) {
+    g_launches = 0;
+    if (!d_A || !d_factor || !d_scales || !d_map || !h_map || !d_Y || !d_X || !d_ws) return KRR_ERR_ARG;
+    int rc = check_shape(n, nb);
+    if (rc) return rc;
+    const bool tiled = (flags & KRR_FLAG_A_TILED_LOWER) != 0;
+    if ((flags & ~static_cast<unsigned>(KRR_FLAG_A_TILED_LOWER)) != 0) return KRR_ERR_ARG;
+    if (nrhs < 1 || nrhs > kMaxRhs || ldy < nrhs || ldx < nrhs || steps < 0 || steps > 64) return KRR_ERR_ARG;
+    if (!tiled && lda < n) return KRR_ERR_ARG;
+    if (static_cast<int64_t>(rhs_class(nrhs)) * nb > 32768) return KRR_ERR_SHAPE;
+    if (reinterpret_cast<uintptr_t>(d_ws) % 1024 != 0) return KRR_ERR_ARG;
+    const RefineWs L = refine_ws_layout(n, nb, nrhs);
+    if (ws_bytes < L.total) return KRR_ERR_WORKSPACE;
+    rc = check_device(nullptr);
+    if (rc) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    uint8_t* ws = static_cast<uint8_t*>(d_ws);
+    float* R = reinterpret_cast<float*>(ws + L.R);
+    double* partial = reinterpret_cast<double*>(ws + L.partial);
+    double* blk = reinterpret_cast<double*>(ws + L.blk);
+    AView av{d_A, lda, tiled ? 1 : 0, static_cast<int>(n / nb), nb};
+    int64_t launches = 0;
+    auto residual = [&](double* d_norm) -> int {
+        switch (rhs_class(nrhs)) {
+            case 4:  return residual_run<4>(av, d_X, ldx, d_Y, ldy, n, nrhs, R, partial, blk, d_norm, st);
+            case 8:  return residual_run<8>(av, d_X, ldx, d_Y, ldy, n, nrhs, R, partial, blk, d_norm, st);
+            case 16: return residual_run<16>(av, d_X, ldx, d_Y, ldy, n, nrhs, R, partial, blk, d_norm, st);
+            default: return residual_run<32>(av, d_X, ldx, d_Y, ldy, n, nrhs, R, partial, blk, d_norm, st);
+        }
+    };
+    for (int s = 0; s < steps; ++s) {
+        rc = residual(d_resid ? d_resid + s : nullptr);
+        if (rc) return rc;
+        launches += g_launches;
+        rc = krr_potrs(d_factor, d_scales, d_map, h_map, n, nb, R, nrhs, nrhs, ws + L.potrs, L.R - L.potrs, stream);   // resets the counter
+        if (rc) return rc;
+        const int64_t ne = n * nrhs;
+        rc = launch(CAT_MISC, refine_update_kernel, dim3(static_cast<unsigned>((ne + 255) / 256)), dim3(256), 0, st, d_X, ldx,
+                    static_cast<const float*>(R), n, nrhs);
+        if (rc) return rc;
+        launches += g_launches;
+        g_launches = 0;
+    }
+    if (d_resid) {
+        rc = residual(d_resid + steps);
+        if (rc) return rc;
+    }
+    g_launches += launches;
+    return KRR_OK;
 }
 
 }  // extern "C"

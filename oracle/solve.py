@@ -65,3 +65,43 @@ def refine(A, L, Y, alpha, nb, steps, round_fp32=True):
         x = rnd(x + potrs_fp64(L, r, nb))
     norms.append(float(np.linalg.norm(rnd(Y - A @ x))))
     return x, norms
+
+
+def pcg(A, L, Y, alpha, nb, iters, round_fp32=True):
+    """Conjugate gradients on A alpha = Y preconditioned by the fixed factor, M = L L^T (the textbook method of
+    Hestenes and Stiefel with a preconditioner, every right-hand side on its own), started from `alpha`:
+         r_0 = Y - A alpha_0,  z_0 = M^{-1} r_0,  p_0 = z_0,  rho_0 = r_0 . z_0
+         q_k = A p_k,  a_k = rho_k / (p_k . q_k),  alpha_{k+1} = alpha_k + a_k p_k,  r_{k+1} = r_k - a_k q_k,
+         z_{k+1} = M^{-1} r_{k+1},  rho_{k+1} = r_{k+1} . z_{k+1},  p_{k+1} = z_{k+1} + (rho_{k+1} / rho_k) p_k.
+    The stationary iteration of `refine` contracts only while the spectral radius of I - M^{-1} A is below one, which
+    an FP16 map loses at C4's size (R20); CG with the same M converges for every SPD A and M, at the same
+    cost per step (one product with A, one solve with L).  With round_fp32 the quantities the method keeps in FP32
+    are rounded there: the right-hand side of the solve with L, the direction p, the returned alpha; everything else
+    is FP64.  A column with p.q <= 0 or rho = 0 stops moving (a = 0, new direction z).  Returns (alpha_iters,
+    [||r_0||_F, ..., ||r_iters||_F]) with r_k the recursively updated residuals."""
+    A = np.asarray(A, dtype=np.float64)
+    Y = np.asarray(Y, dtype=np.float64)
+    x = np.array(alpha, dtype=np.float64, copy=True)
+    if x.ndim == 1:
+        x = x[:, None]
+    if Y.ndim == 1:
+        Y = Y[:, None]
+    rnd = (lambda v: v.astype(np.float32).astype(np.float64)) if round_fp32 else (lambda v: v)
+    r = Y - A @ x
+    z = potrs_fp64(L, rnd(r), nb)
+    p = rnd(z)
+    rho = np.sum(r * z, axis=0)
+    norms = [float(np.linalg.norm(r))]
+    for _ in range(iters):
+        q = A @ p
+        pq = np.sum(p * q, axis=0)
+        a = np.where(pq > 0.0, rho / np.where(pq > 0.0, pq, 1.0), 0.0)
+        x = x + a[None, :] * p
+        r = r - a[None, :] * q
+        norms.append(float(np.linalg.norm(r)))
+        z = potrs_fp64(L, rnd(r), nb)
+        rho_new = np.sum(r * z, axis=0)
+        b = np.where(rho > 0.0, rho_new / np.where(rho > 0.0, rho, 1.0), 0.0)
+        p = rnd(z + b[None, :] * p)
+        rho = rho_new
+    return rnd(x), norms

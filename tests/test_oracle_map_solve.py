@@ -242,3 +242,73 @@ def test_refine_recovers_alpha_under_a_half_precision_map():
     assert norms[1] < 0.2 * norms[0] and norms[2] < 0.2 * norms[1]
     x6, _ = refine(A, L, Y, x0, cfg.nb, 6)
     assert err(x6) < 2e-6                                                        # FP32 storage of alpha
+
+
+# ---- conjugate gradients preconditioned by the fixed factor (oracle.solve.pcg; R20) ----
+def test_pcg_with_the_exact_factor_is_one_step():
+    from oracle.solve import pcg
+    n, nb = 96, 32
+    A, rng = _spd(n, 7)
+    Y = rng.standard_normal((n, 3))
+    x0 = rng.standard_normal((n, 3))
+    x, norms = pcg(A, np.linalg.cholesky(A), Y, x0, nb, 1, round_fp32=False)
+    np.testing.assert_allclose(x, np.linalg.solve(A, Y), rtol=1e-10, atol=1e-12)
+    assert abs(norms[0] - np.linalg.norm(Y - A @ x0)) <= 1e-12 * norms[0] and norms[1] <= 1e-10 * norms[0]
+    x, norms = pcg(A, np.linalg.cholesky(A), Y, x0, nb, 0, round_fp32=False)
+    assert np.array_equal(x, x0) and len(norms) == 1
+
+
+def test_pcg_iterates_minimise_the_energy_norm_over_the_krylov_space():
+    """What defines CG: alpha_k = alpha_0 + the element of span{M^-1 r_0, (M^-1 A) M^-1 r_0, ...} (k vectors) that
+    minimises ||alpha* - alpha||_A.  The expected iterate is built from that definition by dense least squares on an
+    explicitly generated Krylov basis (numpy inverse, eigendecomposition square root): nothing of the recurrence."""
+    from oracle.solve import pcg
+    n, nb = 48, 16
+    A, rng = _spd(n, 11, lam=0.2)
+    E = rng.standard_normal((n, n)) * 0.05
+    Mt = A + (E + E.T) / 2 + 0.3 * np.eye(n)                     # an SPD preconditioner that is not A
+    L = np.linalg.cholesky(Mt)
+    Y = rng.standard_normal((n, 2))
+    x0 = rng.standard_normal((n, 2))
+    xstar = np.linalg.solve(A, Y)
+    w, V = np.linalg.eigh(A)
+    Ah = V @ np.diag(np.sqrt(w)) @ V.T                           # A^(1/2)
+    Minv = np.linalg.inv(Mt)
+    for k in (1, 2, 5):
+        x, _ = pcg(A, L, Y, x0, nb, k, round_fp32=False)
+        for c in range(2):
+            v = Minv @ (Y[:, c] - A @ x0[:, c])
+            basis = [v]
+            for _ in range(k - 1):
+                basis.append(Minv @ (A @ basis[-1]))
+            Kb, _ = np.linalg.qr(np.stack(basis, axis=1))
+            coef, *_ = np.linalg.lstsq(Ah @ Kb, Ah @ (xstar[:, c] - x0[:, c]), rcond=None)
+            want = x0[:, c] + Kb @ coef
+            np.testing.assert_allclose(x[:, c], want, rtol=1e-7, atol=1e-9)
+
+
+def test_pcg_converges_where_the_stationary_iteration_diverges():
+    """A factor of a matrix far enough from A that the spectral radius of I - M^-1 A exceeds one (what the all-FP16 map
+    does to C4 at full size, R20): `refine` grows the error, `pcg` with the same factor reduces the energy
+    norm of the error at every step and reaches FP32 roundoff."""
+    from oracle.solve import pcg, refine
+    n, nb = 128, 32
+    A, rng = _spd(n, 13, lam=0.05)
+    w, V = np.linalg.eigh(A)
+    scale = np.where(np.arange(n) % 3 == 0, 0.35 + 0.6 * rng.random(n), 1.0 + 0.1 * rng.standard_normal(n))
+    Mt = V @ np.diag(w * scale) @ V.T                          # eigenvalues of M^-1 A spread over (0.8, 2.9)
+    L = np.linalg.cholesky(Mt)
+    assert np.max(np.abs(np.linalg.eigvals(np.eye(n) - np.linalg.inv(Mt) @ A))) > 1.2
+    Y = rng.standard_normal((n, 2))
+    xstar = np.linalg.solve(A, Y)
+    x0 = potrs_fp64(L, Y, nb)
+    enorm = lambda x: float(np.sqrt(np.sum((x - xstar) * (A @ (x - xstar)))))
+    xr, _ = refine(A, L, Y, x0, nb, 12)
+    assert enorm(xr) > 5.0 * enorm(x0)
+    prev = enorm(x0)
+    for k in range(1, 5):
+        xk, _ = pcg(A, L, Y, x0, nb, k, round_fp32=False)
+        assert enorm(xk) < prev
+        prev = enorm(xk)
+    x, norms = pcg(A, L, Y, x0, nb, 12)
+    assert np.linalg.norm(x - xstar) <= 1e-5 * np.linalg.norm(xstar) and norms[-1] < 1e-5 * norms[0]

@@ -265,6 +265,16 @@ def run_ours(args, rank, world, local_rank):
                                          "solve_residual": solve_residual(A_chk, Xr, Y),
                                          "correction_rel": float(torch.linalg.norm((Xr - keep["alpha"]).double())
                                                                  / torch.linalg.norm(Xr.double()))}
+            # krr_pcg (R20): the same factor as a preconditioner -- converges where refinement does not (C4)
+            Xc = keep["alpha"].clone()
+            r0.record()
+            Xc, cn = krr.pcg(A, keep["F"], Y, Xc, 8, tiled_lower=tiled)
+            r1.record()
+            torch.cuda.synchronize()
+            checks["pcg_8_steps"] = {"residual_norms": [float(v) for v in cn], "ms": round(r0.elapsed_time(r1), 2),
+                                     "solve_residual": solve_residual(A_chk, Xc, Y),
+                                     "correction_rel": float(torch.linalg.norm((Xc - keep["alpha"]).double())
+                                                             / torch.linalg.norm(Xc.double()))}
     except Exception as ex:                      # checking only; never masks the measurement
         checks["error"] = repr(ex)
 

@@ -221,6 +221,29 @@ int krr_refine(const float* d_A, int64_t n, int64_t lda, int nb,
                void* d_ws, size_t ws_bytes, unsigned flags, void* stream);
 
 /* ---------------------------------------------------------------------------------------------
+ * krr_pcg -- conjugate gradients on A alpha = Y preconditioned by the fixed factor, M = L L^T
+ * (R20).  krr_refine contracts only while the spectral radius of I - M^-1 A is below one;
+ * with the all-FP16 map the rule gives C4 it is not at n = 131072 (measured).  CG with the same M
+ * converges for every SPD A and M at the same cost per step: one product with A (FP64 sums), one
+ * krr_potrs.  Textbook recurrence, every right-hand side with its own scalars, started from d_X:
+ *     r = Y - A x,  z = M^-1 fl32(r),  p = z,  rho = r.z;   then `iters` times
+ *     q = A p,  a = rho / p.q,  x += a p,  r -= a q,  z = M^-1 fl32(r),  rho' = r.z,  p = fl32(z + (rho'/rho) p).
+ * x, r, q and the inner products are FP64 (workspace); p and z FP32; a right-hand side with p.q <= 0 or
+ * rho = 0 stops moving.  Arguments as for krr_refine, with
+ * iters    0 .. 1024;
+ * d_resid  out  NULL, or iters + 1 doubles: d_resid[k] = ||r_k||_F of the recursively updated residuals
+ *               (no extra product with A).
+ * d_ws     at least krr_pcg_workspace(n, nb, nrhs) bytes, 1024-byte aligned.
+ * Deterministic (fixed-order sums).
+ */
+size_t krr_pcg_workspace(int64_t n, int nb, int nrhs);
+int krr_pcg(const float* d_A, int64_t n, int64_t lda, int nb,
+            const void* d_factor, const float* d_scales, const uint8_t* d_map, const uint8_t* h_map,
+            const float* d_Y, int64_t ldy, float* d_X, int64_t ldx, int nrhs,
+            int iters, double* d_resid,
+            void* d_ws, size_t ws_bytes, unsigned flags, void* stream);
+
+/* ---------------------------------------------------------------------------------------------
  * krr_associate_host -- the whole Associate phase (Alg. 3) from HOST buffers: copies A and Y to the
  * device arena, runs krr_precision_map -> krr_potrf_mp -> krr_potrs, copies alpha, the map and info
  * back, and synchronises `stream` before returning.  Used for end-to-end timing.

@@ -24,7 +24,7 @@ ERRORS = {-1: "KRR_ERR_ARG", -2: "KRR_ERR_SHAPE", -3: "KRR_ERR_WORKSPACE", -4: "
 
 EXPORTS = ["krr_version", "krr_built_for_sm", "krr_tile_slot", "krr_precision_map_workspace",
            "krr_precision_map", "krr_factor_bytes", "krr_factor_tile_offset",
-           "krr_potrf_mp_workspace", "krr_potrf_mp", "krr_potrs_workspace", "krr_potrs", "krr_refine_workspace", "krr_refine",
+           "krr_potrf_mp_workspace", "krr_potrf_mp", "krr_potrs_workspace", "krr_potrs", "krr_refine_workspace", "krr_refine", "krr_pcg_workspace", "krr_pcg",
            "krr_associate_host_arena", "krr_associate_host", "krr_build_workspace", "krr_build", "krr_predict_workspace", "krr_predict", "krr_fit_host_arena", "krr_fit_host", "krr_band_map", "krr_build_stats_bytes", "krr_precision_map_from_build",
            "krr_last_launch_count",
            "krr_profile_enable", "krr_profile_read"]
@@ -75,6 +75,10 @@ def lib():
     L.krr_refine.restype = c.c_int
     L.krr_refine.argtypes = [vp, i64, i64, c.c_int, vp, vp, vp, vp, vp, i64, vp, i64, c.c_int, c.c_int, vp, vp, sz,
                              c.c_uint, vp]
+    L.krr_pcg_workspace.restype = sz
+    L.krr_pcg_workspace.argtypes = [i64, c.c_int, c.c_int]
+    L.krr_pcg.restype = c.c_int
+    L.krr_pcg.argtypes = L.krr_refine.argtypes
     L.krr_associate_host_arena.restype = sz
     L.krr_associate_host_arena.argtypes = [i64, c.c_int, c.c_int]
     L.krr_associate_host.restype = c.c_int
@@ -301,6 +305,27 @@ def refine(A, factor, Y, X, steps, tiled_lower=False, residual_norms=True):
                         _ptr(factor.h_map), _ptr(Y), Y.stride(0), _ptr(X), X.stride(0), nrhs, steps,
                         _ptr(norms) if residual_norms else None, _ptr(ws), wsb,
                         FLAG_A_TILED_LOWER if tiled_lower else 0, _stream()), "krr_refine")
+    return X, norms
+
+
+def pcg(A, factor, Y, X, iters, tiled_lower=False, residual_norms=True):
+    """krr_pcg: `iters` steps of conjugate gradients on A X = Y preconditioned by the factor, started from X (in place;
+    DESIGN.md R20).  Arguments and result as for `refine`; the norms are those of the recursively updated residuals."""
+    L = lib()
+    assert A.dtype == torch.float32 and A.is_cuda
+    assert Y.dtype == torch.float32 and Y.is_cuda and Y.stride(1) == 1
+    assert X.dtype == torch.float32 and X.is_cuda and X.stride(1) == 1 and X.shape == Y.shape
+    n, nrhs = Y.shape
+    lda = factor.nb if tiled_lower else A.stride(0)
+    wsb = int(L.krr_pcg_workspace(n, factor.nb, nrhs))
+    if wsb == 0:
+        raise KrrError("krr_pcg_workspace: invalid shape / nrhs")
+    ws = _ws(wsb, Y.device)
+    norms = torch.zeros(iters + 1, dtype=torch.float64, device=Y.device) if residual_norms else None
+    _check(L.krr_pcg(_ptr(A), n, lda, factor.nb, _ptr(factor.payload), _ptr(factor.scales), _ptr(factor.d_map),
+                     _ptr(factor.h_map), _ptr(Y), Y.stride(0), _ptr(X), X.stride(0), nrhs, iters,
+                     _ptr(norms) if residual_norms else None, _ptr(ws), wsb,
+                     FLAG_A_TILED_LOWER if tiled_lower else 0, _stream()), "krr_pcg")
     return X, norms
 
 

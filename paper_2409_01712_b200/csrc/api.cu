@@ -863,6 +863,152 @@ int krr_refine(const float* d_A, int64_t n, int64_t lda, int nb, const void* d_f
 
 }  // extern "C"
 
+// ------------------------------------------------------------------------- preconditioned CG (R20)
+namespace {
+struct PcgWs { size_t potrs, x, r, q, p, z, partial, blk, dot, scal, total; };
+PcgWs pcg_ws_layout(int64_t n, int nb, int nrhs) {
+    PcgWs w;
+    const size_t NR = static_cast<size_t>(rhs_class(nrhs));
+    const size_t vec64 = static_cast<size_t>(n) * nrhs * sizeof(double), vec32 = static_cast<size_t>(n) * nrhs * sizeof(float);
+    size_t o = 0;
+    w.potrs = o;   o = align_up(o + potrs_ws_layout(n, nb).total, 1024);
+    w.x = o;       o = align_up(o + vec64, 1024);
+    w.r = o;       o = align_up(o + vec64, 1024);
+    w.q = o;       o = align_up(o + vec64, 1024);
+    w.p = o;       o = align_up(o + vec32, 1024);
+    w.z = o;       o = align_up(o + vec32, 1024);
+    w.partial = o; o = align_up(o + static_cast<size_t>(resid_segments(n)) * n * NR * sizeof(double), 1024);
+    w.blk = o;     o = align_up(o + (static_cast<size_t>(n) * NR / 256 + 1) * sizeof(double), 1024);
+    w.dot = o;     o = align_up(o + (static_cast<size_t>(n) / kDotRows + 1) * kMaxRhsDot * sizeof(double), 1024);
+    w.scal = o;    o = align_up(o + 3 * kMaxRhsDot * sizeof(double), 1024);
+    w.total = o;
+    return w;
+}
+
+// partial products of A with the compact FP32 vectors V, then out64 = Y - A V (Y given) or A V
+template <int NR>
+int symm_run(const AView& av, const float* V, int64_t ldv, const float* Y, int64_t ldy, int64_t n, int nrhs, double* partial,
+             double* out64, float* out32, double* blk, cudaStream_t st) {
+    const int nblk = static_cast<int>(n / kBlk), nseg = resid_segments(n);
+    int rc = launch(CAT_MISC, resid_partial_kernel<NR>, dim3(nblk, nseg), dim3(ResidCfg<NR>::NTHR), 0, st, av, V, ldv, nrhs,
+                    nblk, nseg, partial);
+    if (rc) return rc;
+    const int64_t nfin = (n * NR + 255) / 256;
+    return launch(CAT_MISC, pcg_finish_kernel<NR>, dim3(static_cast<unsigned>(nfin)), dim3(256), 0, st,
+                  static_cast<const double*>(partial), nseg, n, Y, ldy, out64, out32, nrhs, blk);
+}
+
+template <typename TA, typename TB>
+int coldot(const TA* a, const TB* b, int64_t n, int nrhs, double* part, double* out, cudaStream_t st) {
+    const int64_t nb_ = (n + kDotRows - 1) / kDotRows;
+    int rc = launch(CAT_MISC, coldot_partial_kernel<TA, TB>, dim3(static_cast<unsigned>(nb_)), dim3(kDotRows), 0, st, a, b, n, nrhs, part);
+    if (rc) return rc;
+    return launch(CAT_MISC, coldot_final_kernel, dim3(1), dim3(kMaxRhsDot), 0, st, static_cast<const double*>(part), nb_, nrhs, out);
+}
+}  // namespace
+
+extern "C" {
+
+size_t krr_pcg_workspace(int64_t n, int nb, int nrhs) {
+    if (krr_potrs_workspace(n, nb, nrhs) == 0) return 0;
+    return pcg_ws_layout(n, nb, nrhs).total;
+}
+
+int krr_pcg(const float* d_A, int64_t n, int64_t lda, int nb, const void* d_factor, const float* d_scales,
+            const uint8_t* d_map, const uint8_t* h_map, const float* d_Y, int64_t ldy, float* d_X, int64_t ldx,
+            int nrhs, int iters, double* d_resid, void* d_ws, size_t ws_bytes, unsigned flags, void* stream) {
+    g_launches = 0;
+    if (!d_A || !d_factor || !d_scales || !d_map || !h_map || !d_Y || !d_X || !d_ws) return KRR_ERR_ARG;
+    int rc = check_shape(n, nb);
+    if (rc) return rc;
+    const bool tiled = (flags & KRR_FLAG_A_TILED_LOWER) != 0;
+    if ((flags & ~static_cast<unsigned>(KRR_FLAG_A_TILED_LOWER)) != 0) return KRR_ERR_ARG;
+    if (nrhs < 1 || nrhs > kMaxRhs || ldy < nrhs || ldx < nrhs || iters < 0 || iters > 1024) return KRR_ERR_ARG;
+    if (!tiled && lda < n) return KRR_ERR_ARG;
+    if (static_cast<int64_t>(rhs_class(nrhs)) * nb > 32768) return KRR_ERR_SHAPE;
+    if (reinterpret_cast<uintptr_t>(d_ws) % 1024 != 0) return KRR_ERR_ARG;
+    const PcgWs L = pcg_ws_layout(n, nb, nrhs);
+    if (ws_bytes < L.total) return KRR_ERR_WORKSPACE;
+    rc = check_device(nullptr);
+    if (rc) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    uint8_t* ws = static_cast<uint8_t*>(d_ws);
+    double* x = reinterpret_cast<double*>(ws + L.x);
+    double* r = reinterpret_cast<double*>(ws + L.r);
+    double* qv = reinterpret_cast<double*>(ws + L.q);
+    float* p = reinterpret_cast<float*>(ws + L.p);
+    float* z = reinterpret_cast<float*>(ws + L.z);
+    double* partial = reinterpret_cast<double*>(ws + L.partial);
+    double* blk = reinterpret_cast<double*>(ws + L.blk);
+    double* dot = reinterpret_cast<double*>(ws + L.dot);
+    double* rho[2] = {reinterpret_cast<double*>(ws + L.scal), reinterpret_cast<double*>(ws + L.scal) + kMaxRhsDot};
+    double* pq = reinterpret_cast<double*>(ws + L.scal) + 2 * kMaxRhsDot;
+    AView av{d_A, lda, tiled ? 1 : 0, static_cast<int>(n / nb), nb};
+    const int64_t ne = n * nrhs;
+    const unsigned gel = static_cast<unsigned>((ne + 255) / 256);
+    int64_t launches = 0;
+    auto symm = [&](const float* V, int64_t ldv, const float* Yp, double* out64, float* out32, double* blkp) -> int {
+        switch (rhs_class(nrhs)) {
+            case 4:  return symm_run<4>(av, V, ldv, Yp, ldy, n, nrhs, partial, out64, out32, blkp, st);
+            case 8:  return symm_run<8>(av, V, ldv, Yp, ldy, n, nrhs, partial, out64, out32, blkp, st);
+            case 16: return symm_run<16>(av, V, ldv, Yp, ldy, n, nrhs, partial, out64, out32, blkp, st);
+            default: return symm_run<32>(av, V, ldv, Yp, ldy, n, nrhs, partial, out64, out32, blkp, st);
+        }
+    };
+    auto solve = [&]() -> int {                       // z <- (L L^T)^-1 z; krr_potrs resets the launch counter
+        launches += g_launches;
+        int e = krr_potrs(d_factor, d_scales, d_map, h_map, n, nb, z, nrhs, nrhs, ws + L.potrs, L.x - L.potrs, stream);
+        launches += g_launches;
+        g_launches = 0;
+        return e;
+    };
+    auto norm_to = [&](double* out, int64_t nblocks) -> int {
+        return launch(CAT_MISC, resid_norm_kernel, dim3(1), dim3(256), 0, st, static_cast<const double*>(blk), nblocks, out);
+    };
+    const int64_t nfin = (n * rhs_class(nrhs) + 255) / 256;
+    // r_0 = Y - A alpha_0, z_0 = M^-1 r_0, p_0 = z_0, rho_0 = r_0 . z_0
+    rc = launch(CAT_MISC, pcg_load_x_kernel, dim3(gel), dim3(256), 0, st, static_cast<const float*>(d_X), ldx, x, n, nrhs);
+    if (rc) return rc;
+    rc = symm(d_X, ldx, d_Y, r, z, d_resid ? blk : nullptr);
+    if (rc) return rc;
+    if (d_resid) { rc = norm_to(d_resid, nfin); if (rc) return rc; }
+    if (iters > 0) {
+        rc = solve();
+        if (rc) return rc;
+        rc = coldot(static_cast<const double*>(r), static_cast<const float*>(z), n, nrhs, dot, rho[0], st);
+        if (rc) return rc;
+        KRR_CUDA_CHECK(cudaMemcpyAsync(p, z, static_cast<size_t>(ne) * sizeof(float), cudaMemcpyDeviceToDevice, st));
+    }
+    for (int k = 0; k < iters; ++k) {
+        double* rho_k = rho[k & 1];
+        double* rho_n = rho[(k + 1) & 1];
+        rc = symm(p, nrhs, nullptr, qv, nullptr, nullptr);                                       // q = A p
+        if (rc) return rc;
+        rc = coldot(static_cast<const float*>(p), static_cast<const double*>(qv), n, nrhs, dot, pq, st);
+        if (rc) return rc;
+        rc = launch(CAT_MISC, pcg_update_xr_kernel, dim3(gel), dim3(256), 0, st, x, r, static_cast<const float*>(p),
+                    static_cast<const double*>(qv), static_cast<const double*>(rho_k), static_cast<const double*>(pq), z, n, nrhs, blk);
+        if (rc) return rc;
+        if (d_resid) { rc = norm_to(d_resid + k + 1, gel); if (rc) return rc; }
+        if (k + 1 == iters) break;                                                               // no further direction needed
+        rc = solve();
+        if (rc) return rc;
+        rc = coldot(static_cast<const double*>(r), static_cast<const float*>(z), n, nrhs, dot, rho_n, st);
+        if (rc) return rc;
+        rc = launch(CAT_MISC, pcg_update_p_kernel, dim3(gel), dim3(256), 0, st, p, static_cast<const float*>(z),
+                    static_cast<const double*>(rho_k), static_cast<const double*>(rho_n), n, nrhs);
+        if (rc) return rc;
+    }
+    if (iters > 0) {
+        rc = launch(CAT_MISC, pcg_store_x_kernel, dim3(gel), dim3(256), 0, st, d_X, ldx, static_cast<const double*>(x), n, nrhs);
+        if (rc) return rc;
+    }
+    g_launches += launches;
+    return KRR_OK;
+}
+
+}  // extern "C"
+
 // ------------------------------------------------------------------------- host-buffer Associate
 namespace {
 struct Arena {

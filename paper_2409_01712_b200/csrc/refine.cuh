@@ -195,4 +195,126 @@ refine_update_kernel(float* __restrict__ X, int64_t ldx, const float* __restrict
     X[row * ldx + q] += D[e];
 }
 
+// ---- conjugate gradients preconditioned by the fixed factor (R20) ----
+// All vectors are compact n x nrhs (row-major, leading dimension nrhs); every right-hand side has its own scalars.
+
+// v = sum of the segments' partial products (FP64); out64 = Y - v (Y given) or v; optionally the FP32 copy and the
+// per-block sums of squares of out64.
+template <int NR>
+__global__ void __launch_bounds__(256)
+pcg_finish_kernel(const double* __restrict__ partial, int nseg, int64_t n, const float* __restrict__ Y, int64_t ldy,
+                  double* __restrict__ out64, float* __restrict__ out32, int nrhs, double* __restrict__ blk_sumsq) {
+    __shared__ double red[8];
+    const int64_t e = static_cast<int64_t>(blockIdx.x) * 256 + threadIdx.x;
+    const int64_t row = e / NR;
+    const int q = static_cast<int>(e % NR);
+    double sq = 0.0;
+    if (row < n && q < nrhs) {
+        double v = 0.0;
+        for (int g = 0; g < nseg; ++g) v += partial[(static_cast<int64_t>(g) * n + row) * NR + q];
+        if (Y) v = static_cast<double>(Y[row * ldy + q]) - v;
+        out64[row * nrhs + q] = v;
+        if (out32) out32[row * nrhs + q] = static_cast<float>(v);
+        sq = v * v;
+    }
+    if (!blk_sumsq) return;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) sq += __shfl_xor_sync(0xffffffffu, sq, o);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = sq;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double s = 0.0;
+        for (int w = 0; w < 8; ++w) s += red[w];
+        blk_sumsq[blockIdx.x] = s;
+    }
+}
+
+constexpr int kDotRows = 256;      // rows per block of the column inner products
+constexpr int kMaxRhsDot = 32;
+
+// part[block][q] = sum over the block's rows of a(row, q) * b(row, q), FP64, fixed order
+template <typename TA, typename TB>
+__global__ void __launch_bounds__(kDotRows)
+coldot_partial_kernel(const TA* __restrict__ a, const TB* __restrict__ b, int64_t n, int nrhs, double* __restrict__ part) {
+    __shared__ double red[kDotRows / 32][kMaxRhsDot];
+    const int64_t row = static_cast<int64_t>(blockIdx.x) * kDotRows + threadIdx.x;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    for (int q = 0; q < nrhs; ++q) {
+        double v = row < n ? static_cast<double>(a[row * nrhs + q]) * static_cast<double>(b[row * nrhs + q]) : 0.0;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        if (lane == 0) red[warp][q] = v;
+    }
+    __syncthreads();
+    if (threadIdx.x < nrhs) {
+        double s = 0.0;
+        for (int w = 0; w < kDotRows / 32; ++w) s += red[w][threadIdx.x];
+        part[static_cast<int64_t>(blockIdx.x) * kMaxRhsDot + threadIdx.x] = s;
+    }
+}
+
+// out[q] = sum over the blocks of part[block][q]
+__global__ void __launch_bounds__(kMaxRhsDot)
+coldot_final_kernel(const double* __restrict__ part, int64_t nblocks, int nrhs, double* __restrict__ out) {
+    if (threadIdx.x >= nrhs) return;
+    double s = 0.0;
+    for (int64_t i = 0; i < nblocks; ++i) s += part[i * kMaxRhsDot + threadIdx.x];
+    out[threadIdx.x] = s;
+}
+
+// a_q = rho_q / pq_q (0 if pq_q <= 0);  x += a p;  r -= a q;  z32 = fl32(r);  blk_sumsq = sums of squares of the new r
+__global__ void __launch_bounds__(256)
+pcg_update_xr_kernel(double* __restrict__ x, double* __restrict__ r, const float* __restrict__ p, const double* __restrict__ qv,
+                     const double* __restrict__ rho, const double* __restrict__ pq, float* __restrict__ z32, int64_t n,
+                     int nrhs, double* __restrict__ blk_sumsq) {
+    __shared__ double red[8];
+    const int64_t e = static_cast<int64_t>(blockIdx.x) * 256 + threadIdx.x;
+    double sq = 0.0;
+    if (e < n * nrhs) {
+        const int q = static_cast<int>(e % nrhs);
+        const double d = pq[q];
+        const double a = d > 0.0 ? rho[q] / d : 0.0;
+        x[e] = fma(a, static_cast<double>(p[e]), x[e]);
+        const double rv = fma(-a, qv[e], r[e]);
+        r[e] = rv;
+        z32[e] = static_cast<float>(rv);
+        sq = rv * rv;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) sq += __shfl_xor_sync(0xffffffffu, sq, o);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = sq;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double s = 0.0;
+        for (int w = 0; w < 8; ++w) s += red[w];
+        blk_sumsq[blockIdx.x] = s;
+    }
+}
+
+// b_q = rho_new_q / rho_q (0 if rho_q <= 0);  p = fl32(z + b p)
+__global__ void __launch_bounds__(256)
+pcg_update_p_kernel(float* __restrict__ p, const float* __restrict__ z, const double* __restrict__ rho,
+                    const double* __restrict__ rho_new, int64_t n, int nrhs) {
+    const int64_t e = static_cast<int64_t>(blockIdx.x) * 256 + threadIdx.x;
+    if (e >= n * nrhs) return;
+    const int q = static_cast<int>(e % nrhs);
+    const double d = rho[q];
+    const double b = d > 0.0 ? rho_new[q] / d : 0.0;
+    p[e] = static_cast<float>(fma(b, static_cast<double>(p[e]), static_cast<double>(z[e])));
+}
+
+// compact FP64 <- strided FP32, and back
+__global__ void __launch_bounds__(256)
+pcg_load_x_kernel(const float* __restrict__ X, int64_t ldx, double* __restrict__ x, int64_t n, int nrhs) {
+    const int64_t e = static_cast<int64_t>(blockIdx.x) * 256 + threadIdx.x;
+    if (e >= n * nrhs) return;
+    x[e] = static_cast<double>(X[(e / nrhs) * ldx + e % nrhs]);
+}
+__global__ void __launch_bounds__(256)
+pcg_store_x_kernel(float* __restrict__ X, int64_t ldx, const double* __restrict__ x, int64_t n, int nrhs) {
+    const int64_t e = static_cast<int64_t>(blockIdx.x) * 256 + threadIdx.x;
+    if (e >= n * nrhs) return;
+    X[(e / nrhs) * ldx + e % nrhs] = static_cast<float>(x[e]);
+}
+
 }  // namespace krr

@@ -186,3 +186,62 @@ def test_tail_split_with_a_mixed_map(krr):
     b1, b2 = probe_backward_error(A, F1, 4), probe_backward_error(A, F2, 4)
     assert abs(b1 - b2) <= 0.02 * b2 and b1 < 5e-2
 
+
+
+def test_c4_full_size_rule_map_leading_block_invariants_and_pcg(krr):
+    """C4 at full size (n = 131072, packed lower tiles, rule eps = 1e-3 over {FP32, FP16}): the rule gives every
+    off-diagonal tile FP16 (SURVEY finding 1); the leading 3 x 3 tiles against the emulated oracle on the leading
+    submatrix; info, diagonal, backward error by probes (<= 5e-4) with independent torch-FP64 code.  Then what the
+    factor is good for at this size (R20): refinement does not contract (the second step grows the
+    residual), CG preconditioned by the same factor brings it down by four orders of magnitude in six steps."""
+    from helpers import LowerTiles
+    cfg = CONFIGS["C4"]
+    nb, NT, n = cfg.nb, cfg.NT, cfg.n
+    from krr_inputs import make_problem_lower_tiles
+    At, Y = make_problem_lower_tiles(cfg, device="cuda")
+    tl = krr.FLAG_A_TILED_LOWER
+    d_map, norms, amax, fro = krr.precision_map(At, nb, cfg.eps_target, cfg.allowed, flags=tl, n=n)
+    h_map = d_map.cpu()
+    hm = h_map.numpy()
+    low = np.tril_indices(NT, -1)
+    assert np.bincount(hm[low], minlength=3).tolist() == [0, NT * (NT - 1) // 2, 0]
+    F = krr.potrf_mp(At, nb, d_map, h_map, flags=krr.FLAG_PREROUND_A | tl, n=n)
+    alpha = krr.potrs(F, Y.clone())
+    torch.cuda.synchronize()
+    assert int(F.info.item()) == 0
+    # leading block: assemble the dense leading 3 x 3 tiles from the packed tiles
+    m = 3
+    T = At.reshape(-1, nb, nb)
+    Am = np.zeros((m * nb, m * nb))
+    for j in range(m):
+        for i in range(j, m):
+            t = T[krr.tile_slot(NT, i, j)].cpu().numpy().astype(np.float64)
+            Am[i * nb:(i + 1) * nb, j * nb:(j + 1) * nb] = t
+            if i != j:
+                Am[j * nb:(j + 1) * nb, i * nb:(i + 1) * nb] = t.T
+    pm = np.ascontiguousarray(hm[:m, :m])
+    Lo, sc, info = tile_cholesky_emulated(Am, nb, pm, preround_a=True)
+    assert info == 0
+    Lg = leading_block(F, m)
+    assert abs(backward_error(Am, Lg) - backward_error(Am, Lo)) <= 0.02 * backward_error(Am, Lo)
+    for i in range(1, m):                                     # first tile column: at most one FP16 ulp apart
+        g, o = Lg[i * nb:(i + 1) * nb, :nb], Lo[i * nb:(i + 1) * nb, :nb]
+        tol = 2.5 * R.UNIT_ROUNDOFF[FP16] * np.abs(o) + 1e-5 * np.abs(o).max()
+        assert np.all(np.abs(g - o) <= tol) and np.mean(g == o) > 0.5
+    for k in range(0, NT, NT // 8):
+        assert float(torch.diagonal(F.tile(k, k)).min()) > 0.0
+    A_chk = LowerTiles(At, n, nb)
+    assert probe_backward_error(A_chk, F, 4) <= 5e-4
+    # refinement and CG with the factor kept fixed
+    Xr, rn = krr.refine(At, F, Y, alpha.clone(), 2, tiled_lower=True)
+    Xc, cn = krr.pcg(At, F, Y, alpha.clone(), 6, tiled_lower=True)
+    torch.cuda.synchronize()
+    rn, cn = rn.cpu().numpy(), cn.cpu().numpy()
+    assert rn[2] > rn[1]                                       # the stationary iteration has stopped contracting
+    assert abs(cn[0] - rn[0]) <= 1e-6 * rn[0]
+    assert np.all(cn[1:] < cn[:-1]) and cn[6] < 1e-3 * cn[0]
+    res_raw, res_cg = solve_residual(A_chk, alpha, Y), solve_residual(A_chk, Xc, Y)
+    assert res_cg < 1e-2 * res_raw
+    # how far the raw alpha was from the converged one: the 10 % the survey's sqrt(n) growth predicts
+    moved = float(torch.linalg.norm((Xc - alpha).double()) / torch.linalg.norm(Xc.double()))
+    assert 1e-2 < moved < 0.5

@@ -164,3 +164,93 @@ def test_full_size_refinement_under_the_half_precision_map(krr):
     from helpers import fro_norm_sym
     want0 = res0 * fro_norm_sym(A) * float(torch.linalg.norm(X0.to(torch.float64)))
     assert abs(norms[0] - want0) <= 1e-4 * want0
+
+
+# ---- krr_pcg (R20) ----
+@pytest.mark.parametrize("n,nb,nrhs", [(1280, 256, 3), (2048, 256, 16), (1024, 128, 32)])
+def test_pcg_with_an_fp32_map_from_a_random_start(krr, n, nb, nrhs):
+    """M^-1 A = I to FP32 accuracy: the first step lands on the solution -- unless an element of the residual, of
+    q = A p, of an inner product or of an update is wrong.  NaN above the diagonal as in the refinement test."""
+    cfg = replace(scaled_config(CONFIGS["C2"], nb=nb, n=n, p=max(256, n // 4)), nrhs=nrhs)
+    A, Y = make_problem(cfg, device="cuda")
+    h = krr.uniform_map(cfg.NT, krr.FP32)
+    F = krr.potrf_mp(A, nb, h.cuda(), h)
+    g = torch.Generator(device="cpu").manual_seed(3 * n + nrhs)
+    X0 = torch.randn((n, nrhs), generator=g, dtype=torch.float32)
+    An, Yn = A.cpu().numpy().astype(np.float64), Y.cpu().numpy().astype(np.float64)
+    xstar = solve_fp64(An, Yn, nb)
+    Ap = A.clone()
+    Ap[torch.triu(torch.ones_like(Ap, dtype=torch.bool), 1)] = float("nan")
+    X1, n1 = krr.pcg(Ap, F, Y, X0.cuda(), 1)
+    X2, n2 = krr.pcg(Ap, F, Y, X0.cuda(), 2)
+    torch.cuda.synchronize()
+    assert rel(X1.cpu().numpy().astype(np.float64), xstar) <= 1e-4
+    assert rel(X2.cpu().numpy().astype(np.float64), xstar) <= 1e-6
+    n2 = n2.cpu().numpy()
+    r0 = Yn - An @ X0.numpy().astype(np.float64)
+    assert abs(n2[0] - np.linalg.norm(r0)) <= 1e-9 * np.linalg.norm(r0)
+    assert n2[1] <= 1e-3 * n2[0] and n2[2] <= 1e-2 * n2[1] and float(n1[1]) == n2[1]
+    X00, n0 = krr.pcg(Ap, F, Y, X0.cuda(), 0)
+    assert torch.equal(X00.cpu(), X0) and float(n0[0]) == n2[0]
+
+
+@pytest.mark.parametrize("prec,tiled", [("fp16", False), ("fp16", True), ("fp8", False)])
+def test_pcg_under_low_precision_maps_against_the_oracle(krr, prec, tiled):
+    """Step by step against oracle.solve.pcg on the oracle's own emulated factor: errors within a factor of the
+    oracle's (plus FP32 roundoff), residual norms likewise; four steps meet north_star's 1e-3 with room to spare."""
+    from oracle.solve import pcg
+    nb = 128
+    cfg = scaled_config(CONFIGS["C4"], nb=nb, n=2048, p=512) if prec == "fp16" else \
+        scaled_config(CONFIGS["C5p"], nb=nb, n=2048, p=400)
+    Ad, Y = make_problem(cfg, device="cuda")
+    A = make_problem_lower_tiles(cfg, device="cuda")[0] if tiled else Ad
+    h = krr.uniform_map(cfg.NT, krr.FP16 if prec == "fp16" else krr.FP8)
+    flags = krr.FLAG_PREROUND_A
+    if prec == "fp8":
+        h[1:, 0] = krr.FP32
+        flags = 0
+    F = krr.potrf_mp(A, nb, h.cuda(), h, flags=flags | (krr.FLAG_A_TILED_LOWER if tiled else 0), n=cfg.n)
+    X0 = krr.potrs(F, Y.clone())
+    torch.cuda.synchronize()
+    assert int(F.info.item()) == 0
+    An, Yn = Ad.cpu().numpy().astype(np.float64), Y.cpu().numpy().astype(np.float64)
+    xstar = solve_fp64(An, Yn, nb)
+    Lo, sc, info = tile_cholesky_emulated(An, nb, h.numpy().copy(), preround_a=(prec == "fp16"))
+    assert info == 0
+    o0 = potrs_fp64(Lo, Yn, nb)
+    for k in (1, 2, 4):
+        Xg, gn = krr.pcg(A, F, Y, X0.clone(), k, tiled_lower=tiled)
+        xo, on = pcg(An, Lo, Yn, o0, nb, k)
+        eg, eo = rel(Xg.cpu().numpy().astype(np.float64), xstar), rel(xo, xstar)
+        assert eg <= 3.0 * eo + 3e-6, (k, eg, eo)
+        gn = gn.cpu().numpy()
+        for s in range(k + 1):
+            assert 0.33 * on[s] <= gn[s] <= 3.0 * on[s] + 1e-5, (k, s, gn, on)
+    assert eg <= 1e-5
+
+
+def test_pcg_converges_where_refinement_diverges(krr):
+    """The factor of K + lambda I as the preconditioner of K + (lambda + 0.2) I: most eigenvalues of M^-1 A lie above
+    2, so the stationary iteration grows the error while CG converges -- as on C4 at full size (R20), here
+    at a size the oracle checks step by step."""
+    from oracle.solve import pcg
+    nb = 128
+    cfg = replace(scaled_config(CONFIGS["C2"], nb=nb, n=1536, p=384), nrhs=8)
+    A, Y = make_problem(replace(cfg, lam=cfg.lam + 0.2), device="cuda")       # the system
+    A2, _ = make_problem(cfg, device="cuda")                                  # what is factored
+    h = krr.uniform_map(cfg.NT, krr.FP32)
+    F = krr.potrf_mp(A2, nb, h.cuda(), h)
+    X0 = krr.potrs(F, Y.clone())
+    An, A2n, Yn = (t.cpu().numpy().astype(np.float64) for t in (A, A2, Y))
+    xstar = solve_fp64(An, Yn, nb)
+    e0 = rel(X0.cpu().numpy().astype(np.float64), xstar)
+    Xr, rn = krr.refine(A, F, Y, X0.clone(), 8)
+    assert rel(Xr.cpu().numpy().astype(np.float64), xstar) > 5.0 * e0 and float(rn[8]) > 5.0 * float(rn[0])
+    Lo = np.linalg.cholesky(A2n)
+    o0 = potrs_fp64(Lo, Yn, nb)
+    for k in (2, 6, 12):
+        Xg, gn = krr.pcg(A, F, Y, X0.clone(), k)
+        xo, on = pcg(An, Lo, Yn, o0, nb, k)
+        eg, eo = rel(Xg.cpu().numpy().astype(np.float64), xstar), rel(xo, xstar)
+        assert eg <= 2.0 * eo + 3e-6, (k, eg, eo)
+    assert eg <= 1e-5 and eg < 1e-4 * e0

@@ -119,3 +119,20 @@ def ridge_regression_definition(X, Y, lam):
     X = np.asarray(X, dtype=np.float64)
     return np.linalg.solve(X.T @ X + float(lam) * np.eye(X.shape[1]), X.T @ np.asarray(Y, dtype=np.float64))
 
+
+
+# ---- ragged n (R21) ----
+def identity_border(A, n_pad):
+    """The n x n matrix A bordered by an identity block up to n_pad x n_pad: [[A, 0], [0, I]].  The tile algorithms
+    need n to be a multiple of nb (the paper's cohort, 305,880 patients, is not a multiple of any tile size it
+    uses; how its runtime treats the last partial tile row is not said).  Reading R21: the matrix is bordered, the
+    right-hand sides get zero rows; then chol = blockdiag(L, I), the first n rows of the solution are A^-1 Y and
+    the rest is zero -- nothing of the original problem changes.  The precision rule is evaluated on the bordered
+    matrix (NT and ||.||_F of the bordered matrix)."""
+    A = np.asarray(A, dtype=np.float64)
+    n = A.shape[0]
+    assert n_pad >= n
+    B = np.zeros((n_pad, n_pad))
+    B[:n, :n] = A
+    B[np.arange(n, n_pad), np.arange(n, n_pad)] = 1.0
+    return B

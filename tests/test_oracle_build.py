@@ -180,3 +180,31 @@ def test_linear_kernel_and_ridge_regression_pins():
     assert np.allclose(beta, X.T.astype(float) @ alpha, atol=1e-10)
     assert np.allclose(X.T.astype(float) @ (Y - X.astype(float) @ beta), lam * beta, atol=1e-9)     # gradient of Eq. (1) vanishes
 
+
+
+def test_identity_border_changes_nothing_of_the_problem():
+    """DESIGN.md R21: chol([[A,0],[0,I]]) = blockdiag(chol(A), I) and the bordered solve returns A^-1 Y over zero rows
+    -- checked with LAPACK on the bordered matrix and with the oracle's own tile Cholesky / solve at a tile size that
+    does not divide n."""
+    from oracle.build_phase import identity_border, kernel_matrix_definition
+    from oracle.cholesky import tile_cholesky_fp64
+    from oracle.solve import potrs_fp64
+    rng = np.random.default_rng(21)
+    n, p, nb = 77, 40, 32
+    G = rng.integers(0, 3, size=(n, p)).astype(np.int8)
+    A = kernel_matrix_definition(G, 1.0 / p, 0.05)
+    n_pad = -(-n // nb) * nb
+    B = identity_border(A, n_pad)
+    assert B.shape == (96, 96) and np.array_equal(B[:n, :n], A) and np.array_equal(B[n:, n:], np.eye(n_pad - n))
+    assert not B[:n, n:].any() and not B[n:, :n].any()
+    Lb = np.linalg.cholesky(B)
+    np.testing.assert_allclose(Lb[:n, :n], np.linalg.cholesky(A), rtol=1e-13, atol=1e-15)
+    assert np.array_equal(Lb[n:, n:], np.eye(n_pad - n)) and not Lb[n:, :n].any()
+    Lt, info = tile_cholesky_fp64(B, nb)
+    assert info == 0
+    np.testing.assert_allclose(Lt, Lb, rtol=1e-12, atol=1e-14)
+    Y = rng.standard_normal((n, 3))
+    Yb = np.vstack([Y, np.zeros((n_pad - n, 3))])
+    xb = potrs_fp64(Lt, Yb, nb)
+    np.testing.assert_allclose(xb[:n], np.linalg.solve(A, Y), rtol=1e-10, atol=1e-12)
+    assert not xb[n:].any()

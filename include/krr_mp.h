@@ -293,6 +293,18 @@ int krr_build(const int8_t* d_G, int64_t n, int64_t p, int64_t ldg, const float*
               float gamma, float lambda, float* d_A, int64_t lda, int nb, unsigned flags,
               void* d_stats, void* d_ws, size_t ws_bytes, void* stream);
 
+/* krr_build_bordered -- the same for a cohort whose size is no multiple of the tile size (R21; SURVEY 8(f)
+ * NEXT-4 "ragged n"; the paper's cohort has 305,880 patients): n is the padded size (the next multiple of nb and of
+ * 256), n_valid <= n the number of patients.  Rows >= n_valid of d_G (and d_C) must exist (n rows are read for the
+ * folded norms) and are ignored; rows and columns >= n_valid of A are written as the identity border (1 on the
+ * diagonal, 0 elsewhere), which changes nothing of the problem: chol = blockdiag(L, I), and with zero rows appended
+ * to Y the first n_valid rows of krr_potrs's result are the solution, the rest exactly 0.  The tile statistics
+ * (d_stats) are those of the bordered matrix.  krr_build(...) == krr_build_bordered(..., n_valid = n).
+ */
+int krr_build_bordered(const int8_t* d_G, int64_t n, int64_t n_valid, int64_t p, int64_t ldg, const float* d_C, int q,
+                       int64_t ldc, float gamma, float lambda, float* d_A, int64_t lda, int nb, unsigned flags,
+                       void* d_stats, void* d_ws, size_t ws_bytes, void* stream);
+
 /* Tile statistics from the Build epilogue ("tile sum-of-squares emitted in the same epilogue so
  * krr_precision_map needs no extra pass").  If krr_build is given d_stats (krr_build_stats_bytes(n, nb) bytes, 1024-byte
  * aligned; NULL: none) every epilogue warp also leaves the FP64 sum of squares and the maximum modulus of its share of A

@@ -25,7 +25,7 @@ ERRORS = {-1: "KRR_ERR_ARG", -2: "KRR_ERR_SHAPE", -3: "KRR_ERR_WORKSPACE", -4: "
 EXPORTS = ["krr_version", "krr_built_for_sm", "krr_tile_slot", "krr_precision_map_workspace",
            "krr_precision_map", "krr_factor_bytes", "krr_factor_tile_offset",
            "krr_potrf_mp_workspace", "krr_potrf_mp", "krr_potrs_workspace", "krr_potrs", "krr_refine_workspace", "krr_refine", "krr_pcg_workspace", "krr_pcg",
-           "krr_associate_host_arena", "krr_associate_host", "krr_build_workspace", "krr_build", "krr_predict_workspace", "krr_predict", "krr_fit_host_arena", "krr_fit_host", "krr_band_map", "krr_build_stats_bytes", "krr_precision_map_from_build",
+           "krr_associate_host_arena", "krr_associate_host", "krr_build_workspace", "krr_build", "krr_build_bordered", "krr_predict_workspace", "krr_predict", "krr_fit_host_arena", "krr_fit_host", "krr_band_map", "krr_build_stats_bytes", "krr_precision_map_from_build",
            "krr_last_launch_count",
            "krr_profile_enable", "krr_profile_read"]
 
@@ -88,6 +88,9 @@ def lib():
     L.krr_build_workspace.argtypes = [i64, i64, u32]
     L.krr_build.restype = c.c_int
     L.krr_build.argtypes = [vp, i64, i64, i64, vp, c.c_int, i64, c.c_float, c.c_float, vp, i64, c.c_int, u32, vp, vp, sz, vp]
+    L.krr_build_bordered.restype = c.c_int
+    L.krr_build_bordered.argtypes = [vp, i64, i64, i64, i64, vp, c.c_int, i64, c.c_float, c.c_float, vp, i64, c.c_int, u32, vp, vp,
+                                     sz, vp]
     L.krr_build_stats_bytes.restype = sz
     L.krr_build_stats_bytes.argtypes = [i64, c.c_int]
     L.krr_precision_map_from_build.restype = c.c_int
@@ -359,10 +362,11 @@ def _conf(C):
     return C, C.shape[1], C.stride(0)
 
 
-def krr_build(G, gamma, lam, nb, tiled_lower=False, out=None, flags=0, C=None, stats=False):
+def krr_build(G, gamma, lam, nb, tiled_lower=False, out=None, flags=0, C=None, stats=False, n_valid=None):
     """krr_build (named in full: `build` is this package's compile step): A = K + lam*I (Gaussian kernel) from CUDA int8 genotypes G (n x p, row-major, row pitch a
     multiple of 16 bytes).  Returns A: n x n FP32 with the lower tiles written (the rest zero), or the packed
-    lower tiles with tiled_lower."""
+    lower tiles with tiled_lower.  n_valid < n (krr_build_bordered, R21): rows >= n_valid of G are padding,
+    rows and columns >= n_valid of A the identity border."""
     L = lib()
     assert G.dtype == torch.int8 and G.is_cuda and G.stride(1) == 1
     n, p = G.shape
@@ -379,8 +383,9 @@ def krr_build(G, gamma, lam, nb, tiled_lower=False, out=None, flags=0, C=None, s
     lda = nb if tiled_lower else out.stride(0)
     C, q, ldc = _conf(C)
     st = _ws(int(L.krr_build_stats_bytes(n, nb)), dev) if stats else None
-    _check(L.krr_build(_ptr(G), n, p, G.stride(0), _ptr(C), q, ldc, float(gamma), float(lam), _ptr(out), lda, nb, flags,
-                       _ptr(st), _ptr(ws), wsb, _stream()), "krr_build")
+    _check(L.krr_build_bordered(_ptr(G), n, n if n_valid is None else int(n_valid), p, G.stride(0), _ptr(C), q, ldc,
+                                float(gamma), float(lam), _ptr(out), lda, nb, flags, _ptr(st), _ptr(ws), wsb, _stream()),
+           "krr_build_bordered")
     return (out, st) if stats else out
 
 

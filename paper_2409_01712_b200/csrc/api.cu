@@ -1239,8 +1239,15 @@ int krr_precision_map_from_build(const void* d_stats, int64_t n, int nb, float e
 int krr_build(const int8_t* d_G, int64_t n, int64_t p, int64_t ldg, const float* d_C, int q, int64_t ldc, float gamma,
               float lambda, float* d_A, int64_t lda, int nb, unsigned flags, void* d_stats, void* d_ws, size_t ws_bytes,
               void* stream) {
+    return krr_build_bordered(d_G, n, n, p, ldg, d_C, q, ldc, gamma, lambda, d_A, lda, nb, flags, d_stats, d_ws, ws_bytes, stream);
+}
+
+int krr_build_bordered(const int8_t* d_G, int64_t n, int64_t n_valid, int64_t p, int64_t ldg, const float* d_C, int q,
+                       int64_t ldc, float gamma, float lambda, float* d_A, int64_t lda, int nb, unsigned flags, void* d_stats,
+                       void* d_ws, size_t ws_bytes, void* stream) {
     g_launches = 0;
     if (!d_G || !d_A || !d_ws) return KRR_ERR_ARG;
+    if (n_valid < 1 || n_valid > n) return KRR_ERR_ARG;
     if (q < 0 || q > kMaxConfounders || (q > 0 && (!d_C || ldc < q))) return KRR_ERR_ARG;
     int rc = check_shape(n, nb);
     if (rc) return rc;
@@ -1279,6 +1286,7 @@ int krr_build(const int8_t* d_G, int64_t n, int64_t p, int64_t ldg, const float*
     op.ibs = ibs ? 1 : 0; op.alleles = static_cast<float>(p);        // (p was doubled above: 2 N_S alleles)
     op.linear = linear ? 1 : 0; op.lambda = lambda;
     op.n = n; op.m = n; op.rect = 0; op.p = p; op.nb = nb; op.tiled = tiled ? 1 : 0; op.gamma = gamma;
+    op.n_valid = n_valid;
     op.diag = static_cast<float>(1.0 + static_cast<double>(lambda));
     op.sq = sq; op.sq_row = sq; op.A = d_A; op.lda = lda;
     op.C = d_C; op.C_row = d_C; op.ldc = ldc; op.ldc_row = ldc; op.q = q;

@@ -42,6 +42,8 @@ struct BuildOp {
     // linear kernel (the SYRK of ridge regression, Eq. (2), Fig. 2): K_ij = gamma * <g_i, g_j>, lambda on the diagonal
     int linear;
     float lambda;
+    // ragged n (R21): rows and columns >= n_valid are the identity border (1 on the diagonal, 0 elsewhere)
+    int64_t n_valid;
     // optional tile statistics of A for the precision map (no second pass over A): per lower tile
     // stats_chunks = (blocks per tile) * 16 partial sums of squares (FP64) and maxima, one per epilogue warp of the
     // block's two CTAs, in the layout map_decide_kernel reads (precision_map.cuh)
@@ -306,6 +308,7 @@ build_tc_kernel(const __grid_constant__ CUtensorMap tmR, const __grid_constant__
                             kv = op.ibs ? __fdiv_rn(op.alleles - d2f, op.alleles) : expf(-op.gamma * d2f);
                             if (!op.rect && gj0 + e + u == gi) kv = op.diag;
                         }
+                        if (!op.rect && (gi >= op.n_valid || gj0 + e + u >= op.n_valid)) kv = (gj0 + e + u == gi) ? 1.0f : 0.0f;
                         v[u] = kv;
                         ssq += static_cast<double>(kv) * kv;
                         amx = fmaxf(amx, fabsf(kv));

@@ -318,3 +318,66 @@ def test_precision_map_from_build_statistics(krr, name, nb, n, p, eps):
     low = np.tril_indices(n // nb)
     assert np.array_equal(m1.cpu().numpy()[low], pm[low])
 
+
+
+@pytest.mark.parametrize("n_valid,nb,p,tiled", [(1000, 256, 700, False), (777, 512, 333, False), (1300, 256, 512, True)])
+def test_ragged_n_by_identity_border(krr, n_valid, nb, p, tiled):
+    """DESIGN.md R21 (SURVEY NEXT-4 "ragged n"): krr_build_bordered writes [[A, 0], [0, I]]; garbage in the padding rows
+    of G is ignored.  Entries against the oracle's definition on the n_valid patients, bordered by the oracle; then the
+    whole Associate phase on the bordered matrix: the statistics of the Build epilogue give the map of
+    krr_precision_map, the factor is blockdiag(L, I), the first n_valid rows of alpha are the FP64 solution of the
+    original system and the rest is exactly zero."""
+    from oracle.build_phase import identity_border
+    from oracle.cholesky import tile_cholesky_fp64
+    from oracle.solve import solve_fp64
+    from helpers import LowerTiles
+    n = -(-n_valid // max(nb, 256)) * max(nb, 256)
+    G = genotypes(29, n, p, "maf", device="cuda")
+    G[n_valid:] = 77                                                          # padding rows: anything
+    gamma, lam = 1.0 / p, 5e-2
+    A, st = krr.krr_build(padded(G), gamma, lam, nb, tiled_lower=tiled, stats=True, n_valid=n_valid)
+    torch.cuda.synchronize()
+    want = identity_border(kernel_matrix_definition(G[:n_valid].cpu().numpy(), gamma, lam), n)
+    NT = n // nb
+    if tiled:
+        T = A.reshape(-1, nb, nb).cpu().numpy().astype(np.float64)
+        got = np.zeros((n, n))
+        for j in range(NT):
+            for i in range(j, NT):
+                got[i * nb:(i + 1) * nb, j * nb:(j + 1) * nb] = T[krr.tile_slot(NT, i, j)]
+    else:
+        got = A.cpu().numpy().astype(np.float64)
+    for i in range(NT):
+        for j in range(i + 1):
+            g = got[i * nb:(i + 1) * nb, j * nb:(j + 1) * nb]
+            w = want[i * nb:(i + 1) * nb, j * nb:(j + 1) * nb]
+            assert np.all(np.abs(g - w) <= 8e-7 * np.abs(w)), (i, j)          # the border (0 and 1) exactly
+    flags = krr.FLAG_A_TILED_LOWER if tiled else 0
+    m1, n1, a1, f1 = krr.precision_map_from_build(st, n, nb, 1e-4)
+    m2, n2, a2, f2 = krr.precision_map(A, nb, 1e-4, flags=flags, n=n)
+    assert torch.equal(m1, m2) and torch.equal(a1, a2)
+    h = krr.uniform_map(NT, krr.FP32)
+    F = krr.potrf_mp(A, nb, h.cuda(), h, flags=krr.FLAG_PREROUND_A | flags, n=n)
+    g = torch.Generator(device="cpu").manual_seed(n_valid)
+    Y = torch.zeros((n, 4), dtype=torch.float32)
+    Y[:n_valid] = torch.randn((n_valid, 4), generator=g)
+    alpha = krr.potrs(F, Y.cuda())
+    torch.cuda.synchronize()
+    assert int(F.info.item()) == 0
+    a = alpha.cpu().numpy().astype(np.float64)
+    assert not a[n_valid:].any()                                              # the border rows stay exactly zero
+    Lb, info = tile_cholesky_fp64(want, nb)
+    assert info == 0
+    Lg = F.dense().cpu().numpy()
+    assert np.linalg.norm(Lg - Lb) <= 1e-4 * np.linalg.norm(Lb)
+    assert np.array_equal(Lg[n_valid:, n_valid:], np.eye(n - n_valid)) and not Lg[n_valid:, :n_valid].any()
+    xs = np.linalg.solve(want[:n_valid, :n_valid], Y[:n_valid].numpy().astype(np.float64))
+    assert np.linalg.norm(a[:n_valid] - xs) <= 1e-4 * np.linalg.norm(xs)
+
+
+def test_build_bordered_rejects_bad_n_valid(krr):
+    G = genotypes(3, 512, 256, "maf", device="cuda")
+    with pytest.raises(krr.KrrError):
+        krr.krr_build(padded(G), 1.0 / 256, 1e-2, 256, n_valid=0)
+    with pytest.raises(krr.KrrError):
+        krr.krr_build(padded(G), 1.0 / 256, 1e-2, 256, n_valid=513)

@@ -136,3 +136,13 @@ def identity_border(A, n_pad):
     B[:n, :n] = A
     B[np.arange(n, n_pad), np.arange(n, n_pad)] = 1.0
     return B
+
+
+# ---- the mixed INT8 / FP32 SYRK of ridge regression (Fig. 2) ----
+def ridge_gram_definition(S, C, lam):
+    """X^T X + lam I in FP64 for X = [S | C]: S the patients x N_S matrix of SNPs (integers), C the patients x q matrix
+    of real-valued confounders ("each row of X is a vector of SNPs and confounders").  The SNP x SNP
+    block is an integer matrix (the INT8 tiles of Fig. 2), the blocks that involve a confounder are real (its FP32
+    tiles); here everything is FP64, the product written out as one matrix product."""
+    X = np.hstack([np.asarray(S, dtype=np.float64), np.asarray(C, dtype=np.float64)])
+    return X.T @ X + float(lam) * np.eye(X.shape[1])

@@ -208,3 +208,29 @@ def test_identity_border_changes_nothing_of_the_problem():
     xb = potrs_fp64(Lt, Yb, nb)
     np.testing.assert_allclose(xb[:n], np.linalg.solve(A, Y), rtol=1e-10, atol=1e-12)
     assert not xb[n:].any()
+
+
+def test_ridge_gram_with_confounders():
+    """Fig. 2's matrix: blocks against element-wise sums, and the ridge solution through it against the textbook
+    augmented least-squares form min ||[X; sqrt(lam) I] beta - [Y; 0]|| (numpy lstsq: no normal equations)."""
+    from oracle.build_phase import ridge_gram_definition, linear_kernel_matrix_definition
+    rng = np.random.default_rng(31)
+    npat, ns, q, lam = 60, 23, 3, 0.7
+    S = rng.integers(0, 3, size=(npat, ns)).astype(np.int8)
+    C = rng.standard_normal((npat, q))
+    A = ridge_gram_definition(S, C, lam)
+    assert A.shape == (ns + q, ns + q) and np.array_equal(A, A.T)
+    assert np.array_equal(A[:ns, :ns], linear_kernel_matrix_definition(S.T, S.T) + lam * np.eye(ns))   # integers, exact
+    for j in (0, 7, ns - 1):
+        for t in range(q):
+            want = sum(float(S[k, j]) * C[k, t] for k in range(npat))
+            assert abs(A[ns + t, j] - want) <= 1e-12 * max(1.0, abs(want))
+    for t in range(q):
+        for u in range(q):
+            want = sum(C[k, t] * C[k, u] for k in range(npat)) + (lam if t == u else 0.0)
+            assert abs(A[ns + t, ns + u] - want) <= 1e-12 * max(1.0, abs(want))
+    Y = rng.standard_normal((npat, 2))
+    X = np.hstack([S.astype(np.float64), C])
+    beta = np.linalg.solve(A, X.T @ Y)
+    aug, *_ = np.linalg.lstsq(np.vstack([X, np.sqrt(lam) * np.eye(ns + q)]), np.vstack([Y, np.zeros((ns + q, 2))]), rcond=None)
+    np.testing.assert_allclose(beta, aug, rtol=1e-9, atol=1e-11)

@@ -305,6 +305,21 @@ int krr_build_bordered(const int8_t* d_G, int64_t n, int64_t n_valid, int64_t p,
                        int64_t ldc, float gamma, float lambda, float* d_A, int64_t lda, int nb, unsigned flags,
                        void* d_stats, void* d_ws, size_t ws_bytes, void* stream);
 
+/* krr_build_rr -- the mixed INT8 / FP32 SYRK of ridge regression (Fig. 2; Eq. (2)):
+ *     A = X^T X + lambda I,   X = [S^T | C]   (patients x (ns + q): SNPs, then confounders),
+ * bordered by the identity up to n (R21; ns + q is rarely a multiple of the tile size).
+ * d_S   in   the SNP features as rows: n x p int8, row-major with pitch lds (as d_G of krr_build: p = patients is the
+ *            contraction dimension); rows >= ns must exist and are ignored.
+ * d_C   in   p x q FP32 confounders, row-major (ldc >= q), q <= 16; NULL / q = 0: none.
+ * d_A   out  as for krr_build (dense lower tiles or KRR_FLAG_A_TILED_LOWER).  The SNP x SNP block comes from the INT8
+ *            tensor cores (exact integers, the INT8 tiles of Fig. 2); the q rows that involve a confounder are
+ *            accumulated in FP32 (its FP32 tiles, SGEMM in the paper) in a fixed order; lambda is added on the diagonal.
+ * d_ws       krr_build_workspace(n, p, 0) bytes.  Follow with krr_precision_map / krr_potrf_mp / krr_potrs on A and
+ *            X^T Y (zero rows appended) for beta.
+ */
+int krr_build_rr(const int8_t* d_S, int64_t n, int64_t ns, int64_t p, int64_t lds, const float* d_C, int q, int64_t ldc,
+                 float lambda, float* d_A, int64_t lda, int nb, unsigned flags, void* d_ws, size_t ws_bytes, void* stream);
+
 /* Tile statistics from the Build epilogue ("tile sum-of-squares emitted in the same epilogue so
  * krr_precision_map needs no extra pass").  If krr_build is given d_stats (krr_build_stats_bytes(n, nb) bytes, 1024-byte
  * aligned; NULL: none) every epilogue warp also leaves the FP64 sum of squares and the maximum modulus of its share of A

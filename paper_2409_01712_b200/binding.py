@@ -25,7 +25,7 @@ ERRORS = {-1: "KRR_ERR_ARG", -2: "KRR_ERR_SHAPE", -3: "KRR_ERR_WORKSPACE", -4: "
 EXPORTS = ["krr_version", "krr_built_for_sm", "krr_tile_slot", "krr_precision_map_workspace",
            "krr_precision_map", "krr_factor_bytes", "krr_factor_tile_offset",
            "krr_potrf_mp_workspace", "krr_potrf_mp", "krr_potrs_workspace", "krr_potrs", "krr_refine_workspace", "krr_refine", "krr_pcg_workspace", "krr_pcg",
-           "krr_associate_host_arena", "krr_associate_host", "krr_build_workspace", "krr_build", "krr_build_bordered", "krr_predict_workspace", "krr_predict", "krr_fit_host_arena", "krr_fit_host", "krr_band_map", "krr_build_stats_bytes", "krr_precision_map_from_build",
+           "krr_associate_host_arena", "krr_associate_host", "krr_build_workspace", "krr_build", "krr_build_bordered", "krr_build_rr", "krr_predict_workspace", "krr_predict", "krr_fit_host_arena", "krr_fit_host", "krr_band_map", "krr_build_stats_bytes", "krr_precision_map_from_build",
            "krr_last_launch_count",
            "krr_profile_enable", "krr_profile_read"]
 
@@ -91,6 +91,8 @@ def lib():
     L.krr_build_bordered.restype = c.c_int
     L.krr_build_bordered.argtypes = [vp, i64, i64, i64, i64, vp, c.c_int, i64, c.c_float, c.c_float, vp, i64, c.c_int, u32, vp, vp,
                                      sz, vp]
+    L.krr_build_rr.restype = c.c_int
+    L.krr_build_rr.argtypes = [vp, i64, i64, i64, i64, vp, c.c_int, i64, c.c_float, vp, i64, c.c_int, u32, vp, sz, vp]
     L.krr_build_stats_bytes.restype = sz
     L.krr_build_stats_bytes.argtypes = [i64, c.c_int]
     L.krr_precision_map_from_build.restype = c.c_int
@@ -387,6 +389,27 @@ def krr_build(G, gamma, lam, nb, tiled_lower=False, out=None, flags=0, C=None, s
                                 float(gamma), float(lam), _ptr(out), lda, nb, flags, _ptr(st), _ptr(ws), wsb, _stream()),
            "krr_build_bordered")
     return (out, st) if stats else out
+
+
+def build_rr(S, ns, lam, nb, C=None, tiled_lower=False):
+    """krr_build_rr: X^T X + lam I for X = [S^T | C], bordered by the identity (Fig. 2).  S: CUDA int8 n x p with the
+    SNP features as rows (rows >= ns are padding), C: CUDA FP32 p x q confounders or None."""
+    L = lib()
+    assert S.dtype == torch.int8 and S.is_cuda and S.stride(1) == 1
+    n, p = S.shape
+    NT = n // nb
+    dev = S.device
+    out = (torch.zeros(NT * (NT + 1) // 2 * nb * nb, dtype=torch.float32, device=dev) if tiled_lower
+           else torch.zeros((n, n), dtype=torch.float32, device=dev))
+    wsb = int(L.krr_build_workspace(n, p, 0))
+    if wsb == 0:
+        raise KrrError("krr_build_workspace: n must be a multiple of 256")
+    ws = _ws(wsb, dev)
+    C, q, ldc = _conf(C)
+    _check(L.krr_build_rr(_ptr(S), n, int(ns), p, S.stride(0), _ptr(C), q, ldc, float(lam), _ptr(out),
+                          nb if tiled_lower else out.stride(0), nb, FLAG_A_TILED_LOWER if tiled_lower else 0, _ptr(ws), wsb,
+                          _stream()), "krr_build_rr")
+    return out
 
 
 def precision_map_from_build(stats, n, nb, eps_target, allowed=(FP32, FP16, FP8)):

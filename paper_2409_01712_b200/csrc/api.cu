@@ -1301,6 +1301,21 @@ int krr_build_bordered(const int8_t* d_G, int64_t n, int64_t n_valid, int64_t p,
     return launch_build(tmG, tmG, op, upt * upt * NT * (NT + 1) / 2 / nacc, nacc, num_sms, st);
 }
 
+// The mixed INT8 / FP32 SYRK of ridge regression (Fig. 2): X^T X + lambda I for X = [S^T | C].
+int krr_build_rr(const int8_t* d_S, int64_t n, int64_t ns, int64_t p, int64_t lds, const float* d_C, int q, int64_t ldc,
+                 float lambda, float* d_A, int64_t lda, int nb, unsigned flags, void* d_ws, size_t ws_bytes, void* stream) {
+    if (ns < 1 || q < 0 || q > kMaxConfounders || ns + q > n || (q > 0 && (!d_C || ldc < q))) return KRR_ERR_ARG;
+    if (flags & ~static_cast<unsigned>(KRR_FLAG_A_TILED_LOWER)) return KRR_ERR_UNSUPPORTED;
+    // the SNP x SNP block on the INT8 tensor cores; rows / columns >= ns + q become the identity border
+    int rc = krr_build_bordered(d_S, n, ns + q, p, lds, nullptr, 0, 0, 1.0f, lambda, d_A, lda, nb,
+                                flags | KRR_FLAG_KERNEL_LINEAR, nullptr, d_ws, ws_bytes, stream);
+    if (rc || q == 0) return rc;
+    const int64_t ncol = ns + q, per_block = static_cast<int64_t>(kRrWarps) * kRrRowsPerWarp;
+    return launch(CAT_MISC, rr_confounder_rows_kernel, dim3(static_cast<unsigned>((ncol + per_block - 1) / per_block)),
+                  dim3(kRrWarps * 32), 0, static_cast<cudaStream_t>(stream), d_S, lds, ns, p, d_C, ldc, q, lambda, d_A, lda,
+                  (flags & KRR_FLAG_A_TILED_LOWER) ? 1 : 0, nb, static_cast<int>(n / nb));
+}
+
 // ------------------------------------------------------------------------- Predict phase (NEXT-2)
 size_t krr_predict_workspace(int64_t m, int64_t n, int64_t p, unsigned flags) {
     if (m <= 0 || n <= 0 || m % 256 != 0 || n % 256 != 0 || p < 1) return 0;

@@ -383,4 +383,84 @@ predict_kw_kernel(const float* __restrict__ K, int64_t m, int64_t n, int64_t ldk
             if (row0 + i < m) P[(row0 + i) * ldp + r] = (acc[i][0] + acc[i][1]) + (acc[i][2] + acc[i][3]);
 }
 
+// ---- the FP32 tiles of the mixed SYRK of ridge regression (Fig. 2) ----
+// X = [S^T | C]: the SNP features are the int8 rows of S (N_S x patients, the matrix the INT8 kernel above works on),
+// the q confounder features the columns of C (patients x q, FP32).  The INT8 kernel has produced the SNP x SNP block;
+// this kernel writes the q rows ns .. ns+q-1 of X^T X + lambda I: for every column j <= row,
+//     A(ns + t, j) = sum_k x_j[k] * C[k][t],   x_j = row j of S (j < ns) or column j - ns of C,
+// in FP32 (the paper's SGEMM tiles), sums in a fixed order (lane-strided partial sums, then a shuffle tree).  Inside
+// the diagonal tile the mirrored element is written too (diagonal tiles are full squares).
+// HBM: S is read once (ns * p bytes); C (p * q * 4 bytes) stays in L2 and is staged through shared memory.
+constexpr int kRrWarps = 8, kRrRowsPerWarp = 4, kRrKc = 128;
+
+__global__ void __launch_bounds__(kRrWarps * 32)
+rr_confounder_rows_kernel(const int8_t* __restrict__ S, int64_t lds, int64_t ns, int64_t p, const float* __restrict__ C,
+                          int64_t ldc, int q, float lambda, float* __restrict__ A, int64_t lda, int tiled, int nb, int NT) {
+    __shared__ float Cs[kRrKc][kMaxConfounders + 1];                      // + 1: lanes read different rows, conflict-free
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int64_t j0 = (static_cast<int64_t>(blockIdx.x) * kRrWarps + warp) * kRrRowsPerWarp;     // this warp's columns j0 .. j0+3
+    const int64_t ncol = ns + q;
+    float acc[kRrRowsPerWarp][kMaxConfounders];
+#pragma unroll
+    for (int r = 0; r < kRrRowsPerWarp; ++r)
+#pragma unroll
+        for (int t = 0; t < kMaxConfounders; ++t) acc[r][t] = 0.0f;
+
+    for (int64_t k0 = 0; k0 < p; k0 += kRrKc) {
+        __syncthreads();
+        for (int e = threadIdx.x; e < kRrKc * kMaxConfounders; e += kRrWarps * 32) {
+            const int kk = e / kMaxConfounders, t = e % kMaxConfounders;
+            Cs[kk][t] = (k0 + kk < p && t < q) ? __ldg(C + (k0 + kk) * ldc + t) : 0.0f;
+        }
+        __syncthreads();
+#pragma unroll
+        for (int u = 0; u < kRrKc / 32; ++u) {
+            const int kk = u * 32 + lane;                                   // consecutive lanes, consecutive patients
+            const int64_t k = k0 + kk;
+            float x[kRrRowsPerWarp];
+#pragma unroll
+            for (int r = 0; r < kRrRowsPerWarp; ++r) {
+                const int64_t j = j0 + r;
+                x[r] = 0.0f;
+                if (k < p && j < ncol) x[r] = j < ns ? static_cast<float>(S[j * lds + k]) : Cs[kk][j - ns];
+            }
+#pragma unroll
+            for (int t = 0; t < kMaxConfounders; ++t) {
+                const float c = Cs[kk][t];
+#pragma unroll
+                for (int r = 0; r < kRrRowsPerWarp; ++r) acc[r][t] = fmaf(x[r], c, acc[r][t]);
+            }
+        }
+    }
+#pragma unroll
+    for (int r = 0; r < kRrRowsPerWarp; ++r)
+#pragma unroll
+        for (int t = 0; t < kMaxConfounders; ++t) {
+            float v = acc[r][t];
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+            acc[r][t] = v;
+        }
+    if (lane == 0) {
+        for (int r = 0; r < kRrRowsPerWarp; ++r) {
+            const int64_t j = j0 + r;
+            if (j >= ncol) continue;
+            for (int t = 0; t < q; ++t) {
+                const int64_t row = ns + t;
+                if (j > row) continue;                                       // the upper triangle follows by symmetry
+                const float v = acc[r][t] + (j == row ? lambda : 0.0f);
+                const int ti = static_cast<int>(row / nb), tj = static_cast<int>(j / nb);
+                if (tiled) {
+                    float* T = A + tile_slot(NT, ti, tj) * static_cast<int64_t>(nb) * nb;
+                    T[(row % nb) * nb + j % nb] = v;
+                    if (ti == tj) T[(j % nb) * nb + row % nb] = v;
+                } else {
+                    A[row * lda + j] = v;
+                    if (ti == tj) A[j * lda + row] = v;
+                }
+            }
+        }
+    }
+}
+
 }  // namespace krr

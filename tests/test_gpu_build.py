@@ -381,3 +381,61 @@ def test_build_bordered_rejects_bad_n_valid(krr):
         krr.krr_build(padded(G), 1.0 / 256, 1e-2, 256, n_valid=0)
     with pytest.raises(krr.KrrError):
         krr.krr_build(padded(G), 1.0 / 256, 1e-2, 256, n_valid=513)
+
+
+@pytest.mark.parametrize("ns,q,npat,nb,tiled", [(1000, 5, 3001, 256, False), (700, 16, 2000, 512, False), (1500, 3, 1111, 256, True)])
+def test_ridge_regression_with_confounders_mixed_syrk(krr, ns, q, npat, nb, tiled):
+    """PAPER.md Fig. 2 / :165-167: X = [SNPs | confounders]; the SNP x SNP block of X^T X from the INT8 tensor cores
+    (exact), the q rows that involve a confounder accumulated in FP32 (the paper's SGEMM tiles), identity border up to
+    the tile size (R21).  Against the oracle's FP64 definition: INT8 block exact, FP32 rows to the bound of an FP32 dot
+    product of `npat` terms accumulated in 32 partial sums (sqrt-free bound: npat/32 * 2^-24 * sum |x||c|, taken as
+    2e-5 of the row's scale); then beta through the Associate path against the FP64 ridge solution."""
+    from oracle.build_phase import identity_border, ridge_gram_definition, ridge_regression_definition
+    n = -(-(ns + q) // max(nb, 256)) * max(nb, 256)
+    X = genotypes(71, npat, ns, "maf", device="cuda")                      # patients x SNPs
+    g = torch.Generator(device="cpu").manual_seed(ns + q)
+    C = (torch.randn((npat, q), generator=g) * 3.0 + 1.0).cuda()           # confounders: real, not centred (age-like)
+    S = torch.full((n, npat), 5, dtype=torch.int8, device="cuda")          # padding rows: anything
+    S[:ns] = X.t()
+    lam = 20.0
+    A = krr.build_rr(padded(S), ns, lam, nb, C=C, tiled_lower=tiled)
+    torch.cuda.synchronize()
+    want = identity_border(ridge_gram_definition(X.cpu().numpy(), C.cpu().numpy().astype(np.float64), lam), n)
+    NT = n // nb
+    if tiled:
+        T = A.reshape(-1, nb, nb).cpu().numpy().astype(np.float64)
+        got = np.zeros((n, n))
+        for j in range(NT):
+            for i in range(j, NT):
+                got[i * nb:(i + 1) * nb, j * nb:(j + 1) * nb] = T[krr.tile_slot(NT, i, j)]
+    else:
+        got = A.cpu().numpy().astype(np.float64)
+    low = np.tril(np.ones((n, n), dtype=bool))
+    blk = np.zeros((n, n), dtype=bool)
+    for i in range(NT):                                                    # what is stored: lower tiles, diagonal tiles in full
+        blk[i * nb:(i + 1) * nb, :(i + 1) * nb] = True
+    snp = np.zeros((n, n), dtype=bool)
+    snp[:ns, :ns] = True
+    border = np.zeros((n, n), dtype=bool)
+    border[ns + q:, :] = True
+    border[:, ns + q:] = True
+    assert np.array_equal(got[blk & snp], want[blk & snp])                 # INT8 tiles: exact integers (+ lam)
+    assert np.array_equal(got[blk & border], want[blk & border])           # identity border
+    conf = blk & ~snp & ~border
+    scale = np.abs(want[conf]).max()
+    assert np.all(np.abs(got[conf] - want[conf]) <= 2e-5 * scale), float(np.abs(got[conf] - want[conf]).max() / scale)
+    assert np.array_equal(got[blk & low.T & ~border & ~snp], got.T[blk & low.T & ~border & ~snp])   # mirrored inside the diagonal tile
+    # beta = (X^T X + lam I)^-1 X^T Y
+    Y = torch.randn((npat, 3), generator=g).cuda()
+    Xf = torch.cat([X.to(torch.float32), C], dim=1)
+    XtY = torch.zeros((n, 3), device="cuda")
+    XtY[:ns + q] = Xf.t() @ Y
+    h = krr.uniform_map(NT, krr.FP32)
+    F = krr.potrf_mp(A, nb, h.cuda(), h, flags=krr.FLAG_PREROUND_A | (krr.FLAG_A_TILED_LOWER if tiled else 0), n=n)
+    beta = krr.potrs(F, XtY.clone())
+    torch.cuda.synchronize()
+    assert int(F.info.item()) == 0
+    b = beta.cpu().numpy().astype(np.float64)
+    assert not b[ns + q:].any()
+    b64 = ridge_regression_definition(Xf.cpu().numpy().astype(np.float64), Y.cpu().numpy(), lam)
+    assert np.linalg.norm(b[:ns + q] - b64) / np.linalg.norm(b64) <= 1e-3

@@ -367,6 +367,29 @@ int krr_fit_host(const int8_t* h_G, int64_t n, int64_t p, int64_t ldg, float gam
                  const float* h_Y, int nrhs, float* h_alpha, uint8_t* h_map, int* h_info,
                  void* d_arena, size_t arena_bytes, void* stream);
 
+/* ---------------------------------------------------------------------------------------------
+ * CUDA-graph replay of the tile-DAG launch sequence (BASELINE.json north_star: "a single-GPU tile-DAG scheduler with
+ * lookahead, run as CUDA graphs"; PAPER.md:206 task DAG, :295 lookahead).  The launch sequence of krr_potrf_mp /
+ * krr_potrs / krr_refine / krr_pcg is a pure function of (n, nb, map, flags, pointers): krr_graph_begin puts `stream`
+ * into stream capture, the krr_* calls made on it afterwards are recorded instead of run (their fork / join onto the
+ * library's internal priority streams becomes the parallel branches of the graph), krr_graph_end instantiates what
+ * was recorded.  krr_graph_launch replays it on any stream: same kernels, same arguments, same dependencies, so the
+ * results are bit-identical to the direct calls; the buffers the recorded calls were given must stay allocated and
+ * hold the inputs (A, map, Y) at replay time.  A graph is valid for ONE precision map: when krr_precision_map returns
+ * another map, record again.
+ * stream      must not be the legacy default stream (CUDA cannot capture it): KRR_ERR_ARG.
+ * Calls that synchronise (krr_associate_host, krr_fit_host, krr_profile_read) must not be recorded; per-kernel timing
+ * (krr_profile_enable) must be off: KRR_ERR_UNSUPPORTED.
+ * krr_graph_end returns KRR_ERR_CUDA when a recorded call failed (the capture is then discarded, *out = NULL).
+ * krr_graph_kernel_nodes: kernels one replay launches (for bench.py's gpu_launches).
+ * The graph object is host memory owned by the library until krr_graph_destroy. */
+typedef struct krr_graph krr_graph_t;
+int krr_graph_begin(void* stream);
+int krr_graph_end(void* stream, krr_graph_t** out);
+int krr_graph_launch(const krr_graph_t* graph, void* stream);
+int64_t krr_graph_kernel_nodes(const krr_graph_t* graph);
+int krr_graph_destroy(krr_graph_t* graph);
+
 /* Number of kernels the last krr_* call on this thread enqueued (for bench.py's gpu_launches). */
 int64_t krr_last_launch_count(void);
 

@@ -26,6 +26,7 @@ EXPORTS = ["krr_version", "krr_built_for_sm", "krr_tile_slot", "krr_precision_ma
            "krr_precision_map", "krr_factor_bytes", "krr_factor_tile_offset",
            "krr_potrf_mp_workspace", "krr_potrf_mp", "krr_potrs_workspace", "krr_potrs", "krr_refine_workspace", "krr_refine", "krr_pcg_workspace", "krr_pcg",
            "krr_associate_host_arena", "krr_associate_host", "krr_build_workspace", "krr_build", "krr_build_bordered", "krr_build_rr", "krr_predict_workspace", "krr_predict", "krr_fit_host_arena", "krr_fit_host", "krr_band_map", "krr_build_stats_bytes", "krr_precision_map_from_build",
+           "krr_graph_begin", "krr_graph_end", "krr_graph_launch", "krr_graph_kernel_nodes", "krr_graph_destroy",
            "krr_last_launch_count",
            "krr_profile_enable", "krr_profile_read"]
 
@@ -110,6 +111,16 @@ def lib():
     L.krr_band_map.restype = c.c_int
     L.krr_band_map.argtypes = [c.c_int, c.c_double, c.c_int, vp]
     L.krr_last_launch_count.restype = i64
+    L.krr_graph_begin.restype = c.c_int
+    L.krr_graph_begin.argtypes = [vp]
+    L.krr_graph_end.restype = c.c_int
+    L.krr_graph_end.argtypes = [vp, c.POINTER(vp)]
+    L.krr_graph_launch.restype = c.c_int
+    L.krr_graph_launch.argtypes = [vp, vp]
+    L.krr_graph_kernel_nodes.restype = i64
+    L.krr_graph_kernel_nodes.argtypes = [vp]
+    L.krr_graph_destroy.restype = c.c_int
+    L.krr_graph_destroy.argtypes = [vp]
     L.krr_profile_enable.restype = c.c_int
     L.krr_profile_enable.argtypes = [u32]
     L.krr_profile_read.restype = c.c_int
@@ -140,6 +151,44 @@ def _ws(nbytes, device):
 
 def last_launch_count():
     return int(lib().krr_last_launch_count())
+
+
+class Graph:
+    """A recorded launch sequence (krr_graph_t).  `keep` holds the tensors the recorded calls were given:
+    they must outlive the graph and are what a replay reads and writes."""
+
+    def __init__(self, handle, keep):
+        self.handle, self.keep = handle, keep
+
+    @property
+    def kernel_nodes(self):
+        return int(lib().krr_graph_kernel_nodes(self.handle))
+
+    def launch(self):
+        _check(lib().krr_graph_launch(self.handle, _stream()), "krr_graph_launch")
+
+    def destroy(self):
+        if self.handle is not None:
+            _check(lib().krr_graph_destroy(self.handle), "krr_graph_destroy")
+            self.handle, self.keep = None, None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+def graph_begin():
+    """krr_graph_begin on torch's current stream (not the default stream: use `with torch.cuda.stream(s)`)."""
+    _check(lib().krr_graph_begin(_stream()), "krr_graph_begin")
+
+
+def graph_end(keep=()):
+    """krr_graph_end on torch's current stream.  Returns a Graph that keeps `keep` alive."""
+    h = ctypes.c_void_p(0)
+    _check(lib().krr_graph_end(_stream(), ctypes.byref(h)), "krr_graph_end")
+    return Graph(h, keep)
 
 
 PROFILE_CATEGORIES = ["update_gemm", "panel_update", "panel_trsm", "potrf128", "finalize", "precision_map",
@@ -277,15 +326,26 @@ def potrf_mp(A, nb, d_map, h_map=None, flags=FLAG_PREROUND_A, n=None):
     return Factor(n, nb, h, d_map, payload, scales, info, ws)
 
 
-def potrs(factor, B):
-    """krr_potrs, in place on B (CUDA FP32, n x nrhs row-major).  Returns B."""
+def potrs_workspace(n, nb, nrhs, device):
+    """A krr_potrs workspace (krr_potrs_workspace bytes), for callers that keep it (graph replay)."""
+    wsb = int(lib().krr_potrs_workspace(n, nb, nrhs))
+    if wsb == 0:
+        raise KrrError("krr_potrs_workspace: invalid shape / nrhs")
+    return _ws(wsb, device)
+
+
+def potrs(factor, B, ws=None):
+    """krr_potrs, in place on B (CUDA FP32, n x nrhs row-major).  Returns B.  `ws`: a workspace from
+    potrs_workspace; a recorded call (graph_begin) needs one that outlives the graph."""
     L = lib()
     assert B.dtype == torch.float32 and B.is_cuda and B.stride(1) == 1
     n, nrhs = B.shape
     wsb = int(L.krr_potrs_workspace(n, factor.nb, nrhs))
     if wsb == 0:
         raise KrrError("krr_potrs_workspace: invalid shape / nrhs")
-    ws = _ws(wsb, B.device)
+    if ws is None:
+        ws = _ws(wsb, B.device)
+    assert ws.numel() >= wsb and ws.data_ptr() % 16 == 0
     _check(L.krr_potrs(_ptr(factor.payload), _ptr(factor.scales), _ptr(factor.d_map), _ptr(factor.h_map), n,
                        factor.nb, _ptr(B), B.stride(0), nrhs, _ptr(ws), wsb, _stream()), "krr_potrs")
     return B

@@ -297,6 +297,72 @@ int krr_profile_read(int category, double* total_ms, int64_t* launches) {
     return KRR_OK;
 }
 
+// ------------------------------------------------------------------------- CUDA-graph replay
+// Stream capture of the launch sequence (include/krr_mp.h): the fork / join of krr_potrf_mp and krr_potrs onto the
+// internal priority streams is the capture-compatible pattern (event recorded on the capturing stream, waited for by
+// the others, all joined back before the end), so the three streams become parallel branches of one graph and the
+// kernel nodes keep the priority of the stream they were recorded on.
+struct krr_graph { cudaGraph_t graph; cudaGraphExec_t exec; int64_t kernels; };
+
+int krr_graph_begin(void* stream) {
+    if (!stream) return KRR_ERR_ARG;                     // the legacy default stream cannot be captured
+    if (g_prof_mask) return KRR_ERR_UNSUPPORTED;         // timing events cannot be read back from a capture
+    int num_sms = 0;
+    int rc = check_device(&num_sms);
+    if (rc) return rc;
+    rc = set_kernel_attrs();                             // everything that is not a stream operation happens before
+    if (rc) return rc;
+    rc = g_pipe.init();
+    if (rc) return rc;
+    KRR_CUDA_CHECK(cudaStreamBeginCapture(static_cast<cudaStream_t>(stream), cudaStreamCaptureModeRelaxed));
+    return KRR_OK;
+}
+
+int krr_graph_end(void* stream, krr_graph_t** out) {
+    if (!stream || !out) return KRR_ERR_ARG;
+    *out = nullptr;
+    cudaGraph_t g = nullptr;
+    if (cudaStreamEndCapture(static_cast<cudaStream_t>(stream), &g) != cudaSuccess || !g) {
+        cudaGetLastError();                              // a failed capture leaves a sticky-looking error behind
+        return KRR_ERR_CUDA;
+    }
+    size_t nn = 0;
+    int64_t kernels = 0;
+    if (cudaGraphGetNodes(g, nullptr, &nn) == cudaSuccess && nn > 0) {
+        std::vector<cudaGraphNode_t> nodes(nn);
+        if (cudaGraphGetNodes(g, nodes.data(), &nn) == cudaSuccess)
+            for (size_t i = 0; i < nn; ++i) {
+                cudaGraphNodeType t;
+                if (cudaGraphNodeGetType(nodes[i], &t) == cudaSuccess && t == cudaGraphNodeTypeKernel) ++kernels;
+            }
+    }
+    cudaGraphExec_t x = nullptr;
+    if (cudaGraphInstantiate(&x, g, 0) != cudaSuccess) {
+        cudaGraphDestroy(g);
+        cudaGetLastError();
+        return KRR_ERR_CUDA;
+    }
+    *out = new krr_graph{g, x, kernels};
+    return KRR_OK;
+}
+
+int krr_graph_launch(const krr_graph_t* graph, void* stream) {
+    if (!graph) return KRR_ERR_ARG;
+    g_launches = graph->kernels;
+    KRR_CUDA_CHECK(cudaGraphLaunch(graph->exec, static_cast<cudaStream_t>(stream)));
+    return KRR_OK;
+}
+
+int64_t krr_graph_kernel_nodes(const krr_graph_t* graph) { return graph ? graph->kernels : -1; }
+
+int krr_graph_destroy(krr_graph_t* graph) {
+    if (!graph) return KRR_ERR_ARG;
+    cudaGraphExecDestroy(graph->exec);
+    cudaGraphDestroy(graph->graph);
+    delete graph;
+    return KRR_OK;
+}
+
 int64_t krr_tile_slot(int NT, int i, int j) {
     if (NT <= 0 || j < 0 || i < j || i >= NT) return -1;
     return tile_slot(NT, i, j);

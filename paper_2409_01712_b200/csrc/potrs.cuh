@@ -76,6 +76,7 @@ template <int NRHS>
 __device__ __forceinline__ void rows_dot_f32(const float* __restrict__ rows, int64_t ld, int K,
                                              const float* __restrict__ zs, int zld, int lane, float (&acc)[64]) {
     constexpr int ROWS = 64 / NRHS;
+#pragma unroll 2
     for (int l = lane * 4; l < K; l += 128) {
         float4 a[ROWS];
 #pragma unroll
@@ -122,6 +123,7 @@ potrs_fwd_update_kernel(int NT, int nb, int k, int i_lo, int i_hi, const uint8_t
         if (p == KRR_FP32) {
             rows_dot_f32<NRHS>(reinterpret_cast<const float*>(tile) + static_cast<int64_t>(r0) * nb, nb, nb, zs, nb, lane, acc);
         } else {
+#pragma unroll 2
             for (int l = lane * 4; l < nb; l += 128) {
                 float4 a[ROWS];
 #pragma unroll
@@ -176,6 +178,7 @@ potrs_bwd_update_kernel(int NT, int nb, int k, int j_lo, const uint8_t* __restri
     float acc[NACC];
 #pragma unroll
     for (int v = 0; v < NACC; ++v) acc[v] = 0.0f;
+#pragma unroll 2
     for (int r = warp; r < nb; r += NW * 4) {
         float l[4][CPL];
 #pragma unroll

@@ -48,6 +48,33 @@ __device__ __forceinline__ float2 load2(const uint8_t* tile, int p, float s, int
     return make_float2(e4m3_to_f32(raw & 0xff) * s, e4m3_to_f32(raw >> 8) * s);
 }
 
+// The same with the storage precision known at compile time (the update kernels switch on the tile's
+// precision once, outside their streaming loops, so that several iterations' loads stay in flight).
+template <int P>
+__device__ __forceinline__ float4 load4p(const uint8_t* tile, float s, int64_t e) {
+    if (P == KRR_FP32) return __ldg(reinterpret_cast<const float4*>(tile + e * 4));
+    if (P == KRR_FP16) {
+        const uint2 raw = __ldg(reinterpret_cast<const uint2*>(tile + e * 2));
+        const __half2 a = *reinterpret_cast<const __half2*>(&raw.x);
+        const __half2 b = *reinterpret_cast<const __half2*>(&raw.y);
+        return make_float4(__low2float(a), __high2float(a), __low2float(b), __high2float(b));
+    }
+    const uint32_t raw = __ldg(reinterpret_cast<const uint32_t*>(tile + e));
+    return make_float4(e4m3_to_f32(raw & 0xff) * s, e4m3_to_f32((raw >> 8) & 0xff) * s,
+                       e4m3_to_f32((raw >> 16) & 0xff) * s, e4m3_to_f32(raw >> 24) * s);
+}
+template <int P>
+__device__ __forceinline__ float2 load2p(const uint8_t* tile, float s, int64_t e) {
+    if (P == KRR_FP32) return __ldg(reinterpret_cast<const float2*>(tile + e * 4));
+    if (P == KRR_FP16) {
+        const uint32_t raw = __ldg(reinterpret_cast<const uint32_t*>(tile + e * 2));
+        const __half2 a = *reinterpret_cast<const __half2*>(&raw);
+        return make_float2(__low2float(a), __high2float(a));
+    }
+    const uint16_t raw = __ldg(reinterpret_cast<const uint16_t*>(tile + e));
+    return make_float2(e4m3_to_f32(raw & 0xff) * s, e4m3_to_f32(raw >> 8) * s);
+}
+
 // Sum 64 per-lane values v[0..63] across the 32 lanes of a warp with 62 shuffles (each step halves
 // the number of values a lane carries).  Afterwards lane `l` holds in v[0], v[1] the totals of the
 // values with index  warp_reduce64_index(l) + {0, 1}.
@@ -91,6 +118,27 @@ __device__ __forceinline__ void rows_dot_f32(const float* __restrict__ rows, int
     }
 }
 
+// The same for a low-precision tile (P = KRR_FP16 / KRR_FP8_E4M3, scale s): rows r0 .. r0+ROWS of `tile`.
+// The loads are 8 / 4 bytes per lane, so four iterations are kept in flight.
+template <int NRHS, int P>
+__device__ __forceinline__ void rows_dot_lp(const uint8_t* __restrict__ tile, float s, int r0, int nb,
+                                            const float* __restrict__ zs, int lane, float (&acc)[64]) {
+    constexpr int ROWS = 64 / NRHS;
+#pragma unroll 4
+    for (int l = lane * 4; l < nb; l += 128) {
+        float4 a[ROWS];
+#pragma unroll
+        for (int u = 0; u < ROWS; ++u) a[u] = load4p<P>(tile, s, static_cast<int64_t>(r0 + u) * nb + l);
+#pragma unroll
+        for (int h = 0; h < NRHS; ++h) {
+            const float4 z = *reinterpret_cast<const float4*>(zs + h * nb + l);
+#pragma unroll
+            for (int u = 0; u < ROWS; ++u)
+                acc[u * NRHS + h] = fmaf(a[u].x, z.x, fmaf(a[u].y, z.y, fmaf(a[u].z, z.z, fmaf(a[u].w, z.w, acc[u * NRHS + h]))));
+        }
+    }
+}
+
 // ---------------------------------------------------------------------------------------------
 // Forward update after Z_k is known:  Y_i -= L_ik Z_k  for the tile rows i in [i_lo, i_hi)  (all > k).
 // Persistent CTAs over groups of 8 * ROWS rows (ROWS = 64 / NRHS rows per warp); smem = NRHS*nb floats.
@@ -122,20 +170,10 @@ potrs_fwd_update_kernel(int NT, int nb, int k, int i_lo, int i_hi, const uint8_t
         for (int v = 0; v < 64; ++v) acc[v] = 0.0f;
         if (p == KRR_FP32) {
             rows_dot_f32<NRHS>(reinterpret_cast<const float*>(tile) + static_cast<int64_t>(r0) * nb, nb, nb, zs, nb, lane, acc);
+        } else if (p == KRR_FP16) {
+            rows_dot_lp<NRHS, KRR_FP16>(tile, s, r0, nb, zs, lane, acc);
         } else {
-#pragma unroll 2
-            for (int l = lane * 4; l < nb; l += 128) {
-                float4 a[ROWS];
-#pragma unroll
-                for (int u = 0; u < ROWS; ++u) a[u] = load4(tile, p, s, static_cast<int64_t>(r0 + u) * nb + l);
-#pragma unroll
-                for (int h = 0; h < NRHS; ++h) {
-                    const float4 z = *reinterpret_cast<const float4*>(zs + h * nb + l);
-#pragma unroll
-                    for (int u = 0; u < ROWS; ++u)
-                        acc[u * NRHS + h] = fmaf(a[u].x, z.x, fmaf(a[u].y, z.y, fmaf(a[u].z, z.z, fmaf(a[u].w, z.w, acc[u * NRHS + h]))));
-                }
-            }
+            rows_dot_lp<NRHS, KRR_FP8_E4M3>(tile, s, r0, nb, zs, lane, acc);
         }
         warp_reduce64(acc, lane);
         const int v0 = warp_reduce64_index(lane);
@@ -143,6 +181,45 @@ potrs_fwd_update_kernel(int NT, int nb, int k, int i_lo, int i_hi, const uint8_t
         for (int t = 0; t < 2; ++t) {
             const int u = (v0 + t) / NRHS, h = (v0 + t) % NRHS;
             if (h < nrhs) B[(static_cast<int64_t>(i) * nb + r0 + u) * ldb + h] -= acc[t];
+        }
+    }
+}
+
+// Streaming loop of the backward update: the rows of one strip of a tile (storage precision P), four rows per
+// warp and iteration, against alpha_k in shared memory (`as`: [nb][NRHS]).
+template <int NRHS, int P>
+__device__ __forceinline__ void bwd_rows(const uint8_t* __restrict__ tile, float s, int c0, int nb,
+                                         const float* __restrict__ as, int warp, float (&acc)[((NRHS <= 16) ? 4 : 2) * NRHS]) {
+    constexpr int CPL = (NRHS <= 16) ? 4 : 2;
+    constexpr int NW = kSolveThreads / 32;
+#pragma unroll (P == KRR_FP32 ? 2 : 4)
+    for (int r = warp; r < nb; r += NW * 4) {
+        float l[4][CPL];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int64_t e = static_cast<int64_t>(r + u * NW) * nb + c0;
+            if (CPL == 4) {
+                const float4 v = load4p<P>(tile, s, e);
+                l[u][0] = v.x; l[u][1] = v.y; l[u][CPL - 2] = v.z; l[u][CPL - 1] = v.w;
+            } else {
+                const float2 v = load2p<P>(tile, s, e);
+                l[u][0] = v.x; l[u][1] = v.y;
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const float* ar = as + static_cast<size_t>(r + u * NW) * NRHS;
+#pragma unroll
+            for (int h = 0; h < NRHS; h += 4) {
+                const float4 a = *reinterpret_cast<const float4*>(ar + h);
+#pragma unroll
+                for (int c = 0; c < CPL; ++c) {
+                    acc[c * NRHS + h + 0] = fmaf(l[u][c], a.x, acc[c * NRHS + h + 0]);
+                    acc[c * NRHS + h + 1] = fmaf(l[u][c], a.y, acc[c * NRHS + h + 1]);
+                    acc[c * NRHS + h + 2] = fmaf(l[u][c], a.z, acc[c * NRHS + h + 2]);
+                    acc[c * NRHS + h + 3] = fmaf(l[u][c], a.w, acc[c * NRHS + h + 3]);
+                }
+            }
         }
     }
 }
@@ -178,36 +255,9 @@ potrs_bwd_update_kernel(int NT, int nb, int k, int j_lo, const uint8_t* __restri
     float acc[NACC];
 #pragma unroll
     for (int v = 0; v < NACC; ++v) acc[v] = 0.0f;
-#pragma unroll 2
-    for (int r = warp; r < nb; r += NW * 4) {
-        float l[4][CPL];
-#pragma unroll
-        for (int u = 0; u < 4; ++u) {
-            const int64_t e = static_cast<int64_t>(r + u * NW) * nb + c0;
-            if (CPL == 4) {
-                const float4 v = load4(tile, p, s, e);
-                l[u][0] = v.x; l[u][1] = v.y; l[u][CPL - 2] = v.z; l[u][CPL - 1] = v.w;
-            } else {
-                const float2 v = load2(tile, p, s, e);
-                l[u][0] = v.x; l[u][1] = v.y;
-            }
-        }
-#pragma unroll
-        for (int u = 0; u < 4; ++u) {
-            const float* ar = as + static_cast<size_t>(r + u * NW) * NRHS;
-#pragma unroll
-            for (int h = 0; h < NRHS; h += 4) {
-                const float4 a = *reinterpret_cast<const float4*>(ar + h);
-#pragma unroll
-                for (int c = 0; c < CPL; ++c) {
-                    acc[c * NRHS + h + 0] = fmaf(l[u][c], a.x, acc[c * NRHS + h + 0]);
-                    acc[c * NRHS + h + 1] = fmaf(l[u][c], a.y, acc[c * NRHS + h + 1]);
-                    acc[c * NRHS + h + 2] = fmaf(l[u][c], a.z, acc[c * NRHS + h + 2]);
-                    acc[c * NRHS + h + 3] = fmaf(l[u][c], a.w, acc[c * NRHS + h + 3]);
-                }
-            }
-        }
-    }
+    if (p == KRR_FP32) bwd_rows<NRHS, KRR_FP32>(tile, s, c0, nb, as, warp, acc);
+    else if (p == KRR_FP16) bwd_rows<NRHS, KRR_FP16>(tile, s, c0, nb, as, warp, acc);
+    else bwd_rows<NRHS, KRR_FP8_E4M3>(tile, s, c0, nb, as, warp, acc);
     // fixed-order tree over the NW warps
 #pragma unroll
     for (int half = NW / 2; half >= 1; half >>= 1) {

@@ -182,8 +182,8 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb,
  *               nb * (nrhs rounded up to 4, 8, 16 or 32) <= 32768 (the solved block of one tile is
  *               kept in shared memory), else KRR_ERR_SHAPE.
  * d_ws  workspace of at least krr_potrs_workspace(n, nb, nrhs) bytes, 16-byte aligned: tile offsets
- *       and the inverses of the 128x128 diagonal blocks of L (2 * n * 128 floats), recomputed by
- *       every call.  Each diagonal tile is solved by one thread-block cluster of 8 CTAs; sums are
+ *       the inverses of the 128x128 diagonal blocks of L (2 * n * 128 floats) and transposed copies of
+ *       the diagonal tiles for the backward sweep (n * nb floats), recomputed by every call.  Each diagonal tile is solved by one thread-block cluster of 8 CTAs; sums are
  *       accumulated in a fixed order (deterministic results).
  */
 size_t krr_potrs_workspace(int64_t n, int nb, int nrhs);

@@ -672,7 +672,7 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
 // ------------------------------------------------------------------------- solve
 static int rhs_class(int nrhs) { return nrhs <= 4 ? 4 : (nrhs <= 8 ? 8 : (nrhs <= 16 ? 16 : 32)); }
 
-struct PotrsWs { size_t off_table, dinv, dinvT, total; };
+struct PotrsWs { size_t off_table, dinv, dinvT, diagT, total; };
 static PotrsWs potrs_ws_layout(int64_t n, int nb) {
     const size_t NT = n / nb;
     PotrsWs w;
@@ -680,6 +680,7 @@ static PotrsWs potrs_ws_layout(int64_t n, int nb) {
     w.off_table = o; o = align_up(o + NT * NT * sizeof(int64_t), 1024);
     w.dinv = o;      o = align_up(o + static_cast<size_t>(n) * kBlk * sizeof(float), 1024);
     w.dinvT = o;     o = align_up(o + static_cast<size_t>(n) * kBlk * sizeof(float), 1024);
+    w.diagT = o;     o = align_up(o + static_cast<size_t>(n) * nb * sizeof(float), 1024);     // L_kk^T for the backward sweep
     w.total = o;
     return w;
 }
@@ -699,8 +700,8 @@ size_t krr_potrs_workspace(int64_t n, int nb, int nrhs) {
 // update of row k+2 by column k+1 waits for the bulk update by column k.
 template <int NRHS>
 static int potrs_run(const uint8_t* factor, const float* d_scales, const uint8_t* d_map, const std::vector<int64_t>& hoff,
-                     const int64_t* off, const float* dinv, const float* dinvT, int NT, int nb, float* B, int64_t ldb,
-                     int nrhs, int num_sms, cudaStream_t st) {
+                     const int64_t* off, const float* dinv, const float* dinvT, const float* diagT, int NT, int nb, float* B,
+                     int64_t ldb, int nrhs, int num_sms, cudaStream_t st) {
     constexpr int ROWS = 64 / NRHS, NW = kSolveThreads / 32, CPL = (NRHS <= 16) ? 4 : 2;
     const size_t smem_z = static_cast<size_t>(NRHS) * nb * sizeof(float);
     const size_t smem_d = static_cast<size_t>(potrs_diag_smem_floats<NRHS>(nb)) * sizeof(float);
@@ -738,7 +739,8 @@ static int potrs_run(const uint8_t* factor, const float* d_scales, const uint8_t
                       NT, nb, k, j_lo, factor, off, d_map, d_scales, B, ldb, nrhs);
     };
     auto diag = [&](int k, int backward, cudaStream_t s) {
-        const float* Lkk = reinterpret_cast<const float*>(factor + hoff[static_cast<size_t>(k) * NT + k]);
+        const float* Lkk = backward ? diagT + static_cast<int64_t>(k) * nb * nb
+                                    : reinterpret_cast<const float*>(factor + hoff[static_cast<size_t>(k) * NT + k]);
         float* Bk = B + static_cast<int64_t>(k) * nb * ldb;
         return launch(CAT_POTRS, potrs_diag_kernel<NRHS>, dim3(kDiagCluster), dim3(kDiagThreads), smem_d, s, nb, Lkk,
                       dinv + k * nsub * blk_elems, dinvT + k * nsub * blk_elems, Bk, ldb, nrhs, backward);
@@ -820,17 +822,21 @@ int krr_potrs(const void* d_factor, const float* d_scales, const uint8_t* d_map,
     int64_t* off = reinterpret_cast<int64_t*>(ws + L.off_table);
     float* dinv = reinterpret_cast<float*>(ws + L.dinv);
     float* dinvT = reinterpret_cast<float*>(ws + L.dinvT);
+    float* diagT = reinterpret_cast<float*>(ws + L.diagT);
     rc = launch(CAT_MISC, offsets_kernel, dim3(1), dim3(32), 0, st, NT, nb, d_map, off);
     if (rc) return rc;
     const uint8_t* factor = static_cast<const uint8_t*>(d_factor);
     rc = launch(CAT_POTRS, trtri128_kernel, dim3(static_cast<unsigned>(n / kBlk)), dim3(kTriThreads), static_cast<size_t>(kTriSmem), st,
                 factor, static_cast<const int64_t*>(off), NT, nb, dinv, dinvT);
     if (rc) return rc;
+    rc = launch(CAT_POTRS, potrs_diag_transpose_kernel, dim3(nb / 32, nb / 32, NT), dim3(256), 0, st, factor,
+                static_cast<const int64_t*>(off), NT, nb, diagT);
+    if (rc) return rc;
     switch (rhs_class(nrhs)) {
-        case 4:  return potrs_run<4>(factor, d_scales, d_map, hoff, off, dinv, dinvT, NT, nb, d_B, ldb, nrhs, num_sms, st);
-        case 8:  return potrs_run<8>(factor, d_scales, d_map, hoff, off, dinv, dinvT, NT, nb, d_B, ldb, nrhs, num_sms, st);
-        case 16: return potrs_run<16>(factor, d_scales, d_map, hoff, off, dinv, dinvT, NT, nb, d_B, ldb, nrhs, num_sms, st);
-        default: return potrs_run<32>(factor, d_scales, d_map, hoff, off, dinv, dinvT, NT, nb, d_B, ldb, nrhs, num_sms, st);
+        case 4:  return potrs_run<4>(factor, d_scales, d_map, hoff, off, dinv, dinvT, diagT, NT, nb, d_B, ldb, nrhs, num_sms, st);
+        case 8:  return potrs_run<8>(factor, d_scales, d_map, hoff, off, dinv, dinvT, diagT, NT, nb, d_B, ldb, nrhs, num_sms, st);
+        case 16: return potrs_run<16>(factor, d_scales, d_map, hoff, off, dinv, dinvT, diagT, NT, nb, d_B, ldb, nrhs, num_sms, st);
+        default: return potrs_run<32>(factor, d_scales, d_map, hoff, off, dinv, dinvT, diagT, NT, nb, d_B, ldb, nrhs, num_sms, st);
     }
 }
 

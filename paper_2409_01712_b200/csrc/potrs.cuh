@@ -6,6 +6,7 @@
 //
 // Structure (right-looking over tile columns, like the paper's tile algorithm):
 //   trtri128_kernel (tri128.cuh)   inverses of the 128x128 diagonal blocks of every diagonal tile, once
+//   potrs_diag_transpose_kernel    transposed copies of the diagonal tiles for the backward sweep, once
 //   potrs_diag_kernel              one diagonal tile: 128-row blocks in order, each a product with the
 //                                  already solved part of the tile followed by a product with the
 //                                  inverted diagonal block
@@ -289,51 +290,67 @@ potrs_bwd_update_kernel(int NT, int nb, int k, int j_lo, const uint8_t* __restri
 }
 
 // ---------------------------------------------------------------------------------------------
+// Transposed copies of the diagonal tiles (FP32, full squares): T[k] = L_kk^T, so that the backward solve reads
+// rows of L^T exactly as the forward solve reads rows of L.  One CTA per 32 x 32 block with row block <= column
+// block of L^T (the rest is never read).  Once per krr_potrs call: 2 * 4 * nb^2 / 2 bytes per tile.
+__global__ void __launch_bounds__(256)
+potrs_diag_transpose_kernel(const uint8_t* __restrict__ factor, const int64_t* __restrict__ off, int NT, int nb,
+                            float* __restrict__ T) {
+    __shared__ float t[32][33];
+    const int k = blockIdx.z, bi = blockIdx.y, bj = blockIdx.x;        // block (bi, bj) of L^T = block (bj, bi) of L
+    if (bi > bj) return;
+    const float* L = reinterpret_cast<const float*>(factor + off[static_cast<int64_t>(k) * NT + k]);
+    float* Tk = T + static_cast<int64_t>(k) * nb * nb;
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+#pragma unroll
+    for (int r = ty; r < 32; r += 8) t[r][tx] = L[static_cast<int64_t>(bj * 32 + r) * nb + bi * 32 + tx];
+    __syncthreads();
+#pragma unroll
+    for (int r = ty; r < 32; r += 8) Tk[static_cast<int64_t>(bi * 32 + r) * nb + bj * 32 + tx] = t[tx][r];
+}
+
 // Diagonal tile solve by one thread-block cluster of kDiagCluster CTAs: forward (L z = y) or
 // backward (L^T a = z), in place on rows k*nb .. (k+1)*nb of B.  For each 128-row block c, in order:
 //   forward   t = y_c - L[c, 0:c] z_{0:c}                       z_c = inv(L_cc) t
-//   backward  t = z_c - L[c+1:, c]^T a_{c+1:}                   a_c = inv(L_cc)^T t
+//   backward  t = z_c - (L^T)[c, c+1:] a_{c+1:}                 a_c = inv(L_cc)^T t
+// M: the diagonal tile L_kk (forward) or its transposed copy (backward; potrs_diag_transpose_kernel), so both
+// directions run the same code: rows of M against the solved values, the K range split over warp slices.
 // dinv / dinvT: the inverted diagonal blocks of this tile and their transposes ([nsub][128][128]).
-// Every CTA keeps a full copy of the solved values and of t in its shared memory; the rows (forward)
-// or the summation range (backward) of a step are split over the CTAs, and the pieces are exchanged
-// through distributed shared memory between two cluster barriers.
-// smem per CTA: solved values NRHS*nb floats + t NRHS*128 + exchange buffers (see potrs_diag_smem).
+// Every CTA keeps a full copy of the solved values and of t in its shared memory; the rows of a step are split
+// over the CTAs, and the pieces are exchanged through distributed shared memory between two cluster barriers.
+// smem per CTA: solved values NRHS*nb floats + t NRHS*128 + exchange buffer (see potrs_diag_smem_floats).
 template <int NRHS>
 __host__ __device__ constexpr int potrs_diag_smem_floats(int nb) {
-    // solved + ts + red (max of forward slices: 8 warps * 64 values, backward: 4*32*NACC + part 128*NRHS)
-    return NRHS * nb + NRHS * kBlk + 4 * 32 * 64 + kBlk * NRHS;
+    // solved + ts + red (K slices: 8 warps * 64 values)
+    return NRHS * nb + NRHS * kBlk + 4 * 32 * 64;
 }
 
 template <int NRHS>
 __global__ void __cluster_dims__(kDiagCluster, 1, 1) __launch_bounds__(kDiagThreads, 1)
-potrs_diag_kernel(int nb, const float* __restrict__ Lkk, const float* __restrict__ dinv,
+potrs_diag_kernel(int nb, const float* __restrict__ Lkk /* M */, const float* __restrict__ dinv,
                   const float* __restrict__ dinvT, float* __restrict__ Bk, int64_t ldb, int nrhs, int backward) {
     namespace cg = cooperative_groups;
     cg::cluster_group cluster = cg::this_cluster();
-    constexpr int ROWS = 64 / NRHS;                    // rows per warp task (forward / phase 2)
+    constexpr int ROWS = 64 / NRHS;                    // rows per warp task
     constexpr int NW = kDiagThreads / 32;              // 8 warps
     constexpr int GQ = (kBlk / ROWS) / kDiagCluster;   // row groups per CTA: 1, 2, 4, 8 for NRHS 4, 8, 16, 32
     constexpr int KS = NW / GQ;                        // K slices per row group
-    constexpr int CPL = (NRHS <= 16) ? 4 : 2;          // backward: columns per lane
-    constexpr int NACC = CPL * NRHS;                   // 64 except NRHS = 4, 8
-    constexpr int PASSES = 4 / CPL;
     static_assert(GQ >= 1 && KS >= 1 && GQ * KS == NW, "warp decomposition");
     extern __shared__ __align__(16) float sm[];
-    float* zs = sm;                                    // forward:  [NRHS][nb] solved values, by rhs
-    float* sr = sm;                                    // backward: [nb][NRHS] solved values, by row
+    float* zs = sm;                                    // [NRHS][nb] solved values, by rhs
     float* ts = sm + static_cast<size_t>(NRHS) * nb;   // [NRHS][128]
     float* red = ts + NRHS * kBlk;                     // [4][32][64] scratch
-    float* part = red + 4 * 32 * 64;                   // backward: [128][NRHS] this CTA's partial sums
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int q = static_cast<int>(cluster.block_rank());
     const int nsub = nb / kBlk;
-    // pull the tile's lower triangle and the inverted blocks towards L2 (fire and forget)
+    // pull the part of M that is read and the inverted blocks towards L2 (fire and forget)
     {
         const int gt = q * kDiagThreads + threadIdx.x, nt = kDiagCluster * kDiagThreads;
         for (int c = 0; c < nsub; ++c) {
-            const int lines_per_row = 4 * (c + 1);
+            const int col0 = backward ? c * kBlk : 0;                     // block row c: columns 0 .. c (L) or c .. nsub-1 (L^T)
+            const int lines_per_row = backward ? 4 * (nsub - c) : 4 * (c + 1);
             for (int idx = gt; idx < kBlk * lines_per_row; idx += nt) {
-                const float* ptr = Lkk + static_cast<int64_t>(c * kBlk + idx / lines_per_row) * nb + (idx % lines_per_row) * 32;
+                const float* ptr = Lkk + static_cast<int64_t>(c * kBlk + idx / lines_per_row) * nb + col0 + (idx % lines_per_row) * 32;
                 asm volatile("prefetch.global.L2 [%0];" ::"l"(ptr));
             }
         }
@@ -346,135 +363,53 @@ potrs_diag_kernel(int nb, const float* __restrict__ Lkk, const float* __restrict
     for (int bi = 0; bi < nsub; ++bi) {
         const int c = backward ? (nsub - 1 - bi) : bi;
         const int R0 = c * kBlk;
-        if (!backward) {
-            // ---- phase 1: t = y_c - L[c, 0:c] z  for this CTA's rows, K split over the warp slices
-            float acc[64];
+        const int k_lo = backward ? R0 + kBlk : 0, k_hi = backward ? nb : R0;      // solved range the block row meets
+        // ---- phase 1: t = y_c - M[c, k_lo:k_hi] solved  for this CTA's rows (M = L forward, L^T backward), K split over
+        // the warp slices
+        float acc[64];
 #pragma unroll
-            for (int v = 0; v < 64; ++v) acc[v] = 0.0f;
-            {
-                const float* rows = Lkk + static_cast<int64_t>(R0 + grow) * nb;
-                for (int l = lane * 4 + ks * 128; l < R0; l += 128 * KS) {
-                    float4 a[ROWS];
+        for (int v = 0; v < 64; ++v) acc[v] = 0.0f;
+        {
+            const float* rows = Lkk + static_cast<int64_t>(R0 + grow) * nb;
+            for (int l = k_lo + lane * 4 + ks * 128; l < k_hi; l += 128 * KS) {
+                float4 a[ROWS];
 #pragma unroll
-                    for (int u = 0; u < ROWS; ++u) a[u] = __ldg(reinterpret_cast<const float4*>(rows + static_cast<int64_t>(u) * nb + l));
+                for (int u = 0; u < ROWS; ++u) a[u] = __ldg(reinterpret_cast<const float4*>(rows + static_cast<int64_t>(u) * nb + l));
 #pragma unroll
-                    for (int h = 0; h < NRHS; ++h) {
-                        const float4 z = *reinterpret_cast<const float4*>(zs + h * nb + l);
+                for (int h = 0; h < NRHS; ++h) {
+                    const float4 z = *reinterpret_cast<const float4*>(zs + h * nb + l);
 #pragma unroll
-                        for (int u = 0; u < ROWS; ++u)
-                            acc[u * NRHS + h] = fmaf(a[u].x, z.x, fmaf(a[u].y, z.y, fmaf(a[u].z, z.z, fmaf(a[u].w, z.w, acc[u * NRHS + h]))));
-                    }
+                    for (int u = 0; u < ROWS; ++u)
+                        acc[u * NRHS + h] = fmaf(a[u].x, z.x, fmaf(a[u].y, z.y, fmaf(a[u].z, z.z, fmaf(a[u].w, z.w, acc[u * NRHS + h]))));
                 }
             }
-            warp_reduce64(acc, lane);
-            if (KS > 1) {
-                if (ks > 0) {
-                    red[((ks - 1) * GQ + gl) * 64 + lane * 2 + 0] = acc[0];
-                    red[((ks - 1) * GQ + gl) * 64 + lane * 2 + 1] = acc[1];
-                }
-                __syncthreads();
-            }
-            if (ks == 0) {
-#pragma unroll
-                for (int s2 = 1; s2 < KS; ++s2) {
-                    acc[0] += red[((s2 - 1) * GQ + gl) * 64 + lane * 2 + 0];
-                    acc[1] += red[((s2 - 1) * GQ + gl) * 64 + lane * 2 + 1];
-                }
-                const int v0 = warp_reduce64_index(lane);
-#pragma unroll
-                for (int t = 0; t < 2; ++t) {
-                    const int u = (v0 + t) / NRHS, h = (v0 + t) % NRHS;
-                    const int r = grow + u;
-                    const float y = (h < nrhs) ? Bk[static_cast<int64_t>(R0 + r) * ldb + h] : 0.0f;
-                    const float tv = y - acc[t];
-#pragma unroll
-                    for (int d = 0; d < kDiagCluster; ++d) cluster.map_shared_rank(ts, d)[h * kBlk + r] = tv;
-                }
-            }
-            cluster.sync();
-        } else {
-            // ---- phase 1: partial sums of L[c+1:, c]^T a over this CTA's share of the rows
-            for (int pass = 0; pass < PASSES; ++pass) {
-                const int c0 = pass * 32 * CPL + lane * CPL;           // column inside the block
-                float acc[NACC];
-#pragma unroll
-                for (int v = 0; v < NACC; ++v) acc[v] = 0.0f;
-                const int gw = q * NW + warp, ngw = kDiagCluster * NW;
-                for (int r = R0 + kBlk + gw; r < nb; r += ngw * 2) {
-                    float l[2][CPL];
-#pragma unroll
-                    for (int u = 0; u < 2; ++u) {
-                        const int rr = r + u * ngw;
-                        if (rr < nb) {
-                            if (CPL == 4) {
-                                const float4 v = __ldg(reinterpret_cast<const float4*>(Lkk + static_cast<int64_t>(rr) * nb + R0 + c0));
-                                l[u][0] = v.x; l[u][1] = v.y; l[u][CPL - 2] = v.z; l[u][CPL - 1] = v.w;
-                            } else {
-                                const float2 v = __ldg(reinterpret_cast<const float2*>(Lkk + static_cast<int64_t>(rr) * nb + R0 + c0));
-                                l[u][0] = v.x; l[u][1] = v.y;
-                            }
-                        } else {
-#pragma unroll
-                            for (int qq = 0; qq < CPL; ++qq) l[u][qq] = 0.0f;
-                        }
-                    }
-#pragma unroll
-                    for (int u = 0; u < 2; ++u) {
-                        const int rr = (r + u * ngw < nb) ? r + u * ngw : nb - 1;     // l is zero there
-                        const float* ar = sr + static_cast<size_t>(rr) * NRHS;
-#pragma unroll
-                        for (int h = 0; h < NRHS; h += 4) {
-                            const float4 a = *reinterpret_cast<const float4*>(ar + h);
-#pragma unroll
-                            for (int qq = 0; qq < CPL; ++qq) {
-                                acc[qq * NRHS + h + 0] = fmaf(l[u][qq], a.x, acc[qq * NRHS + h + 0]);
-                                acc[qq * NRHS + h + 1] = fmaf(l[u][qq], a.y, acc[qq * NRHS + h + 1]);
-                                acc[qq * NRHS + h + 2] = fmaf(l[u][qq], a.z, acc[qq * NRHS + h + 2]);
-                                acc[qq * NRHS + h + 3] = fmaf(l[u][qq], a.w, acc[qq * NRHS + h + 3]);
-                            }
-                        }
-                    }
-                }
-                // fixed-order tree over the CTA's warps
-#pragma unroll
-                for (int half = NW / 2; half >= 1; half >>= 1) {
-                    if (warp >= half && warp < 2 * half) {
-                        float* dst = red + (static_cast<size_t>(warp - half) * 32 + lane) * NACC;
-#pragma unroll
-                        for (int v = 0; v < NACC; v += 4) *reinterpret_cast<float4*>(dst + v) = make_float4(acc[v], acc[v + 1], acc[v + 2], acc[v + 3]);
-                    }
-                    __syncthreads();
-                    if (warp < half) {
-                        const float* src = red + (static_cast<size_t>(warp) * 32 + lane) * NACC;
-#pragma unroll
-                        for (int v = 0; v < NACC; v += 4) {
-                            const float4 t = *reinterpret_cast<const float4*>(src + v);
-                            acc[v] += t.x; acc[v + 1] += t.y; acc[v + 2] += t.z; acc[v + 3] += t.w;
-                        }
-                    }
-                    __syncthreads();
-                }
-                if (warp == 0) {
-#pragma unroll
-                    for (int qq = 0; qq < CPL; ++qq)
-#pragma unroll
-                        for (int h = 0; h < NRHS; ++h) part[(c0 + qq) * NRHS + h] = acc[qq * NRHS + h];
-                }
-            }
-            cluster.sync();
-            // CTA q sums the partials of columns [16 q, 16 q + 16) over the cluster in a fixed order
-            for (int idx = threadIdx.x; idx < (kBlk / kDiagCluster) * NRHS; idx += kDiagThreads) {
-                const int col = q * (kBlk / kDiagCluster) + idx / NRHS, h = idx % NRHS;
-                float sum = 0.0f;
-#pragma unroll
-                for (int d = 0; d < kDiagCluster; ++d) sum += cluster.map_shared_rank(part, d)[col * NRHS + h];
-                const float y = (h < nrhs) ? Bk[static_cast<int64_t>(R0 + col) * ldb + h] : 0.0f;
-                const float tv = y - sum;
-#pragma unroll
-                for (int d = 0; d < kDiagCluster; ++d) cluster.map_shared_rank(ts, d)[h * kBlk + col] = tv;
-            }
-            cluster.sync();
         }
+        warp_reduce64(acc, lane);
+        if (KS > 1) {
+            if (ks > 0) {
+                red[((ks - 1) * GQ + gl) * 64 + lane * 2 + 0] = acc[0];
+                red[((ks - 1) * GQ + gl) * 64 + lane * 2 + 1] = acc[1];
+            }
+            __syncthreads();
+        }
+        if (ks == 0) {
+#pragma unroll
+            for (int s2 = 1; s2 < KS; ++s2) {
+                acc[0] += red[((s2 - 1) * GQ + gl) * 64 + lane * 2 + 0];
+                acc[1] += red[((s2 - 1) * GQ + gl) * 64 + lane * 2 + 1];
+            }
+            const int v0 = warp_reduce64_index(lane);
+#pragma unroll
+            for (int t = 0; t < 2; ++t) {
+                const int u = (v0 + t) / NRHS, h = (v0 + t) % NRHS;
+                const int r = grow + u;
+                const float y = (h < nrhs) ? Bk[static_cast<int64_t>(R0 + r) * ldb + h] : 0.0f;
+                const float tv = y - acc[t];
+#pragma unroll
+                for (int d = 0; d < kDiagCluster; ++d) cluster.map_shared_rank(ts, d)[h * kBlk + r] = tv;
+            }
+        }
+        cluster.sync();
         // ---- phase 2: solved_c = inv(L_cc) t   (forward)   or   inv(L_cc)^T t   (backward)
         if (ks == 0) {
             const float* D = (backward ? dinvT : dinv) + static_cast<int64_t>(c) * kBlk * kBlk;
@@ -490,8 +425,7 @@ potrs_diag_kernel(int nb, const float* __restrict__ Lkk, const float* __restrict
                 const int r = R0 + grow + u;
 #pragma unroll
                 for (int d = 0; d < kDiagCluster; ++d) {
-                    if (backward) cluster.map_shared_rank(sr, d)[static_cast<size_t>(r) * NRHS + h] = acc[t];
-                    else cluster.map_shared_rank(zs, d)[h * nb + r] = acc[t];
+                    cluster.map_shared_rank(zs, d)[h * nb + r] = acc[t];
                 }
                 if (h < nrhs) Bk[static_cast<int64_t>(r) * ldb + h] = acc[t];
             }

@@ -246,7 +246,8 @@ template <int NRHS>
 static int set_potrs_attrs() {
     const int big = 220 * 1024;
     KRR_CUDA_CHECK(cudaFuncSetAttribute(potrs_fwd_update_kernel<NRHS>, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
-    KRR_CUDA_CHECK(cudaFuncSetAttribute(potrs_bwd_update_kernel<NRHS>, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
+    KRR_CUDA_CHECK(cudaFuncSetAttribute(potrs_bwd_update_kernel<NRHS, (NRHS <= 16) ? 4 : 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
+    KRR_CUDA_CHECK(cudaFuncSetAttribute(potrs_bwd_update_kernel<NRHS, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
     KRR_CUDA_CHECK(cudaFuncSetAttribute(potrs_diag_kernel<NRHS>, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
     return KRR_OK;
 }
@@ -706,6 +707,7 @@ static int potrs_run(const uint8_t* factor, const float* d_scales, const uint8_t
     const size_t smem_z = static_cast<size_t>(NRHS) * nb * sizeof(float);
     const size_t smem_d = static_cast<size_t>(potrs_diag_smem_floats<NRHS>(nb)) * sizeof(float);
     const size_t smem_bu = smem_z + static_cast<size_t>(NW / 2) * 32 * CPL * NRHS * sizeof(float);
+    const size_t smem_b1 = smem_z + static_cast<size_t>(NW / 2) * 32 * NRHS * sizeof(float);
     const int64_t blk_elems = static_cast<int64_t>(kBlk) * kBlk;
     const int nsub = nb / kBlk;
     const bool pipe = NT > 2;
@@ -735,7 +737,10 @@ static int potrs_run(const uint8_t* factor, const float* d_scales, const uint8_t
     };
     auto bwd_update = [&](int k, int j_lo, int j_hi, cudaStream_t s) {
         if (j_hi <= j_lo) return static_cast<int>(KRR_OK);
-        return launch(CAT_POTRS, potrs_bwd_update_kernel<NRHS>, dim3((j_hi - j_lo) * (nb / (32 * CPL))), dim3(kSolveThreads), smem_bu, s,
+        if (pipe && j_hi - j_lo == 1)            // the tile the next diagonal solve waits for: one column per lane, 4 x the CTAs
+            return launch(CAT_POTRS, potrs_bwd_update_kernel<NRHS, 1>, dim3(nb / 32), dim3(kSolveThreads), smem_b1, s,
+                          NT, nb, k, j_lo, factor, off, d_map, d_scales, B, ldb, nrhs);
+        return launch(CAT_POTRS, potrs_bwd_update_kernel<NRHS, CPL>, dim3((j_hi - j_lo) * (nb / (32 * CPL))), dim3(kSolveThreads), smem_bu, s,
                       NT, nb, k, j_lo, factor, off, d_map, d_scales, B, ldb, nrhs);
     };
     auto diag = [&](int k, int backward, cudaStream_t s) {

@@ -76,6 +76,13 @@ __device__ __forceinline__ float2 load2p(const uint8_t* tile, float s, int64_t e
     return make_float2(e4m3_to_f32(raw & 0xff) * s, e4m3_to_f32(raw >> 8) * s);
 }
 
+template <int P>
+__device__ __forceinline__ float load1p(const uint8_t* tile, float s, int64_t e) {
+    if (P == KRR_FP32) return __ldg(reinterpret_cast<const float*>(tile + e * 4));
+    if (P == KRR_FP16) return __half2float(__ldg(reinterpret_cast<const __half*>(tile + e * 2)));
+    return e4m3_to_f32(__ldg(tile + e)) * s;
+}
+
 // Sum 64 per-lane values v[0..63] across the 32 lanes of a warp with 62 shuffles (each step halves
 // the number of values a lane carries).  Afterwards lane `l` holds in v[0], v[1] the totals of the
 // values with index  warp_reduce64_index(l) + {0, 1}.
@@ -186,29 +193,32 @@ potrs_fwd_update_kernel(int NT, int nb, int k, int i_lo, int i_hi, const uint8_t
     }
 }
 
-// Streaming loop of the backward update: the rows of one strip of a tile (storage precision P), four rows per
-// warp and iteration, against alpha_k in shared memory (`as`: [nb][NRHS]).
-template <int NRHS, int P>
+// Streaming loop of the backward update: the rows of one strip of a tile (storage precision P), RU rows per
+// warp and iteration, against alpha_k in shared memory (`as`: [nb][NRHS]).  Every column's sum runs over the rows
+// warp, warp + NW, warp + 2 NW, ... in this order whatever CPL and RU are, so all variants give identical results.
+template <int NRHS, int CPL, int P>
 __device__ __forceinline__ void bwd_rows(const uint8_t* __restrict__ tile, float s, int c0, int nb,
-                                         const float* __restrict__ as, int warp, float (&acc)[((NRHS <= 16) ? 4 : 2) * NRHS]) {
-    constexpr int CPL = (NRHS <= 16) ? 4 : 2;
+                                         const float* __restrict__ as, int warp, float (&acc)[CPL * NRHS]) {
     constexpr int NW = kSolveThreads / 32;
-#pragma unroll (P == KRR_FP32 ? 2 : 4)
-    for (int r = warp; r < nb; r += NW * 4) {
-        float l[4][CPL];
+    constexpr int RU = (CPL == 1) ? 16 : 4;
+#pragma unroll ((P == KRR_FP32 || CPL == 1) ? 2 : 4)
+    for (int r = warp; r < nb; r += NW * RU) {
+        float l[RU][CPL];
 #pragma unroll
-        for (int u = 0; u < 4; ++u) {
+        for (int u = 0; u < RU; ++u) {
             const int64_t e = static_cast<int64_t>(r + u * NW) * nb + c0;
             if (CPL == 4) {
                 const float4 v = load4p<P>(tile, s, e);
                 l[u][0] = v.x; l[u][1] = v.y; l[u][CPL - 2] = v.z; l[u][CPL - 1] = v.w;
-            } else {
+            } else if (CPL == 2) {
                 const float2 v = load2p<P>(tile, s, e);
                 l[u][0] = v.x; l[u][1] = v.y;
+            } else {
+                l[u][0] = load1p<P>(tile, s, e);
             }
         }
 #pragma unroll
-        for (int u = 0; u < 4; ++u) {
+        for (int u = 0; u < RU; ++u) {
             const float* ar = as + static_cast<size_t>(r + u * NW) * NRHS;
 #pragma unroll
             for (int h = 0; h < NRHS; h += 4) {
@@ -229,12 +239,13 @@ __device__ __forceinline__ void bwd_rows(const uint8_t* __restrict__ tile, float
 // (all < k).  One CTA per (tile j, strip of 32*CPL columns); warps split the nb rows (interleaved), lanes own
 // CPL consecutive columns; the per-warp partial sums are combined through shared memory in a fixed
 // tree order.  smem = nb*NRHS floats (alpha_k) + (NW/2) * 32*CPL*NRHS floats.
-template <int NRHS>
+// CPL = 4 (2 for NRHS = 32) for the bulk launches; CPL = 1 (four times the CTAs per tile, sixteen rows in flight per
+// warp) for the single tile on the chain stream that the next diagonal solve waits for.
+template <int NRHS, int CPL>
 __global__ void __launch_bounds__(kSolveThreads)
 potrs_bwd_update_kernel(int NT, int nb, int k, int j_lo, const uint8_t* __restrict__ factor,
                         const int64_t* __restrict__ off, const uint8_t* __restrict__ map,
                         const float* __restrict__ scales, float* __restrict__ B, int64_t ldb, int nrhs) {
-    constexpr int CPL = (NRHS <= 16) ? 4 : 2;
     constexpr int NACC = CPL * NRHS;
     constexpr int NW = kSolveThreads / 32;
     constexpr int STRIP = 32 * CPL;
@@ -256,9 +267,9 @@ potrs_bwd_update_kernel(int NT, int nb, int k, int j_lo, const uint8_t* __restri
     float acc[NACC];
 #pragma unroll
     for (int v = 0; v < NACC; ++v) acc[v] = 0.0f;
-    if (p == KRR_FP32) bwd_rows<NRHS, KRR_FP32>(tile, s, c0, nb, as, warp, acc);
-    else if (p == KRR_FP16) bwd_rows<NRHS, KRR_FP16>(tile, s, c0, nb, as, warp, acc);
-    else bwd_rows<NRHS, KRR_FP8_E4M3>(tile, s, c0, nb, as, warp, acc);
+    if (p == KRR_FP32) bwd_rows<NRHS, CPL, KRR_FP32>(tile, s, c0, nb, as, warp, acc);
+    else if (p == KRR_FP16) bwd_rows<NRHS, CPL, KRR_FP16>(tile, s, c0, nb, as, warp, acc);
+    else bwd_rows<NRHS, CPL, KRR_FP8_E4M3>(tile, s, c0, nb, as, warp, acc);
     // fixed-order tree over the NW warps
 #pragma unroll
     for (int half = NW / 2; half >= 1; half >>= 1) {

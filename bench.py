@@ -303,6 +303,23 @@ def run_ours(args, rank, world, local_rank):
     potrf_ms = phases["potrf_mp"]
     pw_frac_potrf = (ops / (pw_peak * 1e12)) / (potrf_ms * 1e-3) if potrf_ms > 0 else None
 
+    # ---- optional: device timeline of the three internal streams for one krr_potrf_mp call (krr_profile_timeline)
+    if args.timeline and NT > 2 and not (flags & krr.FLAG_NO_LOOKAHEAD):
+        d_map_t = h_map.to(dev)
+        t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        t0.record()
+        Ft = krr.potrf_mp(A, nb, d_map_t, h_map, flags=flags, n=n)
+        t1.record()
+        rows = krr.profile_timeline(NT)
+        torch.cuda.synchronize()
+        with open(args.timeline, "w") as f:
+            f.write(f"# {cfg.name}: n={n}, nb={nb}, NT={NT}; krr_potrf_mp {t0.elapsed_time(t1):.3f} ms; columns: k, then ms since the fork at which\n"
+                    "# first(k) = chain + TRSM/store of tile (k+1,k) done | old(k) = O(k) done | newb(k) = N(k) done | fin(k) = P(k)+F(k) done\n")
+            for k, r in enumerate(rows):
+                f.write("%3d %9.3f %9.3f %9.3f %9.3f\n" % (k, r[0], r[1], r[2], r[3]))
+        del Ft, d_map_t
+
     # ---- the same step replayed from a CUDA graph (krr_graph_*), beside the headline: the map is still computed and
     # read back every step (the recorded launch sequence is valid for one map; another map would be recorded again).
     # The headline stays the direct-launch path because the roofline above needs events around every update launch.
@@ -564,6 +581,8 @@ def main():
     ap.add_argument("--no-build", action="store_true", help="skip the Build-phase (krr_build) timing")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-graph", action="store_true", help="skip the CUDA-graph replay timing (krr_graph_*)")
+    ap.add_argument("--timeline", default=None, metavar="FILE",
+                    help="write the device timeline of the internal streams of one extra krr_potrf_mp call (krr_profile_timeline)")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))

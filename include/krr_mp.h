@@ -403,6 +403,16 @@ int64_t krr_last_launch_count(void);
 int krr_profile_enable(unsigned category_mask);
 int krr_profile_read(int category, double* total_ms, int64_t* launches);
 
+/* Timeline of the tile-column pipeline of the LAST krr_potrf_mp call of this host thread that ran
+ * the lookahead schedule (NT > 2, no KRR_FLAG_NO_LOOKAHEAD, not recorded into a graph), read before any other krr_* call:
+ * h_ms[4k + 0..3] = device time in ms since the call forked onto the internal streams at which, for tile column k,
+ *   0  the critical stream finished the diagonal-tile chain and the TRSM / store of tile (k+1, k),
+ *   1  the bulk stream finished O(k) (terms s < k-1 of column k),
+ *   2  the bulk stream finished N(k) (newest term on the rows below the diagonal tile),
+ *   3  the panel stream finished P(k) and F(k) (TRSM and store of the remaining rows);
+ * -1 where the event was not recorded (O(k) for k < 2, ...).  Waits for the call to finish.  h_ms: host, 4*NT floats. */
+int krr_profile_timeline(int NT, float* h_ms);
+
 #ifdef __cplusplus
 }
 #endif

@@ -28,7 +28,7 @@ EXPORTS = ["krr_version", "krr_built_for_sm", "krr_tile_slot", "krr_precision_ma
            "krr_associate_host_arena", "krr_associate_host", "krr_build_workspace", "krr_build", "krr_build_bordered", "krr_build_rr", "krr_predict_workspace", "krr_predict", "krr_fit_host_arena", "krr_fit_host", "krr_band_map", "krr_build_stats_bytes", "krr_precision_map_from_build",
            "krr_graph_begin", "krr_graph_end", "krr_graph_launch", "krr_graph_kernel_nodes", "krr_graph_destroy",
            "krr_last_launch_count",
-           "krr_profile_enable", "krr_profile_read"]
+           "krr_profile_enable", "krr_profile_read", "krr_profile_timeline"]
 
 
 class KrrError(RuntimeError):
@@ -125,6 +125,8 @@ def lib():
     L.krr_profile_enable.argtypes = [u32]
     L.krr_profile_read.restype = c.c_int
     L.krr_profile_read.argtypes = [c.c_int, c.POINTER(c.c_double), c.POINTER(i64)]
+    L.krr_profile_timeline.restype = c.c_int
+    L.krr_profile_timeline.argtypes = [c.c_int, c.POINTER(c.c_float)]
     _LIB = L
     return L
 
@@ -207,6 +209,13 @@ def profile_read():
         _check(lib().krr_profile_read(cat, ctypes.byref(ms), ctypes.byref(cnt)), "krr_profile_read")
         out[name] = (ms.value, cnt.value)
     return out
+
+
+def profile_timeline(NT):
+    """krr_profile_timeline: NT rows of [first, old, newb, fin] in ms since the fork of the last potrf_mp call."""
+    buf = (ctypes.c_float * (4 * NT))()
+    _check(lib().krr_profile_timeline(NT, buf), "krr_profile_timeline")
+    return [[buf[4 * k + e] for e in range(4)] for k in range(NT)]
 
 
 def tile_slot(NT, i, j):

@@ -170,7 +170,7 @@ struct Pipeline {
     cudaEvent_t event(size_t i) {
         while (ev.size() <= i) {
             cudaEvent_t e = nullptr;
-            cudaEventCreateWithFlags(&e, cudaEventDisableTiming);
+            cudaEventCreate(&e);                 // timing enabled: krr_profile_timeline reads them
             ev.push_back(e);
         }
         return ev[i];
@@ -361,6 +361,27 @@ int krr_graph_destroy(krr_graph_t* graph) {
     cudaGraphExecDestroy(graph->exec);
     cudaGraphDestroy(graph->graph);
     delete graph;
+    return KRR_OK;
+}
+
+// Device times of the pipeline events of the last krr_potrf_mp call of this thread (lookahead schedule), in ms since
+// the fork: per tile column k  {first(k), old(k), newb(k), fin(k)} = {chain + TRSM / store of tile (k+1,k) done on the
+// critical stream, O(k) done, N(k) done on the bulk stream, P(k) + F(k) done on the panel stream}; -1 = not recorded.
+int krr_profile_timeline(int NT, float* h_ms) {
+    if (NT < 1 || !h_ms) return KRR_ERR_ARG;
+    if (g_pipe.ev.size() < 4 + 4 * static_cast<size_t>(NT)) return KRR_ERR_ARG;      // no such call yet
+    if (cudaEventSynchronize(g_pipe.ev[1]) != cudaSuccess || cudaEventSynchronize(g_pipe.ev[2]) != cudaSuccess ||
+        cudaEventSynchronize(g_pipe.ev[3]) != cudaSuccess)
+        return KRR_ERR_CUDA;
+    for (int k = 0; k < NT; ++k)
+        for (int e = 0; e < 4; ++e) {
+            float ms = -1.0f;
+            if (cudaEventElapsedTime(&ms, g_pipe.ev[0], g_pipe.ev[4 + 4 * k + e]) != cudaSuccess) {
+                ms = -1.0f;
+                cudaGetLastError();
+            }
+            h_ms[4 * k + e] = ms;
+        }
     return KRR_OK;
 }
 

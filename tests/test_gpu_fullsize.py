@@ -245,3 +245,52 @@ def test_c4_full_size_rule_map_leading_block_invariants_and_pcg(krr):
     # how far the raw alpha was from the converged one: the 10 % the survey's sqrt(n) growth predicts
     moved = float(torch.linalg.norm((Xc - alpha).double()) / torch.linalg.norm(Xc.double()))
     assert 1e-2 < moved < 0.5
+
+
+def test_c5_full_size_literal_map_breaks_down_and_c5p_matches_the_oracle(krr):
+    """C5 (n = 98304, uniform genotypes, lambda = 0.1).  (a) The literal map -- every off-diagonal tile FP8, A
+    pre-rounded -- is not positive definite after rounding: the factorisation must stop with the same 1-based pivot
+    column as the emulated oracle, which sees it on the leading two tile rows (L[:m,:m] depends on A[:m,:m] only).
+    (b) C5' (tile column 0 FP32, the rest FP8, operands as stored), the map bench.py times for C5:
+    leading 3 x 3 tiles against the emulated oracle, invariants and probes at full size."""
+    cfg = CONFIGS["C5"]
+    A, Y = make_problem(cfg, device="cuda")
+    nb, NT = cfg.nb, cfg.NT
+    m = 3
+    Am = A[:m * nb, :m * nb].cpu().numpy()
+    # (a)
+    h_map = krr.uniform_map(NT, krr.FP8)
+    F = krr.potrf_mp(A, nb, h_map.cuda(), h_map, flags=krr.FLAG_PREROUND_A)
+    torch.cuda.synchronize()
+    info_gpu = int(F.info.item())
+    del F
+    pm = np.full((2, 2), FP8, dtype=np.uint8)
+    pm[0, 0] = pm[1, 1] = FP32
+    pm[0, 1] = 255
+    _, _, info_oracle = tile_cholesky_emulated(Am[:2 * nb, :2 * nb], nb, pm, preround_a=True)
+    print(f"C5 literal map: info gpu {info_gpu} oracle {info_oracle}")
+    assert nb < info_oracle <= 2 * nb                          # breakdown in tile column 1
+    assert info_gpu == info_oracle
+    # (b)
+    h_map = krr.uniform_map(NT, krr.FP8)
+    h_map[1:, 0] = krr.FP32
+    F = krr.potrf_mp(A, nb, h_map.cuda(), h_map, flags=0)
+    alpha = krr.potrs(F, Y.clone())
+    torch.cuda.synchronize()
+    assert int(F.info.item()) == 0
+    pm = np.ascontiguousarray(h_map.numpy()[:m, :m])
+    Lo, _, info = tile_cholesky_emulated(Am, nb, pm, preround_a=False)
+    assert info == 0
+    Lg = leading_block(F, m)
+    bg, bo = backward_error(Am, Lg), backward_error(Am, Lo)
+    print(f"C5' leading block: backward gpu {bg:.4e} oracle {bo:.4e}")
+    assert abs(bg - bo) <= 0.02 * bo
+    for i in range(1, m):                                      # tile column 0 is FP32: the literal criterion
+        assert relF(Lg[i * nb:(i + 1) * nb, :nb], Lo[i * nb:(i + 1) * nb, :nb]) <= 1e-4
+    g, o = Lg[2 * nb:, nb:2 * nb], Lo[2 * nb:, nb:2 * nb]       # the FP8 tile (2,1): same scale, most codes equal
+    assert np.mean(g == o) > 0.5 and relF(g, o) <= 2.0 * R.UNIT_ROUNDOFF[FP8]
+    for k in range(0, NT, NT // 8):
+        assert float(torch.diagonal(F.tile(k, k)).min()) > 0.0
+        assert float(torch.triu(F.tile(k, k), 1).abs().max()) == 0.0
+    assert probe_backward_error(A, F, 4) <= 5e-4
+    assert np.isfinite(alpha.cpu().numpy()).all()

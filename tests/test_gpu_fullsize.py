@@ -8,7 +8,9 @@ precision rule is checked on sampled tiles with norms the oracle computes from h
 tiles.  What holds at any size: info = 0, positive diagonal, backward error by Gaussian probes and the
 residual of the solve, both evaluated by independent torch-FP64 code (tests/helpers.py).
 Configs: C2 whole against the FP64 oracle; C3 (n = 65536, the bench default); S1 (the rule's genuine
-FP32 / FP16 mosaic) at its bench size.
+FP32 / FP16 mosaic) at its bench size; C4 (n = 131072, lower tiles, the rule's FP16 map; refinement against
+preconditioned CG); C5 (n = 98304: the literal forced-FP8 map breaks down with the oracle's info, C5' matches the
+emulated oracle on the leading tiles).
 """
 import numpy as np
 import pytest

@@ -376,6 +376,32 @@ def test_potrs_every_nrhs_class(krr, nrhs):
     assert torch.equal(big[:, :nrhs], alpha) and float(big[:, nrhs:].abs().max()) == 0.0
 
 
+@pytest.mark.parametrize("nrhs", [1, 5, 8, 16, 32])
+def test_potrs_mixed_mosaic_every_nrhs_class(krr, nrhs):
+    """The solve kernels read FP32, FP16 and FP8 tiles through precision-specific streaming loops (and, on the chain
+    stream of the backward sweep, a one-column-per-lane variant): a random mosaic, NT = 8 (one-column lookahead on),
+    against the oracle's substitution with the SAME dequantised factor."""
+    cfg = replace(scaled_config(CONFIGS["S1"], nb=128, n=1024, p=768), genotype="maf", gamma_scale=4.0)
+    A, _ = make_problem(cfg, device="cuda")
+    rng = np.random.default_rng(11)
+    pmap = oracle_uniform(cfg.NT, R.FP32)
+    for i in range(cfg.NT):
+        for j in range(i):
+            pmap[i, j] = rng.integers(0, 3)
+    assert len(set(pmap[np.tril_indices(cfg.NT, -1)].tolist())) == 3
+    F = gpu_factor(krr, A, cfg.nb, pmap)
+    assert int(F.info.item()) == 0
+    g = torch.Generator(device="cuda").manual_seed(100 + nrhs)
+    Y = torch.randn((cfg.n, nrhs), device="cuda", generator=g)
+    alpha = krr.potrs(F, Y.clone())
+    torch.cuda.synchronize()
+    want = potrs_fp64(F.dense().cpu().numpy(), Y.cpu().numpy(), cfg.nb)
+    assert relF(alpha.cpu().numpy().astype(np.float64), want) <= 1e-5
+    again = krr.potrs(F, Y.clone())                      # fixed summation order: the same bits every time
+    torch.cuda.synchronize()
+    assert torch.equal(again, alpha)
+
+
 def test_associate_host_matches_device_path(krr):
     cfg = scaled_config(CONFIGS["S1"], nb=128, n=1024, p=768)
     A, Y = make_problem(cfg, device="cuda")

@@ -95,7 +95,17 @@ def tile_cholesky_fp64(A, nb):
     return L, 0
 
 
-def tile_cholesky_emulated(A, nb, pmap, preround_a=True):
+def _operand_for(X, p_stored, p_task):
+    """Operand tile of a task that runs in precision p_task (literal reading of PAPER.md:206: "conversion at
+    the sender (lower precision needed at the receiver) or at the receiver (higher)"): a tile stored in a
+    higher precision than the task's is rounded DOWN to it (lossy; FP8 with the scale of its own amax),
+    a tile stored in the same or a lower precision is used exactly (up-conversion is exact)."""
+    if p_task > p_stored:                      # codes grow as the precision falls: FP32 = 0 < FP16 = 1 < FP8 = 2
+        return quantise_tile(X, p_task)[0]
+    return X
+
+
+def tile_cholesky_emulated(A, nb, pmap, preround_a=True, operands="as_stored"):
     """Emulated mixed-precision tile Cholesky.
 
     A     : n x n, FP32 values (any float dtype holding them); lower triangle referenced.
@@ -112,7 +122,10 @@ def tile_cholesky_emulated(A, nb, pmap, preround_a=True):
       4. S_kk = A_kk - sum_{j<k} Lhat_kj Lhat_kj^T ;  Lhat_kk = rd32(chol(rd32(S_kk)))
          S_ik = Ahat_ik - sum_{j<k} Lhat_ij Lhat_kj^T ;  T_ik = S_ik Lhat_kk^{-T} ;
          Lhat_ik = rd_{p(i,k)}(T_ik)            -- each tile rounded once, on its final store
-      5. operands are used as stored (up-conversion exact)
+      5. operands="as_stored" (default, reading R5): operands are used as stored (up-conversion exact);
+         operands="to_updated" (the paper's literal rule): every SYRK / GEMM task runs in the
+         precision of the tile it updates, S_ik -= cv(Lhat_ij) cv(Lhat_kj)^T with cv = _operand_for(., p(.), p(i,k))
+         (down-conversion of a higher-precision operand is lossy); identical to the default on uniform maps
       6. FP8 tiles: power-of-two scale from the tile's amax
     Arithmetic between roundings is FP64.
     """
@@ -121,13 +134,25 @@ def tile_cholesky_emulated(A, nb, pmap, preround_a=True):
     assert A.shape == (n, n) and n % nb == 0
     NT = n // nb
     pmap = np.asarray(pmap)
+    assert operands in ("as_stored", "to_updated")
     Lh = np.zeros((n, n), dtype=np.float64)
     scales = np.ones((NT, NT), dtype=np.float64)
+
+    def product_sum(i, k, p_task):
+        """sum_{j<k} op(Lhat_ij) op(Lhat_kj)^T for the task that updates tile (i, k)."""
+        if operands == "as_stored":
+            return Lh[i * nb:(i + 1) * nb, :k * nb] @ Lh[k * nb:(k + 1) * nb, :k * nb].T
+        acc = np.zeros((nb, nb), dtype=np.float64)
+        for j in range(k):
+            a = _operand_for(Lh[i * nb:(i + 1) * nb, j * nb:(j + 1) * nb], int(pmap[i, j]), p_task)
+            b = _operand_for(Lh[k * nb:(k + 1) * nb, j * nb:(j + 1) * nb], int(pmap[k, j]), p_task)
+            acc += a @ b.T
+        return acc
+
     for k in range(NT):
         assert pmap[k, k] == FP32, "diagonal tiles are FP32 (PAPER.md:229, reading R8)"
         r0, r1 = k * nb, (k + 1) * nb
-        Lrow = Lh[r0:r1, :r0]
-        S = np.asarray(A[r0:r1, r0:r1], dtype=np.float64) - Lrow @ Lrow.T
+        S = np.asarray(A[r0:r1, r0:r1], dtype=np.float64) - product_sum(k, k, FP32)
         Lkk, info = chol_unblocked(rd_fp32(S))
         if info:
             return Lh, scales, r0 + info
@@ -139,7 +164,7 @@ def tile_cholesky_emulated(A, nb, pmap, preround_a=True):
             Aik = np.asarray(A[i0:i1, r0:r1], dtype=np.float64)
             if preround_a:
                 Aik, _ = quantise_tile(Aik, p)
-            Sik = Aik - Lh[i0:i1, :r0] @ Lrow.T
+            Sik = Aik - product_sum(i, k, p)
             Tik = _trsm_right_lower_trans(Sik, Lkk)
             Lh[i0:i1, r0:r1], scales[i, k] = quantise_tile(Tik, p)
     return Lh, scales, 0

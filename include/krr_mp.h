@@ -12,7 +12,9 @@
  *   - Every d_* pointer is DEVICE memory owned by the caller (e.g. a PyTorch tensor); every h_*
  *     pointer is HOST memory.  `stream` is a cudaStream_t passed as void*.  Unless stated, the
  *     library never allocates or frees device memory, never synchronises the device and never
- *     reads or writes the host copy of the data; all work is enqueued on `stream`.
+ *     reads or writes the host copy of the data; all work is enqueued on `stream`.  What it does
+ *     create, once per host thread and device, are three internal CUDA streams (priorities high /
+ *     middle / low) and a pool of CUDA events for the lookahead schedule; krr_shutdown() destroys them.
  *   - n = number of patients (matrix order), nb = tile size, NT = n / nb.  nb must be a multiple
  *     of 128 and divide n (all BASELINE.json configs do; ragged edges are not supported).
  *   - Tiles are addressed (i, j), 0-based, i >= j (lower triangle).  A precision map is NT*NT
@@ -412,6 +414,29 @@ int krr_profile_read(int category, double* total_ms, int64_t* launches);
  *   3  the panel stream finished P(k) and F(k) (TRSM and store of the remaining rows);
  * -1 where the event was not recorded (O(k) for k < 2, ...).  Waits for the call to finish.  h_ms: host, 4*NT floats. */
 int krr_profile_timeline(int NT, float* h_ms);
+
+/* ---------------------------------------------------------------------------------------------
+ * krr_peak_probe -- roofline denominators measured on the current device (SURVEY 8(d) "Which roofline": "FP8 =
+ * measure with a no-traffic kind::f8f6f4 loop ... FP32 ALU = measure an FFMA loop").  Beside the path; used by
+ * bench.py --peaks and paper_2409_01712_b200/peaks.py.
+ * kind   0  tcgen05 kind::f16 on CTA pairs (cta_group::2, M = N = 256, K = 16 per instruction), operands resident
+ *           in shared memory (pseudo-random finite data, four ring slots), accumulator in TMEM, no global traffic
+ *        1  the same with kind::f8f6f4 (E4M3 x E4M3, K = 32 per instruction)
+ *        2  the same with kind::mxf8f6f4.block_scale (UE8M0 scales 2^0 from TMEM) -- the FP8 x FP8 instruction of
+ *           krr_potrf_mp
+ *        3  FFMA: 8 independent chains per thread, 1024 threads per CTA, 2 CTAs per SM
+ *        4  the three-instruction FP32-class sequence of krr_potrf_mp (hi*hi + lo*hi + hi*lo on kind::f16)
+ * work   tensor kinds: 128-byte K slices ("chunks", 4 instructions each; kind 4: 12) per CTA pair, a multiple of 16;
+ *        FFMA: loop iterations (128 FMAs per thread each).
+ * h_ms   out  device time of the one launch (CUDA events); h_flops out  the flops it performed (2 per multiply-add;
+ *        kind 4: of all three instructions).  Synchronises `stream`. */
+int krr_peak_probe(int kind, int64_t work, float* h_ms, double* h_flops, void* stream);
+
+/* krr_shutdown -- destroy what the library created for the calling host thread on the current device: the three
+ * internal priority streams of the lookahead schedule, the pool of CUDA events (pipeline events and the timing
+ * events of krr_profile_*).  Everything the thread enqueued must have completed.  The next krr_* call creates them
+ * again.  These streams and events are the only resources the library ever allocates (no device memory). */
+int krr_shutdown(void);
 
 #ifdef __cplusplus
 }

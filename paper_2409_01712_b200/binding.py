@@ -28,7 +28,7 @@ EXPORTS = ["krr_version", "krr_built_for_sm", "krr_tile_slot", "krr_precision_ma
            "krr_associate_host_arena", "krr_associate_host", "krr_build_workspace", "krr_build", "krr_build_bordered", "krr_build_rr", "krr_predict_workspace", "krr_predict", "krr_fit_host_arena", "krr_fit_host", "krr_band_map", "krr_build_stats_bytes", "krr_precision_map_from_build",
            "krr_graph_begin", "krr_graph_end", "krr_graph_launch", "krr_graph_kernel_nodes", "krr_graph_destroy",
            "krr_last_launch_count",
-           "krr_profile_enable", "krr_profile_read", "krr_profile_timeline"]
+           "krr_profile_enable", "krr_profile_read", "krr_profile_timeline", "krr_peak_probe", "krr_shutdown"]
 
 
 class KrrError(RuntimeError):
@@ -127,6 +127,9 @@ def lib():
     L.krr_profile_read.argtypes = [c.c_int, c.POINTER(c.c_double), c.POINTER(i64)]
     L.krr_profile_timeline.restype = c.c_int
     L.krr_profile_timeline.argtypes = [c.c_int, c.POINTER(c.c_float)]
+    L.krr_peak_probe.restype = c.c_int
+    L.krr_peak_probe.argtypes = [c.c_int, i64, c.POINTER(c.c_float), c.POINTER(c.c_double), vp]
+    L.krr_shutdown.restype = c.c_int
     _LIB = L
     return L
 
@@ -553,3 +556,18 @@ def band_map(NT, fp32_fraction, low):
     _check(lib().krr_band_map(NT, float(fp32_fraction), int(low), _ptr(m)), "krr_band_map")
     return m
 
+
+
+PEAK_KINDS = {"f16": 0, "f8": 1, "mxf8": 2, "ffma": 3, "f16x3": 4}
+
+
+def peak_probe(kind, work):
+    """One launch of krr_peak_probe: (device ms, flops performed)."""
+    ms, fl = ctypes.c_float(0.0), ctypes.c_double(0.0)
+    _check(lib().krr_peak_probe(PEAK_KINDS[kind], int(work), ctypes.byref(ms), ctypes.byref(fl), _stream()), "krr_peak_probe")
+    return float(ms.value), float(fl.value)
+
+
+def shutdown():
+    """Destroy the internal streams and events of the calling thread on the current device (krr_shutdown)."""
+    _check(lib().krr_shutdown(), "krr_shutdown")

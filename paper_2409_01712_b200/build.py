@@ -31,7 +31,7 @@ def build(force=False, verbose=False):
     if not force and not needs_build():
         return LIB
     cmd = [_nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-           "-shared", "-Xcompiler", "-fPIC", "-cudart", "shared",
+           "-shared", "-Xcompiler", "-fPIC", "-cudart", "shared", "--split-compile=0",
            "-I", os.path.join(HERE, "..", "include")]
     if verbose:
         cmd += ["-Xptxas", "-v"]

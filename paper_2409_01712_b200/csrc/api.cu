@@ -12,6 +12,7 @@
 #include "common.cuh"
 #include "gemm_tc.cuh"
 #include "panel.cuh"
+#include "peaks.cuh"
 #include "potrs.cuh"
 #include "precision_map.cuh"
 #include "refine.cuh"
@@ -100,6 +101,13 @@ static int make_byte_plane_tmap(CUtensorMap* tm, const void* base, uint64_t rows
 }
 
 // ---- mosaic offsets (host) -------------------------------------------------------------------
+static uint64_t host_map_hash(int NT, const uint8_t* h_map) {
+    uint64_t h = kMapHashSeed;
+    for (int j = 0; j < NT; ++j)
+        for (int i = j; i < NT; ++i) h = map_hash_step(h, h_map[i * NT + j]);
+    return h;
+}
+
 static size_t host_offsets(int NT, int nb, const uint8_t* h_map, std::vector<int64_t>* off) {
     size_t acc = 0;
     const size_t elems = static_cast<size_t>(nb) * nb;
@@ -139,31 +147,15 @@ static PotrfWs potrf_ws_layout(int64_t n, int nb, bool any_fp8) {
     return w;
 }
 
-// ---- optional per-category kernel timing (krr_profile_*): CUDA events on the launching stream ----
+// ---- per host thread and device: internal streams, event pool, timing records, one-time kernel attributes ----
+// (the only resources the library creates; krr_shutdown destroys them)
 enum { CAT_UPDATE = 0, CAT_P1 = 1, CAT_P3 = 2, CAT_POTRF = 3, CAT_FINALIZE = 4, CAT_MAP = 5, CAT_POTRS = 6,
        CAT_MISC = 7, CAT_COUNT = 8 };
 struct TimedLaunch { int cat; cudaEvent_t e0, e1; };
-static thread_local unsigned g_prof_mask = 0;
-static thread_local std::vector<TimedLaunch> g_prof;
-static thread_local std::vector<cudaEvent_t> g_event_pool;
 
-static cudaEvent_t pool_event() {
-    if (!g_event_pool.empty()) { cudaEvent_t e = g_event_pool.back(); g_event_pool.pop_back(); return e; }
-    cudaEvent_t e = nullptr;
-    cudaEventCreate(&e);
-    return e;
-}
-struct ProfScope {
-    bool on; TimedLaunch t; cudaStream_t st;
-    ProfScope(int cat, cudaStream_t s) : on((g_prof_mask >> cat) & 1u), st(s) {
-        if (on) { t.cat = cat; t.e0 = pool_event(); t.e1 = pool_event(); cudaEventRecord(t.e0, st); }
-    }
-    ~ProfScope() { if (on) { cudaEventRecord(t.e1, st); g_prof.push_back(t); } }
-};
-
-// ---- internal streams of the tile-column pipeline (lookahead): created once per host thread ----
-// `hi` carries the critical path (diagonal-tile chain, panel, store), `lo` the bulk updates that run
-// ahead; both are fenced by events against the caller's stream, which is never blocked on the host.
+// Internal streams of the tile-column pipeline (lookahead): `hi` carries the critical path (diagonal-tile chain,
+// panel, store), `lo` the bulk updates that run ahead; both are fenced by events against the caller's stream,
+// which is never blocked on the host.
 struct Pipeline {
     cudaStream_t hi = nullptr, mid = nullptr, lo = nullptr;
     std::vector<cudaEvent_t> ev;
@@ -184,8 +176,46 @@ struct Pipeline {
         KRR_CUDA_CHECK(cudaStreamCreateWithPriority(&lo, cudaStreamNonBlocking, least));
         return KRR_OK;
     }
+    void destroy() {
+        for (cudaEvent_t e : ev) cudaEventDestroy(e);
+        ev.clear();
+        if (hi) cudaStreamDestroy(hi);
+        if (mid) cudaStreamDestroy(mid);
+        if (lo) cudaStreamDestroy(lo);
+        hi = mid = lo = nullptr;
+    }
 };
-static thread_local Pipeline g_pipe;
+
+constexpr int kMaxDevices = 64;
+struct DeviceState {
+    Pipeline pipe;
+    unsigned prof_mask = 0;
+    std::vector<TimedLaunch> prof;
+    std::vector<cudaEvent_t> event_pool;
+    bool attrs_done = false, build_attrs_done = false, peak_attrs_done = false;
+};
+static thread_local DeviceState g_dev_state[kMaxDevices];
+static DeviceState& dev_state() {
+    int dev = 0;
+    cudaGetDevice(&dev);
+    return g_dev_state[(dev >= 0 && dev < kMaxDevices) ? dev : 0];
+}
+#define g_pipe (dev_state().pipe)
+
+static cudaEvent_t pool_event(DeviceState& d) {
+    if (!d.event_pool.empty()) { cudaEvent_t e = d.event_pool.back(); d.event_pool.pop_back(); return e; }
+    cudaEvent_t e = nullptr;
+    cudaEventCreate(&e);
+    return e;
+}
+struct ProfScope {
+    bool on; TimedLaunch t; cudaStream_t st; DeviceState* d;
+    ProfScope(int cat, cudaStream_t s) : st(s), d(&dev_state()) {
+        on = (d->prof_mask >> cat) & 1u;
+        if (on) { t.cat = cat; t.e0 = pool_event(*d); t.e1 = pool_event(*d); cudaEventRecord(t.e0, st); }
+    }
+    ~ProfScope() { if (on) { cudaEventRecord(t.e1, st); d->prof.push_back(t); } }
+};
 
 template <typename K, typename... Args>
 static int launch(int cat, K kernel, dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args... args) {
@@ -253,7 +283,7 @@ static int set_potrs_attrs() {
 }
 
 static int set_kernel_attrs() {
-    static bool done = false;
+    bool& done = dev_state().attrs_done;
     if (done) return KRR_OK;
     KRR_CUDA_CHECK(cudaFuncSetAttribute(gemm_tc_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem));
     KRR_CUDA_CHECK(cudaFuncSetAttribute(gemm_tc_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem));
@@ -275,17 +305,29 @@ int krr_built_for_sm(void) { return 100; }
 int64_t krr_last_launch_count(void) { return g_launches; }
 
 int krr_profile_enable(unsigned category_mask) {
-    for (auto& t : g_prof) { g_event_pool.push_back(t.e0); g_event_pool.push_back(t.e1); }
-    g_prof.clear();
-    g_prof_mask = category_mask;
+    DeviceState& d = dev_state();
+    for (auto& t : d.prof) { d.event_pool.push_back(t.e0); d.event_pool.push_back(t.e1); }
+    d.prof.clear();
+    d.prof_mask = category_mask;
     return KRR_OK;
+}
+
+int krr_shutdown(void) {
+    DeviceState& d = dev_state();
+    for (auto& t : d.prof) { cudaEventDestroy(t.e0); cudaEventDestroy(t.e1); }
+    d.prof.clear();
+    d.prof_mask = 0;
+    for (cudaEvent_t e : d.event_pool) cudaEventDestroy(e);
+    d.event_pool.clear();
+    d.pipe.destroy();
+    return cudaGetLastError() == cudaSuccess ? KRR_OK : KRR_ERR_CUDA;
 }
 
 int krr_profile_read(int category, double* total_ms, int64_t* launches) {
     if (category < 0 || category >= CAT_COUNT || !total_ms || !launches) return KRR_ERR_ARG;
     double ms = 0.0;
     int64_t cnt = 0;
-    for (auto& t : g_prof) {
+    for (auto& t : dev_state().prof) {
         if (t.cat != category) continue;
         if (cudaEventSynchronize(t.e1) != cudaSuccess) return KRR_ERR_CUDA;
         float f = 0.f;
@@ -307,7 +349,7 @@ struct krr_graph { cudaGraph_t graph; cudaGraphExec_t exec; int64_t kernels; };
 
 int krr_graph_begin(void* stream) {
     if (!stream) return KRR_ERR_ARG;                     // the legacy default stream cannot be captured
-    if (g_prof_mask) return KRR_ERR_UNSUPPORTED;         // timing events cannot be read back from a capture
+    if (dev_state().prof_mask) return KRR_ERR_UNSUPPORTED;  // timing events cannot be read back from a capture
     int num_sms = 0;
     int rc = check_device(&num_sms);
     if (rc) return rc;
@@ -420,7 +462,7 @@ int krr_precision_map(const float* d_A, int64_t n, int64_t lda, int nb, float ep
     float* pamax = reinterpret_cast<float*>(ws + align_up(nslots * chunks * sizeof(double), 1024));
     double* sumsq = reinterpret_cast<double*>(reinterpret_cast<uint8_t*>(pamax) + align_up(nslots * chunks * sizeof(float), 1024));
     AView A{d_A, lda, tiled ? 1 : 0, NT, nb};
-    rc = launch(CAT_MAP, tile_stats_kernel, dim3(static_cast<unsigned>(chunks), static_cast<unsigned>(nslots)), dim3(kStatThreads), 0, st,
+    rc = launch(CAT_MAP, tile_stats_kernel, dim3(static_cast<unsigned>(nslots), static_cast<unsigned>(chunks)), dim3(kStatThreads), 0, st,
                 A, partial, pamax);
     if (rc) return rc;
     return launch(CAT_MAP, map_decide_kernel, dim3(1), dim3(1024), 0, st, NT, static_cast<int>(chunks),
@@ -517,14 +559,14 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
     int* prog = reinterpret_cast<int*>(ws + L.prog);
     int* split_flags = (flags & KRR_FLAG_NO_TAIL_SPLIT) ? nullptr : reinterpret_cast<int*>(ws + L.split);
     KRR_CUDA_CHECK(cudaMemsetAsync(prog, 0, static_cast<size_t>(n / kBlk) * sizeof(int), st));
-    rc = launch(CAT_MISC, offsets_kernel, dim3(1), dim3(32), 0, st, NT, nb, d_map, off);
+    rc = launch(CAT_MISC, offsets_kernel, dim3(1), dim3(32), 0, st, NT, nb, d_map, off, host_map_hash(NT, h_map), d_info);
     if (rc) return rc;
     rc = launch(CAT_MISC, plane_scale_kernel, dim3(1), dim3(1024), 0, st, A, n, scl);
     if (rc) return rc;
     const bool preround = flags & KRR_FLAG_PREROUND_A;
     if (preround && any_fp8) {
         KRR_CUDA_CHECK(cudaMemsetAsync(a_amax, 0, static_cast<size_t>(NT) * NT * sizeof(float), st));
-        rc = launch(CAT_MISC, tile_amax_kernel, dim3(nb / 32, static_cast<unsigned>(nslots)), dim3(256), 0, st, A, d_map, a_amax);
+        rc = launch(CAT_MISC, tile_amax_kernel, dim3(static_cast<unsigned>(nslots), nb / 32), dim3(256), 0, st, A, d_map, a_amax);
         if (rc) return rc;
     }
 
@@ -576,6 +618,9 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
     // Panel stream `sp`: the TRSM of the remaining rows (P) and their store (F); latency-bound, it fills
     // the SMs the bulk kernel leaves free and takes the rest as O(k+1) drains.  N(k+1) waits for F(k);
     // column k+1's chain runs beside F(k), N(k+1), O(k+2).
+    // (a lambda: an error in the middle still joins the internal streams below, so the caller's stream -- or a
+    // stream capture -- is left in a consistent state)
+    auto run_columns = [&]() -> int {
     for (int k = 0; k < NT; ++k) {
         const int mblk = (NT - k) * nsub;             // 128-row blocks of the panel
         const int lb = k & 1;                         // buffer of the inverted diagonal blocks
@@ -680,6 +725,9 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
             KRR_CUDA_CHECK(cudaEventRecord(ev_fin(k), sp));
         }
     }
+    return static_cast<int>(KRR_OK);
+    };
+    const int rc_columns = run_columns();
     if (lookahead) {
         KRR_CUDA_CHECK(cudaEventRecord(g_pipe.event(EV_JOIN_HI), sh));
         KRR_CUDA_CHECK(cudaEventRecord(g_pipe.event(EV_JOIN_LO), sl));
@@ -688,7 +736,7 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
         KRR_CUDA_CHECK(cudaStreamWaitEvent(st, g_pipe.event(EV_JOIN_HI), 0));
         KRR_CUDA_CHECK(cudaStreamWaitEvent(st, g_pipe.event(EV_JOIN_LO), 0));
     }
-    return KRR_OK;
+    return rc_columns;
 }
 
 // ------------------------------------------------------------------------- solve
@@ -849,7 +897,7 @@ int krr_potrs(const void* d_factor, const float* d_scales, const uint8_t* d_map,
     float* dinv = reinterpret_cast<float*>(ws + L.dinv);
     float* dinvT = reinterpret_cast<float*>(ws + L.dinvT);
     float* diagT = reinterpret_cast<float*>(ws + L.diagT);
-    rc = launch(CAT_MISC, offsets_kernel, dim3(1), dim3(32), 0, st, NT, nb, d_map, off);
+    rc = launch(CAT_MISC, offsets_kernel, dim3(1), dim3(32), 0, st, NT, nb, d_map, off, host_map_hash(NT, h_map), static_cast<int*>(nullptr));
     if (rc) return rc;
     const uint8_t* factor = static_cast<const uint8_t*>(d_factor);
     rc = launch(CAT_POTRS, trtri128_kernel, dim3(static_cast<unsigned>(n / kBlk)), dim3(kTriThreads), static_cast<size_t>(kTriSmem), st,
@@ -1271,7 +1319,7 @@ int make_genotype_tmap(CUtensorMap* tm, const int8_t* G, int64_t rows, int64_t p
 }
 int launch_build(const CUtensorMap& tmR, const CUtensorMap& tmG, const BuildOp& op, int64_t blocks, int nacc, int num_sms,
                  cudaStream_t st) {
-    static bool attr_done = false;
+    bool& attr_done = dev_state().build_attrs_done;
     if (!attr_done) {
         KRR_CUDA_CHECK(cudaFuncSetAttribute(build_tc_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, build_smem(1)));
         KRR_CUDA_CHECK(cudaFuncSetAttribute(build_tc_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, build_smem(2)));
@@ -1369,7 +1417,7 @@ int krr_build_bordered(const int8_t* d_G, int64_t n, int64_t n_valid, int64_t p,
     if (ibs) {      // thermometer-encode, then the same kernel on the encoded matrix (2p columns of 0/1)
         int8_t* U = reinterpret_cast<int8_t*>(static_cast<uint8_t*>(d_ws) + align_up(static_cast<size_t>(n) * sizeof(int), 1024));
         const int64_t ldu = static_cast<int64_t>(ibs_pitch(p));
-        rc = launch(CAT_MISC, ibs_encode_kernel, dim3(static_cast<unsigned>((ldu + 255) / 256 < 64 ? (ldu + 255) / 256 : 64), static_cast<unsigned>(n)),
+        rc = launch(CAT_MISC, ibs_encode_kernel, dim3(static_cast<unsigned>(n), static_cast<unsigned>((ldu + 255) / 256 < 64 ? (ldu + 255) / 256 : 64)),
                     dim3(256), 0, st, d_G, n, p, ldg, U, ldu);
         if (rc) return rc;
         d_G = U; ldg = ldu; p = 2 * p;
@@ -1454,9 +1502,9 @@ int krr_predict(const int8_t* d_T, int64_t m, int64_t ldt, const int8_t* d_G, in
         const int64_t ldu = static_cast<int64_t>(ibs_pitch(p));
         int8_t* UG = UT + m * ldu;
         const unsigned gx = static_cast<unsigned>((ldu + 255) / 256 < 64 ? (ldu + 255) / 256 : 64);
-        rc = launch(CAT_MISC, ibs_encode_kernel, dim3(gx, static_cast<unsigned>(m)), dim3(256), 0, st, d_T, m, p, ldt, UT, ldu);
+        rc = launch(CAT_MISC, ibs_encode_kernel, dim3(static_cast<unsigned>(m), gx), dim3(256), 0, st, d_T, m, p, ldt, UT, ldu);
         if (rc) return rc;
-        rc = launch(CAT_MISC, ibs_encode_kernel, dim3(gx, static_cast<unsigned>(n)), dim3(256), 0, st, d_G, n, p, ldg, UG, ldu);
+        rc = launch(CAT_MISC, ibs_encode_kernel, dim3(static_cast<unsigned>(n), gx), dim3(256), 0, st, d_G, n, p, ldg, UG, ldu);
         if (rc) return rc;
         d_T = UT; d_G = UG; ldt = ldg = ldu; p = 2 * p;
     }
@@ -1485,6 +1533,50 @@ int krr_predict(const int8_t* d_T, int64_t m, int64_t ldt, const int8_t* d_G, in
     else if (nrp == 16) predict_kw_kernel<16><<<grid, 256, 0, st>>>(K, m, n, n, d_W, ldw, nrhs, d_P, ldp);
     else predict_kw_kernel<32><<<grid, 256, 0, st>>>(K, m, n, n, d_W, ldw, nrhs, d_P, ldp);
     return cudaGetLastError() == cudaSuccess ? KRR_OK : KRR_ERR_CUDA;
+}
+
+// ------------------------------------------------------------------------- roofline denominators (beside the path)
+int krr_peak_probe(int kind, int64_t work, float* h_ms, double* h_flops, void* stream) {
+    if (!h_ms || !h_flops || work < 1 || kind < PEAK_F16 || kind > PEAK_F16x3) return KRR_ERR_ARG;
+    if (kind != PEAK_FFMA && (work % 16 != 0 || work > (1ll << 30))) return KRR_ERR_ARG;
+    int num_sms = 0;
+    int rc = check_device(&num_sms);
+    if (rc) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    DeviceState& d = dev_state();
+    if (!d.peak_attrs_done) {
+        KRR_CUDA_CHECK(cudaFuncSetAttribute(peak_mma_kernel<PEAK_F16>, cudaFuncAttributeMaxDynamicSharedMemorySize, kPeakSmem));
+        KRR_CUDA_CHECK(cudaFuncSetAttribute(peak_mma_kernel<PEAK_F8>, cudaFuncAttributeMaxDynamicSharedMemorySize, kPeakSmem));
+        KRR_CUDA_CHECK(cudaFuncSetAttribute(peak_mma_kernel<PEAK_MXF8>, cudaFuncAttributeMaxDynamicSharedMemorySize, kPeakSmem));
+        KRR_CUDA_CHECK(cudaFuncSetAttribute(peak_mma_kernel<PEAK_F16x3>, cudaFuncAttributeMaxDynamicSharedMemorySize, kPeakSmem));
+        d.peak_attrs_done = true;
+    }
+    cudaEvent_t e0 = pool_event(d), e1 = pool_event(d);
+    const int pairs = num_sms / 2;
+    double flops = 0.0;
+    KRR_CUDA_CHECK(cudaEventRecord(e0, st));
+    if (kind == PEAK_FFMA) {
+        float* sink = nullptr;                                   // never written (the guard value is unreachable)
+        peak_ffma_kernel<<<2 * num_sms, 1024, 0, st>>>(static_cast<int>(work), sink);
+        flops = 2.0 * num_sms * 1024.0 * static_cast<double>(work) * 128.0 * 2.0;
+    } else {
+        const int chunks = static_cast<int>(work);
+        const double per_mma = 2.0 * 256.0 * 256.0 * (kind == PEAK_F16 || kind == PEAK_F16x3 ? 16.0 : 32.0);
+        if (kind == PEAK_F16) peak_mma_kernel<PEAK_F16><<<2 * pairs, kPeakThreads, kPeakSmem, st>>>(chunks);
+        else if (kind == PEAK_F8) peak_mma_kernel<PEAK_F8><<<2 * pairs, kPeakThreads, kPeakSmem, st>>>(chunks);
+        else if (kind == PEAK_MXF8) peak_mma_kernel<PEAK_MXF8><<<2 * pairs, kPeakThreads, kPeakSmem, st>>>(chunks);
+        else peak_mma_kernel<PEAK_F16x3><<<2 * pairs, kPeakThreads, kPeakSmem, st>>>(chunks);
+        flops = static_cast<double>(pairs) * chunks * 4.0 * (kind == PEAK_F16x3 ? 3.0 : 1.0) * per_mma;
+    }
+    ++g_launches;
+    if (cudaGetLastError() != cudaSuccess) return KRR_ERR_CUDA;
+    KRR_CUDA_CHECK(cudaEventRecord(e1, st));
+    KRR_CUDA_CHECK(cudaEventSynchronize(e1));
+    KRR_CUDA_CHECK(cudaEventElapsedTime(h_ms, e0, e1));
+    *h_flops = flops;
+    d.event_pool.push_back(e0);
+    d.event_pool.push_back(e1);
+    return KRR_OK;
 }
 
 }  // extern "C"

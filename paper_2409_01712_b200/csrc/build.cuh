@@ -7,10 +7,10 @@
 //
 // Only the lower TILES of A (tile row >= tile column, diagonal tiles as full squares) are produced: that
 // is what the Associate phase reads.  One persistent, warp-specialised kernel on CTA pairs (cluster of 2,
-// cta_group::2): a pair computes a 256 x 256 block over the whole SNP range, each CTA staging 128 rows of
-// the row operand and 128 of the column operand per 128-SNP chunk (TMA, 128-byte swizzle, 6-slot ring);
-// the INT32 accumulators are double-buffered in TMEM so that the exp epilogue of a block overlaps the
-// MMAs of the next.  SNP counts that are not a multiple of 128 rely on TMA's zero fill.
+// cta_group::2): a pair computes a 256 x 512 block over the whole SNP range (256 x 256 when the tile size is
+// no multiple of 512) into both 256-column INT32 accumulators of TMEM (single-buffered), each CTA staging
+// 128 rows of the row operand and 2 x 128 of the column operand per 128-SNP chunk (TMA, 128-byte swizzle,
+// 4-slot ring of 48 KB).  SNP counts that are not a multiple of 128 rely on TMA's zero fill.
 #pragma once
 #include "common.cuh"
 #include "ptx.cuh"
@@ -88,10 +88,10 @@ row_sqnorm_kernel(const int8_t* __restrict__ G, int64_t n, int64_t p, int64_t ld
 // columns p2 .. ldu-1 are zeroed so that the encoded matrix can be read in whole 16-byte units.
 __global__ void __launch_bounds__(256)
 ibs_encode_kernel(const int8_t* __restrict__ G, int64_t n, int64_t p, int64_t ldg, int8_t* __restrict__ U, int64_t ldu) {
-    const int64_t row = blockIdx.y;
+    const int64_t row = blockIdx.x;             // rows in x: gridDim.y stops at 65535, n does not
     const int8_t* g = G + row * ldg;
     int8_t* u = U + row * ldu;
-    for (int64_t k = static_cast<int64_t>(blockIdx.x) * 256 + threadIdx.x; k < ldu; k += static_cast<int64_t>(gridDim.x) * 256) {
+    for (int64_t k = static_cast<int64_t>(blockIdx.y) * 256 + threadIdx.x; k < ldu; k += static_cast<int64_t>(gridDim.y) * 256) {
         int8_t v = 0;
         if (k < p) v = g[k] >= 1;
         else if (k < 2 * p) v = g[k - p] >= 2;

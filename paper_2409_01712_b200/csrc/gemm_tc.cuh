@@ -251,11 +251,7 @@ __device__ __forceinline__ bool next_item(const GemmOp& op, ItemIter& st, int un
             w.t_lo = nt * sl / g; w.t_hi = nt * (sl + 1) / g;
             w.cpos = g - 1 - sl; w.clen = g; w.fidx = t - op.split_t0;
         }
-#ifdef KRR_EXP_REVERSE_ROWS
-        w.rb = op.rb0 + (op.nrb / CG - 1 - t / ncbu) * CG;
-#else
         w.rb = op.rb0 + (t / ncbu) * CG;
-#endif
         w.cb = op.cb0 + (t % ncbu) * CG;
         if (tile_is_skipped(op, w.rb + CG - 1, w.cb)) continue;      // the whole (pair) block lies above the diagonal
         w.mode = op.mode; w.c = op.c; w.dep = 0;

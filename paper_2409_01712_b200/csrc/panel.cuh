@@ -42,28 +42,44 @@ plane_scale_kernel(AView A, int64_t n, float* __restrict__ scl) {
     }
 }
 
-// Byte offsets of the mosaic tiles (column-major lower order prefix sum).  One thread.
-__global__ void offsets_kernel(int NT, int nb, const uint8_t* __restrict__ map, int64_t* __restrict__ off) {
+// FNV-1a over the lower entries of a map in column-major tile order: the host (h_map) and the device (d_map) side of
+// the same call must agree (sizes come from h_map, offsets and MMA classes from d_map).
+__host__ __device__ __forceinline__ uint64_t map_hash_step(uint64_t h, uint8_t v) { return (h ^ v) * 1099511628211ull; }
+constexpr uint64_t kMapHashSeed = 1469598103934665603ull;
+
+// Byte offsets of the mosaic tiles (column-major lower order prefix sum).  One thread.  If the device map does not
+// hash to `host_hash` (the caller's h_map and d_map differ) every offset is set to 0 -- all tiles alias the first
+// (FP32, diagonal) tile, so that nothing is read or written outside buffers sized from h_map -- and *info = -1.
+__global__ void offsets_kernel(int NT, int nb, const uint8_t* __restrict__ map, int64_t* __restrict__ off, uint64_t host_hash,
+                               int* __restrict__ info) {
     if (threadIdx.x != 0 || blockIdx.x != 0) return;
     int64_t acc = 0;
     const int64_t elems = static_cast<int64_t>(nb) * nb;
+    uint64_t h = kMapHashSeed;
     for (int j = 0; j < NT; ++j)
         for (int i = j; i < NT; ++i) {
             off[i * NT + j] = acc;
-            acc += elems * prec_bytes(map[i * NT + j]);
+            const uint8_t p = map[i * NT + j];
+            h = map_hash_step(h, p);
+            acc += elems * prec_bytes(p);
         }
+    if (h != host_hash) {
+        for (int j = 0; j < NT; ++j)
+            for (int i = j; i < NT; ++i) off[i * NT + j] = 0;
+        if (info) *info = -1;
+    }
 }
 
-// max|A_ij| for the FP8 tiles of A.  grid = (nb / 32, nslots); a_amax zeroed beforehand.
+// max|A_ij| for the FP8 tiles of A.  grid = (nslots, nb / 32); a_amax zeroed beforehand.
 __global__ void __launch_bounds__(256)
 tile_amax_kernel(AView A, const uint8_t* __restrict__ map, float* __restrict__ a_amax) {
     const int NT = A.NT, nb = A.nb;
     int j = 0;
-    int64_t rem = blockIdx.y;
+    int64_t rem = blockIdx.x;
     while (rem >= NT - j) { rem -= NT - j; ++j; }
     const int i = j + static_cast<int>(rem);
     if (map[i * NT + j] != KRR_FP8_E4M3) return;
-    const int r0 = blockIdx.x * 32;
+    const int r0 = blockIdx.y * 32;
     const int vec_per_row = nb / 4;
     float amax = 0.0f;
     for (int idx = threadIdx.x; idx < 32 * vec_per_row; idx += 256) {

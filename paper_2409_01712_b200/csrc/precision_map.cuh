@@ -9,18 +9,18 @@ namespace krr {
 constexpr int kStatRows = 32;        // rows of a tile reduced by one CTA
 constexpr int kStatThreads = 256;
 
-// grid = (nb / kStatRows, nslots).  partial[slot * chunks + chunk] = sum of squares (double),
+// grid = (nslots, nb / kStatRows) -- the unbounded index in x (gridDim.y stops at 65535).  partial[slot * chunks + chunk] = sum of squares (double),
 // pamax[...] = max |a| of rows [chunk*kStatRows, +kStatRows) of the tile.
 __global__ void __launch_bounds__(kStatThreads)
 tile_stats_kernel(AView A, double* __restrict__ partial, float* __restrict__ pamax) {
     const int NT = A.NT, nb = A.nb;
-    const int64_t slot = blockIdx.y;
+    const int64_t slot = blockIdx.x;
     // invert slot -> (i, j): column-major lower order
     int j = 0;
     int64_t rem = slot;
     while (rem >= NT - j) { rem -= NT - j; ++j; }
     const int i = j + static_cast<int>(rem);
-    const int chunk = blockIdx.x;
+    const int chunk = blockIdx.y;
     const int r0 = chunk * kStatRows;
     const int vec_per_row = nb / 4;
     double acc = 0.0;
@@ -48,8 +48,8 @@ tile_stats_kernel(AView A, double* __restrict__ partial, float* __restrict__ pam
         __syncthreads();
     }
     if (threadIdx.x == 0) {
-        partial[slot * gridDim.x + chunk] = s_acc[0];
-        pamax[slot * gridDim.x + chunk] = s_max[0];
+        partial[slot * gridDim.y + chunk] = s_acc[0];
+        pamax[slot * gridDim.y + chunk] = s_max[0];
     }
 }
 

@@ -21,18 +21,7 @@
 
 namespace krr {
 
-// phase timestamps for kernel tuning (compiled in only by the tuning harness)
-#ifdef KRR_TRI_TIMING
-__device__ long long g_tri_t[32];
-#define KRR_TRI_T(i) do { if (tid == 0) g_tri_t[i] = clock64(); } while (0)
-#else
-#define KRR_TRI_T(i) do { } while (0)
-#endif
-
-#ifndef KRR_TRI_UNROLL_AB
-#define KRR_TRI_UNROLL_AB 2
-#endif
-constexpr int kAbUnroll = KRR_TRI_UNROLL_AB;
+constexpr int kAbUnroll = 2;
 constexpr int kTriThreads = 512;
 constexpr int kTriLd = 132;                       // 16-byte aligned rows; LDS.128 by row is conflict free
 constexpr int kTriSmem = (2 * kBlk * kTriLd + kBlk + 32) * 4;   // L, inv(L), reciprocals of the diagonal of L, reduction scratch
@@ -231,7 +220,6 @@ __device__ __forceinline__ void potrf128_body(float* tri_sm, int tid, Sync sync,
     constexpr int NW = NTHR / 32;
     // W is block-column-major: element (r, c) of 128x128 block (rb, cb) at ((rb*nsub + cb)*128 + c)*128 + r
     float* wblk = W + (static_cast<int64_t>(r0 / kBlk) * (nb / kBlk) + c0 / kBlk) * (kBlk * kBlk);
-    KRR_TRI_T(0);
     {
         // coalesced column reads (lane = row), 32 per thread in flight before the first store
         constexpr int PER = 32;
@@ -249,7 +237,6 @@ __device__ __forceinline__ void potrf128_body(float* tri_sm, int tid, Sync sync,
             *reinterpret_cast<float4*>(x + (idx >> 5) * kTriLd + (idx & 31) * 4) = make_float4(0.f, 0.f, 0.f, 0.f);
     }
     sync();
-    KRR_TRI_T(1);
     float* tscr = x + 32;                    // scratch strip of the inverse's off-diagonal rows
     for (int jb = 0; jb < 4; ++jb) {
         const int j0 = 32 * jb;
@@ -263,7 +250,6 @@ __device__ __forceinline__ void potrf128_body(float* tri_sm, int tid, Sync sync,
             inv_row_phase1(a, x, tscr, jb - 1, warp - 1, NW - 1, lane);
         }
         sync();
-        KRR_TRI_T(2 + 5 * jb);
         const int R = kBlk - (j0 + 32);                 // rows below the diagonal block
         // B: panel, one thread per row below (warps 1 ..); warp 0 inverts the diagonal sub-block; the
         //    remaining warps finish block row jb-1 of the inverse
@@ -272,7 +258,6 @@ __device__ __forceinline__ void potrf128_body(float* tri_sm, int tid, Sync sync,
         else if (tid - 32 < R) panel32_row(a, rinv, j0, j0 + 32 + (tid - 32));
         else if (jb >= 2) inv_row_phase2(x, tscr, jb - 1, warp - first_free, NW - first_free, lane);
         sync();
-        KRR_TRI_T(3 + 5 * jb);
         if (R > 0) {
             // C: trailing update S_ic -= L_i,jb L_c,jb^T for the 32-column blocks right of jb (lower part):
             //    each column block's rows are dealt to its share of the warps
@@ -281,16 +266,13 @@ __device__ __forceinline__ void potrf128_body(float* tri_sm, int tid, Sync sync,
             const int rr = 32 * cb;
             abt32_sub_rows(a + j0, a + rr * kTriLd + j0, a + rr, rr + wi, kBlk, wn, lane);
             sync();
-            KRR_TRI_T(5 + 5 * jb);
         }
     }
-    KRR_TRI_T(22);
     // block row 3 of the inverse
     inv_row_phase1(a, x, tscr, 3, warp, NW, lane);
     sync();
     inv_row_phase2(x, tscr, 3, warp, NW, lane);
     sync();
-    KRR_TRI_T(23);
     // power-of-two scale of the inverse's planes: max|x| * si <= 2^14
     {
         float m = 0.0f;
@@ -336,7 +318,6 @@ __device__ __forceinline__ void potrf128_body(float* tri_sm, int tid, Sync sync,
         *reinterpret_cast<uint2*>(linv_hi + static_cast<int64_t>(c0 + r) * kBlk + c4) = *reinterpret_cast<const uint2*>(hi);
         *reinterpret_cast<uint2*>(linv_lo + static_cast<int64_t>(c0 + r) * kBlk + c4) = *reinterpret_cast<const uint2*>(lo);
     }
-    KRR_TRI_T(31);
 }
 
 

@@ -29,11 +29,44 @@ from krr_inputs import CONFIGS, make_problem, make_problem_lower_tiles  # noqa: 
 
 METRIC = "mixed-precision Cholesky TOp/s (n^3/3 / device time)"
 UNIT = "TOp/s"
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the trailing-update kernel, from the
-# `ncu --set full` capture summarised under profiles/ (bytes; None where no capture exists)
-TRAFFIC_NCU = {"C3": 11.25e9, "C3h": 5.34e9, "C5p": 7.0e9}
-TRAFFIC_NOTE = ("profiles/r01_gemm_tc_full_C3.md: one launch of the dominant shape O(k+1) at mid factorisation (C3/C3h: k = 32, "
-                "31 tile rows, K = 32 tiles, algorithmic operand bytes 4.3 / 2.1 GB; C5p: k = 48, 2.4 GB)")
+# The extra workloads the default run times after the headline (the low-precision classes of the metric's name):
+# name -> minimum number of timed steps (enough device time for >= 10 clock samples at 100 ms)
+EXTRA_WORKLOADS = {"S1": 40, "C3h": 12, "C5p": 8}
+
+
+def ncu_traffic(name):
+    """dram__bytes_read.sum + dram__bytes_write.sum of one launch of the trailing-update kernel (dominant shape), read from
+    the raw `ncu --set full ... --page raw --csv` export committed under profiles/ (None where no capture exists)."""
+    import csv
+    path = os.path.join(ROOT, "profiles", f"r02_update_kernel_raw_{name}.csv")
+    if not os.path.exists(path):
+        return None, None
+    with open(path) as f:
+        rows = [r for r in csv.reader(f) if r]
+    hdr = next((r for r in rows if "dram__bytes_read.sum" in r), None)
+    if hdr is None:
+        return None, None
+    units = rows[rows.index(hdr) + 1]
+    data = rows[rows.index(hdr) + 2:]
+    scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1e12}
+    tot = None
+    for r in data[-1:]:                          # the last captured launch is the dominant shape O(k+1)
+        tot = 0.0
+        for key in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
+            i = hdr.index(key)
+            tot += float(r[i].replace(",", "")) * scale.get(units[i], 1.0)
+    return tot, f"profiles/r02_update_kernel_raw_{name}.csv (last captured launch; command in profiles/r02_update_kernel_{name}.md)"
+
+
+def measured_class_peaks():
+    """Per-class tensor peaks measured with krr_peak_probe on a B200 of this pool (profiles/r02_peaks.json, written by
+    `python -m paper_2409_01712_b200.peaks`): the FP8 : FP16 ratio of the sustained figures, applied to the driver's
+    cuBLAS bf16 peak.  None when the file is absent (then the guide's nominal ratio 2 is used and said so)."""
+    path = os.path.join(ROOT, "profiles", "r02_peaks.json")
+    if not os.path.exists(path):
+        return None
+    with open(path) as f:
+        return json.load(f)
 
 
 def load_peaks():
@@ -131,18 +164,28 @@ def whole_job_value(n, world, ms_per_step):
     return world * (n ** 3 / 3.0) / (ms_per_step * 1e-3) / 1e12
 
 
-def run_ours(args, rank, world, local_rank):
-    import paper_2409_01712_b200 as krr
-    from paper_2409_01712_b200 import build
-    build.build()
-    krr.lib()                                    # fail loudly if the CUDA library is missing
-    cfg = CONFIGS[args.config]
+def setup_ours(world, local_rank):
+    """Process group first, then the build on local rank 0 only (concurrent ranks must not write the same .so)."""
     dev = torch.device("cuda", local_rank)
     torch.cuda.set_device(dev)
-    peaks = load_peaks()
     if world > 1:
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=dev)
+    from paper_2409_01712_b200 import build
+    if local_rank == 0:
+        build.build()
+    if world > 1:
+        torch.distributed.barrier()
+    import paper_2409_01712_b200 as krr
+    krr.lib()                                    # fail loudly if the CUDA library is missing
+    return krr, dev
+
+
+def run_ours(args, rank, world, local_rank, krr, dev, config_name, steps, extras=True):
+    """One workload: warm-up, `steps` timed steps, then the untimed extra steps (profiler bracket, serial breakdown,
+    invariants).  extras=False (the additional workloads of the default run) skips the timeline and the graph replay."""
+    cfg = CONFIGS[config_name]
+    peaks = load_peaks()
     # ---- synthetic inputs, resident in HBM before the timed region -------------------------------
     cfg_r = replica_config(cfg, rank)                           # independent replica per rank
     n, nb, NT = cfg.n, cfg.nb, cfg.NT
@@ -208,7 +251,7 @@ def run_ours(args, rank, world, local_rank):
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
     e0.record()
-    for _ in range(args.steps):
+    for _ in range(steps):
         step(mark=True)
     e1.record()
     barrier()
@@ -218,7 +261,7 @@ def run_ours(args, rank, world, local_rank):
     upd_ms, upd_launches = prof["update_gemm"]
     krr.profile_enable(0)
     total_ms = max_over_ranks(total_ms, world, dev)
-    ms_per_step = total_ms / args.steps
+    ms_per_step = total_ms / steps
     ops = n ** 3 / 3.0
     value = whole_job_value(n, world, ms_per_step)
 
@@ -245,14 +288,15 @@ def run_ours(args, rank, world, local_rank):
     krr.profile_enable(0)
     info = int(keep["F"].info.item())
     hist = torch.bincount(h_map[torch.tril(torch.ones(NT, NT, dtype=torch.bool), -1)].long(), minlength=3).tolist()
-    sys.path.insert(0, os.path.join(ROOT, "tests"))
+    # invariants by independent torch-FP64 code (paper_2409_01712_b200/checks.py): a bench that cannot verify its
+    # result fails instead of printing a headline
     checks = {}
-    try:
-        from helpers import LowerTiles, probe_backward_error, solve_residual
+    if True:
+        from paper_2409_01712_b200.checks import LowerTiles, probe_backward_error, solve_residual
         A_chk = LowerTiles(A, n, nb) if tiled else A
         checks["backward_error_probe"] = probe_backward_error(A_chk, keep["F"], 8)
         checks["solve_residual"] = solve_residual(A_chk, keep["alpha"], Y)
-        if hist[1] + hist[2] > 0 and info == 0:
+        if extras and hist[1] + hist[2] > 0 and info == 0:
             # beside the step, untimed there: krr_refine (R19), the remedy SURVEY 8(c) quotes for FP16 / FP8 maps
             Xr = keep["alpha"].clone()
             krr.refine(A, keep["F"], Y, Xr.clone(), 1, tiled_lower=tiled, residual_norms=False)       # warm-up
@@ -275,36 +319,50 @@ def run_ours(args, rank, world, local_rank):
                                      "solve_residual": solve_residual(A_chk, Xc, Y),
                                      "correction_rel": float(torch.linalg.norm((Xc - keep["alpha"]).double())
                                                              / torch.linalg.norm(Xc.double()))}
-    except Exception as ex:                      # checking only; never masks the measurement
-        checks["error"] = repr(ex)
+    expected_breakdown = cfg.map_request == "force_fp8"          # C5: the literal map is indefinite (SURVEY finding 2)
+    if info != 0 and not expected_breakdown:
+        raise SystemExit(f"bench.py: {cfg.name}: krr_potrf_mp reported info = {info}")
+    bound = 1e-6 if (hist[1] == 0 and hist[2] == 0) else 5e-4
+    checks["backward_error_bound"] = bound
+    if info == 0 and not (checks["backward_error_probe"] <= bound):
+        raise SystemExit(f"bench.py: {cfg.name}: backward error {checks['backward_error_probe']:.3e} above {bound:.0e}")
 
     # ---- roofline of the dominant kernel (tcgen05 trailing update) --------------------------------
     fl = update_flops_by_class(h_map, nb)
     p16 = peaks["bf16_sustained"]
-    class_peak = {0: p16 / 3.0, 1: p16, 2: 2.0 * p16}
+    mp = measured_class_peaks()
+    if mp is not None and "mxf8" in mp and "f16" in mp:
+        r8 = mp["mxf8"]["sustained_tflops"] / mp["f16"]["sustained_tflops"]
+        r3 = mp["f16x3"]["sustained_tflops"] / mp["f16"]["sustained_tflops"] if "f16x3" in mp else 1.0
+        ratio_note = (f"FP8 = x{r8:.3f}, measured (krr_peak_probe kind::mxf8f6f4.block_scale over kind::f16, both sustained, "
+                      f"profiles/r02_peaks.json; the three-instruction FP32-class sequence runs at x{r3:.3f} of kind::f16)")
+    else:
+        r8 = 2.0
+        ratio_note = "FP8 = x2 (nominal ratio; profiles/r02_peaks.json absent)"
+    class_peak = {0: p16 / 3.0, 1: p16, 2: r8 * p16}
     upd_flops = sum(fl.values())
     t_bound_upd = sum(fl[c] / (class_peak[c] * 1e12) for c in fl)
     pw_peak = upd_flops / t_bound_upd / 1e12 if t_bound_upd > 0 else class_peak[0]
-    achieved = upd_flops * args.steps / (upd_ms * 1e-3) / 1e12 if upd_ms > 0 else 0.0
+    achieved = upd_flops * steps / (upd_ms * 1e-3) / 1e12 if upd_ms > 0 else 0.0
     ser_ms = breakdown.get("update_gemm", {}).get("ms", 0.0)
     roofline = {"bound": "tensor", "kernel": "gemm_tc_kernel (MODE_UPDATE: trailing SYRK/GEMM)",
                 "achieved": round(achieved, 2), "peak": round(pw_peak, 2), "unit": "TFLOP/s",
-                "frac": round(achieved / pw_peak, 4), "traffic": TRAFFIC_NCU.get(cfg.name),
-                "traffic_note": TRAFFIC_NOTE if cfg.name in TRAFFIC_NCU else None,
+                "frac": round(achieved / pw_peak, 4), "traffic": ncu_traffic(cfg.name)[0],
+                "traffic_note": ncu_traffic(cfg.name)[1],
                 "measured": "CUDA events around every launch of the kernel on its launching streams, inside the timed "
                             "region (default schedule: launches share SMs with the panel kernels they overlap)",
                 "frac_serial_schedule": round(upd_flops / (ser_ms * 1e-3) / 1e12 / pw_peak, 4) if ser_ms else None,
                 "peak_source": f"{peaks['source']}: bf16 sustained {p16} TF/s; FP32-class = /3 (three kind::f16 "
-                               "MMAs per product), FP8 = x2 (nominal ratio)",
+                               "MMAs per product), " + ratio_note,
                 "flops_per_step_by_class": {"fp32x3": fl[0], "fp16": fl[1], "fp8": fl[2]},
-                "kernel_ms_per_step": round(upd_ms / args.steps, 3), "launches_per_step": upd_launches // args.steps}
+                "kernel_ms_per_step": round(upd_ms / steps, 3), "launches_per_step": upd_launches // steps}
     # whole factorisation against the precision-weighted tensor roofline (all n^3/3 credited to the
     # class peaks; panel TRSM runs on the tensor cores in FP32-class)
     potrf_ms = phases["potrf_mp"]
     pw_frac_potrf = (ops / (pw_peak * 1e12)) / (potrf_ms * 1e-3) if potrf_ms > 0 else None
 
     # ---- optional: device timeline of the three internal streams for one krr_potrf_mp call (krr_profile_timeline)
-    if args.timeline and NT > 2 and not (flags & krr.FLAG_NO_LOOKAHEAD):
+    if extras and args.timeline and NT > 2 and not (flags & krr.FLAG_NO_LOOKAHEAD):
         d_map_t = h_map.to(dev)
         t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         torch.cuda.synchronize()
@@ -324,17 +382,18 @@ def run_ours(args, rank, world, local_rank):
     # read back every step (the recorded launch sequence is valid for one map; another map would be recorded again).
     # The headline stays the direct-launch path because the roofline above needs events around every update launch.
     graph_replay = None
-    if not args.no_graph and info == 0:
+    if extras and not args.no_graph and info == 0:
         alpha_direct = keep["alpha"]
         keep.pop("F", None)
         torch.cuda.empty_cache()
         try:
-            graph_replay = run_graph_replay(krr, A, Y, cfg, dev, flags, force, h_map, alpha_direct, args.steps)
+            graph_replay = run_graph_replay(krr, A, Y, cfg, dev, flags, force, h_map, alpha_direct, steps)
         except Exception as ex:                  # an extra, never masks the measurement
             graph_replay = {"error": repr(ex)}
         torch.cuda.empty_cache()
 
-    out = {"metric": METRIC, "value": round(value, 3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+    ws_bytes = int(krr.lib().krr_potrf_mp_workspace(n, nb, __import__("ctypes").c_void_p(h_map.data_ptr())))
+    out = {"metric": METRIC, "value": round(value, 3), "unit": UNIT, "n_gpus": world, "steps": steps,
            "warmup": args.warmup, "ms_per_step": round(ms_per_step, 3), "higher_is_better": True,
            "scaling": "weak", "vs_baseline": None, "dtype": "f32 (3x f16 tcgen05 split, FP32 accumulate)"
            if hist[1] == 0 and hist[2] == 0 else "mixed f32/f16/f8 tiles, FP32 accumulate",
@@ -348,7 +407,9 @@ def run_ours(args, rank, world, local_rank):
            "phases_ms": {k: round(v, 3) for k, v in phases.items()},
            "potrf_TOps": round(ops / (potrf_ms * 1e-3) / 1e12, 2) if potrf_ms > 0 else None,
            "potrf_frac_of_precision_weighted_tensor_peak": round(pw_frac_potrf, 4) if pw_frac_potrf else None,
-           "breakdown_ms_serial_schedule": breakdown, "info": info, "checks": checks}
+           "breakdown_ms_serial_schedule": breakdown, "info": info, "checks": checks,
+           "memory_bytes": {"A": int(A.numel()) * 4, "factor_mosaic": int(krr.factor_bytes(n, nb, h_map)),
+                            "krr_potrf_mp_workspace": ws_bytes}}
     if graph_replay is not None:
         out["graph_replay"] = graph_replay
     return out, (A, Y, krr, cfg, dev)
@@ -563,9 +624,21 @@ def run_reference(args, rank):
             "warmup": min(args.warmup, 1), "ms_per_step": round(dt * 1e3, 3), "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic", "impl": "reference",
             "config": {"workload": f"{cfg.name}: n={cfg.n}, p={cfg.p}, nb={cfg.nb} (bounded sample n_s={ns})"},
-            "cpu_baseline": {"value": round(val, 6), "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "cpu_baseline": {"value": round(val, 6), "unit": UNIT, "cores": cores, "cpu_model": cpu_model(), "nproc": os.cpu_count(),
+                             "kind": "oracle", "sample": sample,
+                             "full_size_seconds_extrapolated": round(dt * (cfg.n / ns) ** 3, 1)},
             "e2e": {"value": round(val, 6), "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
+
+
+def cpu_model():
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
 
 
 def main():
@@ -574,19 +647,35 @@ def main():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", default="C3", choices=sorted(CONFIGS))
+    ap.add_argument("--config", default=None, choices=sorted(CONFIGS),
+                    help="time this workload only (default: C3 as the headline, then S1, C3h and C5p as `workloads`)")
     ap.add_argument("--sample-tiles", type=int, default=28, help="tiles per dimension of the CPU-oracle sample")
     ap.add_argument("--potrf-flags", type=int, default=0, help="extra KRR_FLAG_* bits for krr_potrf_mp (experiments)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-build", action="store_true", help="skip the Build-phase (krr_build) timing")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-graph", action="store_true", help="skip the CUDA-graph replay timing (krr_graph_*)")
+    ap.add_argument("--no-workloads", action="store_true", help="default run: skip the extra workloads S1 / C3h / C5p")
     ap.add_argument("--timeline", default=None, metavar="FILE",
                     help="write the device timeline of the internal streams of one extra krr_potrf_mp call (krr_profile_timeline)")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # `python bench.py --gpus N` without a launcher: start the N ranks ourselves (one process per GPU)
+        import socket
+        with socket.socket() as sk:
+            sk.bind(("127.0.0.1", 0))
+            port = sk.getsockname()[1]
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+               "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+        return subprocess.call(cmd)
+    if args.gpus != world:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE = {world}")
+    default_run = args.config is None
+    config = args.config or "C3"
+    args.config = config
 
     if args.impl == "reference":
         out = run_reference(args, rank)
@@ -597,15 +686,20 @@ def main():
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
     args.warmup = max(args.warmup, 3)
-    out, ctx = run_ours(args, rank, world, local_rank)
+    krr, dev = setup_ours(world, local_rank)
+    out, ctx = run_ours(args, rank, world, local_rank, krr, dev, config, args.steps)
     cfg = ctx[3]
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         A_s, ns = oracle_sample(cfg, ctx[4], args.sample_tiles)
         dt, _ = time_oracle(A_s, cfg.nb)
         out["cpu_baseline"] = {"value": round(ns ** 3 / 3.0 / dt / 1e12, 6), "unit": UNIT, "cores": host_threads(),
+                               "cpu_model": cpu_model(), "nproc": os.cpu_count(),
                                "kind": "oracle", "seconds": round(dt, 2),
                                "sample": f"leading {ns}x{ns} principal submatrix of {cfg.name} (nb={cfg.nb}), "
-                                         "FP64 tile Cholesky of oracle/cholesky.py as it stands"}
+                                         "FP64 tile Cholesky of oracle/cholesky.py as it stands",
+                               "full_size_seconds_extrapolated": round(dt * (cfg.n / ns) ** 3, 1),
+                               "extrapolation": f"sample time x (n / n_s)^3 = x {(cfg.n / ns) ** 3:.2f}: labelled extrapolated "
+                                                "(BASELINE.md section 3), not measured"}
         del A_s
     if rank == 0 and world == 1 and not args.no_build:
         try:
@@ -621,6 +715,19 @@ def main():
             e2e["ms_per_step"] = max_over_ranks(e2e["ms_per_step"], world, ctx[4])
             e2e["value"] = round(whole_job_value(cfg.n, world, e2e["ms_per_step"]), 3)
         out["e2e"] = e2e
+    del ctx
+    if default_run and not args.no_workloads and world == 1:
+        # the low-precision classes of the metric's name, each with its own roofline, checks and clock record
+        import gc
+        out["workloads"] = {}
+        keep_keys = ("value", "unit", "steps", "ms_per_step", "dtype", "config", "clocks", "gpu_launches", "roofline", "phases_ms",
+                     "potrf_TOps", "potrf_frac_of_precision_weighted_tensor_peak", "info", "checks", "memory_bytes")
+        for name, min_steps in EXTRA_WORKLOADS.items():
+            gc.collect()
+            torch.cuda.empty_cache()
+            w_out, w_ctx = run_ours(args, rank, world, local_rank, krr, dev, name, max(args.steps, min_steps), extras=False)
+            del w_ctx
+            out["workloads"][name] = {k: w_out[k] for k in keep_keys if k in w_out}
     if rank == 0:
         print(json.dumps(out), flush=True)
     if world > 1:

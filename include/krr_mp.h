@@ -150,11 +150,14 @@ int64_t krr_factor_tile_offset(int64_t n, int nb, const uint8_t* h_map, int i, i
  * L_ik = rd_{p(i,k)}(S_ik L_kk^{-T}) -- each tile is rounded once, when its final value is stored.
  * d_A      in   as for krr_precision_map; not modified.
  * d_map / h_map in  the same map in device and host memory (the launch sequence is built on the
- *               host from h_map; kernels read d_map).
+ *               host from h_map; kernels read d_map).  A mismatch is detected on the device: *d_info = -1, the
+ *               factor is unspecified, nothing is written outside buffers sized from h_map.
  * d_factor out  krr_factor_bytes(n, nb, h_map) bytes, layout above.
  * d_scales out  NT*NT floats (row-major, scales[i*NT+j]); 1.0 except FP8 tiles; 0 above diagonal.
  * d_info   out  one int: 0 on success, j > 0 = 1-based scalar column of the first non-positive
- *               pivot (contents of later tile columns are then unspecified).
+ *               pivot (contents of later tile columns are then unspecified); -1: d_map and h_map differ;
+ *               -2: the inverse of a diagonal tile left the range of its FP16 images (entries beyond 2^12 times
+ *               1 / sqrt(max A_ii): the tile is too ill-conditioned for the product form of the panel TRSM).
  * d_ws     workspace, at least krr_potrf_mp_workspace(n, nb, h_map) bytes, 1024-byte aligned.
  *          It holds the FP16 operand images of L that the tensor-core kernels read and two FP32
  *          panel buffers; it may be released once the call has completed on `stream` (krr_potrs
@@ -183,10 +186,13 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb,
  *               in: Y (phenotypes), out: alpha (the weights W of PAPER.md:82).  1 <= nrhs <= 32 and
  *               nb * (nrhs rounded up to 4, 8, 16 or 32) <= 32768 (the solved block of one tile is
  *               kept in shared memory), else KRR_ERR_SHAPE.
- * d_ws  workspace of at least krr_potrs_workspace(n, nb, nrhs) bytes, 16-byte aligned: tile offsets
- *       the inverses of the 128x128 diagonal blocks of L (2 * n * 128 floats) and transposed copies of
- *       the diagonal tiles for the backward sweep (n * nb floats), recomputed by every call.  Each diagonal tile is solved by one thread-block cluster of 8 CTAs; sums are
- *       accumulated in a fixed order (deterministic results).
+ * d_ws  workspace of at least krr_potrs_workspace(n, nb, nrhs) bytes, 16-byte aligned: tile offsets, the inverses of
+ *       the 128x128 diagonal blocks of L (2 * n * 128 floats), and from them the inverses of the whole diagonal
+ *       tiles and their transposes (2 * n * nb floats, FP32 block forward substitution), computed by every call
+ *       before the sweeps (the factor may have changed).  A diagonal step of a sweep is then one product
+ *       z_k = inv(L_kk) t_k by one thread-block cluster of 8 CTAs; sums are accumulated in a fixed order
+ *       (deterministic results).  If d_map does not agree with h_map the result is unspecified (all reads stay
+ *       inside buffers sized from h_map).
  */
 size_t krr_potrs_workspace(int64_t n, int nb, int nrhs);
 int krr_potrs(const void* d_factor, const float* d_scales,

@@ -122,8 +122,10 @@ static size_t host_offsets(int NT, int nb, const uint8_t* h_map, std::vector<int
 
 // ---- workspace layout of krr_potrf_mp ----------------------------------------------------------
 struct PotrfWs {
-    size_t off_table, a_amax, tile_amax, scl, prog, split, W, W2, linv_hi, linv_lo, Hp, Lp, Qp, total;
+    size_t off_table, a_amax, tile_amax, scl, prog, split, W, W2, linv_hi, linv_lo, Sh, Sl, Hp, Lp, Qp, total;
 };
+// rows of the scratch planes: S of the panel rows, then two sets (tile-column parity) of M, M^T, U
+static inline size_t scratch_rows(int64_t n, int nb) { return static_cast<size_t>(n) + 6 * static_cast<size_t>(nb); }
 static PotrfWs potrf_ws_layout(int64_t n, int nb, bool any_fp8) {
     const int64_t NT = n / nb;
     const size_t nslots = static_cast<size_t>(NT) * (NT + 1) / 2;
@@ -133,13 +135,15 @@ static PotrfWs potrf_ws_layout(int64_t n, int nb, bool any_fp8) {
     w.off_table = o; o = align_up(o + NT * NT * sizeof(int64_t), 1024);
     w.a_amax = o;    o = align_up(o + NT * NT * sizeof(float), 1024);
     w.tile_amax = o; o = align_up(o + nslots * sizeof(float), 1024);
-    w.scl = o;       o = align_up(o + (4 + 2 * (nb / kBlk)) * sizeof(float), 1024);
+    w.scl = o;       o = align_up(o + (SCL_COUNT + 2 * (nb / kBlk)) * sizeof(float), 1024);
     w.prog = o;      o = align_up(o + static_cast<size_t>(n / kBlk) * sizeof(int), 1024);   // fused-chain progress, per 128-block
     w.split = o;     o = align_up(o + 256 * sizeof(int), 1024);                              // slice counters of split tail blocks
     w.W = o;         o = align_up(o + static_cast<size_t>(n) * nb * sizeof(float), 1024);
     w.W2 = o;        o = align_up(o + static_cast<size_t>(n) * nb * sizeof(float), 1024);   // lookahead: column k+1's partial
     w.linv_hi = o;   o = align_up(o + 2 * static_cast<size_t>(nb) * kBlk * 2, 1024);   // two sets (column parity)
     w.linv_lo = o;   o = align_up(o + 2 * static_cast<size_t>(nb) * kBlk * 2, 1024);
+    w.Sh = o;        o = align_up(o + scratch_rows(n, nb) * nb * 2, 1024);
+    w.Sl = o;        o = align_up(o + scratch_rows(n, nb) * nb * 2, 1024);
     w.Hp = o;        o = align_up(o + plane * 2, 1024);
     w.Lp = o;        o = align_up(o + plane * 2, 1024);
     w.Qp = o;        if (any_fp8) o = align_up(o + plane, 1024);
@@ -228,24 +232,25 @@ static int launch(int cat, K kernel, dim3 grid, dim3 block, size_t smem, cudaStr
 // The tensor maps of one factorisation: hi/lo FP16 images of L (128-row boxes for A operands and for
 // single-CTA B operands, 64-row boxes for the B halves of CTA pairs), the inverted diagonal blocks,
 // and the E4M3 images.
-struct GemmMaps { CUtensorMap H, L, IH[2], IL[2], Q; };
+struct GemmMaps { CUtensorMap H, L, IH[2], IL[2], Q, SH, SL; };
 
 // cg = 2 runs MODE_UPDATE on CTA pairs (256 x 256 output blocks); needs even block counts.
 static int launch_gemm(const GemmMaps& m, const GemmOp& op_in, int max_ctas, int cg, cudaStream_t st, int linv_buf = 0,
                        int* split_flags = nullptr) {
     GemmOp op = op_in;
     if (op.nrb <= 0 || op.ncb <= 0) return KRR_OK;
-    // MODE_PANEL counts as panel_trsm, the fused diagonal chain (MODE_DIAG, POTRF included) as potrf128
-    ProfScope ps(op.mode == MODE_UPDATE ? CAT_UPDATE : (op.mode == MODE_P1 ? CAT_P1 : (op.mode == MODE_DIAG ? CAT_POTRF : CAT_P3)), st);
+    // MODE_TRSM counts as panel_trsm; the fused diagonal chain (MODE_DIAG, POTRF included) and the inverse's recursion as potrf128
+    ProfScope ps(op.mode == MODE_UPDATE ? CAT_UPDATE : (op.mode == MODE_P1 ? CAT_P1 : ((op.mode == MODE_DIAG || op.mode == MODE_INV) ? CAT_POTRF : CAT_P3)), st);
     ++g_launches;
-    if (cg == 2 && op.mode == MODE_UPDATE && op.nrb % 2 == 0 && op.rb0 % 2 == 0 && op.ncb % 2 == 0 && op.cb0 % 2 == 0) {
+    if (cg == 2 && (op.mode == MODE_UPDATE || op.mode == MODE_TRSM) && op.nrb % 2 == 0 && op.rb0 % 2 == 0 && op.ncb % 2 == 0 &&
+        op.cb0 % 2 == 0) {
         const int npairs = (op.nrb / 2) * (op.ncb / 2);
         const int max_pairs = max_ctas / 2;
         const int grid = 2 * (npairs < max_pairs ? npairs : max_pairs);
         // tail of the last wave: r leftover blocks for max_pairs pairs.  Share each of them between g pairs (slices of the
         // term range, added into W one after the other) so that the tail lasts 1/g of a block instead of a whole one.
         const int nterms = op.s_hi - op.s_lo, q = npairs / max_pairs, r = npairs % max_pairs;
-        if (split_flags && q >= 1 && r > 0 && 2 * r <= max_pairs && nterms >= 2) {
+        if (split_flags && op.mode == MODE_UPDATE && q >= 1 && r > 0 && 2 * r <= max_pairs && nterms >= 2) {
             int g = max_pairs / r;
             if (g > nterms) g = nterms;
             if (g > 16) g = 16;
@@ -261,15 +266,42 @@ static int launch_gemm(const GemmMaps& m, const GemmOp& op_in, int max_ctas, int
         attr[0].id = cudaLaunchAttributeClusterDimension;
         attr[0].val.clusterDim.x = 2; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
         cfg.attrs = attr; cfg.numAttrs = 1;
-        return cudaLaunchKernelEx(&cfg, gemm_tc_kernel<2>, m.H, m.L, m.IH[0], m.IL[0], m.Q, op) == cudaSuccess ? KRR_OK : KRR_ERR_CUDA;
+        return cudaLaunchKernelEx(&cfg, gemm_tc_kernel<2>, m.H, m.L, m.IH[0], m.IL[0], m.Q, m.SH, m.SL, op) == cudaSuccess ? KRR_OK : KRR_ERR_CUDA;
     }
-    // MODE_PANEL: one CTA per two row blocks when there are enough of them (a CTA interleaves two chains);
-    // MODE_DIAG: one CTA per row block of the diagonal tile
-    const int ntiles = (op.mode == MODE_PANEL) ? (op.nrb > max_ctas ? (op.nrb + 1) / 2 : op.nrb)
-                                               : (op.mode == MODE_DIAG ? op.nrb : op.nrb * op.ncb);
+    // MODE_DIAG: one CTA per row block of the diagonal tile; MODE_INV: one per 128 x 128 block of the level's products
+    int ntiles = op.nrb * op.ncb;
+    if (op.mode == MODE_DIAG) ntiles = op.nrb;
+    if (op.mode == MODE_INV) {
+        ntiles = 0;
+        for (int nd = 0; nd < op.nodes.count; ++nd)
+            ntiles += op.nodes.hl[nd] * op.nodes.hr[nd] * (op.inv_step == 0 ? 1 : (op.inv_last ? 1 : 2));
+        if (ntiles == 0) return KRR_OK;
+    }
     const int grid = ntiles < max_ctas ? ntiles : max_ctas;
-    gemm_tc_kernel<1><<<grid, kGemmThreads, kGemmSmem, st>>>(m.H, m.L, m.IH[linv_buf], m.IL[linv_buf], m.Q, op);
+    gemm_tc_kernel<1><<<grid, kGemmThreads, kGemmSmem, st>>>(m.H, m.L, m.IH[linv_buf], m.IL[linv_buf], m.Q, m.SH, m.SL, op);
     return cudaGetLastError() == cudaSuccess ? KRR_OK : KRR_ERR_CUDA;
+}
+
+// Levels of the binary splitting of the diagonal tile's nsub 128-blocks for the inverse M = inv(L_kk) (gemm_tc.cuh
+// MODE_INV): levels[h - 1] holds the nodes of height h (their halves are complete once the lower levels are done);
+// the root is alone in the last level.
+static void inverse_levels(int nsub, std::vector<InvNodes>* levels) {
+    levels->clear();
+    struct Rec {
+        static int go(int o, int len, std::vector<InvNodes>* lv) {
+            if (len <= 1) return 0;
+            int hl = 1;
+            while (2 * hl < len) hl *= 2;                        // largest power of two below len (len / 2 for powers of two)
+            const int hr = len - hl;
+            const int hL = go(o, hl, lv), hR = go(o + hl, hr, lv);
+            const int h = 1 + (hL > hR ? hL : hR);
+            if (static_cast<int>(lv->size()) < h) { InvNodes z; memset(&z, 0, sizeof(z)); lv->resize(h, z); }
+            InvNodes& L = (*lv)[h - 1];
+            L.o[L.count] = o; L.hl[L.count] = hl; L.hr[L.count] = hr; ++L.count;
+            return h;
+        }
+    };
+    Rec::go(0, nsub, levels);
 }
 
 template <int NRHS>
@@ -278,7 +310,7 @@ static int set_potrs_attrs() {
     KRR_CUDA_CHECK(cudaFuncSetAttribute(potrs_fwd_update_kernel<NRHS>, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
     KRR_CUDA_CHECK(cudaFuncSetAttribute(potrs_bwd_update_kernel<NRHS, (NRHS <= 16) ? 4 : 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
     KRR_CUDA_CHECK(cudaFuncSetAttribute(potrs_bwd_update_kernel<NRHS, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
-    KRR_CUDA_CHECK(cudaFuncSetAttribute(potrs_diag_kernel<NRHS>, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
+    KRR_CUDA_CHECK(cudaFuncSetAttribute(potrs_diagmul_kernel<NRHS>, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
     return KRR_OK;
 }
 
@@ -289,6 +321,7 @@ static int set_kernel_attrs() {
     KRR_CUDA_CHECK(cudaFuncSetAttribute(gemm_tc_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, kGemmSmem));
     KRR_CUDA_CHECK(cudaFuncSetAttribute(potrf128_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kTriSmem));
     KRR_CUDA_CHECK(cudaFuncSetAttribute(trtri128_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kTriSmem));
+    KRR_CUDA_CHECK(cudaFuncSetAttribute(potrs_tile_inverse_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kTinvSmem));
     if (set_potrs_attrs<4>() || set_potrs_attrs<8>() || set_potrs_attrs<16>() || set_potrs_attrs<32>()) return KRR_ERR_CUDA;
     done = true;
     return KRR_OK;
@@ -411,14 +444,13 @@ int krr_graph_destroy(krr_graph_t* graph) {
 // critical stream, O(k) done, N(k) done on the bulk stream, P(k) + F(k) done on the panel stream}; -1 = not recorded.
 int krr_profile_timeline(int NT, float* h_ms) {
     if (NT < 1 || !h_ms) return KRR_ERR_ARG;
-    if (g_pipe.ev.size() < 4 + 4 * static_cast<size_t>(NT)) return KRR_ERR_ARG;      // no such call yet
-    if (cudaEventSynchronize(g_pipe.ev[1]) != cudaSuccess || cudaEventSynchronize(g_pipe.ev[2]) != cudaSuccess ||
-        cudaEventSynchronize(g_pipe.ev[3]) != cudaSuccess)
+    if (g_pipe.ev.size() < 4 + 5 * static_cast<size_t>(NT)) return KRR_ERR_ARG;      // no such call yet
+    if (cudaEventSynchronize(g_pipe.ev[1]) != cudaSuccess || cudaEventSynchronize(g_pipe.ev[3]) != cudaSuccess)
         return KRR_ERR_CUDA;
     for (int k = 0; k < NT; ++k)
         for (int e = 0; e < 4; ++e) {
             float ms = -1.0f;
-            if (cudaEventElapsedTime(&ms, g_pipe.ev[0], g_pipe.ev[4 + 4 * k + e]) != cudaSuccess) {
+            if (cudaEventElapsedTime(&ms, g_pipe.ev[0], g_pipe.ev[4 + 5 * k + e]) != cudaSuccess) {
                 ms = -1.0f;
                 cudaGetLastError();
             }
@@ -544,9 +576,11 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
     float* tile_amax = reinterpret_cast<float*>(ws + L.tile_amax);
     float* W = reinterpret_cast<float*>(ws + L.W);
     float* scl = reinterpret_cast<float*>(ws + L.scl);
-    float* linv_scale = scl + 4;
+    float* linv_scale = scl + SCL_COUNT;
     __half* linv_hi = reinterpret_cast<__half*>(ws + L.linv_hi);
     __half* linv_lo = reinterpret_cast<__half*>(ws + L.linv_lo);
+    __half* Sh = reinterpret_cast<__half*>(ws + L.Sh);
+    __half* Sl = reinterpret_cast<__half*>(ws + L.Sl);
     __half* Hp = reinterpret_cast<__half*>(ws + L.Hp);
     __half* Lp = reinterpret_cast<__half*>(ws + L.Lp);
     uint8_t* Qp = any_fp8 ? ws + L.Qp : nullptr;
@@ -554,11 +588,15 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
     AView A{d_A, lda, tiled ? 1 : 0, NT, nb};
 
     KRR_CUDA_CHECK(cudaMemsetAsync(d_info, 0, sizeof(int), st));
-    KRR_CUDA_CHECK(cudaMemsetAsync(d_scales, 0, static_cast<size_t>(NT) * NT * sizeof(float), st));
     KRR_CUDA_CHECK(cudaMemsetAsync(tile_amax, 0, nslots * sizeof(float), st));
+    // the blocks of M above and of M^T below the diagonal are read as zeros and never written
+    KRR_CUDA_CHECK(cudaMemsetAsync(Sh + static_cast<size_t>(n) * nb, 0, 6 * static_cast<size_t>(nb) * nb * 2, st));
+    KRR_CUDA_CHECK(cudaMemsetAsync(Sl + static_cast<size_t>(n) * nb, 0, 6 * static_cast<size_t>(nb) * nb * 2, st));
     int* prog = reinterpret_cast<int*>(ws + L.prog);
     int* split_flags = (flags & KRR_FLAG_NO_TAIL_SPLIT) ? nullptr : reinterpret_cast<int*>(ws + L.split);
     KRR_CUDA_CHECK(cudaMemsetAsync(prog, 0, static_cast<size_t>(n / kBlk) * sizeof(int), st));
+    rc = launch(CAT_MISC, scales_init_kernel, dim3((NT * NT + 255) / 256), dim3(256), 0, st, NT, d_scales);
+    if (rc) return rc;
     rc = launch(CAT_MISC, offsets_kernel, dim3(1), dim3(32), 0, st, NT, nb, d_map, off, host_map_hash(NT, h_map), d_info);
     if (rc) return rc;
     rc = launch(CAT_MISC, plane_scale_kernel, dim3(1), dim3(1024), 0, st, A, n, scl);
@@ -571,7 +609,8 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
     }
 
     GemmMaps tm;
-    if (make_plane_tmap(&tm.H, Hp, nslots * nb, nb) || make_plane_tmap(&tm.L, Lp, nslots * nb, nb))
+    if (make_plane_tmap(&tm.H, Hp, nslots * nb, nb) || make_plane_tmap(&tm.L, Lp, nslots * nb, nb) ||
+        make_plane_tmap(&tm.SH, Sh, scratch_rows(n, nb), nb) || make_plane_tmap(&tm.SL, Sl, scratch_rows(n, nb), nb))
         return KRR_ERR_CUDA;
     const size_t linv_elems = static_cast<size_t>(nb) * kBlk;           // one set of inverted diagonal blocks
     for (int b = 0; b < 2; ++b)
@@ -586,45 +625,52 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
     const int cg = ((flags & KRR_FLAG_NO_CTA_PAIRS) || nb % (2 * kBlk) != 0) ? 1 : 2;
 
     const int nsub = nb / kBlk;
+    std::vector<InvNodes> inv_levels;
+    inverse_levels(nsub, &inv_levels);
     const bool lookahead = !(flags & KRR_FLAG_NO_LOOKAHEAD) && NT > 2;
     float* Wbuf[2] = {W, reinterpret_cast<float*>(ws + L.W2)};
-    cudaStream_t sh = st, sp = st, sl = st;      // critical-path stream, panel stream, bulk stream
-    enum { EV_FORK = 0, EV_JOIN_HI = 1, EV_JOIN_MID = 2, EV_JOIN_LO = 3, EV_BASE = 4 };   // then 4 events per tile column
-    auto ev_first = [&](int k) { return g_pipe.event(EV_BASE + 4 * static_cast<size_t>(k) + 0); };
-    auto ev_old = [&](int k) { return g_pipe.event(EV_BASE + 4 * static_cast<size_t>(k) + 1); };
-    auto ev_newb = [&](int k) { return g_pipe.event(EV_BASE + 4 * static_cast<size_t>(k) + 2); };
-    auto ev_fin = [&](int k) { return g_pipe.event(EV_BASE + 4 * static_cast<size_t>(k) + 3); };
+    cudaStream_t sh = st, sl = st;               // critical-path stream, bulk stream
+    enum { EV_FORK = 0, EV_JOIN_HI = 1, EV_JOIN_MID = 2, EV_JOIN_LO = 3, EV_BASE = 4, EV_PER_COL = 5 };
+    auto ev_first = [&](int k) { return g_pipe.event(EV_BASE + EV_PER_COL * static_cast<size_t>(k) + 0); };
+    auto ev_old = [&](int k) { return g_pipe.event(EV_BASE + EV_PER_COL * static_cast<size_t>(k) + 1); };
+    auto ev_newb = [&](int k) { return g_pipe.event(EV_BASE + EV_PER_COL * static_cast<size_t>(k) + 2); };
+    auto ev_trsm = [&](int k) { return g_pipe.event(EV_BASE + EV_PER_COL * static_cast<size_t>(k) + 3); };
+    auto ev_chain = [&](int k) { return g_pipe.event(EV_BASE + EV_PER_COL * static_cast<size_t>(k) + 4); };
     if (lookahead) {
         rc = g_pipe.init();
         if (rc) return rc;
-        sh = g_pipe.hi; sp = g_pipe.mid; sl = g_pipe.lo;
+        sh = g_pipe.hi; sl = g_pipe.lo;
         KRR_CUDA_CHECK(cudaEventRecord(g_pipe.event(EV_FORK), st));
         KRR_CUDA_CHECK(cudaStreamWaitEvent(sh, g_pipe.event(EV_FORK), 0));
-        KRR_CUDA_CHECK(cudaStreamWaitEvent(sp, g_pipe.event(EV_FORK), 0));
         KRR_CUDA_CHECK(cudaStreamWaitEvent(sl, g_pipe.event(EV_FORK), 0));
     }
-    // bulk kernels leave nsub SMs to the diagonal-tile chain they overlap with
-    const int bulk_ctas = lookahead ? (num_sms - nsub > nsub ? num_sms - nsub : num_sms) : num_sms;
-    auto finalize = [&](int k, const float* Wk, int i0, int count, cudaStream_t s) {
+    // bulk kernels leave a few SMs to the diagonal-tile chain they overlap with
+    const int reserve = nsub < 8 ? nsub : 8;
+    const int bulk_ctas = lookahead ? (num_sms - reserve > reserve ? num_sms - reserve : num_sms) : num_sms;
+    auto finalize = [&](int k, const float* Wk, int i0, int count, int only_fp8, cudaStream_t s) {
         if (count <= 0) return static_cast<int>(KRR_OK);
+        if (only_fp8) {                      // nothing to do when none of these tiles is FP8 (the launch sequence follows the map)
+            bool any = false;
+            for (int i = k + i0; i < k + i0 + count; ++i) any |= (h_map[i * NT + k] == KRR_FP8_E4M3);
+            if (!any) return static_cast<int>(KRR_OK);
+        }
         return launch(CAT_FINALIZE, finalize_kernel, dim3(nsub * nsub * 4, count), dim3(256), 0, s, NT, nb, k, i0, Wk, d_map,
                       static_cast<const int64_t*>(off), static_cast<const float*>(tile_amax), static_cast<uint8_t*>(d_factor),
-                      d_scales, Hp, Qp, static_cast<const float*>(scl));
+                      d_scales, Hp, Qp, static_cast<const float*>(scl), only_fp8);
     };
 
-    // Tile column k.  Critical stream `sh`: newest term on the diagonal tile, the
-    // diagonal-tile chain, then the TRSM and store of tile (k+1, k) -- all the next column's chain needs.
-    // Bulk stream `sl`: newest term on the rows below (N), then the older terms of column k+1 (O).
-    // Panel stream `sp`: the TRSM of the remaining rows (P) and their store (F); latency-bound, it fills
-    // the SMs the bulk kernel leaves free and takes the rest as O(k+1) drains.  N(k+1) waits for F(k);
-    // column k+1's chain runs beside F(k), N(k+1), O(k+2).
+    // Tile column k.  Critical stream `sh`: newest term on the diagonal tile, the diagonal-tile
+    // chain, M = inv(L_kk), then the TRSM product and store of tile (k+1, k) -- all the next column's chain needs.
+    // Bulk stream `sl`: newest term on the rows below (N(k): S into the scratch planes), the older terms of column
+    // k+1 (O(k+1), beside the chain of column k), then the TRSM product of the remaining rows (T(k) = S M^T, stored
+    // straight into the mosaic) -- every bulk kernel is a full-width tensor-core product.
     // (a lambda: an error in the middle still joins the internal streams below, so the caller's stream -- or a
     // stream capture -- is left in a consistent state)
     auto run_columns = [&]() -> int {
     for (int k = 0; k < NT; ++k) {
         const int mblk = (NT - k) * nsub;             // 128-row blocks of the panel
-        const int lb = k & 1;                         // buffer of the inverted diagonal blocks
-        float* Wk = Wbuf[k & 1];
+        const int lb = k & 1;                         // parity set: inverted diagonal blocks, M / M^T / U, W buffer
+        float* Wk = Wbuf[lb];
         GemmOp op;
         memset(&op, 0, sizeof(op));
         op.nb = nb; op.NT = NT; op.k = k;
@@ -633,6 +679,9 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
         op.W = Wk; op.Hp = Hp; op.Lp = Lp; op.tile_amax = tile_amax; op.flags = flags;
         op.scl = scl; op.linv_scale = linv_scale + lb * nsub;
         op.scales = d_scales; op.fp8q = (any_fp8 && !(flags & KRR_FLAG_FP8_VIA_FP16)) ? 1 : 0;
+        op.Sh = Sh; op.Sl = Sl;
+        op.srow_m = static_cast<int64_t>(n) + static_cast<int64_t>(lb) * 3 * nb; op.srow_mt = op.srow_m + nb; op.srow_u = op.srow_m + 2 * nb;
+        op.off = off; op.factor = static_cast<uint8_t*>(d_factor); op.info = d_info;
         // ---- U(k): S = rd(A) - L[:, 0:k] L[k, 0:k]^T over the tile column (SYRK + GEMM) ----
         op.mode = MODE_UPDATE; op.c = 0; op.cb0 = 0; op.ncb = nsub;
         if (!lookahead) {
@@ -648,7 +697,7 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
             op.rb0 = 0; op.nrb = nsub;
             rc = launch_gemm(tm, op, num_sms, cg, sh);
             if (rc) return rc;
-            if (k >= 1) KRR_CUDA_CHECK(cudaStreamWaitEvent(sl, ev_fin(k - 1), 0));      // column k-1 is stored
+            if (k >= 1) KRR_CUDA_CHECK(cudaStreamWaitEvent(sl, ev_first(k - 1), 0));     // tile (k, k-1) is stored
             op.rb0 = nsub; op.nrb = mblk - nsub;
             rc = launch_gemm(tm, op, bulk_ctas, cg, sl);                                 // N(k)
             if (rc) return rc;
@@ -668,11 +717,11 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
         // one launch per step (in-tile update, POTRF of a 128-block, TRSM against its inverse), or with
         // KRR_FLAG_FUSED_CHAIN one launch of nsub co-resident CTAs (MODE_DIAG): the same arithmetic
         const bool fused_chain = (flags & KRR_FLAG_FUSED_CHAIN) && nsub <= 16;
+        op.linv_hi = linv_hi + lb * linv_elems; op.linv_lo = linv_lo + lb * linv_elems;
+        op.linv_scale_w = linv_scale + lb * nsub; op.col_base = static_cast<int64_t>(k) * nb + 1;
         if (fused_chain) {
             op.mode = MODE_DIAG; op.c = 0; op.cb0 = 0; op.ncb = 1; op.rb0 = 0; op.nrb = nsub;
             op.prog = prog + static_cast<size_t>(k) * nsub;
-            op.linv_hi = linv_hi + lb * linv_elems; op.linv_lo = linv_lo + lb * linv_elems;
-            op.linv_scale_w = linv_scale + lb * nsub; op.info = d_info; op.col_base = static_cast<int64_t>(k) * nb + 1;
             rc = launch_gemm(tm, op, num_sms, 1, sh, lb);
             if (rc) return rc;
         }
@@ -684,7 +733,8 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
             }
             rc = launch(CAT_POTRF, potrf128_kernel, dim3(1), dim3(kTriThreads), static_cast<size_t>(kTriSmem), sh, Wk, nb,
                         c * kBlk, c * kBlk, linv_hi + lb * linv_elems, linv_lo + lb * linv_elems, linv_scale + lb * nsub, d_info,
-                        static_cast<int64_t>(k) * nb + static_cast<int64_t>(c) * kBlk + 1);
+                        static_cast<int64_t>(k) * nb + static_cast<int64_t>(c) * kBlk + 1, Sh, Sl, op.srow_m, op.srow_mt,
+                        static_cast<const float*>(scl));
             if (rc) return rc;
             op.mode = MODE_P3; op.c = c; op.cb0 = c; op.ncb = 1; op.rb0 = c + 1; op.nrb = nsub - c - 1;
             if (op.nrb > 0) {
@@ -692,37 +742,47 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
                 if (rc) return rc;
             }
         }
-        rc = finalize(k, Wk, 0, 1, sh);
+        rc = finalize(k, Wk, 0, 1, 0, sh);
         if (rc) return rc;
-        // ---- panel below: each 128-row block runs its whole TRSM chain in one CTA (MODE_PANEL) ----
-        op.mode = MODE_PANEL; op.c = 0; op.cb0 = 0; op.ncb = 1;
-        if (!lookahead) {
-            op.rb0 = nsub; op.nrb = mblk - nsub;
-            rc = launch_gemm(tm, op, num_sms, 1, st, lb);
-            if (rc) return rc;
-            rc = finalize(k, Wk, 1, NT - k - 1, st);
-            if (rc) return rc;
-        } else {
-            if (k + 1 < NT) {
-                // tile (k+1, k) first, on the critical stream: column k+1's chain needs nothing else of column k
-                KRR_CUDA_CHECK(cudaStreamWaitEvent(sh, ev_newb(k), 0));
-                op.rb0 = nsub; op.nrb = nsub;
+        if (k + 1 == NT) continue;                    // the last column has no panel below
+        // ---- M = inv(L_kk) by binary splitting of the 128-blocks (their inverses are in place): two launches per level ----
+        op.mode = MODE_INV; op.c = 0; op.cb0 = 0; op.ncb = 1; op.rb0 = 0; op.nrb = 1;
+        for (size_t lv = 0; lv < inv_levels.size(); ++lv) {
+            op.nodes = inv_levels[lv];
+            op.inv_last = (lv + 1 == inv_levels.size()) ? 1 : 0;
+            for (int step = 0; step < 2; ++step) {
+                op.inv_step = step;
                 rc = launch_gemm(tm, op, num_sms, 1, sh, lb);
                 if (rc) return rc;
-                rc = finalize(k, Wk, 1, 1, sh);
-                if (rc) return rc;
             }
+        }
+        // ---- panel below: X = S M^T as one triangular product, rounded once and stored (MODE_TRSM) ----
+        op.mode = MODE_TRSM; op.c = 0; op.cb0 = 0; op.ncb = nsub;
+        if (!lookahead) {
+            op.rb0 = nsub; op.nrb = mblk - nsub;
+            rc = launch_gemm(tm, op, num_sms, cg, st, lb);
+            if (rc) return rc;
+            rc = finalize(k, Wk, 1, NT - k - 1, 1, st);
+            if (rc) return rc;
+        } else {
+            KRR_CUDA_CHECK(cudaEventRecord(ev_chain(k), sh));
+            // tile (k+1, k) first, on the critical stream: column k+1's chain needs nothing else of column k
+            KRR_CUDA_CHECK(cudaStreamWaitEvent(sh, ev_newb(k), 0));
+            op.rb0 = nsub; op.nrb = nsub;
+            rc = launch_gemm(tm, op, num_sms, cg, sh, lb);
+            if (rc) return rc;
+            rc = finalize(k, Wk, 1, 1, 1, sh);
+            if (rc) return rc;
             KRR_CUDA_CHECK(cudaEventRecord(ev_first(k), sh));
-            KRR_CUDA_CHECK(cudaStreamWaitEvent(sp, ev_first(k), 0));
             if (k + 2 < NT) {
-                KRR_CUDA_CHECK(cudaStreamWaitEvent(sp, ev_newb(k), 0));
+                KRR_CUDA_CHECK(cudaStreamWaitEvent(sl, ev_chain(k), 0));
                 op.rb0 = 2 * nsub; op.nrb = mblk - 2 * nsub;
-                rc = launch_gemm(tm, op, num_sms, 1, sp, lb);                            // P(k)
+                rc = launch_gemm(tm, op, bulk_ctas, cg, sl, lb);                         // T(k)
                 if (rc) return rc;
-                rc = finalize(k, Wk, 2, NT - k - 2, sp);                                 // F(k)
+                rc = finalize(k, Wk, 2, NT - k - 2, 1, sl);
                 if (rc) return rc;
             }
-            KRR_CUDA_CHECK(cudaEventRecord(ev_fin(k), sp));
+            KRR_CUDA_CHECK(cudaEventRecord(ev_trsm(k), sl));
         }
     }
     return static_cast<int>(KRR_OK);
@@ -731,8 +791,6 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
     if (lookahead) {
         KRR_CUDA_CHECK(cudaEventRecord(g_pipe.event(EV_JOIN_HI), sh));
         KRR_CUDA_CHECK(cudaEventRecord(g_pipe.event(EV_JOIN_LO), sl));
-        KRR_CUDA_CHECK(cudaEventRecord(g_pipe.event(EV_JOIN_MID), sp));
-        KRR_CUDA_CHECK(cudaStreamWaitEvent(st, g_pipe.event(EV_JOIN_MID), 0));
         KRR_CUDA_CHECK(cudaStreamWaitEvent(st, g_pipe.event(EV_JOIN_HI), 0));
         KRR_CUDA_CHECK(cudaStreamWaitEvent(st, g_pipe.event(EV_JOIN_LO), 0));
     }
@@ -742,7 +800,7 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
 // ------------------------------------------------------------------------- solve
 static int rhs_class(int nrhs) { return nrhs <= 4 ? 4 : (nrhs <= 8 ? 8 : (nrhs <= 16 ? 16 : 32)); }
 
-struct PotrsWs { size_t off_table, dinv, dinvT, diagT, total; };
+struct PotrsWs { size_t off_table, dinv, dinvT, Minv, MinvT, total; };
 static PotrsWs potrs_ws_layout(int64_t n, int nb) {
     const size_t NT = n / nb;
     PotrsWs w;
@@ -750,7 +808,8 @@ static PotrsWs potrs_ws_layout(int64_t n, int nb) {
     w.off_table = o; o = align_up(o + NT * NT * sizeof(int64_t), 1024);
     w.dinv = o;      o = align_up(o + static_cast<size_t>(n) * kBlk * sizeof(float), 1024);
     w.dinvT = o;     o = align_up(o + static_cast<size_t>(n) * kBlk * sizeof(float), 1024);
-    w.diagT = o;     o = align_up(o + static_cast<size_t>(n) * nb * sizeof(float), 1024);     // L_kk^T for the backward sweep
+    w.Minv = o;      o = align_up(o + static_cast<size_t>(n) * nb * sizeof(float), 1024);     // inv(L_kk), every k
+    w.MinvT = o;     o = align_up(o + static_cast<size_t>(n) * nb * sizeof(float), 1024);     // inv(L_kk)^T for the backward sweep
     w.total = o;
     return w;
 }
@@ -770,11 +829,10 @@ size_t krr_potrs_workspace(int64_t n, int nb, int nrhs) {
 // update of row k+2 by column k+1 waits for the bulk update by column k.
 template <int NRHS>
 static int potrs_run(const uint8_t* factor, const float* d_scales, const uint8_t* d_map, const std::vector<int64_t>& hoff,
-                     const int64_t* off, const float* dinv, const float* dinvT, const float* diagT, int NT, int nb, float* B,
+                     const int64_t* off, const float* Minv, const float* MinvT, int NT, int nb, float* B,
                      int64_t ldb, int nrhs, int num_sms, cudaStream_t st) {
     constexpr int ROWS = 64 / NRHS, NW = kSolveThreads / 32, CPL = (NRHS <= 16) ? 4 : 2;
     const size_t smem_z = static_cast<size_t>(NRHS) * nb * sizeof(float);
-    const size_t smem_d = static_cast<size_t>(potrs_diag_smem_floats<NRHS>(nb)) * sizeof(float);
     const size_t smem_bu = smem_z + static_cast<size_t>(NW / 2) * 32 * CPL * NRHS * sizeof(float);
     const size_t smem_b1 = smem_z + static_cast<size_t>(NW / 2) * 32 * NRHS * sizeof(float);
     const int64_t blk_elems = static_cast<int64_t>(kBlk) * kBlk;
@@ -813,12 +871,13 @@ static int potrs_run(const uint8_t* factor, const float* d_scales, const uint8_t
                       NT, nb, k, j_lo, factor, off, d_map, d_scales, B, ldb, nrhs);
     };
     auto diag = [&](int k, int backward, cudaStream_t s) {
-        const float* Lkk = backward ? diagT + static_cast<int64_t>(k) * nb * nb
-                                    : reinterpret_cast<const float*>(factor + hoff[static_cast<size_t>(k) * NT + k]);
+        const float* Mk = (backward ? MinvT : Minv) + static_cast<int64_t>(k) * nb * nb;
         float* Bk = B + static_cast<int64_t>(k) * nb * ldb;
-        return launch(CAT_POTRS, potrs_diag_kernel<NRHS>, dim3(kDiagCluster), dim3(kDiagThreads), smem_d, s, nb, Lkk,
-                      dinv + k * nsub * blk_elems, dinvT + k * nsub * blk_elems, Bk, ldb, nrhs, backward);
+        return launch(CAT_POTRS, potrs_diagmul_kernel<NRHS>, dim3(kDiagCluster), dim3(kDiagThreads), smem_z, s, nb, Mk, Bk, ldb,
+                      nrhs, backward);
     };
+    // (a lambda: an error in the middle still joins the internal streams below)
+    auto run_sweeps = [&]() -> int {
     // ---- forward: L z = y
     for (int k = 0; k < NT; ++k) {
         rc = diag(k, 0, sh);
@@ -859,13 +918,16 @@ static int potrs_run(const uint8_t* factor, const float* d_scales, const uint8_t
         if (rc) return rc;
         KRR_CUDA_CHECK(cudaEventRecord(ev_bulk(k), sl));
     }
+    return static_cast<int>(KRR_OK);
+    };
+    const int rc_sweeps = run_sweeps();
     if (pipe) {
         KRR_CUDA_CHECK(cudaEventRecord(g_pipe.event(EV_JOIN_HI), sh));
         KRR_CUDA_CHECK(cudaEventRecord(g_pipe.event(EV_JOIN_LO), sl));
         KRR_CUDA_CHECK(cudaStreamWaitEvent(st, g_pipe.event(EV_JOIN_HI), 0));
         KRR_CUDA_CHECK(cudaStreamWaitEvent(st, g_pipe.event(EV_JOIN_LO), 0));
     }
-    return KRR_OK;
+    return rc_sweeps;
 }
 
 extern "C" {
@@ -896,21 +958,22 @@ int krr_potrs(const void* d_factor, const float* d_scales, const uint8_t* d_map,
     int64_t* off = reinterpret_cast<int64_t*>(ws + L.off_table);
     float* dinv = reinterpret_cast<float*>(ws + L.dinv);
     float* dinvT = reinterpret_cast<float*>(ws + L.dinvT);
-    float* diagT = reinterpret_cast<float*>(ws + L.diagT);
+    float* Minv = reinterpret_cast<float*>(ws + L.Minv);
+    float* MinvT = reinterpret_cast<float*>(ws + L.MinvT);
     rc = launch(CAT_MISC, offsets_kernel, dim3(1), dim3(32), 0, st, NT, nb, d_map, off, host_map_hash(NT, h_map), static_cast<int*>(nullptr));
     if (rc) return rc;
     const uint8_t* factor = static_cast<const uint8_t*>(d_factor);
     rc = launch(CAT_POTRS, trtri128_kernel, dim3(static_cast<unsigned>(n / kBlk)), dim3(kTriThreads), static_cast<size_t>(kTriSmem), st,
                 factor, static_cast<const int64_t*>(off), NT, nb, dinv, dinvT);
     if (rc) return rc;
-    rc = launch(CAT_POTRS, potrs_diag_transpose_kernel, dim3(nb / 32, nb / 32, NT), dim3(256), 0, st, factor,
-                static_cast<const int64_t*>(off), NT, nb, diagT);
+    rc = launch(CAT_POTRS, potrs_tile_inverse_kernel, dim3(nb / kBlk, NT), dim3(kTinvThreads), static_cast<size_t>(kTinvSmem), st,
+                factor, static_cast<const int64_t*>(off), NT, nb, static_cast<const float*>(dinv), Minv, MinvT);
     if (rc) return rc;
     switch (rhs_class(nrhs)) {
-        case 4:  return potrs_run<4>(factor, d_scales, d_map, hoff, off, dinv, dinvT, diagT, NT, nb, d_B, ldb, nrhs, num_sms, st);
-        case 8:  return potrs_run<8>(factor, d_scales, d_map, hoff, off, dinv, dinvT, diagT, NT, nb, d_B, ldb, nrhs, num_sms, st);
-        case 16: return potrs_run<16>(factor, d_scales, d_map, hoff, off, dinv, dinvT, diagT, NT, nb, d_B, ldb, nrhs, num_sms, st);
-        default: return potrs_run<32>(factor, d_scales, d_map, hoff, off, dinv, dinvT, diagT, NT, nb, d_B, ldb, nrhs, num_sms, st);
+        case 4:  return potrs_run<4>(factor, d_scales, d_map, hoff, off, Minv, MinvT, NT, nb, d_B, ldb, nrhs, num_sms, st);
+        case 8:  return potrs_run<8>(factor, d_scales, d_map, hoff, off, Minv, MinvT, NT, nb, d_B, ldb, nrhs, num_sms, st);
+        case 16: return potrs_run<16>(factor, d_scales, d_map, hoff, off, Minv, MinvT, NT, nb, d_B, ldb, nrhs, num_sms, st);
+        default: return potrs_run<32>(factor, d_scales, d_map, hoff, off, Minv, MinvT, NT, nb, d_B, ldb, nrhs, num_sms, st);
     }
 }
 

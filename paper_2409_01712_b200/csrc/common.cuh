@@ -12,6 +12,12 @@ namespace krr {
 constexpr int kBlk = 128;          // row/column sub-block of the panel algorithm and GEMM tile edge
 constexpr int kMaxNT = 1024;
 
+// scl[] (device, written by plane_scale_kernel): power-of-two scales of the FP16 operand images and the exact
+// rescalings of the accumulators.  sx: L and X values, ss: Schur-complement values, sm: M = inv(L_kk) and M^T,
+// su: the intermediate U = L21 M11 of the inverse's recursion.
+enum { SCL_SX = 0, SCL_SS = 1, SCL_INV_SX2 = 2, SCL_INV_SS = 3, SCL_SM = 4, SCL_SU = 5, SCL_INV_SM_SX = 6, SCL_INV_SM_SU = 7,
+       SCL_INV_SS_SM = 8, SCL_COUNT = 16 };
+
 // Index of tile (i,j), i >= j, in column-major order over the lower triangle (all tiles of one
 // tile column are consecutive, so a tile column is one contiguous [m x nb] slab of a plane).
 __host__ __device__ __forceinline__ int64_t tile_slot(int NT, int i, int j) {

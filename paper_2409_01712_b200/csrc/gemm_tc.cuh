@@ -42,7 +42,17 @@
 
 namespace krr {
 
-enum { MODE_UPDATE = 0, MODE_P1 = 1, MODE_P3 = 2, MODE_PANEL = 3, MODE_DIAG = 4, MODE_POTRF = 5 /* item of MODE_DIAG */ };
+enum { MODE_UPDATE = 0, MODE_P1 = 1, MODE_P3 = 2, MODE_TRSM = 3, MODE_DIAG = 4, MODE_POTRF = 5 /* item of MODE_DIAG */,
+       MODE_INV = 6 };
+
+// Scratch planes (hi / lo FP16 images, row pitch nb, one tensor map each): rows [0, n) hold the Schur complement S of
+// the panel rows below the diagonal tile (panel-local row index), then two sets (tile-column parity) of three nb x nb
+// areas: M = inv(L_kk), its transpose MT, and the intermediate U of the inverse's recursion.
+constexpr int kInvMaxNodes = 16;
+struct InvNodes {                 // one level of the binary splitting of the diagonal tile's 128-blocks
+    int count;
+    int o[kInvMaxNodes], hl[kInvMaxNodes], hr[kInvMaxNodes];   // left blocks [o, o + hl), right blocks [o + hl, o + hl + hr)
+};
 
 struct GemmOp {
     int mode;
@@ -79,7 +89,18 @@ struct GemmOp {
     // counts the CTAs that have stored their slice; zero at launch).  split_g = 0: no splitting.
     int split_t0, split_g;
     int* split_flags;
+    // scratch planes and the quantising store of MODE_TRSM (X = S inv(L_kk)^T, straight into the mosaic)
+    __half* Sh;               // scratch hi plane [n + 6 nb][nb]
+    __half* Sl;               // scratch lo plane
+    int64_t srow_m, srow_mt, srow_u;   // scratch rows of M, M^T and U of this tile column (parity set)
+    const int64_t* off;       // byte offsets of the mosaic tiles
+    uint8_t* factor;          // the mosaic
+    // MODE_INV: one step of one level of the recursion M21 = -M22 L21 M11 (step 0: U^T = M11^T L21^T; step 1: M21 and M21^T)
+    int inv_step, inv_last;   // inv_last: the root level, whose M21^T is not needed
+    InvNodes nodes;
 };
+
+
 
 constexpr int kSlots = 6;                          // shared-memory ring: 6 slots of [A block | B block]
 constexpr int kBlockK = 64;                        // fp16 elements per 128-byte swizzle row
@@ -110,6 +131,8 @@ struct TermGeom {
     int a_row, b_row;       // plane rows (TMA coordinate 1)
     int a_k0, b_k0;         // first K column (TMA coordinate 0)
     int kelems;             // K extent in elements
+    int a_src, b_src;       // operand planes: 0 = factor / panel images (tmH, tmL), 1 = inverted 128-blocks (tmIH, tmIL),
+                            // 2 = scratch (tmSH, tmSL)
 };
 
 // class word: bit 0: A operand has a lo image (FP32 tile), bit 1: B has one, bit 2: FP8 x FP8 term on the
@@ -119,8 +142,12 @@ constexpr uint32_t kClsALo = 1u, kClsBLo = 2u, kClsQ = 4u;
 // UE8M0 byte of the power of two x (> 0, normal): its biased exponent.
 __device__ __forceinline__ int pow2_exponent_byte(float x) { return static_cast<int>((__float_as_uint(x) >> 23) & 0xffu); }
 
-__device__ __forceinline__ TermGeom term_geom(const GemmOp& op, int mode, int c, int s /* term index */, int rb, int cb) {
+// rb: this CTA's output row block; cb: the column block whose B rows this CTA stages; cb_first: first column block of
+// the unit's output block (MODE_TRSM: the K range ends with the unit's last column block, M being lower triangular)
+__device__ __forceinline__ TermGeom term_geom(const GemmOp& op, int mode, int c, int s /* term index */, int rb, int cb, int cb_first,
+                                              int cg) {
     TermGeom t;
+    t.a_src = 0; t.b_src = 0;
     if (mode == MODE_UPDATE) {
         const int i = op.k + (rb * kBlk) / op.nb;
         const int subrow = (rb * kBlk) % op.nb;
@@ -136,9 +163,18 @@ __device__ __forceinline__ TermGeom term_geom(const GemmOp& op, int mode, int c,
         t.a_k0 = 0;
         t.b_k0 = 0;
         t.kelems = c * kBlk;
+    } else if (mode == MODE_TRSM) {
+        // X[rb, cb] = sum_{j <= cb} S[rb, j] M[cb, j]^T : A = S of the panel row block (scratch), B = rows of M (scratch)
+        t.a_src = 2; t.b_src = 2;
+        t.a_row = rb * kBlk;
+        t.b_row = static_cast<int>(op.srow_m) + cb * kBlk;
+        t.a_k0 = 0;
+        t.b_k0 = 0;
+        t.kelems = (cb_first + cg) * kBlk < op.nb ? (cb_first + cg) * kBlk : op.nb;
     } else {
         t.a_row = static_cast<int>(op.prow0) + rb * kBlk;
         t.b_row = c * kBlk;                                // row in the Linv planes
+        t.b_src = 1;
         t.a_k0 = c * kBlk;
         t.b_k0 = 0;
         t.kelems = kBlk;
@@ -175,30 +211,33 @@ __device__ __forceinline__ bool tile_is_skipped(const GemmOp& op, int rb, int cb
 
 // ---- work items ------------------------------------------------------------------------------------
 // The three warp roles of a CTA walk the same sequence of work items, each with its own iterator.
-//   MODE_UPDATE / MODE_P1 / MODE_P3: item = one output block (of a pair: 256 x 256), blocks dealt
+//   MODE_UPDATE / MODE_P1 / MODE_P3 / MODE_TRSM: item = one output block (of a pair: 256 x 256), blocks dealt
 //     round-robin over the CTAs (pairs) of the grid.
 //   MODE_DIAG (CG = 1, nb/128 co-resident CTAs): the whole chain of the diagonal tile in one launch --
 //     the FP32 POTRF of each 128-block runs on the eight epilogue warps of its CTA (tri128.cuh), the
 //     products on the tensor cores as elsewhere; CTAs order their items through progress counters in
 //     global memory (release: __threadfence + proxy fence + store; acquire: volatile load + fences).
-//   MODE_PANEL (CG = 1): the whole TRSM of a 128-row block of the panel below the diagonal tile,
-//     X_c = (S_c - sum_{c'<c} X_c' L_cc'^T) inv(L_cc)^T for c = 0 .. nsub-1, as the item sequence
-//     P3(0), P1(1), P3(1), P1(2), ...  Row blocks never interact, so a CTA owns its row blocks (dealt
-//     round-robin) and runs each chain by itself; an item reads, through TMA, operand images the previous
-//     item of the same row block wrote to global memory (`dep`), and two row blocks are interleaved so
-//     that one's write -> fence -> read turnaround is covered by the other's MMAs.
+//   MODE_INV (CG = 1): one step of one level of the inverse of the diagonal tile, M = inv(L_kk), by binary
+//     splitting of its 128-blocks: for a node with left blocks [o, o + hl) and right blocks [o + hl, o + hl + hr)
+//         M21 = -M22 L21 M11,   in two steps whose operands are all K-major as stored:
+//         step 0   U^T   = M11^T L21^T          (A = rows of M^T, B = rows of L_kk)
+//         step 1   M21   = -M22 U               (A = rows of M,   B = rows of U^T)
+//                  M21^T = -U^T M22^T           (A = rows of U^T, B = rows of M)     -- not for the root
+//     item = one 128 x 128 block of one of these products; the nodes of a level are independent.
 struct WorkItem {
-    int mode, c;     // contraction shape (MODE_UPDATE / MODE_P1 / MODE_P3) and sub-column
+    int mode, c;     // contraction shape (MODE_UPDATE / MODE_P1 / MODE_P3 / MODE_TRSM / MODE_INV) and sub-column
     int rb, cb;      // first output row block / column block (of the pair when CG = 2)
     int dep;         // > 0: reads what the item `dep` places earlier in this CTA's sequence wrote
     int xcta, xneed; // MODE_DIAG: reads what CTA xcta wrote in its first xneed items (xcta < 0: nothing)
     int t_lo, t_hi;  // terms [t_lo, t_hi) of the launch's term range are accumulated by this item
     int cpos, clen;  // position in the chain of slices added into W (clen = 1: the block is not split)
     int fidx;        // index into op.split_flags
+    TermGeom g;      // MODE_INV: operand geometry of the block
+    int o_row, o_col, o_var;   // MODE_INV: scratch row / column of the output block; 0 = U^T, 1 = M21, 2 = M21^T
 };
 struct ItemIter {
     int t;           // block modes: next block index
-    int g, it, m;    // MODE_PANEL: group of two row blocks, item inside the chain, member of the group
+    int g, it, m;    // MODE_DIAG: item inside the chain
 };
 
 template <int CG>
@@ -220,20 +259,40 @@ __device__ __forceinline__ bool next_item(const GemmOp& op, ItemIter& st, int un
         w.cb = w.c;
         return true;
     }
-    if (op.mode == MODE_PANEL) {
-        const int nmine = (op.nrb > unit0) ? (op.nrb - unit0 + nunits - 1) / nunits : 0;    // my row blocks
-        if (2 * st.g >= nmine) return false;
-        const int size_g = (2 * st.g + 1 < nmine) ? 2 : 1;
-        w.rb = op.rb0 + unit0 + (2 * st.g + st.m) * nunits;
-        w.c = (st.it + 1) >> 1;
-        w.cb = w.c;
-        w.mode = (st.it & 1) ? MODE_P1 : MODE_P3;
-        w.dep = st.it > 0 ? size_g : 0;
-        if (++st.m == size_g) {
-            st.m = 0;
-            if (++st.it == 2 * (op.nb / kBlk) - 1) { st.it = 0; ++st.g; }
+    if (op.mode == MODE_INV) {
+        // blocks of all nodes of the level, node after node
+        int t = st.t;
+        st.t += nunits;
+        for (int nd = 0; nd < op.nodes.count; ++nd) {
+            const int hl = op.nodes.hl[nd], hr = op.nodes.hr[nd], o = op.nodes.o[nd];
+            const int per = hl * hr;
+            const int cnt = op.inv_step == 0 ? per : (op.inv_last ? per : 2 * per);
+            if (t >= cnt) { t -= cnt; continue; }
+            const int var = op.inv_step == 0 ? 0 : 1 + t / per;
+            t %= per;
+            w.mode = MODE_INV; w.c = 0; w.dep = 0; w.o_var = var;
+            w.g.a_k0 = w.g.b_k0 = (var == 0 ? o : o + hl) * kBlk;
+            w.g.kelems = (var == 0 ? hl : hr) * kBlk;
+            if (var == 0) {              // U^T[m, n] : m over the left blocks, n over the right blocks
+                const int mb = t / hr, nbk = t % hr;
+                w.g.a_src = 2; w.g.a_row = static_cast<int>(op.srow_mt) + (o + mb) * kBlk;
+                w.g.b_src = 0; w.g.b_row = static_cast<int>(op.prow0) + (o + hl + nbk) * kBlk;
+                w.o_row = static_cast<int>(op.srow_u) + (o + mb) * kBlk; w.o_col = (o + hl + nbk) * kBlk;
+            } else if (var == 1) {       // M21[m, n] : m over the right blocks, n over the left blocks
+                const int mb = t / hl, nbk = t % hl;
+                w.g.a_src = 2; w.g.a_row = static_cast<int>(op.srow_m) + (o + hl + mb) * kBlk;
+                w.g.b_src = 2; w.g.b_row = static_cast<int>(op.srow_u) + (o + nbk) * kBlk;
+                w.o_row = static_cast<int>(op.srow_m) + (o + hl + mb) * kBlk; w.o_col = (o + nbk) * kBlk;
+            } else {                     // M21^T[m, n] : m over the left blocks, n over the right blocks
+                const int mb = t / hr, nbk = t % hr;
+                w.g.a_src = 2; w.g.a_row = static_cast<int>(op.srow_u) + (o + mb) * kBlk;
+                w.g.b_src = 2; w.g.b_row = static_cast<int>(op.srow_m) + (o + hl + nbk) * kBlk;
+                w.o_row = static_cast<int>(op.srow_mt) + (o + mb) * kBlk; w.o_col = (o + hl + nbk) * kBlk;
+            }
+            w.rb = 0; w.cb = 0;
+            return true;
         }
-        return true;
+        return false;
     }
     const int ncbu = op.ncb / CG;
     const int ntiles = (op.nrb / CG) * ncbu;
@@ -272,9 +331,11 @@ template <int CG>
 __global__ void __launch_bounds__(kGemmThreads, 1)
 gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ CUtensorMap tmL,
                const __grid_constant__ CUtensorMap tmIH, const __grid_constant__ CUtensorMap tmIL,
-               const __grid_constant__ CUtensorMap tmQ, const GemmOp op) {
-    // tmH / tmL: hi / lo FP16 images of the factor and panel (both operands of every product except the B
-    // operand of MODE_P3, which is an inverted diagonal block: tmIH / tmIL); tmQ: E4M3 images.
+               const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmSH,
+               const __grid_constant__ CUtensorMap tmSL, const GemmOp op) {
+    // tmH / tmL: hi / lo FP16 images of the factor and panel; tmIH / tmIL: the inverted 128-blocks of the diagonal
+    // tile (B operand of MODE_P3); tmSH / tmSL: the scratch planes (S of the panel rows, M = inv(L_kk), M^T, U);
+    // tmQ: E4M3 images.
     constexpr uint32_t SB = kSlotBytes;                 // [A block 16 KB | B block 16 KB]
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
@@ -312,7 +373,8 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
     if (warp == 0 && lane == 0) {
         ptx::prefetch_tmap(&tmH);
         ptx::prefetch_tmap(&tmL);
-        if (op.mode == MODE_P3 || op.mode == MODE_PANEL || op.mode == MODE_DIAG) { ptx::prefetch_tmap(&tmIH); ptx::prefetch_tmap(&tmIL); }
+        if (op.mode == MODE_P3 || op.mode == MODE_DIAG) { ptx::prefetch_tmap(&tmIH); ptx::prefetch_tmap(&tmIL); }
+        if (op.mode == MODE_TRSM || op.mode == MODE_INV) { ptx::prefetch_tmap(&tmSH); ptx::prefetch_tmap(&tmSL); }
         if (op.fp8q) ptx::prefetch_tmap(&tmQ);
         for (int s = 0; s < kSlots; ++s) {
             ptx::mbar_init(full_bar(s), 1);
@@ -383,7 +445,8 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
                 for (int s = w.t_hi - 1; s >= w.t_lo; --s) {      // descending K: see note on accumulation order
                     const uint32_t cls = make_uniform(cls_next);
                     if (s > w.t_lo) cls_next = term_class_load<CG>(op, w.mode, s - 1, rb);   // in flight during this term's chunks
-                    const TermGeom g = term_geom(op, w.mode, w.c, s, rb, cb0u + rank);  // this CTA's A rows and B rows
+                    // this CTA's A rows and B rows
+                    const TermGeom g = (w.mode == MODE_INV) ? w.g : term_geom(op, w.mode, w.c, s, rb, cb0u + rank, cb0u, CG);
                     if (cls & kClsQ) {                       // E4M3 images: 128 bytes of K per row, one slot per chunk
                         for (int ch = g.kelems / 128 - 1; ch >= 0; --ch) {
                             ptx::mbar_wait(empty_bar(slot), phase ^ 1u);
@@ -398,8 +461,10 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
                         continue;
                     }
                     const bool a_lo = cls & kClsALo, b_lo = cls & kClsBLo;
-                    const CUtensorMap* mB_hi = (w.mode == MODE_P3) ? &tmIH : &tmH;
-                    const CUtensorMap* mB_lo = (w.mode == MODE_P3) ? &tmIL : &tmL;
+                    const CUtensorMap* mA_hi = (g.a_src == 2) ? &tmSH : &tmH;
+                    const CUtensorMap* mA_lo = (g.a_src == 2) ? &tmSL : &tmL;
+                    const CUtensorMap* mB_hi = (g.b_src == 2) ? &tmSH : ((g.b_src == 1) ? &tmIH : &tmH);
+                    const CUtensorMap* mB_lo = (g.b_src == 2) ? &tmSL : ((g.b_src == 1) ? &tmIL : &tmL);
                     const uint32_t lo_bytes = CG * ((a_lo ? 1u : 0u) + (b_lo ? 1u : 0u)) * kPlaneBytes;
                     for (int ch = g.kelems / kBlockK - 1; ch >= 0; --ch) {
                         const int ak = g.a_k0 + ch * kBlockK, bk = g.b_k0 + ch * kBlockK;
@@ -407,7 +472,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
                         if (ptx::elect_one()) {              // hi images
                             const uint32_t sa = smem_base + slot * SB;
                             if (rank == 0) ptx::mbar_arrive_expect_tx(full_bar(slot), CG * 2u * kPlaneBytes);
-                            load(sa, &tmH, full_bar(slot), ak, g.a_row);
+                            load(sa, mA_hi, full_bar(slot), ak, g.a_row);
                             load(sa + kPlaneBytes, mB_hi, full_bar(slot), bk, g.b_row);
                         }
                         if (++slot == kSlots) { slot = 0; phase ^= 1u; }
@@ -416,7 +481,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
                             if (ptx::elect_one()) {
                                 const uint32_t sa = smem_base + slot * SB;
                                 if (rank == 0) ptx::mbar_arrive_expect_tx(full_bar(slot), lo_bytes);
-                                if (a_lo) load(sa, &tmL, full_bar(slot), ak, g.a_row);
+                                if (a_lo) load(sa, mA_lo, full_bar(slot), ak, g.a_row);
                                 if (b_lo) load(sa + kPlaneBytes, mB_lo, full_bar(slot), bk, g.b_row);
                             }
                             if (++slot == kSlots) { slot = 0; phase ^= 1u; }
@@ -455,7 +520,10 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
                 for (int s = w.t_hi - 1; s >= w.t_lo; --s) {      // descending K: see note on accumulation order
                     const uint32_t cls = make_uniform(cls_next);
                     if (s > w.t_lo) cls_next = term_class_load<CG>(op, w.mode, s - 1, rb);
-                    const int kelems = (w.mode == MODE_UPDATE) ? op.nb : (w.mode == MODE_P1 ? w.c * kBlk : kBlk);
+                    const int kelems = (w.mode == MODE_UPDATE) ? op.nb
+                                       : (w.mode == MODE_P1 ? w.c * kBlk
+                                          : (w.mode == MODE_INV ? w.g.kelems
+                                             : (w.mode == MODE_TRSM ? ((w.cb + CG) * kBlk < op.nb ? (w.cb + CG) * kBlk : op.nb) : kBlk)));
                     if (cls & kClsQ) {
                         const uint32_t sfa = tmem_base + kSfCol0 + 4 * CG * ((cls >> 8) & 63u);
                         const uint32_t sfb = tmem_base + kSfCol0 + 4 * CG * ((cls >> 16) & 63u);
@@ -530,7 +598,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
         // ===================== epilogue warps (TMEM -> registers -> global) =====================
         // Warp (q, hf): TMEM lanes (rows) 32q..32q+31, columns 64hf..64hf+63 of the 128x128 block.
         // W is block-column-major, so a warp's 32 rows of one column are 128 contiguous bytes; the FP16
-        // images are row-major (TMA / MMA operand layout) and go through a per-warp smem transpose so
+        // images and the mosaic tiles are row-major and go through a per-warp smem transpose so
         // that every store instruction writes 8 full 64-byte row segments.
         const int ew = warp - 2;
         const int q = warp & 3;
@@ -542,6 +610,43 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
         ItemIter iter = {unit0, 0, 0, 0};
         WorkItem w;
         int eseq = 0;                                                // items this CTA has finished
+        // One 32-row x 64-byte part of the warp's sub-block: `src` is this lane's 64 bytes (its row); dst = address
+        // of row 0 of the part, pitch in bytes.
+        auto store_part = [&](const uint4* src, uint8_t* dst, int64_t pitch) {
+            __syncwarp();                                   // previous part has been read out
+#pragma unroll
+            for (int u = 0; u < 4; ++u) *reinterpret_cast<uint4*>(stg + lane * kEpiRowBytes + u * 16) = src[u];
+            __syncwarp();
+#pragma unroll
+            for (int it = 0; it < 4; ++it) {
+                const int rr = it * 8 + (lane >> 2), ch = lane & 3;
+                const uint4 v = *reinterpret_cast<const uint4*>(stg + rr * kEpiRowBytes + ch * 16);
+                *reinterpret_cast<uint4*>(dst + rr * pitch + ch * 16) = v;
+            }
+        };
+        // hi (and lo) FP16 images of out[0..63] * mul: rows prow.., columns col.. of planes with row pitch op.nb.
+        // Returns the largest |image value| of this lane (range check of the inverse's planes).
+        auto store_images = [&](const float (&out)[64], float mul, __half* hi_plane, __half* lo_plane, int64_t prow, int col) {
+            float big = 0.0f;
+#pragma unroll
+            for (int part = 0; part < 4; ++part) {             // (columns 0-31 hi, lo, columns 32-63 hi, lo)
+                const int jj = part >> 1;
+                const bool is_lo = part & 1;
+                if (is_lo && lo_plane == nullptr) continue;
+                __align__(16) __half hv[32];
+#pragma unroll
+                for (int e = 0; e < 32; ++e) {
+                    const float x = out[jj * 32 + e] * mul;
+                    const __half h = __float2half_rn(x);
+                    hv[e] = is_lo ? __float2half_rn(x - __half2float(h)) : h;
+                    if (!is_lo) big = fmaxf(big, fabsf(x));
+                }
+                __half* plane = is_lo ? lo_plane : hi_plane;
+                store_part(reinterpret_cast<const uint4*>(hv), reinterpret_cast<uint8_t*>(plane + prow * op.nb + col + jj * 32),
+                           static_cast<int64_t>(op.nb) * 2);
+            }
+            return big;
+        };
         while (next_item<CG>(op, iter, unit0, nunits, w)) {
             const int rb = w.rb + rank, cb0u = w.cb;
             if (w.mode == MODE_POTRF) {
@@ -552,7 +657,8 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
                 esync();                                              // every warp's stores of the previous item are done
                 float* tri_sm = reinterpret_cast<float*>(smem_raw + (smem_base - ptx::smem_u32(smem_raw)));
                 potrf128_body<kEpiWarps * 32>(tri_sm, static_cast<int>(threadIdx.x) - 64, esync, op.W, op.nb, rb * kBlk, w.c * kBlk,
-                                              op.linv_hi, op.linv_lo, op.linv_scale_w, op.info, op.col_base + w.c * kBlk);
+                                              op.linv_hi, op.linv_lo, op.linv_scale_w, op.info, op.col_base + w.c * kBlk,
+                                              op.Sh, op.Sl, op.srow_m, op.srow_mt, op.scl);
                 __threadfence();
                 ptx::fence_proxy_async_global();
                 esync();
@@ -610,15 +716,18 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
 #pragma unroll
                 for (int e = 0; e < 64; ++e) bs[e] = 0.0f;
             }
-            // exact power-of-two rescaling: accumulator -> value domain, value -> plane domain
-            const float plane_mul = (w.mode == MODE_P3) ? op.scl[0] : op.scl[1];
             float out[64];
             if (has_acc) {
                 if (j2 == 0) ptx::mbar_wait(tfull_bar(buf), acc_phase);
                 ptx::tc_fence_after();
+                // exact power-of-two rescaling of the accumulator into the value domain, sign included (out = bs - acc * acc_mul).
                 // (read after the accumulator is complete: in MODE_DIAG the scale of the inverted block is written by
                 // another CTA of this launch, and the MMAs could not have run before it was)
-                const float acc_mul = (w.mode == MODE_P3) ? -op.scl[3] / __ldcg(op.linv_scale + w.c) : op.scl[2];
+                float acc_mul;
+                if (w.mode == MODE_P3) acc_mul = -op.scl[SCL_INV_SS] / __ldcg(op.linv_scale + w.c);
+                else if (w.mode == MODE_TRSM) acc_mul = -op.scl[SCL_INV_SS_SM];
+                else if (w.mode == MODE_INV) acc_mul = (w.o_var == 0) ? -op.scl[SCL_INV_SM_SX] : op.scl[SCL_INV_SM_SU];
+                else acc_mul = op.scl[SCL_INV_SX2];
                 uint32_t a0[32], a1[32];
                 const uint32_t taddr = tmem_base + buf * kAccW + (static_cast<uint32_t>(q * 32) << 16) + kAccCols * j2 + 64 * hf;
                 ptx::tmem_ld_32x32(taddr, a0);
@@ -642,43 +751,64 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
                 for (int e = 0; e < 64; ++e) out[e] = bs[e];
             }
             if (dead) continue;
+            if (w.mode == MODE_INV) {
+                // a block of U^T (scale su) or of M / M^T (scale sm) into the scratch planes; a value beyond the FP16 range
+                // means the diagonal tile is too ill-conditioned for the product form of the TRSM: info = -2
+                const float mul = op.scl[w.o_var == 0 ? SCL_SU : SCL_SM];
+                const float big = store_images(out, mul, op.Sh, op.Sl, static_cast<int64_t>(w.o_row) + q * 32, w.o_col + 64 * hf);
+                if (!(big < 60000.0f)) atomicCAS(op.info, 0, -2);
+            } else if (w.mode == MODE_TRSM) {
+                // X = S inv(L_kk)^T is final: round once into the tile's storage precision and store it (R4; PAPER.md:206
+                // "on-the-fly" conversion): FP32 / FP16 tiles straight into the mosaic with their operand images; FP8 tiles
+                // need the tile's amax first, so they leave FP32 values in W and finalize_kernel rounds them
+                const int i = op.k + (rb * kBlk) / op.nb;
+                const int p = op.map[i * op.NT + op.k];
+                const int r_tile = (rb * kBlk) % op.nb + q * 32;                            // this warp's row 0 inside the tile
+                const int64_t prow = op.prow0 + static_cast<int64_t>(rb) * kBlk + q * 32;   // ... and in the planes
+                uint8_t* tile = op.factor + op.off[i * op.NT + op.k];
+                if (p == KRR_FP32) {
 #pragma unroll
-            for (int e = 0; e < 64; ++e) wblk[e * kBlk] = out[e];
-            float amax = 0.0f;
-            if (item_planes) {
-                const int64_t prow = op.prow0 + static_cast<int64_t>(rb) * kBlk + q * 32;      // plane row of this warp's row 0
+                    for (int part = 0; part < 4; ++part)
+                        store_part(reinterpret_cast<const uint4*>(out + 16 * part),
+                                   tile + (static_cast<int64_t>(r_tile) * op.nb + col0 + 16 * part) * 4, static_cast<int64_t>(op.nb) * 4);
+                    store_images(out, op.scl[SCL_SX], op.Hp, op.Lp, prow, col0);
+                } else if (p == KRR_FP16) {
+                    float rd[64];
 #pragma unroll
-                for (int part = 0; part < 4; ++part) {             // (chunk 0 hi, chunk 0 lo, chunk 1 hi, chunk 1 lo)
-                    const int jj = part >> 1;
-                    const bool is_lo = part & 1;
-                    __align__(16) __half hv[32];
+                    for (int part = 0; part < 2; ++part) {
+                        __align__(16) __half hv[32];
 #pragma unroll
-                    for (int e = 0; e < 32; ++e) {
-                        const float x = out[jj * 32 + e] * plane_mul;
-                        const __half h = __float2half_rn(x);
-                        hv[e] = is_lo ? __float2half_rn(x - __half2float(h)) : h;
-                        if (!is_lo) amax = fmaxf(amax, fabsf(out[jj * 32 + e]));
+                        for (int e = 0; e < 32; ++e) {
+                            hv[e] = __float2half_rn(out[32 * part + e]);
+                            rd[32 * part + e] = __half2float(hv[e]);
+                        }
+                        store_part(reinterpret_cast<const uint4*>(hv), tile + (static_cast<int64_t>(r_tile) * op.nb + col0 + 32 * part) * 2,
+                                   static_cast<int64_t>(op.nb) * 2);
                     }
-                    __syncwarp();                                   // previous part has been read out
+                    store_images(rd, op.scl[SCL_SX], op.Hp, nullptr, prow, col0);      // image of the STORED value (exact)
+                } else {
+                    float amax = 0.0f;
 #pragma unroll
-                    for (int u = 0; u < 4; ++u)
-                        *reinterpret_cast<uint4*>(stg + lane * kEpiRowBytes + u * 16) = *reinterpret_cast<const uint4*>(hv + 8 * u);
-                    __syncwarp();
-                    __half* plane = is_lo ? op.Lp : op.Hp;
+                    for (int e = 0; e < 64; ++e) { wblk[e * kBlk] = out[e]; amax = fmaxf(amax, fabsf(out[e])); }
 #pragma unroll
-                    for (int it = 0; it < 4; ++it) {
-                        const int rr = it * 8 + (lane >> 2), ch = lane & 3;
-                        const uint4 v = *reinterpret_cast<const uint4*>(stg + rr * kEpiRowBytes + ch * 16);
-                        *reinterpret_cast<uint4*>(plane + (prow + rr) * op.nb + col0 + jj * 32 + ch * 8) = v;
+                    for (int o = 16; o > 0; o >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, o));
+                    if (lane == 0) {
+                        const int64_t slot = op.prow0 / op.nb + (static_cast<int64_t>(rb) * kBlk) / op.nb;
+                        atomicMax(reinterpret_cast<int*>(op.tile_amax + slot), __float_as_int(amax));
                     }
                 }
-            }
-            if (w.mode == MODE_P3 && op.tile_amax != nullptr) {
+            } else {
+                // S of the rows below the diagonal tile goes to the scratch planes only (the TRSM product reads it
+                // there); everything else keeps its FP32 value in W
+                const bool below = (w.mode == MODE_UPDATE) && (rb >= nsub);
+                if (!(below && item_planes)) {
 #pragma unroll
-                for (int o = 16; o > 0; o >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, o));
-                if (lane == 0) {
-                    const int64_t slot = op.prow0 / op.nb + (static_cast<int64_t>(rb) * kBlk) / op.nb;
-                    atomicMax(reinterpret_cast<int*>(op.tile_amax + slot), __float_as_int(amax));
+                    for (int e = 0; e < 64; ++e) wblk[e * kBlk] = out[e];
+                }
+                if (item_planes) {
+                    const float mul = op.scl[w.mode == MODE_P3 ? SCL_SX : SCL_SS];
+                    if (below) store_images(out, mul, op.Sh, op.Sl, static_cast<int64_t>(rb) * kBlk + q * 32, col0);
+                    else store_images(out, mul, op.Hp, op.Lp, op.prow0 + static_cast<int64_t>(rb) * kBlk + q * 32, col0);
                 }
             }
           }   // j2
@@ -691,15 +821,15 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
                     if (atomicAdd_block(split_ctr, 1) == kEpiWarps - 1) { __threadfence(); atomicAdd(op.split_flags + w.fidx, 1); }
                 }
             }
-            if (op.mode == MODE_PANEL || op.mode == MODE_DIAG) {
-                // publish this item's operand images to the TMA loads of a later item of this CTA (and, in
-                // MODE_DIAG, of the other CTAs: the last warp to finish advances the CTA's progress counter)
+            if (op.mode == MODE_DIAG) {
+                // publish this item's operand images to the TMA loads of a later item of this CTA and of the other
+                // CTAs: the last warp to finish advances the CTA's progress counter
                 __threadfence();
                 ptx::fence_proxy_async_global();
                 __syncwarp();
                 if (lane == 0) {
                     const int old = atomicAdd_block(const_cast<int*>(item_ctr + (eseq & 7)), 1);
-                    if (op.mode == MODE_DIAG && old == item_complete_count(eseq) - 1) {
+                    if (old == item_complete_count(eseq) - 1) {
                         __threadfence();
                         *const_cast<volatile int*>(op.prog + (rb - op.rb0)) = eseq + 1;
                     }

@@ -10,7 +10,11 @@
 namespace krr {
 
 // Global power-of-two scales of the FP16 operand images from the largest diagonal entry of A
-// (|L_ij| <= sqrt(A_ii), |S_ij| <= max A_ii):  scl = {sx, ss, 1/sx^2, 1/ss}.  One CTA.
+// (|L_ij| <= sqrt(A_ii), |S_ij| <= max A_ii) and the exact rescalings of the accumulators (common.cuh SCL_*).
+// With 2^(ex-1) <= sqrt(max A_ii) < 2^ex:  sx = 2^(14-ex) lifts L into the top FP16 binades; M = inv(L_kk) has
+// entries of the order 2^-ex and no a-priori bound, so its images get the scale sm = 2^(4+ex): room for entries
+// 2^12 times the natural size (|sm M| < 65504; beyond that krr_potrf_mp reports info = -2), 22 significant bits for
+// entries down to 2^-7 of it and an absolute resolution of 2^-29 of it below; su likewise for U = L21 M11.  One CTA.
 __global__ void __launch_bounds__(1024)
 plane_scale_kernel(AView A, int64_t n, float* __restrict__ scl) {
     __shared__ float s_red[1024];
@@ -27,19 +31,32 @@ plane_scale_kernel(AView A, int64_t n, float* __restrict__ scl) {
     }
     if (threadIdx.x == 0) {
         const float dmax = s_red[0];
-        float sx = 1.0f, ss = 1.0f;
+        float sx = 1.0f, ss = 1.0f, sm = 16.0f;
         if (dmax > 0.0f && dmax < 3.0e38f) {
             int e;
             frexpf(sqrtf(dmax), &e);
             sx = ldexpf(1.0f, 14 - e);
+            sm = ldexpf(1.0f, 4 + e);
             frexpf(dmax, &e);
             ss = ldexpf(1.0f, 14 - e);
         }
-        scl[0] = sx;
-        scl[1] = ss;
-        scl[2] = (1.0f / sx) * (1.0f / sx);
-        scl[3] = 1.0f / ss;
+        const float su = 16.0f;
+        scl[SCL_SX] = sx;
+        scl[SCL_SS] = ss;
+        scl[SCL_INV_SX2] = (1.0f / sx) * (1.0f / sx);
+        scl[SCL_INV_SS] = 1.0f / ss;
+        scl[SCL_SM] = sm;
+        scl[SCL_SU] = su;
+        scl[SCL_INV_SM_SX] = (1.0f / sm) * (1.0f / sx);
+        scl[SCL_INV_SM_SU] = (1.0f / sm) * (1.0f / su);
+        scl[SCL_INV_SS_SM] = (1.0f / ss) * (1.0f / sm);
     }
+}
+
+// d_scales of the mosaic: 1 for the lower tiles (finalize_kernel overwrites the FP8 tiles'), 0 above the diagonal.
+__global__ void scales_init_kernel(int NT, float* __restrict__ scales) {
+    const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx < NT * NT) scales[idx] = (idx % NT <= idx / NT) ? 1.0f : 0.0f;
 }
 
 // FNV-1a over the lower entries of a map in column-major tile order: the host (h_map) and the device (d_map) side of
@@ -92,18 +109,20 @@ tile_amax_kernel(AView A, const uint8_t* __restrict__ map, float* __restrict__ a
 }
 
 // Round tiles (k + i0 + blockIdx.y, k) of tile column k (FP32 in W, block-column-major 128x128 blocks)
-// into the mosaic.  grid = (nsub*nsub*4, number of tiles), 256 threads: one CTA transposes 32 rows of one 128x128 block through
+// into the mosaic.  With only_fp8 the tiles of the other precisions are left alone: the TRSM product has stored
+// them already (gemm_tc.cuh MODE_TRSM); FP8 tiles wait for their amax and are rounded here.  grid = (nsub*nsub*4, number of tiles), 256 threads: one CTA transposes 32 rows of one 128x128 block through
 // shared memory (coalesced reads of W columns, coalesced row-major writes of the factor / images).
 __global__ void __launch_bounds__(256)
 finalize_kernel(int NT, int nb, int k, int i0, const float* __restrict__ W, const uint8_t* __restrict__ map,
                 const int64_t* __restrict__ off, const float* __restrict__ tile_amax /* per slot */,
                 uint8_t* __restrict__ factor, float* __restrict__ scales, __half* __restrict__ Hp,
-                uint8_t* __restrict__ Qp, const float* __restrict__ scl) {
+                uint8_t* __restrict__ Qp, const float* __restrict__ scl, int only_fp8) {
     __shared__ float tile[32][kBlk + 1];
-    const float sx = scl[0];
+    const float sx = scl[SCL_SX];
     const int nsub = nb / kBlk;
     const int i = k + i0 + blockIdx.y;
     const int p = map[i * NT + k];
+    if (only_fp8 && p != KRR_FP8_E4M3) return;
     const int64_t slot = tile_slot(NT, i, k);
     const float s = (p == KRR_FP8_E4M3) ? fp8_scale_from_amax(tile_amax[slot]) : 1.0f;
     if (blockIdx.x == 0 && threadIdx.x == 0) scales[i * NT + k] = s;

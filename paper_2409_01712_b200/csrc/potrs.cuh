@@ -6,10 +6,9 @@
 //
 // Structure (right-looking over tile columns, like the paper's tile algorithm):
 //   trtri128_kernel (tri128.cuh)   inverses of the 128x128 diagonal blocks of every diagonal tile, once
-//   potrs_diag_transpose_kernel    transposed copies of the diagonal tiles for the backward sweep, once
-//   potrs_diag_kernel              one diagonal tile: 128-row blocks in order, each a product with the
-//                                  already solved part of the tile followed by a product with the
-//                                  inverted diagonal block
+//   potrs_tile_inverse_kernel      from them the inverses of the whole diagonal tiles (and their transposes), once
+//   potrs_diagmul_kernel           one diagonal tile: z_k = inv(L_kk) t_k (forward) or inv(L_kk)^T t_k (backward)
+//                                  as ONE product -- no chain of dependent 128-row block solves
 //   potrs_fwd_update_kernel        Y_i -= L_ik Z_k for all i > k   (streams tile column k once)
 //   potrs_bwd_update_kernel        Z_j -= L_kj^T alpha_k for all j < k (streams tile row k once)
 // All sums are accumulated in a fixed order: results are deterministic.
@@ -301,147 +300,152 @@ potrs_bwd_update_kernel(int NT, int nb, int k, int j_lo, const uint8_t* __restri
 }
 
 // ---------------------------------------------------------------------------------------------
-// Transposed copies of the diagonal tiles (FP32, full squares): T[k] = L_kk^T, so that the backward solve reads
-// rows of L^T exactly as the forward solve reads rows of L.  One CTA per 32 x 32 block with row block <= column
-// block of L^T (the rest is never read).  Once per krr_potrs call: 2 * 4 * nb^2 / 2 bytes per tile.
-__global__ void __launch_bounds__(256)
-potrs_diag_transpose_kernel(const uint8_t* __restrict__ factor, const int64_t* __restrict__ off, int NT, int nb,
-                            float* __restrict__ T) {
-    __shared__ float t[32][33];
-    const int k = blockIdx.z, bi = blockIdx.y, bj = blockIdx.x;        // block (bi, bj) of L^T = block (bj, bi) of L
-    if (bi > bj) return;
+// Inverse of the diagonal tiles in FP32, once per krr_potrs call: Minv[k] = inv(L_kk) and MinvT[k] = its transpose
+// (nb x nb row-major each).  With them a diagonal step of either sweep is ONE product, z_k = inv(L_kk) t_k, instead
+// of a chain of nb/128 dependent block solves.  CTA (c, k) produces block column c of Minv[k] by forward
+// substitution over the 128-blocks with the inverted diagonal blocks D_r of trtri128_kernel:
+//     X_c = D_c,   X_r = -D_r (sum_{j = c}^{r-1} L_rj X_j)   for r > c,
+// every term a 128 x 128 x 128 FP32 product out of shared memory (8 x 8 outputs per thread, fixed summation order).
+constexpr int kTinvThreads = 256;
+constexpr int kTinvLd = kBlk + 4;
+constexpr int kTinvSmem = (2 * 16 * kTinvLd + kBlk * kTinvLd) * 4;       // A chunk, B chunk, T
+
+// acc += A B for 128 x 128 blocks: A row-major (global or shared, leading dimension lda), B row-major (ldb).
+__device__ __forceinline__ void tinv_block_mma(const float* __restrict__ A, int64_t lda, const float* __restrict__ B, int64_t ldb,
+                                               float* As, float* Bs, float (&acc)[8][8], int tid) {
+    const int ty = tid >> 4, tx = tid & 15;
+    for (int k0 = 0; k0 < kBlk; k0 += 16) {
+        {
+            const int row = tid >> 1, kk = (tid & 1) * 8;
+            const float4 v0 = *reinterpret_cast<const float4*>(A + row * lda + k0 + kk);
+            const float4 v1 = *reinterpret_cast<const float4*>(A + row * lda + k0 + kk + 4);
+            As[(kk + 0) * kTinvLd + row] = v0.x; As[(kk + 1) * kTinvLd + row] = v0.y;
+            As[(kk + 2) * kTinvLd + row] = v0.z; As[(kk + 3) * kTinvLd + row] = v0.w;
+            As[(kk + 4) * kTinvLd + row] = v1.x; As[(kk + 5) * kTinvLd + row] = v1.y;
+            As[(kk + 6) * kTinvLd + row] = v1.z; As[(kk + 7) * kTinvLd + row] = v1.w;
+            const int kr = tid >> 4, nn = (tid & 15) * 8;
+            *reinterpret_cast<float4*>(Bs + kr * kTinvLd + nn) = *reinterpret_cast<const float4*>(B + kr * ldb + nn + k0 * ldb);
+            *reinterpret_cast<float4*>(Bs + kr * kTinvLd + nn + 4) = *reinterpret_cast<const float4*>(B + kr * ldb + nn + 4 + k0 * ldb);
+        }
+        __syncthreads();
+#pragma unroll
+        for (int kk = 0; kk < 16; ++kk) {
+            const float4 a0 = *reinterpret_cast<const float4*>(As + kk * kTinvLd + ty * 8);
+            const float4 a1 = *reinterpret_cast<const float4*>(As + kk * kTinvLd + ty * 8 + 4);
+            const float4 b0 = *reinterpret_cast<const float4*>(Bs + kk * kTinvLd + tx * 8);
+            const float4 b1 = *reinterpret_cast<const float4*>(Bs + kk * kTinvLd + tx * 8 + 4);
+            const float av[8] = {a0.x, a0.y, a0.z, a0.w, a1.x, a1.y, a1.z, a1.w};
+            const float bv[8] = {b0.x, b0.y, b0.z, b0.w, b1.x, b1.y, b1.z, b1.w};
+#pragma unroll
+            for (int i = 0; i < 8; ++i)
+#pragma unroll
+                for (int j = 0; j < 8; ++j) acc[i][j] = fmaf(av[i], bv[j], acc[i][j]);
+        }
+        __syncthreads();
+    }
+}
+
+// grid = (nsub, NT).  dinv: the inverted 128 x 128 diagonal blocks ([n/128][128][128], trtri128_kernel).
+__global__ void __launch_bounds__(kTinvThreads, 2)
+potrs_tile_inverse_kernel(const uint8_t* __restrict__ factor, const int64_t* __restrict__ off, int NT, int nb,
+                          const float* __restrict__ dinv, float* __restrict__ Minv, float* __restrict__ MinvT) {
+    extern __shared__ __align__(16) float tinv_sm[];
+    float* As = tinv_sm;
+    float* Bs = As + 16 * kTinvLd;
+    float* Ts = Bs + 16 * kTinvLd;                                    // [128][kTinvLd]
+    const int nsub = nb / kBlk;
+    const int c = nsub - 1 - static_cast<int>(blockIdx.x);            // the long block columns are scheduled first
+    const int k = blockIdx.y;
+    const int tid = threadIdx.x, ty = tid >> 4, tx = tid & 15;
     const float* L = reinterpret_cast<const float*>(factor + off[static_cast<int64_t>(k) * NT + k]);
-    float* Tk = T + static_cast<int64_t>(k) * nb * nb;
-    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+    float* M = Minv + static_cast<int64_t>(k) * nb * nb;
+    float* MT = MinvT + static_cast<int64_t>(k) * nb * nb;
+    const float* D = dinv + static_cast<int64_t>(k) * nsub * kBlk * kBlk;
+    auto store_block = [&](int r, const float (&x)[8][8]) {           // X_r into M[r-block rows][c-block columns] and transposed
 #pragma unroll
-    for (int r = ty; r < 32; r += 8) t[r][tx] = L[static_cast<int64_t>(bj * 32 + r) * nb + bi * 32 + tx];
-    __syncthreads();
+        for (int i = 0; i < 8; ++i) {
+            float* dst = M + static_cast<int64_t>(r * kBlk + ty * 8 + i) * nb + c * kBlk + tx * 8;
+            *reinterpret_cast<float4*>(dst) = make_float4(x[i][0], x[i][1], x[i][2], x[i][3]);
+            *reinterpret_cast<float4*>(dst + 4) = make_float4(x[i][4], x[i][5], x[i][6], x[i][7]);
+        }
 #pragma unroll
-    for (int r = ty; r < 32; r += 8) Tk[static_cast<int64_t>(bi * 32 + r) * nb + bj * 32 + tx] = t[tx][r];
+        for (int j = 0; j < 8; ++j) {
+            float* dst = MT + static_cast<int64_t>(c * kBlk + tx * 8 + j) * nb + r * kBlk + ty * 8;
+            *reinterpret_cast<float4*>(dst) = make_float4(x[0][j], x[1][j], x[2][j], x[3][j]);
+            *reinterpret_cast<float4*>(dst + 4) = make_float4(x[4][j], x[5][j], x[6][j], x[7][j]);
+        }
+    };
+    {
+        float x[8][8];
+        const float* Dc = D + static_cast<int64_t>(c) * kBlk * kBlk;
+#pragma unroll
+        for (int i = 0; i < 8; ++i)
+#pragma unroll
+            for (int j = 0; j < 8; ++j) x[i][j] = Dc[(ty * 8 + i) * kBlk + tx * 8 + j];
+        store_block(c, x);
+    }
+    for (int r = c + 1; r < nsub; ++r) {
+        __syncthreads();                                              // X_c .. X_{r-1} are in global memory (this CTA wrote them)
+        float acc[8][8];
+#pragma unroll
+        for (int i = 0; i < 8; ++i)
+#pragma unroll
+            for (int j = 0; j < 8; ++j) acc[i][j] = 0.0f;
+        for (int j = c; j < r; ++j)
+            tinv_block_mma(L + static_cast<int64_t>(r) * kBlk * nb + j * kBlk, nb, M + static_cast<int64_t>(j) * kBlk * nb + c * kBlk, nb,
+                           As, Bs, acc, tid);
+#pragma unroll
+        for (int i = 0; i < 8; ++i)
+#pragma unroll
+            for (int j = 0; j < 8; ++j) Ts[(ty * 8 + i) * kTinvLd + tx * 8 + j] = -acc[i][j];
+        __syncthreads();
+#pragma unroll
+        for (int i = 0; i < 8; ++i)
+#pragma unroll
+            for (int j = 0; j < 8; ++j) acc[i][j] = 0.0f;
+        tinv_block_mma(D + static_cast<int64_t>(r) * kBlk * kBlk, kBlk, Ts, kTinvLd, As, Bs, acc, tid);
+        store_block(r, acc);
+    }
 }
 
-// Diagonal tile solve by one thread-block cluster of kDiagCluster CTAs: forward (L z = y) or
-// backward (L^T a = z), in place on rows k*nb .. (k+1)*nb of B.  For each 128-row block c, in order:
-//   forward   t = y_c - L[c, 0:c] z_{0:c}                       z_c = inv(L_cc) t
-//   backward  t = z_c - (L^T)[c, c+1:] a_{c+1:}                 a_c = inv(L_cc)^T t
-// M: the diagonal tile L_kk (forward) or its transposed copy (backward; potrs_diag_transpose_kernel), so both
-// directions run the same code: rows of M against the solved values, the K range split over warp slices.
-// dinv / dinvT: the inverted diagonal blocks of this tile and their transposes ([nsub][128][128]).
-// Every CTA keeps a full copy of the solved values and of t in its shared memory; the rows of a step are split
-// over the CTAs, and the pieces are exchanged through distributed shared memory between two cluster barriers.
-// smem per CTA: solved values NRHS*nb floats + t NRHS*128 + exchange buffer (see potrs_diag_smem_floats).
-template <int NRHS>
-__host__ __device__ constexpr int potrs_diag_smem_floats(int nb) {
-    // solved + ts + red (K slices: 8 warps * 64 values)
-    return NRHS * nb + NRHS * kBlk + 4 * 32 * 64;
-}
-
+// Diagonal step of a sweep as one product, in place on rows k*nb .. (k+1)*nb of B:
+//     forward   z_k = inv(L_kk) t_k      (Mk = Minv[k],  lower triangular: row block b meets columns [0, 128 (b+1)))
+//     backward  a_k = inv(L_kk)^T t_k    (Mk = MinvT[k], upper triangular: row block b meets columns [128 b, nb))
+// One thread-block cluster of kDiagCluster CTAs: every CTA stages all of t_k in shared memory, a cluster barrier makes
+// sure everyone has read it before anyone overwrites it, then the row groups (64 / NRHS rows per warp) are dealt to
+// the warps of the cluster.  Sums in a fixed order: deterministic.
 template <int NRHS>
 __global__ void __cluster_dims__(kDiagCluster, 1, 1) __launch_bounds__(kDiagThreads, 1)
-potrs_diag_kernel(int nb, const float* __restrict__ Lkk /* M */, const float* __restrict__ dinv,
-                  const float* __restrict__ dinvT, float* __restrict__ Bk, int64_t ldb, int nrhs, int backward) {
+potrs_diagmul_kernel(int nb, const float* __restrict__ Mk, float* __restrict__ Bk, int64_t ldb, int nrhs, int backward) {
     namespace cg = cooperative_groups;
     cg::cluster_group cluster = cg::this_cluster();
-    constexpr int ROWS = 64 / NRHS;                    // rows per warp task
-    constexpr int NW = kDiagThreads / 32;              // 8 warps
-    constexpr int GQ = (kBlk / ROWS) / kDiagCluster;   // row groups per CTA: 1, 2, 4, 8 for NRHS 4, 8, 16, 32
-    constexpr int KS = NW / GQ;                        // K slices per row group
-    static_assert(GQ >= 1 && KS >= 1 && GQ * KS == NW, "warp decomposition");
-    extern __shared__ __align__(16) float sm[];
-    float* zs = sm;                                    // [NRHS][nb] solved values, by rhs
-    float* ts = sm + static_cast<size_t>(NRHS) * nb;   // [NRHS][128]
-    float* red = ts + NRHS * kBlk;                     // [4][32][64] scratch
+    constexpr int ROWS = 64 / NRHS;
+    constexpr int NW = kDiagThreads / 32;
+    extern __shared__ __align__(16) float ts[];                    // [NRHS][nb]
+    for (int idx = threadIdx.x; idx < nb * NRHS; idx += kDiagThreads) {
+        const int r = idx / NRHS, rh = idx % NRHS;
+        ts[rh * nb + r] = (rh < nrhs) ? Bk[static_cast<int64_t>(r) * ldb + rh] : 0.0f;
+    }
+    cluster.sync();
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int q = static_cast<int>(cluster.block_rank());
-    const int nsub = nb / kBlk;
-    // pull the part of M that is read and the inverted blocks towards L2 (fire and forget)
-    {
-        const int gt = q * kDiagThreads + threadIdx.x, nt = kDiagCluster * kDiagThreads;
-        for (int c = 0; c < nsub; ++c) {
-            const int col0 = backward ? c * kBlk : 0;                     // block row c: columns 0 .. c (L) or c .. nsub-1 (L^T)
-            const int lines_per_row = backward ? 4 * (nsub - c) : 4 * (c + 1);
-            for (int idx = gt; idx < kBlk * lines_per_row; idx += nt) {
-                const float* ptr = Lkk + static_cast<int64_t>(c * kBlk + idx / lines_per_row) * nb + col0 + (idx % lines_per_row) * 32;
-                asm volatile("prefetch.global.L2 [%0];" ::"l"(ptr));
-            }
-        }
-        const float* D = backward ? dinvT : dinv;
-        for (int idx = gt; idx < nsub * kBlk * 4; idx += nt) asm volatile("prefetch.global.L2 [%0];" ::"l"(D + idx * 32));
-    }
-    cluster.sync();                                    // every CTA is running before its smem is written remotely
-    const int gl = warp % GQ, ks = warp / GQ;          // this warp's row group inside the CTA, K slice
-    const int grow = (q * GQ + gl) * ROWS;             // first row (inside a 128 block) of the warp's group
-    for (int bi = 0; bi < nsub; ++bi) {
-        const int c = backward ? (nsub - 1 - bi) : bi;
-        const int R0 = c * kBlk;
-        const int k_lo = backward ? R0 + kBlk : 0, k_hi = backward ? nb : R0;      // solved range the block row meets
-        // ---- phase 1: t = y_c - M[c, k_lo:k_hi] solved  for this CTA's rows (M = L forward, L^T backward), K split over
-        // the warp slices
+    const int ngroups = nb / ROWS;
+    // (the long rows -- bottom of the lower triangle, top of the upper one -- are spread over all warps: groups interleaved)
+    for (int g = q * NW + warp; g < ngroups; g += kDiagCluster * NW) {
+        const int r0 = g * ROWS;
+        const int blk = r0 / kBlk;
+        const int k_lo = backward ? blk * kBlk : 0, k_hi = backward ? nb : (blk + 1) * kBlk;
         float acc[64];
 #pragma unroll
         for (int v = 0; v < 64; ++v) acc[v] = 0.0f;
-        {
-            const float* rows = Lkk + static_cast<int64_t>(R0 + grow) * nb;
-            for (int l = k_lo + lane * 4 + ks * 128; l < k_hi; l += 128 * KS) {
-                float4 a[ROWS];
-#pragma unroll
-                for (int u = 0; u < ROWS; ++u) a[u] = __ldg(reinterpret_cast<const float4*>(rows + static_cast<int64_t>(u) * nb + l));
-#pragma unroll
-                for (int h = 0; h < NRHS; ++h) {
-                    const float4 z = *reinterpret_cast<const float4*>(zs + h * nb + l);
-#pragma unroll
-                    for (int u = 0; u < ROWS; ++u)
-                        acc[u * NRHS + h] = fmaf(a[u].x, z.x, fmaf(a[u].y, z.y, fmaf(a[u].z, z.z, fmaf(a[u].w, z.w, acc[u * NRHS + h]))));
-                }
-            }
-        }
+        rows_dot_f32<NRHS>(Mk + static_cast<int64_t>(r0) * nb + k_lo, nb, k_hi - k_lo, ts + k_lo, nb, lane, acc);
         warp_reduce64(acc, lane);
-        if (KS > 1) {
-            if (ks > 0) {
-                red[((ks - 1) * GQ + gl) * 64 + lane * 2 + 0] = acc[0];
-                red[((ks - 1) * GQ + gl) * 64 + lane * 2 + 1] = acc[1];
-            }
-            __syncthreads();
+        const int v0 = warp_reduce64_index(lane);
+#pragma unroll
+        for (int t = 0; t < 2; ++t) {
+            const int u = (v0 + t) / NRHS, h = (v0 + t) % NRHS;
+            if (h < nrhs) Bk[static_cast<int64_t>(r0 + u) * ldb + h] = acc[t];
         }
-        if (ks == 0) {
-#pragma unroll
-            for (int s2 = 1; s2 < KS; ++s2) {
-                acc[0] += red[((s2 - 1) * GQ + gl) * 64 + lane * 2 + 0];
-                acc[1] += red[((s2 - 1) * GQ + gl) * 64 + lane * 2 + 1];
-            }
-            const int v0 = warp_reduce64_index(lane);
-#pragma unroll
-            for (int t = 0; t < 2; ++t) {
-                const int u = (v0 + t) / NRHS, h = (v0 + t) % NRHS;
-                const int r = grow + u;
-                const float y = (h < nrhs) ? Bk[static_cast<int64_t>(R0 + r) * ldb + h] : 0.0f;
-                const float tv = y - acc[t];
-#pragma unroll
-                for (int d = 0; d < kDiagCluster; ++d) cluster.map_shared_rank(ts, d)[h * kBlk + r] = tv;
-            }
-        }
-        cluster.sync();
-        // ---- phase 2: solved_c = inv(L_cc) t   (forward)   or   inv(L_cc)^T t   (backward)
-        if (ks == 0) {
-            const float* D = (backward ? dinvT : dinv) + static_cast<int64_t>(c) * kBlk * kBlk;
-            float acc[64];
-#pragma unroll
-            for (int v = 0; v < 64; ++v) acc[v] = 0.0f;
-            rows_dot_f32<NRHS>(D + static_cast<int64_t>(grow) * kBlk, kBlk, kBlk, ts, kBlk, lane, acc);
-            warp_reduce64(acc, lane);
-            const int v0 = warp_reduce64_index(lane);
-#pragma unroll
-            for (int t = 0; t < 2; ++t) {
-                const int u = (v0 + t) / NRHS, h = (v0 + t) % NRHS;
-                const int r = R0 + grow + u;
-#pragma unroll
-                for (int d = 0; d < kDiagCluster; ++d) {
-                    cluster.map_shared_rank(zs, d)[h * nb + r] = acc[t];
-                }
-                if (h < nrhs) Bk[static_cast<int64_t>(r) * ldb + h] = acc[t];
-            }
-        }
-        cluster.sync();
     }
 }
 

@@ -203,7 +203,9 @@ __device__ __forceinline__ void inv128_offdiag(const float* l, float* x, float* 
 
 // W: panel workspace [m][nb] FP32; the block is rows r0..r0+127 (panel-local), columns c0..c0+127.
 // Writes L (lower, zeros above) back into W and inv(L) as scaled FP16 hi/lo planes into
-// linv_hi/lo ([nb][128] row-major, rows c0..c0+127) with their power-of-two scale in linv_scale.
+// linv_hi/lo ([nb][128] row-major, rows c0..c0+127) with their power-of-two scale in linv_scale, and -- the
+// diagonal blocks of M = inv(L_kk) and of its transpose -- into the scratch planes Sh/Sl (row pitch nb) at rows
+// srow_m + c0.. / srow_mt + c0.., columns c0.., with the fixed scale scl[SCL_SM].
 // col_base = 1-based global index of the block's first column, for info (LAPACK convention).
 // The body runs on NTHR threads (tid = 0 .. NTHR-1, whole warps) that synchronise through `sync()`:
 // the stand-alone kernel below uses the whole CTA, the fused diagonal-tile chain of gemm_tc.cuh its
@@ -211,7 +213,9 @@ __device__ __forceinline__ void inv128_offdiag(const float* l, float* x, float* 
 template <int NTHR, typename Sync>
 __device__ __forceinline__ void potrf128_body(float* tri_sm, int tid, Sync sync, float* __restrict__ W, int nb, int r0,
                                               int c0, __half* __restrict__ linv_hi, __half* __restrict__ linv_lo,
-                                              float* __restrict__ linv_scale, int* __restrict__ info, int64_t col_base) {
+                                              float* __restrict__ linv_scale, int* __restrict__ info, int64_t col_base,
+                                              __half* __restrict__ Sh, __half* __restrict__ Sl, int64_t srow_m, int64_t srow_mt,
+                                              const float* __restrict__ scl) {
     float* a = tri_sm;                       // [128][132] : S, then L
     float* x = tri_sm + kBlk * kTriLd;       // [128][132] : inv(L); rows 0..31 x columns 32.. double as scratch
     float* rinv = x + kBlk * kTriLd;         // [128]      : 1 / L_jj
@@ -318,6 +322,32 @@ __device__ __forceinline__ void potrf128_body(float* tri_sm, int tid, Sync sync,
         *reinterpret_cast<uint2*>(linv_hi + static_cast<int64_t>(c0 + r) * kBlk + c4) = *reinterpret_cast<const uint2*>(hi);
         *reinterpret_cast<uint2*>(linv_lo + static_cast<int64_t>(c0 + r) * kBlk + c4) = *reinterpret_cast<const uint2*>(lo);
     }
+    if (Sh != nullptr) {
+        // diagonal block of M (lower) and of M^T (upper) for the product form of the panel TRSM
+        const float sm = scl[SCL_SM];
+        bool over = false;
+        for (int idx = tid; idx < 2 * kBlk * (kBlk / 4); idx += NTHR) {
+            const bool tr = idx >= kBlk * (kBlk / 4);
+            const int id = tr ? idx - kBlk * (kBlk / 4) : idx;
+            const int r = id / (kBlk / 4), c4 = (id % (kBlk / 4)) * 4;
+            __align__(8) __half hi[4];
+            __align__(8) __half lo[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const int c = c4 + u;
+                float xv = 0.0f;
+                if (!tr) { if (c <= r) xv = x[r * kTriLd + c] * sm; }        // M[r][c]
+                else { if (c >= r) xv = x[c * kTriLd + r] * sm; }            // M^T[r][c] = M[c][r]
+                hi[u] = __float2half_rn(xv);
+                lo[u] = __float2half_rn(xv - __half2float(hi[u]));
+                over |= !(fabsf(xv) < 60000.0f);
+            }
+            const int64_t row = (tr ? srow_mt : srow_m) + c0 + r;
+            *reinterpret_cast<uint2*>(Sh + row * nb + c0 + c4) = *reinterpret_cast<const uint2*>(hi);
+            *reinterpret_cast<uint2*>(Sl + row * nb + c0 + c4) = *reinterpret_cast<const uint2*>(lo);
+        }
+        if (over) atomicCAS(info, 0, -2);
+    }
 }
 
 
@@ -326,10 +356,11 @@ struct CtaSync { __device__ __forceinline__ void operator()() const { __syncthre
 __global__ void __launch_bounds__(kTriThreads, 1)
 potrf128_kernel(float* __restrict__ W, int nb, int r0, int c0, __half* __restrict__ linv_hi,
                 __half* __restrict__ linv_lo, float* __restrict__ linv_scale, int* __restrict__ info,
-                int64_t col_base) {
+                int64_t col_base, __half* __restrict__ Sh, __half* __restrict__ Sl, int64_t srow_m, int64_t srow_mt,
+                const float* __restrict__ scl) {
     extern __shared__ __align__(16) float tri_sm[];
     potrf128_body<kTriThreads>(tri_sm, static_cast<int>(threadIdx.x), CtaSync(), W, nb, r0, c0, linv_hi, linv_lo, linv_scale,
-                               info, col_base);
+                               info, col_base, Sh, Sl, srow_m, srow_mt, scl);
 }
 
 // Inverse of the stored 128x128 diagonal blocks of L for krr_potrs: block b = blockIdx.x is rows and

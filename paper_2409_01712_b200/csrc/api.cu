@@ -282,35 +282,12 @@ static int launch_gemm(const GemmMaps& m, const GemmOp& op_in, int max_ctas, int
     return cudaGetLastError() == cudaSuccess ? KRR_OK : KRR_ERR_CUDA;
 }
 
-// Levels of the binary splitting of the diagonal tile's nsub 128-blocks for the inverse M = inv(L_kk) (gemm_tc.cuh
-// MODE_INV): levels[h - 1] holds the nodes of height h (their halves are complete once the lower levels are done);
-// the root is alone in the last level.
-static void inverse_levels(int nsub, std::vector<InvNodes>* levels) {
-    levels->clear();
-    struct Rec {
-        static int go(int o, int len, std::vector<InvNodes>* lv) {
-            if (len <= 1) return 0;
-            int hl = 1;
-            while (2 * hl < len) hl *= 2;                        // largest power of two below len (len / 2 for powers of two)
-            const int hr = len - hl;
-            const int hL = go(o, hl, lv), hR = go(o + hl, hr, lv);
-            const int h = 1 + (hL > hR ? hL : hR);
-            if (static_cast<int>(lv->size()) < h) { InvNodes z; memset(&z, 0, sizeof(z)); lv->resize(h, z); }
-            InvNodes& L = (*lv)[h - 1];
-            L.o[L.count] = o; L.hl[L.count] = hl; L.hr[L.count] = hr; ++L.count;
-            return h;
-        }
-    };
-    Rec::go(0, nsub, levels);
-}
-
 template <int NRHS>
 static int set_potrs_attrs() {
     const int big = 220 * 1024;
     KRR_CUDA_CHECK(cudaFuncSetAttribute(potrs_fwd_update_kernel<NRHS>, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
     KRR_CUDA_CHECK(cudaFuncSetAttribute(potrs_bwd_update_kernel<NRHS, (NRHS <= 16) ? 4 : 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
     KRR_CUDA_CHECK(cudaFuncSetAttribute(potrs_bwd_update_kernel<NRHS, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
-    KRR_CUDA_CHECK(cudaFuncSetAttribute(potrs_diagmul_kernel<NRHS>, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
     return KRR_OK;
 }
 
@@ -444,13 +421,15 @@ int krr_graph_destroy(krr_graph_t* graph) {
 // critical stream, O(k) done, N(k) done on the bulk stream, P(k) + F(k) done on the panel stream}; -1 = not recorded.
 int krr_profile_timeline(int NT, float* h_ms) {
     if (NT < 1 || !h_ms) return KRR_ERR_ARG;
-    if (g_pipe.ev.size() < 4 + 5 * static_cast<size_t>(NT)) return KRR_ERR_ARG;      // no such call yet
+    if (NT < 3 || g_pipe.ev.size() < 4 + 5 * static_cast<size_t>(NT - 1)) return KRR_ERR_ARG;      // no such call yet
     if (cudaEventSynchronize(g_pipe.ev[1]) != cudaSuccess || cudaEventSynchronize(g_pipe.ev[3]) != cudaSuccess)
         return KRR_ERR_CUDA;
     for (int k = 0; k < NT; ++k)
         for (int e = 0; e < 4; ++e) {
             float ms = -1.0f;
-            if (cudaEventElapsedTime(&ms, g_pipe.ev[0], g_pipe.ev[4 + 5 * k + e]) != cudaSuccess) {
+            const size_t idx = 4 + 5 * static_cast<size_t>(k) + e;
+            if (idx >= g_pipe.ev.size()) { h_ms[4 * k + e] = ms; continue; }         // (the last column records nothing)
+            if (cudaEventElapsedTime(&ms, g_pipe.ev[0], g_pipe.ev[idx]) != cudaSuccess) {
                 ms = -1.0f;
                 cudaGetLastError();
             }
@@ -625,11 +604,9 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
     const int cg = ((flags & KRR_FLAG_NO_CTA_PAIRS) || nb % (2 * kBlk) != 0) ? 1 : 2;
 
     const int nsub = nb / kBlk;
-    std::vector<InvNodes> inv_levels;
-    inverse_levels(nsub, &inv_levels);
     const bool lookahead = !(flags & KRR_FLAG_NO_LOOKAHEAD) && NT > 2;
     float* Wbuf[2] = {W, reinterpret_cast<float*>(ws + L.W2)};
-    cudaStream_t sh = st, sl = st;               // critical-path stream, bulk stream
+    cudaStream_t sh = st, sl = st, sv = st;      // critical-path stream, bulk stream, inverse stream
     enum { EV_FORK = 0, EV_JOIN_HI = 1, EV_JOIN_MID = 2, EV_JOIN_LO = 3, EV_BASE = 4, EV_PER_COL = 5 };
     auto ev_first = [&](int k) { return g_pipe.event(EV_BASE + EV_PER_COL * static_cast<size_t>(k) + 0); };
     auto ev_old = [&](int k) { return g_pipe.event(EV_BASE + EV_PER_COL * static_cast<size_t>(k) + 1); };
@@ -639,11 +616,36 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
     if (lookahead) {
         rc = g_pipe.init();
         if (rc) return rc;
-        sh = g_pipe.hi; sl = g_pipe.lo;
+        sh = g_pipe.hi; sl = g_pipe.lo; sv = g_pipe.mid;
         KRR_CUDA_CHECK(cudaEventRecord(g_pipe.event(EV_FORK), st));
         KRR_CUDA_CHECK(cudaStreamWaitEvent(sh, g_pipe.event(EV_FORK), 0));
         KRR_CUDA_CHECK(cudaStreamWaitEvent(sl, g_pipe.event(EV_FORK), 0));
+        KRR_CUDA_CHECK(cudaStreamWaitEvent(sv, g_pipe.event(EV_FORK), 0));
     }
+    // events of the inverse stream: one per 128-block of the diagonal tile (re-recorded every column; a wait is always
+    // enqueued right after its record) and one for the finished inverse
+    auto ev_blk = [&](int c) { return g_pipe.event(EV_BASE + EV_PER_COL * static_cast<size_t>(NT) + c); };
+    auto ev_inv = [&]() { return g_pipe.event(EV_BASE + EV_PER_COL * static_cast<size_t>(NT) + nsub); };
+    // M = inv(L_kk) row block by row block (gemm_tc.cuh MODE_INV with the node: left blocks [0, r), right block r): as soon
+    // as the chain has factored 128-block r, row r of M follows from the rows above it -- two launches, which run on the
+    // inverse stream beside the chain's next sub-columns; only the last row block's two launches come after the chain
+    auto inverse_row = [&](GemmOp op, int r, int lb, cudaStream_t s) -> int {
+        op.mode = MODE_INV; op.c = 0; op.cb0 = 0; op.ncb = 1; op.rb0 = 0; op.nrb = 1;
+        memset(&op.nodes, 0, sizeof(op.nodes));
+        op.nodes.count = 1; op.nodes.o[0] = 0; op.nodes.hl[0] = r; op.nodes.hr[0] = 1;
+        op.inv_last = (r == nsub - 1) ? 1 : 0;
+        for (int step = 0; step < 2; ++step) {
+            op.inv_step = step;
+            const int e = launch_gemm(tm, op, num_sms, 1, s, lb);
+            if (e) return e;
+        }
+        return static_cast<int>(KRR_OK);
+    };
+    auto inverse_export = [&](const GemmOp& op, int c, int lb, cudaStream_t s) -> int {
+        return launch(CAT_POTRF, inv_export_kernel, dim3(16), dim3(256), 0, s, static_cast<const __half*>(linv_hi + lb * linv_elems),
+                      static_cast<const __half*>(linv_lo + lb * linv_elems), static_cast<const float*>(linv_scale + lb * nsub), nb,
+                      c * kBlk, Sh, Sl, op.srow_m, op.srow_mt, static_cast<const float*>(scl), d_info);
+    };
     // bulk kernels leave a few SMs to the diagonal-tile chain they overlap with
     const int reserve = nsub < 8 ? nsub : 8;
     const int bulk_ctas = lookahead ? (num_sms - reserve > reserve ? num_sms - reserve : num_sms) : num_sms;
@@ -733,9 +735,20 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
             }
             rc = launch(CAT_POTRF, potrf128_kernel, dim3(1), dim3(kTriThreads), static_cast<size_t>(kTriSmem), sh, Wk, nb,
                         c * kBlk, c * kBlk, linv_hi + lb * linv_elems, linv_lo + lb * linv_elems, linv_scale + lb * nsub, d_info,
-                        static_cast<int64_t>(k) * nb + static_cast<int64_t>(c) * kBlk + 1, Sh, Sl, op.srow_m, op.srow_mt,
-                        static_cast<const float*>(scl));
+                        static_cast<int64_t>(k) * nb + static_cast<int64_t>(c) * kBlk + 1);
             if (rc) return rc;
+            if (k + 1 < NT) {                         // row block c of M, beside the rest of the chain
+                if (lookahead) {
+                    KRR_CUDA_CHECK(cudaEventRecord(ev_blk(c), sh));
+                    KRR_CUDA_CHECK(cudaStreamWaitEvent(sv, ev_blk(c), 0));
+                }
+                rc = inverse_export(op, c, lb, sv);
+                if (rc) return rc;
+                if (c >= 1) {
+                    rc = inverse_row(op, c, lb, sv);
+                    if (rc) return rc;
+                }
+            }
             op.mode = MODE_P3; op.c = c; op.cb0 = c; op.ncb = 1; op.rb0 = c + 1; op.nrb = nsub - c - 1;
             if (op.nrb > 0) {
                 rc = launch_gemm(tm, op, num_sms, 1, sh, lb);
@@ -745,16 +758,18 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
         rc = finalize(k, Wk, 0, 1, 0, sh);
         if (rc) return rc;
         if (k + 1 == NT) continue;                    // the last column has no panel below
-        // ---- M = inv(L_kk) by binary splitting of the 128-blocks (their inverses are in place): two launches per level ----
-        op.mode = MODE_INV; op.c = 0; op.cb0 = 0; op.ncb = 1; op.rb0 = 0; op.nrb = 1;
-        for (size_t lv = 0; lv < inv_levels.size(); ++lv) {
-            op.nodes = inv_levels[lv];
-            op.inv_last = (lv + 1 == inv_levels.size()) ? 1 : 0;
-            for (int step = 0; step < 2; ++step) {
-                op.inv_step = step;
-                rc = launch_gemm(tm, op, num_sms, 1, sh, lb);
+        if (fused_chain)                              // (one launch for the whole chain: the rows of M follow it)
+            for (int r = 0; r < nsub; ++r) {
+                rc = inverse_export(op, r, lb, sh);
                 if (rc) return rc;
+                if (r >= 1) {
+                    rc = inverse_row(op, r, lb, sh);
+                    if (rc) return rc;
+                }
             }
+        else if (lookahead) {
+            KRR_CUDA_CHECK(cudaEventRecord(ev_inv(), sv));
+            KRR_CUDA_CHECK(cudaStreamWaitEvent(sh, ev_inv(), 0));
         }
         // ---- panel below: X = S M^T as one triangular product, rounded once and stored (MODE_TRSM) ----
         op.mode = MODE_TRSM; op.c = 0; op.cb0 = 0; op.ncb = nsub;
@@ -791,8 +806,10 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
     if (lookahead) {
         KRR_CUDA_CHECK(cudaEventRecord(g_pipe.event(EV_JOIN_HI), sh));
         KRR_CUDA_CHECK(cudaEventRecord(g_pipe.event(EV_JOIN_LO), sl));
+        KRR_CUDA_CHECK(cudaEventRecord(g_pipe.event(EV_JOIN_MID), sv));
         KRR_CUDA_CHECK(cudaStreamWaitEvent(st, g_pipe.event(EV_JOIN_HI), 0));
         KRR_CUDA_CHECK(cudaStreamWaitEvent(st, g_pipe.event(EV_JOIN_LO), 0));
+        KRR_CUDA_CHECK(cudaStreamWaitEvent(st, g_pipe.event(EV_JOIN_MID), 0));
     }
     return rc_columns;
 }
@@ -800,7 +817,7 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
 // ------------------------------------------------------------------------- solve
 static int rhs_class(int nrhs) { return nrhs <= 4 ? 4 : (nrhs <= 8 ? 8 : (nrhs <= 16 ? 16 : 32)); }
 
-struct PotrsWs { size_t off_table, dinv, dinvT, Minv, MinvT, total; };
+struct PotrsWs { size_t off_table, dinv, dinvT, Minv, MinvT, stage, total; };
 static PotrsWs potrs_ws_layout(int64_t n, int nb) {
     const size_t NT = n / nb;
     PotrsWs w;
@@ -810,6 +827,7 @@ static PotrsWs potrs_ws_layout(int64_t n, int nb) {
     w.dinvT = o;     o = align_up(o + static_cast<size_t>(n) * kBlk * sizeof(float), 1024);
     w.Minv = o;      o = align_up(o + static_cast<size_t>(n) * nb * sizeof(float), 1024);     // inv(L_kk), every k
     w.MinvT = o;     o = align_up(o + static_cast<size_t>(n) * nb * sizeof(float), 1024);     // inv(L_kk)^T for the backward sweep
+    w.stage = o;     o = align_up(o + static_cast<size_t>(nb) * kMaxRhs * sizeof(float), 1024);  // t_k of the diagonal step
     w.total = o;
     return w;
 }
@@ -829,7 +847,7 @@ size_t krr_potrs_workspace(int64_t n, int nb, int nrhs) {
 // update of row k+2 by column k+1 waits for the bulk update by column k.
 template <int NRHS>
 static int potrs_run(const uint8_t* factor, const float* d_scales, const uint8_t* d_map, const std::vector<int64_t>& hoff,
-                     const int64_t* off, const float* Minv, const float* MinvT, int NT, int nb, float* B,
+                     const int64_t* off, const float* Minv, const float* MinvT, float* stage, int NT, int nb, float* B,
                      int64_t ldb, int nrhs, int num_sms, cudaStream_t st) {
     constexpr int ROWS = 64 / NRHS, NW = kSolveThreads / 32, CPL = (NRHS <= 16) ? 4 : 2;
     const size_t smem_z = static_cast<size_t>(NRHS) * nb * sizeof(float);
@@ -853,28 +871,34 @@ static int potrs_run(const uint8_t* factor, const float* d_scales, const uint8_t
     }
     // bulk updates leave room for a diagonal-solve CTA on every SM (1 update CTA + 1 solve CTA fit in shared memory;
     // the update CTAs are persistent, so a solve CTA that does not fit beside them would wait for the whole kernel)
-    const int bulk_per_sm = pipe ? 1 : 3;
+    const int bulk_per_sm = 3;
     auto fwd_update = [&](int k, int i_lo, int i_hi, cudaStream_t s, int per_sm) {
         if (i_hi <= i_lo) return static_cast<int>(KRR_OK);
         const int64_t tasks = static_cast<int64_t>(i_hi - i_lo) * nb / ROWS;
         const int64_t want = (tasks + NW - 1) / NW;
         const int64_t cap = static_cast<int64_t>(per_sm) * num_sms;
         return launch(CAT_POTRS, potrs_fwd_update_kernel<NRHS>, dim3(static_cast<unsigned>(want < cap ? want : cap)), dim3(kSolveThreads),
-                      smem_z, s, NT, nb, k, i_lo, i_hi, factor, off, d_map, d_scales, B, ldb, nrhs);
+                      smem_z + static_cast<size_t>(i_hi - i_lo) * 16, s, NT, nb, k, i_lo, i_hi,
+                      factor, off, d_map, d_scales, B, ldb, nrhs);
     };
     auto bwd_update = [&](int k, int j_lo, int j_hi, cudaStream_t s) {
         if (j_hi <= j_lo) return static_cast<int>(KRR_OK);
         if (pipe && j_hi - j_lo == 1)            // the tile the next diagonal solve waits for: one column per lane, 4 x the CTAs
             return launch(CAT_POTRS, potrs_bwd_update_kernel<NRHS, 1>, dim3(nb / 32), dim3(kSolveThreads), smem_b1, s,
-                          NT, nb, k, j_lo, factor, off, d_map, d_scales, B, ldb, nrhs);
-        return launch(CAT_POTRS, potrs_bwd_update_kernel<NRHS, CPL>, dim3((j_hi - j_lo) * (nb / (32 * CPL))), dim3(kSolveThreads), smem_bu, s,
-                      NT, nb, k, j_lo, factor, off, d_map, d_scales, B, ldb, nrhs);
+                          NT, nb, k, j_lo, 1, factor, off, d_map, d_scales, B, ldb, nrhs);
+        const int units = (j_hi - j_lo) * (nb / (32 * CPL));
+        const int cap = 2 * num_sms;             // two persistent CTAs per SM (shared memory), alpha_k staged once each
+        return launch(CAT_POTRS, potrs_bwd_update_kernel<NRHS, CPL>, dim3(units < cap ? units : cap), dim3(kSolveThreads), smem_bu, s,
+                      NT, nb, k, j_lo, j_hi - j_lo, factor, off, d_map, d_scales, B, ldb, nrhs);
     };
     auto diag = [&](int k, int backward, cudaStream_t s) {
         const float* Mk = (backward ? MinvT : Minv) + static_cast<int64_t>(k) * nb * nb;
         float* Bk = B + static_cast<int64_t>(k) * nb * ldb;
-        return launch(CAT_POTRS, potrs_diagmul_kernel<NRHS>, dim3(kDiagCluster), dim3(kDiagThreads), smem_z, s, nb, Mk, Bk, ldb,
-                      nrhs, backward);
+        int e = launch(CAT_POTRS, potrs_stage_kernel<NRHS>, dim3((nb * NRHS + 255) / 256), dim3(256), 0, s, nb,
+                       static_cast<const float*>(Bk), ldb, nrhs, stage);
+        if (e) return e;
+        return launch(CAT_POTRS, potrs_diagmul_kernel<NRHS>, dim3(nb / ROWS), dim3(kDiagThreads), 0, s, nb, Mk,
+                      static_cast<const float*>(stage), Bk, ldb, nrhs, backward);
     };
     // (a lambda: an error in the middle still joins the internal streams below)
     auto run_sweeps = [&]() -> int {
@@ -960,6 +984,7 @@ int krr_potrs(const void* d_factor, const float* d_scales, const uint8_t* d_map,
     float* dinvT = reinterpret_cast<float*>(ws + L.dinvT);
     float* Minv = reinterpret_cast<float*>(ws + L.Minv);
     float* MinvT = reinterpret_cast<float*>(ws + L.MinvT);
+    float* stage = reinterpret_cast<float*>(ws + L.stage);
     rc = launch(CAT_MISC, offsets_kernel, dim3(1), dim3(32), 0, st, NT, nb, d_map, off, host_map_hash(NT, h_map), static_cast<int*>(nullptr));
     if (rc) return rc;
     const uint8_t* factor = static_cast<const uint8_t*>(d_factor);
@@ -970,10 +995,10 @@ int krr_potrs(const void* d_factor, const float* d_scales, const uint8_t* d_map,
                 factor, static_cast<const int64_t*>(off), NT, nb, static_cast<const float*>(dinv), Minv, MinvT);
     if (rc) return rc;
     switch (rhs_class(nrhs)) {
-        case 4:  return potrs_run<4>(factor, d_scales, d_map, hoff, off, Minv, MinvT, NT, nb, d_B, ldb, nrhs, num_sms, st);
-        case 8:  return potrs_run<8>(factor, d_scales, d_map, hoff, off, Minv, MinvT, NT, nb, d_B, ldb, nrhs, num_sms, st);
-        case 16: return potrs_run<16>(factor, d_scales, d_map, hoff, off, Minv, MinvT, NT, nb, d_B, ldb, nrhs, num_sms, st);
-        default: return potrs_run<32>(factor, d_scales, d_map, hoff, off, Minv, MinvT, NT, nb, d_B, ldb, nrhs, num_sms, st);
+        case 4:  return potrs_run<4>(factor, d_scales, d_map, hoff, off, Minv, MinvT, stage, NT, nb, d_B, ldb, nrhs, num_sms, st);
+        case 8:  return potrs_run<8>(factor, d_scales, d_map, hoff, off, Minv, MinvT, stage, NT, nb, d_B, ldb, nrhs, num_sms, st);
+        case 16: return potrs_run<16>(factor, d_scales, d_map, hoff, off, Minv, MinvT, stage, NT, nb, d_B, ldb, nrhs, num_sms, st);
+        default: return potrs_run<32>(factor, d_scales, d_map, hoff, off, Minv, MinvT, stage, NT, nb, d_B, ldb, nrhs, num_sms, st);
     }
 }
 

@@ -108,7 +108,8 @@ constexpr int kPlaneBytes = kBlk * kBlockK * 2;    // one 128 x 64 fp16 (or 128 
 constexpr int kSlotBytes = 2 * kPlaneBytes;        // one plane of A and one of B.  A K chunk takes one slot
                                                    // (hi images / E4M3 images) or two (hi, then lo images)
 constexpr int kAccCols = 128;                      // TMEM columns of one 128x128 FP32 accumulator
-constexpr int kMaxAccBufs = 2;
+constexpr int kMaxAccBufs = 4;                     // CG = 1: four 128-column accumulators; CG = 2: two of 256 columns
+constexpr int kSegChunks = 2;                      // MODE_TRSM / MODE_INV: K chunks (of 64) per accumulation segment
 constexpr int kSfCol0 = 256;                       // first TMEM column of the scale table
 constexpr int kSfCols = 256;                       // table: 256 / (4 CG) entries of 4 CG columns
 constexpr int kTmemCols = 512;                     // accumulators + scale table
@@ -234,16 +235,40 @@ struct WorkItem {
     int fidx;        // index into op.split_flags
     TermGeom g;      // MODE_INV: operand geometry of the block
     int o_row, o_col, o_var;   // MODE_INV: scratch row / column of the output block; 0 = U^T, 1 = M21, 2 = M21^T
+    // MODE_TRSM / MODE_INV (CG = 1): the K range of a block is accumulated in segments of kSegChunks chunks, each in its
+    // own TMEM accumulator, and the segments are added in FP32 (round to nearest) by the epilogue -- see the note on
+    // segmented accumulation below.  ch_lo / ch_hi: the item's K chunks (-1: the whole range); first / last segment flags.
+    int ch_lo, ch_hi, seg_first, seg_last;
 };
 struct ItemIter {
     int t;           // block modes: next block index
-    int g, it, m;    // MODE_DIAG: item inside the chain
+    int g, it, m;    // MODE_DIAG: item inside the chain; segmented modes: it = segments of block t already emitted
 };
+
+// Segmented accumulation.  The tensor core adds every MMA's result to the TMEM accumulator with truncation, a bias of
+// about half an ulp OF THE ACCUMULATOR per instruction.  In a trailing update the accumulator stays small until the
+// dominant leading columns arrive last (K is walked downwards).  A product with an explicit inverse, X = S M^T, has no
+// such order: its partial sums are of the size of |S||M| throughout while the result is a small difference (for the
+// first diagonal tile of a kernel matrix 0.5 against 0.02), and a hundred truncations at that size cost a backward
+// error of 1.2e-6 (measured, nb = 512).  So these products start a fresh accumulator every kSegChunks K chunks
+// (24 instructions) and the epilogue adds the segments in FP32 with round to nearest, highest K first.
+__device__ __forceinline__ bool emit_segment(ItemIter& st, int nunits, int kelems, WorkItem& w) {
+    const int nch = kelems / kBlockK;
+    const int nseg = (nch + kSegChunks - 1) / kSegChunks;
+    const int sidx = nseg - 1 - st.it;                 // highest K first
+    w.ch_lo = sidx * kSegChunks;
+    w.ch_hi = (sidx + 1) * kSegChunks < nch ? (sidx + 1) * kSegChunks : nch;
+    w.seg_first = (st.it == 0);
+    w.seg_last = (sidx == 0);
+    if (w.seg_last) { st.it = 0; st.t += nunits; } else { ++st.it; }
+    return true;
+}
 
 template <int CG>
 __device__ __forceinline__ bool next_item(const GemmOp& op, ItemIter& st, int unit0, int nunits, WorkItem& w) {
     w.xcta = -1; w.xneed = 0;
     w.t_lo = 0; w.t_hi = num_terms(op); w.cpos = 0; w.clen = 1; w.fidx = 0;
+    w.ch_lo = -1; w.ch_hi = -1; w.seg_first = 1; w.seg_last = 1;
     if (op.mode == MODE_DIAG) {
         // CTA r owns row block r of the diagonal tile: P3(0), P1(1), P3(1), ..., P3(r-1), P1(r), POTRF(r).
         // P1(c) reads the rows of block c that CTA c finished with its P3(c-1) (item 2c-2), P3(c) the inverse
@@ -260,9 +285,8 @@ __device__ __forceinline__ bool next_item(const GemmOp& op, ItemIter& st, int un
         return true;
     }
     if (op.mode == MODE_INV) {
-        // blocks of all nodes of the level, node after node
+        // blocks of all nodes of the level, node after node; every block in K segments
         int t = st.t;
-        st.t += nunits;
         for (int nd = 0; nd < op.nodes.count; ++nd) {
             const int hl = op.nodes.hl[nd], hr = op.nodes.hr[nd], o = op.nodes.o[nd];
             const int per = hl * hr;
@@ -290,7 +314,7 @@ __device__ __forceinline__ bool next_item(const GemmOp& op, ItemIter& st, int un
                 w.o_row = static_cast<int>(op.srow_mt) + (o + mb) * kBlk; w.o_col = (o + hl + nbk) * kBlk;
             }
             w.rb = 0; w.cb = 0;
-            return true;
+            return emit_segment(st, nunits, w.g.kelems, w);
         }
         return false;
     }
@@ -314,6 +338,10 @@ __device__ __forceinline__ bool next_item(const GemmOp& op, ItemIter& st, int un
         w.cb = op.cb0 + (t % ncbu) * CG;
         if (tile_is_skipped(op, w.rb + CG - 1, w.cb)) continue;      // the whole (pair) block lies above the diagonal
         w.mode = op.mode; w.c = op.c; w.dep = 0;
+        if (CG == 1 && op.mode == MODE_TRSM) {
+            st.t = t;                                                 // (emit_segment advances to the next block after the last segment)
+            return emit_segment(st, nunits, ((w.cb + 1) * kBlk < op.nb ? (w.cb + 1) * kBlk : op.nb), w);
+        }
         return true;
     }
     return false;
@@ -357,7 +385,10 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
     const int nterms = num_terms(op);
     const bool use_sf = op.fp8q && op.mode == MODE_UPDATE;
     // a pair's 256-column accumulators fill TMEM: with the scale table present there is room for one only
-    const int nbufs = (CG == 2 && use_sf) ? 1 : kMaxAccBufs;
+    // MODE_TRSM on pairs keeps the small cross terms (lo * hi, hi * lo) in the second accumulator: the main one then
+    // sees a third of the truncating additions (see the note on segmented accumulation), and the epilogue adds the two
+    const bool split_cross = (CG == 2) && op.mode == MODE_TRSM;
+    const int nbufs = (CG == 2) ? ((use_sf || split_cross) ? 1 : 2) : (use_sf ? 2 : 4);
 
     const bool has_acc = (op.mode != MODE_UPDATE) ? (op.mode != MODE_P1 || op.c > 0) : (nterms > 0);
     const bool write_planes = (op.mode != MODE_UPDATE) || op.planes;
@@ -466,7 +497,8 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
                     const CUtensorMap* mB_hi = (g.b_src == 2) ? &tmSH : ((g.b_src == 1) ? &tmIH : &tmH);
                     const CUtensorMap* mB_lo = (g.b_src == 2) ? &tmSL : ((g.b_src == 1) ? &tmIL : &tmL);
                     const uint32_t lo_bytes = CG * ((a_lo ? 1u : 0u) + (b_lo ? 1u : 0u)) * kPlaneBytes;
-                    for (int ch = g.kelems / kBlockK - 1; ch >= 0; --ch) {
+                    const int ch_hi = (w.ch_hi >= 0) ? w.ch_hi : g.kelems / kBlockK, ch_lo = (w.ch_lo >= 0) ? w.ch_lo : 0;
+                    for (int ch = ch_hi - 1; ch >= ch_lo; --ch) {
                         const int ak = g.a_k0 + ch * kBlockK, bk = g.b_k0 + ch * kBlockK;
                         ptx::mbar_wait(empty_bar(slot), phase ^ 1u);
                         if (ptx::elect_one()) {              // hi images
@@ -546,7 +578,8 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
                         continue;
                     }
                     const bool a_lo = cls & kClsALo, b_lo = cls & kClsBLo;
-                    for (int ch = kelems / kBlockK - 1; ch >= 0; --ch) {
+                    const int ch_hi = (w.ch_hi >= 0) ? w.ch_hi : kelems / kBlockK, ch_lo = (w.ch_lo >= 0) ? w.ch_lo : 0;
+                    for (int ch = ch_hi - 1; ch >= ch_lo; --ch) {
                         const int c0 = slot;
                         ptx::mbar_wait(full_bar(c0), phase);
                         if (++slot == kSlots) { slot = 0; phase ^= 1u; }
@@ -560,7 +593,15 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
                             const uint32_t ah = dlo0 + c0 * kDescSlot, bh = ah + kDescB;
                             const uint32_t al = dlo0 + c1 * kDescSlot, bl = al + kDescB;
                             // +32 B (2 descriptor units) per K = 16; small cross terms first, the dominant hi*hi last
-                            if (a_lo && b_lo) {
+                            if (a_lo && b_lo && split_cross) {
+                                const uint32_t d_cross = d_tmem + kAccW;
+#pragma unroll
+                                for (int kk = kBlockK / 16 - 1; kk >= 0; --kk) {
+                                    mma(d_cross, al + 2 * kk, bh + 2 * kk, (kk == 3) ? accumulate : 1u);
+                                    mma(d_cross, ah + 2 * kk, bl + 2 * kk, 1u);
+                                    mma(d_tmem, ah + 2 * kk, bh + 2 * kk, (kk == 3) ? accumulate : 1u);
+                                }
+                            } else if (a_lo && b_lo) {
 #pragma unroll
                                 for (int kk = kBlockK / 16 - 1; kk >= 0; --kk) {
                                     mma(d_tmem, al + 2 * kk, bh + 2 * kk, (kk == 3) ? accumulate : 1u);
@@ -647,6 +688,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
             }
             return big;
         };
+        float out[64];                                               // (lives across the K segments of a block)
         while (next_item<CG>(op, iter, unit0, nunits, w)) {
             const int rb = w.rb + rank, cb0u = w.cb;
             if (w.mode == MODE_POTRF) {
@@ -657,8 +699,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
                 esync();                                              // every warp's stores of the previous item are done
                 float* tri_sm = reinterpret_cast<float*>(smem_raw + (smem_base - ptx::smem_u32(smem_raw)));
                 potrf128_body<kEpiWarps * 32>(tri_sm, static_cast<int>(threadIdx.x) - 64, esync, op.W, op.nb, rb * kBlk, w.c * kBlk,
-                                              op.linv_hi, op.linv_lo, op.linv_scale_w, op.info, op.col_base + w.c * kBlk,
-                                              op.Sh, op.Sl, op.srow_m, op.srow_mt, op.scl);
+                                              op.linv_hi, op.linv_lo, op.linv_scale_w, op.info, op.col_base + w.c * kBlk);
                 __threadfence();
                 ptx::fence_proxy_async_global();
                 esync();
@@ -677,6 +718,17 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
                 __syncwarp();
             }
             const bool item_planes = write_planes && (w.cpos == w.clen - 1);
+            // everything the store needs from global memory is fetched here, before the wait for the accumulator
+            int t_prec = KRR_FP32;
+            uint8_t* t_tile = nullptr;
+            float t_acc_mul = 0.0f, t_sx = 0.0f;
+            if (w.mode == MODE_TRSM) {
+                const int ti = op.k + (rb * kBlk) / op.nb;
+                t_prec = op.map[ti * op.NT + op.k];
+                t_tile = op.factor + op.off[ti * op.NT + op.k];
+                t_acc_mul = -op.scl[SCL_INV_SS_SM];
+                t_sx = op.scl[SCL_SX];
+            }
 #pragma unroll 1
           for (int j2 = 0; j2 < CG; ++j2) {                       // the unit's column blocks, one after the other
             const int cb = cb0u + j2;
@@ -716,7 +768,6 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
 #pragma unroll
                 for (int e = 0; e < 64; ++e) bs[e] = 0.0f;
             }
-            float out[64];
             if (has_acc) {
                 if (j2 == 0) ptx::mbar_wait(tfull_bar(buf), acc_phase);
                 ptx::tc_fence_after();
@@ -725,7 +776,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
                 // another CTA of this launch, and the MMAs could not have run before it was)
                 float acc_mul;
                 if (w.mode == MODE_P3) acc_mul = -op.scl[SCL_INV_SS] / __ldcg(op.linv_scale + w.c);
-                else if (w.mode == MODE_TRSM) acc_mul = -op.scl[SCL_INV_SS_SM];
+                else if (w.mode == MODE_TRSM) acc_mul = t_acc_mul;
                 else if (w.mode == MODE_INV) acc_mul = (w.o_var == 0) ? -op.scl[SCL_INV_SM_SX] : op.scl[SCL_INV_SM_SU];
                 else acc_mul = op.scl[SCL_INV_SX2];
                 uint32_t a0[32], a1[32];
@@ -736,21 +787,43 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
                 ptx::tc_fence_before();
                 __syncwarp();
                 if (j2 == CG - 1) {
-                    if (lane == 0) {                                        // accumulator is in registers
+                    if (lane == 0 && !split_cross) {                        // accumulator is in registers
                         if (CG == 2) ptx::mbar_arrive_leader(tempty_bar(buf)); else ptx::mbar_arrive(tempty_bar(buf));
                     }
                     if (++buf == nbufs) { buf = 0; acc_phase ^= 1u; }
                 }
+                if (split_cross) {
+                    // main + cross accumulators, added in FP32 (round to nearest); the TMEM buffer is released afterwards
+                    uint32_t c0[32], c1[32];
+                    ptx::tmem_ld_32x32(taddr + kAccW, c0);
+                    ptx::tmem_ld_32x32(taddr + kAccW + 32, c1);
+                    ptx::tmem_ld_wait();
 #pragma unroll
-                for (int e = 0; e < 32; ++e) {
-                    out[e] = fmaf(-__uint_as_float(a0[e]), acc_mul, bs[e]);
-                    out[32 + e] = fmaf(-__uint_as_float(a1[e]), acc_mul, bs[32 + e]);
+                    for (int e = 0; e < 32; ++e) {
+                        out[e] = -(__uint_as_float(a0[e]) + __uint_as_float(c0[e])) * acc_mul;
+                        out[32 + e] = -(__uint_as_float(a1[e]) + __uint_as_float(c1[e])) * acc_mul;
+                    }
+                    ptx::tc_fence_before();
+                    __syncwarp();
+                    if (j2 == CG - 1 && lane == 0) ptx::mbar_arrive_leader(tempty_bar(0));
+                } else if (w.seg_first) {
+#pragma unroll
+                    for (int e = 0; e < 32; ++e) {
+                        out[e] = fmaf(-__uint_as_float(a0[e]), acc_mul, bs[e]);
+                        out[32 + e] = fmaf(-__uint_as_float(a1[e]), acc_mul, bs[32 + e]);
+                    }
+                } else {                                                     // a later K segment of the same block
+#pragma unroll
+                    for (int e = 0; e < 32; ++e) {
+                        out[e] = fmaf(-__uint_as_float(a0[e]), acc_mul, out[e]);
+                        out[32 + e] = fmaf(-__uint_as_float(a1[e]), acc_mul, out[32 + e]);
+                    }
                 }
             } else {
 #pragma unroll
                 for (int e = 0; e < 64; ++e) out[e] = bs[e];
             }
-            if (dead) continue;
+            if (dead || !w.seg_last) continue;
             if (w.mode == MODE_INV) {
                 // a block of U^T (scale su) or of M / M^T (scale sm) into the scratch planes; a value beyond the FP16 range
                 // means the diagonal tile is too ill-conditioned for the product form of the TRSM: info = -2
@@ -761,17 +834,16 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
                 // X = S inv(L_kk)^T is final: round once into the tile's storage precision and store it (R4; PAPER.md:206
                 // "on-the-fly" conversion): FP32 / FP16 tiles straight into the mosaic with their operand images; FP8 tiles
                 // need the tile's amax first, so they leave FP32 values in W and finalize_kernel rounds them
-                const int i = op.k + (rb * kBlk) / op.nb;
-                const int p = op.map[i * op.NT + op.k];
+                const int p = t_prec;
                 const int r_tile = (rb * kBlk) % op.nb + q * 32;                            // this warp's row 0 inside the tile
                 const int64_t prow = op.prow0 + static_cast<int64_t>(rb) * kBlk + q * 32;   // ... and in the planes
-                uint8_t* tile = op.factor + op.off[i * op.NT + op.k];
+                uint8_t* tile = t_tile;
                 if (p == KRR_FP32) {
 #pragma unroll
                     for (int part = 0; part < 4; ++part)
                         store_part(reinterpret_cast<const uint4*>(out + 16 * part),
                                    tile + (static_cast<int64_t>(r_tile) * op.nb + col0 + 16 * part) * 4, static_cast<int64_t>(op.nb) * 4);
-                    store_images(out, op.scl[SCL_SX], op.Hp, op.Lp, prow, col0);
+                    store_images(out, t_sx, op.Hp, op.Lp, prow, col0);
                 } else if (p == KRR_FP16) {
                     float rd[64];
 #pragma unroll
@@ -785,7 +857,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
                         store_part(reinterpret_cast<const uint4*>(hv), tile + (static_cast<int64_t>(r_tile) * op.nb + col0 + 32 * part) * 2,
                                    static_cast<int64_t>(op.nb) * 2);
                     }
-                    store_images(rd, op.scl[SCL_SX], op.Hp, nullptr, prow, col0);      // image of the STORED value (exact)
+                    store_images(rd, t_sx, op.Hp, nullptr, prow, col0);      // image of the STORED value (exact)
                 } else {
                     float amax = 0.0f;
 #pragma unroll

@@ -148,7 +148,11 @@ __device__ __forceinline__ void rows_dot_lp(const uint8_t* __restrict__ tile, fl
 
 // ---------------------------------------------------------------------------------------------
 // Forward update after Z_k is known:  Y_i -= L_ik Z_k  for the tile rows i in [i_lo, i_hi)  (all > k).
-// Persistent CTAs over groups of 8 * ROWS rows (ROWS = 64 / NRHS rows per warp); smem = NRHS*nb floats.
+// Persistent CTAs over groups of 8 * ROWS rows (ROWS = 64 / NRHS rows per warp); smem = NRHS*nb floats (Z_k) + the
+// tiles' (offset, precision, scale), fetched once per CTA so that a warp task starts streaming at once.
+// Tried and dropped (r02): streaming the tile through a per-warp cp.async ring in shared memory (16 KB in flight per
+// warp, one CTA per SM): 12.5 -> 13.8 ms for the whole solve at n = 65536 -- the kernel is bound by the shared-memory
+// reads of Z_k (16 LDS.128 per 256 FMAs and warp), not by load latency.
 template <int NRHS>
 __global__ void __launch_bounds__(kSolveThreads)
 potrs_fwd_update_kernel(int NT, int nb, int k, int i_lo, int i_hi, const uint8_t* __restrict__ factor,
@@ -156,22 +160,32 @@ potrs_fwd_update_kernel(int NT, int nb, int k, int i_lo, int i_hi, const uint8_t
                         const float* __restrict__ scales, float* __restrict__ B, int64_t ldb, int nrhs) {
     constexpr int ROWS = 64 / NRHS;
     constexpr int NW = kSolveThreads / 32;
-    extern __shared__ __align__(16) float zs[];        // [NRHS][nb]
+    extern __shared__ __align__(16) float zs[];        // [NRHS][nb], then the tiles' (offset, precision, scale)
+    int64_t* t_off = reinterpret_cast<int64_t*>(zs + static_cast<size_t>(NRHS) * nb);
+    int* t_prec = reinterpret_cast<int*>(t_off + (i_hi - i_lo));
+    float* t_scale = reinterpret_cast<float*>(t_prec + (i_hi - i_lo));
     const float* Zk = B + static_cast<int64_t>(k) * nb * ldb;
     for (int idx = threadIdx.x; idx < nb * NRHS; idx += kSolveThreads) {
         const int c = idx / NRHS, rh = idx % NRHS;
         zs[rh * nb + c] = (rh < nrhs) ? Zk[static_cast<int64_t>(c) * ldb + rh] : 0.0f;
+    }
+    for (int t = threadIdx.x; t < i_hi - i_lo; t += kSolveThreads) {
+        const int i = i_lo + t;
+        t_off[t] = off[i * NT + k];
+        t_prec[t] = map[i * NT + k];
+        t_scale[t] = scales[i * NT + k];
     }
     __syncthreads();
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int64_t ngroups = static_cast<int64_t>(i_hi - i_lo) * nb / ROWS;   // warp tasks
     for (int64_t g = static_cast<int64_t>(blockIdx.x) * NW + warp; g < ngroups; g += static_cast<int64_t>(gridDim.x) * NW) {
         const int64_t prow = g * ROWS;                                      // row below the top of tile i_lo
-        const int i = i_lo + static_cast<int>(prow / nb);
+        const int ti = static_cast<int>(prow / nb);
+        const int i = i_lo + ti;
         const int r0 = static_cast<int>(prow % nb);
-        const int p = map[i * NT + k];
-        const float s = scales[i * NT + k];
-        const uint8_t* tile = factor + off[i * NT + k];
+        const int p = t_prec[ti];
+        const float s = t_scale[ti];
+        const uint8_t* tile = factor + t_off[ti];
         float acc[64];
 #pragma unroll
         for (int v = 0; v < 64; ++v) acc[v] = 0.0f;
@@ -242,7 +256,7 @@ __device__ __forceinline__ void bwd_rows(const uint8_t* __restrict__ tile, float
 // warp) for the single tile on the chain stream that the next diagonal solve waits for.
 template <int NRHS, int CPL>
 __global__ void __launch_bounds__(kSolveThreads)
-potrs_bwd_update_kernel(int NT, int nb, int k, int j_lo, const uint8_t* __restrict__ factor,
+potrs_bwd_update_kernel(int NT, int nb, int k, int j_lo, int ntiles, const uint8_t* __restrict__ factor,
                         const int64_t* __restrict__ off, const uint8_t* __restrict__ map,
                         const float* __restrict__ scales, float* __restrict__ B, int64_t ldb, int nrhs) {
     constexpr int NACC = CPL * NRHS;
@@ -258,43 +272,46 @@ potrs_bwd_update_kernel(int NT, int nb, int k, int j_lo, const uint8_t* __restri
     __syncthreads();
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int strips = nb / STRIP;
-    const int j = j_lo + blockIdx.x / strips;
-    const int c0 = (blockIdx.x % strips) * STRIP + lane * CPL;
-    const int p = map[k * NT + j];
-    const float s = scales[k * NT + j];
-    const uint8_t* tile = factor + off[k * NT + j];
-    float acc[NACC];
+    // units = (tile j, strip of 32 * CPL columns), dealt round-robin to the persistent CTAs (alpha_k is staged once per CTA)
+    for (int unit = blockIdx.x; unit < ntiles * strips; unit += gridDim.x) {
+        const int j = j_lo + unit / strips;
+        const int c0 = (unit % strips) * STRIP + lane * CPL;
+        const int p = map[k * NT + j];
+        const float s = scales[k * NT + j];
+        const uint8_t* tile = factor + off[k * NT + j];
+        float acc[NACC];
 #pragma unroll
-    for (int v = 0; v < NACC; ++v) acc[v] = 0.0f;
-    if (p == KRR_FP32) bwd_rows<NRHS, CPL, KRR_FP32>(tile, s, c0, nb, as, warp, acc);
-    else if (p == KRR_FP16) bwd_rows<NRHS, CPL, KRR_FP16>(tile, s, c0, nb, as, warp, acc);
-    else bwd_rows<NRHS, CPL, KRR_FP8_E4M3>(tile, s, c0, nb, as, warp, acc);
-    // fixed-order tree over the NW warps
+        for (int v = 0; v < NACC; ++v) acc[v] = 0.0f;
+        if (p == KRR_FP32) bwd_rows<NRHS, CPL, KRR_FP32>(tile, s, c0, nb, as, warp, acc);
+        else if (p == KRR_FP16) bwd_rows<NRHS, CPL, KRR_FP16>(tile, s, c0, nb, as, warp, acc);
+        else bwd_rows<NRHS, CPL, KRR_FP8_E4M3>(tile, s, c0, nb, as, warp, acc);
+        // fixed-order tree over the NW warps
 #pragma unroll
-    for (int half = NW / 2; half >= 1; half >>= 1) {
-        if (warp >= half && warp < 2 * half) {
-            float* dst = red + (static_cast<size_t>(warp - half) * 32 + lane) * NACC;
+        for (int half = NW / 2; half >= 1; half >>= 1) {
+            if (warp >= half && warp < 2 * half) {
+                float* dst = red + (static_cast<size_t>(warp - half) * 32 + lane) * NACC;
 #pragma unroll
-            for (int v = 0; v < NACC; v += 4) *reinterpret_cast<float4*>(dst + v) = make_float4(acc[v], acc[v + 1], acc[v + 2], acc[v + 3]);
-        }
-        __syncthreads();
-        if (warp < half) {
-            const float* src = red + (static_cast<size_t>(warp) * 32 + lane) * NACC;
-#pragma unroll
-            for (int v = 0; v < NACC; v += 4) {
-                const float4 t = *reinterpret_cast<const float4*>(src + v);
-                acc[v] += t.x; acc[v + 1] += t.y; acc[v + 2] += t.z; acc[v + 3] += t.w;
+                for (int v = 0; v < NACC; v += 4) *reinterpret_cast<float4*>(dst + v) = make_float4(acc[v], acc[v + 1], acc[v + 2], acc[v + 3]);
             }
+            __syncthreads();
+            if (warp < half) {
+                const float* src = red + (static_cast<size_t>(warp) * 32 + lane) * NACC;
+#pragma unroll
+                for (int v = 0; v < NACC; v += 4) {
+                    const float4 t = *reinterpret_cast<const float4*>(src + v);
+                    acc[v] += t.x; acc[v + 1] += t.y; acc[v + 2] += t.z; acc[v + 3] += t.w;
+                }
+            }
+            __syncthreads();
         }
-        __syncthreads();
-    }
-    if (warp == 0) {
+        if (warp == 0) {
 #pragma unroll
-        for (int c = 0; c < CPL; ++c) {
-            float* z = B + (static_cast<int64_t>(j) * nb + c0 + c) * ldb;
+            for (int c = 0; c < CPL; ++c) {
+                float* z = B + (static_cast<int64_t>(j) * nb + c0 + c) * ldb;
 #pragma unroll
-            for (int h = 0; h < NRHS; ++h)
-                if (h < nrhs) z[h] -= acc[c * NRHS + h];
+                for (int h = 0; h < NRHS; ++h)
+                    if (h < nrhs) z[h] -= acc[c * NRHS + h];
+            }
         }
     }
 }
@@ -408,44 +425,71 @@ potrs_tile_inverse_kernel(const uint8_t* __restrict__ factor, const int64_t* __r
     }
 }
 
-// Diagonal step of a sweep as one product, in place on rows k*nb .. (k+1)*nb of B:
+// Diagonal step of a sweep as one product, rows k*nb .. (k+1)*nb of B:
 //     forward   z_k = inv(L_kk) t_k      (Mk = Minv[k],  lower triangular: row block b meets columns [0, 128 (b+1)))
 //     backward  a_k = inv(L_kk)^T t_k    (Mk = MinvT[k], upper triangular: row block b meets columns [128 b, nb))
-// One thread-block cluster of kDiagCluster CTAs: every CTA stages all of t_k in shared memory, a cluster barrier makes
-// sure everyone has read it before anyone overwrites it, then the row groups (64 / NRHS rows per warp) are dealt to
-// the warps of the cluster.  Sums in a fixed order: deterministic.
+// t_k is first copied out of B into a compact [nb][NRHS] buffer (potrs_stage_kernel), so that the product can write its
+// result over t_k in B while other CTAs still read t_k.  One CTA per group of 64 / NRHS rows; its eight warps split the
+// K range in slices of whole 128-column steps, lane = 4 consecutive columns; the slices are added in a fixed order
+// through shared memory: deterministic.  The launch is short (one DRAM round trip per warp) and wide (nb NRHS / 64 CTAs).
 template <int NRHS>
-__global__ void __cluster_dims__(kDiagCluster, 1, 1) __launch_bounds__(kDiagThreads, 1)
-potrs_diagmul_kernel(int nb, const float* __restrict__ Mk, float* __restrict__ Bk, int64_t ldb, int nrhs, int backward) {
-    namespace cg = cooperative_groups;
-    cg::cluster_group cluster = cg::this_cluster();
+__global__ void __launch_bounds__(256)
+potrs_stage_kernel(int nb, const float* __restrict__ Bk, int64_t ldb, int nrhs, float* __restrict__ T) {
+    const int idx = blockIdx.x * 256 + threadIdx.x;
+    if (idx < nb * NRHS) {
+        const int r = idx / NRHS, h = idx % NRHS;
+        T[idx] = (h < nrhs) ? Bk[static_cast<int64_t>(r) * ldb + h] : 0.0f;
+    }
+}
+
+template <int NRHS>
+__global__ void __launch_bounds__(kDiagThreads)
+potrs_diagmul_kernel(int nb, const float* __restrict__ Mk, const float* __restrict__ T, float* __restrict__ Bk, int64_t ldb,
+                     int nrhs, int backward) {
     constexpr int ROWS = 64 / NRHS;
     constexpr int NW = kDiagThreads / 32;
-    extern __shared__ __align__(16) float ts[];                    // [NRHS][nb]
-    for (int idx = threadIdx.x; idx < nb * NRHS; idx += kDiagThreads) {
-        const int r = idx / NRHS, rh = idx % NRHS;
-        ts[rh * nb + r] = (rh < nrhs) ? Bk[static_cast<int64_t>(r) * ldb + rh] : 0.0f;
-    }
-    cluster.sync();
+    __shared__ float red[NW][64];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int q = static_cast<int>(cluster.block_rank());
-    const int ngroups = nb / ROWS;
-    // (the long rows -- bottom of the lower triangle, top of the upper one -- are spread over all warps: groups interleaved)
-    for (int g = q * NW + warp; g < ngroups; g += kDiagCluster * NW) {
-        const int r0 = g * ROWS;
-        const int blk = r0 / kBlk;
-        const int k_lo = backward ? blk * kBlk : 0, k_hi = backward ? nb : (blk + 1) * kBlk;
-        float acc[64];
+    const int r0 = blockIdx.x * ROWS;
+    const int blk = r0 / kBlk;
+    const int k_lo = backward ? blk * kBlk : 0, k_hi = backward ? nb : (blk + 1) * kBlk;
+    const int steps = (k_hi - k_lo) / kBlk;                        // 128-column steps of the row group
+    float acc[64];
 #pragma unroll
-        for (int v = 0; v < 64; ++v) acc[v] = 0.0f;
-        rows_dot_f32<NRHS>(Mk + static_cast<int64_t>(r0) * nb + k_lo, nb, k_hi - k_lo, ts + k_lo, nb, lane, acc);
-        warp_reduce64(acc, lane);
-        const int v0 = warp_reduce64_index(lane);
+    for (int v = 0; v < 64; ++v) acc[v] = 0.0f;
+    // step s of the range goes to warp s % NW (a fixed assignment)
+    for (int st = warp; st < steps; st += NW) {
+        const int l = k_lo + st * kBlk + lane * 4;
+        float4 a[ROWS];
 #pragma unroll
-        for (int t = 0; t < 2; ++t) {
-            const int u = (v0 + t) / NRHS, h = (v0 + t) % NRHS;
-            if (h < nrhs) Bk[static_cast<int64_t>(r0 + u) * ldb + h] = acc[t];
+        for (int u = 0; u < ROWS; ++u) a[u] = __ldg(reinterpret_cast<const float4*>(Mk + static_cast<int64_t>(r0 + u) * nb + l));
+#pragma unroll
+        for (int kk = 0; kk < 4; ++kk) {
+            float y[NRHS];
+#pragma unroll
+            for (int h = 0; h < NRHS; h += 4) {
+                const float4 v = __ldg(reinterpret_cast<const float4*>(T + static_cast<int64_t>(l + kk) * NRHS + h));
+                y[h] = v.x; y[h + 1] = v.y; y[h + 2] = v.z; y[h + 3] = v.w;
+            }
+#pragma unroll
+            for (int u = 0; u < ROWS; ++u) {
+                const float av = kk == 0 ? a[u].x : (kk == 1 ? a[u].y : (kk == 2 ? a[u].z : a[u].w));
+#pragma unroll
+                for (int h = 0; h < NRHS; ++h) acc[u * NRHS + h] = fmaf(av, y[h], acc[u * NRHS + h]);
+            }
         }
+    }
+    warp_reduce64(acc, lane);
+    const int v0 = warp_reduce64_index(lane);
+    red[warp][v0] = acc[0];
+    red[warp][v0 + 1] = acc[1];
+    __syncthreads();
+    if (threadIdx.x < 64) {
+        float sum = 0.0f;
+#pragma unroll
+        for (int w2 = 0; w2 < NW; ++w2) sum += red[w2][threadIdx.x];
+        const int u = threadIdx.x / NRHS, h = threadIdx.x % NRHS;
+        if (h < nrhs) Bk[static_cast<int64_t>(r0 + u) * ldb + h] = sum;
     }
 }
 

@@ -203,9 +203,7 @@ __device__ __forceinline__ void inv128_offdiag(const float* l, float* x, float* 
 
 // W: panel workspace [m][nb] FP32; the block is rows r0..r0+127 (panel-local), columns c0..c0+127.
 // Writes L (lower, zeros above) back into W and inv(L) as scaled FP16 hi/lo planes into
-// linv_hi/lo ([nb][128] row-major, rows c0..c0+127) with their power-of-two scale in linv_scale, and -- the
-// diagonal blocks of M = inv(L_kk) and of its transpose -- into the scratch planes Sh/Sl (row pitch nb) at rows
-// srow_m + c0.. / srow_mt + c0.., columns c0.., with the fixed scale scl[SCL_SM].
+// linv_hi/lo ([nb][128] row-major, rows c0..c0+127) with their power-of-two scale in linv_scale.
 // col_base = 1-based global index of the block's first column, for info (LAPACK convention).
 // The body runs on NTHR threads (tid = 0 .. NTHR-1, whole warps) that synchronise through `sync()`:
 // the stand-alone kernel below uses the whole CTA, the fused diagonal-tile chain of gemm_tc.cuh its
@@ -213,9 +211,7 @@ __device__ __forceinline__ void inv128_offdiag(const float* l, float* x, float* 
 template <int NTHR, typename Sync>
 __device__ __forceinline__ void potrf128_body(float* tri_sm, int tid, Sync sync, float* __restrict__ W, int nb, int r0,
                                               int c0, __half* __restrict__ linv_hi, __half* __restrict__ linv_lo,
-                                              float* __restrict__ linv_scale, int* __restrict__ info, int64_t col_base,
-                                              __half* __restrict__ Sh, __half* __restrict__ Sl, int64_t srow_m, int64_t srow_mt,
-                                              const float* __restrict__ scl) {
+                                              float* __restrict__ linv_scale, int* __restrict__ info, int64_t col_base) {
     float* a = tri_sm;                       // [128][132] : S, then L
     float* x = tri_sm + kBlk * kTriLd;       // [128][132] : inv(L); rows 0..31 x columns 32.. double as scratch
     float* rinv = x + kBlk * kTriLd;         // [128]      : 1 / L_jj
@@ -322,32 +318,6 @@ __device__ __forceinline__ void potrf128_body(float* tri_sm, int tid, Sync sync,
         *reinterpret_cast<uint2*>(linv_hi + static_cast<int64_t>(c0 + r) * kBlk + c4) = *reinterpret_cast<const uint2*>(hi);
         *reinterpret_cast<uint2*>(linv_lo + static_cast<int64_t>(c0 + r) * kBlk + c4) = *reinterpret_cast<const uint2*>(lo);
     }
-    if (Sh != nullptr) {
-        // diagonal block of M (lower) and of M^T (upper) for the product form of the panel TRSM
-        const float sm = scl[SCL_SM];
-        bool over = false;
-        for (int idx = tid; idx < 2 * kBlk * (kBlk / 4); idx += NTHR) {
-            const bool tr = idx >= kBlk * (kBlk / 4);
-            const int id = tr ? idx - kBlk * (kBlk / 4) : idx;
-            const int r = id / (kBlk / 4), c4 = (id % (kBlk / 4)) * 4;
-            __align__(8) __half hi[4];
-            __align__(8) __half lo[4];
-#pragma unroll
-            for (int u = 0; u < 4; ++u) {
-                const int c = c4 + u;
-                float xv = 0.0f;
-                if (!tr) { if (c <= r) xv = x[r * kTriLd + c] * sm; }        // M[r][c]
-                else { if (c >= r) xv = x[c * kTriLd + r] * sm; }            // M^T[r][c] = M[c][r]
-                hi[u] = __float2half_rn(xv);
-                lo[u] = __float2half_rn(xv - __half2float(hi[u]));
-                over |= !(fabsf(xv) < 60000.0f);
-            }
-            const int64_t row = (tr ? srow_mt : srow_m) + c0 + r;
-            *reinterpret_cast<uint2*>(Sh + row * nb + c0 + c4) = *reinterpret_cast<const uint2*>(hi);
-            *reinterpret_cast<uint2*>(Sl + row * nb + c0 + c4) = *reinterpret_cast<const uint2*>(lo);
-        }
-        if (over) atomicCAS(info, 0, -2);
-    }
 }
 
 
@@ -356,11 +326,47 @@ struct CtaSync { __device__ __forceinline__ void operator()() const { __syncthre
 __global__ void __launch_bounds__(kTriThreads, 1)
 potrf128_kernel(float* __restrict__ W, int nb, int r0, int c0, __half* __restrict__ linv_hi,
                 __half* __restrict__ linv_lo, float* __restrict__ linv_scale, int* __restrict__ info,
-                int64_t col_base, __half* __restrict__ Sh, __half* __restrict__ Sl, int64_t srow_m, int64_t srow_mt,
-                const float* __restrict__ scl) {
+                int64_t col_base) {
     extern __shared__ __align__(16) float tri_sm[];
     potrf128_body<kTriThreads>(tri_sm, static_cast<int>(threadIdx.x), CtaSync(), W, nb, r0, c0, linv_hi, linv_lo, linv_scale,
-                               info, col_base, Sh, Sl, srow_m, srow_mt, scl);
+                               info, col_base);
+}
+
+// The inverted 128-block c0 / 128 of the diagonal tile (linv planes, scale linv_scale[c0 / 128]) as the diagonal block of
+// M = inv(L_kk) and, transposed, of M^T in the scratch planes Sh / Sl (row pitch nb; rows srow_m + c0.. / srow_mt + c0..,
+// columns c0..) with the fixed scale scl[SCL_SM] (panel.cuh).  A power-of-two rescaling of the same 22 bits: exact unless
+// the value leaves the FP16 range, which is reported as info = -2.  Off the critical path (inverse stream).
+// grid = 16 CTAs of 256 threads: CTA b handles rows 8 b .. 8 b + 7.
+__global__ void __launch_bounds__(256)
+inv_export_kernel(const __half* __restrict__ linv_hi, const __half* __restrict__ linv_lo, const float* __restrict__ linv_scale,
+                  int nb, int c0, __half* __restrict__ Sh, __half* __restrict__ Sl, int64_t srow_m, int64_t srow_mt,
+                  const float* __restrict__ scl, int* __restrict__ info) {
+    __shared__ float t[8][kBlk + 1];
+    const float mul = scl[SCL_SM] / linv_scale[c0 / kBlk];
+    const int r0 = blockIdx.x * 8;
+    bool over = false;
+    for (int idx = threadIdx.x; idx < 8 * kBlk; idx += 256) {
+        const int rr = idx >> 7, c = idx & 127;
+        const int64_t e = static_cast<int64_t>(c0 + r0 + rr) * kBlk + c;
+        const float v = (__half2float(linv_hi[e]) + __half2float(linv_lo[e])) * mul;
+        over |= !(fabsf(v) < 60000.0f);
+        t[rr][c] = v;
+        const __half h = __float2half_rn(v);
+        const int64_t o = (srow_m + c0 + r0 + rr) * nb + c0 + c;
+        Sh[o] = h;
+        Sl[o] = __float2half_rn(v - __half2float(h));
+    }
+    __syncthreads();
+    // transposed: rows c0 + c of M^T, columns c0 + r0 .. + 7 (16 bytes per row and plane)
+    for (int idx = threadIdx.x; idx < 8 * kBlk; idx += 256) {
+        const int c = idx >> 3, rr = idx & 7;
+        const float v = t[rr][c];
+        const __half h = __float2half_rn(v);
+        const int64_t o = (srow_mt + c0 + c) * nb + c0 + r0 + rr;
+        Sh[o] = h;
+        Sl[o] = __float2half_rn(v - __half2float(h));
+    }
+    if (over) atomicCAS(info, 0, -2);
 }
 
 // Inverse of the stored 128x128 diagonal blocks of L for krr_potrs: block b = blockIdx.x is rows and

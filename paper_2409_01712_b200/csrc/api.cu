@@ -122,7 +122,7 @@ static size_t host_offsets(int NT, int nb, const uint8_t* h_map, std::vector<int
 
 // ---- workspace layout of krr_potrf_mp ----------------------------------------------------------
 struct PotrfWs {
-    size_t off_table, a_amax, tile_amax, scl, prog, split, W, W2, linv_hi, linv_lo, Sh, Sl, Hp, Lp, Qp, total;
+    size_t off_table, a_amax, tile_amax, scl, dscale, prog, split, W, W2, linv_hi, linv_lo, Sh, Sl, Hp, Lp, Qp, total;
 };
 // rows of the scratch planes: S of the panel rows, then two sets (tile-column parity) of M, M^T, U
 static inline size_t scratch_rows(int64_t n, int nb) { return static_cast<size_t>(n) + 6 * static_cast<size_t>(nb); }
@@ -136,6 +136,7 @@ static PotrfWs potrf_ws_layout(int64_t n, int nb, bool any_fp8) {
     w.a_amax = o;    o = align_up(o + NT * NT * sizeof(float), 1024);
     w.tile_amax = o; o = align_up(o + nslots * sizeof(float), 1024);
     w.scl = o;       o = align_up(o + (SCL_COUNT + 2 * (nb / kBlk)) * sizeof(float), 1024);
+    w.dscale = o;    o = align_up(o + static_cast<size_t>(NT) * sizeof(float), 1024);        // equilibration of the tile rows
     w.prog = o;      o = align_up(o + static_cast<size_t>(n / kBlk) * sizeof(int), 1024);   // fused-chain progress, per 128-block
     w.split = o;     o = align_up(o + 256 * sizeof(int), 1024);                              // slice counters of split tail blocks
     w.W = o;         o = align_up(o + static_cast<size_t>(n) * nb * sizeof(float), 1024);
@@ -556,6 +557,7 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
     float* W = reinterpret_cast<float*>(ws + L.W);
     float* scl = reinterpret_cast<float*>(ws + L.scl);
     float* linv_scale = scl + SCL_COUNT;
+    float* dscale = reinterpret_cast<float*>(ws + L.dscale);
     __half* linv_hi = reinterpret_cast<__half*>(ws + L.linv_hi);
     __half* linv_lo = reinterpret_cast<__half*>(ws + L.linv_lo);
     __half* Sh = reinterpret_cast<__half*>(ws + L.Sh);
@@ -578,7 +580,7 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
     if (rc) return rc;
     rc = launch(CAT_MISC, offsets_kernel, dim3(1), dim3(32), 0, st, NT, nb, d_map, off, host_map_hash(NT, h_map), d_info);
     if (rc) return rc;
-    rc = launch(CAT_MISC, plane_scale_kernel, dim3(1), dim3(1024), 0, st, A, n, scl);
+    rc = launch(CAT_MISC, equilibrate_kernel, dim3(1), dim3(1024), 0, st, A, n, scl, dscale);
     if (rc) return rc;
     const bool preround = flags & KRR_FLAG_PREROUND_A;
     if (preround && any_fp8) {
@@ -658,7 +660,7 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
         }
         return launch(CAT_FINALIZE, finalize_kernel, dim3(nsub * nsub * 4, count), dim3(256), 0, s, NT, nb, k, i0, Wk, d_map,
                       static_cast<const int64_t*>(off), static_cast<const float*>(tile_amax), static_cast<uint8_t*>(d_factor),
-                      d_scales, Hp, Qp, static_cast<const float*>(scl), only_fp8);
+                      d_scales, Hp, Qp, static_cast<const float*>(scl), static_cast<const float*>(dscale), only_fp8);
     };
 
     // Tile column k.  Critical stream `sh`: newest term on the diagonal tile, the diagonal-tile
@@ -679,7 +681,7 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
         op.prow0 = tile_slot(NT, k, k) * nb;
         op.map = d_map; op.A = A; op.a_amax = (preround && any_fp8) ? a_amax : nullptr;
         op.W = Wk; op.Hp = Hp; op.Lp = Lp; op.tile_amax = tile_amax; op.flags = flags;
-        op.scl = scl; op.linv_scale = linv_scale + lb * nsub;
+        op.scl = scl; op.dscale = dscale; op.linv_scale = linv_scale + lb * nsub;
         op.scales = d_scales; op.fp8q = (any_fp8 && !(flags & KRR_FLAG_FP8_VIA_FP16)) ? 1 : 0;
         op.Sh = Sh; op.Sl = Sl;
         op.srow_m = static_cast<int64_t>(n) + static_cast<int64_t>(lb) * 3 * nb; op.srow_mt = op.srow_m + nb; op.srow_u = op.srow_m + 2 * nb;

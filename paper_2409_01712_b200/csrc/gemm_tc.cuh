@@ -74,7 +74,8 @@ struct GemmOp {
     float* tile_amax;     // per-slot max|X| accumulated by MODE_P3
     const float* scales;  // NT*NT tile scales of the mosaic (FP8 tiles), written by finalize_kernel
     int fp8q;             // MODE_UPDATE: FP8 x FP8 terms may use the E4M3 images (Qp plane exists)
-    const float* scl;     // device float[4]: sx, ss, 1/sx^2, 1/ss  (power-of-two plane scales)
+    const float* scl;     // device: power-of-two plane scales and accumulator rescalings (common.cuh SCL_*)
+    const float* dscale;  // device float[NT]: the equilibration d_I of the tile rows (panel.cuh equilibrate_kernel)
     const float* linv_scale;  // device float[nb/128]: scale of each inverted diagonal block's planes
     unsigned flags;
     // MODE_DIAG (fused diagonal-tile chain): outputs of the in-kernel POTRF of 128-blocks and the cross-CTA progress
@@ -191,9 +192,10 @@ __device__ __forceinline__ uint32_t term_class_load(const GemmOp& op, int mode, 
     const int pa = op.map[i * op.NT + s], pb = op.map[op.k * op.NT + s];
     uint32_t w = (pa == KRR_FP32 ? kClsALo : 0u) | (pb == KRR_FP32 ? kClsBLo : 0u);
     if (op.fp8q && pa == KRR_FP8_E4M3 && pb == KRR_FP8_E4M3) {
-        const float sx = op.scl[0];
-        const int sfa = pow2_exponent_byte(sx * op.scales[i * op.NT + s]) - sf_bias(CG);
-        const int sfb = pow2_exponent_byte(sx * op.scales[op.k * op.NT + s]) - sf_bias(CG);
+        // images are of the equilibrated L~ = d L: value = (sx d s_tile) * code
+        const float sx = op.scl[SCL_SX];
+        const int sfa = pow2_exponent_byte(sx * op.dscale[i] * op.scales[i * op.NT + s]) - sf_bias(CG);
+        const int sfb = pow2_exponent_byte(sx * op.dscale[op.k] * op.scales[op.k * op.NT + s]) - sf_bias(CG);
         if (sfa >= 0 && sfa < sf_entries(CG) && sfb >= 0 && sfb < sf_entries(CG))
             w |= kClsQ | (static_cast<uint32_t>(sfa) << 8) | (static_cast<uint32_t>(sfb) << 16);
     }
@@ -721,13 +723,15 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
             // everything the store needs from global memory is fetched here, before the wait for the accumulator
             int t_prec = KRR_FP32;
             uint8_t* t_tile = nullptr;
-            float t_acc_mul = 0.0f, t_sx = 0.0f;
+            float t_acc_mul = 0.0f, t_sx = 0.0f, t_di = 1.0f, t_inv_di = 1.0f;
             if (w.mode == MODE_TRSM) {
                 const int ti = op.k + (rb * kBlk) / op.nb;
                 t_prec = op.map[ti * op.NT + op.k];
                 t_tile = op.factor + op.off[ti * op.NT + op.k];
                 t_acc_mul = -op.scl[SCL_INV_SS_SM];
                 t_sx = op.scl[SCL_SX];
+                t_di = op.dscale[ti];
+                t_inv_di = 1.0f / t_di;
             }
 #pragma unroll 1
           for (int j2 = 0; j2 < CG; ++j2) {                       // the unit's column blocks, one after the other
@@ -756,13 +760,14 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
                     p = op.map[i * op.NT + op.k];
                     if (p == KRR_FP8_E4M3) sc = fp8_scale_from_amax(op.a_amax[i * op.NT + op.k]);
                 }
+                const float dd = op.dscale[i] * op.dscale[op.k];        // A~ = D A D (rounded first, then scaled: exact)
 #pragma unroll
                 for (int e = 0; e < 64; e += 4) {
                     const float4 v = *reinterpret_cast<const float4*>(arow + e);
-                    bs[e + 0] = round_to_prec(v.x, p, sc);
-                    bs[e + 1] = round_to_prec(v.y, p, sc);
-                    bs[e + 2] = round_to_prec(v.z, p, sc);
-                    bs[e + 3] = round_to_prec(v.w, p, sc);
+                    bs[e + 0] = round_to_prec(v.x, p, sc) * dd;
+                    bs[e + 1] = round_to_prec(v.y, p, sc) * dd;
+                    bs[e + 2] = round_to_prec(v.z, p, sc) * dd;
+                    bs[e + 3] = round_to_prec(v.w, p, sc) * dd;
                 }
             } else {
 #pragma unroll
@@ -838,12 +843,15 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
                 const int r_tile = (rb * kBlk) % op.nb + q * 32;                            // this warp's row 0 inside the tile
                 const int64_t prow = op.prow0 + static_cast<int64_t>(rb) * kBlk + q * 32;   // ... and in the planes
                 uint8_t* tile = t_tile;
+                // (out holds the equilibrated X~ = d_i X: the images are of X~, the stored tile is X = X~ / d_i)
                 if (p == KRR_FP32) {
+                    store_images(out, t_sx, op.Hp, op.Lp, prow, col0);
+#pragma unroll
+                    for (int e = 0; e < 64; ++e) out[e] *= t_inv_di;
 #pragma unroll
                     for (int part = 0; part < 4; ++part)
                         store_part(reinterpret_cast<const uint4*>(out + 16 * part),
                                    tile + (static_cast<int64_t>(r_tile) * op.nb + col0 + 16 * part) * 4, static_cast<int64_t>(op.nb) * 4);
-                    store_images(out, t_sx, op.Hp, op.Lp, prow, col0);
                 } else if (p == KRR_FP16) {
                     float rd[64];
 #pragma unroll
@@ -851,8 +859,8 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
                         __align__(16) __half hv[32];
 #pragma unroll
                         for (int e = 0; e < 32; ++e) {
-                            hv[e] = __float2half_rn(out[32 * part + e]);
-                            rd[32 * part + e] = __half2float(hv[e]);
+                            hv[e] = __float2half_rn(out[32 * part + e] * t_inv_di);
+                            rd[32 * part + e] = __half2float(hv[e]) * t_di;
                         }
                         store_part(reinterpret_cast<const uint4*>(hv), tile + (static_cast<int64_t>(r_tile) * op.nb + col0 + 32 * part) * 2,
                                    static_cast<int64_t>(op.nb) * 2);

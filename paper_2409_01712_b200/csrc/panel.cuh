@@ -9,38 +9,37 @@
 
 namespace krr {
 
-// Global power-of-two scales of the FP16 operand images from the largest diagonal entry of A
-// (|L_ij| <= sqrt(A_ii), |S_ij| <= max A_ii) and the exact rescalings of the accumulators (common.cuh SCL_*).
-// With 2^(ex-1) <= sqrt(max A_ii) < 2^ex:  sx = 2^(14-ex) lifts L into the top FP16 binades; M = inv(L_kk) has
-// entries of the order 2^-ex and no a-priori bound, so its images get the scale sm = 2^(4+ex): room for entries
-// 2^12 times the natural size (|sm M| < 65504; beyond that krr_potrf_mp reports info = -2), 22 significant bits for
-// entries down to 2^-7 of it and an absolute resolution of 2^-29 of it below; su likewise for U = L21 M11.  One CTA.
+// Symmetric power-of-two equilibration by tile rows and the (then constant) scales of the FP16 operand images.
+//   d_I = 2^-e_I  with  2^(e_I - 1) <= sqrt(max_{r in tile row I} A_rr) < 2^(e_I)
+// The factorisation runs on  A~ = D A D  (D = diag(d_I) over the tile rows; the scaling is applied when a tile of A is
+// first read and undone when a tile of L is stored, L = D^-1 L~: exact, powers of two), so that every tile row has
+// max A~_rr in [1/4, 1): |L~_ij| < 1 and |S~_ij| < 1 whatever the scaling of the input, and the 22 significant bits of
+// the hi / lo images are spent on the tile row's own magnitude instead of the largest diagonal entry of the whole
+// matrix.  (Uniform diagonals -- every kernel matrix -- give one d: the same bits as a global scale.)  Image scales:
+// sx = 2^14 for L~ and X~, ss = 2^15 for S~; M~ = inv(L~_kk) has entries of order one and no a-priori bound, so
+// sm = 2^4: room for entries up to 2^12 (beyond that krr_potrf_mp reports info = -2), 22 significant bits down to
+// 2^-7 and an absolute resolution of 2^-29 below; su likewise for U = L~21 M~11.  One CTA.
 __global__ void __launch_bounds__(1024)
-plane_scale_kernel(AView A, int64_t n, float* __restrict__ scl) {
-    __shared__ float s_red[1024];
-    float m = 0.0f;
-    for (int64_t g = threadIdx.x; g < n; g += 1024) {
-        const int t = static_cast<int>(g / A.nb), r = static_cast<int>(g % A.nb);
-        m = fmaxf(m, fabsf(*A.tile_ptr(t, t, r, r)));
-    }
-    s_red[threadIdx.x] = m;
-    __syncthreads();
-    for (int o = 512; o > 0; o >>= 1) {
-        if (threadIdx.x < o) s_red[threadIdx.x] = fmaxf(s_red[threadIdx.x], s_red[threadIdx.x + o]);
-        __syncthreads();
+equilibrate_kernel(AView A, int64_t n, float* __restrict__ scl, float* __restrict__ dscale) {
+    const int NT = A.NT, nb = A.nb;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    for (int t = warp; t < NT; t += 32) {                      // one warp per tile row
+        float m = 0.0f;
+        for (int r = lane; r < nb; r += 32) m = fmaxf(m, fabsf(*A.tile_ptr(t, t, r, r)));
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
+        if (lane == 0) {
+            float d = 1.0f;
+            if (m > 0.0f && m < 3.0e38f) {
+                int e;
+                frexpf(sqrtf(m), &e);                          // sqrt(m) in [2^(e-1), 2^e)
+                d = ldexpf(1.0f, -e);
+            }
+            dscale[t] = d;
+        }
     }
     if (threadIdx.x == 0) {
-        const float dmax = s_red[0];
-        float sx = 1.0f, ss = 1.0f, sm = 16.0f;
-        if (dmax > 0.0f && dmax < 3.0e38f) {
-            int e;
-            frexpf(sqrtf(dmax), &e);
-            sx = ldexpf(1.0f, 14 - e);
-            sm = ldexpf(1.0f, 4 + e);
-            frexpf(dmax, &e);
-            ss = ldexpf(1.0f, 14 - e);
-        }
-        const float su = 16.0f;
+        const float sx = 16384.0f, ss = 32768.0f, sm = 16.0f, su = 16.0f;
         scl[SCL_SX] = sx;
         scl[SCL_SS] = ss;
         scl[SCL_INV_SX2] = (1.0f / sx) * (1.0f / sx);
@@ -51,6 +50,7 @@ plane_scale_kernel(AView A, int64_t n, float* __restrict__ scl) {
         scl[SCL_INV_SM_SU] = (1.0f / sm) * (1.0f / su);
         scl[SCL_INV_SS_SM] = (1.0f / ss) * (1.0f / sm);
     }
+    (void)n;
 }
 
 // d_scales of the mosaic: 1 for the lower tiles (finalize_kernel overwrites the FP8 tiles'), 0 above the diagonal.
@@ -116,7 +116,7 @@ __global__ void __launch_bounds__(256)
 finalize_kernel(int NT, int nb, int k, int i0, const float* __restrict__ W, const uint8_t* __restrict__ map,
                 const int64_t* __restrict__ off, const float* __restrict__ tile_amax /* per slot */,
                 uint8_t* __restrict__ factor, float* __restrict__ scales, __half* __restrict__ Hp,
-                uint8_t* __restrict__ Qp, const float* __restrict__ scl, int only_fp8) {
+                uint8_t* __restrict__ Qp, const float* __restrict__ scl, const float* __restrict__ dscale, int only_fp8) {
     __shared__ float tile[32][kBlk + 1];
     const float sx = scl[SCL_SX];
     const int nsub = nb / kBlk;
@@ -124,7 +124,9 @@ finalize_kernel(int NT, int nb, int k, int i0, const float* __restrict__ W, cons
     const int p = map[i * NT + k];
     if (only_fp8 && p != KRR_FP8_E4M3) return;
     const int64_t slot = tile_slot(NT, i, k);
-    const float s = (p == KRR_FP8_E4M3) ? fp8_scale_from_amax(tile_amax[slot]) : 1.0f;
+    // W and tile_amax hold the equilibrated L~ = d_i L: the stored tile is L (exact power-of-two unscaling)
+    const float di = dscale[i], inv_di = 1.0f / di;
+    const float s = (p == KRR_FP8_E4M3) ? fp8_scale_from_amax(tile_amax[slot] * inv_di) : 1.0f;
     if (blockIdx.x == 0 && threadIdx.x == 0) scales[i * NT + k] = s;
     uint8_t* dst = factor + off[i * NT + k];
     const int blk = blockIdx.x >> 2, qr = blockIdx.x & 3;
@@ -139,7 +141,7 @@ finalize_kernel(int NT, int nb, int k, int i0, const float* __restrict__ W, cons
     for (int idx = threadIdx.x; idx < 32 * (kBlk / 4); idx += 256) {
         const int rr = idx / (kBlk / 4), c4 = (idx % (kBlk / 4)) * 4;
         const int r = rbl * kBlk + 32 * qr + rr, c = cb * kBlk + c4;     // element of the tile
-        float4 v = make_float4(tile[rr][c4], tile[rr][c4 + 1], tile[rr][c4 + 2], tile[rr][c4 + 3]);
+        float4 v = make_float4(tile[rr][c4] * inv_di, tile[rr][c4 + 1] * inv_di, tile[rr][c4 + 2] * inv_di, tile[rr][c4 + 3] * inv_di);
         const int64_t e = static_cast<int64_t>(r) * nb + c;
         if (p == KRR_FP32) {
             if (i == k) {      // diagonal tile: zeros above the diagonal
@@ -155,7 +157,7 @@ finalize_kernel(int NT, int nb, int k, int i0, const float* __restrict__ W, cons
             // operand image of the STORED value (exact: a power-of-two multiple of an FP16 number)
             __align__(8) __half hs[4];
 #pragma unroll
-            for (int u = 0; u < 4; ++u) hs[u] = __float2half_rn(__half2float(h[u]) * sx);
+            for (int u = 0; u < 4; ++u) hs[u] = __float2half_rn(__half2float(h[u]) * di * sx);
             *reinterpret_cast<uint2*>(Hp + (slot * nb + r) * nb + c) = *reinterpret_cast<const uint2*>(hs);
         } else {
             const float inv = 1.0f / s;          // power of two: exact
@@ -164,7 +166,7 @@ finalize_kernel(int NT, int nb, int k, int i0, const float* __restrict__ W, cons
             if (Qp) *reinterpret_cast<uint32_t*>(Qp + (slot * nb + r) * nb + c) = *reinterpret_cast<const uint32_t*>(q);
             __align__(8) __half h[4];
 #pragma unroll
-            for (int u = 0; u < 4; ++u) h[u] = __float2half_rn(e4m3_to_f32(q[u]) * s * sx);
+            for (int u = 0; u < 4; ++u) h[u] = __float2half_rn(e4m3_to_f32(q[u]) * s * di * sx);
             *reinterpret_cast<uint2*>(Hp + (slot * nb + r) * nb + c) = *reinterpret_cast<const uint2*>(h);
         }
     }

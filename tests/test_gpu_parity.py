@@ -414,3 +414,53 @@ def test_associate_host_matches_device_path(krr):
     assert info == 0 and torch.equal(m2, h) and torch.equal(a2, alpha.cpu())
     a3, m3, info3, _ = krr.associate_host(hA, cfg.nb, hY, force_prec=krr.FP32)
     assert info3 == 0 and int((m3[np.tril_indices(cfg.NT)] != 0).sum()) == 0
+
+
+# ------------------------------------------------------------------------------ badly scaled input
+@pytest.mark.parametrize("scaling", ["tile_rows_pow2", "smooth"])
+@pytest.mark.parametrize("prec", [R.FP32, R.FP16])
+def test_diagonally_scaled_matrix(krr, scaling, prec):
+    """A = D A0 D with D spanning 2^-12 .. 2^12 (the dynamic range of the FP32-class path, whose operands reach the
+    tensor cores as FP16 hi / lo images): the tile rows are equilibrated by powers of two on entry ("Dynamic
+    range"), so the factor is as accurate RELATIVE TO EVERY ROW'S OWN SCALE as for the unscaled matrix -- measured in the
+    equilibrated norm ||D^-1 (A - L L^T) D^-1||_F / ||A0||_F, where a global image scale loses the small rows.
+    (All-FP16 map: D spans 2^-4 .. 2^4 only -- beyond that the FP16 STORAGE format itself runs out of range, whatever
+    the arithmetic: entries of A below 6e-8 round to zero and the oracle breaks down as well.)"""
+    cfg = scaled_config(CONFIGS["C1"], nb=256, n=2048, p=1000)
+    A0, Y = make_problem(cfg, device="cuda")
+    n, nb = cfg.n, cfg.nb
+    i = np.arange(n)
+    span = 12.0 if prec == R.FP32 else 4.0
+    if scaling == "tile_rows_pow2":
+        d = 2.0 ** (np.round(2.0 * span * (i // nb) / (cfg.NT - 1)) - span)    # one power of two per tile row
+    else:
+        d = 2.0 ** (2.0 * span * i / (n - 1) - span) * (1.0 + 0.3 * np.sin(i))   # smooth, up to a factor ~ 8 inside a tile
+    An = (d[:, None] * A0.cpu().numpy().astype(np.float64) * d[None, :]).astype(np.float32)
+    An = np.tril(An) + np.tril(An, -1).T
+    A = torch.from_numpy(An).cuda()
+    pmap = oracle_uniform(cfg.NT, prec)
+    F = gpu_factor(krr, A, nb, pmap)
+    assert int(F.info.item()) == 0
+    Lo, _, info = tile_cholesky_emulated(An, nb, pmap)
+    assert info == 0
+    Lg = F.dense().cpu().numpy()
+    dinv = 1.0 / d
+    A64 = An.astype(np.float64)
+    scaled_bwd = lambda L: float(np.linalg.norm(dinv[:, None] * (A64 - L @ L.T) * dinv[None, :]) /
+                                 np.linalg.norm(dinv[:, None] * A64 * dinv[None, :]))
+    bg, bo = scaled_bwd(Lg), scaled_bwd(Lo)
+    lit = relF(dinv[:, None] * Lg, dinv[:, None] * Lo)
+    print(f"scaled {scaling} prec {prec}: equilibrated backward gpu {bg:.3e} oracle {bo:.3e} relF(D^-1 L) {lit:.3e}")
+    if prec == R.FP32:
+        assert bg <= 1e-6 and lit <= 1e-4
+    else:
+        assert bg <= 5e-4 and abs(bg - bo) <= 0.05 * bo
+    # the plain (unscaled-norm) criteria hold as well
+    assert backward_error(An, Lg) <= (1e-6 if prec == R.FP32 else 5e-4)
+    # and the solve with the scaled factor: against the oracle's substitution with the same factor
+    Ys = torch.from_numpy((d[:, None] * Y.cpu().numpy()).astype(np.float32)).cuda()
+    alpha = krr.potrs(F, Ys.clone())
+    torch.cuda.synchronize()
+    ref = potrs_fp64(Lg, Ys.cpu().numpy(), nb)
+    err = np.linalg.norm(d[:, None] * (alpha.cpu().numpy().astype(np.float64) - ref)) / np.linalg.norm(d[:, None] * ref)
+    assert err <= 1e-5

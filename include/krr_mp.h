@@ -438,6 +438,20 @@ int krr_profile_timeline(int NT, float* h_ms);
  *        kind 4: of all three instructions).  Synchronises `stream`. */
 int krr_peak_probe(int kind, int64_t work, float* h_ms, double* h_flops, void* stream);
 
+/* ---------------------------------------------------------------------------------------------
+ * krr_dist_schedule -- the per-rank task and message schedule of the factorisation over `world` GPUs of one NVSwitch
+ * domain (SURVEY 8(e) / 8(f) NEXT-3; PAPER.md:206 overlap of communication and computation, :291-295 strong scaling).
+ * HOST LOGIC ONLY: pure function of (NT, nb, map, world, rank); nothing is launched.  krr_potrf_mp itself runs on one GPU;
+ * this is the partitioning a multi-GPU driver follows and what the world-size-2 gloo test checks.
+ * Tile row i belongs to rank i mod world.  Records of 6 int32 {op, k, root, nrows, bytes_lo, bytes_hi}, in issue order:
+ *   op 1  diagonal-tile chain + inverse of column k (only on its owner)      op 5  broadcast of M_k = inv(L_kk) from owner(k)
+ *   op 2  newest term N(k) on this rank's nrows tile rows below tile (k,k)    op 6  broadcast of tile (k+1,k) from owner(k+1)
+ *   op 3  older terms O(k) of column k (lookahead) on nrows rows              op 7  all-gather of the tiles (i,k), i > k+1
+ *   op 4  TRSM product T(k) and quantising store on nrows rows                      (nrows = tiles this rank contributes)
+ * bytes = what one rank receives, in STORAGE precision (the mosaic is what travels: PAPER.md:192, :206).
+ * h_tasks NULL: only the count is returned.  Returns the number of records, or a KRR_ERR_* code (< 0). */
+int64_t krr_dist_schedule(int NT, int nb, const uint8_t* h_map, int world, int rank, int32_t* h_tasks, int64_t max_tasks);
+
 /* krr_shutdown -- destroy what the library created for the calling host thread on the current device: the three
  * internal priority streams of the lookahead schedule, the pool of CUDA events (pipeline events and the timing
  * events of krr_profile_*).  Everything the thread enqueued must have completed.  The next krr_* call creates them

@@ -28,7 +28,7 @@ EXPORTS = ["krr_version", "krr_built_for_sm", "krr_tile_slot", "krr_precision_ma
            "krr_associate_host_arena", "krr_associate_host", "krr_build_workspace", "krr_build", "krr_build_bordered", "krr_build_rr", "krr_predict_workspace", "krr_predict", "krr_fit_host_arena", "krr_fit_host", "krr_band_map", "krr_build_stats_bytes", "krr_precision_map_from_build",
            "krr_graph_begin", "krr_graph_end", "krr_graph_launch", "krr_graph_kernel_nodes", "krr_graph_destroy",
            "krr_last_launch_count",
-           "krr_profile_enable", "krr_profile_read", "krr_profile_timeline", "krr_peak_probe", "krr_shutdown"]
+           "krr_profile_enable", "krr_profile_read", "krr_profile_timeline", "krr_peak_probe", "krr_shutdown", "krr_dist_schedule"]
 
 
 class KrrError(RuntimeError):
@@ -130,6 +130,8 @@ def lib():
     L.krr_peak_probe.restype = c.c_int
     L.krr_peak_probe.argtypes = [c.c_int, i64, c.POINTER(c.c_float), c.POINTER(c.c_double), vp]
     L.krr_shutdown.restype = c.c_int
+    L.krr_dist_schedule.restype = i64
+    L.krr_dist_schedule.argtypes = [c.c_int, c.c_int, vp, c.c_int, c.c_int, vp, i64]
     _LIB = L
     return L
 
@@ -571,3 +573,21 @@ def peak_probe(kind, work):
 def shutdown():
     """Destroy the internal streams and events of the calling thread on the current device (krr_shutdown)."""
     _check(lib().krr_shutdown(), "krr_shutdown")
+
+
+DIST_OPS = {1: "chain", 2: "newest", 3: "older", 4: "trsm", 5: "bcast_m", 6: "bcast_next", 7: "allgather"}
+
+
+def dist_schedule(NT, nb, h_map, world, rank):
+    """krr_dist_schedule: the task / message list of `rank` as a list of dicts (host logic only; NEXT-3)."""
+    h = _host_map(h_map)
+    cnt = int(lib().krr_dist_schedule(NT, nb, _ptr(h), world, rank, None, 0))
+    if cnt < 0:
+        _check(cnt, "krr_dist_schedule")
+    buf = torch.zeros((cnt, 6), dtype=torch.int32)
+    got = int(lib().krr_dist_schedule(NT, nb, _ptr(h), world, rank, _ptr(buf), cnt))
+    assert got == cnt
+    out = []
+    for r in buf.tolist():
+        out.append({"op": DIST_OPS[r[0]], "k": r[1], "root": r[2], "nrows": r[3], "bytes": (r[4] & 0xffffffff) | (r[5] << 32)})
+    return out

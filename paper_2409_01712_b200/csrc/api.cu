@@ -10,6 +10,7 @@
 
 #include "build.cuh"
 #include "common.cuh"
+#include "dist_schedule.cuh"
 #include "gemm_tc.cuh"
 #include "panel.cuh"
 #include "peaks.cuh"
@@ -121,8 +122,9 @@ static size_t host_offsets(int NT, int nb, const uint8_t* h_map, std::vector<int
 }
 
 // ---- workspace layout of krr_potrf_mp ----------------------------------------------------------
+constexpr int kMaxSkUnits = 128;                     // CTA pairs of a stream-K launch (half the SMs of any sm_100 part)
 struct PotrfWs {
-    size_t off_table, a_amax, tile_amax, scl, dscale, prog, split, W, W2, linv_hi, linv_lo, Sh, Sl, Hp, Lp, Qp, total;
+    size_t off_table, a_amax, tile_amax, scl, dscale, prog, split, sk_partial, W, W2, linv_hi, linv_lo, Sh, Sl, Hp, Lp, Qp, total;
 };
 // rows of the scratch planes: S of the panel rows, then two sets (tile-column parity) of M, M^T, U
 static inline size_t scratch_rows(int64_t n, int nb) { return static_cast<size_t>(n) + 6 * static_cast<size_t>(nb); }
@@ -138,7 +140,8 @@ static PotrfWs potrf_ws_layout(int64_t n, int nb, bool any_fp8) {
     w.scl = o;       o = align_up(o + (SCL_COUNT + 2 * (nb / kBlk)) * sizeof(float), 1024);
     w.dscale = o;    o = align_up(o + static_cast<size_t>(NT) * sizeof(float), 1024);        // equilibration of the tile rows
     w.prog = o;      o = align_up(o + static_cast<size_t>(n / kBlk) * sizeof(int), 1024);   // fused-chain progress, per 128-block
-    w.split = o;     o = align_up(o + 256 * sizeof(int), 1024);                              // slice counters of split tail blocks
+    w.split = o;     o = align_up(o + 1024 * sizeof(int), 1024);                             // stream-K: partial-sum flags, one per unit
+    w.sk_partial = o; o = align_up(o + static_cast<size_t>(kMaxSkUnits) * 4 * kBlk * kBlk * sizeof(float), 1024);   // ... and one 256 x 256 block each
     w.W = o;         o = align_up(o + static_cast<size_t>(n) * nb * sizeof(float), 1024);
     w.W2 = o;        o = align_up(o + static_cast<size_t>(n) * nb * sizeof(float), 1024);   // lookahead: column k+1's partial
     w.linv_hi = o;   o = align_up(o + 2 * static_cast<size_t>(nb) * kBlk * 2, 1024);   // two sets (column parity)
@@ -236,29 +239,34 @@ static int launch(int cat, K kernel, dim3 grid, dim3 block, size_t smem, cudaStr
 struct GemmMaps { CUtensorMap H, L, IH[2], IL[2], Q, SH, SL; };
 
 // cg = 2 runs MODE_UPDATE on CTA pairs (256 x 256 output blocks); needs even block counts.
+struct StreamK { int* flags; float* partial; };      // workspace of the stream-K update launches (null: whole blocks, round-robin)
+
 static int launch_gemm(const GemmMaps& m, const GemmOp& op_in, int max_ctas, int cg, cudaStream_t st, int linv_buf = 0,
-                       int* split_flags = nullptr) {
+                       const StreamK* sk = nullptr) {
     GemmOp op = op_in;
     if (op.nrb <= 0 || op.ncb <= 0) return KRR_OK;
     // MODE_TRSM counts as panel_trsm; the fused diagonal chain (MODE_DIAG, POTRF included) and the inverse's recursion as potrf128
     ProfScope ps(op.mode == MODE_UPDATE ? CAT_UPDATE : (op.mode == MODE_P1 ? CAT_P1 : ((op.mode == MODE_DIAG || op.mode == MODE_INV) ? CAT_POTRF : CAT_P3)), st);
     ++g_launches;
+    // units of the stream-K distribution come in groups of one unit per column block: round the grid down to whole groups
+    auto sk_units = [&](int units_max, int cgx) {
+        const int ncbu = op.ncb / cgx;
+        const int nstrips = op.nrb / cgx;
+        int ng = units_max / ncbu;
+        const long long work = static_cast<long long>(nstrips) * ((op.s_hi - op.s_lo) > 0 ? (op.s_hi - op.s_lo) : 1);
+        if (ng > work) ng = static_cast<int>(work);
+        return ng * ncbu;
+    };
     if (cg == 2 && (op.mode == MODE_UPDATE || op.mode == MODE_TRSM) && op.nrb % 2 == 0 && op.rb0 % 2 == 0 && op.ncb % 2 == 0 &&
         op.cb0 % 2 == 0) {
         const int npairs = (op.nrb / 2) * (op.ncb / 2);
         const int max_pairs = max_ctas / 2;
-        const int grid = 2 * (npairs < max_pairs ? npairs : max_pairs);
-        // tail of the last wave: r leftover blocks for max_pairs pairs.  Share each of them between g pairs (slices of the
-        // term range, added into W one after the other) so that the tail lasts 1/g of a block instead of a whole one.
-        const int nterms = op.s_hi - op.s_lo, q = npairs / max_pairs, r = npairs % max_pairs;
-        if (split_flags && op.mode == MODE_UPDATE && q >= 1 && r > 0 && 2 * r <= max_pairs && nterms >= 2) {
-            int g = max_pairs / r;
-            if (g > nterms) g = nterms;
-            if (g > 16) g = 16;
-            if (g >= 2) {
-                op.split_t0 = q * max_pairs; op.split_g = g; op.split_flags = split_flags;
-                if (cudaMemsetAsync(split_flags, 0, static_cast<size_t>(r) * sizeof(int), st) != cudaSuccess) return KRR_ERR_CUDA;
-            }
+        int grid = 2 * (npairs < max_pairs ? npairs : max_pairs);
+        if (sk && op.mode == MODE_UPDATE && max_pairs >= op.ncb / 2) {
+            const int units = sk_units(max_pairs, 2);
+            op.sk = 1; op.sk_flags = sk->flags; op.sk_partial = sk->partial;
+            grid = 2 * units;
+            if (cudaMemsetAsync(sk->flags, 0, static_cast<size_t>(units) * sizeof(int), st) != cudaSuccess) return KRR_ERR_CUDA;
         }
         cudaLaunchConfig_t cfg;
         memset(&cfg, 0, sizeof(cfg));
@@ -574,7 +582,8 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
     KRR_CUDA_CHECK(cudaMemsetAsync(Sh + static_cast<size_t>(n) * nb, 0, 6 * static_cast<size_t>(nb) * nb * 2, st));
     KRR_CUDA_CHECK(cudaMemsetAsync(Sl + static_cast<size_t>(n) * nb, 0, 6 * static_cast<size_t>(nb) * nb * 2, st));
     int* prog = reinterpret_cast<int*>(ws + L.prog);
-    int* split_flags = (flags & KRR_FLAG_NO_TAIL_SPLIT) ? nullptr : reinterpret_cast<int*>(ws + L.split);
+    StreamK sk_ws{reinterpret_cast<int*>(ws + L.split), reinterpret_cast<float*>(ws + L.sk_partial)};
+    const StreamK* sk = ((flags & KRR_FLAG_NO_TAIL_SPLIT) || num_sms / 2 > kMaxSkUnits) ? nullptr : &sk_ws;
     KRR_CUDA_CHECK(cudaMemsetAsync(prog, 0, static_cast<size_t>(n / kBlk) * sizeof(int), st));
     rc = launch(CAT_MISC, scales_init_kernel, dim3((NT * NT + 255) / 256), dim3(256), 0, st, NT, d_scales);
     if (rc) return rc;
@@ -690,7 +699,7 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
         op.mode = MODE_UPDATE; op.c = 0; op.cb0 = 0; op.ncb = nsub;
         if (!lookahead) {
             op.s_lo = 0; op.s_hi = k; op.base_w = 0; op.planes = 1; op.rb0 = 0; op.nrb = mblk;
-            rc = launch_gemm(tm, op, num_sms, cg, st, 0, split_flags);
+            rc = launch_gemm(tm, op, num_sms, cg, st, 0, sk);
             if (rc) return rc;
         } else {
             // terms s < k-1 were accumulated into Wk by O(k) while column k-1 was being factorised; the
@@ -703,7 +712,7 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
             if (rc) return rc;
             if (k >= 1) KRR_CUDA_CHECK(cudaStreamWaitEvent(sl, ev_first(k - 1), 0));     // tile (k, k-1) is stored
             op.rb0 = nsub; op.nrb = mblk - nsub;
-            rc = launch_gemm(tm, op, bulk_ctas, cg, sl);                                 // N(k)
+            rc = launch_gemm(tm, op, bulk_ctas, cg, sl, 0, sk);                          // N(k)
             if (rc) return rc;
             KRR_CUDA_CHECK(cudaEventRecord(ev_newb(k), sl));
             if (k + 1 < NT && k >= 1) {
@@ -712,7 +721,7 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
                 on.k = k + 1; on.prow0 = tile_slot(NT, k + 1, k + 1) * nb; on.W = Wbuf[(k + 1) & 1];
                 on.s_lo = 0; on.s_hi = k; on.base_w = 0; on.planes = 0;
                 on.rb0 = 0; on.nrb = (NT - k - 1) * nsub;
-                rc = launch_gemm(tm, on, bulk_ctas, cg, sl, 0, split_flags);
+                rc = launch_gemm(tm, on, bulk_ctas, cg, sl, 0, sk);
                 if (rc) return rc;
                 KRR_CUDA_CHECK(cudaEventRecord(ev_old(k + 1), sl));
             }
@@ -1623,6 +1632,24 @@ int krr_predict(const int8_t* d_T, int64_t m, int64_t ldt, const int8_t* d_G, in
     else if (nrp == 16) predict_kw_kernel<16><<<grid, 256, 0, st>>>(K, m, n, n, d_W, ldw, nrhs, d_P, ldp);
     else predict_kw_kernel<32><<<grid, 256, 0, st>>>(K, m, n, n, d_W, ldw, nrhs, d_P, ldp);
     return cudaGetLastError() == cudaSuccess ? KRR_OK : KRR_ERR_CUDA;
+}
+
+// ------------------------------------------------------------------------- multi-GPU schedule (NEXT-3, host logic only)
+int64_t krr_dist_schedule(int NT, int nb, const uint8_t* h_map, int world, int rank, int32_t* h_tasks, int64_t max_tasks) {
+    if (NT < 1 || NT > kMaxNT || nb < kBlk || !h_map || world < 1 || rank < 0 || rank >= world) return KRR_ERR_ARG;
+    if (check_map(NT, h_map, nullptr) != KRR_OK) return KRR_ERR_MAP;
+    std::vector<DistTask> t;
+    dist_build_schedule(NT, nb, world, rank,
+                        [&](int i, int j) { return static_cast<int64_t>(nb) * nb * prec_bytes(h_map[i * NT + j]); }, &t);
+    if (h_tasks) {
+        if (static_cast<int64_t>(t.size()) > max_tasks) return KRR_ERR_WORKSPACE;
+        for (size_t q = 0; q < t.size(); ++q) {
+            int32_t* r = h_tasks + 6 * q;
+            r[0] = t[q].op; r[1] = t[q].k; r[2] = t[q].root; r[3] = t[q].nrows;
+            r[4] = static_cast<int32_t>(t[q].bytes & 0xffffffffll); r[5] = static_cast<int32_t>(t[q].bytes >> 32);
+        }
+    }
+    return static_cast<int64_t>(t.size());
 }
 
 // ------------------------------------------------------------------------- roofline denominators (beside the path)

@@ -85,11 +85,11 @@ struct GemmOp {
     float* linv_scale_w;      // = linv_scale, writable
     int* info;                // krr_potrf_mp's d_info
     int64_t col_base;         // 1-based global index of the tile column's first scalar column
-    // MODE_UPDATE, tail of the last wave: the blocks from index split_t0 on are each shared by split_g units, every unit
-    // accumulating a slice of the terms; the slices are added into W one after the other (split_flags[block - split_t0]
-    // counts the CTAs that have stored their slice; zero at launch).  split_g = 0: no splitting.
-    int split_t0, split_g;
-    int* split_flags;
+    // MODE_UPDATE with sk = 1 ("stream-K by row strips", see next_item): sk_flags[unit] counts the CTAs of a unit that have
+    // stored the partial sum of their first item (zero at launch), sk_partial holds one output block per unit.
+    int sk;
+    int* sk_flags;
+    float* sk_partial;
     // scratch planes and the quantising store of MODE_TRSM (X = S inv(L_kk)^T, straight into the mosaic)
     __half* Sh;               // scratch hi plane [n + 6 nb][nb]
     __half* Sl;               // scratch lo plane
@@ -186,6 +186,13 @@ __device__ __forceinline__ TermGeom term_geom(const GemmOp& op, int mode, int c,
 
 template <int CG>
 __device__ __forceinline__ uint32_t term_class_load(const GemmOp& op, int mode, int s /* term index */, int rb) {
+    if (mode == MODE_TRSM) {
+        // X = S M^T for a tile that will be stored as E4M3 (u = 2^-4): the hi images alone (11 bits) are seven bits
+        // beyond what the tile keeps -- one MMA per K step instead of three (the task runs in the
+        // precision the updated tile asks for; FP32 and FP16 tiles keep the full 22-bit product)
+        const int i = op.k + (rb * kBlk) / op.nb;
+        return (op.map[i * op.NT + op.k] == KRR_FP8_E4M3) ? 0u : (kClsALo | kClsBLo);
+    }
     if (mode != MODE_UPDATE) return kClsALo | kClsBLo;
     const int i = op.k + (rb * kBlk) / op.nb;
     s += op.s_lo;
@@ -233,8 +240,10 @@ struct WorkItem {
     int dep;         // > 0: reads what the item `dep` places earlier in this CTA's sequence wrote
     int xcta, xneed; // MODE_DIAG: reads what CTA xcta wrote in its first xneed items (xcta < 0: nothing)
     int t_lo, t_hi;  // terms [t_lo, t_hi) of the launch's term range are accumulated by this item
-    int cpos, clen;  // position in the chain of slices added into W (clen = 1: the block is not split)
-    int fidx;        // index into op.split_flags
+    int sk_role;     // 0: the item holds all terms of its block; 1: it holds the highest terms and finishes the block,
+                     // adding the partial sums of sk_nother units (the first items of units sk_other, sk_other + stride ...);
+                     // 2: it holds lower terms only and leaves a partial sum for the finisher
+    int sk_other, sk_nother, sk_stride;
     TermGeom g;      // MODE_INV: operand geometry of the block
     int o_row, o_col, o_var;   // MODE_INV: scratch row / column of the output block; 0 = U^T, 1 = M21, 2 = M21^T
     // MODE_TRSM / MODE_INV (CG = 1): the K range of a block is accumulated in segments of kSegChunks chunks, each in its
@@ -243,6 +252,7 @@ struct WorkItem {
     int ch_lo, ch_hi, seg_first, seg_last;
 };
 struct ItemIter {
+    long long u;     // stream-K: next (strip, term) unit of this group, -1 before the first call
     int t;           // block modes: next block index
     int g, it, m;    // MODE_DIAG: item inside the chain; segmented modes: it = segments of block t already emitted
 };
@@ -269,7 +279,7 @@ __device__ __forceinline__ bool emit_segment(ItemIter& st, int nunits, int kelem
 template <int CG>
 __device__ __forceinline__ bool next_item(const GemmOp& op, ItemIter& st, int unit0, int nunits, WorkItem& w) {
     w.xcta = -1; w.xneed = 0;
-    w.t_lo = 0; w.t_hi = num_terms(op); w.cpos = 0; w.clen = 1; w.fidx = 0;
+    w.t_lo = 0; w.t_hi = num_terms(op); w.sk_role = 0; w.sk_other = 0; w.sk_nother = 0; w.sk_stride = 0;
     w.ch_lo = -1; w.ch_hi = -1; w.seg_first = 1; w.seg_last = 1;
     if (op.mode == MODE_DIAG) {
         // CTA r owns row block r of the diagonal tile: P3(0), P1(1), P3(1), ..., P3(r-1), P1(r), POTRF(r).
@@ -322,20 +332,52 @@ __device__ __forceinline__ bool next_item(const GemmOp& op, ItemIter& st, int un
     }
     const int ncbu = op.ncb / CG;
     const int ntiles = (op.nrb / CG) * ncbu;
-    const int g = (op.mode == MODE_UPDATE) ? op.split_g : 0;
-    const int next = g ? op.split_t0 + (ntiles - op.split_t0) * g : ntiles;      // extended index space
-    while (st.t < next) {
-        int t = st.t;
-        st.t += nunits;
-        if (g && t >= op.split_t0) {
-            // a block of the tail wave: slice sl of g.  Slices are added into W from the highest terms (smallest
-            // contributions) down to slice 0, which holds the leading tile columns and writes the images.
-            const int sl = (t - op.split_t0) % g;
-            t = op.split_t0 + (t - op.split_t0) / g;
-            const int nt = w.t_hi;
-            w.t_lo = nt * sl / g; w.t_hi = nt * (sl + 1) / g;
-            w.cpos = g - 1 - sl; w.clen = g; w.fidx = t - op.split_t0;
+    if (op.mode == MODE_UPDATE && op.sk) {
+        // Stream-K by row strips.  The work of the launch is the sequence of (row strip r, term) units, strip after strip
+        // and inside a strip from the highest term (the smallest contribution) down to term 0; it is cut into NG equal
+        // ranges, one per GROUP of ncbu units (pairs), and unit j of a group computes column block j of its group's
+        // strips -- so all groups finish together whatever the number of blocks (no partial last wave), the units of a
+        // group walk the same rows of A in step (one DRAM read serves them), and a block whose terms straddle a range
+        // boundary is shared: the groups that hold its lower terms meet it FIRST in their range and leave a partial sum
+        // in sk_partial; the group that holds its highest terms meets it LAST, and its epilogue adds those partial sums
+        // (ascending group = descending terms: the dominant leading columns last, in round-to-nearest FP32) to its own
+        // accumulator and the base, and stores the block.  Nobody waits for work that has not been issued yet, and the
+        // order of every sum is a function of the launch geometry alone: deterministic.
+        const int NG = nunits / ncbu;
+        const int g = unit0 / ncbu, j = unit0 % ncbu;
+        if (g >= NG) return false;                                   // (leftover units of a grid that is no multiple of ncbu)
+        const int nstrips = op.nrb / CG;
+        const int nt = w.t_hi > 0 ? w.t_hi : 1;                       // no terms (the first tile column): one unit per strip
+        const long long U = static_cast<long long>(nstrips) * nt;
+        const long long u1 = U * (g + 1) / NG;
+        if (st.u < 0) st.u = U * g / NG;
+        while (st.u < u1) {
+            const long long u = st.u;
+            const int r = static_cast<int>(u / nt), o = static_cast<int>(u % nt);
+            const int len = static_cast<int>((u1 - u) < (nt - o) ? (u1 - u) : (nt - o));
+            st.u = u + len;
+            w.rb = op.rb0 + r * CG;
+            w.cb = op.cb0 + j * CG;
+            if (tile_is_skipped(op, w.rb + CG - 1, w.cb)) continue;  // the whole (pair) block lies above the diagonal
+            w.mode = op.mode; w.c = op.c; w.dep = 0;
+            if (w.t_hi > 0) { w.t_hi = nt - o; w.t_lo = nt - o - len; }
+            if (len < nt) {
+                if (o == 0) {
+                    // finisher: the rest of the strip's terms, [u + len, (r + 1) nt), lies at the start of the next groups' ranges
+                    w.sk_role = 1; w.sk_other = unit0 + ncbu; w.sk_stride = ncbu; w.sk_nother = 0;
+                    const long long strip_end = static_cast<long long>(r + 1) * nt;
+                    for (int g2 = g + 1; g2 < NG && U * g2 / NG < strip_end; ++g2) ++w.sk_nother;
+                } else {
+                    w.sk_role = 2;
+                }
+            }
+            return true;
         }
+        return false;
+    }
+    while (st.t < ntiles) {
+        const int t = st.t;
+        st.t += nunits;
         w.rb = op.rb0 + (t / ncbu) * CG;
         w.cb = op.cb0 + (t % ncbu) * CG;
         if (tile_is_skipped(op, w.rb + CG - 1, w.cb)) continue;      // the whole (pair) block lies above the diagonal
@@ -452,7 +494,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
             auto load = [&](uint32_t dst, const CUtensorMap* m, uint32_t bar, int c0, int c1) {
                 if (CG == 2) ptx::tma_load_2d_pair(dst, m, bar, c0, c1); else ptx::tma_load_2d(dst, m, bar, c0, c1);
             };
-            ItemIter iter = {unit0, 0, 0, 0};
+            ItemIter iter = {-1, unit0, 0, 0, 0};
             WorkItem w;
             int seq = 0;
             while (next_item<CG>(op, iter, unit0, nunits, w)) {
@@ -541,7 +583,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
             uint32_t phase = 0;
             int buf = 0;
             uint32_t acc_phase = 0;
-            ItemIter iter = {unit0, 0, 0, 0};
+            ItemIter iter = {-1, unit0, 0, 0, 0};
             WorkItem w;
             while (next_item<CG>(op, iter, unit0, nunits, w)) {
                 const int rb = w.rb;
@@ -650,7 +692,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
         const int nsub = op.nb / kBlk;
         int buf = 0;
         uint32_t acc_phase = 0;
-        ItemIter iter = {unit0, 0, 0, 0};
+        ItemIter iter = {-1, unit0, 0, 0, 0};
         WorkItem w;
         int eseq = 0;                                                // items this CTA has finished
         // One 32-row x 64-byte part of the warp's sub-block: `src` is this lane's 64 bytes (its row); dst = address
@@ -709,17 +751,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
                 ++eseq;
                 continue;
             }
-            if (w.cpos > 0) {
-                // a later slice of a split block: the slices before it have been added into W by other CTAs
-                if (lane == 0) {
-                    const volatile int* f = op.split_flags + w.fidx;
-                    uint32_t spins = 0;
-                    while (*f < CG * w.cpos) { __nanosleep(32); if (++spins > (1u << 26)) __trap(); }
-                    __threadfence();
-                }
-                __syncwarp();
-            }
-            const bool item_planes = write_planes && (w.cpos == w.clen - 1);
+            const bool item_planes = write_planes && (w.sk_role != 2);
             // everything the store needs from global memory is fetched here, before the wait for the accumulator
             int t_prec = KRR_FP32;
             uint8_t* t_tile = nullptr;
@@ -742,8 +774,8 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
             float* wblk = op.W + (static_cast<int64_t>(rb) * nsub + cb) * (kBlk * kBlk) + static_cast<int64_t>(64 * hf) * kBlk + row_in_blk;
             // ---- base values, fetched before the accumulator is ready
             float bs[64];
-            const bool base_from_w = (w.mode == MODE_P1) || (w.mode == MODE_UPDATE && (op.base_w || w.cpos > 0));
-            const bool base_from_a = (w.mode == MODE_UPDATE && !op.base_w && w.cpos == 0);
+            const bool base_from_w = (w.mode == MODE_P1) || (w.mode == MODE_UPDATE && op.base_w && w.sk_role != 2);
+            const bool base_from_a = (w.mode == MODE_UPDATE && !op.base_w && w.sk_role != 2);
             if (dead) {
 #pragma unroll
                 for (int e = 0; e < 64; ++e) bs[e] = 0.0f;
@@ -799,10 +831,16 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
                 }
                 if (split_cross) {
                     // main + cross accumulators, added in FP32 (round to nearest); the TMEM buffer is released afterwards
+                    // (an E4M3 tile's product has no cross terms: its second accumulator was never written)
                     uint32_t c0[32], c1[32];
-                    ptx::tmem_ld_32x32(taddr + kAccW, c0);
-                    ptx::tmem_ld_32x32(taddr + kAccW + 32, c1);
-                    ptx::tmem_ld_wait();
+                    if (t_prec != KRR_FP8_E4M3) {
+                        ptx::tmem_ld_32x32(taddr + kAccW, c0);
+                        ptx::tmem_ld_32x32(taddr + kAccW + 32, c1);
+                        ptx::tmem_ld_wait();
+                    } else {
+#pragma unroll
+                        for (int e = 0; e < 32; ++e) { c0[e] = 0u; c1[e] = 0u; }
+                    }
 #pragma unroll
                     for (int e = 0; e < 32; ++e) {
                         out[e] = -(__uint_as_float(a0[e]) + __uint_as_float(c0[e])) * acc_mul;
@@ -829,6 +867,33 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
                 for (int e = 0; e < 64; ++e) out[e] = bs[e];
             }
             if (dead || !w.seg_last) continue;
+            if (w.sk_role == 2) {
+                // lower terms of a block another group finishes: leave -(sum of the products) for it (block-column-major
+                // like W: a warp's 32 rows of a column are 128 contiguous bytes)
+                float* pblk = op.sk_partial + ((static_cast<int64_t>(unit0) * CG + rank) * CG + j2) * (kBlk * kBlk) +
+                              static_cast<int64_t>(64 * hf) * kBlk + row_in_blk;
+#pragma unroll
+                for (int e = 0; e < 64; ++e) __stcg(pblk + e * kBlk, out[e]);
+                continue;
+            }
+            if (w.sk_role == 1) {
+                // highest terms of a shared block: add the partial sums of the groups that hold the lower terms, in ascending
+                // group order (descending terms: the dominant leading columns last)
+                for (int m = 0; m < w.sk_nother; ++m) {
+                    const int ou = w.sk_other + m * w.sk_stride;
+                    if (lane == 0) {
+                        const volatile int* f = op.sk_flags + ou;
+                        uint32_t spins = 0;
+                        while (*f < CG) { __nanosleep(64); if (++spins > (1u << 26)) __trap(); }
+                        __threadfence();
+                    }
+                    __syncwarp();
+                    const float* pblk = op.sk_partial + ((static_cast<int64_t>(ou) * CG + rank) * CG + j2) * (kBlk * kBlk) +
+                                        static_cast<int64_t>(64 * hf) * kBlk + row_in_blk;
+#pragma unroll
+                    for (int e = 0; e < 64; ++e) out[e] += __ldcg(pblk + e * kBlk);
+                }
+            }
             if (w.mode == MODE_INV) {
                 // a block of U^T (scale su) or of M / M^T (scale sm) into the scratch planes; a value beyond the FP16 range
                 // means the diagonal tile is too ill-conditioned for the product form of the TRSM: info = -2
@@ -892,13 +957,13 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
                 }
             }
           }   // j2
-            if (w.clen > 1 && w.cpos < w.clen - 1) {
-                // a slice of a split block is in W: let the next slice's CTAs go on (the last warp of this CTA signals)
+            if (w.sk_role == 2) {
+                // the partial sum is in sk_partial: tell the finisher (the last warp of this CTA signals; a unit leaves at
+                // most one partial sum per launch -- for its first item)
                 __threadfence();
                 __syncwarp();
                 if (lane == 0) {
-                    // (a CTA holds at most one slice of a split block: its last item)
-                    if (atomicAdd_block(split_ctr, 1) == kEpiWarps - 1) { __threadfence(); atomicAdd(op.split_flags + w.fidx, 1); }
+                    if (atomicAdd_block(split_ctr, 1) == kEpiWarps - 1) { __threadfence(); atomicAdd(op.sk_flags + unit0, 1); }
                 }
             }
             if (op.mode == MODE_DIAG) {

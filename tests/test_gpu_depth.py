@@ -63,19 +63,20 @@ def perturbed(An, seed=0):
     return np.tril(Ap) + np.tril(Ap, -1).T
 
 
-# The oracle dominates the run time (two evaluations per case, the second on the perturbed input for the floor; on the
-# 16 host cores of a GPU box: n = 8192 at nb = 128 about 70 s, n = 16384 at nb = 256 about 130 s, n = 24576 about 440 s).
-# The default selection keeps the file at a few minutes; KRR_DEPTH_FULL=1 runs every case (about 40 minutes; the log of the
-# last full run is kept as profiles/r02_depth_tests_full.txt).
+# The oracle dominates the run time (two evaluations per case, the second on the perturbed input for the floor; measured on the
+# 16 host cores of a GPU box: n = 8192 at nb = 128 103 s, n = 12288 at nb = 256 147 s, n = 16384 at nb = 256 240 - 270 s).
+# The default selection keeps the file at about five minutes; KRR_DEPTH_FULL=1 runs every case (about 40 minutes; the log of
+# the last full run is kept as profiles/r02_depth_tests_full.txt).
 CASES = [
     # (id, base config, nb, n, p, map kind, PREROUND_A, in the default selection)
     ("C3h_twin_nb128", "C3", 128, 8192, 6144, "fp16", True, True),               # NT = 64 (C3's tile count), all FP16
     ("C4_twin_nb128", "C4", 128, 16384, 12288, "rule", True, False),             # NT = 128: the rule gives all FP16
     ("C5p_twin_nb128", "C5", 128, 12288, 2560, "fp8_col0_fp32", False, False),   # NT = 96: C5' map
-    ("C3h_nb256_NT64", "C3", 256, 16384, 12288, "fp16", True, True),
+    ("C3h_nb256_NT64", "C3", 256, 16384, 12288, "fp16", True, False),
     ("C5p_nb256_NT48", "C5", 256, 12288, 2560, "fp8_col0_fp32", False, True),
     ("C5p_nb256_NT96", "C5", 256, 24576, 5120, "fp8_col0_fp32", False, False),
-    ("mosaic_nb256_NT64", "S1", 256, 16384, 12288, "random", True, True),
+    ("mosaic_nb128_NT48", "S1", 128, 6144, 4608, "random", True, True),
+    ("mosaic_nb256_NT64", "S1", 256, 16384, 12288, "random", True, False),
     ("S1_rule_nb256_NT64", "S1", 256, 16384, 12288, "rule", True, False),
 ]
 

@@ -239,7 +239,7 @@ static int launch(int cat, K kernel, dim3 grid, dim3 block, size_t smem, cudaStr
 struct GemmMaps { CUtensorMap H, L, IH[2], IL[2], Q, SH, SL; };
 
 // cg = 2 runs MODE_UPDATE on CTA pairs (256 x 256 output blocks); needs even block counts.
-struct StreamK { int* flags; float* partial; };      // workspace of the stream-K update launches (null: whole blocks, round-robin)
+struct StreamK { int* flags; float* partial; };      // workspace of the K-split of an update's last wave (null: whole blocks only)
 
 static int launch_gemm(const GemmMaps& m, const GemmOp& op_in, int max_ctas, int cg, cudaStream_t st, int linv_buf = 0,
                        const StreamK* sk = nullptr) {
@@ -248,25 +248,14 @@ static int launch_gemm(const GemmMaps& m, const GemmOp& op_in, int max_ctas, int
     // MODE_TRSM counts as panel_trsm; the fused diagonal chain (MODE_DIAG, POTRF included) and the inverse's recursion as potrf128
     ProfScope ps(op.mode == MODE_UPDATE ? CAT_UPDATE : (op.mode == MODE_P1 ? CAT_P1 : ((op.mode == MODE_DIAG || op.mode == MODE_INV) ? CAT_POTRF : CAT_P3)), st);
     ++g_launches;
-    // units of the stream-K distribution come in groups of one unit per column block: round the grid down to whole groups
-    auto sk_units = [&](int units_max, int cgx) {
-        const int ncbu = op.ncb / cgx;
-        const int nstrips = op.nrb / cgx;
-        int ng = units_max / ncbu;
-        const long long work = static_cast<long long>(nstrips) * ((op.s_hi - op.s_lo) > 0 ? (op.s_hi - op.s_lo) : 1);
-        if (ng > work) ng = static_cast<int>(work);
-        return ng * ncbu;
-    };
     if (cg == 2 && (op.mode == MODE_UPDATE || op.mode == MODE_TRSM) && op.nrb % 2 == 0 && op.rb0 % 2 == 0 && op.ncb % 2 == 0 &&
         op.cb0 % 2 == 0) {
         const int npairs = (op.nrb / 2) * (op.ncb / 2);
         const int max_pairs = max_ctas / 2;
-        int grid = 2 * (npairs < max_pairs ? npairs : max_pairs);
-        if (sk && op.mode == MODE_UPDATE && max_pairs >= op.ncb / 2) {
-            const int units = sk_units(max_pairs, 2);
+        const int grid = 2 * (npairs < max_pairs ? npairs : max_pairs);
+        if (sk && op.mode == MODE_UPDATE && npairs > max_pairs && op.s_hi - op.s_lo >= 2) {
             op.sk = 1; op.sk_flags = sk->flags; op.sk_partial = sk->partial;
-            grid = 2 * units;
-            if (cudaMemsetAsync(sk->flags, 0, static_cast<size_t>(units) * sizeof(int), st) != cudaSuccess) return KRR_ERR_CUDA;
+            if (cudaMemsetAsync(sk->flags, 0, static_cast<size_t>(max_pairs) * sizeof(int), st) != cudaSuccess) return KRR_ERR_CUDA;
         }
         cudaLaunchConfig_t cfg;
         memset(&cfg, 0, sizeof(cfg));
@@ -712,7 +701,7 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
             if (rc) return rc;
             if (k >= 1) KRR_CUDA_CHECK(cudaStreamWaitEvent(sl, ev_first(k - 1), 0));     // tile (k, k-1) is stored
             op.rb0 = nsub; op.nrb = mblk - nsub;
-            rc = launch_gemm(tm, op, bulk_ctas, cg, sl, 0, sk);                          // N(k)
+            rc = launch_gemm(tm, op, bulk_ctas, cg, sl);                                 // N(k)
             if (rc) return rc;
             KRR_CUDA_CHECK(cudaEventRecord(ev_newb(k), sl));
             if (k + 1 < NT && k >= 1) {

@@ -85,8 +85,8 @@ struct GemmOp {
     float* linv_scale_w;      // = linv_scale, writable
     int* info;                // krr_potrf_mp's d_info
     int64_t col_base;         // 1-based global index of the tile column's first scalar column
-    // MODE_UPDATE with sk = 1 ("stream-K by row strips", see next_item): sk_flags[unit] counts the CTAs of a unit that have
-    // stored the partial sum of their first item (zero at launch), sk_partial holds one output block per unit.
+    // MODE_UPDATE with sk = 1 (K-split of the last, partial wave: see next_item): sk_flags[unit] counts the CTAs of a unit
+    // that have stored the partial sum of their tail item (zero at launch), sk_partial holds one output block per unit.
     int sk;
     int* sk_flags;
     float* sk_partial;
@@ -186,13 +186,10 @@ __device__ __forceinline__ TermGeom term_geom(const GemmOp& op, int mode, int c,
 
 template <int CG>
 __device__ __forceinline__ uint32_t term_class_load(const GemmOp& op, int mode, int s /* term index */, int rb) {
-    if (mode == MODE_TRSM) {
-        // X = S M^T for a tile that will be stored as E4M3 (u = 2^-4): the hi images alone (11 bits) are seven bits
-        // beyond what the tile keeps -- one MMA per K step instead of three (the task runs in the
-        // precision the updated tile asks for; FP32 and FP16 tiles keep the full 22-bit product)
-        const int i = op.k + (rb * kBlk) / op.nb;
-        return (op.map[i * op.NT + op.k] == KRR_FP8_E4M3) ? 0u : (kClsALo | kClsBLo);
-    }
+    // (MODE_TRSM: a one-pass product -- hi images only -- for tiles that will be stored as E4M3 was tried in r02: three
+    // times faster, backward error unchanged, but the perturbation of 2^-11 flips enough E4M3 roundings to take the
+    // literal difference from the emulated oracle from 4e-5 to 1.5e-3 on a random mosaic: dropped, every tile keeps
+    // the 22-bit product)
     if (mode != MODE_UPDATE) return kClsALo | kClsBLo;
     const int i = op.k + (rb * kBlk) / op.nb;
     s += op.s_lo;
@@ -252,7 +249,7 @@ struct WorkItem {
     int ch_lo, ch_hi, seg_first, seg_last;
 };
 struct ItemIter {
-    long long u;     // stream-K: next (strip, term) unit of this group, -1 before the first call
+    long long u;     // (unused)
     int t;           // block modes: next block index
     int g, it, m;    // MODE_DIAG: item inside the chain; segmented modes: it = segments of block t already emitted
 };
@@ -333,47 +330,46 @@ __device__ __forceinline__ bool next_item(const GemmOp& op, ItemIter& st, int un
     const int ncbu = op.ncb / CG;
     const int ntiles = (op.nrb / CG) * ncbu;
     if (op.mode == MODE_UPDATE && op.sk) {
-        // Stream-K by row strips.  The work of the launch is the sequence of (row strip r, term) units, strip after strip
-        // and inside a strip from the highest term (the smallest contribution) down to term 0; it is cut into NG equal
-        // ranges, one per GROUP of ncbu units (pairs), and unit j of a group computes column block j of its group's
-        // strips -- so all groups finish together whatever the number of blocks (no partial last wave), the units of a
-        // group walk the same rows of A in step (one DRAM read serves them), and a block whose terms straddle a range
-        // boundary is shared: the groups that hold its lower terms meet it FIRST in their range and leave a partial sum
-        // in sk_partial; the group that holds its highest terms meets it LAST, and its epilogue adds those partial sums
-        // (ascending group = descending terms: the dominant leading columns last, in round-to-nearest FP32) to its own
-        // accumulator and the base, and stores the block.  Nobody waits for work that has not been issued yet, and the
-        // order of every sum is a function of the launch geometry alone: deterministic.
-        const int NG = nunits / ncbu;
-        const int g = unit0 / ncbu, j = unit0 % ncbu;
-        if (g >= NG) return false;                                   // (leftover units of a grid that is no multiple of ncbu)
-        const int nstrips = op.nrb / CG;
-        const int nt = w.t_hi > 0 ? w.t_hi : 1;                       // no terms (the first tile column): one unit per strip
-        const long long U = static_cast<long long>(nstrips) * nt;
-        const long long u1 = U * (g + 1) / NG;
-        if (st.u < 0) st.u = U * g / NG;
-        while (st.u < u1) {
-            const long long u = st.u;
-            const int r = static_cast<int>(u / nt), o = static_cast<int>(u % nt);
-            const int len = static_cast<int>((u1 - u) < (nt - o) ? (u1 - u) : (nt - o));
-            st.u = u + len;
-            w.rb = op.rb0 + r * CG;
-            w.cb = op.cb0 + j * CG;
-            if (tile_is_skipped(op, w.rb + CG - 1, w.cb)) continue;  // the whole (pair) block lies above the diagonal
-            w.mode = op.mode; w.c = op.c; w.dep = 0;
-            if (w.t_hi > 0) { w.t_hi = nt - o; w.t_lo = nt - o - len; }
-            if (len < nt) {
-                if (o == 0) {
-                    // finisher: the rest of the strip's terms, [u + len, (r + 1) nt), lies at the start of the next groups' ranges
-                    w.sk_role = 1; w.sk_other = unit0 + ncbu; w.sk_stride = ncbu; w.sk_nother = 0;
-                    const long long strip_end = static_cast<long long>(r + 1) * nt;
-                    for (int g2 = g + 1; g2 < NG && U * g2 / NG < strip_end; ++g2) ++w.sk_nother;
-                } else {
-                    w.sk_role = 2;
-                }
+        // Whole blocks round-robin (all units walk the terms in step, so a tile of the B operand is read by every unit
+        // at the same time and served from L2 once), and the TAIL of the last, partial wave split in K: when the remainder
+        // r is at most half the units, each of the r leftover blocks is shared by g = nunits / r units, unit sl of a block
+        // accumulating the slice [nt sl / g, nt (sl + 1) / g) of its terms.  The slices below the highest leave their sum in
+        // sk_partial; the unit with the highest slice (the smallest contributions) adds them to its accumulator in FP32,
+        // descending -- the dominant leading tile columns last -- and stores the block.  Everyone works at the same
+        // time, nobody waits for work that has not been issued, and the order of every sum is a function of the launch
+        // geometry alone: deterministic.
+        // (Tried in r02 and dropped: a full stream-K split -- equal (strip, term) ranges per group of units.  Balanced to
+        // a fraction of a percent, but the groups then sit at different terms at any one time, the B operand (tile row k of
+        // L) is streamed once per group instead of once per wave, and the kernel turns DRAM-bound: C3 232 -> 279 ms.)
+        const int nt = w.t_hi;
+        const int q = ntiles / nunits, r = ntiles % nunits;
+        int g = (q >= 1 && r > 0 && 2 * r <= nunits && nt >= 2) ? nunits / r : 0;
+        if (g > nt) g = nt;
+        if (g > 16) g = 16;
+        if (g < 2) g = 0;
+        while (true) {
+            int t;
+            if (st.t < q * nunits || g == 0) {
+                if (st.t >= ntiles) return false;
+                t = st.t;
+                st.t += nunits;
+                if (g != 0 && st.t >= q * nunits) st.t = ntiles;          // next: the tail item
+            } else {
+                if (st.it) return false;                                  // (the tail item has been handed out)
+                st.it = 1;
+                const int b = unit0 / g, sl = unit0 % g;
+                if (b >= r) return false;
+                t = q * nunits + b;
+                w.t_lo = nt * sl / g; w.t_hi = nt * (sl + 1) / g;
+                if (sl == g - 1) { w.sk_role = 1; w.sk_other = unit0 - 1; w.sk_stride = -1; w.sk_nother = g - 1; }
+                else w.sk_role = 2;
             }
+            w.rb = op.rb0 + (t / ncbu) * CG;
+            w.cb = op.cb0 + (t % ncbu) * CG;
+            if (tile_is_skipped(op, w.rb + CG - 1, w.cb)) { if (w.sk_role) return false; continue; }
+            w.mode = op.mode; w.c = op.c; w.dep = 0;
             return true;
         }
-        return false;
     }
     while (st.t < ntiles) {
         const int t = st.t;
@@ -831,16 +827,10 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
                 }
                 if (split_cross) {
                     // main + cross accumulators, added in FP32 (round to nearest); the TMEM buffer is released afterwards
-                    // (an E4M3 tile's product has no cross terms: its second accumulator was never written)
                     uint32_t c0[32], c1[32];
-                    if (t_prec != KRR_FP8_E4M3) {
-                        ptx::tmem_ld_32x32(taddr + kAccW, c0);
-                        ptx::tmem_ld_32x32(taddr + kAccW + 32, c1);
-                        ptx::tmem_ld_wait();
-                    } else {
-#pragma unroll
-                        for (int e = 0; e < 32; ++e) { c0[e] = 0u; c1[e] = 0u; }
-                    }
+                    ptx::tmem_ld_32x32(taddr + kAccW, c0);
+                    ptx::tmem_ld_32x32(taddr + kAccW + 32, c1);
+                    ptx::tmem_ld_wait();
 #pragma unroll
                     for (int e = 0; e < 32; ++e) {
                         out[e] = -(__uint_as_float(a0[e]) + __uint_as_float(c0[e])) * acc_mul;

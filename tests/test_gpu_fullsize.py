@@ -139,11 +139,13 @@ def test_full_size_leading_block_and_invariants(krr, name):
 
 
 def test_tail_split_of_the_last_wave(krr):
-    """More output blocks than CTA pairs with a small remainder (NT = 80 tiles of 256: 75-79 pair blocks per tile
-    column for 73-74 pairs): the blocks of the last, partial wave are shared between pairs, each accumulating a slice
-    of the terms, the slices added into the FP32 partial sums in a fixed order.  Same products, another summation
-    order for those blocks: against KRR_FLAG_NO_TAIL_SPLIT to FP32 noise, against the FP64 oracle as usual, and
-    deterministic, in both schedules."""
+    """Stream-K distribution of the trailing updates (r02; the r01 split of the last partial wave generalised): with NT = 80
+    tiles of 256 every update launch has more (strip, term) units than CTA pairs, and every block whose terms straddle
+    the boundary between two pairs' ranges is shared -- the later pair leaves the partial sum of the lower terms, the
+    earlier one adds it to its accumulator in FP32.  Same products, another (fixed) summation order for those blocks:
+    against KRR_FLAG_NO_TAIL_SPLIT (whole blocks, round-robin) to FP32 noise -- 2e-5 at n = 20480, where the two orders
+    differ in about one block per pair and tile column instead of the last wave's few --, against the FP64 oracle as usual,
+    and deterministic, in both schedules."""
     from dataclasses import replace
     from krr_inputs import scaled_config
     cfg = replace(scaled_config(CONFIGS["C2"], nb=256, n=20480, p=4000))
@@ -161,7 +163,7 @@ def test_tail_split_of_the_last_wave(krr):
         assert torch.equal(F1.payload, F3.payload)                        # deterministic
         assert not torch.equal(F1.payload, F2.payload)                    # the split path was taken
         L1, L2 = F1.dense().cpu().numpy(), F2.dense().cpu().numpy()
-        assert relF(L1, L2) <= 1e-5
+        assert relF(L1, L2) <= 2e-5
         assert relF(L1, Lo) <= 1e-4 and relF(L2, Lo) <= 1e-4
         assert probe_backward_error(A, F1, 4) <= 1e-6
 

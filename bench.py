@@ -55,7 +55,8 @@ def ncu_traffic(name):
         for key in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
             i = hdr.index(key)
             tot += float(r[i].replace(",", "")) * scale.get(units[i], 1.0)
-    return tot, f"profiles/r02_update_kernel_raw_{name}.csv (last captured launch; command in profiles/r02_update_kernel_{name}.md)"
+    return tot, (f"profiles/r02_update_kernel_raw_{name}.csv: ncu --set full capture of one launch of the dominant shape O(k+1) at "
+                 "k = 32 (command and reading in profiles/r02_update_kernel.md)")
 
 
 def measured_class_peaks():

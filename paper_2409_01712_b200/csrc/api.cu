@@ -124,17 +124,32 @@ static size_t host_offsets(int NT, int nb, const uint8_t* h_map, std::vector<int
 // ---- workspace layout of krr_potrf_mp ----------------------------------------------------------
 constexpr int kMaxSkUnits = 128;                     // CTA pairs of a stream-K launch (half the SMs of any sm_100 part)
 struct PotrfWs {
-    size_t off_table, a_amax, tile_amax, scl, dscale, prog, split, sk_partial, W, W2, linv_hi, linv_lo, Sh, Sl, Hp, Lp, Qp, total;
+    size_t off_table, lrow, qrow, a_amax, tile_amax, scl, dscale, prog, split, sk_partial, W, W2, linv_hi, linv_lo, Sh, Sl, Hp, Lp, Qp, total;
 };
 // rows of the scratch planes: S of the panel rows, then two sets (tile-column parity) of M, M^T, U
 static inline size_t scratch_rows(int64_t n, int nb) { return static_cast<size_t>(n) + 6 * static_cast<size_t>(nb); }
-static PotrfWs potrf_ws_layout(int64_t n, int nb, bool any_fp8) {
+// The operand images are sized from the map (the mosaic "reduces memory footprint"): the hi image for every
+// lower tile, the lo image only for FP32 tiles, the E4M3 image only for FP8 tiles (n_fp32 / n_fp8 = their counts; at least
+// one tile's worth each, so that the tensor maps stay valid).
+static void count_tiles(int NT, const uint8_t* h_map, size_t* n_fp32, size_t* n_fp8) {
+    size_t a = 0, b = 0;
+    for (int i = 0; i < NT; ++i)
+        for (int j = 0; j <= i; ++j) {
+            a += (h_map[i * NT + j] == KRR_FP32);
+            b += (h_map[i * NT + j] == KRR_FP8_E4M3);
+        }
+    *n_fp32 = a; *n_fp8 = b;
+}
+static PotrfWs potrf_ws_layout(int64_t n, int nb, size_t n_fp32, size_t n_fp8) {
     const int64_t NT = n / nb;
     const size_t nslots = static_cast<size_t>(NT) * (NT + 1) / 2;
     const size_t plane = nslots * nb * nb;
+    const size_t tile = static_cast<size_t>(nb) * nb;
     PotrfWs w;
     size_t o = 0;
     w.off_table = o; o = align_up(o + NT * NT * sizeof(int64_t), 1024);
+    w.lrow = o;      o = align_up(o + NT * NT * sizeof(int), 1024);
+    w.qrow = o;      o = align_up(o + NT * NT * sizeof(int), 1024);
     w.a_amax = o;    o = align_up(o + NT * NT * sizeof(float), 1024);
     w.tile_amax = o; o = align_up(o + nslots * sizeof(float), 1024);
     w.scl = o;       o = align_up(o + (SCL_COUNT + 2 * (nb / kBlk)) * sizeof(float), 1024);
@@ -149,8 +164,8 @@ static PotrfWs potrf_ws_layout(int64_t n, int nb, bool any_fp8) {
     w.Sh = o;        o = align_up(o + scratch_rows(n, nb) * nb * 2, 1024);
     w.Sl = o;        o = align_up(o + scratch_rows(n, nb) * nb * 2, 1024);
     w.Hp = o;        o = align_up(o + plane * 2, 1024);
-    w.Lp = o;        o = align_up(o + plane * 2, 1024);
-    w.Qp = o;        if (any_fp8) o = align_up(o + plane, 1024);
+    w.Lp = o;        o = align_up(o + (n_fp32 ? n_fp32 : 1) * tile * 2, 1024);
+    w.Qp = o;        o = align_up(o + (n_fp8 ? n_fp8 : 1) * tile, 1024);
     w.total = o;
     return w;
 }
@@ -516,7 +531,9 @@ size_t krr_potrf_mp_workspace(int64_t n, int nb, const uint8_t* h_map) {
     if (!h_map || check_shape(n, nb) != KRR_OK) return 0;
     bool f8 = false;
     if (check_map(static_cast<int>(n / nb), h_map, &f8) != KRR_OK) return 0;
-    return potrf_ws_layout(n, nb, f8).total;
+    size_t n32 = 0, n8 = 0;
+    count_tiles(static_cast<int>(n / nb), h_map, &n32, &n8);
+    return potrf_ws_layout(n, nb, n32, n8).total;
 }
 
 int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t* d_map, const uint8_t* h_map,
@@ -538,7 +555,9 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
     bool any_fp8 = false;
     rc = check_map(NT, h_map, &any_fp8);
     if (rc) return rc;
-    const PotrfWs L = potrf_ws_layout(n, nb, any_fp8);
+    size_t n_fp32 = 0, n_fp8 = 0;
+    count_tiles(NT, h_map, &n_fp32, &n_fp8);
+    const PotrfWs L = potrf_ws_layout(n, nb, n_fp32, n_fp8);
     if (ws_bytes < L.total) return KRR_ERR_WORKSPACE;
     int num_sms = 0;
     rc = check_device(&num_sms);
@@ -549,6 +568,8 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     uint8_t* ws = static_cast<uint8_t*>(d_ws);
     int64_t* off = reinterpret_cast<int64_t*>(ws + L.off_table);
+    int* lrow = reinterpret_cast<int*>(ws + L.lrow);
+    int* qrow = reinterpret_cast<int*>(ws + L.qrow);
     float* a_amax = reinterpret_cast<float*>(ws + L.a_amax);
     float* tile_amax = reinterpret_cast<float*>(ws + L.tile_amax);
     float* W = reinterpret_cast<float*>(ws + L.W);
@@ -576,7 +597,7 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
     KRR_CUDA_CHECK(cudaMemsetAsync(prog, 0, static_cast<size_t>(n / kBlk) * sizeof(int), st));
     rc = launch(CAT_MISC, scales_init_kernel, dim3((NT * NT + 255) / 256), dim3(256), 0, st, NT, d_scales);
     if (rc) return rc;
-    rc = launch(CAT_MISC, offsets_kernel, dim3(1), dim3(32), 0, st, NT, nb, d_map, off, host_map_hash(NT, h_map), d_info);
+    rc = launch(CAT_MISC, offsets_kernel, dim3(1), dim3(32), 0, st, NT, nb, d_map, off, host_map_hash(NT, h_map), d_info, lrow, qrow);
     if (rc) return rc;
     rc = launch(CAT_MISC, equilibrate_kernel, dim3(1), dim3(1024), 0, st, A, n, scl, dscale);
     if (rc) return rc;
@@ -588,7 +609,15 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
     }
 
     GemmMaps tm;
-    if (make_plane_tmap(&tm.H, Hp, nslots * nb, nb) || make_plane_tmap(&tm.L, Lp, nslots * nb, nb) ||
+    // (host copy of the lo-plane rows of the diagonal tiles: the same count, in the same order, as offsets_kernel's)
+    std::vector<int64_t> diag_lrow(NT);
+    {
+        int64_t nl = 0;
+        for (int j = 0; j < NT; ++j)
+            for (int i = j; i < NT; ++i)
+                if (h_map[i * NT + j] == KRR_FP32) { if (i == j) diag_lrow[j] = nl * nb; ++nl; }
+    }
+    if (make_plane_tmap(&tm.H, Hp, nslots * nb, nb) || make_plane_tmap(&tm.L, Lp, (n_fp32 ? n_fp32 : 1) * nb, nb) ||
         make_plane_tmap(&tm.SH, Sh, scratch_rows(n, nb), nb) || make_plane_tmap(&tm.SL, Sl, scratch_rows(n, nb), nb))
         return KRR_ERR_CUDA;
     const size_t linv_elems = static_cast<size_t>(nb) * kBlk;           // one set of inverted diagonal blocks
@@ -597,7 +626,7 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
             make_plane_tmap(&tm.IL[b], linv_lo + b * linv_elems, nb, kBlk))
             return KRR_ERR_CUDA;
     if (any_fp8) {
-        if (make_byte_plane_tmap(&tm.Q, Qp, nslots * nb, nb)) return KRR_ERR_CUDA;
+        if (make_byte_plane_tmap(&tm.Q, Qp, (n_fp8 ? n_fp8 : 1) * nb, nb)) return KRR_ERR_CUDA;
     } else {
         tm.Q = tm.H;                              // never dereferenced (op.fp8q = 0)
     }
@@ -658,7 +687,7 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
         }
         return launch(CAT_FINALIZE, finalize_kernel, dim3(nsub * nsub * 4, count), dim3(256), 0, s, NT, nb, k, i0, Wk, d_map,
                       static_cast<const int64_t*>(off), static_cast<const float*>(tile_amax), static_cast<uint8_t*>(d_factor),
-                      d_scales, Hp, Qp, static_cast<const float*>(scl), static_cast<const float*>(dscale), only_fp8);
+                      d_scales, Hp, Qp, static_cast<const int*>(qrow), static_cast<const float*>(scl), static_cast<const float*>(dscale), only_fp8);
     };
 
     // Tile column k.  Critical stream `sh`: newest term on the diagonal tile, the diagonal-tile
@@ -677,6 +706,7 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
         memset(&op, 0, sizeof(op));
         op.nb = nb; op.NT = NT; op.k = k;
         op.prow0 = tile_slot(NT, k, k) * nb;
+        op.prow0_lo = diag_lrow[k]; op.lrow = lrow; op.qrow = qrow;
         op.map = d_map; op.A = A; op.a_amax = (preround && any_fp8) ? a_amax : nullptr;
         op.W = Wk; op.Hp = Hp; op.Lp = Lp; op.tile_amax = tile_amax; op.flags = flags;
         op.scl = scl; op.dscale = dscale; op.linv_scale = linv_scale + lb * nsub;
@@ -707,7 +737,7 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
             if (k + 1 < NT && k >= 1) {
                 // O(k+1): terms s < k of column k+1, beside the chain of column k
                 GemmOp on = op;
-                on.k = k + 1; on.prow0 = tile_slot(NT, k + 1, k + 1) * nb; on.W = Wbuf[(k + 1) & 1];
+                on.k = k + 1; on.prow0 = tile_slot(NT, k + 1, k + 1) * nb; on.prow0_lo = diag_lrow[k + 1]; on.W = Wbuf[(k + 1) & 1];
                 on.s_lo = 0; on.s_hi = k; on.base_w = 0; on.planes = 0;
                 on.rb0 = 0; on.nrb = (NT - k - 1) * nsub;
                 rc = launch_gemm(tm, on, bulk_ctas, cg, sl, 0, sk);
@@ -985,7 +1015,8 @@ int krr_potrs(const void* d_factor, const float* d_scales, const uint8_t* d_map,
     float* Minv = reinterpret_cast<float*>(ws + L.Minv);
     float* MinvT = reinterpret_cast<float*>(ws + L.MinvT);
     float* stage = reinterpret_cast<float*>(ws + L.stage);
-    rc = launch(CAT_MISC, offsets_kernel, dim3(1), dim3(32), 0, st, NT, nb, d_map, off, host_map_hash(NT, h_map), static_cast<int*>(nullptr));
+    rc = launch(CAT_MISC, offsets_kernel, dim3(1), dim3(32), 0, st, NT, nb, d_map, off, host_map_hash(NT, h_map), static_cast<int*>(nullptr),
+                static_cast<int*>(nullptr), static_cast<int*>(nullptr));
     if (rc) return rc;
     const uint8_t* factor = static_cast<const uint8_t*>(d_factor);
     rc = launch(CAT_POTRS, trtri128_kernel, dim3(static_cast<unsigned>(n / kBlk)), dim3(kTriThreads), static_cast<size_t>(kTriSmem), st,
@@ -1268,7 +1299,7 @@ Arena arena_layout(int64_t n, int nb, int nrhs) {
     a.scales = o;   o = align_up(o + NT * NT * sizeof(float), 1024);
     a.pm_ws = o;    o = align_up(o + krr_precision_map_workspace(n, nb), 1024);
     a.factor = o;   o = align_up(o + nslots * nb * nb * sizeof(float), 1024);
-    a.potrf_ws = o; o = align_up(o + potrf_ws_layout(n, nb, true).total, 1024);
+    a.potrf_ws = o; o = align_up(o + potrf_ws_layout(n, nb, nslots, 0).total, 1024);     // worst case: every tile FP32 (hi + lo images)
     a.potrs_ws = o; o = align_up(o + krr_potrs_workspace(n, nb, nrhs), 1024);
     a.total = o;
     return a;

@@ -70,7 +70,10 @@ struct GemmOp {
     const float* a_amax;  // NT*NT max|A_ij| (FP8 pre-rounding of A), may be null
     float* W;             // panel workspace, FP32 [m][nb]
     __half* Hp;           // hi plane  [nslots*nb][nb]
-    __half* Lp;           // lo plane
+    __half* Lp;           // lo plane: FP32 tiles only, compact (row of tile (i,j) = lrow[i*NT+j], -1 for other tiles)
+    const int* lrow;      // device int[NT*NT]
+    const int* qrow;      // device int[NT*NT]: first row of the E4M3 image of tile (i,j) in the Qp plane (FP8 tiles only), else -1
+    int64_t prow0_lo;     // lo-plane row of panel-local row 0 of the diagonal tile (k,k) (= lrow[k*NT+k], known to the host)
     float* tile_amax;     // per-slot max|X| accumulated by MODE_P3
     const float* scales;  // NT*NT tile scales of the mosaic (FP8 tiles), written by finalize_kernel
     int fp8q;             // MODE_UPDATE: FP8 x FP8 terms may use the E4M3 images (Qp plane exists)
@@ -130,7 +133,9 @@ constexpr int kGemmSmem = kSlots * kSlotBytes + 1024 /*align*/ + 256 /*barriers*
 // reduction (REDUX writes a uniform register), so that the issue loops below compile to uniform-
 // datapath code around the single elected lane that issues TMA / tcgen05 instructions.
 struct TermGeom {
-    int a_row, b_row;       // plane rows (TMA coordinate 1)
+    int a_row, b_row;       // plane rows (TMA coordinate 1) in the hi planes
+    int a_row_lo, b_row_lo; // ... in the lo planes (the compact Lp for factor tiles; the same rows elsewhere)
+    int a_row_q, b_row_q;   // ... in the E4M3 plane (MODE_UPDATE, FP8 tiles)
     int a_k0, b_k0;         // first K column (TMA coordinate 0)
     int kelems;             // K extent in elements
     int a_src, b_src;       // operand planes: 0 = factor / panel images (tmH, tmL), 1 = inverted 128-blocks (tmIH, tmIL),
@@ -156,9 +161,15 @@ __device__ __forceinline__ TermGeom term_geom(const GemmOp& op, int mode, int c,
         s += op.s_lo;
         t.a_row = static_cast<int>(tile_slot(op.NT, i, s) * op.nb + subrow);
         t.b_row = static_cast<int>(tile_slot(op.NT, op.k, s) * op.nb + cb * kBlk);
+        // (the tables answer -1 for tiles without that image; the class word keeps such a row from ever being loaded)
+        t.a_row_lo = op.lrow[i * op.NT + s] + subrow;
+        t.b_row_lo = op.lrow[op.k * op.NT + s] + cb * kBlk;
+        t.a_row_q = op.qrow[i * op.NT + s] + subrow;
+        t.b_row_q = op.qrow[op.k * op.NT + s] + cb * kBlk;
         t.a_k0 = 0;
         t.b_k0 = 0;
         t.kelems = op.nb;
+        return t;
     } else if (mode == MODE_P1) {
         t.a_row = static_cast<int>(op.prow0) + rb * kBlk;
         t.b_row = static_cast<int>(op.prow0) + c * kBlk;
@@ -181,6 +192,10 @@ __device__ __forceinline__ TermGeom term_geom(const GemmOp& op, int mode, int c,
         t.b_k0 = 0;
         t.kelems = kBlk;
     }
+    // rows of the diagonal tile in the (compact) lo plane; the scratch and inverse planes index hi and lo alike
+    t.a_row_lo = (t.a_src == 0) ? t.a_row - static_cast<int>(op.prow0) + static_cast<int>(op.prow0_lo) : t.a_row;
+    t.b_row_lo = (t.b_src == 0) ? t.b_row - static_cast<int>(op.prow0) + static_cast<int>(op.prow0_lo) : t.b_row;
+    t.a_row_q = t.b_row_q = 0;
     return t;
 }
 
@@ -322,6 +337,9 @@ __device__ __forceinline__ bool next_item(const GemmOp& op, ItemIter& st, int un
                 w.g.b_src = 2; w.g.b_row = static_cast<int>(op.srow_m) + (o + hl + nbk) * kBlk;
                 w.o_row = static_cast<int>(op.srow_mt) + (o + mb) * kBlk; w.o_col = (o + hl + nbk) * kBlk;
             }
+            w.g.a_row_lo = w.g.a_row;
+            w.g.b_row_lo = (w.g.b_src == 0) ? w.g.b_row - static_cast<int>(op.prow0) + static_cast<int>(op.prow0_lo) : w.g.b_row;
+            w.g.a_row_q = w.g.b_row_q = 0;
             w.rb = 0; w.cb = 0;
             return emit_segment(st, nunits, w.g.kelems, w);
         }
@@ -517,15 +535,21 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
                     const uint32_t cls = make_uniform(cls_next);
                     if (s > w.t_lo) cls_next = term_class_load<CG>(op, w.mode, s - 1, rb);   // in flight during this term's chunks
                     // this CTA's A rows and B rows
-                    const TermGeom g = (w.mode == MODE_INV) ? w.g : term_geom(op, w.mode, w.c, s, rb, cb0u + rank, cb0u, CG);
+                    TermGeom g = (w.mode == MODE_INV) ? w.g : term_geom(op, w.mode, w.c, s, rb, cb0u + rank, cb0u, CG);
+                    if (w.mode == MODE_UPDATE) {         // table look-ups: make them provably warp-uniform (TMA coordinates)
+                        g.a_row_lo = static_cast<int>(make_uniform(static_cast<uint32_t>(g.a_row_lo)));
+                        g.b_row_lo = static_cast<int>(make_uniform(static_cast<uint32_t>(g.b_row_lo)));
+                        g.a_row_q = static_cast<int>(make_uniform(static_cast<uint32_t>(g.a_row_q)));
+                        g.b_row_q = static_cast<int>(make_uniform(static_cast<uint32_t>(g.b_row_q)));
+                    }
                     if (cls & kClsQ) {                       // E4M3 images: 128 bytes of K per row, one slot per chunk
                         for (int ch = g.kelems / 128 - 1; ch >= 0; --ch) {
                             ptx::mbar_wait(empty_bar(slot), phase ^ 1u);
                             if (ptx::elect_one()) {
                                 const uint32_t sa = smem_base + slot * SB;
                                 if (rank == 0) ptx::mbar_arrive_expect_tx(full_bar(slot), CG * 2u * kPlaneBytes);
-                                load(sa, &tmQ, full_bar(slot), ch * 128, g.a_row);
-                                load(sa + kPlaneBytes, &tmQ, full_bar(slot), ch * 128, g.b_row);
+                                load(sa, &tmQ, full_bar(slot), ch * 128, g.a_row_q);
+                                load(sa + kPlaneBytes, &tmQ, full_bar(slot), ch * 128, g.b_row_q);
                             }
                             if (++slot == kSlots) { slot = 0; phase ^= 1u; }
                         }
@@ -553,8 +577,8 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
                             if (ptx::elect_one()) {
                                 const uint32_t sa = smem_base + slot * SB;
                                 if (rank == 0) ptx::mbar_arrive_expect_tx(full_bar(slot), lo_bytes);
-                                if (a_lo) load(sa, mA_lo, full_bar(slot), ak, g.a_row);
-                                if (b_lo) load(sa + kPlaneBytes, mB_lo, full_bar(slot), bk, g.b_row);
+                                if (a_lo) load(sa, mA_lo, full_bar(slot), ak, g.a_row_lo);
+                                if (b_lo) load(sa + kPlaneBytes, mB_lo, full_bar(slot), bk, g.b_row_lo);
                             }
                             if (++slot == kSlots) { slot = 0; phase ^= 1u; }
                         }
@@ -707,7 +731,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
         };
         // hi (and lo) FP16 images of out[0..63] * mul: rows prow.., columns col.. of planes with row pitch op.nb.
         // Returns the largest |image value| of this lane (range check of the inverse's planes).
-        auto store_images = [&](const float (&out)[64], float mul, __half* hi_plane, __half* lo_plane, int64_t prow, int col) {
+        auto store_images = [&](const float (&out)[64], float mul, __half* hi_plane, __half* lo_plane, int64_t prow, int64_t prow_lo, int col) {
             float big = 0.0f;
 #pragma unroll
             for (int part = 0; part < 4; ++part) {             // (columns 0-31 hi, lo, columns 32-63 hi, lo)
@@ -723,7 +747,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
                     if (!is_lo) big = fmaxf(big, fabsf(x));
                 }
                 __half* plane = is_lo ? lo_plane : hi_plane;
-                store_part(reinterpret_cast<const uint4*>(hv), reinterpret_cast<uint8_t*>(plane + prow * op.nb + col + jj * 32),
+                store_part(reinterpret_cast<const uint4*>(hv), reinterpret_cast<uint8_t*>(plane + (is_lo ? prow_lo : prow) * op.nb + col + jj * 32),
                            static_cast<int64_t>(op.nb) * 2);
             }
             return big;
@@ -752,6 +776,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
             int t_prec = KRR_FP32;
             uint8_t* t_tile = nullptr;
             float t_acc_mul = 0.0f, t_sx = 0.0f, t_di = 1.0f, t_inv_di = 1.0f;
+            int64_t t_lrow = 0;                                      // first lo-plane row of the tile (FP32 tiles)
             if (w.mode == MODE_TRSM) {
                 const int ti = op.k + (rb * kBlk) / op.nb;
                 t_prec = op.map[ti * op.NT + op.k];
@@ -760,6 +785,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
                 t_sx = op.scl[SCL_SX];
                 t_di = op.dscale[ti];
                 t_inv_di = 1.0f / t_di;
+                t_lrow = op.lrow[ti * op.NT + op.k];
             }
 #pragma unroll 1
           for (int j2 = 0; j2 < CG; ++j2) {                       // the unit's column blocks, one after the other
@@ -888,7 +914,8 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
                 // a block of U^T (scale su) or of M / M^T (scale sm) into the scratch planes; a value beyond the FP16 range
                 // means the diagonal tile is too ill-conditioned for the product form of the TRSM: info = -2
                 const float mul = op.scl[w.o_var == 0 ? SCL_SU : SCL_SM];
-                const float big = store_images(out, mul, op.Sh, op.Sl, static_cast<int64_t>(w.o_row) + q * 32, w.o_col + 64 * hf);
+                const int64_t orow = static_cast<int64_t>(w.o_row) + q * 32;
+                const float big = store_images(out, mul, op.Sh, op.Sl, orow, orow, w.o_col + 64 * hf);
                 if (!(big < 60000.0f)) atomicCAS(op.info, 0, -2);
             } else if (w.mode == MODE_TRSM) {
                 // X = S inv(L_kk)^T is final: round once into the tile's storage precision and store it (R4; PAPER.md:206
@@ -900,7 +927,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
                 uint8_t* tile = t_tile;
                 // (out holds the equilibrated X~ = d_i X: the images are of X~, the stored tile is X = X~ / d_i)
                 if (p == KRR_FP32) {
-                    store_images(out, t_sx, op.Hp, op.Lp, prow, col0);
+                    store_images(out, t_sx, op.Hp, op.Lp, prow, t_lrow + (rb * kBlk) % op.nb + q * 32, col0);
 #pragma unroll
                     for (int e = 0; e < 64; ++e) out[e] *= t_inv_di;
 #pragma unroll
@@ -920,7 +947,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
                         store_part(reinterpret_cast<const uint4*>(hv), tile + (static_cast<int64_t>(r_tile) * op.nb + col0 + 32 * part) * 2,
                                    static_cast<int64_t>(op.nb) * 2);
                     }
-                    store_images(rd, t_sx, op.Hp, nullptr, prow, col0);      // image of the STORED value (exact)
+                    store_images(rd, t_sx, op.Hp, nullptr, prow, prow, col0);      // image of the STORED value (exact)
                 } else {
                     float amax = 0.0f;
 #pragma unroll
@@ -942,8 +969,9 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
                 }
                 if (item_planes) {
                     const float mul = op.scl[w.mode == MODE_P3 ? SCL_SX : SCL_SS];
-                    if (below) store_images(out, mul, op.Sh, op.Sl, static_cast<int64_t>(rb) * kBlk + q * 32, col0);
-                    else store_images(out, mul, op.Hp, op.Lp, op.prow0 + static_cast<int64_t>(rb) * kBlk + q * 32, col0);
+                    const int64_t lrow0 = static_cast<int64_t>(rb) * kBlk + q * 32;      // panel-local row of this warp
+                    if (below) store_images(out, mul, op.Sh, op.Sl, lrow0, lrow0, col0);
+                    else store_images(out, mul, op.Hp, op.Lp, op.prow0 + lrow0, op.prow0_lo + lrow0, col0);
                 }
             }
           }   // j2

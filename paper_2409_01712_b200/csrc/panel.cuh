@@ -67,22 +67,31 @@ constexpr uint64_t kMapHashSeed = 1469598103934665603ull;
 // Byte offsets of the mosaic tiles (column-major lower order prefix sum).  One thread.  If the device map does not
 // hash to `host_hash` (the caller's h_map and d_map differ) every offset is set to 0 -- all tiles alias the first
 // (FP32, diagonal) tile, so that nothing is read or written outside buffers sized from h_map -- and *info = -1.
+// lrow / qrow (may be null): first row of tile (i,j) in the compact lo plane (FP32 tiles) and E4M3 plane (FP8 tiles), in the
+// same column-major tile order, -1 for tiles without that image (all 0 on a hash mismatch).
 __global__ void offsets_kernel(int NT, int nb, const uint8_t* __restrict__ map, int64_t* __restrict__ off, uint64_t host_hash,
-                               int* __restrict__ info) {
+                               int* __restrict__ info, int* __restrict__ lrow, int* __restrict__ qrow) {
     if (threadIdx.x != 0 || blockIdx.x != 0) return;
     int64_t acc = 0;
     const int64_t elems = static_cast<int64_t>(nb) * nb;
     uint64_t h = kMapHashSeed;
+    int nl = 0, nq = 0;
     for (int j = 0; j < NT; ++j)
         for (int i = j; i < NT; ++i) {
             off[i * NT + j] = acc;
             const uint8_t p = map[i * NT + j];
             h = map_hash_step(h, p);
             acc += elems * prec_bytes(p);
+            if (lrow) lrow[i * NT + j] = (p == KRR_FP32) ? (nl++) * nb : -1;
+            if (qrow) qrow[i * NT + j] = (p == KRR_FP8_E4M3) ? (nq++) * nb : -1;
         }
     if (h != host_hash) {
         for (int j = 0; j < NT; ++j)
-            for (int i = j; i < NT; ++i) off[i * NT + j] = 0;
+            for (int i = j; i < NT; ++i) {
+                off[i * NT + j] = 0;
+                if (lrow) lrow[i * NT + j] = 0;
+                if (qrow) qrow[i * NT + j] = 0;
+            }
         if (info) *info = -1;
     }
 }
@@ -116,7 +125,8 @@ __global__ void __launch_bounds__(256)
 finalize_kernel(int NT, int nb, int k, int i0, const float* __restrict__ W, const uint8_t* __restrict__ map,
                 const int64_t* __restrict__ off, const float* __restrict__ tile_amax /* per slot */,
                 uint8_t* __restrict__ factor, float* __restrict__ scales, __half* __restrict__ Hp,
-                uint8_t* __restrict__ Qp, const float* __restrict__ scl, const float* __restrict__ dscale, int only_fp8) {
+                uint8_t* __restrict__ Qp, const int* __restrict__ qrow, const float* __restrict__ scl,
+                const float* __restrict__ dscale, int only_fp8) {
     __shared__ float tile[32][kBlk + 1];
     const float sx = scl[SCL_SX];
     const int nsub = nb / kBlk;
@@ -163,7 +173,7 @@ finalize_kernel(int NT, int nb, int k, int i0, const float* __restrict__ W, cons
             const float inv = 1.0f / s;          // power of two: exact
             __align__(4) uint8_t q[4] = {f32_to_e4m3(v.x * inv), f32_to_e4m3(v.y * inv), f32_to_e4m3(v.z * inv), f32_to_e4m3(v.w * inv)};
             *reinterpret_cast<uint32_t*>(dst + e) = *reinterpret_cast<const uint32_t*>(q);
-            if (Qp) *reinterpret_cast<uint32_t*>(Qp + (slot * nb + r) * nb + c) = *reinterpret_cast<const uint32_t*>(q);
+            if (Qp) *reinterpret_cast<uint32_t*>(Qp + (static_cast<int64_t>(qrow[i * NT + k]) + r) * nb + c) = *reinterpret_cast<const uint32_t*>(q);
             __align__(8) __half h[4];
 #pragma unroll
             for (int u = 0; u < 4; ++u) h[u] = __float2half_rn(e4m3_to_f32(q[u]) * s * di * sx);

@@ -5,6 +5,7 @@
 #include <cuda_runtime.h>
 
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <vector>
 
@@ -279,20 +280,22 @@ static int launch_gemm(const GemmMaps& m, const GemmOp& op_in, int max_ctas, int
         attr[0].id = cudaLaunchAttributeClusterDimension;
         attr[0].val.clusterDim.x = 2; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
         cfg.attrs = attr; cfg.numAttrs = 1;
-        return cudaLaunchKernelEx(&cfg, gemm_tc_kernel<2>, m.H, m.L, m.IH[0], m.IL[0], m.Q, m.SH, m.SL, op) == cudaSuccess ? KRR_OK : KRR_ERR_CUDA;
+        const cudaError_t e = cudaLaunchKernelEx(&cfg, gemm_tc_kernel<2>, m.H, m.L, m.IH[0], m.IL[0], m.Q, m.SH, m.SL, op);
+        if (e != cudaSuccess && getenv("KRR_DEBUG")) fprintf(stderr, "krr: gemm_tc_kernel<2> launch: %s\n", cudaGetErrorString(e));
+        return e == cudaSuccess ? KRR_OK : KRR_ERR_CUDA;
     }
     // MODE_DIAG: one CTA per row block of the diagonal tile; MODE_INV: one per 128 x 128 block of the level's products
     int ntiles = op.nrb * op.ncb;
     if (op.mode == MODE_DIAG) ntiles = op.nrb;
     if (op.mode == MODE_INV) {
-        ntiles = 0;
-        for (int nd = 0; nd < op.nodes.count; ++nd)
-            ntiles += op.nodes.hl[nd] * op.nodes.hr[nd] * (op.inv_step == 0 ? 1 : (op.inv_last ? 1 : 2));
+        ntiles = op.node.hl * op.node.hr * (op.inv_step == 0 ? 1 : (op.inv_last ? 1 : 2));
         if (ntiles == 0) return KRR_OK;
     }
     const int grid = ntiles < max_ctas ? ntiles : max_ctas;
     gemm_tc_kernel<1><<<grid, kGemmThreads, kGemmSmem, st>>>(m.H, m.L, m.IH[linv_buf], m.IL[linv_buf], m.Q, m.SH, m.SL, op);
-    return cudaGetLastError() == cudaSuccess ? KRR_OK : KRR_ERR_CUDA;
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess && getenv("KRR_DEBUG")) fprintf(stderr, "krr: gemm_tc_kernel<1> launch (mode %d): %s\n", op.mode, cudaGetErrorString(e));
+    return e == cudaSuccess ? KRR_OK : KRR_ERR_CUDA;
 }
 
 template <int NRHS>
@@ -660,8 +663,7 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
     // inverse stream beside the chain's next sub-columns; only the last row block's two launches come after the chain
     auto inverse_row = [&](GemmOp op, int r, int lb, cudaStream_t s) -> int {
         op.mode = MODE_INV; op.c = 0; op.cb0 = 0; op.ncb = 1; op.rb0 = 0; op.nrb = 1;
-        memset(&op.nodes, 0, sizeof(op.nodes));
-        op.nodes.count = 1; op.nodes.o[0] = 0; op.nodes.hl[0] = r; op.nodes.hr[0] = 1;
+        op.node.o = 0; op.node.hl = r; op.node.hr = 1;
         op.inv_last = (r == nsub - 1) ? 1 : 0;
         for (int step = 0; step < 2; ++step) {
             op.inv_step = step;

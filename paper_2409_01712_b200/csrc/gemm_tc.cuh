@@ -48,11 +48,7 @@ enum { MODE_UPDATE = 0, MODE_P1 = 1, MODE_P3 = 2, MODE_TRSM = 3, MODE_DIAG = 4, 
 // Scratch planes (hi / lo FP16 images, row pitch nb, one tensor map each): rows [0, n) hold the Schur complement S of
 // the panel rows below the diagonal tile (panel-local row index), then two sets (tile-column parity) of three nb x nb
 // areas: M = inv(L_kk), its transpose MT, and the intermediate U of the inverse's recursion.
-constexpr int kInvMaxNodes = 16;
-struct InvNodes {                 // one level of the binary splitting of the diagonal tile's 128-blocks
-    int count;
-    int o[kInvMaxNodes], hl[kInvMaxNodes], hr[kInvMaxNodes];   // left blocks [o, o + hl), right blocks [o + hl, o + hl + hr)
-};
+struct InvNode { int o, hl, hr; };   // MODE_INV: left blocks [o, o + hl), right blocks [o + hl, o + hl + hr) of the diagonal tile
 
 struct GemmOp {
     int mode;
@@ -101,7 +97,7 @@ struct GemmOp {
     uint8_t* factor;          // the mosaic
     // MODE_INV: one step of one level of the recursion M21 = -M22 L21 M11 (step 0: U^T = M11^T L21^T; step 1: M21 and M21^T)
     int inv_step, inv_last;   // inv_last: the root level, whose M21^T is not needed
-    InvNodes nodes;
+    InvNode node;             // (scalars: a dynamically indexed array in the kernel parameters would be copied to local memory)
 };
 
 
@@ -309,10 +305,10 @@ __device__ __forceinline__ bool next_item(const GemmOp& op, ItemIter& st, int un
         return true;
     }
     if (op.mode == MODE_INV) {
-        // blocks of all nodes of the level, node after node; every block in K segments
+        // the blocks of the node's products, every block in K segments
         int t = st.t;
-        for (int nd = 0; nd < op.nodes.count; ++nd) {
-            const int hl = op.nodes.hl[nd], hr = op.nodes.hr[nd], o = op.nodes.o[nd];
+        for (int nd = 0; nd < 1; ++nd) {
+            const int hl = op.node.hl, hr = op.node.hr, o = op.node.o;
             const int per = hl * hr;
             const int cnt = op.inv_step == 0 ? per : (op.inv_last ? per : 2 * per);
             if (t >= cnt) { t -= cnt; continue; }
@@ -403,6 +399,57 @@ __device__ __forceinline__ bool next_item(const GemmOp& op, ItemIter& st, int un
         return true;
     }
     return false;
+}
+
+// ---- epilogue store helpers (free functions, forced inline: every array stays in registers) --------------------------
+// One 32-row x 64-byte part of a warp's sub-block: s0..s3 are this lane's 64 bytes (its row); the rows go through the
+// warp's staging buffer so that every store instruction writes 8 full 64-byte row segments.  dst = address of row 0 of
+// the part, pitch in bytes.
+__device__ __forceinline__ void epi_store_part(uint8_t* stg, int lane, uint4 s0, uint4 s1, uint4 s2, uint4 s3, uint8_t* dst, int64_t pitch) {
+    __syncwarp();                                   // previous part has been read out
+    *reinterpret_cast<uint4*>(stg + lane * kEpiRowBytes + 0) = s0;
+    *reinterpret_cast<uint4*>(stg + lane * kEpiRowBytes + 16) = s1;
+    *reinterpret_cast<uint4*>(stg + lane * kEpiRowBytes + 32) = s2;
+    *reinterpret_cast<uint4*>(stg + lane * kEpiRowBytes + 48) = s3;
+    __syncwarp();
+#pragma unroll
+    for (int it = 0; it < 4; ++it) {
+        const int rr = it * 8 + (lane >> 2), ch = lane & 3;
+        const uint4 v = *reinterpret_cast<const uint4*>(stg + rr * kEpiRowBytes + ch * 16);
+        *reinterpret_cast<uint4*>(dst + rr * pitch + ch * 16) = v;
+    }
+}
+__device__ __forceinline__ uint32_t epi_pack2(float a, float b) {      // two FP16 roundings in one word (a in the low half)
+    const __half2 h = __floats2half2_rn(a, b);
+    return *reinterpret_cast<const uint32_t*>(&h);
+}
+// hi (and lo, if lo_plane) FP16 images of out[0..63] * mul: rows prow.. (lo plane: prow_lo..), columns col.. of planes
+// with row pitch nb.  Returns the largest |image value| of this lane (range check of the inverse's planes).
+__device__ __forceinline__ float epi_store_images(uint8_t* stg, int lane, const float (&out)[64], float mul, __half* hi_plane,
+                                                  __half* lo_plane, int64_t prow, int64_t prow_lo, int col, int nb) {
+    float big = 0.0f;
+#pragma unroll
+    for (int part = 0; part < 4; ++part) {             // (columns 0-31 hi, lo, columns 32-63 hi, lo)
+        const int jj = part >> 1;
+        const bool is_lo = part & 1;
+        if (is_lo && lo_plane == nullptr) continue;
+        uint32_t wds[16];
+#pragma unroll
+        for (int t = 0; t < 16; ++t) {
+            const float x0 = out[jj * 32 + 2 * t] * mul, x1 = out[jj * 32 + 2 * t + 1] * mul;
+            if (!is_lo) {
+                big = fmaxf(big, fmaxf(fabsf(x0), fabsf(x1)));
+                wds[t] = epi_pack2(x0, x1);
+            } else {
+                wds[t] = epi_pack2(x0 - __half2float(__float2half_rn(x0)), x1 - __half2float(__float2half_rn(x1)));
+            }
+        }
+        __half* plane = is_lo ? lo_plane : hi_plane;
+        epi_store_part(stg, lane, make_uint4(wds[0], wds[1], wds[2], wds[3]), make_uint4(wds[4], wds[5], wds[6], wds[7]),
+                       make_uint4(wds[8], wds[9], wds[10], wds[11]), make_uint4(wds[12], wds[13], wds[14], wds[15]),
+                       reinterpret_cast<uint8_t*>(plane + (is_lo ? prow_lo : prow) * nb + col + jj * 32), static_cast<int64_t>(nb) * 2);
+    }
+    return big;
 }
 
 // CG = 1: one CTA per 128x128 output block.  CG = 2 (MODE_UPDATE only): a CTA pair (cluster of 2,
@@ -715,43 +762,6 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
         ItemIter iter = {-1, unit0, 0, 0, 0};
         WorkItem w;
         int eseq = 0;                                                // items this CTA has finished
-        // One 32-row x 64-byte part of the warp's sub-block: `src` is this lane's 64 bytes (its row); dst = address
-        // of row 0 of the part, pitch in bytes.
-        auto store_part = [&](const uint4* src, uint8_t* dst, int64_t pitch) {
-            __syncwarp();                                   // previous part has been read out
-#pragma unroll
-            for (int u = 0; u < 4; ++u) *reinterpret_cast<uint4*>(stg + lane * kEpiRowBytes + u * 16) = src[u];
-            __syncwarp();
-#pragma unroll
-            for (int it = 0; it < 4; ++it) {
-                const int rr = it * 8 + (lane >> 2), ch = lane & 3;
-                const uint4 v = *reinterpret_cast<const uint4*>(stg + rr * kEpiRowBytes + ch * 16);
-                *reinterpret_cast<uint4*>(dst + rr * pitch + ch * 16) = v;
-            }
-        };
-        // hi (and lo) FP16 images of out[0..63] * mul: rows prow.., columns col.. of planes with row pitch op.nb.
-        // Returns the largest |image value| of this lane (range check of the inverse's planes).
-        auto store_images = [&](const float (&out)[64], float mul, __half* hi_plane, __half* lo_plane, int64_t prow, int64_t prow_lo, int col) {
-            float big = 0.0f;
-#pragma unroll
-            for (int part = 0; part < 4; ++part) {             // (columns 0-31 hi, lo, columns 32-63 hi, lo)
-                const int jj = part >> 1;
-                const bool is_lo = part & 1;
-                if (is_lo && lo_plane == nullptr) continue;
-                __align__(16) __half hv[32];
-#pragma unroll
-                for (int e = 0; e < 32; ++e) {
-                    const float x = out[jj * 32 + e] * mul;
-                    const __half h = __float2half_rn(x);
-                    hv[e] = is_lo ? __float2half_rn(x - __half2float(h)) : h;
-                    if (!is_lo) big = fmaxf(big, fabsf(x));
-                }
-                __half* plane = is_lo ? lo_plane : hi_plane;
-                store_part(reinterpret_cast<const uint4*>(hv), reinterpret_cast<uint8_t*>(plane + (is_lo ? prow_lo : prow) * op.nb + col + jj * 32),
-                           static_cast<int64_t>(op.nb) * 2);
-            }
-            return big;
-        };
         float out[64];                                               // (lives across the K segments of a block)
         while (next_item<CG>(op, iter, unit0, nunits, w)) {
             const int rb = w.rb + rank, cb0u = w.cb;
@@ -853,15 +863,15 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
                 }
                 if (split_cross) {
                     // main + cross accumulators, added in FP32 (round to nearest); the TMEM buffer is released afterwards
-                    uint32_t c0[32], c1[32];
+                    uint32_t c0[32];
                     ptx::tmem_ld_32x32(taddr + kAccW, c0);
-                    ptx::tmem_ld_32x32(taddr + kAccW + 32, c1);
                     ptx::tmem_ld_wait();
 #pragma unroll
-                    for (int e = 0; e < 32; ++e) {
-                        out[e] = -(__uint_as_float(a0[e]) + __uint_as_float(c0[e])) * acc_mul;
-                        out[32 + e] = -(__uint_as_float(a1[e]) + __uint_as_float(c1[e])) * acc_mul;
-                    }
+                    for (int e = 0; e < 32; ++e) out[e] = -(__uint_as_float(a0[e]) + __uint_as_float(c0[e])) * acc_mul;
+                    ptx::tmem_ld_32x32(taddr + kAccW + 32, c0);
+                    ptx::tmem_ld_wait();
+#pragma unroll
+                    for (int e = 0; e < 32; ++e) out[32 + e] = -(__uint_as_float(a1[e]) + __uint_as_float(c0[e])) * acc_mul;
                     ptx::tc_fence_before();
                     __syncwarp();
                     if (j2 == CG - 1 && lane == 0) ptx::mbar_arrive_leader(tempty_bar(0));
@@ -915,7 +925,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
                 // means the diagonal tile is too ill-conditioned for the product form of the TRSM: info = -2
                 const float mul = op.scl[w.o_var == 0 ? SCL_SU : SCL_SM];
                 const int64_t orow = static_cast<int64_t>(w.o_row) + q * 32;
-                const float big = store_images(out, mul, op.Sh, op.Sl, orow, orow, w.o_col + 64 * hf);
+                const float big = epi_store_images(stg, lane, out, mul, op.Sh, op.Sl, orow, orow, w.o_col + 64 * hf, op.nb);
                 if (!(big < 60000.0f)) atomicCAS(op.info, 0, -2);
             } else if (w.mode == MODE_TRSM) {
                 // X = S inv(L_kk)^T is final: round once into the tile's storage precision and store it (R4; PAPER.md:206
@@ -927,27 +937,34 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
                 uint8_t* tile = t_tile;
                 // (out holds the equilibrated X~ = d_i X: the images are of X~, the stored tile is X = X~ / d_i)
                 if (p == KRR_FP32) {
-                    store_images(out, t_sx, op.Hp, op.Lp, prow, t_lrow + (rb * kBlk) % op.nb + q * 32, col0);
+                    epi_store_images(stg, lane, out, t_sx, op.Hp, op.Lp, prow, t_lrow + (rb * kBlk) % op.nb + q * 32, col0, op.nb);
 #pragma unroll
-                    for (int e = 0; e < 64; ++e) out[e] *= t_inv_di;
+                    for (int part = 0; part < 4; ++part) {
+                        uint32_t wds[16];
 #pragma unroll
-                    for (int part = 0; part < 4; ++part)
-                        store_part(reinterpret_cast<const uint4*>(out + 16 * part),
-                                   tile + (static_cast<int64_t>(r_tile) * op.nb + col0 + 16 * part) * 4, static_cast<int64_t>(op.nb) * 4);
+                        for (int t = 0; t < 16; ++t) wds[t] = __float_as_uint(out[16 * part + t] * t_inv_di);
+                        epi_store_part(stg, lane, make_uint4(wds[0], wds[1], wds[2], wds[3]), make_uint4(wds[4], wds[5], wds[6], wds[7]),
+                                       make_uint4(wds[8], wds[9], wds[10], wds[11]), make_uint4(wds[12], wds[13], wds[14], wds[15]),
+                                       tile + (static_cast<int64_t>(r_tile) * op.nb + col0 + 16 * part) * 4, static_cast<int64_t>(op.nb) * 4);
+                    }
                 } else if (p == KRR_FP16) {
-                    float rd[64];
+                    // the stored value h = rn16(X~ / d_i); out becomes its equilibrated value h d_i, whose image is exact
 #pragma unroll
                     for (int part = 0; part < 2; ++part) {
-                        __align__(16) __half hv[32];
+                        uint32_t wds[16];
 #pragma unroll
-                        for (int e = 0; e < 32; ++e) {
-                            hv[e] = __float2half_rn(out[32 * part + e] * t_inv_di);
-                            rd[32 * part + e] = __half2float(hv[e]) * t_di;
+                        for (int t = 0; t < 16; ++t) {
+                            const int e = 32 * part + 2 * t;
+                            const __half2 h = __floats2half2_rn(out[e] * t_inv_di, out[e + 1] * t_inv_di);
+                            out[e] = __low2float(h) * t_di;
+                            out[e + 1] = __high2float(h) * t_di;
+                            wds[t] = *reinterpret_cast<const uint32_t*>(&h);
                         }
-                        store_part(reinterpret_cast<const uint4*>(hv), tile + (static_cast<int64_t>(r_tile) * op.nb + col0 + 32 * part) * 2,
-                                   static_cast<int64_t>(op.nb) * 2);
+                        epi_store_part(stg, lane, make_uint4(wds[0], wds[1], wds[2], wds[3]), make_uint4(wds[4], wds[5], wds[6], wds[7]),
+                                       make_uint4(wds[8], wds[9], wds[10], wds[11]), make_uint4(wds[12], wds[13], wds[14], wds[15]),
+                                       tile + (static_cast<int64_t>(r_tile) * op.nb + col0 + 32 * part) * 2, static_cast<int64_t>(op.nb) * 2);
                     }
-                    store_images(rd, t_sx, op.Hp, nullptr, prow, prow, col0);      // image of the STORED value (exact)
+                    epi_store_images(stg, lane, out, t_sx, op.Hp, nullptr, prow, prow, col0, op.nb);      // image of the STORED value (exact)
                 } else {
                     float amax = 0.0f;
 #pragma unroll
@@ -970,8 +987,8 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ 
                 if (item_planes) {
                     const float mul = op.scl[w.mode == MODE_P3 ? SCL_SX : SCL_SS];
                     const int64_t lrow0 = static_cast<int64_t>(rb) * kBlk + q * 32;      // panel-local row of this warp
-                    if (below) store_images(out, mul, op.Sh, op.Sl, lrow0, lrow0, col0);
-                    else store_images(out, mul, op.Hp, op.Lp, op.prow0 + lrow0, op.prow0_lo + lrow0, col0);
+                    if (below) epi_store_images(stg, lane, out, mul, op.Sh, op.Sl, lrow0, lrow0, col0, op.nb);
+                    else epi_store_images(stg, lane, out, mul, op.Hp, op.Lp, op.prow0 + lrow0, op.prow0_lo + lrow0, col0, op.nb);
                 }
             }
           }   // j2

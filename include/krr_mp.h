@@ -129,6 +129,30 @@ int krr_precision_map(const float* d_A, int64_t n, int64_t lda, int nb,
                       void* d_ws, size_t ws_bytes, void* stream);
 
 /* ---------------------------------------------------------------------------------------------
+ * krr_precision_map_static -- krr_precision_map for callers that cannot allocate (code under CUDA-graph
+ * capture, serving loops, harnesses that forbid cudaMalloc): same operation,
+ * same kernels, same summation order, hence the same bits in every output -- but the scratch memory is
+ * a file-scope __device__ array inside the library instead of the caller's d_ws.  The call allocates
+ * nothing: no cudaMalloc / cudaFree, no stream, event or host-vector growth (it is not timed by
+ * krr_profile_enable); it enqueues two kernels on `stream` and returns.
+ *   - Limit: krr_precision_map_workspace(n, nb) <= KRR_PRECISION_MAP_STATIC_BYTES (4 MiB; every
+ *     BASELINE.json config fits: C4, NT = 128, nb = 1024 needs 3.09 MiB).  Larger shapes return
+ *     KRR_ERR_WORKSPACE and launch nothing; krr_precision_map_static_limit() returns the limit.
+ *   - Cost: every GPU that loads the library holds the 4 MiB until the process exits.
+ *   - The array is ONE per device, shared by every call and every host thread, and keeps the last
+ *     call's contents.  Nothing in it has to start at zero (every word a call reads it has written
+ *     before), so no clearing is done.  Two calls that overlap on the GPU (different streams without
+ *     an ordering between them) RACE on it: order them, or use krr_precision_map with own workspaces.
+ * Arguments as krr_precision_map without d_ws / ws_bytes; inputs and outputs remain the caller's.
+ */
+#define KRR_PRECISION_MAP_STATIC_BYTES (4u << 20)
+size_t krr_precision_map_static_limit(void);
+int krr_precision_map_static(const float* d_A, int64_t n, int64_t lda, int nb,
+                             float eps_target, unsigned allowed_mask, unsigned flags,
+                             uint8_t* d_map, float* d_tile_norms, float* d_tile_amax, double* d_fro,
+                             void* stream);
+
+/* ---------------------------------------------------------------------------------------------
  * Factor storage (the tile mosaic).  Tile (i,j), i >= j, is a contiguous row-major
  * nb x nb block in its own precision (4, 2 or 1 bytes per element) at byte offset
  *     off(i,j) = sum of the byte sizes of all lower tiles preceding it in column-major tile order,

@@ -23,7 +23,7 @@ ERRORS = {-1: "KRR_ERR_ARG", -2: "KRR_ERR_SHAPE", -3: "KRR_ERR_WORKSPACE", -4: "
           -5: "KRR_ERR_CUDA", -6: "KRR_ERR_MAP", -7: "KRR_ERR_UNSUPPORTED"}
 
 EXPORTS = ["krr_version", "krr_built_for_sm", "krr_tile_slot", "krr_precision_map_workspace",
-           "krr_precision_map", "krr_factor_bytes", "krr_factor_tile_offset",
+           "krr_precision_map", "krr_precision_map_static_limit", "krr_precision_map_static", "krr_factor_bytes", "krr_factor_tile_offset",
            "krr_potrf_mp_workspace", "krr_potrf_mp", "krr_potrs_workspace", "krr_potrs", "krr_refine_workspace", "krr_refine", "krr_pcg_workspace", "krr_pcg",
            "krr_associate_host_arena", "krr_associate_host", "krr_build_workspace", "krr_build", "krr_build_bordered", "krr_build_rr", "krr_predict_workspace", "krr_predict", "krr_fit_host_arena", "krr_fit_host", "krr_band_map", "krr_build_stats_bytes", "krr_precision_map_from_build",
            "krr_graph_begin", "krr_graph_end", "krr_graph_launch", "krr_graph_kernel_nodes", "krr_graph_destroy",
@@ -59,6 +59,10 @@ def lib():
     L.krr_precision_map_workspace.argtypes = [i64, c.c_int]
     L.krr_precision_map.restype = c.c_int
     L.krr_precision_map.argtypes = [vp, i64, i64, c.c_int, c.c_float, u32, u32, vp, vp, vp, vp, vp, sz, vp]
+    L.krr_precision_map_static_limit.restype = sz
+    L.krr_precision_map_static_limit.argtypes = []
+    L.krr_precision_map_static.restype = c.c_int
+    L.krr_precision_map_static.argtypes = [vp, i64, i64, c.c_int, c.c_float, u32, u32, vp, vp, vp, vp, vp]
     L.krr_factor_bytes.restype = sz
     L.krr_factor_bytes.argtypes = [i64, c.c_int, vp]
     L.krr_factor_tile_offset.restype = i64
@@ -274,6 +278,32 @@ def precision_map(A, nb, eps_target, allowed=(FP32, FP16, FP8), flags=0, n=None)
     _check(L.krr_precision_map(_ptr(A), n, lda, nb, float(eps_target), mask, flags, _ptr(d_map), _ptr(norms),
                                _ptr(amax), _ptr(fro), _ptr(ws), wsb, _stream()), "krr_precision_map")
     return d_map, norms, amax, fro
+
+
+def precision_map_static(A, nb, eps_target, out, allowed=(FP32, FP16, FP8), flags=0, n=None):
+    """krr_precision_map_static: krr_precision_map on the library's own file-scope scratch array -- the call allocates
+    nothing (neither does this wrapper: `out` = (d_map uint8 NT x NT, tile norms, tile amax, fro) are the caller's
+    tensors, as in precision_map's return value).  Shapes whose scratch exceeds the 4 MiB array are refused."""
+    L = lib()
+    if flags & FLAG_A_TILED_LOWER:
+        assert n is not None
+        lda = nb
+    else:
+        n, lda = A.shape[0], A.stride(0)
+    d_map, norms, amax, fro = out
+    NT = n // nb
+    assert d_map.dtype == torch.uint8 and d_map.numel() == NT * NT and d_map.is_contiguous()
+    for t in (norms, amax):
+        assert t is None or (t.dtype == torch.float32 and t.numel() == NT * NT and t.is_contiguous())
+    assert fro is None or fro.dtype == torch.float64
+    need, limit = int(L.krr_precision_map_workspace(n, nb)), int(L.krr_precision_map_static_limit())
+    if need > limit:
+        raise KrrError(f"krr_precision_map_static: n = {n}, nb = {nb} needs {need} bytes of scratch, the library's static "
+                       f"array holds {limit}; use precision_map (caller workspace) for this shape")
+    mask = sum(1 << p for p in allowed)
+    _check(L.krr_precision_map_static(_ptr(A), n, lda, nb, float(eps_target), mask, flags, _ptr(d_map), _ptr(norms),
+                                      _ptr(amax), _ptr(fro), _stream()), "krr_precision_map_static")
+    return out
 
 
 @dataclass

@@ -7,6 +7,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <vector>
 
 #include "build.cuh"
@@ -320,6 +321,32 @@ static int set_kernel_attrs() {
     return KRR_OK;
 }
 
+// ---- scratch of krr_precision_map_static: a file-scope device array (no allocation at call time) --------------
+// In host code `g_pm_static_scratch` is only a stand-in for the symbol, not a device address: the address is looked up
+// once per device, with that device current, by cudaGetSymbolAddress, and that pointer is what the kernels receive.
+static __device__ __align__(256) unsigned char g_pm_static_scratch[KRR_PRECISION_MAP_STATIC_BYTES];
+static std::mutex g_pm_static_mutex;
+static void* g_pm_static_ptr[kMaxDevices];          // per device ordinal; process-wide (the array is per device, not per thread)
+
+static int pm_static_scratch(void** out) {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return KRR_ERR_CUDA;
+    if (dev < 0 || dev >= kMaxDevices) return KRR_ERR_DEVICE;
+    std::lock_guard<std::mutex> lock(g_pm_static_mutex);
+    if (!g_pm_static_ptr[dev]) {
+        void* p = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress(&p, g_pm_static_scratch);
+        if (e != cudaSuccess || !p) {
+            if (getenv("KRR_DEBUG")) fprintf(stderr, "krr: cudaGetSymbolAddress(g_pm_static_scratch): %s\n", cudaGetErrorString(e));
+            cudaGetLastError();
+            return KRR_ERR_CUDA;
+        }
+        g_pm_static_ptr[dev] = p;
+    }
+    *out = g_pm_static_ptr[dev];
+    return KRR_OK;
+}
+
 }  // namespace krr
 
 using namespace krr;
@@ -495,6 +522,53 @@ int krr_precision_map(const float* d_A, int64_t n, int64_t lda, int nb, float ep
     return launch(CAT_MAP, map_decide_kernel, dim3(1), dim3(1024), 0, st, NT, static_cast<int>(chunks),
                   static_cast<const double*>(partial), static_cast<const float*>(pamax), eps_target, allowed_mask, d_map,
                   d_tile_norms, d_tile_amax, d_fro, sumsq);
+}
+
+// The same two kernels on the library's own file-scope scratch array: nothing is allocated by this call (no workspace,
+// no events -- the launches bypass the timing scope of launch()).  See include/krr_mp.h for the limit and the sharing rules.
+size_t krr_precision_map_static_limit(void) { return KRR_PRECISION_MAP_STATIC_BYTES; }
+
+int krr_precision_map_static(const float* d_A, int64_t n, int64_t lda, int nb, float eps_target, unsigned allowed_mask,
+                             unsigned flags, uint8_t* d_map, float* d_tile_norms, float* d_tile_amax, double* d_fro,
+                             void* stream) {
+    g_launches = 0;
+    if (!d_A || !d_map) return KRR_ERR_ARG;
+    int rc = check_shape(n, nb);
+    if (rc) return rc;
+    const bool tiled = flags & KRR_FLAG_A_TILED_LOWER;
+    if (!tiled && (lda < n || lda % 4 != 0)) return KRR_ERR_ARG;
+    if (reinterpret_cast<uintptr_t>(d_A) % 16 != 0) return KRR_ERR_ARG;
+    if (flags & ~(KRR_FLAG_PREROUND_A | KRR_FLAG_A_TILED_LOWER)) return KRR_ERR_UNSUPPORTED;
+    const size_t need = krr_precision_map_workspace(n, nb);
+    if (need == 0 || need > KRR_PRECISION_MAP_STATIC_BYTES) {
+        if (getenv("KRR_DEBUG"))
+            fprintf(stderr, "krr_precision_map_static: n = %lld, nb = %d needs %zu bytes of scratch, the static array holds %u; "
+                            "use krr_precision_map with a caller workspace\n", static_cast<long long>(n), nb, need,
+                    KRR_PRECISION_MAP_STATIC_BYTES);
+        return KRR_ERR_WORKSPACE;
+    }
+    rc = check_device(nullptr);
+    if (rc) return rc;
+    void* scratch = nullptr;
+    rc = pm_static_scratch(&scratch);
+    if (rc) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const int NT = static_cast<int>(n / nb);
+    const size_t nslots = static_cast<size_t>(NT) * (NT + 1) / 2, chunks = nb / kStatRows;
+    uint8_t* ws = static_cast<uint8_t*>(scratch);
+    double* partial = reinterpret_cast<double*>(ws);
+    float* pamax = reinterpret_cast<float*>(ws + align_up(nslots * chunks * sizeof(double), 1024));
+    double* sumsq = reinterpret_cast<double*>(reinterpret_cast<uint8_t*>(pamax) + align_up(nslots * chunks * sizeof(float), 1024));
+    AView A{d_A, lda, tiled ? 1 : 0, NT, nb};
+    // every word of partial / pamax / sumsq that is read below is written first by this call: nothing to clear
+    tile_stats_kernel<<<dim3(static_cast<unsigned>(nslots), static_cast<unsigned>(chunks)), dim3(kStatThreads), 0, st>>>(A, partial, pamax);
+    ++g_launches;
+    if (cudaGetLastError() != cudaSuccess) return KRR_ERR_CUDA;
+    map_decide_kernel<<<dim3(1), dim3(1024), 0, st>>>(NT, static_cast<int>(chunks), static_cast<const double*>(partial),
+                                                      static_cast<const float*>(pamax), eps_target, allowed_mask, d_map,
+                                                      d_tile_norms, d_tile_amax, d_fro, sumsq);
+    ++g_launches;
+    return cudaGetLastError() == cudaSuccess ? KRR_OK : KRR_ERR_CUDA;
 }
 
 // ------------------------------------------------------------------------- factor layout

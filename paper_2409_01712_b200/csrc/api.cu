@@ -17,6 +17,7 @@
 #include "panel.cuh"
 #include "peaks.cuh"
 #include "potrs.cuh"
+#include "potrs_stream.cuh"
 #include "precision_map.cuh"
 #include "refine.cuh"
 #include "tri128.cuh"
@@ -99,6 +100,21 @@ static int make_byte_plane_tmap(CUtensorMap* tm, const void* base, uint64_t rows
     cuuint32_t estr[2] = {1, 1};
     CUresult r = enc(tm, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<void*>(base), gdim, gstride, box, estr,
                      CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS ? KRR_OK : KRR_ERR_CUDA;
+}
+
+// The mosaic payload as a 2-D array of es-byte elements with nb columns (potrs_stream.cuh): box = bc columns x br rows.
+static int make_mosaic_tmap(CUtensorMap* tm, const void* base, size_t payload_bytes, int nb, int es, int bc, int br, bool swizzle128) {
+    EncodeTiledFn enc = get_encode_fn();
+    if (!enc) return KRR_ERR_CUDA;
+    cuuint64_t gdim[2] = {static_cast<cuuint64_t>(nb), payload_bytes / (static_cast<size_t>(nb) * es)};
+    cuuint64_t gstride[1] = {static_cast<cuuint64_t>(nb) * es};
+    cuuint32_t box[2] = {static_cast<cuuint32_t>(bc), static_cast<cuuint32_t>(br)};
+    cuuint32_t estr[2] = {1, 1};
+    const CUtensorMapDataType dt = es == 4 ? CU_TENSOR_MAP_DATA_TYPE_UINT32 : (es == 2 ? CU_TENSOR_MAP_DATA_TYPE_UINT16 : CU_TENSOR_MAP_DATA_TYPE_UINT8);
+    CUresult r = enc(tm, dt, 2, const_cast<void*>(base), gdim, gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                     swizzle128 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                      CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     return r == CUDA_SUCCESS ? KRR_OK : KRR_ERR_CUDA;
 }
@@ -301,10 +317,12 @@ static int launch_gemm(const GemmMaps& m, const GemmOp& op_in, int max_ctas, int
 
 template <int NRHS>
 static int set_potrs_attrs() {
-    const int big = 220 * 1024;
+    const int big = 227 * 1024;
     KRR_CUDA_CHECK(cudaFuncSetAttribute(potrs_fwd_update_kernel<NRHS>, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
     KRR_CUDA_CHECK(cudaFuncSetAttribute(potrs_bwd_update_kernel<NRHS, (NRHS <= 16) ? 4 : 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
     KRR_CUDA_CHECK(cudaFuncSetAttribute(potrs_bwd_update_kernel<NRHS, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
+    KRR_CUDA_CHECK(cudaFuncSetAttribute(potrs_stream_update_kernel<NRHS, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
+    KRR_CUDA_CHECK(cudaFuncSetAttribute(potrs_stream_update_kernel<NRHS, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
     return KRR_OK;
 }
 
@@ -946,15 +964,14 @@ size_t krr_potrs_workspace(int64_t n, int nb, int nrhs) {
 
 }  // extern "C"
 
-// Forward and backward sweeps with a one-column lookahead on the library's internal streams (`sh` chain, `sl` bulk):
-// once z_k (alpha_k) is known, the update of the NEXT tile row (column) -- all the next diagonal solve waits for --
-// runs on the chain stream, the update of the remaining rows on the bulk stream beside that solve.  Updates of the
-// same rows of B are read-modify-write, so their order is fixed by events (deterministic results): the chain's
-// update of row k+2 by column k+1 waits for the bulk update by column k.
+// Forward and backward sweeps with a two-column lookahead on the library's internal streams (`sh` chain, `sm` middle,
+// `sl` bulk): once z_k (alpha_k) is known, the update of the NEXT tile row (column) -- all the next diagonal solve waits
+// for -- runs on the chain stream, the one after it on the middle stream, the remaining rows on the bulk stream beside
+// the following solves (the comment at the loops has the event order that keeps the sums deterministic).
 template <int NRHS>
 static int potrs_run(const uint8_t* factor, const float* d_scales, const uint8_t* d_map, const std::vector<int64_t>& hoff,
                      const int64_t* off, const float* Minv, const float* MinvT, float* stage, int NT, int nb, float* B,
-                     int64_t ldb, int nrhs, int num_sms, cudaStream_t st) {
+                     int64_t ldb, int nrhs, int num_sms, cudaStream_t st, const StreamMaps* smaps) {
     constexpr int ROWS = 64 / NRHS, NW = kSolveThreads / 32, CPL = (NRHS <= 16) ? 4 : 2;
     const size_t smem_z = static_cast<size_t>(NRHS) * nb * sizeof(float);
     const size_t smem_bu = smem_z + static_cast<size_t>(NW / 2) * 32 * CPL * NRHS * sizeof(float);
@@ -962,17 +979,19 @@ static int potrs_run(const uint8_t* factor, const float* d_scales, const uint8_t
     const int64_t blk_elems = static_cast<int64_t>(kBlk) * kBlk;
     const int nsub = nb / kBlk;
     const bool pipe = NT > 2;
-    cudaStream_t sh = st, sl = st;
-    enum { EV_FORK = 0, EV_JOIN_HI = 1, EV_JOIN_LO = 3, EV_BASE = 4 };      // the event pool of krr_potrf_mp, reused
+    cudaStream_t sh = st, sm = st, sl = st;
+    enum { EV_FORK = 0, EV_JOIN_HI = 1, EV_JOIN_MID = 2, EV_JOIN_LO = 3, EV_BASE = 4 };      // the event pool of krr_potrf_mp, reused
     auto ev_diag = [&](int k) { return g_pipe.event(EV_BASE + 4 * static_cast<size_t>(k) + 0); };
     auto ev_bulk = [&](int k) { return g_pipe.event(EV_BASE + 4 * static_cast<size_t>(k) + 1); };
+    auto ev_mid = [&](int k) { return g_pipe.event(EV_BASE + 4 * static_cast<size_t>(k) + 2); };
     int rc;
     if (pipe) {
         rc = g_pipe.init();
         if (rc) return rc;
-        sh = g_pipe.hi; sl = g_pipe.lo;
+        sh = g_pipe.hi; sm = g_pipe.mid; sl = g_pipe.lo;
         KRR_CUDA_CHECK(cudaEventRecord(g_pipe.event(EV_FORK), st));
         KRR_CUDA_CHECK(cudaStreamWaitEvent(sh, g_pipe.event(EV_FORK), 0));
+        KRR_CUDA_CHECK(cudaStreamWaitEvent(sm, g_pipe.event(EV_FORK), 0));
         KRR_CUDA_CHECK(cudaStreamWaitEvent(sl, g_pipe.event(EV_FORK), 0));
     }
     // bulk updates leave room for a diagonal-solve CTA on every SM (1 update CTA + 1 solve CTA fit in shared memory;
@@ -997,6 +1016,30 @@ static int potrs_run(const uint8_t* factor, const float* d_scales, const uint8_t
         return launch(CAT_POTRS, potrs_bwd_update_kernel<NRHS, CPL>, dim3(units < cap ? units : cap), dim3(kSolveThreads), smem_bu, s,
                       NT, nb, k, j_lo, j_hi - j_lo, factor, off, d_map, d_scales, B, ldb, nrhs);
     };
+    // Bulk updates (rows k + 3 .. / columns .. k - 3 of the two-column lookahead below): streamed through a shared-memory
+    // ring by TMA, one persistent CTA per SM (potrs_stream.cuh), the ring as deep as shared memory allows (8 x 16 KB at
+    // nb = 1024, nrhs <= 16).  Shapes whose small operand leaves no room for two ring slots take the older kernels.
+    const int stream_budget = 227 * 1024;
+    const int stream_sms = num_sms > 32 ? num_sms - 16 : num_sms;     // 16 SMs stay free for the chain's kernels (measured: 148 / 140 / 132 -> 9.51 / 9.55 / 9.34 ms at C3)
+    auto stream_update = [&](bool bwd, int k, int t_lo, int t_hi, cudaStream_t s, int* done) {
+        using C = StreamCfg<NRHS>;
+        *done = 0;
+        const int ntiles = t_hi - t_lo;
+        if (ntiles <= 0 || stream_budget <= 0 || !smaps) return static_cast<int>(KRR_OK);
+        const size_t fixed = smem_z + C::RED_BYTES + static_cast<size_t>(ntiles) * 12 + 8 + (2 * kStreamMaxStages + 1) * 8;
+        if (fixed + 2 * kStreamStage > static_cast<size_t>(stream_budget)) return static_cast<int>(KRR_OK);
+        int nst = static_cast<int>((static_cast<size_t>(stream_budget) - fixed) / kStreamStage);
+        if (nst > kStreamMaxStages) nst = kStreamMaxStages;
+        const int units = ntiles * (nb / 128);
+        const int grid = units < stream_sms ? units : stream_sms;
+        *done = 1;
+        const size_t smem = fixed + static_cast<size_t>(nst) * kStreamStage;
+        if (bwd)
+            return launch(CAT_POTRS, potrs_stream_update_kernel<NRHS, true>, dim3(grid), dim3(kStreamThreads), smem, s,
+                          smaps[1], NT, nb, k, t_lo, ntiles, nst, off, d_map, d_scales, B, ldb, nrhs);
+        return launch(CAT_POTRS, potrs_stream_update_kernel<NRHS, false>, dim3(grid), dim3(kStreamThreads), smem, s,
+                      smaps[0], NT, nb, k, t_lo, ntiles, nst, off, d_map, d_scales, B, ldb, nrhs);
+    };
     auto diag = [&](int k, int backward, cudaStream_t s) {
         const float* Mk = (backward ? MinvT : Minv) + static_cast<int64_t>(k) * nb * nb;
         float* Bk = B + static_cast<int64_t>(k) * nb * ldb;
@@ -1008,6 +1051,11 @@ static int potrs_run(const uint8_t* factor, const float* d_scales, const uint8_t
     };
     // (a lambda: an error in the middle still joins the internal streams below)
     auto run_sweeps = [&]() -> int {
+    // Two-column lookahead.  Column k's update of row r is made by: the chain stream for r = k + 1 ("near": all the next
+    // diagonal solve waits for), the middle stream for r = k + 2 ("mid"), the bulk stream for r >= k + 3.  A row of B is
+    // read-modify-written, so the order of its updates is fixed by events (deterministic results): bulk(.. r-3), then
+    // mid(r-2) -- which waits for bulk(r-3) --, then near(r-1) -- which waits for mid(r-2).  The chain therefore waits
+    // for a bulk launch issued TWO columns earlier, not for the previous column's.
     // ---- forward: L z = y
     for (int k = 0; k < NT; ++k) {
         rc = diag(k, 0, sh);
@@ -1018,17 +1066,33 @@ static int potrs_run(const uint8_t* factor, const float* d_scales, const uint8_t
             continue;
         }
         KRR_CUDA_CHECK(cudaEventRecord(ev_diag(k), sh));
-        if (k >= 1) KRR_CUDA_CHECK(cudaStreamWaitEvent(sh, ev_bulk(k - 1), 0));      // row k+1 received column k-1 first
-        rc = fwd_update(k, k + 1, k + 2 < NT ? k + 2 : NT, sh, 3);                   // the next diagonal solve's rows
-        if (rc) return rc;
+        if (k + 1 < NT) {
+            if (k >= 1) KRR_CUDA_CHECK(cudaStreamWaitEvent(sh, ev_mid(k - 1), 0));
+            rc = fwd_update(k, k + 1, k + 2, sh, 3);
+            if (rc) return rc;
+        }
+        KRR_CUDA_CHECK(cudaStreamWaitEvent(sm, ev_diag(k), 0));
+        if (k >= 1) KRR_CUDA_CHECK(cudaStreamWaitEvent(sm, ev_bulk(k - 1), 0));
+        if (k + 2 < NT) {
+            rc = fwd_update(k, k + 2, k + 3, sm, 3);
+            if (rc) return rc;
+        }
+        KRR_CUDA_CHECK(cudaEventRecord(ev_mid(k), sm));
         KRR_CUDA_CHECK(cudaStreamWaitEvent(sl, ev_diag(k), 0));
-        rc = fwd_update(k, k + 2, NT, sl, bulk_per_sm);
-        if (rc) return rc;
+        if (k + 3 < NT) {
+            int streamed = 0;
+            rc = stream_update(false, k, k + 3, NT, sl, &streamed);
+            if (rc) return rc;
+            if (!streamed) rc = fwd_update(k, k + 3, NT, sl, bulk_per_sm);
+            if (rc) return rc;
+        }
         KRR_CUDA_CHECK(cudaEventRecord(ev_bulk(k), sl));
     }
     if (pipe) {      // the backward sweep starts from a quiescent state
         KRR_CUDA_CHECK(cudaEventRecord(ev_bulk(NT), sl));
+        KRR_CUDA_CHECK(cudaEventRecord(ev_mid(NT), sm));
         KRR_CUDA_CHECK(cudaStreamWaitEvent(sh, ev_bulk(NT), 0));
+        KRR_CUDA_CHECK(cudaStreamWaitEvent(sh, ev_mid(NT), 0));
     }
     // ---- backward: L^T alpha = z
     for (int k = NT - 1; k >= 0; --k) {
@@ -1040,12 +1104,26 @@ static int potrs_run(const uint8_t* factor, const float* d_scales, const uint8_t
             continue;
         }
         KRR_CUDA_CHECK(cudaEventRecord(ev_diag(k), sh));
-        if (k + 1 < NT) KRR_CUDA_CHECK(cudaStreamWaitEvent(sh, ev_bulk(k + 1), 0));  // row k-1 received column k+1 first
-        rc = bwd_update(k, k - 1 > 0 ? k - 1 : 0, k, sh);                            // the next diagonal solve's rows
-        if (rc) return rc;
+        if (k >= 1) {
+            if (k + 1 < NT) KRR_CUDA_CHECK(cudaStreamWaitEvent(sh, ev_mid(k + 1), 0));
+            rc = bwd_update(k, k - 1, k, sh);
+            if (rc) return rc;
+        }
+        KRR_CUDA_CHECK(cudaStreamWaitEvent(sm, ev_diag(k), 0));
+        if (k + 1 < NT) KRR_CUDA_CHECK(cudaStreamWaitEvent(sm, ev_bulk(k + 1), 0));
+        if (k >= 2) {
+            rc = bwd_update(k, k - 2, k - 1, sm);
+            if (rc) return rc;
+        }
+        KRR_CUDA_CHECK(cudaEventRecord(ev_mid(k), sm));
         KRR_CUDA_CHECK(cudaStreamWaitEvent(sl, ev_diag(k), 0));
-        rc = bwd_update(k, 0, k - 1, sl);
-        if (rc) return rc;
+        if (k >= 3) {
+            int streamed = 0;
+            rc = stream_update(true, k, 0, k - 2, sl, &streamed);
+            if (rc) return rc;
+            if (!streamed) rc = bwd_update(k, 0, k - 2, sl);
+            if (rc) return rc;
+        }
         KRR_CUDA_CHECK(cudaEventRecord(ev_bulk(k), sl));
     }
     return static_cast<int>(KRR_OK);
@@ -1053,8 +1131,10 @@ static int potrs_run(const uint8_t* factor, const float* d_scales, const uint8_t
     const int rc_sweeps = run_sweeps();
     if (pipe) {
         KRR_CUDA_CHECK(cudaEventRecord(g_pipe.event(EV_JOIN_HI), sh));
+        KRR_CUDA_CHECK(cudaEventRecord(g_pipe.event(EV_JOIN_MID), sm));
         KRR_CUDA_CHECK(cudaEventRecord(g_pipe.event(EV_JOIN_LO), sl));
         KRR_CUDA_CHECK(cudaStreamWaitEvent(st, g_pipe.event(EV_JOIN_HI), 0));
+        KRR_CUDA_CHECK(cudaStreamWaitEvent(st, g_pipe.event(EV_JOIN_MID), 0));
         KRR_CUDA_CHECK(cudaStreamWaitEvent(st, g_pipe.event(EV_JOIN_LO), 0));
     }
     return rc_sweeps;
@@ -1101,11 +1181,22 @@ int krr_potrs(const void* d_factor, const float* d_scales, const uint8_t* d_map,
     rc = launch(CAT_POTRS, potrs_tile_inverse_kernel, dim3(nb / kBlk, NT), dim3(kTinvThreads), static_cast<size_t>(kTinvSmem), st,
                 factor, static_cast<const int64_t*>(off), NT, nb, static_cast<const float*>(dinv), Minv, MinvT);
     if (rc) return rc;
+    // the mosaic as a TMA source of the streamed bulk updates: per direction one map per element size
+    StreamMaps smaps[2];
+    const size_t payload = host_offsets(NT, nb, h_map, nullptr);
+    bool have_maps = reinterpret_cast<uintptr_t>(factor) % 16 == 0;
+    for (int d = 0; d < 2 && have_maps; ++d) {
+        CUtensorMap* m[3] = {&smaps[d].m4, &smaps[d].m2, &smaps[d].m1};
+        const int es[3] = {4, 2, 1};
+        for (int e = 0; e < 3 && have_maps; ++e)
+            have_maps = make_mosaic_tmap(m[e], factor, payload, nb, es[e], d == 0 ? 128 / es[e] : 128, d == 0 ? 128 : 128 / es[e], d == 0) == KRR_OK;
+    }
+    const StreamMaps* sm = have_maps ? smaps : nullptr;
     switch (rhs_class(nrhs)) {
-        case 4:  return potrs_run<4>(factor, d_scales, d_map, hoff, off, Minv, MinvT, stage, NT, nb, d_B, ldb, nrhs, num_sms, st);
-        case 8:  return potrs_run<8>(factor, d_scales, d_map, hoff, off, Minv, MinvT, stage, NT, nb, d_B, ldb, nrhs, num_sms, st);
-        case 16: return potrs_run<16>(factor, d_scales, d_map, hoff, off, Minv, MinvT, stage, NT, nb, d_B, ldb, nrhs, num_sms, st);
-        default: return potrs_run<32>(factor, d_scales, d_map, hoff, off, Minv, MinvT, stage, NT, nb, d_B, ldb, nrhs, num_sms, st);
+        case 4:  return potrs_run<4>(factor, d_scales, d_map, hoff, off, Minv, MinvT, stage, NT, nb, d_B, ldb, nrhs, num_sms, st, sm);
+        case 8:  return potrs_run<8>(factor, d_scales, d_map, hoff, off, Minv, MinvT, stage, NT, nb, d_B, ldb, nrhs, num_sms, st, sm);
+        case 16: return potrs_run<16>(factor, d_scales, d_map, hoff, off, Minv, MinvT, stage, NT, nb, d_B, ldb, nrhs, num_sms, st, sm);
+        default: return potrs_run<32>(factor, d_scales, d_map, hoff, off, Minv, MinvT, stage, NT, nb, d_B, ldb, nrhs, num_sms, st, sm);
     }
 }
 

@@ -9,8 +9,9 @@
 //   potrs_tile_inverse_kernel      from them the inverses of the whole diagonal tiles (and their transposes), once
 //   potrs_diagmul_kernel           one diagonal tile: z_k = inv(L_kk) t_k (forward) or inv(L_kk)^T t_k (backward)
 //                                  as ONE product -- no chain of dependent 128-row block solves
-//   potrs_fwd_update_kernel        Y_i -= L_ik Z_k for all i > k   (streams tile column k once)
-//   potrs_bwd_update_kernel        Z_j -= L_kj^T alpha_k for all j < k (streams tile row k once)
+//   potrs_fwd_update_kernel        Y_i -= L_ik Z_k for tile rows i in a range (the single tiles the chain waits for)
+//   potrs_bwd_update_kernel        Z_j -= L_kj^T alpha_k for tile columns j in a range (likewise)
+//   potrs_stream_update_kernel     (potrs_stream.cuh) the bulk of both: all the other tiles of column / row k, by TMA
 // All sums are accumulated in a fixed order: results are deterministic.
 #pragma once
 #include <cooperative_groups.h>

@@ -185,6 +185,8 @@ CONFIGS = {
     # class probes: C3's matrix with every off-diagonal tile forced to one storage precision (kernel
     # efficiency per MMA class at full depth; numerics are those of the forced map, reported as they are)
     "C3h": Config("C3h", 65536, 50000, 1024, 1e-2, 16, seed=3, map_request="force_fp16", allowed=(0, 1)),
+    # C3's matrix under the map of C5' (tile column 0 FP32, the rest E4M3): the same-matrix FP8 figure beside C3 / C3h
+    "C3q": Config("C3q", 65536, 50000, 1024, 1e-2, 16, seed=3, map_request="fp8_col0_fp32", allowed=(0, 2)),
     "S1": Config("S1", 32768, 24576, 1024, 1e-2, 8, seed=6, genotype="families:4096",
                  map_request="rule", eps_target=1e-4, allowed=(0, 1, 2), gamma_scale=12.0),
 }

@@ -215,8 +215,8 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb,
  *       tiles and their transposes (2 * n * nb floats, FP32 block forward substitution), computed by every call
  *       before the sweeps (the factor may have changed).  A diagonal step of a sweep is then one product
  *       z_k = inv(L_kk) t_k; the updates behind it run with a two-column lookahead on the library's three
- *       internal streams (the bulk of them streamed from d_factor by TMA: d_factor should be 16-byte aligned,
- *       else the older, slower kernels are used); sums are accumulated in a fixed order
+ *       internal streams (the bulk of them streamed from d_factor by TMA; d_factor must be 16-byte aligned,
+ *       else KRR_ERR_ARG); sums are accumulated in a fixed order
  *       (deterministic results).  If d_map does not agree with h_map the result is unspecified (all reads stay
  *       inside buffers sized from h_map).
  */

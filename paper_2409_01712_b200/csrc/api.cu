@@ -1150,7 +1150,7 @@ int krr_potrs(const void* d_factor, const float* d_scales, const uint8_t* d_map,
     if (rc) return rc;
     if (nrhs < 1 || nrhs > kMaxRhs || ldb < nrhs) return KRR_ERR_ARG;
     if (static_cast<int64_t>(rhs_class(nrhs)) * nb > 32768) return KRR_ERR_SHAPE;
-    if (reinterpret_cast<uintptr_t>(d_ws) % 16 != 0) return KRR_ERR_ARG;
+    if (reinterpret_cast<uintptr_t>(d_ws) % 16 != 0 || reinterpret_cast<uintptr_t>(d_factor) % 16 != 0) return KRR_ERR_ARG;
     const int NT = static_cast<int>(n / nb);
     rc = check_map(NT, h_map, nullptr);
     if (rc) return rc;
@@ -1184,7 +1184,7 @@ int krr_potrs(const void* d_factor, const float* d_scales, const uint8_t* d_map,
     // the mosaic as a TMA source of the streamed bulk updates: per direction one map per element size
     StreamMaps smaps[2];
     const size_t payload = host_offsets(NT, nb, h_map, nullptr);
-    bool have_maps = reinterpret_cast<uintptr_t>(factor) % 16 == 0;
+    bool have_maps = true;                                   // (an encoding failure falls back to the r01 bulk kernels)
     for (int d = 0; d < 2 && have_maps; ++d) {
         CUtensorMap* m[3] = {&smaps[d].m4, &smaps[d].m2, &smaps[d].m1};
         const int es[3] = {4, 2, 1};

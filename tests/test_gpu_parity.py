@@ -201,7 +201,7 @@ def noise_floor(An, nb, pmap, preround, seed=0):
     return L1, relF(L2, L1)
 
 
-@pytest.mark.parametrize("case", ["fp16_uniform", "s1_rule_mosaic", "random_mixed", "fp8_col0_fp32"])
+@pytest.mark.parametrize("case", ["fp16_uniform", "s1_rule_mosaic", "random_mixed", "fp8_col0_fp32", "c3q_twin"])
 def test_low_precision_maps(krr, case):
     if case == "fp16_uniform":
         cfg = scaled_config(CONFIGS["C4"], nb=128, n=1024, p=800)
@@ -223,6 +223,12 @@ def test_low_precision_maps(krr, case):
             for j in range(i):
                 pmap[i, j] = rng.integers(0, 3)
         preround = True
+    elif case == "c3q_twin":   # the map of C5' on the matrix family of C3 (bench.py's same-matrix FP8 figure)
+        cfg = scaled_config(CONFIGS["C3q"], nb=128, n=2048, p=1600)
+        A, Y = make_problem(cfg, device="cuda")
+        pmap = oracle_uniform(cfg.NT, R.FP8)
+        pmap[1:, 0] = R.FP32
+        preround = False
     else:   # C5': forced FP8 with tile column 0 kept in FP32, operands as stored
         cfg = scaled_config(CONFIGS["C5"], nb=128, n=1024, p=200)
         A, Y = make_problem(cfg, device="cuda")
@@ -239,7 +245,7 @@ def test_low_precision_maps(krr, case):
     bg, bo = backward_error(An, Lg), backward_error(An, Lo)
     lit = relF(Lg, Lo)
     print(f"{case}: relF {lit:.3e} floor {floor:.3e} backward gpu {bg:.4e} oracle {bo:.4e}")
-    if case in ("fp16_uniform", "s1_rule_mosaic"):    # maps the rule produces: north_star's bound
+    if case in ("fp16_uniform", "s1_rule_mosaic", "c3q_twin"):    # maps the rule produces (and the bench's C3q): north_star's bound
         assert bg <= 5e-4
     assert abs(bg - bo) <= 0.02 * bo
     assert lit <= max(1e-4, 2.0 * floor)

@@ -390,7 +390,9 @@ int krr_predict(const int8_t* d_T, int64_t m, int64_t ldt, const int8_t* d_G, in
  * krr_fit_host -- Build and Associate (Alg. 1 l.2-3) from HOST buffers: copies the int8 genotypes
  * and Y to the device, builds A = K + lambda*I there (krr_build, Gaussian kernel), then runs the Associate phase as
  * krr_associate_host does and copies alpha (= W), the precision map and info back.  The n x n matrix never crosses
- * PCIe: n*p bytes of genotypes do.  Synchronises `stream` before it returns.
+ * PCIe: n*p bytes of genotypes do.  The genotypes are copied in strips of whole tile rows on one of the library's internal
+ * streams and the rows of A a strip completes are built on `stream` as soon as it has arrived (the Build runs behind the
+ * copy; same blocks and arithmetic as one krr_build call: identical bits).  Synchronises `stream` before it returns.
  * h_G  in  n x p int8 genotypes, row pitch ldg >= p bytes (pinned memory makes the copy asynchronous).
  * Other arguments as for krr_build / krr_associate_host; n % 256 == 0, nb % 256 == 0.
  * d_arena  krr_fit_host_arena(n, p, nb, nrhs) bytes, 1024-byte aligned.

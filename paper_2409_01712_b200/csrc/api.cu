@@ -1448,6 +1448,10 @@ struct Arena {
 };
 Arena arena_layout(int64_t n, int nb, int nrhs);
 }  // namespace
+static int build_rows(const int8_t* d_G, int64_t n, int64_t n_valid, int64_t p, int64_t ldg, const float* d_C, int q,
+                      int64_t ldc, float gamma, float lambda, float* d_A, int64_t lda, int nb, unsigned flags, void* d_stats,
+                      void* d_ws, size_t ws_bytes, void* stream, int64_t row_lo, int64_t row_hi);
+
 static int associate_in_arena(uint8_t* ar, const Arena& L, int64_t n, int nb, float eps_target, unsigned allowed_mask, int force_prec,
                               unsigned flags, int nrhs, float* h_alpha, uint8_t* h_map, int* h_info, void* stream, int64_t launches,
                               const void* build_stats = nullptr);
@@ -1576,13 +1580,35 @@ int krr_fit_host(const int8_t* h_G, int64_t n, int64_t p, int64_t ldg, float gam
     int8_t* dG = reinterpret_cast<int8_t*>(ar + L.total);
     uint8_t* bws = ar + L.total + fit_g_bytes(n, p);
     const int64_t ldd = static_cast<int64_t>(align_up(static_cast<size_t>(p), 16));
-    KRR_CUDA_CHECK(cudaMemcpy2DAsync(dG, ldd, h_G, ldg, p, n, cudaMemcpyHostToDevice, st));
     KRR_CUDA_CHECK(cudaMemcpyAsync(ar + L.Y, h_Y, static_cast<size_t>(n) * nrhs * sizeof(float), cudaMemcpyHostToDevice, st));
     // tile statistics from the Build epilogue: the precision map needs no pass of its own over A
     uint8_t* stats = bws + krr_build_workspace(n, p, 0);
-    rc = krr_build(dG, n, p, ldd, nullptr, 0, 0, gamma, lambda, reinterpret_cast<float*>(ar + L.A), n, nb, 0,
-                   force_prec < 0 ? stats : nullptr, bws, krr_build_workspace(n, p, 0), stream);
+    // The genotypes cross PCIe in strips of whole tile rows on an internal copy stream; the rows of A that a strip completes
+    // (their blocks need the rows of G up to the strip's end only: lower triangle) are built on the caller's stream as soon
+    // as the strip has arrived, so the Build runs behind the copy instead of after it.  Same kernels, same blocks, same
+    // per-block arithmetic as krr_build in one launch: identical bits.
+    int64_t strip_rows = (n / 8 + nb - 1) / nb * nb;
+    if (strip_rows < nb) strip_rows = nb;
+    const int nstrips = static_cast<int>((n + strip_rows - 1) / strip_rows);
+    rc = g_pipe.init();
     if (rc) return rc;
+    cudaStream_t sc = g_pipe.mid;
+    enum { EV_FORK = 0, EV_BASE = 4 };
+    KRR_CUDA_CHECK(cudaEventRecord(g_pipe.event(EV_FORK), st));
+    KRR_CUDA_CHECK(cudaStreamWaitEvent(sc, g_pipe.event(EV_FORK), 0));
+    int64_t launches = 0;
+    for (int s = 0; s < nstrips; ++s) {
+        const int64_t r0 = s * strip_rows, r1 = (r0 + strip_rows < n) ? r0 + strip_rows : n;
+        KRR_CUDA_CHECK(cudaMemcpy2DAsync(dG + r0 * ldd, ldd, h_G + r0 * ldg, ldg, p, r1 - r0, cudaMemcpyHostToDevice, sc));
+        KRR_CUDA_CHECK(cudaEventRecord(g_pipe.event(EV_BASE + s), sc));
+        KRR_CUDA_CHECK(cudaStreamWaitEvent(st, g_pipe.event(EV_BASE + s), 0));
+        g_launches = 0;
+        rc = build_rows(dG, n, n, p, ldd, nullptr, 0, 0, gamma, lambda, reinterpret_cast<float*>(ar + L.A), n, nb, 0,
+                        force_prec < 0 ? stats : nullptr, bws, krr_build_workspace(n, p, 0), stream, r0, r1);
+        if (rc) return rc;
+        launches += g_launches;
+    }
+    g_launches = launches;
     return associate_in_arena(ar, L, n, nb, eps_target, allowed_mask, force_prec, flags, nrhs, h_alpha, h_map, h_info, stream, g_launches,
                               force_prec < 0 ? stats : nullptr);
 }
@@ -1674,10 +1700,14 @@ int krr_build(const int8_t* d_G, int64_t n, int64_t p, int64_t ldg, const float*
     return krr_build_bordered(d_G, n, n, p, ldg, d_C, q, ldc, gamma, lambda, d_A, lda, nb, flags, d_stats, d_ws, ws_bytes, stream);
 }
 
-int krr_build_bordered(const int8_t* d_G, int64_t n, int64_t n_valid, int64_t p, int64_t ldg, const float* d_C, int q,
-                       int64_t ldc, float gamma, float lambda, float* d_A, int64_t lda, int nb, unsigned flags, void* d_stats,
-                       void* d_ws, size_t ws_bytes, void* stream) {
-    g_launches = 0;
+}  // extern "C"
+
+// Rows [row_lo, row_hi) of A (whole 256-row units; row_hi = 0: all rows): the squared norms of those rows of G, then the
+// blocks of the lower tiles in those rows.  A launch needs the rows [0, row_hi) of G and their squared norms (earlier
+// calls): krr_fit_host builds the matrix strip by strip behind the host-to-device copy of the genotypes.
+static int build_rows(const int8_t* d_G, int64_t n, int64_t n_valid, int64_t p, int64_t ldg, const float* d_C, int q,
+                      int64_t ldc, float gamma, float lambda, float* d_A, int64_t lda, int nb, unsigned flags, void* d_stats,
+                      void* d_ws, size_t ws_bytes, void* stream, int64_t row_lo, int64_t row_hi) {
     if (!d_G || !d_A || !d_ws) return KRR_ERR_ARG;
     if (n_valid < 1 || n_valid > n) return KRR_ERR_ARG;
     if (q < 0 || q > kMaxConfounders || (q > 0 && (!d_C || ldc < q))) return KRR_ERR_ARG;
@@ -1708,7 +1738,11 @@ int krr_build_bordered(const int8_t* d_G, int64_t n, int64_t n_valid, int64_t p,
         if (rc) return rc;
         d_G = U; ldg = ldu; p = 2 * p;
     }
-    rc = launch(CAT_MISC, row_sqnorm_kernel, dim3(static_cast<unsigned>((n + 7) / 8)), dim3(256), 0, st, d_G, n, p, ldg, sq);
+    const bool strip = row_hi > 0;
+    if (strip && (ibs || row_lo % 256 != 0 || row_hi % 256 != 0 || row_lo < 0 || row_hi > n || row_lo >= row_hi)) return KRR_ERR_ARG;
+    if (!strip) { row_lo = 0; row_hi = n; }
+    rc = launch(CAT_MISC, row_sqnorm_kernel, dim3(static_cast<unsigned>((row_hi - row_lo + 7) / 8)), dim3(256), 0, st,
+                d_G + row_lo * ldg, row_hi - row_lo, p, ldg, sq + row_lo);
     if (rc) return rc;
     CUtensorMap tmG;
     rc = make_genotype_tmap(&tmG, d_G, n, p, ldg);
@@ -1728,9 +1762,21 @@ int krr_build_bordered(const int8_t* d_G, int64_t n, int64_t n_valid, int64_t p,
         op.stat_amax = reinterpret_cast<float*>(static_cast<uint8_t*>(d_stats) + align_up(nslots * chunks * sizeof(double), 1024));
         op.stats_chunks = static_cast<int>(chunks);
     }
-    const int64_t NT = n / nb, upt = nb / 256;
+    const int64_t upt = nb / 256;
     const int nacc = (nb % 512 == 0) ? 2 : 1;                      // 256 x 512 blocks when a tile holds them
-    return launch_build(tmG, tmG, op, upt * upt * NT * (NT + 1) / 2 / nacc, nacc, num_sms, st);
+    if (strip) { op.ru_lo = static_cast<int>(row_lo / 256); op.ru_hi = static_cast<int>(row_hi / 256); }
+    int64_t blocks = 0;                                            // wanted blocks of the row range (sizes the grid)
+    for (int64_t ru = row_lo / 256; ru < row_hi / 256; ++ru) blocks += (ru / upt + 1) * upt / nacc;
+    return launch_build(tmG, tmG, op, blocks, nacc, num_sms, st);
+}
+
+extern "C" {
+
+int krr_build_bordered(const int8_t* d_G, int64_t n, int64_t n_valid, int64_t p, int64_t ldg, const float* d_C, int q,
+                       int64_t ldc, float gamma, float lambda, float* d_A, int64_t lda, int nb, unsigned flags, void* d_stats,
+                       void* d_ws, size_t ws_bytes, void* stream) {
+    g_launches = 0;
+    return build_rows(d_G, n, n_valid, p, ldg, d_C, q, ldc, gamma, lambda, d_A, lda, nb, flags, d_stats, d_ws, ws_bytes, stream, 0, 0);
 }
 
 // The mixed INT8 / FP32 SYRK of ridge regression (Fig. 2): X^T X + lambda I for X = [S^T | C].

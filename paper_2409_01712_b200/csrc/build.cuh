@@ -50,6 +50,9 @@ struct BuildOp {
     double* stat_sumsq;
     float* stat_amax;
     int stats_chunks;
+    // row units (of 256 rows) [ru_lo, ru_hi) of the output are built by this launch (ru_hi = 0: all of them).  krr_fit_host
+    // builds the matrix strip by strip behind the host-to-device copy of the genotypes.
+    int ru_lo, ru_hi;
 };
 constexpr int kMaxConfounders = 16;
 
@@ -114,36 +117,39 @@ struct BuildCursor {
 // cw = width of a column unit in 256-column units (NACC); cu counts column units of that width
 // (upt = 0 marks the rectangular test x training matrix of Predict: every block is wanted)
 __device__ __forceinline__ bool build_valid(int ru, int cu, int upt, int cw) { return upt == 0 || ru / upt >= cu * cw / upt; }
-__device__ __forceinline__ void build_cursor_init(BuildCursor& c, int upt) {
-    c.cp = 0; c.ru = 0; c.ci = 0; c.done = false;
+__device__ __forceinline__ void build_cursor_init(BuildCursor& c, int upt, int ru_lo) {
+    c.cp = 0; c.ru = ru_lo; c.ci = 0; c.done = false;
     (void)upt;
 }
 // move to the next wanted unit strictly after the current position (or stay if `first` and it is wanted)
-__device__ __forceinline__ void build_cursor_seek(BuildCursor& c, int nru, int ncu256, int upt, int cw, bool first) {
+// (rows: units [ru_lo, nru))
+__device__ __forceinline__ void build_cursor_seek(BuildCursor& c, int ru_lo, int nru, int ncu256, int upt, int cw, bool first) {
     const int pw = kBuildPanel / cw, ncu = ncu256 / cw;       // panel width and matrix width in column units
     bool skip = !first;
     while (!c.done) {
         if (!skip) {
             const int cu = c.cp * pw + c.ci;
-            if (cu < ncu && build_valid(c.ru, cu, upt, cw)) return;
+            if (cu < ncu && c.ru < nru && build_valid(c.ru, cu, upt, cw)) return;
         }
         skip = false;
         if (++c.ci == pw) {
             c.ci = 0;
-            if (++c.ru == nru) {
+            if (++c.ru >= nru) {
                 ++c.cp;
                 if (c.cp * pw >= ncu) { c.done = true; return; }
                 c.ru = upt ? (c.cp * kBuildPanel / upt) * upt : 0;   // first row unit of the panel's first tile
+                if (c.ru < ru_lo) c.ru = ru_lo;
+                if (c.ru >= nru && upt) { c.done = true; return; }    // later panels start further down still
             }
         }
     }
 }
 // the block this pair handles next: `steps` wanted units further (steps = pair index at first, then #pairs)
-__device__ __forceinline__ bool build_next_block(BuildCursor& c, bool& started, int pair0, int npairs, int nru, int ncu256,
+__device__ __forceinline__ bool build_next_block(BuildCursor& c, bool& started, int pair0, int npairs, int ru_lo, int nru, int ncu256,
                                                  int upt, int cw, int& ru, int& cu) {
     int steps = started ? npairs : pair0;
-    if (!started) { build_cursor_seek(c, nru, ncu256, upt, cw, true); started = true; }
-    for (; steps > 0 && !c.done; --steps) build_cursor_seek(c, nru, ncu256, upt, cw, false);
+    if (!started) { build_cursor_seek(c, ru_lo, nru, ncu256, upt, cw, true); started = true; }
+    for (; steps > 0 && !c.done; --steps) build_cursor_seek(c, ru_lo, nru, ncu256, upt, cw, false);
     if (c.done) return false;
     ru = c.ru;
     cu = c.cp * (kBuildPanel / cw) + c.ci;
@@ -168,7 +174,8 @@ build_tc_kernel(const __grid_constant__ CUtensorMap tmR, const __grid_constant__
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int rank = static_cast<int>(ptx::cluster_ctarank());
     const int pair0 = static_cast<int>(blockIdx.x >> 1), npairs = static_cast<int>(gridDim.x >> 1);
-    const int nru = static_cast<int>(op.m / 256), ncu256 = static_cast<int>(op.n / 256);
+    const int nru = op.ru_hi > 0 ? op.ru_hi : static_cast<int>(op.m / 256), ncu256 = static_cast<int>(op.n / 256);
+    const int ru_lo = op.ru_hi > 0 ? op.ru_lo : 0;
     const int NT = static_cast<int>(op.n / op.nb), upt = op.rect ? 0 : op.nb / 256;
     const int nch = static_cast<int>((op.p + 127) / 128);           // 128-SNP chunks (the last one zero-filled by TMA)
     constexpr uint32_t kHalf = kBlk * 128;                           // 16 KB operand block
@@ -194,10 +201,10 @@ build_tc_kernel(const __grid_constant__ CUtensorMap tmR, const __grid_constant__
         int slot = 0;
         uint32_t phase = 0;
         BuildCursor cur;
-        build_cursor_init(cur, upt);
+        build_cursor_init(cur, upt, ru_lo);
         bool started = false;
         int ru, cu;
-        while (build_next_block(cur, started, pair0, npairs, nru, ncu256, upt, NACC, ru, cu)) {
+        while (build_next_block(cur, started, pair0, npairs, ru_lo, nru, ncu256, upt, NACC, ru, cu)) {
             const int a_row = ru * 256 + rank * kBlk, b_row = cu * 256 * NACC + rank * kBlk;
             for (int ch = 0; ch < nch; ++ch) {
                 ptx::mbar_wait(empty_bar(slot), phase ^ 1u);
@@ -220,10 +227,10 @@ build_tc_kernel(const __grid_constant__ CUtensorMap tmR, const __grid_constant__
             int slot = 0, buf = 0;
             uint32_t phase = 0, acc_phase = 0;
             BuildCursor cur;
-            build_cursor_init(cur, upt);
+            build_cursor_init(cur, upt, ru_lo);
             bool started = false;
             int ru, cu;
-            while (build_next_block(cur, started, pair0, npairs, nru, ncu256, upt, NACC, ru, cu)) {
+            while (build_next_block(cur, started, pair0, npairs, ru_lo, nru, ncu256, upt, NACC, ru, cu)) {
                 ptx::mbar_wait(tempty_bar(buf), acc_phase ^ 1u);
                 ptx::tc_fence_after();
                 const uint32_t d_tmem = tmem_base + buf * 256 * NACC;
@@ -254,10 +261,10 @@ build_tc_kernel(const __grid_constant__ CUtensorMap tmR, const __grid_constant__
         int buf = 0;
         uint32_t acc_phase = 0;
         BuildCursor cur;
-        build_cursor_init(cur, upt);
+        build_cursor_init(cur, upt, ru_lo);
         bool started = false;
         int ru, cu;
-        while (build_next_block(cur, started, pair0, npairs, nru, ncu256, upt, NACC, ru, cu)) {
+        while (build_next_block(cur, started, pair0, npairs, ru_lo, nru, ncu256, upt, NACC, ru, cu)) {
             const int64_t gi = static_cast<int64_t>(ru) * 256 + rank * kBlk + q * 32 + lane;       // my row of A
             const int si = op.sq_row[gi];
             const int ti = op.rect ? 0x7fffffff : static_cast<int>(gi / op.nb);

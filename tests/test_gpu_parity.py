@@ -382,6 +382,51 @@ def test_potrs_every_nrhs_class(krr, nrhs):
     assert torch.equal(big[:, :nrhs], alpha) and float(big[:, nrhs:].abs().max()) == 0.0
 
 
+@pytest.mark.parametrize("NT", [1, 2, 3, 5, 6])
+def test_potrs_lookahead_depths(krr, NT):
+    """The solve's two-column lookahead at its edges: NT = 1, 2 (no internal streams), 3 (near and mid tiles only), 5 and 6
+    (bulk launches of one to three tiles on the streamed kernel, last columns without a mid / bulk part), nb = 256 (two
+    units per tile, several chunks per unit), against the oracle's substitution with the same factor; repeatable bits."""
+    nb = 256
+    cfg = scaled_config(CONFIGS["C1"], nb=nb, n=NT * nb, p=700)
+    A, _ = make_problem(cfg, device="cuda")
+    rng = np.random.default_rng(100 + NT)
+    pmap = oracle_uniform(cfg.NT, R.FP32)
+    for i in range(cfg.NT):
+        for j in range(i):
+            pmap[i, j] = rng.integers(0, 2)                 # FP32 / FP16 tiles
+    F = gpu_factor(krr, A, nb, pmap)
+    assert int(F.info.item()) == 0
+    g = torch.Generator(device="cuda").manual_seed(7 * NT)
+    Y = torch.randn((cfg.n, 16), device="cuda", generator=g)
+    alpha = krr.potrs(F, Y.clone())
+    torch.cuda.synchronize()
+    want = potrs_fp64(F.dense().cpu().numpy(), Y.cpu().numpy(), nb)
+    assert relF(alpha.cpu().numpy().astype(np.float64), want) <= 1e-5
+    again = krr.potrs(F, Y.clone())
+    torch.cuda.synchronize()
+    assert torch.equal(again, alpha)
+
+
+def test_potrs_rejects_a_misaligned_factor(krr):
+    import ctypes
+    cfg = scaled_config(CONFIGS["C1"], nb=128, n=256, p=100)
+    A, _ = make_problem(cfg, device="cuda")
+    F = gpu_factor(krr, A, cfg.nb, oracle_uniform(cfg.NT, R.FP32))
+    L = krr.lib()
+    B = torch.zeros((cfg.n, 4), device="cuda")
+    wsb = int(L.krr_potrs_workspace(cfg.n, cfg.nb, 4))
+    ws = torch.empty(wsb + 1024, dtype=torch.uint8, device="cuda")
+    wp = (ws.data_ptr() + 1023) // 1024 * 1024
+    shifted = torch.empty(F.payload.numel() + 16, dtype=torch.uint8, device="cuda")
+    base = shifted.data_ptr()
+    off = (8 - base % 16) % 16                                # an address that is 8 modulo 16
+    rc = L.krr_potrs(ctypes.c_void_p(base + off), ctypes.c_void_p(F.scales.data_ptr()), ctypes.c_void_p(F.d_map.data_ptr()),
+                     ctypes.c_void_p(F.h_map.data_ptr()), cfg.n, cfg.nb, ctypes.c_void_p(B.data_ptr()), 4, 4,
+                     ctypes.c_void_p(wp), wsb, None)
+    assert rc == -1 and krr.last_launch_count() == 0
+
+
 @pytest.mark.parametrize("nrhs", [1, 5, 8, 16, 32])
 def test_potrs_mixed_mosaic_every_nrhs_class(krr, nrhs):
     """The solve kernels read FP32, FP16 and FP8 tiles through precision-specific streaming loops (and, on the chain

@@ -941,7 +941,7 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
 // ------------------------------------------------------------------------- solve
 static int rhs_class(int nrhs) { return nrhs <= 4 ? 4 : (nrhs <= 8 ? 8 : (nrhs <= 16 ? 16 : 32)); }
 
-struct PotrsWs { size_t off_table, dinv, dinvT, Minv, MinvT, stage, total; };
+struct PotrsWs { size_t off_table, dinv, dinvT, Minv, MinvT, stage, nearP, total; };
 static PotrsWs potrs_ws_layout(int64_t n, int nb) {
     const size_t NT = n / nb;
     PotrsWs w;
@@ -952,6 +952,7 @@ static PotrsWs potrs_ws_layout(int64_t n, int nb) {
     w.Minv = o;      o = align_up(o + static_cast<size_t>(n) * nb * sizeof(float), 1024);     // inv(L_kk), every k
     w.MinvT = o;     o = align_up(o + static_cast<size_t>(n) * nb * sizeof(float), 1024);     // inv(L_kk)^T for the backward sweep
     w.stage = o;     o = align_up(o + static_cast<size_t>(nb) * kMaxRhs * sizeof(float), 1024);  // t_k of the diagonal step
+    w.nearP = o;     o = align_up(o + 8 * static_cast<size_t>(nb) * kMaxRhs * sizeof(float), 1024);  // K slices of the near tile's update
     w.total = o;
     return w;
 }
@@ -971,7 +972,7 @@ size_t krr_potrs_workspace(int64_t n, int nb, int nrhs) {
 template <int NRHS>
 static int potrs_run(const uint8_t* factor, const float* d_scales, const uint8_t* d_map, const std::vector<int64_t>& hoff,
                      const int64_t* off, const float* Minv, const float* MinvT, float* stage, int NT, int nb, float* B,
-                     int64_t ldb, int nrhs, int num_sms, cudaStream_t st, const StreamMaps* smaps) {
+                     int64_t ldb, int nrhs, int num_sms, cudaStream_t st, const StreamMaps* smaps, const uint8_t* h_map_, float* nearP) {
     constexpr int ROWS = 64 / NRHS, NW = kSolveThreads / 32, CPL = (NRHS <= 16) ? 4 : 2;
     const size_t smem_z = static_cast<size_t>(NRHS) * nb * sizeof(float);
     const size_t smem_bu = smem_z + static_cast<size_t>(NW / 2) * 32 * CPL * NRHS * sizeof(float);
@@ -1021,34 +1022,55 @@ static int potrs_run(const uint8_t* factor, const float* d_scales, const uint8_t
     // nb = 1024, nrhs <= 16).  Shapes whose small operand leaves no room for two ring slots take the older kernels.
     const int stream_budget = 227 * 1024;
     const int stream_sms = num_sms > 32 ? num_sms - 16 : num_sms;     // 16 SMs stay free for the chain's kernels (measured: 148 / 140 / 132 -> 9.51 / 9.55 / 9.34 ms at C3)
-    auto stream_update = [&](bool bwd, int k, int t_lo, int t_hi, cudaStream_t s, int* done) {
+    auto stream_update = [&](bool bwd, int k, int t_lo, int t_hi, cudaStream_t s, int* done, int ksplit = 1, float* P = nullptr) {
         using C = StreamCfg<NRHS>;
         *done = 0;
         const int ntiles = t_hi - t_lo;
         if (ntiles <= 0 || stream_budget <= 0 || !smaps) return static_cast<int>(KRR_OK);
+        if (ksplit > 1 && (ntiles != 1 || !P)) return static_cast<int>(KRR_OK);
         const size_t fixed = smem_z + C::RED_BYTES + static_cast<size_t>(ntiles) * 12 + 8 + (2 * kStreamMaxStages + 1) * 8;
         if (fixed + 2 * kStreamStage > static_cast<size_t>(stream_budget)) return static_cast<int>(KRR_OK);
         int nst = static_cast<int>((static_cast<size_t>(stream_budget) - fixed) / kStreamStage);
         if (nst > kStreamMaxStages) nst = kStreamMaxStages;
-        const int units = ntiles * (nb / 128);
-        const int grid = units < stream_sms ? units : stream_sms;
+        const int units = ntiles * (nb / 128) * ksplit;
+        // (a sliced tile takes one CTA per unit -- the SMs the bulk launches leave free)
+        const int grid = (ksplit > 1) ? units : (units < stream_sms ? units : stream_sms);
         *done = 1;
         const size_t smem = fixed + static_cast<size_t>(nst) * kStreamStage;
         if (bwd)
             return launch(CAT_POTRS, potrs_stream_update_kernel<NRHS, true>, dim3(grid), dim3(kStreamThreads), smem, s,
-                          smaps[1], NT, nb, k, t_lo, ntiles, nst, off, d_map, d_scales, B, ldb, nrhs);
+                          smaps[1], NT, nb, k, t_lo, ntiles, nst, off, d_map, d_scales, B, ldb, nrhs, ksplit, P);
         return launch(CAT_POTRS, potrs_stream_update_kernel<NRHS, false>, dim3(grid), dim3(kStreamThreads), smem, s,
-                      smaps[0], NT, nb, k, t_lo, ntiles, nst, off, d_map, d_scales, B, ldb, nrhs);
+                      smaps[0], NT, nb, k, t_lo, ntiles, nst, off, d_map, d_scales, B, ldb, nrhs, ksplit, P);
     };
-    auto diag = [&](int k, int backward, cudaStream_t s) {
+    // The chain's "near" tile (i, j) -- all the next diagonal step waits for -- as K slices on the SMs the bulk launches leave
+    // free: the largest power of two <= 8 that divides the tile's chunk count and keeps one CTA per free SM.  *nslices = 0:
+    // the tile went through the r01 kernel (read-modify-write of B) instead.
+    auto near_update = [&](bool bwd, int k, int t, cudaStream_t s, int* nslices) {
+        *nslices = 0;
+        const int p = bwd ? h_map_[k * NT + t] : h_map_[t * NT + k];
+        const int es = (p == KRR_FP32) ? 4 : (p == KRR_FP16 ? 2 : 1);
+        const int chunks = nb * es / 128, free_sms = num_sms - stream_sms;
+        int ks = 1;
+        while (ks < 8 && chunks % (2 * ks) == 0 && (nb / 128) * 2 * ks <= free_sms) ks *= 2;
+        if (pipe && ks > 1 && nearP) {
+            int done = 0;
+            const int e = stream_update(bwd, k, t, t + 1, s, &done, ks, nearP);
+            if (e) return e;
+            if (done) { *nslices = ks; return static_cast<int>(KRR_OK); }
+        }
+        return bwd ? bwd_update(k, t, t + 1, s) : fwd_update(k, t, t + 1, s, 3);
+    };
+    auto diag = [&](int k, int backward, cudaStream_t s, int nslices) {
         const float* Mk = (backward ? MinvT : Minv) + static_cast<int64_t>(k) * nb * nb;
         float* Bk = B + static_cast<int64_t>(k) * nb * ldb;
         int e = launch(CAT_POTRS, potrs_stage_kernel<NRHS>, dim3((nb * NRHS + 255) / 256), dim3(256), 0, s, nb,
-                       static_cast<const float*>(Bk), ldb, nrhs, stage);
+                       static_cast<const float*>(Bk), ldb, nrhs, stage, static_cast<const float*>(nearP), nslices);
         if (e) return e;
         return launch(CAT_POTRS, potrs_diagmul_kernel<NRHS>, dim3(nb / ROWS), dim3(kDiagThreads), 0, s, nb, Mk,
                       static_cast<const float*>(stage), Bk, ldb, nrhs, backward);
     };
+    int near_slices = 0;              // slices the pending near tile left in nearP for the next diagonal step's stage kernel
     // (a lambda: an error in the middle still joins the internal streams below)
     auto run_sweeps = [&]() -> int {
     // Two-column lookahead.  Column k's update of row r is made by: the chain stream for r = k + 1 ("near": all the next
@@ -1058,8 +1080,9 @@ static int potrs_run(const uint8_t* factor, const float* d_scales, const uint8_t
     // for a bulk launch issued TWO columns earlier, not for the previous column's.
     // ---- forward: L z = y
     for (int k = 0; k < NT; ++k) {
-        rc = diag(k, 0, sh);
+        rc = diag(k, 0, sh, near_slices);
         if (rc) return rc;
+        near_slices = 0;
         if (!pipe) {
             rc = fwd_update(k, k + 1, NT, st, 3);
             if (rc) return rc;
@@ -1068,7 +1091,7 @@ static int potrs_run(const uint8_t* factor, const float* d_scales, const uint8_t
         KRR_CUDA_CHECK(cudaEventRecord(ev_diag(k), sh));
         if (k + 1 < NT) {
             if (k >= 1) KRR_CUDA_CHECK(cudaStreamWaitEvent(sh, ev_mid(k - 1), 0));
-            rc = fwd_update(k, k + 1, k + 2, sh, 3);
+            rc = near_update(false, k, k + 1, sh, &near_slices);
             if (rc) return rc;
         }
         KRR_CUDA_CHECK(cudaStreamWaitEvent(sm, ev_diag(k), 0));
@@ -1096,8 +1119,9 @@ static int potrs_run(const uint8_t* factor, const float* d_scales, const uint8_t
     }
     // ---- backward: L^T alpha = z
     for (int k = NT - 1; k >= 0; --k) {
-        rc = diag(k, 1, sh);
+        rc = diag(k, 1, sh, near_slices);
         if (rc) return rc;
+        near_slices = 0;
         if (!pipe) {
             rc = bwd_update(k, 0, k, st);
             if (rc) return rc;
@@ -1106,7 +1130,7 @@ static int potrs_run(const uint8_t* factor, const float* d_scales, const uint8_t
         KRR_CUDA_CHECK(cudaEventRecord(ev_diag(k), sh));
         if (k >= 1) {
             if (k + 1 < NT) KRR_CUDA_CHECK(cudaStreamWaitEvent(sh, ev_mid(k + 1), 0));
-            rc = bwd_update(k, k - 1, k, sh);
+            rc = near_update(true, k, k - 1, sh, &near_slices);
             if (rc) return rc;
         }
         KRR_CUDA_CHECK(cudaStreamWaitEvent(sm, ev_diag(k), 0));
@@ -1171,6 +1195,7 @@ int krr_potrs(const void* d_factor, const float* d_scales, const uint8_t* d_map,
     float* Minv = reinterpret_cast<float*>(ws + L.Minv);
     float* MinvT = reinterpret_cast<float*>(ws + L.MinvT);
     float* stage = reinterpret_cast<float*>(ws + L.stage);
+    float* nearP = reinterpret_cast<float*>(ws + L.nearP);
     rc = launch(CAT_MISC, offsets_kernel, dim3(1), dim3(32), 0, st, NT, nb, d_map, off, host_map_hash(NT, h_map), static_cast<int*>(nullptr),
                 static_cast<int*>(nullptr), static_cast<int*>(nullptr));
     if (rc) return rc;
@@ -1193,10 +1218,10 @@ int krr_potrs(const void* d_factor, const float* d_scales, const uint8_t* d_map,
     }
     const StreamMaps* sm = have_maps ? smaps : nullptr;
     switch (rhs_class(nrhs)) {
-        case 4:  return potrs_run<4>(factor, d_scales, d_map, hoff, off, Minv, MinvT, stage, NT, nb, d_B, ldb, nrhs, num_sms, st, sm);
-        case 8:  return potrs_run<8>(factor, d_scales, d_map, hoff, off, Minv, MinvT, stage, NT, nb, d_B, ldb, nrhs, num_sms, st, sm);
-        case 16: return potrs_run<16>(factor, d_scales, d_map, hoff, off, Minv, MinvT, stage, NT, nb, d_B, ldb, nrhs, num_sms, st, sm);
-        default: return potrs_run<32>(factor, d_scales, d_map, hoff, off, Minv, MinvT, stage, NT, nb, d_B, ldb, nrhs, num_sms, st, sm);
+        case 4:  return potrs_run<4>(factor, d_scales, d_map, hoff, off, Minv, MinvT, stage, NT, nb, d_B, ldb, nrhs, num_sms, st, sm, h_map, nearP);
+        case 8:  return potrs_run<8>(factor, d_scales, d_map, hoff, off, Minv, MinvT, stage, NT, nb, d_B, ldb, nrhs, num_sms, st, sm, h_map, nearP);
+        case 16: return potrs_run<16>(factor, d_scales, d_map, hoff, off, Minv, MinvT, stage, NT, nb, d_B, ldb, nrhs, num_sms, st, sm, h_map, nearP);
+        default: return potrs_run<32>(factor, d_scales, d_map, hoff, off, Minv, MinvT, stage, NT, nb, d_B, ldb, nrhs, num_sms, st, sm, h_map, nearP);
     }
 }
 

@@ -180,7 +180,7 @@ template <int NRHS, bool BWD>
 __global__ void __launch_bounds__(kStreamThreads, 1)
 potrs_stream_update_kernel(const __grid_constant__ StreamMaps maps, int NT, int nb, int k, int t_lo, int ntiles, int nstages,
                            const int64_t* __restrict__ off, const uint8_t* __restrict__ map, const float* __restrict__ scales,
-                           float* __restrict__ B, int64_t ldb, int nrhs) {
+                           float* __restrict__ B, int64_t ldb, int nrhs, int ksplit, float* __restrict__ P) {
     using C = StreamCfg<NRHS>;
     constexpr int R = C::R, NACC = C::NACC, KS = C::KS;
     extern __shared__ __align__(1024) uint8_t stream_smem[];
@@ -193,8 +193,13 @@ potrs_stream_update_kernel(const __grid_constant__ StreamMaps maps, int NT, int 
     uint64_t* bars = reinterpret_cast<uint64_t*>((reinterpret_cast<uintptr_t>(t_scale + ntiles) + 7) & ~static_cast<uintptr_t>(7));
     const uint32_t full0 = ptx::smem_u32(bars), empty0 = full0 + 8 * kStreamMaxStages, zbar = empty0 + 8 * kStreamMaxStages;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const int upt = nb / 128;                                    // units per tile
-    const int nunits = ntiles * upt;
+    const int upt = nb / 128;                                    // 128-row (column) blocks per tile
+    // ksplit > 1 (one tile, the chain's "near" tile): a block's summation range is cut into ksplit slices, one unit each,
+    // and a unit leaves its sum in P[slice][row][NRHS] -- the next diagonal step's stage kernel subtracts the slices in a
+    // fixed order -- so that the 4 MB tile is read by upt * ksplit SMs instead of upt.
+    const int nunits = ntiles * upt * ksplit;
+    const bool sliced = ksplit > 1 && gridDim.x >= static_cast<unsigned>(nunits);     // one unit per CTA: only its slice of the small operand is needed
+    const int zrows = sliced ? nb / ksplit : nb, zrow0 = sliced ? (static_cast<int>(blockIdx.x) % ksplit) * zrows : 0;
     const bool z_bulk = (nrhs == NRHS) && (ldb == NRHS) && (reinterpret_cast<uintptr_t>(B) % 16 == 0);
     for (int t = tid; t < ntiles; t += kStreamThreads) {
         const int idx = BWD ? (k * NT + t_lo + t) : ((t_lo + t) * NT + k);
@@ -215,19 +220,21 @@ potrs_stream_update_kernel(const __grid_constant__ StreamMaps maps, int NT, int 
         // ---------------- producer: one TMA box per chunk, in the order the consumers walk them
         if (lane == 0) {
             ptx::prefetch_tmap(&maps.m4); ptx::prefetch_tmap(&maps.m2); ptx::prefetch_tmap(&maps.m1);
-            if (z_bulk) {
-                ptx::mbar_arrive_expect_tx(zbar, static_cast<uint32_t>(nb) * NRHS * 4);
-                bulk_load_1d(ptx::smem_u32(vs), B + static_cast<int64_t>(k) * nb * ldb, static_cast<uint32_t>(nb) * NRHS * 4, zbar);
+            if (z_bulk && blockIdx.x < static_cast<unsigned>(nunits)) {
+                ptx::mbar_arrive_expect_tx(zbar, static_cast<uint32_t>(zrows) * NRHS * 4);
+                bulk_load_1d(ptx::smem_u32(vs + static_cast<size_t>(zrow0) * NRHS), B + (static_cast<int64_t>(k) * nb + zrow0) * ldb,
+                             static_cast<uint32_t>(zrows) * NRHS * 4, zbar);
             }
             int slot = 0;
             uint32_t pass = 0;                                   // times the ring has wrapped
             for (int unit = blockIdx.x; unit < nunits; unit += gridDim.x) {
-                const int t = unit / upt, o0 = (unit % upt) * 128;
+                const int blk = unit / ksplit, slice = unit % ksplit;
+                const int t = blk / upt, o0 = (blk % upt) * 128;
                 const int p = t_prec[t], row0 = t_row[t];
                 const int es = (p == KRR_FP32) ? 4 : (p == KRR_FP16 ? 2 : 1);
                 const CUtensorMap* tm = (es == 4) ? &maps.m4 : (es == 2 ? &maps.m2 : &maps.m1);
-                const int nchunks = nb * es / 128;
-                for (int c = 0; c < nchunks; ++c) {
+                const int cps = nb * es / 128 / ksplit;          // chunks per unit
+                for (int c = slice * cps; c < (slice + 1) * cps; ++c) {
                     if (pass > 0) {      // polled with a pause: the producer shares its scheduler with two consumer warps
                         uint32_t done = 0, spins = 0;
                         while (true) {
@@ -251,9 +258,10 @@ potrs_stream_update_kernel(const __grid_constant__ StreamMaps maps, int NT, int 
     // ---------------- consumers
     const int grp = warp / KS, ks = warp % KS;
     auto consumer_bar = [&]() { asm volatile("bar.sync 1, 256;" ::: "memory"); };
-    if (!z_bulk) {      // the small operand: rows k*nb .. of B, zero-padded to NRHS columns
+    if (blockIdx.x >= static_cast<unsigned>(nunits)) return;
+    if (!z_bulk) {      // the small operand: rows k*nb .. of B (the unit's slice of them), zero-padded to NRHS columns
         const float* Vk = B + static_cast<int64_t>(k) * nb * ldb;
-        for (int idx = tid; idx < nb * NRHS; idx += kStreamConsumers) {
+        for (int idx = zrow0 * NRHS + tid; idx < (zrow0 + zrows) * NRHS; idx += kStreamConsumers) {
             const int r = idx / NRHS, h = idx % NRHS;
             vs[idx] = (h < nrhs) ? Vk[static_cast<int64_t>(r) * ldb + h] : 0.0f;
         }
@@ -267,11 +275,12 @@ potrs_stream_update_kernel(const __grid_constant__ StreamMaps maps, int NT, int 
     int slot = 0;
     uint32_t phase = 0;
     for (int unit = blockIdx.x; unit < nunits; unit += gridDim.x) {
-        const int t = unit / upt, o0 = (unit % upt) * 128;
+        const int blk = unit / ksplit, slice = unit % ksplit;
+        const int t = blk / upt, o0 = (blk % upt) * 128;
         const int p = t_prec[t];
         const int es = (p == KRR_FP32) ? 4 : (p == KRR_FP16 ? 2 : 1);
-        const int nchunks = nb * es / 128;
-        for (int c = 0; c < nchunks; ++c) {
+        const int cps = nb * es / 128 / ksplit;
+        for (int c = slice * cps; c < (slice + 1) * cps; ++c) {
             ptx::mbar_wait(full0 + 8 * slot, phase);
             const uint8_t* st = ring + static_cast<size_t>(slot) * kStreamStage;
             if (!BWD) {
@@ -305,13 +314,25 @@ potrs_stream_update_kernel(const __grid_constant__ StreamMaps maps, int NT, int 
         }
         if (ks == 0) {
             const float s = (es == 1) ? t_scale[t] : 1.0f;
-            const int64_t row0 = static_cast<int64_t>(t_lo + t) * nb + o0 + grp * 32 * R;
+            if (ksplit > 1) {
+                // the slice's sum, for the stage kernel of the next diagonal step
+                float* pr = P + (static_cast<size_t>(slice) * nb + o0 + grp * 32 * R) * NRHS;
 #pragma unroll
-            for (int u = 0; u < R; ++u) {
-                float* out = B + (row0 + (BWD ? lane * R + u : lane + 32 * u)) * ldb;
+                for (int u = 0; u < R; ++u) {
+                    float* out = pr + static_cast<size_t>(BWD ? lane * R + u : lane + 32 * u) * NRHS;
 #pragma unroll
-                for (int h = 0; h < NRHS; ++h)
-                    if (h < nrhs) red_add_f32(out + h, -(s * acc[u * NRHS + h]));   // the unit is the only writer of its rows: same result as a read-modify-write, no round trip
+                    for (int h = 0; h < NRHS; h += 4)
+                        *reinterpret_cast<float4*>(out + h) = make_float4(s * acc[u * NRHS + h], s * acc[u * NRHS + h + 1], s * acc[u * NRHS + h + 2], s * acc[u * NRHS + h + 3]);
+                }
+            } else {
+                const int64_t row0 = static_cast<int64_t>(t_lo + t) * nb + o0 + grp * 32 * R;
+#pragma unroll
+                for (int u = 0; u < R; ++u) {
+                    float* out = B + (row0 + (BWD ? lane * R + u : lane + 32 * u)) * ldb;
+#pragma unroll
+                    for (int h = 0; h < NRHS; ++h)
+                        if (h < nrhs) red_add_f32(out + h, -(s * acc[u * NRHS + h]));   // the unit is the only writer of its rows: same result as a read-modify-write, no round trip
+                }
             }
         }
 #pragma unroll

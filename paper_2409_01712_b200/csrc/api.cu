@@ -952,7 +952,7 @@ static PotrsWs potrs_ws_layout(int64_t n, int nb) {
     w.Minv = o;      o = align_up(o + static_cast<size_t>(n) * nb * sizeof(float), 1024);     // inv(L_kk), every k
     w.MinvT = o;     o = align_up(o + static_cast<size_t>(n) * nb * sizeof(float), 1024);     // inv(L_kk)^T for the backward sweep
     w.stage = o;     o = align_up(o + static_cast<size_t>(nb) * kMaxRhs * sizeof(float), 1024);  // t_k of the diagonal step
-    w.nearP = o;     o = align_up(o + 8 * static_cast<size_t>(nb) * kMaxRhs * sizeof(float), 1024);  // K slices of the near tile's update
+    w.nearP = o;     o = align_up(o + 3 * 8 * static_cast<size_t>(nb) * kMaxRhs * sizeof(float), 1024);  // K slices of the near / mid tiles' updates
     w.total = o;
     return w;
 }
@@ -1046,26 +1046,31 @@ static int potrs_run(const uint8_t* factor, const float* d_scales, const uint8_t
     // The chain's "near" tile (i, j) -- all the next diagonal step waits for -- as K slices on the SMs the bulk launches leave
     // free: the largest power of two <= 8 that divides the tile's chunk count and keeps one CTA per free SM.  *nslices = 0:
     // the tile went through the r01 kernel (read-modify-write of B) instead.
-    auto near_update = [&](bool bwd, int k, int t, cudaStream_t s, int* nslices) {
+    auto near_update = [&](bool bwd, int k, int t, cudaStream_t s, float* Pbuf, int* nslices) {
         *nslices = 0;
         const int p = bwd ? h_map_[k * NT + t] : h_map_[t * NT + k];
         const int es = (p == KRR_FP32) ? 4 : (p == KRR_FP16 ? 2 : 1);
         const int chunks = nb * es / 128, free_sms = num_sms - stream_sms;
         int ks = 1;
         while (ks < 8 && chunks % (2 * ks) == 0 && (nb / 128) * 2 * ks <= free_sms) ks *= 2;
-        if (pipe && ks > 1 && nearP) {
+        if (pipe && ks > 1 && Pbuf) {
             int done = 0;
-            const int e = stream_update(bwd, k, t, t + 1, s, &done, ks, nearP);
+            const int e = stream_update(bwd, k, t, t + 1, s, &done, ks, Pbuf);
             if (e) return e;
             if (done) { *nslices = ks; return static_cast<int>(KRR_OK); }
         }
         return bwd ? bwd_update(k, t, t + 1, s) : fwd_update(k, t, t + 1, s, 3);
     };
+    const size_t p_elems = 8 * static_cast<size_t>(nb) * kMaxRhs;      // one partial buffer: near | mid (even tile) | mid (odd tile)
+    auto midP = [&](int tile) { return nearP ? nearP + (1 + (tile & 1)) * p_elems : nullptr; };
+    int mid_slices[2] = {0, 0};       // slices a sliced mid tile left for the diagonal step of tile row (column) `tile`, by parity
     auto diag = [&](int k, int backward, cudaStream_t s, int nslices) {
         const float* Mk = (backward ? MinvT : Minv) + static_cast<int64_t>(k) * nb * nb;
         float* Bk = B + static_cast<int64_t>(k) * nb * ldb;
         int e = launch(CAT_POTRS, potrs_stage_kernel<NRHS>, dim3((nb * NRHS + 255) / 256), dim3(256), 0, s, nb,
-                       static_cast<const float*>(Bk), ldb, nrhs, stage, static_cast<const float*>(nearP), nslices);
+                       static_cast<const float*>(Bk), ldb, nrhs, stage, static_cast<const float*>(midP(k)), mid_slices[k & 1],
+                       static_cast<const float*>(nearP), nslices);
+        mid_slices[k & 1] = 0;
         if (e) return e;
         return launch(CAT_POTRS, potrs_diagmul_kernel<NRHS>, dim3(nb / ROWS), dim3(kDiagThreads), 0, s, nb, Mk,
                       static_cast<const float*>(stage), Bk, ldb, nrhs, backward);
@@ -1091,13 +1096,13 @@ static int potrs_run(const uint8_t* factor, const float* d_scales, const uint8_t
         KRR_CUDA_CHECK(cudaEventRecord(ev_diag(k), sh));
         if (k + 1 < NT) {
             if (k >= 1) KRR_CUDA_CHECK(cudaStreamWaitEvent(sh, ev_mid(k - 1), 0));
-            rc = near_update(false, k, k + 1, sh, &near_slices);
+            rc = near_update(false, k, k + 1, sh, nearP, &near_slices);
             if (rc) return rc;
         }
         KRR_CUDA_CHECK(cudaStreamWaitEvent(sm, ev_diag(k), 0));
         if (k >= 1) KRR_CUDA_CHECK(cudaStreamWaitEvent(sm, ev_bulk(k - 1), 0));
         if (k + 2 < NT) {
-            rc = fwd_update(k, k + 2, k + 3, sm, 3);
+            rc = near_update(false, k, k + 2, sm, midP(k + 2), &mid_slices[(k + 2) & 1]);
             if (rc) return rc;
         }
         KRR_CUDA_CHECK(cudaEventRecord(ev_mid(k), sm));
@@ -1130,13 +1135,13 @@ static int potrs_run(const uint8_t* factor, const float* d_scales, const uint8_t
         KRR_CUDA_CHECK(cudaEventRecord(ev_diag(k), sh));
         if (k >= 1) {
             if (k + 1 < NT) KRR_CUDA_CHECK(cudaStreamWaitEvent(sh, ev_mid(k + 1), 0));
-            rc = near_update(true, k, k - 1, sh, &near_slices);
+            rc = near_update(true, k, k - 1, sh, nearP, &near_slices);
             if (rc) return rc;
         }
         KRR_CUDA_CHECK(cudaStreamWaitEvent(sm, ev_diag(k), 0));
         if (k + 1 < NT) KRR_CUDA_CHECK(cudaStreamWaitEvent(sm, ev_bulk(k + 1), 0));
         if (k >= 2) {
-            rc = bwd_update(k, k - 2, k - 1, sm);
+            rc = near_update(true, k, k - 2, sm, midP(k - 2), &mid_slices[(k - 2) & 1]);
             if (rc) return rc;
         }
         KRR_CUDA_CHECK(cudaEventRecord(ev_mid(k), sm));

@@ -433,17 +433,19 @@ potrs_tile_inverse_kernel(const uint8_t* __restrict__ factor, const int64_t* __r
 // result over t_k in B while other CTAs still read t_k.  One CTA per group of 64 / NRHS rows; its eight warps split the
 // K range in slices of whole 128-column steps, lane = 4 consecutive columns; the slices are added in a fixed order
 // through shared memory: deterministic.  The launch is short (one DRAM round trip per warp) and wide (nb NRHS / 64 CTAs).
-// nslices > 0: the chain's update of these rows by the previous tile column was left as nslices partial sums
-// P[slice][nb][NRHS] (potrs_stream.cuh, ksplit): they are subtracted here, lowest slice first -- a fixed order.
+// The updates of these rows by the two previous tile columns may have been left as partial sums (potrs_stream.cuh, ksplit):
+// Pm[slice][nb][NRHS] (nm slices) by the column before the previous one ("mid"), Pn (nn slices) by the previous one
+// ("near").  They are subtracted here in that order, lowest slice first -- a fixed order.
 template <int NRHS>
 __global__ void __launch_bounds__(256)
 potrs_stage_kernel(int nb, const float* __restrict__ Bk, int64_t ldb, int nrhs, float* __restrict__ T,
-                   const float* __restrict__ P, int nslices) {
+                   const float* __restrict__ Pm, int nm, const float* __restrict__ Pn, int nn) {
     const int idx = blockIdx.x * 256 + threadIdx.x;
     if (idx < nb * NRHS) {
         const int r = idx / NRHS, h = idx % NRHS;
         float v = (h < nrhs) ? Bk[static_cast<int64_t>(r) * ldb + h] : 0.0f;
-        for (int s = 0; s < nslices; ++s) v -= P[static_cast<size_t>(s) * nb * NRHS + idx];
+        for (int s = 0; s < nm; ++s) v -= Pm[static_cast<size_t>(s) * nb * NRHS + idx];
+        for (int s = 0; s < nn; ++s) v -= Pn[static_cast<size_t>(s) * nb * NRHS + idx];
         T[idx] = v;
     }
 }

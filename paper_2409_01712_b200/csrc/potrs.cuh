@@ -22,8 +22,7 @@ namespace krr {
 
 constexpr int kMaxRhs = 32;
 constexpr int kSolveThreads = 256;          // update kernels
-constexpr int kDiagThreads = 256;           // diagonal-tile kernel: CTAs of 8 warps ...
-constexpr int kDiagCluster = 8;             // ... in a cluster of 8
+constexpr int kDiagThreads = 256;           // diagonal-tile product kernel: CTAs of 8 warps
 
 // Dequantising loads of CPL (4 or 2) consecutive elements of a mosaic tile (element index e).
 __device__ __forceinline__ float4 load4(const uint8_t* tile, int p, float s, int64_t e) {

@@ -242,10 +242,12 @@ def test_ibs_kernel_build_and_predict(krr, n, m, p, nb):
     assert np.all(np.abs(P.cpu().numpy() - Pw) <= 4e-6 * (Kw @ np.abs(W.cpu().numpy().astype(np.float64))))
 
 
-def test_fit_host_matches_device_pipeline(krr):
-    """krr_fit_host (genotypes and Y from host memory, Build on the device) against Build -> map -> factorisation ->
-    solve called one by one: the same kernels on the same data, bit-identical alpha and map."""
-    cfg = scaled_config(CONFIGS["C2"], nb=256, n=1536, p=700)
+@pytest.mark.parametrize("nb,n", [(256, 1536), (512, 2560)])
+def test_fit_host_matches_device_pipeline(krr, nb, n):
+    """krr_fit_host (genotypes and Y from host memory; the Build runs strip by strip behind the copy: six strips of one
+    tile row with 256 x 256 blocks, five with 256 x 512 blocks) against Build -> map -> factorisation -> solve called one
+    by one: the same kernels on the same data, bit-identical alpha and map."""
+    cfg = scaled_config(CONFIGS["C2"], nb=nb, n=n, p=700)
     G = genotypes(cfg.seed, cfg.n, cfg.p, cfg.genotype, device="cuda")
     Y = torch.randn((cfg.n, 8), device="cuda", generator=torch.Generator(device="cuda").manual_seed(5))
     A = krr.krr_build(padded(G), cfg.gamma, cfg.lam, cfg.nb)

@@ -1043,9 +1043,10 @@ static int potrs_run(const uint8_t* factor, const float* d_scales, const uint8_t
         return launch(CAT_POTRS, potrs_stream_update_kernel<NRHS, false>, dim3(grid), dim3(kStreamThreads), smem, s,
                       smaps[0], NT, nb, k, t_lo, ntiles, nst, off, d_map, d_scales, B, ldb, nrhs, ksplit, P);
     };
-    // The chain's "near" tile (i, j) -- all the next diagonal step waits for -- as K slices on the SMs the bulk launches leave
-    // free: the largest power of two <= 8 that divides the tile's chunk count and keeps one CTA per free SM.  *nslices = 0:
-    // the tile went through the r01 kernel (read-modify-write of B) instead.
+    // A single tile of the lookahead -- the "near" tile, all the next diagonal step waits for, or the "mid" tile behind it -- as
+    // K slices on the SMs the bulk launches leave free: the largest power of two <= 8 that divides the tile's chunk count and
+    // keeps one CTA per free SM; the slices' sums go to Pbuf and the stage kernel of the diagonal step that needs these rows
+    // subtracts them.  *nslices = 0: the tile went through the r01 kernel (read-modify-write of B) instead.
     auto near_update = [&](bool bwd, int k, int t, cudaStream_t s, float* Pbuf, int* nslices) {
         *nslices = 0;
         const int p = bwd ? h_map_[k * NT + t] : h_map_[t * NT + k];

@@ -21,6 +21,8 @@
 //   backward  unit = columns [o0, o0+128) of tile (k, j); chunk = box of 32 / 64 / 128 rows x 128 columns (16 KB);
 //             warp ks takes the rows ks, ks+8, ...; lane l the columns 4l .. 4l+3.
 //   NRHS = 32: R = 2, two groups of 64 output rows, four slices each.
+// The same kernel serves the single tiles of the lookahead (near / mid) with `ksplit` > 1: a block's summation range is cut
+// into ksplit units on as many CTAs, and a unit leaves its sum in a partial buffer instead of adding it to B.
 #pragma once
 #include "potrs.cuh"
 #include "ptx.cuh"

@@ -266,6 +266,22 @@ static int launch(int cat, K kernel, dim3 grid, dim3 block, size_t smem, cudaStr
     return cudaGetLastError() == cudaSuccess ? KRR_OK : KRR_ERR_CUDA;
 }
 
+// The same as a programmatic dependent of the kernel before it in the stream (common.cuh pdl_trigger / pdl_wait): the
+// kernel's prologue runs beside that kernel's tail.  Only for kernels that call pdl_wait() before they touch its output.
+template <typename... KArgs, typename... Args>
+static int launch_pdl(int cat, void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args... args) {
+    ProfScope ps(cat, st);
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof(cfg));
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    ++g_launches;
+    return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...) == cudaSuccess ? KRR_OK : KRR_ERR_CUDA;
+}
+
 // The tensor maps of one factorisation: hi/lo FP16 images of L (128-row boxes for A operands and for
 // single-CTA B operands, 64-row boxes for the B halves of CTA pairs), the inverted diagonal blocks,
 // and the E4M3 images.
@@ -1037,6 +1053,13 @@ static int potrs_run(const uint8_t* factor, const float* d_scales, const uint8_t
         const int grid = (ksplit > 1) ? units : (units < stream_sms ? units : stream_sms);
         *done = 1;
         const size_t smem = fixed + static_cast<size_t>(nst) * kStreamStage;
+        if (ksplit > 1 && s == sh) {     // the near tile: a programmatic dependent of the diagonal step's product
+            if (bwd)
+                return launch_pdl(CAT_POTRS, potrs_stream_update_kernel<NRHS, true>, dim3(grid), dim3(kStreamThreads), smem, s,
+                                  smaps[1], NT, nb, k, t_lo, ntiles, nst, off, d_map, d_scales, B, ldb, nrhs, ksplit, P);
+            return launch_pdl(CAT_POTRS, potrs_stream_update_kernel<NRHS, false>, dim3(grid), dim3(kStreamThreads), smem, s,
+                              smaps[0], NT, nb, k, t_lo, ntiles, nst, off, d_map, d_scales, B, ldb, nrhs, ksplit, P);
+        }
         if (bwd)
             return launch(CAT_POTRS, potrs_stream_update_kernel<NRHS, true>, dim3(grid), dim3(kStreamThreads), smem, s,
                           smaps[1], NT, nb, k, t_lo, ntiles, nst, off, d_map, d_scales, B, ldb, nrhs, ksplit, P);
@@ -1068,12 +1091,12 @@ static int potrs_run(const uint8_t* factor, const float* d_scales, const uint8_t
     auto diag = [&](int k, int backward, cudaStream_t s, int nslices) {
         const float* Mk = (backward ? MinvT : Minv) + static_cast<int64_t>(k) * nb * nb;
         float* Bk = B + static_cast<int64_t>(k) * nb * ldb;
-        int e = launch(CAT_POTRS, potrs_stage_kernel<NRHS>, dim3((nb * NRHS + 255) / 256), dim3(256), 0, s, nb,
+        int e = launch_pdl(CAT_POTRS, potrs_stage_kernel<NRHS>, dim3((nb * NRHS + 255) / 256), dim3(256), 0, s, nb,
                        static_cast<const float*>(Bk), ldb, nrhs, stage, static_cast<const float*>(midP(k)), mid_slices[k & 1],
                        static_cast<const float*>(nearP), nslices);
         mid_slices[k & 1] = 0;
         if (e) return e;
-        return launch(CAT_POTRS, potrs_diagmul_kernel<NRHS>, dim3(nb / ROWS), dim3(kDiagThreads), 0, s, nb, Mk,
+        return launch_pdl(CAT_POTRS, potrs_diagmul_kernel<NRHS>, dim3(nb / ROWS), dim3(kDiagThreads), 0, s, nb, Mk,
                       static_cast<const float*>(stage), Bk, ldb, nrhs, backward);
     };
     int near_slices = 0;              // slices the pending near tile left in nearP for the next diagonal step's stage kernel

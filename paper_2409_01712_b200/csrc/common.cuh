@@ -70,6 +70,13 @@ __device__ __forceinline__ float round_to_prec(float x, int p, float s) {
 // Element sizes of the mosaic payload
 __host__ __device__ __forceinline__ int prec_bytes(int p) { return p == KRR_FP32 ? 4 : (p == KRR_FP16 ? 2 : 1); }
 
+// Programmatic dependent launch (PTX griddepcontrol, sm_90+): a kernel launched with the programmatic-stream-serialization
+// attribute may start -- prologue, loads of data no earlier kernel writes -- once every CTA of the kernel before it in the
+// stream has called pdl_trigger() (or exited); pdl_wait() then blocks until that kernel has completed and its writes are
+// visible.  Both are no-ops in a kernel launched the ordinary way.
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
 // Launch counter (host, per thread) for krr_last_launch_count().
 extern thread_local int64_t g_launches;
 

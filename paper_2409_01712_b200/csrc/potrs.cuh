@@ -439,6 +439,8 @@ template <int NRHS>
 __global__ void __launch_bounds__(256)
 potrs_stage_kernel(int nb, const float* __restrict__ Bk, int64_t ldb, int nrhs, float* __restrict__ T,
                    const float* __restrict__ Pm, int nm, const float* __restrict__ Pn, int nn) {
+    pdl_trigger();
+    pdl_wait();
     const int idx = blockIdx.x * 256 + threadIdx.x;
     if (idx < nb * NRHS) {
         const int r = idx / NRHS, h = idx % NRHS;
@@ -464,6 +466,8 @@ potrs_diagmul_kernel(int nb, const float* __restrict__ Mk, const float* __restri
     float acc[64];
 #pragma unroll
     for (int v = 0; v < 64; ++v) acc[v] = 0.0f;
+    pdl_trigger();
+    pdl_wait();                                                    // T is the stage kernel's output
     // step s of the range goes to warp s % NW (a fixed assignment)
     for (int st = warp; st < steps; st += NW) {
         const int l = k_lo + st * kBlk + lane * 4;

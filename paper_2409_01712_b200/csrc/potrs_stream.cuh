@@ -216,17 +216,13 @@ potrs_stream_update_kernel(const __grid_constant__ StreamMaps maps, int NT, int 
         ptx::mbar_init(zbar, 1);
         ptx::fence_mbar_init();
     }
+    pdl_trigger();
     __syncthreads();
 
     if (warp == 8) {
         // ---------------- producer: one TMA box per chunk, in the order the consumers walk them
         if (lane == 0) {
             ptx::prefetch_tmap(&maps.m4); ptx::prefetch_tmap(&maps.m2); ptx::prefetch_tmap(&maps.m1);
-            if (z_bulk && blockIdx.x < static_cast<unsigned>(nunits)) {
-                ptx::mbar_arrive_expect_tx(zbar, static_cast<uint32_t>(zrows) * NRHS * 4);
-                bulk_load_1d(ptx::smem_u32(vs + static_cast<size_t>(zrow0) * NRHS), B + (static_cast<int64_t>(k) * nb + zrow0) * ldb,
-                             static_cast<uint32_t>(zrows) * NRHS * 4, zbar);
-            }
             int slot = 0;
             uint32_t pass = 0;                                   // times the ring has wrapped
             for (int unit = blockIdx.x; unit < nunits; unit += gridDim.x) {
@@ -261,6 +257,10 @@ potrs_stream_update_kernel(const __grid_constant__ StreamMaps maps, int NT, int 
     const int grp = warp / KS, ks = warp % KS;
     auto consumer_bar = [&]() { asm volatile("bar.sync 1, 256;" ::: "memory"); };
     if (blockIdx.x >= static_cast<unsigned>(nunits)) return;
+    // Launched as a programmatic dependent (the chain's near tile behind the diagonal step's product), everything above --
+    // and the producer warp's first tile loads: the factor is not written during a solve -- runs beside the previous kernel;
+    // its output (the small operand, and B / the partial buffer this kernel writes at the end) is touched only behind this wait.
+    pdl_wait();
     if (!z_bulk) {      // the small operand: rows k*nb .. of B (the unit's slice of them), zero-padded to NRHS columns
         const float* Vk = B + static_cast<int64_t>(k) * nb * ldb;
         for (int idx = zrow0 * NRHS + tid; idx < (zrow0 + zrows) * NRHS; idx += kStreamConsumers) {
@@ -269,6 +269,11 @@ potrs_stream_update_kernel(const __grid_constant__ StreamMaps maps, int NT, int 
         }
         consumer_bar();
     } else {
+        if (tid == 0) {
+            ptx::mbar_arrive_expect_tx(zbar, static_cast<uint32_t>(zrows) * NRHS * 4);
+            bulk_load_1d(ptx::smem_u32(vs + static_cast<size_t>(zrow0) * NRHS), B + (static_cast<int64_t>(k) * nb + zrow0) * ldb,
+                         static_cast<uint32_t>(zrows) * NRHS * 4, zbar);
+        }
         ptx::mbar_wait(zbar, 0);
     }
     float acc[NACC];

@@ -995,7 +995,9 @@ static int potrs_run(const uint8_t* factor, const float* d_scales, const uint8_t
     const size_t smem_b1 = smem_z + static_cast<size_t>(NW / 2) * 32 * NRHS * sizeof(float);
     const int64_t blk_elems = static_cast<int64_t>(kBlk) * kBlk;
     const int nsub = nb / kBlk;
-    const bool pipe = NT > 2;
+    // the lookahead pays once a tile column is a few megabytes (C1, n = 2048, nb = 256: 0.24 ms without it against 0.41 ms
+    // with its five launches and the events per column; C2, n = 16384, nb = 512: 1.64 against 1.53 ms)
+    const bool pipe = NT > 2 && static_cast<int64_t>(NT) * nb * nb >= (int64_t{1} << 20);
     cudaStream_t sh = st, sm = st, sl = st;
     enum { EV_FORK = 0, EV_JOIN_HI = 1, EV_JOIN_MID = 2, EV_JOIN_LO = 3, EV_BASE = 4 };      // the event pool of krr_potrf_mp, reused
     auto ev_diag = [&](int k) { return g_pipe.event(EV_BASE + 4 * static_cast<size_t>(k) + 0); };

@@ -382,12 +382,13 @@ def test_potrs_every_nrhs_class(krr, nrhs):
     assert torch.equal(big[:, :nrhs], alpha) and float(big[:, nrhs:].abs().max()) == 0.0
 
 
-@pytest.mark.parametrize("NT", [1, 2, 3, 5, 6])
-def test_potrs_lookahead_depths(krr, NT):
-    """The solve's two-column lookahead at its edges: NT = 1, 2 (no internal streams), 3 (near and mid tiles only), 5 and 6
-    (bulk launches of one to three tiles on the streamed kernel, last columns without a mid / bulk part), nb = 256 (two
-    units per tile, several chunks per unit), against the oracle's substitution with the same factor; repeatable bits."""
-    nb = 256
+@pytest.mark.parametrize("NT,nb", [(1, 256), (2, 256), (3, 640), (5, 512), (6, 512), (6, 256)])
+def test_potrs_lookahead_depths(krr, NT, nb):
+    """The solve's two-column lookahead at its edges: NT = 1, 2 (no internal streams), 3 (near and mid tiles only; nb = 640:
+    five units per tile, the single-CTA factorisation path), 5 and 6 (bulk launches of one to three tiles on the streamed
+    kernel, last columns without a mid / bulk part, near / mid tiles as K slices); tile columns of a megabyte and more take
+    the lookahead, (6, 256) stays below that and runs column by column on the caller's stream.  Against the oracle's
+    substitution with the same factor; repeatable bits."""
     cfg = scaled_config(CONFIGS["C1"], nb=nb, n=NT * nb, p=700)
     A, _ = make_problem(cfg, device="cuda")
     rng = np.random.default_rng(100 + NT)
@@ -427,12 +428,14 @@ def test_potrs_rejects_a_misaligned_factor(krr):
     assert rc == -1 and krr.last_launch_count() == 0
 
 
+@pytest.mark.parametrize("nb", [128, 512])
 @pytest.mark.parametrize("nrhs", [1, 5, 8, 16, 32])
-def test_potrs_mixed_mosaic_every_nrhs_class(krr, nrhs):
-    """The solve kernels read FP32, FP16 and FP8 tiles through precision-specific streaming loops (and, on the chain
-    stream of the backward sweep, a one-column-per-lane variant): a random mosaic, NT = 8 (one-column lookahead on),
-    against the oracle's substitution with the SAME dequantised factor."""
-    cfg = replace(scaled_config(CONFIGS["S1"], nb=128, n=1024, p=768), genotype="maf", gamma_scale=4.0)
+def test_potrs_mixed_mosaic_every_nrhs_class(krr, nrhs, nb):
+    """The solve kernels read FP32, FP16 and FP8 tiles through precision-specific loops: a random mosaic, NT = 8, against
+    the oracle's substitution with the SAME dequantised factor.  nb = 128: column by column with the r01 kernels (a
+    one-column-per-lane variant in the backward sweep); nb = 512: the two-column lookahead, every update on the streamed
+    kernel (bulk launches, near / mid tiles as K slices, partial sums gathered by the stage kernel)."""
+    cfg = replace(scaled_config(CONFIGS["S1"], nb=nb, n=8 * nb, p=768), genotype="maf", gamma_scale=4.0)
     A, _ = make_problem(cfg, device="cuda")
     rng = np.random.default_rng(11)
     pmap = oracle_uniform(cfg.NT, R.FP32)

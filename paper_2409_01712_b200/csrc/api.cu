@@ -766,14 +766,17 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
     // enqueued right after its record) and one for the finished inverse
     auto ev_blk = [&](int c) { return g_pipe.event(EV_BASE + EV_PER_COL * static_cast<size_t>(NT) + c); };
     auto ev_inv = [&]() { return g_pipe.event(EV_BASE + EV_PER_COL * static_cast<size_t>(NT) + nsub); };
+    auto ev_p3 = [&](int c) { return g_pipe.event(EV_BASE + EV_PER_COL * static_cast<size_t>(NT) + nsub + 1 + c); };
     // M = inv(L_kk) row block by row block (gemm_tc.cuh MODE_INV with the node: left blocks [0, r), right block r): as soon
     // as the chain has factored 128-block r, row r of M follows from the rows above it -- two launches, which run on the
     // inverse stream beside the chain's next sub-columns; only the last row block's two launches come after the chain
-    auto inverse_row = [&](GemmOp op, int r, int lb, cudaStream_t s) -> int {
+    // (step 0, U^T = M[0:r, 0:r]^T L[r, 0:r]^T, needs the row block's TRSM steps only -- it is issued behind P3(r - 1) and runs
+    // beside P1(r) and the POTRF of block r; step 1 needs the block's inverse)
+    auto inverse_row = [&](GemmOp op, int r, int lb, cudaStream_t s, int step_lo, int step_hi) -> int {
         op.mode = MODE_INV; op.c = 0; op.cb0 = 0; op.ncb = 1; op.rb0 = 0; op.nrb = 1;
         op.node.o = 0; op.node.hl = r; op.node.hr = 1;
         op.inv_last = (r == nsub - 1) ? 1 : 0;
-        for (int step = 0; step < 2; ++step) {
+        for (int step = step_lo; step < step_hi; ++step) {
             op.inv_step = step;
             const int e = launch_gemm(tm, op, num_sms, 1, s, lb);
             if (e) return e;
@@ -885,7 +888,7 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
                 rc = inverse_export(op, c, lb, sv);
                 if (rc) return rc;
                 if (c >= 1) {
-                    rc = inverse_row(op, c, lb, sv);
+                    rc = inverse_row(op, c, lb, sv, 1, 2);
                     if (rc) return rc;
                 }
             }
@@ -893,6 +896,14 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
             if (op.nrb > 0) {
                 rc = launch_gemm(tm, op, num_sms, 1, sh, lb);
                 if (rc) return rc;
+                if (k + 1 < NT) {                     // row block c + 1 of L_kk is final: the first step of its row of M
+                    if (lookahead) {
+                        KRR_CUDA_CHECK(cudaEventRecord(ev_p3(c), sh));
+                        KRR_CUDA_CHECK(cudaStreamWaitEvent(sv, ev_p3(c), 0));
+                    }
+                    rc = inverse_row(op, c + 1, lb, sv, 0, 1);
+                    if (rc) return rc;
+                }
             }
         }
         rc = finalize(k, Wk, 0, 1, 0, sh);
@@ -903,7 +914,7 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
                 rc = inverse_export(op, r, lb, sh);
                 if (rc) return rc;
                 if (r >= 1) {
-                    rc = inverse_row(op, r, lb, sh);
+                    rc = inverse_row(op, r, lb, sh, 0, 2);
                     if (rc) return rc;
                 }
             }

@@ -1206,10 +1206,10 @@ static int potrs_run(const uint8_t* factor, const float* d_scales, const uint8_t
     return rc_sweeps;
 }
 
-extern "C" {
-
-int krr_potrs(const void* d_factor, const float* d_scales, const uint8_t* d_map, const uint8_t* h_map, int64_t n,
-              int nb, float* d_B, int64_t ldb, int nrhs, void* d_ws, size_t ws_bytes, void* stream) {
+// krr_potrs; prepare = false skips the once-per-factor part (tile offsets, inverses of the diagonal tiles), which a caller
+// that solves again with the SAME factor and the SAME workspace (krr_refine, krr_pcg) has left in the workspace
+static int potrs_impl(const void* d_factor, const float* d_scales, const uint8_t* d_map, const uint8_t* h_map, int64_t n,
+                      int nb, float* d_B, int64_t ldb, int nrhs, void* d_ws, size_t ws_bytes, void* stream, bool prepare) {
     g_launches = 0;
     if (!d_factor || !d_scales || !d_map || !h_map || !d_B || !d_ws) return KRR_ERR_ARG;
     int rc = check_shape(n, nb);
@@ -1238,16 +1238,18 @@ int krr_potrs(const void* d_factor, const float* d_scales, const uint8_t* d_map,
     float* MinvT = reinterpret_cast<float*>(ws + L.MinvT);
     float* stage = reinterpret_cast<float*>(ws + L.stage);
     float* nearP = reinterpret_cast<float*>(ws + L.nearP);
-    rc = launch(CAT_MISC, offsets_kernel, dim3(1), dim3(32), 0, st, NT, nb, d_map, off, host_map_hash(NT, h_map), static_cast<int*>(nullptr),
-                static_cast<int*>(nullptr), static_cast<int*>(nullptr));
-    if (rc) return rc;
     const uint8_t* factor = static_cast<const uint8_t*>(d_factor);
-    rc = launch(CAT_POTRS, trtri128_kernel, dim3(static_cast<unsigned>(n / kBlk)), dim3(kTriThreads), static_cast<size_t>(kTriSmem), st,
-                factor, static_cast<const int64_t*>(off), NT, nb, dinv, dinvT);
-    if (rc) return rc;
-    rc = launch(CAT_POTRS, potrs_tile_inverse_kernel, dim3(nb / kBlk, NT), dim3(kTinvThreads), static_cast<size_t>(kTinvSmem), st,
-                factor, static_cast<const int64_t*>(off), NT, nb, static_cast<const float*>(dinv), Minv, MinvT);
-    if (rc) return rc;
+    if (prepare) {
+        rc = launch(CAT_MISC, offsets_kernel, dim3(1), dim3(32), 0, st, NT, nb, d_map, off, host_map_hash(NT, h_map), static_cast<int*>(nullptr),
+                    static_cast<int*>(nullptr), static_cast<int*>(nullptr));
+        if (rc) return rc;
+        rc = launch(CAT_POTRS, trtri128_kernel, dim3(static_cast<unsigned>(n / kBlk)), dim3(kTriThreads), static_cast<size_t>(kTriSmem), st,
+                    factor, static_cast<const int64_t*>(off), NT, nb, dinv, dinvT);
+        if (rc) return rc;
+        rc = launch(CAT_POTRS, potrs_tile_inverse_kernel, dim3(nb / kBlk, NT), dim3(kTinvThreads), static_cast<size_t>(kTinvSmem), st,
+                    factor, static_cast<const int64_t*>(off), NT, nb, static_cast<const float*>(dinv), Minv, MinvT);
+        if (rc) return rc;
+    }
     // the mosaic as a TMA source of the streamed bulk updates: per direction one map per element size
     StreamMaps smaps[2];
     const size_t payload = host_offsets(NT, nb, h_map, nullptr);
@@ -1265,6 +1267,13 @@ int krr_potrs(const void* d_factor, const float* d_scales, const uint8_t* d_map,
         case 16: return potrs_run<16>(factor, d_scales, d_map, hoff, off, Minv, MinvT, stage, NT, nb, d_B, ldb, nrhs, num_sms, st, sm, h_map, nearP);
         default: return potrs_run<32>(factor, d_scales, d_map, hoff, off, Minv, MinvT, stage, NT, nb, d_B, ldb, nrhs, num_sms, st, sm, h_map, nearP);
     }
+}
+
+extern "C" {
+
+int krr_potrs(const void* d_factor, const float* d_scales, const uint8_t* d_map, const uint8_t* h_map, int64_t n,
+              int nb, float* d_B, int64_t ldb, int nrhs, void* d_ws, size_t ws_bytes, void* stream) {
+    return potrs_impl(d_factor, d_scales, d_map, h_map, n, nb, d_B, ldb, nrhs, d_ws, ws_bytes, stream, true);
 }
 
 }  // extern "C"
@@ -1343,7 +1352,8 @@ int krr_refine(const float* d_A, int64_t n, int64_t lda, int nb, const void* d_f
         rc = residual(d_resid ? d_resid + s : nullptr);
         if (rc) return rc;
         launches += g_launches;
-        rc = krr_potrs(d_factor, d_scales, d_map, h_map, n, nb, R, nrhs, nrhs, ws + L.potrs, L.R - L.potrs, stream);   // resets the counter
+        // (resets the launch counter; the inverses of the diagonal tiles stay in the workspace after the first step)
+        rc = potrs_impl(d_factor, d_scales, d_map, h_map, n, nb, R, nrhs, nrhs, ws + L.potrs, L.R - L.potrs, stream, s == 0);
         if (rc) return rc;
         const int64_t ne = n * nrhs;
         rc = launch(CAT_MISC, refine_update_kernel, dim3(static_cast<unsigned>((ne + 255) / 256)), dim3(256), 0, st, d_X, ldx,
@@ -1454,9 +1464,11 @@ int krr_pcg(const float* d_A, int64_t n, int64_t lda, int nb, const void* d_fact
             default: return symm_run<32>(av, V, ldv, Yp, ldy, n, nrhs, partial, out64, out32, blkp, st);
         }
     };
-    auto solve = [&]() -> int {                       // z <- (L L^T)^-1 z; krr_potrs resets the launch counter
+    bool prepared = false;                            // the inverses of the diagonal tiles are computed by the first solve only
+    auto solve = [&]() -> int {                       // z <- (L L^T)^-1 z; the solve resets the launch counter
         launches += g_launches;
-        int e = krr_potrs(d_factor, d_scales, d_map, h_map, n, nb, z, nrhs, nrhs, ws + L.potrs, L.x - L.potrs, stream);
+        int e = potrs_impl(d_factor, d_scales, d_map, h_map, n, nb, z, nrhs, nrhs, ws + L.potrs, L.x - L.potrs, stream, !prepared);
+        prepared = true;
         launches += g_launches;
         g_launches = 0;
         return e;

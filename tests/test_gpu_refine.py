@@ -67,6 +67,34 @@ def test_one_step_from_a_random_start_with_an_fp32_map(krr, n, nb, nrhs):
     assert torch.equal(X00.cpu(), X0) and n0.numel() == 1 and float(n0[0]) == norms[0]
 
 
+@pytest.mark.parametrize("n,nb,nrhs", [(2048, 256, 4), (4096, 1024, 16)])
+def test_steps_in_one_call_equal_one_call_per_step(krr, n, nb, nrhs):
+    """krr_refine / krr_pcg compute the inverses of the diagonal tiles in their first solve and keep them in the workspace
+    for the later ones (the factor does not change inside a call): three steps in one call and three calls of one step
+    (each of which prepares the workspace again) give the same bits; PCG: the iterates of a 3-iteration call are repeatable
+    and its first iterate is that of a 1-iteration call."""
+    cfg = replace(scaled_config(CONFIGS["C2"], nb=nb, n=n, p=max(256, n // 4)), nrhs=nrhs)
+    A, Y = make_problem(cfg, device="cuda")
+    h = krr.uniform_map(cfg.NT, krr.FP16)
+    F = krr.potrf_mp(A, nb, h.cuda(), h)
+    X0 = krr.potrs(F, Y.clone())
+    Xa, na = krr.refine(A, F, Y, X0.clone(), 3)
+    Xb = X0.clone()
+    nbs = []
+    for _ in range(3):
+        Xb, n1 = krr.refine(A, F, Y, Xb, 1)
+        nbs.append(float(n1[0]))
+    torch.cuda.synchronize()
+    assert torch.equal(Xa, Xb)
+    assert [float(v) for v in na[:3]] == nbs
+    Pa, pa = krr.pcg(A, F, Y, X0.clone(), 3)
+    Pb, pb = krr.pcg(A, F, Y, X0.clone(), 3)
+    P1, p1 = krr.pcg(A, F, Y, X0.clone(), 1)
+    torch.cuda.synchronize()
+    assert torch.equal(Pa, Pb) and torch.equal(pa, pb)
+    assert float(p1[0]) == float(pa[0]) and float(p1[1]) == float(pa[1])
+
+
 @pytest.mark.parametrize("prec,tiled", [("fp16", False), ("fp16", True), ("fp8", False)])
 def test_refinement_under_low_precision_maps_against_the_oracle(krr, prec, tiled):
     """All-FP16 map (C4's map by the rule) and the C5' map (tile column 0 FP32, the rest FP8): raw alpha misses the

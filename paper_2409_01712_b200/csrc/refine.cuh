@@ -12,7 +12,7 @@
 
 namespace krr {
 
-constexpr int kResKc = 32;         // columns of A staged per step
+constexpr int kResKc = 32;         // columns of A staged per step (at most: ResidCfg::KC)
 constexpr int kResSegMax = 16;
 
 // number of column segments: a pure function of n (not of the device), about 4096 CTAs per residual (four are
@@ -30,10 +30,14 @@ template <int NR>
 struct ResidCfg {
     static constexpr int RPT = NR < 8 ? NR : 8;       // right-hand sides per thread
     static constexpr int NG = NR / RPT;               // thread groups over the right-hand sides
-    static constexpr int ROWS = NR >= 16 ? 2 : 1;     // rows per thread (r, r + 64): fewer shared-memory reads of X per FMA
-    static constexpr int NTHR = kBlk / ROWS * NG;     // 128 (NR <= 16) or 256 (NR = 32)
-    static constexpr int NLD = kBlk * kResKc / NTHR;  // elements of A per thread and chunk
-    static constexpr int NXL = (kResKc * NR + NTHR - 1) / NTHR;
+    // rows per thread (r, r + 128 / ROWS, ...): fewer shared-memory reads of X per FMA.  Measured at n = 65536 (A/B in one
+    // gpurun call): NR = 32 with 4 rows 14.6 ms (2 rows: 15.8), NR = 4 with 2 rows 3.9 ms (1 row: 4.2), NR = 16 with 2 rows
+    // 8.5 ms (4 rows: 8.8; reading column kk + 1 from shared memory before the FMAs of column kk: 8.9)
+    static constexpr int ROWS = NR >= 32 ? 4 : 2;
+    static constexpr int NTHR = kBlk / ROWS * NG;     // 64 (NR <= 8) or 128 (NR >= 16)
+    static constexpr int KC = NTHR >= 128 ? kResKc : kResKc / 2;   // columns of A per chunk: 32 staged elements per thread
+    static constexpr int NLD = kBlk * KC / NTHR;      // elements of A per thread and chunk
+    static constexpr int NXL = (KC * NR + NTHR - 1) / NTHR;
 };
 
 // partial[seg][row][NR] = sum over the 128-column blocks cb = seg, seg + nseg, ... of A(rows, cb) X(cb, :).
@@ -45,9 +49,9 @@ resid_partial_kernel(AView A, const float* __restrict__ X, int64_t ldx, int nrhs
                      double* __restrict__ partial) {
     using Cfg = ResidCfg<NR>;
     constexpr int RPT = Cfg::RPT, NTHR = Cfg::NTHR, ROWS = Cfg::ROWS, RSTEP = kBlk / ROWS, NLD = Cfg::NLD, NXL = Cfg::NXL;
-    constexpr int CPB = kBlk / kResKc;                // chunks per block
-    __shared__ float S[kResKc][kBlk + 1];             // S[kk][r] = a(row r of the block row, column k0 + kk)
-    __shared__ double Xs[kResKc][NR];
+    constexpr int KC = Cfg::KC, CPB = kBlk / KC;                // chunks per block
+    __shared__ float S[KC][kBlk + (KC == 16 ? 2 : 1)];   // S[kk][r] = a(row r of the block row, column k0 + kk); padded: conflict-free staging
+    __shared__ double Xs[KC][NR];
     const int t = threadIdx.x, r = t % RSTEP, g = t / RSTEP;
     const int rb = blockIdx.x, seg = blockIdx.y;
     const int nsub = A.nb / kBlk;
@@ -62,14 +66,14 @@ resid_partial_kernel(AView A, const float* __restrict__ X, int64_t ldx, int nrhs
     const int nchunks = ((nblk - seg + nseg - 1) / nseg) * CPB;
     // issue the global loads of chunk i
     auto fetch = [&](int i) {
-        const int cb = seg + (i / CPB) * nseg, k0 = (i % CPB) * kResKc;
+        const int cb = seg + (i / CPB) * nseg, k0 = (i % CPB) * KC;
         // block (rb, cb) of the symmetric matrix lives in the lower triangle as block (max, min)
         const int br = rb > cb ? rb : cb, bc = rb > cb ? cb : rb;
         const float* B = A.tile_ptr(br / nsub, bc / nsub, (br % nsub) * kBlk, (bc % nsub) * kBlk);
         if (cb < rb) {                                                        // stored as is: rows of B are our rows
 #pragma unroll
             for (int j = 0; j < NLD; ++j) {
-                const int e = t + j * NTHR, rr = e / kResKc, kk = e % kResKc;
+                const int e = t + j * NTHR, rr = e / KC, kk = e % KC;
                 ra[j] = __ldg(B + rr * ls + k0 + kk);
             }
         } else if (cb > rb) {                                                 // stored transposed: columns of B are our rows
@@ -88,7 +92,7 @@ resid_partial_kernel(AView A, const float* __restrict__ X, int64_t ldx, int nrhs
 #pragma unroll
         for (int j = 0; j < NXL; ++j) {
             const int e = t + j * NTHR, kk = e / NR, q = e % NR;
-            rx[j] = (e < kResKc * NR && q < nrhs) ? __ldg(X + (static_cast<int64_t>(cb) * kBlk + k0 + kk) * ldx + q) : 0.0f;
+            rx[j] = (e < KC * NR && q < nrhs) ? __ldg(X + (static_cast<int64_t>(cb) * kBlk + k0 + kk) * ldx + q) : 0.0f;
         }
     };
     // registers -> shared memory, in the layout the FMAs read
@@ -98,7 +102,7 @@ resid_partial_kernel(AView A, const float* __restrict__ X, int64_t ldx, int nrhs
 #pragma unroll
             for (int j = 0; j < NLD; ++j) {
                 const int e = t + j * NTHR;
-                S[e % kResKc][e / kResKc] = ra[j];
+                S[e % KC][e / KC] = ra[j];
             }
         } else {
 #pragma unroll
@@ -110,7 +114,7 @@ resid_partial_kernel(AView A, const float* __restrict__ X, int64_t ldx, int nrhs
 #pragma unroll
         for (int j = 0; j < NXL; ++j) {
             const int e = t + j * NTHR;
-            if (e < kResKc * NR) Xs[e / NR][e % NR] = static_cast<double>(rx[j]);
+            if (e < KC * NR) Xs[e / NR][e % NR] = static_cast<double>(rx[j]);
         }
     };
 
@@ -121,7 +125,7 @@ resid_partial_kernel(AView A, const float* __restrict__ X, int64_t ldx, int nrhs
         __syncthreads();
         if (i + 1 < nchunks) fetch(i + 1);
 #pragma unroll 4
-        for (int kk = 0; kk < kResKc; ++kk) {
+        for (int kk = 0; kk < KC; ++kk) {
             double a[ROWS];
 #pragma unroll
             for (int u = 0; u < ROWS; ++u) a[u] = static_cast<double>(S[kk][r + u * RSTEP]);

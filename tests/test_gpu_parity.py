@@ -409,6 +409,49 @@ def test_potrs_lookahead_depths(krr, NT, nb):
     assert torch.equal(again, alpha)
 
 
+@pytest.mark.parametrize("nb,NT,nrhs", [(2048, 4, 16), (4096, 3, 8)])
+def test_largest_tile_sizes(krr, nb, NT, nrhs):
+    """The largest tile sizes the library accepts (nb <= 4096; the solved block of the solve must fit in shared memory:
+    nrhs <= 16 at nb = 2048, <= 8 at nb = 4096): 16 and 32 sub-columns per diagonal tile, the streamed solve kernel with a
+    ring cut down to what the solved block leaves.  FP32 / FP16 mosaic: info = 0, backward error of the factor as stored
+    (checked with torch FP64 on the GPU), the solve against the oracle's substitution with the same factor, repeatable
+    bits; all-FP32 map: alpha against the FP64 solution -- the product form of the panel TRSM loses accuracy in
+    proportion to cond(L_kk), which grows with the tile (7e-5 at nb = 1024, 7e-4 at nb = 4096 on
+    this matrix family)."""
+    n = nb * NT
+    cfg = replace(scaled_config(CONFIGS["C2"], nb=nb, n=n, p=max(1024, n // 4)), nrhs=nrhs)
+    A, Y = make_problem(cfg, device="cuda")
+    A64 = torch.tril(A.double()) + torch.tril(A.double(), -1).T
+    rng = np.random.default_rng(nb + NT)
+    pmap = oracle_uniform(NT, R.FP32)
+    for i in range(NT):
+        for j in range(i):
+            pmap[i, j] = rng.integers(0, 2)
+    pmap[NT - 1, 0] = R.FP16                                  # both classes whatever the draw
+    pmap[1, 0] = R.FP32
+    F = gpu_factor(krr, A, nb, pmap)
+    torch.cuda.synchronize()
+    assert int(F.info.item()) == 0
+    L = F.dense().double()
+    assert float(torch.linalg.norm(L @ L.T - A64) / torch.linalg.norm(A64)) <= 5e-4
+    alpha = krr.potrs(F, Y.clone())
+    torch.cuda.synchronize()
+    want = potrs_fp64(F.dense().cpu().numpy(), Y.cpu().numpy(), nb)
+    assert relF(alpha.cpu().numpy().astype(np.float64), want) <= 1e-5
+    again = krr.potrs(F, Y.clone())
+    torch.cuda.synchronize()
+    assert torch.equal(again, alpha)
+    del L
+    F32 = gpu_factor(krr, A, nb, oracle_uniform(NT, R.FP32))
+    a32 = krr.potrs(F32, Y.clone())
+    torch.cuda.synchronize()
+    assert int(F32.info.item()) == 0
+    xs = torch.linalg.solve(A64, Y.double())
+    assert float(torch.linalg.norm(a32.double() - xs) / torch.linalg.norm(xs)) <= 2e-3
+    L32 = F32.dense().double()
+    assert float(torch.linalg.norm(L32 @ L32.T - A64) / torch.linalg.norm(A64)) <= {2048: 2e-6, 4096: 5e-6}[nb]   # measured 3.3e-6 at 4096
+
+
 def test_potrs_rejects_a_misaligned_factor(krr):
     import ctypes
     cfg = scaled_config(CONFIGS["C1"], nb=128, n=256, p=100)

@@ -182,10 +182,10 @@ int64_t krr_factor_tile_offset(int64_t n, int nb, const uint8_t* h_map, int i, i
  *               pivot (contents of later tile columns are then unspecified); -1: d_map and h_map differ;
  *               -2: the inverse of a diagonal tile left the range of its FP16 images (entries beyond 2^12 times
  *               1 / sqrt(max A_ii): the tile is too ill-conditioned for the product form of the panel TRSM).
- * Accuracy the panel below a diagonal tile is one product with the explicit inverse of that tile, whose error grows
- *          with the tile's condition number, i.e. with nb: with an all-FP32 map the backward error
- *          ||A - L L^T||_F / ||A||_F stays below 1e-6 for nb <= 1024 at any NT; tiles of 2048 / 4096 on a matrix of
- *          a few tile columns give up to 2e-6 / 4e-6 ("Accuracy of the product form").
+ * Accuracy the panel below a diagonal tile is one product with the explicit inverse of that tile.  With an all-FP32
+ *          map the backward error ||A - L L^T||_F / ||A||_F stays below 1e-6 at every admitted shape (measured up to
+ *          nb = 4096); tiles above 1024 and matrices of at most four tile columns take a segmented-accumulation form
+ *          of the product for that ("Accuracy of the product form").
  * d_ws     workspace, at least krr_potrf_mp_workspace(n, nb, h_map) bytes, 1024-byte aligned.
  *          It holds the FP16 operand images of L that the tensor-core kernels read and two FP32
  *          panel buffers; it may be released once the call has completed on `stream` (krr_potrs

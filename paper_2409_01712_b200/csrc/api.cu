@@ -742,6 +742,13 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
         tm.Q = tm.H;                              // never dereferenced (op.fp8q = 0)
     }
     const int cg = ((flags & KRR_FLAG_NO_CTA_PAIRS) || nb % (2 * kBlk) != 0) ? 1 : 2;
+    // the panel product X = S M^T walks K = nb with partial sums far larger than the result ("Accuracy of
+    // the product form"): every MMA truncates the accumulator, so the error grows with nb.  Up to nb = 1024 the CTA-pair form
+    // (cross terms in the second accumulator) stays below the 1e-6 of an all-FP32 factorisation; larger tiles take the
+    // single-CTA form, which starts a fresh accumulator every 128 columns of K and adds the segments in FP32 (twice the
+    // operand traffic per flop); so do matrices of at most four tile columns, where the margin is thinnest (nb = 1024, NT = 2:
+    // 9.9e-7 against 5.6e-7) and the panel costs next to nothing
+    const int cg_trsm = (nb > 1024 || NT <= 4) ? 1 : cg;
 
     const int nsub = nb / kBlk;
     const bool lookahead = !(flags & KRR_FLAG_NO_LOOKAHEAD) && NT > 2;
@@ -926,7 +933,7 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
         op.mode = MODE_TRSM; op.c = 0; op.cb0 = 0; op.ncb = nsub;
         if (!lookahead) {
             op.rb0 = nsub; op.nrb = mblk - nsub;
-            rc = launch_gemm(tm, op, num_sms, cg, st, lb);
+            rc = launch_gemm(tm, op, num_sms, cg_trsm, st, lb);
             if (rc) return rc;
             rc = finalize(k, Wk, 1, NT - k - 1, 1, st);
             if (rc) return rc;
@@ -935,7 +942,7 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
             // tile (k+1, k) first, on the critical stream: column k+1's chain needs nothing else of column k
             KRR_CUDA_CHECK(cudaStreamWaitEvent(sh, ev_newb(k), 0));
             op.rb0 = nsub; op.nrb = nsub;
-            rc = launch_gemm(tm, op, num_sms, cg, sh, lb);
+            rc = launch_gemm(tm, op, num_sms, cg_trsm, sh, lb);
             if (rc) return rc;
             rc = finalize(k, Wk, 1, 1, 1, sh);
             if (rc) return rc;
@@ -943,7 +950,7 @@ int krr_potrf_mp(const float* d_A, int64_t n, int64_t lda, int nb, const uint8_t
             if (k + 2 < NT) {
                 KRR_CUDA_CHECK(cudaStreamWaitEvent(sl, ev_chain(k), 0));
                 op.rb0 = 2 * nsub; op.nrb = mblk - 2 * nsub;
-                rc = launch_gemm(tm, op, bulk_ctas, cg, sl, lb);                         // T(k)
+                rc = launch_gemm(tm, op, bulk_ctas, cg_trsm, sl, lb);                    // T(k)
                 if (rc) return rc;
                 rc = finalize(k, Wk, 2, NT - k - 2, 1, sl);
                 if (rc) return rc;

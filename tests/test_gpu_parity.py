@@ -415,9 +415,9 @@ def test_largest_tile_sizes(krr, nb, NT, nrhs):
     nrhs <= 16 at nb = 2048, <= 8 at nb = 4096): 16 and 32 sub-columns per diagonal tile, the streamed solve kernel with a
     ring cut down to what the solved block leaves.  FP32 / FP16 mosaic: info = 0, backward error of the factor as stored
     (checked with torch FP64 on the GPU), the solve against the oracle's substitution with the same factor, repeatable
-    bits; all-FP32 map: alpha against the FP64 solution -- the product form of the panel TRSM loses accuracy in
-    proportion to cond(L_kk), which grows with the tile (7e-5 at nb = 1024, 7e-4 at nb = 4096 on
-    this matrix family)."""
+    bits; all-FP32 map: backward error and alpha against the FP64 solution inside the north_star's 1e-6 / 1e-3 -- tiles
+    above 1024 take the segmented-accumulation form of the panel product (the CTA-pair form gives
+    3.6e-6 / 6.7e-4 at nb = 4096)."""
     n = nb * NT
     cfg = replace(scaled_config(CONFIGS["C2"], nb=nb, n=n, p=max(1024, n // 4)), nrhs=nrhs)
     A, Y = make_problem(cfg, device="cuda")
@@ -447,9 +447,9 @@ def test_largest_tile_sizes(krr, nb, NT, nrhs):
     torch.cuda.synchronize()
     assert int(F32.info.item()) == 0
     xs = torch.linalg.solve(A64, Y.double())
-    assert float(torch.linalg.norm(a32.double() - xs) / torch.linalg.norm(xs)) <= 2e-3
+    assert float(torch.linalg.norm(a32.double() - xs) / torch.linalg.norm(xs)) <= 5e-4
     L32 = F32.dense().double()
-    assert float(torch.linalg.norm(L32 @ L32.T - A64) / torch.linalg.norm(A64)) <= {2048: 2e-6, 4096: 5e-6}[nb]   # measured 3.3e-6 at 4096
+    assert float(torch.linalg.norm(L32 @ L32.T - A64) / torch.linalg.norm(A64)) <= 1e-6
 
 
 def test_potrs_rejects_a_misaligned_factor(krr):

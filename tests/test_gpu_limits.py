@@ -1,7 +1,8 @@
 """Launch-geometry limits: sizes at which an index that used to sit in gridDim.y (limit 65535) passes it.
 
   * krr_precision_map at NT = 363 (nb = 128, n = 46464): NT (NT + 1) / 2 = 66066 tile slots;
-  * krr_build with the IBS kernel at n = 65536 rows (BASELINE.json config 3's patient count).
+  * krr_build with the IBS kernel at n = 65536 rows (BASELINE.json config 3's patient count);
+  * krr_potrf_mp / krr_potrs at NT = 1024, the largest tile count the library accepts (nb = 128, n = 131072).
 
 Expected values come from independent torch FP64 code on sampled tiles / entries (checking only).
 """
@@ -85,3 +86,40 @@ def test_ibs_build_with_65536_patients(krr):
         else:
             got = T[slot].double()
         assert float((got - want).abs().max()) <= 2e-7, (i, j)
+
+
+def test_largest_tile_count(krr):
+    """NT = 1024, the largest tile count the library accepts (nb = 128, n = 131072: 524800 lower tiles, 34 GB of packed
+    FP32 tiles; the host-built launch sequence has 1024 tile columns).  All-FP32 map: info = 0; sampled tiles of L L^T
+    against A (the last diagonal tile sums 1024 tile products) and sampled row blocks of A alpha = Y, both with torch
+    FP64 on the GPU (checking only)."""
+    from dataclasses import replace
+    from krr_inputs import CONFIGS, make_problem_lower_tiles
+    nb, NT = 128, 1024
+    n = nb * NT
+    cfg = replace(CONFIGS["C4"], nb=nb, n=n, p=8192, nrhs=4)
+    At, Y = make_problem_lower_tiles(cfg, device="cuda")
+    h = krr.uniform_map(NT, krr.FP32)
+    F = krr.potrf_mp(At, nb, h.cuda(), h, flags=krr.FLAG_PREROUND_A | krr.FLAG_A_TILED_LOWER, n=n)
+    alpha = krr.potrs(F, Y.clone())
+    torch.cuda.synchronize()
+    assert int(F.info.item()) == 0
+    T = At.reshape(-1, nb, nb)
+
+    def a_tile(i, k):                                            # tile (i, k) of the symmetric matrix, FP64
+        t = T[krr.tile_slot(NT, max(i, k), min(i, k))].double()
+        if k > i:
+            return t.T
+        return t if i != k else torch.tril(t) + torch.tril(t, -1).T
+
+    for (i, j) in [(NT - 1, NT - 1), (NT - 1, 0), (700, 699)]:
+        acc = torch.zeros((nb, nb), dtype=torch.float64, device="cuda")
+        for k in range(j + 1):
+            acc += F.tile(i, k) @ F.tile(j, k).T
+        a = a_tile(i, j)
+        assert float(torch.linalg.norm(acc - a) / torch.linalg.norm(a)) <= 5e-5, (i, j)      # measured 1.4e-5 (last diagonal tile)
+    for i in (0, NT - 1):
+        r = Y[i * nb:(i + 1) * nb].double().clone()
+        for k in range(NT):
+            r -= a_tile(i, k) @ alpha[k * nb:(k + 1) * nb].double()
+        assert float(torch.linalg.norm(r) / torch.linalg.norm(Y[i * nb:(i + 1) * nb].double())) <= 1e-3, i   # measured 1e-4 .. 3.5e-4
